@@ -1,0 +1,242 @@
+"""Pins for oracle/quant.py (step a0) -- none of them re-types the oracle's own formula.
+
+* footprints the paper prints;
+* the golden group and E4M3 spot values (tests/golden);
+* "nearest representable value, ties to even" by brute force over the whole code book with
+  exact rationals -- an independent definition of RNE, against the oracle's threshold chains;
+* exact round trips on grid-valued groups; error bounds; BF16-exactness of dequantised keys.
+"""
+from fractions import Fraction
+
+import numpy as np
+import pytest
+
+from oracle import quant
+from oracle.bf16 import bf16_bits_to_f64, f64_to_bf16_bits_exact
+from workloads.bf16 import f32_to_bf16_bits
+
+
+def _bits(vals):
+    return f32_to_bf16_bits(np.asarray(vals, dtype=np.float32))
+
+
+def test_footprints_printed_by_the_paper(golden):
+    g = golden("footprint.txt")
+    n = int(g["tokens"][0][0]) * int(g["layers"][0][0]) * int(g["h_idx"][0][0]) * int(g["d_idx"][0][0])
+    GiB = 2.0 ** 30
+    assert quant.selector_k_bytes("bf16", n) / GiB == pytest.approx(float(g["bf16_gib"][0][0]), abs=0.005)
+    assert quant.selector_k_bytes("bf16", n) == 131072 * 36 * 4 * 128 * 2
+    # 1.27 GiB <=> 4.5 bit/elt (16-bit group metadata); 1.20 GiB <=> 4.25 bit/elt (8-bit scale)
+    assert quant.selector_k_bytes("int4_scale16", n) / GiB == pytest.approx(float(g["int4_gib"][0][0]), abs=0.005)
+    assert quant.selector_k_bytes("mxfp4", n) / GiB == pytest.approx(float(g["fp4_gib"][0][0]), abs=0.005)
+    assert quant.selector_k_bytes("int4_scale16", n) / quant.selector_k_bytes("bf16", n) == \
+        pytest.approx(float(g["ratio_4p5bit"][0][0]), abs=0.0005)
+    assert quant.selector_k_bytes("int4_e4m3", n) * 32 == n * 17           # 4.25 bit/elt
+    # BASELINE.json geometry: 4 heads x 64 -> 512 B/token BF16, 136 B/token 4-bit
+    assert quant.selector_k_bytes("bf16", 256) == 512
+    assert quant.selector_k_bytes("mxfp4", 256) == 136
+
+
+def _golden_group():
+    v = [(i - 15.5) * 0.17 * (1.3 if i % 5 == 0 else 1.0) for i in range(32)]
+    return _bits(v)
+
+
+def test_golden_group_mxfp4(golden):
+    g = golden("quant_group.txt")
+    bits = _golden_group()
+    vals = bf16_bits_to_f64(bits)
+    assert np.abs(vals).max() == float(g["amax"][0][0])
+    codes, scale = quant.quantize_mxfp4(bits)
+    assert scale.tolist() == [int(g["mxfp4_scale"][0][0])]
+    assert "".join("%x" % c for c in codes) == g["mxfp4_codes"][0][0]
+    dq = quant.dequantize_mxfp4(codes, scale)
+    assert np.abs(dq - vals).max() == float(g["mxfp4_max_abs_err"][0][0])
+
+
+def test_golden_group_int4(golden):
+    g = golden("quant_group.txt")
+    bits = _golden_group()
+    vals = bf16_bits_to_f64(bits)
+    q, code = quant.quantize_int4_e4m3(bits)
+    assert code.tolist() == [int(g["int4_scale_code"][0][0], 16)]
+    assert q.tolist() == [int(x) for x in g["int4_q"][0]]
+    dq = quant.dequantize_int4_e4m3(q, code)
+    assert np.abs(dq - vals).max() == pytest.approx(float(g["int4_max_abs_err"][0][0]), abs=5e-6)
+
+
+def test_e4m3_spot_values(golden):
+    with open(__import__("os").path.join(__import__("conftest").GOLDEN, "e4m3_spot.txt")) as f:
+        rows = [l.split() for l in f if l.strip() and not l.startswith("#")]
+    for val, code in rows:
+        got = int(quant.encode_e4m3_rne_satfinite(np.float32(float(val))))
+        assert got == int(code, 16), (val, hex(got), code)
+
+
+# ---- brute-force "nearest representable, ties to even" with exact rationals -----------------
+
+def _e4m3_table():
+    tab = []
+    for code in range(0x7F):
+        E, m = code >> 3, code & 7
+        v = Fraction(m, 512) if E == 0 else Fraction(8 + m, 8) * Fraction(2) ** (E - 7)
+        tab.append((v, code))
+    return tab
+
+
+def _nearest_even(x, table):
+    """table: ascending [(value, code)]; ties -> even code (even mantissa lsb)."""
+    best = None
+    for v, c in table:
+        d = abs(x - v)
+        if best is None or d < best[0] or (d == best[0] and c % 2 == 0 and best[1] % 2 == 1):
+            best = (d, c)
+    return best[1]
+
+
+def test_e4m3_value_table_is_the_ocp_format():
+    v = quant.e4m3_value(np.arange(0x7F))
+    assert v[0] == 0 and v[1] == 2.0 ** -9 and v[7] == 7 * 2.0 ** -9
+    assert v[8] == 2.0 ** -6 and v[0x38] == 1.0 and v[0x30] == 0.5 and v[0x7E] == 448.0
+    assert np.all(np.diff(v) > 0)
+    tab = _e4m3_table()
+    assert [float(t[0]) for t in tab] == v.tolist()
+
+
+def test_e4m3_encode_matches_bruteforce_rne():
+    tab = _e4m3_table()
+    rng = np.random.default_rng(7)
+    xs = list(np.exp(rng.uniform(np.log(2.0 ** -12), np.log(600.0), 3000)).astype(np.float32))
+    vals = [float(t[0]) for t in tab]
+    # every exact value, every midpoint (ties), and neighbours of midpoints
+    xs += [np.float32(v) for v in vals]
+    for a, b in zip(vals[:-1], vals[1:]):
+        mid = np.float32((a + b) / 2)
+        xs += [mid, np.nextafter(mid, np.float32(0)), np.nextafter(mid, np.float32(1e9))]
+    xs += [np.float32(0), np.float32(448), np.float32(464), np.float32(463.9), np.float32(1e6)]
+    got = quant.encode_e4m3_rne_satfinite(np.asarray(xs, dtype=np.float32))
+    for x, c in zip(xs, got):
+        fx = Fraction(float(x))
+        want = 0x7E if fx >= 448 else _nearest_even(fx, tab)
+        # above 448 the format saturates (satfinite); the tie 464 also saturates
+        assert int(c) == want, (float(x), hex(int(c)), hex(want))
+
+
+def _e2m1_table():
+    return [(Fraction(v).limit_denominator(2), c) for c, v in enumerate([0, .5, 1, 1.5, 2, 3, 4, 6])]
+
+
+def test_mxfp4_codes_match_bruteforce_rne():
+    rng = np.random.default_rng(11)
+    tab = _e2m1_table()
+    vals = rng.standard_normal((200, 32)).astype(np.float32) * np.exp(rng.uniform(-6, 6, (200, 1))).astype(np.float32)
+    # inject exact ties relative to the group scale: multiples of 0.25 * 2^k
+    vals[0] = np.array([0.25, 0.75, 1.25, 1.75, 2.5, 3.5, 5.0, 6.0, 7.0, 7.9, -0.25, -0.75, -1.25, -1.75,
+                        -2.5, -3.5, -5.0, 4.0, 0.0, -0.0, 0.1, 0.3, 0.6, 0.9, 1.1, 1.4, 1.6, 2.2, 2.9, 3.2, 4.4, 5.5],
+                       dtype=np.float32)
+    bits = _bits(vals)
+    v = bf16_bits_to_f64(bits)
+    codes, scale = quant.quantize_mxfp4(bits)
+    for r in range(v.shape[0]):
+        amax = max(abs(Fraction(x)) for x in v[r])
+        e = 0
+        if amax > 0:                                  # floor(log2 amax) by exact comparison
+            while Fraction(2) ** (e + 1) <= amax:
+                e += 1
+            while Fraction(2) ** e > amax:
+                e -= 1
+            e = max(-127, min(127, e - 2))
+        assert int(scale[r, 0]) == e + 127
+        X = Fraction(2) ** e
+        for i in range(32):
+            a = abs(Fraction(float(v[r, i]))) / X
+            want = 7 if a >= 6 else _nearest_even(a, tab)
+            assert int(codes[r, i]) & 7 == want, (r, i, float(a))
+            assert (int(codes[r, i]) >> 3) == int(np.signbit(v[r, i]))
+
+
+def test_mxfp4_tie_rule_spelled_out():
+    # ties go to the even mantissa bit: 0.25->0, 0.75->1, 1.25->1, 1.75->2, 2.5->2, 3.5->4, 5->4
+    grp = np.zeros(32, dtype=np.float32)
+    grp[:8] = [4.0, 0.25, 0.75, 1.25, 1.75, 2.5, 3.5, 5.0]     # amax 5 -> e = 0, X = 1
+    codes, scale = quant.quantize_mxfp4(_bits(grp))
+    assert scale.tolist() == [127]
+    assert quant.dequantize_mxfp4(codes, scale)[:8].tolist() == [4.0, 0.0, 1.0, 1.0, 2.0, 2.0, 4.0, 4.0]
+
+
+def test_mxfp4_roundtrip_on_grid_and_zero_group():
+    rng = np.random.default_rng(3)
+    grid = np.array([0, .5, 1, 1.5, 2, 3, 4, 6])
+    for k in (-20, -3, 0, 5, 40):
+        g = rng.choice(grid, 32) * rng.choice([-1.0, 1.0], 32) * 2.0 ** k
+        g[0] = 6 * 2.0 ** k                                  # pins the scale
+        bits = _bits(g)
+        dq = quant.dequantize_mxfp4(*quant.quantize_mxfp4(bits))
+        assert np.array_equal(dq, bf16_bits_to_f64(bits))
+    z = np.zeros(32, dtype=np.float32)
+    z[3] = -0.0
+    codes, scale = quant.quantize_mxfp4(_bits(z))
+    assert scale.tolist() == [127] and (codes & 7).max() == 0 and codes[3] == 8
+
+
+def test_int4_roundtrip_on_grid_zero_group_and_tiny_group():
+    rng = np.random.default_rng(5)
+    for code in (0x01, 0x08, 0x30, 0x38, 0x45, 0x7E):
+        s = float(quant.e4m3_value(code))
+        q = rng.integers(-7, 8, 32)
+        q[0] = 7                                             # amax = 7 s -> sf = s exactly
+        bits = _bits(q * s)
+        qq, cc = quant.quantize_int4_e4m3(bits)
+        assert cc.tolist() == [code] and qq.tolist() == q.tolist()
+        assert np.array_equal(quant.dequantize_int4_e4m3(qq, cc), bf16_bits_to_f64(bits))
+    qq, cc = quant.quantize_int4_e4m3(_bits(np.zeros(32)))
+    assert cc.tolist() == [0] and not qq.any()
+    tiny = np.zeros(32, dtype=np.float32)
+    tiny[5] = 1e-5                                           # amax/7 rounds to E4M3 zero -> bumped to 0x01
+    qq, cc = quant.quantize_int4_e4m3(_bits(tiny))
+    assert cc.tolist() == [1] and qq[5] == 0                 # 1e-5 / 2^-9 = 0.005 -> 0
+    tiny[5] = 0.0015                                         # 0.0015 / 2^-9 = 0.768 -> 1
+    qq, cc = quant.quantize_int4_e4m3(_bits(tiny))
+    assert cc.tolist() == [1] and qq[5] == 1
+
+
+def test_int4_q_is_nearest_integer_of_binary32_quotient_and_error_bound():
+    rng = np.random.default_rng(13)
+    vals = rng.standard_normal((300, 64)).astype(np.float32) * np.exp(rng.uniform(-4, 4, (300, 1))).astype(np.float32)
+    bits = _bits(vals)
+    v = bf16_bits_to_f64(bits)
+    q, code = quant.quantize_int4_e4m3(bits)
+    s = quant.e4m3_value(code)                                # [300, 2]
+    vg = v.reshape(300, 2, 32)
+    qg = q.reshape(300, 2, 32)
+    amax = np.abs(vg).max(-1)
+    # the scale is the E4M3 value nearest amax/7: within half an E4M3 step
+    # (<= 1/16 relative for normals, <= 2^-10 absolute in the subnormal range)
+    assert np.all(np.abs(s - amax / 7) <= np.maximum(amax / 7 / 16, 2.0 ** -10) + 1e-9)
+    # q is within 1/2 (+ one binary32 ulp of the quotient) of v/s, clamped to [-7, 7]
+    t = vg / s[..., None]
+    tc = np.clip(t, -7, 7)
+    assert np.all(np.abs(qg - tc) <= 0.5 + 1e-6)
+    assert qg.min() >= -7 and qg.max() <= 7
+    # reconstruction error: half a step, plus the clipped excess when amax/s > 7
+    dq = quant.dequantize_int4_e4m3(q, code).reshape(300, 2, 32)
+    bound = s[..., None] * (0.5 + 1e-6) + np.maximum(0, np.abs(vg) - 7 * s[..., None])
+    assert np.all(np.abs(dq - vg) <= bound)
+
+
+def test_dequantised_keys_are_bf16_exact_and_sign_of_zero():
+    rng = np.random.default_rng(17)
+    bits = _bits(rng.standard_normal((64, 4, 64)).astype(np.float32) * 3)
+    for fmt in ("mxfp4", "int4_e4m3"):
+        dq = quant.quantize_dequantize(fmt, bits)
+        f64_to_bf16_bits_exact(dq)                            # raises if not exact
+        v = bf16_bits_to_f64(bits)
+        assert np.all(np.sign(dq) * np.sign(v) >= 0)          # never flips a sign
+    q, code = quant.quantize_int4_e4m3(bits)
+    dq = quant.dequantize_int4_e4m3(q, code)
+    assert not np.any(np.signbit(dq[dq == 0]))                # INT4 zero is +0.0
+    # MXFP4 error bound: X/2 below 2X... worst spacing 2X (between 4X and 6X) -> X; saturation < 2X
+    codes, scale = quant.quantize_mxfp4(bits)
+    X = np.ldexp(1.0, scale.astype(int) - 127)
+    err = np.abs(quant.dequantize_mxfp4(codes, scale) - bf16_bits_to_f64(bits)).reshape(64, 4, 2, 32)
+    assert np.all(err < 2 * X[..., None])
