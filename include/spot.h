@@ -1,0 +1,227 @@
+/*
+ * spot.h -- C ABI of the SpotAttention per-step hot path, B200 (sm_100a) build.
+ *
+ * The operations follow the paper's statement of the method (arxiv 2606.22874; cited below as
+ * PAPER.md:<line> of the extracted text, plus the reading numbers R* of DESIGN.md section 3):
+ *
+ *   a0  spot_quantize_selector_k   group-32 "microscale" 4-bit selector K-cache
+ *   a1  spot_select (scoring)      s_s[q,t] = sum_h w_h ReLU(q^I_h . k^I_{h,t})
+ *                                  s_bar[q,b] = max_{t in b} s_s[q,t]
+ *   a2  spot_select (selection)    static top-K (Eq. 6) or dual top-p: reserved sink/recency
+ *                                  tier + nucleus on the residual softmax + K_min floor (Eq. 7-8)
+ *   a3  spot_sparse_attn_decode    attention over the gathered K_I, V_I only           (PAPER.md:47 Fig. 2, :71)
+ *   a3' spot_sparse_attn_prefill   the same under a causal mask, one index list per 64-token query block
+ *
+ *
+ * Conventions
+ *   - Every pointer is a DEVICE pointer unless its name ends in _host.  The caller owns every buffer; the
+ *     library never allocates, frees or keeps a pointer after the call returns.
+ *   - Every call is asynchronous on the caller's stream (a cudaStream_t passed as void*; NULL = legacy
+ *     default stream) and never synchronises.  All argument checks run on the host before any launch.
+ *   - Return value: spot_status.  SPOT_ERR_CUDA means a CUDA runtime call failed; the code is kept
+ *     per thread and returned by spot_last_cuda_error().
+ *   - BF16 tensors are passed as uint16_t bit patterns.  Pointers must be 16-byte aligned.
+ *   - "block" = blk consecutive key tokens (the selection granularity).  This build supports blk == 64.
+ *   - No global state, no environment variables, no CPU fallback: on a device that is not compute
+ *     capability 10.x every launching call returns SPOT_ERR_UNSUPPORTED.
+ */
+#ifndef SPOT_H_
+#define SPOT_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+    SPOT_OK = 0,
+    SPOT_ERR_INVALID_ARG = 1,
+    SPOT_ERR_UNSUPPORTED = 2,
+    SPOT_ERR_WORKSPACE_TOO_SMALL = 3,
+    SPOT_ERR_CUDA = 4
+} spot_status;
+
+/* Selector K-cache storage formats (R16/R17). */
+typedef enum {
+    SPOT_SELK_BF16 = 0,      /* [B][cache_stride_tokens][H_idx][d_idx] BF16                              */
+    SPOT_SELK_INT4_E4M3 = 1, /* signed 4-bit codes, group 32 along d_idx, one FP8-E4M3 scale per group   */
+    SPOT_SELK_MXFP4 = 2      /* E2M1 codes, group 32 along d_idx, one E8M0 scale per group (OCP MX)      */
+} spot_selk_format;
+
+typedef enum {
+    SPOT_MODE_TOPK = 0,      /* Eq. 6; K counts the reserved blocks (R10)                                */
+    SPOT_MODE_DUAL_TOPP = 1  /* Eq. 7-8                                                                  */
+} spot_select_mode;
+
+const char* spot_status_string(spot_status s);
+/* cudaError_t (as int) of the last failing CUDA call on this host thread; 0 if none. */
+int spot_last_cuda_error(void);
+/* Library version, "major.minor". */
+const char* spot_version(void);
+/* sizeof() of the parameter blocks as this library was compiled (which: 0 = spot_select_params,
+ * 1 = spot_attn_params, 2 = spot_decode_step_host_params; anything else: 0) -- lets a binding verify its layout. */
+size_t spot_struct_size(int which);
+
+/* ---------------------------------------------------------------------------------------------------
+ * a0 -- selector K-cache formats.
+ *
+ * The quantised layout is OPAQUE: only spot_selector_k_bytes, spot_quantize_selector_k,
+ * spot_dequantize_selector_k and spot_select define it.  (It is tiled by 64 tokens: the codes of a tile
+ * followed by its scales, so that one tile is a single contiguous HBM stream.)
+ *
+ * Bytes of a cache holding B sequences of cache_stride_tokens tokens each (a multiple of 64 for the 4-bit
+ * formats): BF16 2*n, 4-bit formats n/2 + n/32 with n = B*tokens*H_idx*d_idx (16 -> 4.25
+ * bit/element).  Returns 0 on invalid arguments.
+ * --------------------------------------------------------------------------------------------------- */
+size_t spot_selector_k_bytes(spot_selk_format fmt, int64_t B, int64_t cache_stride_tokens, int H_idx, int d_idx);
+
+/* Quantise tokens [token_offset, token_offset + n_tokens) of every sequence.
+ *   k_bf16   in   [B][n_tokens][H_idx][d_idx] BF16 (the new tokens only; dense)
+ *   k_cache  out  cache in format fmt (SPOT_SELK_INT4_E4M3 or SPOT_SELK_MXFP4; SPOT_SELK_BF16 copies)
+ * Prefill: the whole prompt; decode: n_tokens = 1 appended.  Requires d_idx % 32 == 0,
+ * token_offset + n_tokens <= cache_stride_tokens.  Quantiser definitions: DESIGN.md R16 (MXFP4: scale
+ * 2^(floor(log2 amax) - 2), RNE onto the E2M1 grid, saturating; INT4: scale = E4M3_rne_satfinite(amax/7),
+ * q = clamp(rint(v/scale), -7, 7)).  Results are bit-exact with that definition. */
+spot_status spot_quantize_selector_k(const uint16_t* k_bf16, void* k_cache, spot_selk_format fmt,
+                                     int64_t B, int64_t n_tokens, int64_t token_offset,
+                                     int64_t cache_stride_tokens, int H_idx, int d_idx, void* stream);
+
+/* Inverse: write the dequantised keys of tokens [token_offset, token_offset + n_tokens) as BF16
+ * [B][n_tokens][H_idx][d_idx] (exact: every dequantised value is representable in BF16). */
+spot_status spot_dequantize_selector_k(const void* k_cache, uint16_t* k_bf16_out, spot_selk_format fmt,
+                                       int64_t B, int64_t n_tokens, int64_t token_offset,
+                                       int64_t cache_stride_tokens, int H_idx, int d_idx, void* stream);
+
+/* ---------------------------------------------------------------------------------------------------
+ * a1 + a2 -- spot_select: scores, block distribution, selection, index list + per-query budget.
+ *
+ * Rows.  The call handles B sequences x n_q selection rows each:
+ *   decode  (q_block == 1, Tq == 1): n_q = 1; the query sits at position seq_len[b]-1 and sees keys
+ *           0..seq_len[b]-1 (the current token is already appended, R15); n_b = ceil(seq_len[b]/blk).
+ *   prefill (q_block == 64): Tq % 64 == 0, n_q = Tq/64; query block i covers absolute positions
+ *           [q_start + 64 i, q_start + 64 i + 64); it sees key blocks 0..n_b(i)-1 with n_b(i) the index
+ *           of the block holding its last token, plus one; one tile score per (query block, key block) =
+ *           max over the block's queries and the block's causally visible keys (R2).
+ * Reserved tier: the first sink_blocks and the last recency_blocks of the row's n_b blocks.
+ * Dual top-p (Eq. 7-8): p~ = softmax over the residual blocks of s_bar/temperature; nucleus = shortest
+ * prefix in (score descending, index ascending) order whose mass is >= p (p >= 1: all residual blocks);
+ * then extended in the same order until the budget reaches min(kmin_blocks, n_b).  Top-K (Eq. 6):
+ * reserved plus the max(0, top_k - |reserved|) best residual blocks.
+ *
+ * Outputs (row r = b*n_q + i):
+ *   indices      int32 [B*n_q][cap]   selected block ids, ascending, padded with -1
+ *   budgets      int32 [B*n_q]        |S_q| including the reserved blocks
+ *   block_scores fp32  [B*n_q][nb_stride]  optional (may be NULL): s_bar; entries >= n_b(row) undefined
+ *   block_probs  fp32  [B*n_q][nb_stride]  optional: p~ on the residual blocks, 0 on reserved ones
+ * cap must be >= the largest budget any row can reach (>= min(n_b, what the mode allows)); a row whose
+ * budget would exceed cap makes the call fail up front when detectable on the host (cap < max n_b for
+ * DUAL_TOPP, cap < min(top_k, max n_b) for TOPK) with SPOT_ERR_INVALID_ARG.
+ * --------------------------------------------------------------------------------------------------- */
+typedef struct {
+    /* inputs */
+    const uint16_t* sel_q;       /* [B][Tq][H_idx][d_idx] BF16 selector queries q^I                       */
+    const float* w;              /* [B][Tq][H_idx] fp32 mixing weights w_h (any sign, R13)               */
+    const void* sel_k;           /* selector K-cache, format fmt                                          */
+    int32_t fmt;                 /* spot_selk_format                                                      */
+    int64_t cache_stride_tokens; /* tokens of capacity per sequence in sel_k                              */
+    const int32_t* seq_len;      /* [B] device; decode: valid tokens per sequence (>= 1).  prefill: NULL  */
+    int32_t max_seq_len;         /* host-side upper bound of seq_len (decode) -- sizes the grid           */
+    int32_t B, Tq, H_idx, d_idx;
+    int32_t q_start;             /* prefill: absolute position of the first query (multiple of 64)        */
+    int32_t blk;                 /* key block size: 64                                                    */
+    int32_t q_block;             /* 1 = decode form, 64 = prefill form                                    */
+    /* rule */
+    int32_t mode;                /* spot_select_mode                                                      */
+    int32_t top_k;
+    double p;                    /* in (0, 1]; fp64 so that the mass threshold is the caller's exact value */
+    int32_t sink_blocks, recency_blocks, kmin_blocks;
+    double temperature;          /* > 0 (default 1.0)                                       */
+    /* outputs */
+    int32_t* indices;
+    int32_t cap;
+    int32_t* budgets;
+    float* block_scores;         /* optional */
+    float* block_probs;          /* optional */
+    int32_t nb_stride;           /* row stride (elements) of block_scores / block_probs; >= max n_b       */
+    /* scratch */
+    void* workspace;
+    size_t workspace_bytes;      /* >= spot_select_workspace_bytes(&params)                               */
+} spot_select_params;
+
+size_t spot_select_workspace_bytes(const spot_select_params* p);
+spot_status spot_select(const spot_select_params* p, void* stream);
+
+/* ---------------------------------------------------------------------------------------------------
+ * a3 / a3' -- block-sparse GQA attention over the selected KV blocks.
+ *
+ *   o_h = sum_{t in T_q} softmax_t(sm_scale * q_h . k_{g,t}) v_{g,t},  g = floor(h / (H_q/H_kv)),
+ *   T_q = tokens of the selected blocks that are valid (t < seq_len[b]; prefill: t <= own position).
+ * One index list per (sequence, query row) shared by all heads (R14).  K and V are BF16 with D = 128
+ * contiguous and element strides for batch / token / head, so both [B][L][H_kv][D] and [B][H_kv][L][D]
+ * work.  fp32 softmax and accumulation, BF16 output.
+ *
+ * decode:  q [B][H_q][D], one row per sequence; indices [B][cap], budgets [B].
+ * prefill: q [B][Tq][H_q][D] at absolute positions q_start.., Tq % 64 == 0, q_start % 64 == 0;
+ *          indices [B*Tq/64][cap], budgets [B*Tq/64]; seq_len unused (keys up to q_start+Tq-1 must exist).
+ * indices == NULL means "every block" (the dense comparator); budgets is then ignored.
+ * lse (optional, fp32 [B][H_q] decode / [B][Tq][H_q] prefill): natural-log sum-exp of the scaled logits.
+ * Requires H_q % H_kv == 0, H_q/H_kv <= 16, D == 128, blk == 64.
+ * --------------------------------------------------------------------------------------------------- */
+typedef struct {
+    const uint16_t* q;
+    const uint16_t* k;
+    const uint16_t* v;
+    int64_t kv_stride_batch, kv_stride_token, kv_stride_head; /* in elements */
+    const int32_t* seq_len;      /* [B] device (decode) */
+    int32_t max_seq_len;         /* host upper bound of seq_len (decode; sizes the dense grid)            */
+    const int32_t* indices;
+    const int32_t* budgets;
+    int32_t cap;                 /* row stride of indices                                                 */
+    int32_t B, Tq, H_q, H_kv, D;
+    int32_t q_start;
+    int32_t blk;
+    float sm_scale;
+    uint16_t* out;               /* BF16, same shape as q                                                 */
+    float* lse;                  /* optional                                                              */
+    void* workspace;
+    size_t workspace_bytes;
+} spot_attn_params;
+
+size_t spot_sparse_attn_decode_workspace_bytes(const spot_attn_params* p);
+spot_status spot_sparse_attn_decode(const spot_attn_params* p, void* stream);
+
+size_t spot_sparse_attn_prefill_workspace_bytes(const spot_attn_params* p);
+spot_status spot_sparse_attn_prefill(const spot_attn_params* p, void* stream);
+
+/* Bench-only comparator: dense flash-decode of the same shapes (every block, no index list).  Same
+ * parameter block; indices / budgets are ignored. */
+size_t spot_dense_attn_decode_workspace_bytes(const spot_attn_params* p);
+spot_status spot_dense_attn_decode(const spot_attn_params* p, void* stream);
+
+/* ---------------------------------------------------------------------------------------------------
+ * Host-buffer convenience (the "e2e" path of bench.py): one decode layer-step with every tensor in HOST
+ * memory.  Copies inputs host->device into caller-provided device staging buffers, runs
+ * spot_select + spot_sparse_attn_decode, copies out/indices/budgets back, all on `stream`, no sync.
+ * (Declared here so that the end-to-end measurement also crosses the C ABI.)
+ * --------------------------------------------------------------------------------------------------- */
+typedef struct {
+    /* host inputs for this step */
+    const uint16_t* sel_q_host;  /* [B][H_idx][d_idx] */
+    const float* w_host;         /* [B][H_idx] */
+    const uint16_t* q_host;      /* [B][H_q][D] */
+    /* host outputs */
+    uint16_t* out_host;          /* [B][H_q][D] */
+    int32_t* budgets_host;       /* [B] */
+    /* device-resident state and staging; select/attn hold the device pointers of everything else */
+    spot_select_params select;   /* sel_q / w point at device staging */
+    spot_attn_params attn;       /* q / out point at device staging   */
+} spot_decode_step_host_params;
+
+spot_status spot_decode_step_host(const spot_decode_step_host_params* p, void* stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SPOT_H_ */

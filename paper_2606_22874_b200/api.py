@@ -1,0 +1,144 @@
+"""Thin Python binding of the C ABI in include/spot.h -- same names, argument marshalling only.
+
+torch supplies device memory (`tensor.data_ptr()`) and the stream; every step of the path runs in libspot.so.
+BF16 tensors may be torch.bfloat16 or raw bit patterns (torch.uint16 / int16)."""
+import ctypes as C
+
+import torch
+
+from . import _lib as L
+from ._lib import AttnParams, DecodeStepHostParams, SelectParams, FORMATS, MODES  # noqa: F401
+
+
+class SpotError(RuntimeError):
+    def __init__(self, status, where):
+        lib = L.load()
+        name = lib.spot_status_string(status).decode()
+        extra = ""
+        if status == L.SPOT_ERR_CUDA:
+            extra = " (cudaError %d)" % lib.spot_last_cuda_error()
+        super().__init__("%s: %s%s" % (where, name, extra))
+        self.status = status
+
+
+def _check(status, where):
+    if status != L.SPOT_OK:
+        raise SpotError(status, where)
+
+
+def _ptr(t):
+    return None if t is None else C.c_void_p(t.data_ptr())
+
+
+def _stream(stream=None):
+    s = torch.cuda.current_stream() if stream is None else stream
+    return C.c_void_p(s.cuda_stream)
+
+
+def _fmt(fmt):
+    return FORMATS[fmt] if isinstance(fmt, str) else int(fmt)
+
+
+def spot_version():
+    return L.load().spot_version().decode()
+
+
+def spot_selector_k_bytes(fmt, B, cache_stride_tokens, H_idx, d_idx):
+    return int(L.load().spot_selector_k_bytes(_fmt(fmt), B, cache_stride_tokens, H_idx, d_idx))
+
+
+def spot_quantize_selector_k(k_bf16, k_cache, fmt, B, n_tokens, token_offset, cache_stride_tokens, H_idx, d_idx,
+                             stream=None):
+    _check(L.load().spot_quantize_selector_k(_ptr(k_bf16), _ptr(k_cache), _fmt(fmt), B, n_tokens, token_offset,
+                                             cache_stride_tokens, H_idx, d_idx, _stream(stream)),
+           "spot_quantize_selector_k")
+
+
+def spot_dequantize_selector_k(k_cache, k_bf16_out, fmt, B, n_tokens, token_offset, cache_stride_tokens, H_idx,
+                               d_idx, stream=None):
+    _check(L.load().spot_dequantize_selector_k(_ptr(k_cache), _ptr(k_bf16_out), _fmt(fmt), B, n_tokens, token_offset,
+                                               cache_stride_tokens, H_idx, d_idx, _stream(stream)),
+           "spot_dequantize_selector_k")
+
+
+def make_select_params(sel_q, w, sel_k, fmt, cache_stride_tokens, seq_len, max_seq_len, B, Tq, H_idx, d_idx, *,
+                       q_start=0, blk=64, q_block=1, mode="dual_topp", top_k=0, p=0.9, sink_blocks=1,
+                       recency_blocks=2, kmin_blocks=8, temperature=1.0, indices=None, cap=0, budgets=None,
+                       block_scores=None, block_probs=None, nb_stride=0, workspace=None):
+    sp = SelectParams()
+    sp.sel_q, sp.w, sp.sel_k = sel_q.data_ptr(), w.data_ptr(), sel_k.data_ptr()
+    sp.fmt = _fmt(fmt)
+    sp.cache_stride_tokens = cache_stride_tokens
+    sp.seq_len = seq_len.data_ptr() if seq_len is not None else None
+    sp.max_seq_len = max_seq_len
+    sp.B, sp.Tq, sp.H_idx, sp.d_idx = B, Tq, H_idx, d_idx
+    sp.q_start, sp.blk, sp.q_block = q_start, blk, q_block
+    sp.mode = MODES[mode] if isinstance(mode, str) else int(mode)
+    sp.top_k, sp.p = top_k, float(p)
+    sp.sink_blocks, sp.recency_blocks, sp.kmin_blocks = sink_blocks, recency_blocks, kmin_blocks
+    sp.temperature = float(temperature)
+    sp.indices = indices.data_ptr() if indices is not None else None
+    sp.cap = cap
+    sp.budgets = budgets.data_ptr() if budgets is not None else None
+    sp.block_scores = block_scores.data_ptr() if block_scores is not None else None
+    sp.block_probs = block_probs.data_ptr() if block_probs is not None else None
+    sp.nb_stride = nb_stride
+    if workspace is not None:
+        sp.workspace, sp.workspace_bytes = workspace.data_ptr(), workspace.numel() * workspace.element_size()
+    return sp
+
+
+def spot_select_workspace_bytes(sp):
+    return int(L.load().spot_select_workspace_bytes(C.byref(sp)))
+
+
+def spot_select(sp, stream=None):
+    _check(L.load().spot_select(C.byref(sp), _stream(stream)), "spot_select")
+
+
+def make_attn_params(q, k, v, kv_strides, seq_len, max_seq_len, indices, budgets, cap, B, Tq, H_q, H_kv, D, *,
+                     q_start=0, blk=64, sm_scale=None, out=None, lse=None, workspace=None):
+    ap = AttnParams()
+    ap.q, ap.k, ap.v = q.data_ptr(), k.data_ptr(), v.data_ptr()
+    ap.kv_stride_batch, ap.kv_stride_token, ap.kv_stride_head = kv_strides
+    ap.seq_len = seq_len.data_ptr() if seq_len is not None else None
+    ap.max_seq_len = max_seq_len
+    ap.indices = indices.data_ptr() if indices is not None else None
+    ap.budgets = budgets.data_ptr() if budgets is not None else None
+    ap.cap = cap
+    ap.B, ap.Tq, ap.H_q, ap.H_kv, ap.D = B, Tq, H_q, H_kv, D
+    ap.q_start, ap.blk = q_start, blk
+    ap.sm_scale = float(D ** -0.5 if sm_scale is None else sm_scale)
+    ap.out = out.data_ptr() if out is not None else None
+    ap.lse = lse.data_ptr() if lse is not None else None
+    if workspace is not None:
+        ap.workspace, ap.workspace_bytes = workspace.data_ptr(), workspace.numel() * workspace.element_size()
+    return ap
+
+
+def spot_sparse_attn_decode_workspace_bytes(ap):
+    return int(L.load().spot_sparse_attn_decode_workspace_bytes(C.byref(ap)))
+
+
+def spot_sparse_attn_decode(ap, stream=None):
+    _check(L.load().spot_sparse_attn_decode(C.byref(ap), _stream(stream)), "spot_sparse_attn_decode")
+
+
+def spot_dense_attn_decode_workspace_bytes(ap):
+    return int(L.load().spot_dense_attn_decode_workspace_bytes(C.byref(ap)))
+
+
+def spot_dense_attn_decode(ap, stream=None):
+    _check(L.load().spot_dense_attn_decode(C.byref(ap), _stream(stream)), "spot_dense_attn_decode")
+
+
+def spot_sparse_attn_prefill_workspace_bytes(ap):
+    return int(L.load().spot_sparse_attn_prefill_workspace_bytes(C.byref(ap)))
+
+
+def spot_sparse_attn_prefill(ap, stream=None):
+    _check(L.load().spot_sparse_attn_prefill(C.byref(ap), _stream(stream)), "spot_sparse_attn_prefill")
+
+
+def spot_decode_step_host(hp, stream=None):
+    _check(L.load().spot_decode_step_host(C.byref(hp), _stream(stream)), "spot_decode_step_host")

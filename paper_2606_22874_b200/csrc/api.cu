@@ -1,0 +1,160 @@
+// C-ABI glue: status strings, device check, spot_select orchestration (score kernel -> selection kernel) and the
+// host-buffer decode step.  All argument validation happens here, on the host, before any launch.
+#include "common.cuh"
+
+namespace spot {
+
+static thread_local int g_last_cuda_error = 0;
+void set_last_cuda_error(int e) { g_last_cuda_error = e; }
+
+spot_status check_device() {
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) { set_last_cuda_error((int)e); return SPOT_ERR_CUDA; }
+    static thread_local int cached_dev = -1, cached_major = 0;
+    if (cached_dev != dev) {
+        int major = 0;
+        e = cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev);
+        if (e != cudaSuccess) { set_last_cuda_error((int)e); return SPOT_ERR_CUDA; }
+        cached_dev = dev; cached_major = major;
+    }
+    return cached_major == 10 ? SPOT_OK : SPOT_ERR_UNSUPPORTED;
+}
+
+int sm_count() {
+    static thread_local int cached = 0;
+    if (!cached) {
+        int dev = 0, n = 0;
+        if (cudaGetDevice(&dev) == cudaSuccess &&
+            cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && n > 0) cached = n;
+        else cached = 148;
+    }
+    return cached;
+}
+
+// kernels implemented in the other translation units
+spot_status score_decode(const spot_select_params* p, float* scores, int nb_stride, cudaStream_t s);
+spot_status score_prefill(const spot_select_params* p, float* scores, int nb_stride, cudaStream_t s);
+spot_status run_select(const spot_select_params* p, const float* scores, int nb_stride, int rows_per_seq, int max_nb,
+                       cudaStream_t s);
+
+namespace {
+
+struct SelectGeom {
+    int rows_per_seq;
+    int max_nb;       // largest number of visible blocks of any row
+    int nb_stride;    // row stride of the score matrix actually used
+    bool own_scores;  // scores live in the workspace
+};
+
+spot_status select_geometry(const spot_select_params* p, SelectGeom* g) {
+    if (!p) return SPOT_ERR_INVALID_ARG;
+    if (!p->sel_q || !p->w || !p->sel_k || !p->indices || !p->budgets) return SPOT_ERR_INVALID_ARG;
+    if (!aligned16(p->sel_q) || !aligned16(p->sel_k) || !aligned16(p->w)) return SPOT_ERR_INVALID_ARG;
+    if (p->fmt != SPOT_SELK_BF16 && p->fmt != SPOT_SELK_INT4_E4M3 && p->fmt != SPOT_SELK_MXFP4) return SPOT_ERR_INVALID_ARG;
+    if (p->mode != SPOT_MODE_TOPK && p->mode != SPOT_MODE_DUAL_TOPP) return SPOT_ERR_INVALID_ARG;
+    if (p->B <= 0 || p->Tq <= 0 || p->H_idx <= 0 || p->d_idx <= 0 || p->d_idx % 32 != 0) return SPOT_ERR_INVALID_ARG;
+    if (p->blk <= 0 || p->cap <= 0 || p->cache_stride_tokens <= 0) return SPOT_ERR_INVALID_ARG;
+    if (p->sink_blocks < 0 || p->recency_blocks < 0 || p->kmin_blocks < 0 || p->top_k < 0) return SPOT_ERR_INVALID_ARG;
+    if (p->mode == SPOT_MODE_DUAL_TOPP && !(p->p > 0.0 && p->p <= 1.0)) return SPOT_ERR_INVALID_ARG;
+    if (!(p->temperature > 0.0)) return SPOT_ERR_INVALID_ARG;
+    if (p->mode == SPOT_MODE_TOPK && p->top_k < p->sink_blocks + p->recency_blocks) return SPOT_ERR_INVALID_ARG;
+    if (p->fmt != SPOT_SELK_BF16 && p->cache_stride_tokens % SELK_TILE != 0) return SPOT_ERR_INVALID_ARG;
+    if (p->blk != 64) return SPOT_ERR_UNSUPPORTED;
+    int64_t max_tokens;
+    if (p->q_block == 1) {
+        if (p->Tq != 1 || !p->seq_len || p->max_seq_len <= 0) return SPOT_ERR_INVALID_ARG;
+        if (p->max_seq_len > p->cache_stride_tokens) return SPOT_ERR_INVALID_ARG;
+        g->rows_per_seq = 1;
+        max_tokens = p->max_seq_len;
+    } else if (p->q_block == 64) {
+        if (p->Tq % 64 != 0 || p->q_start < 0 || p->q_start % 64 != 0) return SPOT_ERR_INVALID_ARG;
+        if ((int64_t)p->q_start + p->Tq > p->cache_stride_tokens) return SPOT_ERR_INVALID_ARG;
+        g->rows_per_seq = p->Tq / 64;
+        max_tokens = (int64_t)p->q_start + p->Tq;
+    } else {
+        return SPOT_ERR_INVALID_ARG;
+    }
+    g->max_nb = (int)ceil_div64(max_tokens, p->blk);
+    int need_cap = p->mode == SPOT_MODE_DUAL_TOPP ? g->max_nb : (p->top_k < g->max_nb ? p->top_k : g->max_nb);
+    if (p->cap < need_cap) return SPOT_ERR_INVALID_ARG;
+    if (p->block_scores || p->block_probs) {
+        if (p->nb_stride < g->max_nb) return SPOT_ERR_INVALID_ARG;
+    }
+    g->own_scores = p->block_scores == nullptr;
+    g->nb_stride = g->own_scores ? ((g->max_nb + 3) & ~3) : p->nb_stride;
+    return SPOT_OK;
+}
+
+}  // namespace
+
+}  // namespace spot
+
+using namespace spot;
+
+extern "C" const char* spot_status_string(spot_status s) {
+    switch (s) {
+        case SPOT_OK: return "SPOT_OK";
+        case SPOT_ERR_INVALID_ARG: return "SPOT_ERR_INVALID_ARG";
+        case SPOT_ERR_UNSUPPORTED: return "SPOT_ERR_UNSUPPORTED";
+        case SPOT_ERR_WORKSPACE_TOO_SMALL: return "SPOT_ERR_WORKSPACE_TOO_SMALL";
+        case SPOT_ERR_CUDA: return "SPOT_ERR_CUDA";
+    }
+    return "SPOT_ERR_UNKNOWN";
+}
+
+extern "C" int spot_last_cuda_error(void) { return g_last_cuda_error; }
+extern "C" const char* spot_version(void) { return "0.1"; }
+extern "C" size_t spot_struct_size(int which) {
+    switch (which) {
+        case 0: return sizeof(spot_select_params);
+        case 1: return sizeof(spot_attn_params);
+        case 2: return sizeof(spot_decode_step_host_params);
+    }
+    return 0;
+}
+
+extern "C" size_t spot_select_workspace_bytes(const spot_select_params* p) {
+    SelectGeom g;
+    if (select_geometry(p, &g) != SPOT_OK) return 0;
+    size_t bytes = 256;
+    if (g.own_scores) bytes += (size_t)p->B * g.rows_per_seq * g.nb_stride * sizeof(float);
+    return bytes;
+}
+
+extern "C" spot_status spot_select(const spot_select_params* p, void* stream) {
+    SelectGeom g;
+    spot_status st = select_geometry(p, &g);
+    if (st != SPOT_OK) return st;
+    if ((st = check_device()) != SPOT_OK) return st;
+    float* scores = p->block_scores;
+    if (g.own_scores) {
+        size_t need = 256 + (size_t)p->B * g.rows_per_seq * g.nb_stride * sizeof(float);
+        if (!p->workspace || p->workspace_bytes < need) return SPOT_ERR_WORKSPACE_TOO_SMALL;
+        scores = reinterpret_cast<float*>(reinterpret_cast<uintptr_t>(p->workspace) + 255 & ~(uintptr_t)255);
+    }
+    cudaStream_t s = (cudaStream_t)stream;
+    if (p->q_block == 1) st = score_decode(p, scores, g.nb_stride, s);
+    else st = score_prefill(p, scores, g.nb_stride, s);
+    if (st != SPOT_OK) return st;
+    return run_select(p, scores, g.nb_stride, g.rows_per_seq, g.max_nb, s);
+}
+
+extern "C" spot_status spot_decode_step_host(const spot_decode_step_host_params* p, void* stream) {
+    if (!p || !p->sel_q_host || !p->w_host || !p->q_host || !p->out_host || !p->budgets_host) return SPOT_ERR_INVALID_ARG;
+    const spot_select_params& sp = p->select;
+    const spot_attn_params& ap = p->attn;
+    if (sp.q_block != 1 || sp.B != ap.B) return SPOT_ERR_INVALID_ARG;
+    cudaStream_t s = (cudaStream_t)stream;
+    SPOT_CUDA_TRY(cudaMemcpyAsync((void*)sp.sel_q, p->sel_q_host, (size_t)sp.B * sp.H_idx * sp.d_idx * 2,
+                                  cudaMemcpyHostToDevice, s));
+    SPOT_CUDA_TRY(cudaMemcpyAsync((void*)sp.w, p->w_host, (size_t)sp.B * sp.H_idx * 4, cudaMemcpyHostToDevice, s));
+    SPOT_CUDA_TRY(cudaMemcpyAsync((void*)ap.q, p->q_host, (size_t)ap.B * ap.H_q * ap.D * 2, cudaMemcpyHostToDevice, s));
+    spot_status st = spot_select(&sp, stream);
+    if (st != SPOT_OK) return st;
+    st = spot_sparse_attn_decode(&ap, stream);
+    if (st != SPOT_OK) return st;
+    SPOT_CUDA_TRY(cudaMemcpyAsync(p->out_host, ap.out, (size_t)ap.B * ap.H_q * ap.D * 2, cudaMemcpyDeviceToHost, s));
+    SPOT_CUDA_TRY(cudaMemcpyAsync(p->budgets_host, sp.budgets, (size_t)sp.B * 4, cudaMemcpyDeviceToHost, s));
+    return SPOT_OK;
+}

@@ -1,0 +1,340 @@
+// Step a3 -- block-sparse GQA flash-decode over the selected 64-token KV blocks (PAPER.md:47 Fig. 2, :71), and the
+// dense comparator (every block) from the same code.
+//
+// HBM-bound: 32 KiB of K+V per (selected block, KV head), 4-8 flop/B.  Split-K over the index list: CTA
+// (chunk, kv head, sequence) owns up to `chunk_blocks` consecutive entries of the sequence's index list.  Inside the
+// CTA every warp runs its OWN cp.async ring over its 16-token quarter of each block (8 KiB of K+V per stage, zero
+// CTA-wide barriers in the main loop), feeds ldmatrix -> mma.sync m16n8k16 with the G = H_q/H_kv query heads of the
+// group as the (padded) M = 16 rows, and keeps a private online-softmax state.  The warps' states are merged through
+// shared memory at the end and written as an unnormalised partial (m, l, O); a second small kernel merges the
+// partials of all chunks (log-sum-exp) and writes BF16.  M is tiny here, so this is mma.sync territory, not tcgen05:
+// the tensor pipe needs < 15 % of the time the HBM stream takes.
+#include "common.cuh"
+
+namespace spot {
+
+namespace {
+
+constexpr int ATT_WARPS = 4;
+constexpr int ATT_STAGES = 3;
+constexpr int ATT_D = 128;
+constexpr int SUB_TOK = 16;                               // tokens per warp per block
+constexpr int STAGE_BYTES = 2 * SUB_TOK * ATT_D * 2;      // K + V sub-tiles: 8 KiB
+constexpr int ATT_SMEM = ATT_WARPS * ATT_STAGES * STAGE_BYTES;   // 96 KiB -> 2 CTAs per SM
+
+struct AttnArgs {
+    const uint16_t* q;
+    const uint16_t* k;
+    const uint16_t* v;
+    int64_t sb, st, sh;          // element strides: batch, token, head
+    const int32_t* seq_len;
+    const int32_t* indices;      // nullptr: dense
+    const int32_t* budgets;
+    int cap;
+    int H_q, H_kv, G;
+    float scale_log2;            // sm_scale * log2(e)
+    int chunk_blocks, n_chunks;
+    float* part_o;               // [B][H_kv][n_chunks][G][128]
+    float* part_ml;              // [B][H_kv][n_chunks][G][2]
+    uint16_t* out;
+    float* lse;
+};
+
+// smem sub-tile: [16 rows][256 B], 16-byte chunk index XOR-swizzled with (row & 7)
+__device__ __forceinline__ uint32_t sw_off(int row, int chunk) { return (uint32_t)(row * 256 + ((chunk ^ (row & 7)) << 4)); }
+
+__device__ __forceinline__ void issue_subtile(uint32_t smem_stage, const uint16_t* kbase, const uint16_t* vbase,
+                                              int64_t st, int tok0, int L, int lane) {
+    // 16 rows x 16 chunks of 16 B for K and again for V: 8 + 8 cp.async per lane
+#pragma unroll
+    for (int i = 0; i < 8; ++i) {
+        int id = i * 32 + lane;
+        int row = id >> 4, ch = id & 15;
+        int tok = tok0 + row;
+        bool ok = tok < L;
+        int64_t off = (int64_t)(ok ? tok : (L - 1)) * st + ch * 8;
+        cp_async16(smem_stage + sw_off(row, ch), kbase + off, ok);
+        cp_async16(smem_stage + SUB_TOK * 256 + sw_off(row, ch), vbase + off, ok);
+    }
+}
+
+__global__ void __launch_bounds__(ATT_WARPS * 32, 2) attn_decode_kernel(AttnArgs a) {
+    extern __shared__ __align__(128) unsigned char smem[];
+    const int chunk = blockIdx.x, hk = blockIdx.y, b = blockIdx.z;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int g = lane >> 2, c = lane & 3;
+    const int L = a.seq_len[b];
+    const int n_b = (L + 63) >> 6;
+    const int budget = a.indices ? min(a.budgets[b], a.cap) : n_b;
+    const int jbeg = chunk * a.chunk_blocks;
+    const int jend = min(jbeg + a.chunk_blocks, budget);
+    if (jbeg >= jend) return;
+    const int G = a.G;
+
+    // Q fragments (A operand): rows = query heads of this KV group, zero-padded to 16.
+    uint32_t qa[8][4];
+    {
+        const uint16_t* qb = a.q + ((int64_t)b * a.H_q + (int64_t)hk * G) * ATT_D;
+#pragma unroll
+        for (int ks = 0; ks < 8; ++ks) {
+            int col = ks * 16 + c * 2;
+            qa[ks][0] = (g < G) ? *reinterpret_cast<const uint32_t*>(qb + g * ATT_D + col) : 0u;
+            qa[ks][1] = (g + 8 < G) ? *reinterpret_cast<const uint32_t*>(qb + (g + 8) * ATT_D + col) : 0u;
+            qa[ks][2] = (g < G) ? *reinterpret_cast<const uint32_t*>(qb + g * ATT_D + col + 8) : 0u;
+            qa[ks][3] = (g + 8 < G) ? *reinterpret_cast<const uint32_t*>(qb + (g + 8) * ATT_D + col + 8) : 0u;
+        }
+    }
+
+    const uint16_t* kbase = a.k + (int64_t)b * a.sb + (int64_t)hk * a.sh;
+    const uint16_t* vbase = a.v + (int64_t)b * a.sb + (int64_t)hk * a.sh;
+    const int32_t* idx = a.indices ? a.indices + (int64_t)b * a.cap : nullptr;
+    const uint32_t my_smem = smem_u32(smem) + warp * (ATT_STAGES * STAGE_BYTES);
+
+    float o[16][4];
+#pragma unroll
+    for (int i = 0; i < 16; ++i) o[i][0] = o[i][1] = o[i][2] = o[i][3] = 0.f;
+    float m0 = -INFINITY, m1 = -INFINITY, l0 = 0.f, l1 = 0.f;
+
+    const int n_it = jend - jbeg;
+    // the chunk's block ids, one per lane (chunk_blocks <= 32), broadcast by shuffle when needed
+    const int my_blk = (lane < n_it) ? (idx ? idx[jbeg + lane] : (jbeg + lane)) : 0;
+    // prologue: fill STAGES-1 stages
+#pragma unroll
+    for (int s = 0; s < ATT_STAGES - 1; ++s) {
+        if (s < n_it) {
+            int blk_id = __shfl_sync(0xffffffffu, my_blk, s);
+            issue_subtile(my_smem + s * STAGE_BYTES, kbase, vbase, a.st, blk_id * 64 + warp * SUB_TOK, L, lane);
+        }
+        cp_async_commit();
+    }
+
+    for (int it = 0; it < n_it; ++it) {
+        {
+            int nx = it + ATT_STAGES - 1;
+            if (nx < n_it) {
+                int blk_id = __shfl_sync(0xffffffffu, my_blk, nx);
+                issue_subtile(my_smem + (nx % ATT_STAGES) * STAGE_BYTES, kbase, vbase, a.st,
+                              blk_id * 64 + warp * SUB_TOK, L, lane);
+            }
+            cp_async_commit();
+        }
+        cp_async_wait<ATT_STAGES - 1>();
+        __syncwarp();
+
+        const uint32_t ks_base = my_smem + (it % ATT_STAGES) * STAGE_BYTES;
+        const uint32_t vs_base = ks_base + SUB_TOK * 256;
+        const int blk_id = __shfl_sync(0xffffffffu, my_blk, it);
+        const int tok0 = blk_id * 64 + warp * SUB_TOK;
+
+        // S = Q K^T : 16 (heads) x 16 (tokens), k = 128
+        float s[2][4] = {{0.f, 0.f, 0.f, 0.f}, {0.f, 0.f, 0.f, 0.f}};
+        {
+            const int mi = lane >> 3, r8 = lane & 7;
+            const int row = (mi >> 1) * 8 + r8;
+#pragma unroll
+            for (int ks = 0; ks < 8; ++ks) {
+                uint32_t b0, b1, b2, b3;
+                ldmatrix_x4(b0, b1, b2, b3, ks_base + sw_off(row, 2 * ks + (mi & 1)));
+                mma_bf16_16816(s[0], qa[ks][0], qa[ks][1], qa[ks][2], qa[ks][3], b0, b1);
+                mma_bf16_16816(s[1], qa[ks][0], qa[ks][1], qa[ks][2], qa[ks][3], b2, b3);
+            }
+        }
+        // scale to the log2 domain, mask tokens beyond the sequence (only the ragged last block can have any)
+#pragma unroll
+        for (int nt = 0; nt < 2; ++nt)
+#pragma unroll
+            for (int e = 0; e < 4; ++e) {
+                int tok = tok0 + nt * 8 + c * 2 + (e & 1);
+                s[nt][e] = (tok < L) ? s[nt][e] * a.scale_log2 : -INFINITY;
+            }
+        // online softmax, rows g (m0, l0) and g + 8 (m1, l1)
+        float mx0 = fmaxf(fmaxf(s[0][0], s[0][1]), fmaxf(s[1][0], s[1][1]));
+        float mx1 = fmaxf(fmaxf(s[0][2], s[0][3]), fmaxf(s[1][2], s[1][3]));
+        mx0 = fmaxf(mx0, __shfl_xor_sync(0xffffffffu, mx0, 1));
+        mx0 = fmaxf(mx0, __shfl_xor_sync(0xffffffffu, mx0, 2));
+        mx1 = fmaxf(mx1, __shfl_xor_sync(0xffffffffu, mx1, 1));
+        mx1 = fmaxf(mx1, __shfl_xor_sync(0xffffffffu, mx1, 2));
+        const float mn0 = fmaxf(m0, mx0), mn1 = fmaxf(m1, mx1);
+        const float mu0 = (mn0 == -INFINITY) ? 0.f : mn0, mu1 = (mn1 == -INFINITY) ? 0.f : mn1;
+        const float c0 = fast_exp2(m0 - mu0), c1 = fast_exp2(m1 - mu1);
+        m0 = mn0; m1 = mn1;
+        float ps0 = 0.f, ps1 = 0.f;
+#pragma unroll
+        for (int nt = 0; nt < 2; ++nt) {
+            s[nt][0] = fast_exp2(s[nt][0] - mu0); s[nt][1] = fast_exp2(s[nt][1] - mu0);
+            s[nt][2] = fast_exp2(s[nt][2] - mu1); s[nt][3] = fast_exp2(s[nt][3] - mu1);
+            ps0 += s[nt][0] + s[nt][1];
+            ps1 += s[nt][2] + s[nt][3];
+        }
+        l0 = l0 * c0 + ps0;
+        l1 = l1 * c1 + ps1;
+#pragma unroll
+        for (int i = 0; i < 16; ++i) { o[i][0] *= c0; o[i][1] *= c0; o[i][2] *= c1; o[i][3] *= c1; }
+
+        // O += P V : P (16 x 16 tokens) as A, V (16 tokens x 128) as B through ldmatrix.trans
+        const uint32_t pa0 = pack_bf16x2(s[0][0], s[0][1]), pa1 = pack_bf16x2(s[0][2], s[0][3]);
+        const uint32_t pa2 = pack_bf16x2(s[1][0], s[1][1]), pa3 = pack_bf16x2(s[1][2], s[1][3]);
+        {
+            const int mi = lane >> 3, r8 = lane & 7;
+            const int row = (mi & 1) * 8 + r8;
+#pragma unroll
+            for (int nd = 0; nd < 16; nd += 2) {
+                uint32_t b0, b1, b2, b3;
+                ldmatrix_x4_trans(b0, b1, b2, b3, vs_base + sw_off(row, nd + (mi >> 1)));
+                mma_bf16_16816(o[nd], pa0, pa1, pa2, pa3, b0, b1);
+                mma_bf16_16816(o[nd + 1], pa0, pa1, pa2, pa3, b2, b3);
+            }
+        }
+        __syncwarp();   // everyone is done reading this stage before a later iteration refills it
+    }
+    cp_async_wait<0>();
+
+    // full row sums
+    l0 += __shfl_xor_sync(0xffffffffu, l0, 1); l0 += __shfl_xor_sync(0xffffffffu, l0, 2);
+    l1 += __shfl_xor_sync(0xffffffffu, l1, 1); l1 += __shfl_xor_sync(0xffffffffu, l1, 2);
+
+    // merge the 4 warps through shared memory (the rings are idle now)
+    __syncthreads();
+    float* so = reinterpret_cast<float*>(smem);                  // [warp][16][128]
+    float* sml = so + ATT_WARPS * 16 * ATT_D;                    // [warp][16][2]
+#pragma unroll
+    for (int nd = 0; nd < 16; ++nd) {
+        int col = nd * 8 + c * 2;
+        *reinterpret_cast<float2*>(so + (warp * 16 + g) * ATT_D + col) = make_float2(o[nd][0], o[nd][1]);
+        *reinterpret_cast<float2*>(so + (warp * 16 + g + 8) * ATT_D + col) = make_float2(o[nd][2], o[nd][3]);
+    }
+    if (c == 0) {
+        sml[(warp * 16 + g) * 2] = m0; sml[(warp * 16 + g) * 2 + 1] = l0;
+        sml[(warp * 16 + g + 8) * 2] = m1; sml[(warp * 16 + g + 8) * 2 + 1] = l1;
+    }
+    __syncthreads();
+    const int64_t pbase = (((int64_t)b * a.H_kv + hk) * a.n_chunks + chunk) * G;
+    for (int r = 0; r < G; ++r) {
+        float mw[ATT_WARPS], M = -INFINITY;
+#pragma unroll
+        for (int w = 0; w < ATT_WARPS; ++w) { mw[w] = sml[(w * 16 + r) * 2]; M = fmaxf(M, mw[w]); }
+        const float Mu = (M == -INFINITY) ? 0.f : M;
+        float acc = 0.f, lsum = 0.f;
+#pragma unroll
+        for (int w = 0; w < ATT_WARPS; ++w) {
+            float f = fast_exp2(mw[w] - Mu);
+            acc += f * so[(w * 16 + r) * ATT_D + threadIdx.x];
+            lsum += f * sml[(w * 16 + r) * 2 + 1];
+        }
+        a.part_o[(pbase + r) * ATT_D + threadIdx.x] = acc;
+        if (threadIdx.x == 0) { a.part_ml[(pbase + r) * 2] = M; a.part_ml[(pbase + r) * 2 + 1] = lsum; }
+    }
+}
+
+// merge the chunk partials of one (sequence, query head); 128 threads = 128 output dims
+__global__ void __launch_bounds__(128) attn_merge_kernel(AttnArgs a) {
+    const int h = blockIdx.x, b = blockIdx.y;
+    const int G = a.G, hk = h / G, r = h - hk * G;
+    const int L = a.seq_len[b];
+    const int budget = a.indices ? min(a.budgets[b], a.cap) : ((L + 63) >> 6);
+    const int nch = (budget + a.chunk_blocks - 1) / a.chunk_blocks;
+    const int64_t base = ((int64_t)b * a.H_kv + hk) * a.n_chunks;
+    float M = -INFINITY;
+    for (int ch = 0; ch < nch; ++ch) M = fmaxf(M, a.part_ml[((base + ch) * G + r) * 2]);
+    const float Mu = (M == -INFINITY) ? 0.f : M;
+    float acc = 0.f, lsum = 0.f;
+    for (int ch = 0; ch < nch; ++ch) {
+        const int64_t pr = (base + ch) * G + r;
+        float f = fast_exp2(a.part_ml[pr * 2] - Mu);
+        acc += f * a.part_o[pr * ATT_D + threadIdx.x];
+        lsum += f * a.part_ml[pr * 2 + 1];
+    }
+    float outv = (lsum > 0.f) ? acc / lsum : 0.f;
+    a.out[((int64_t)b * a.H_q + h) * ATT_D + threadIdx.x] = __bfloat16_as_ushort(__float2bfloat16_rn(outv));
+    if (a.lse && threadIdx.x == 0)
+        a.lse[(int64_t)b * a.H_q + h] = (lsum > 0.f) ? (M + log2f(lsum)) * 0.6931471805599453f : -INFINITY;
+}
+
+int pick_chunk_blocks(const spot_attn_params* p, bool dense) {
+    // enough CTAs for ~4 waves of 2 CTAs/SM at the largest possible budget, at most 8 blocks (256 KiB of KV per
+    // head) per CTA so that the partials stay < 2 % of the traffic
+    int64_t max_blocks = dense ? (p->max_seq_len + 63) / 64 : p->cap;
+    int64_t total = max_blocks * p->H_kv * p->B;
+    int64_t want = (int64_t)sm_count() * 2 * 4;
+    int64_t cb = total / want;
+    if (cb < 1) cb = 1;
+    if (cb > 8) cb = 8;   // must stay <= 32 (one block id per lane)
+    return (int)cb;
+}
+
+spot_status check_attn(const spot_attn_params* p, bool dense, bool prefill) {
+    if (!p || !p->q || !p->k || !p->v || !p->out) return SPOT_ERR_INVALID_ARG;
+    if (!aligned16(p->q) || !aligned16(p->k) || !aligned16(p->v) || !aligned16(p->out)) return SPOT_ERR_INVALID_ARG;
+    if (p->B <= 0 || p->H_q <= 0 || p->H_kv <= 0 || p->H_q % p->H_kv != 0) return SPOT_ERR_INVALID_ARG;
+    if (p->H_q / p->H_kv > 16) return SPOT_ERR_UNSUPPORTED;
+    if (p->D != 128 || p->blk != 64) return SPOT_ERR_UNSUPPORTED;
+    if (p->kv_stride_token < p->D || p->kv_stride_token % 8 || p->kv_stride_head % 8 || p->kv_stride_batch % 8)
+        return SPOT_ERR_INVALID_ARG;
+    if (!dense && p->indices && (!p->budgets || p->cap <= 0)) return SPOT_ERR_INVALID_ARG;
+    if (!prefill) {
+        if (!p->seq_len || p->max_seq_len <= 0) return SPOT_ERR_INVALID_ARG;
+    }
+    return SPOT_OK;
+}
+
+size_t decode_ws_bytes(const spot_attn_params* p, bool dense) {
+    const bool use_idx = !dense && p->indices;
+    int cb = pick_chunk_blocks(p, !use_idx);
+    int64_t max_blocks = use_idx ? p->cap : (p->max_seq_len + 63) / 64;
+    int64_t n_chunks = (max_blocks + cb - 1) / cb;
+    return (size_t)((int64_t)p->B * p->H_q * n_chunks * (ATT_D + 2) * 4);
+}
+
+spot_status run_decode(const spot_attn_params* p, bool dense, cudaStream_t s) {
+    spot_status stt = check_attn(p, dense, false);
+    if (stt != SPOT_OK) return stt;
+    if ((stt = check_device()) != SPOT_OK) return stt;
+    const bool use_idx = !dense && p->indices;
+    int cb = pick_chunk_blocks(p, !use_idx);
+    int64_t max_blocks = use_idx ? p->cap : (p->max_seq_len + 63) / 64;
+    int n_chunks = (int)((max_blocks + cb - 1) / cb);
+    size_t need = (size_t)((int64_t)p->B * p->H_q * n_chunks * (ATT_D + 2) * 4);
+    if (!p->workspace || p->workspace_bytes < need) return SPOT_ERR_WORKSPACE_TOO_SMALL;
+    AttnArgs a;
+    a.q = p->q; a.k = p->k; a.v = p->v;
+    a.sb = p->kv_stride_batch; a.st = p->kv_stride_token; a.sh = p->kv_stride_head;
+    a.seq_len = p->seq_len; a.indices = use_idx ? p->indices : nullptr; a.budgets = p->budgets; a.cap = p->cap;
+    a.H_q = p->H_q; a.H_kv = p->H_kv; a.G = p->H_q / p->H_kv;
+    a.scale_log2 = p->sm_scale * 1.4426950408889634f;
+    a.chunk_blocks = cb; a.n_chunks = n_chunks;
+    a.part_o = reinterpret_cast<float*>(p->workspace);
+    a.part_ml = a.part_o + (int64_t)p->B * p->H_q * n_chunks * ATT_D;
+    a.out = p->out; a.lse = p->lse;
+    static bool attr_set = false;
+    if (!attr_set) {
+        SPOT_CUDA_TRY(cudaFuncSetAttribute(attn_decode_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, ATT_SMEM));
+        attr_set = true;
+    }
+    dim3 grid((unsigned)n_chunks, (unsigned)p->H_kv, (unsigned)p->B);
+    attn_decode_kernel<<<grid, ATT_WARPS * 32, ATT_SMEM, s>>>(a);
+    SPOT_LAUNCH_CHECK();
+    attn_merge_kernel<<<dim3((unsigned)p->H_q, (unsigned)p->B), 128, 0, s>>>(a);
+    SPOT_LAUNCH_CHECK();
+    return SPOT_OK;
+}
+
+}  // namespace
+
+}  // namespace spot
+
+using namespace spot;
+
+extern "C" size_t spot_sparse_attn_decode_workspace_bytes(const spot_attn_params* p) {
+    if (!p || check_attn(p, false, false) != SPOT_OK) return 0;
+    return decode_ws_bytes(p, false);
+}
+extern "C" spot_status spot_sparse_attn_decode(const spot_attn_params* p, void* stream) {
+    return run_decode(p, false, (cudaStream_t)stream);
+}
+extern "C" size_t spot_dense_attn_decode_workspace_bytes(const spot_attn_params* p) {
+    if (!p || check_attn(p, true, false) != SPOT_OK) return 0;
+    return decode_ws_bytes(p, true);
+}
+extern "C" spot_status spot_dense_attn_decode(const spot_attn_params* p, void* stream) {
+    return run_decode(p, true, (cudaStream_t)stream);
+}

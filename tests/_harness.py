@@ -1,0 +1,145 @@
+"""Test-side glue: moves a seeded workload to the GPU, calls the C ABI through the Python binding, and runs the
+fp64 oracle on the same bits.  Holds the parity protocol for index lists."""
+import numpy as np
+
+from oracle import attention as OA
+from oracle import quant as OQ
+from oracle import selection as OS
+from oracle.bf16 import bf16_bits_to_f64, f64_to_bf16_bits_exact
+
+
+def dev_u16(arr):
+    import torch
+    return torch.from_numpy(np.ascontiguousarray(arr).view(np.int16)).cuda()
+
+
+def to_np_u16(t):
+    return t.cpu().numpy().view(np.uint16)
+
+
+class DeviceDecode:
+    """A DecodeWorkload resident on the GPU, selector cache in one format."""
+
+    def __init__(self, wl, fmt="bf16", with_kv=True):
+        import torch
+        from paper_2606_22874_b200 import api
+        self.wl, self.fmt, self.api = wl, fmt, api
+        self.sel_q = dev_u16(wl.sel_q)
+        self.w = torch.from_numpy(wl.w).cuda()
+        self.seq_len = torch.from_numpy(wl.seq_len).cuda()
+        self.max_seq_len = int(wl.seq_len.max())
+        self.L_cap = wl.L_cap
+        sel_k_bf16 = dev_u16(wl.sel_k)
+        if fmt == "bf16":
+            self.sel_k = sel_k_bf16
+        else:
+            assert wl.L_cap % 64 == 0
+            nbytes = api.spot_selector_k_bytes(fmt, wl.B, wl.L_cap, wl.H_idx, wl.d_idx)
+            self.sel_k = torch.zeros(nbytes, dtype=torch.uint8, device="cuda")
+            api.spot_quantize_selector_k(sel_k_bf16, self.sel_k, fmt, wl.B, wl.L_cap, 0, wl.L_cap, wl.H_idx, wl.d_idx)
+        if with_kv and wl.K is not None:
+            self.q = dev_u16(wl.q)
+            self.K = dev_u16(wl.K)
+            self.V = dev_u16(wl.V)
+            self.kv_strides = (wl.H_kv * wl.L_cap * wl.D, wl.D, wl.L_cap * wl.D)   # [B][H_kv][L][D]
+        self.n_b_max = -(-self.max_seq_len // wl.blk)
+
+    def select(self, cap=None, want_scores=True, want_probs=True, **over):
+        import torch
+        wl, api = self.wl, self.api
+        kw = dict(mode=wl.mode, top_k=wl.top_k, p=wl.p, sink_blocks=wl.sink_blocks,
+                  recency_blocks=wl.recency_blocks, kmin_blocks=wl.kmin_blocks, temperature=wl.temperature)
+        kw.update(over)
+        cap = self.n_b_max if cap is None else cap
+        self.cap = cap
+        self.indices = torch.full((wl.B, cap), -7, dtype=torch.int32, device="cuda")
+        self.budgets = torch.full((wl.B,), -7, dtype=torch.int32, device="cuda")
+        nb_stride = (self.n_b_max + 3) & ~3
+        scores = torch.full((wl.B, nb_stride), float("nan"), device="cuda") if want_scores else None
+        probs = torch.full((wl.B, nb_stride), float("nan"), device="cuda") if want_probs else None
+        sp = api.make_select_params(self.sel_q, self.w, self.sel_k, self.fmt, self.L_cap, self.seq_len,
+                                    self.max_seq_len, wl.B, 1, wl.H_idx, wl.d_idx, blk=wl.blk, q_block=1,
+                                    indices=self.indices, cap=cap, budgets=self.budgets, block_scores=scores,
+                                    block_probs=probs, nb_stride=nb_stride, **kw)
+        ws = torch.empty(max(api.spot_select_workspace_bytes(sp), 16), dtype=torch.uint8, device="cuda")
+        sp.workspace, sp.workspace_bytes = ws.data_ptr(), ws.numel()
+        api.spot_select(sp)
+        torch.cuda.synchronize()
+        return (self.indices.cpu().numpy(), self.budgets.cpu().numpy(),
+                None if scores is None else scores.cpu().numpy(), None if probs is None else probs.cpu().numpy())
+
+    def attend(self, indices_np=None, budgets_np=None, dense=False, want_lse=True):
+        import torch
+        wl, api = self.wl, self.api
+        out = torch.zeros((wl.B, wl.H_q, wl.D), dtype=torch.int16, device="cuda")
+        lse = torch.zeros((wl.B, wl.H_q), device="cuda") if want_lse else None
+        if dense:
+            idx = bud = None
+            cap = 0
+        else:
+            idx = torch.from_numpy(np.ascontiguousarray(indices_np, dtype=np.int32)).cuda()
+            bud = torch.from_numpy(np.ascontiguousarray(budgets_np, dtype=np.int32)).cuda()
+            cap = idx.shape[1]
+        ap = api.make_attn_params(self.q, self.K, self.V, self.kv_strides, self.seq_len, self.max_seq_len, idx, bud,
+                                  cap, wl.B, 1, wl.H_q, wl.H_kv, wl.D, blk=wl.blk, sm_scale=wl.sm_scale, out=out,
+                                  lse=lse)
+        fn_ws = api.spot_dense_attn_decode_workspace_bytes if dense else api.spot_sparse_attn_decode_workspace_bytes
+        ws = torch.empty(max(fn_ws(ap), 16), dtype=torch.uint8, device="cuda")
+        ap.workspace, ap.workspace_bytes = ws.data_ptr(), ws.numel()
+        (api.spot_dense_attn_decode if dense else api.spot_sparse_attn_decode)(ap)
+        torch.cuda.synchronize()
+        return bf16_bits_to_f64(to_np_u16(out)), (None if lse is None else lse.cpu().numpy())
+
+
+# ------------------------------------------------------------------------------------------------------
+# oracle side
+# ------------------------------------------------------------------------------------------------------
+
+def oracle_keys(wl, fmt, b):
+    """fp64 selector keys of sequence b as the given cache format stores them."""
+    return OQ.quantize_dequantize(fmt, wl.sel_k[b])
+
+
+def oracle_select(wl, fmt, b, **over):
+    kw = wl.select_kwargs()
+    kw.update(over)
+    mode = kw.pop("mode", wl.mode)
+    return OS.select_decode(bf16_bits_to_f64(wl.sel_q[b]), wl.w[b].astype(np.float64), oracle_keys(wl, fmt, b),
+                            int(wl.seq_len[b]), wl.blk, mode, **kw)
+
+
+def oracle_attend(wl, b, blocks):
+    K = bf16_bits_to_f64(wl.K[b]).transpose(1, 0, 2)    # [L][H_kv][D]
+    V = bf16_bits_to_f64(wl.V[b]).transpose(1, 0, 2)
+    return OA.sparse_attn_decode(bf16_bits_to_f64(wl.q[b]), K, V, blocks, int(wl.seq_len[b]), wl.blk, wl.sm_scale)
+
+
+# ------------------------------------------------------------------------------------------------------
+# parity protocol for index lists (north_star: bit-exact "except where two block scores differ by less than 1e-6
+# relative at the cut, which is reported"; DESIGN.md section 6 adds the mass-near-cut class)
+# ------------------------------------------------------------------------------------------------------
+
+def classify_selection(s_bar, sel, gpu_idx, gpu_budget, p=None, rel=1e-6):
+    """-> 'exact' | 'score-near-tie' | 'mass-near-cut' | 'FAIL: ...'."""
+    want = sel.indices.tolist()
+    got = [int(x) for x in gpu_idx[:gpu_budget]]
+    if got != sorted(set(got)) or any(x < 0 for x in got):
+        return "FAIL: index list not strictly ascending / negative"
+    if got == want and gpu_budget == sel.budget:
+        return "exact"
+    diff = set(got) ^ set(want)
+    order = sel.order.tolist()
+    if sel.n_taken == 0 or sel.n_taken > len(order):
+        return "FAIL: sets differ %s" % sorted(diff)
+    cut_score = s_bar[order[sel.n_taken - 1]]
+    tol = rel * max(abs(cut_score), 1e-30)
+    if len(got) == len(want) and all(abs(s_bar[b] - cut_score) <= tol for b in diff):
+        return "score-near-tie"
+    if p is not None and sel.cum is not None and abs(len(got) - len(want)) == 1 and sel.n_taken == sel.n_star:
+        n = sel.n_star
+        below = sel.cum[n - 2] if n >= 2 else 0.0
+        margin = min(p - below, sel.cum[n - 1] - p)
+        rank_pos = {b: r for r, b in enumerate(order)}
+        if margin < rel and all(abs(rank_pos.get(b, -99) - (n - 1)) <= 1 for b in diff):
+            return "mass-near-cut"
+    return "FAIL: sets differ %s (budget %d vs %d)" % (sorted(diff)[:8], gpu_budget, sel.budget)

@@ -1,0 +1,165 @@
+"""GPU parity, decode path (-m gpu): the CUDA library behind the C ABI vs the fp64 oracle on the same seeded bits.
+
+Tolerances (BASELINE.json north_star): indices/budgets bit-exact except reported near-ties at the cut (1e-6
+relative); dequantised selector keys bit-exact (+0 == -0); probabilities within 1e-3 abs; attention within
+max-abs 2e-2 / mean-abs 2e-3 on the oracle's selected set."""
+import numpy as np
+import pytest
+
+from tests import _harness as H
+from oracle import quant as OQ
+from oracle.bf16 import bf16_bits_to_f64
+from workloads import make_config, make_decode_workload
+
+pytestmark = pytest.mark.gpu
+
+MAX_ABS, MEAN_ABS, PROB_ABS = 2e-2, 2e-3, 1e-3
+
+
+@pytest.fixture(scope="module")
+def torch_cuda():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    from paper_2606_22874_b200 import _lib
+    _lib.load()          # fails loudly if libspot.so is missing: no fallback
+    return torch
+
+
+# ---------------------------------------------------------------- a0 quantisers
+@pytest.mark.parametrize("fmt", ["mxfp4", "int4_e4m3"])
+def test_quantise_dequantise_bit_exact(torch_cuda, fmt):
+    torch = torch_cuda
+    from paper_2606_22874_b200 import api
+    rng = np.random.Generator(np.random.Philox(11))
+    B, L, Hh, d = 2, 192, 4, 64
+    x = rng.standard_normal((B, L, Hh, d)).astype(np.float32)
+    x[0, 0, 0, :32] = 0.0                                  # all-zero group
+    x[0, 1, 0, :32] *= 1e-30                               # tiny group
+    x[0, 2, 0, :32] *= 1e30                                # huge group (INT4 scale saturates at 448)
+    x[0, 3, 0, :8] = [-0.0, 0.25, 0.75, 1.25, 1.75, 2.5, 3.5, 5.0]      # E2M1 ties (with amax 6 -> X = 1)
+    x[0, 3, 0, 8] = 6.0
+    x[0, 4, 0, :32] = np.arange(-16, 16) * 0.5              # INT4 ties at .5
+    from workloads import f32_to_bf16_bits
+    bits = f32_to_bf16_bits(x).reshape(B, L, Hh, d)
+    k = H.dev_u16(bits)
+    cache = torch.zeros(api.spot_selector_k_bytes(fmt, B, L, Hh, d), dtype=torch.uint8, device="cuda")
+    # quantise in two calls (prefill part + appended tokens) to cover token_offset
+    api.spot_quantize_selector_k(k[:, :130].contiguous(), cache, fmt, B, 130, 0, L, Hh, d)
+    api.spot_quantize_selector_k(k[:, 130:].contiguous(), cache, fmt, B, L - 130, 130, L, Hh, d)
+    out = torch.zeros((B, L, Hh, d), dtype=torch.int16, device="cuda")
+    api.spot_dequantize_selector_k(cache, out, fmt, B, L, 0, L, Hh, d)
+    torch.cuda.synchronize()
+    got = bf16_bits_to_f64(H.to_np_u16(out))
+    want = OQ.quantize_dequantize(fmt, bits)
+    assert np.array_equal(got, want)                        # numeric equality: +0 == -0, everything else bit-exact
+    assert cache.numel() == OQ.selector_k_bytes(fmt, B * L * Hh * d)
+
+
+# ---------------------------------------------------------------- a1 + a2
+def _check_select(dd, fmt, report, **over):
+    wl = dd.wl
+    idx, bud, scores, probs = dd.select(**over)
+    p = over.get("p", wl.p)
+    mode = over.get("mode", wl.mode)
+    for b in range(wl.B):
+        s_bar, sel = H.oracle_select(wl, fmt, b, **over)
+        n_b = len(s_bar)
+        assert np.allclose(scores[b, :n_b], s_bar, rtol=2e-5, atol=2e-5), (b, np.abs(scores[b, :n_b] - s_bar).max())
+        if mode == "dual_topp":
+            assert np.abs(probs[b, :n_b] - sel.probs).max() <= PROB_ABS
+        cls = H.classify_selection(s_bar, sel, idx[b], int(bud[b]), p if mode == "dual_topp" else None)
+        assert not cls.startswith("FAIL"), (wl.name, fmt, b, cls)
+        report.append((wl.name, fmt, b, cls, int(bud[b])))
+        assert np.all(idx[b, int(bud[b]):] == -1)
+    return idx, bud
+
+
+@pytest.mark.parametrize("fmt", ["bf16", "mxfp4", "int4_e4m3"])
+@pytest.mark.parametrize("cfg", ["cfg1", "mini2", "mini3", "mini4"])
+def test_select_matches_oracle(torch_cuda, cfg, fmt):
+    wl = make_config(cfg, with_kv=False)
+    dd = H.DeviceDecode(wl, fmt, with_kv=False)
+    report = []
+    _check_select(dd, fmt, report)
+    if wl.mode == "dual_topp":
+        for p in (0.7, 0.95, 1.0):
+            _check_select(dd, fmt, report, p=p)
+        _check_select(dd, fmt, report, mode="topk", top_k=16)
+    non_exact = [r for r in report if r[3] != "exact"]
+    print("near-tie report:", non_exact)
+    assert len(non_exact) <= max(1, len(report) // 10)
+
+
+def test_select_edge_cases(torch_cuda):
+    # tiny contexts (n_b <= reserved), ragged tails, negative weights, exact score ties, d_idx = 128
+    for seed, L, seqs, kind, d_idx in [(1, 64, [1, 63, 64], "gauss", 64), (2, 320, [65, 129, 320], "gauss", 64),
+                                       (3, 1024, [1000, 1024, 513], "gauss", 128), (4, 2048, [2048, 1999, 777], "zipf", 128)]:
+        wl = make_decode_workload("edge%d" % seed, seed, B=3, L=L, kind=kind, seq_lens=seqs, d_idx=d_idx,
+                                  with_kv=False)
+        if seed == 2:
+            wl.sel_k[2, 64:128] = wl.sel_k[2, 128:192]      # blocks 1 and 2 tie exactly -> index tie-break (R7)
+        for fmt in ("bf16", "mxfp4", "int4_e4m3"):
+            dd = H.DeviceDecode(wl, fmt, with_kv=False)
+            report = []
+            for over in (dict(), dict(p=0.5, kmin_blocks=0), dict(sink_blocks=0, recency_blocks=0, kmin_blocks=0),
+                         dict(mode="topk", top_k=5), dict(mode="topk", top_k=3, sink_blocks=0, recency_blocks=0)):
+                _check_select(dd, fmt, report, **over)
+
+
+# ---------------------------------------------------------------- a3
+def _check_attend(dd, idx_lists, dense=False):
+    wl = dd.wl
+    cap = max(len(x) for x in idx_lists)
+    idx = np.full((wl.B, cap), -1, dtype=np.int32)
+    for b, x in enumerate(idx_lists):
+        idx[b, :len(x)] = x
+    bud = np.array([len(x) for x in idx_lists], dtype=np.int32)
+    out, lse = dd.attend(idx, bud, dense=dense)
+    for b in range(wl.B):
+        want, want_lse = H.oracle_attend(wl, b, idx_lists[b])
+        err = np.abs(out[b] - want)
+        assert err.max() <= MAX_ABS and err.mean() <= MEAN_ABS, (wl.name, b, err.max(), err.mean())
+        assert np.abs(lse[b] - want_lse).max() <= 1e-3
+
+
+@pytest.mark.parametrize("cfg", ["cfg1", "mini2", "mini4"])
+def test_sparse_attention_on_oracle_selection(torch_cuda, cfg):
+    wl = make_config(cfg)
+    dd = H.DeviceDecode(wl, "bf16")
+    lists = [H.oracle_select(wl, "bf16", b)[1].indices.tolist() for b in range(wl.B)]
+    _check_attend(dd, lists)
+
+
+def test_dense_comparator_and_p1_equal_dense(torch_cuda):
+    wl = make_config("mini4")
+    dd = H.DeviceDecode(wl, "bf16")
+    all_blocks = [list(range(-(-int(L) // wl.blk))) for L in wl.seq_len]
+    _check_attend(dd, all_blocks, dense=True)
+    _check_attend(dd, all_blocks, dense=False)          # p = 1: every block through the index list
+
+
+def test_attention_token_major_layout_and_tiny(torch_cuda):
+    torch = torch_cuda
+    wl = make_decode_workload("nhd", 9, B=2, L=200, kind="gauss", seq_lens=[200, 70])
+    dd = H.DeviceDecode(wl, "bf16")
+    # re-layout K/V as [B][L][H_kv][D]
+    dd.K = H.dev_u16(np.ascontiguousarray(wl.K.transpose(0, 2, 1, 3)))
+    dd.V = H.dev_u16(np.ascontiguousarray(wl.V.transpose(0, 2, 1, 3)))
+    dd.kv_strides = (wl.L_cap * wl.H_kv * wl.D, wl.H_kv * wl.D, wl.D)
+    _check_attend(dd, [[0, 2, 3], [1]])
+    _check_attend(dd, [[3], [0, 1]])                     # ragged last blocks only
+
+
+def test_end_to_end_step_matches_oracle(torch_cuda):
+    """select -> attend on the GPU's own index list; compare with the oracle attending over the ORACLE's list
+    (identical whenever the selection is exact, which the test requires here)."""
+    wl = make_config("mini2")
+    dd = H.DeviceDecode(wl, "bf16")
+    idx, bud, _, _ = dd.select()
+    out, _ = dd.attend(idx, bud)
+    for b in range(wl.B):
+        s_bar, sel = H.oracle_select(wl, "bf16", b)
+        assert idx[b, :bud[b]].tolist() == sel.indices.tolist()
+        want, _ = H.oracle_attend(wl, b, sel.indices)
+        err = np.abs(out[b] - want)
+        assert err.max() <= MAX_ABS and err.mean() <= MEAN_ABS
