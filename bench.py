@@ -1,0 +1,351 @@
+#!/usr/bin/env python
+"""bench.py -- one decode layer-step of the SpotAttention hot path (selector scoring -> dual top-p -> block-sparse
+GQA attention) on synthetic Qwen3-shaped inputs, through the C ABI of include/spot.h.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg3] [--fmt bf16|mxfp4|int4_e4m3] [--p 0.9]
+    python bench.py --impl reference ...       # the fp64 CPU oracle on a bounded sample (rank 0 only)
+
+Prints ONE JSON line (rank 0).  A "step" = spot_select + spot_sparse_attn_decode over one batch (all of SURVEY.md
+section 8(a)'s decode rows: a1 score + block max, a2 distribution + selection, a3 sparse attention; a0 runs once, before
+the timed region, because the cache is quantised when tokens are appended, not per step).  The L2 is flushed (a
+read sweep over a 512 MiB buffer) before every timed step; each step is timed with its own CUDA-event pair on the
+launching stream and the flush sits outside the pairs.  DESIGN.md section 7 states the byte accounting."""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "decode us/layer-step (selector+sparse attn) @L=128K; % of HBM roofline"
+N_LAYERS = {32: 36, 64: 64}       # Qwen3-8B-shaped: 36 layers; 32B-shaped: 64 (model card)
+
+
+def measured_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as f:
+            d = json.load(f)
+        return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled during the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index=0):
+        self.index, self.rows, self._stop = index, [], threading.Event()
+        self.t = threading.Thread(target=self._run, daemon=True)
+
+    def _run(self):
+        while not self._stop.is_set():
+            try:
+                out = subprocess.run(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                                      "--format=csv,noheader,nounits"], capture_output=True, text=True, timeout=5).stdout
+                parts = [x.strip() for x in out.strip().split(",")]
+                if len(parts) >= 7:
+                    self.rows.append(parts)
+            except Exception:
+                pass
+            self._stop.wait(0.1)
+
+    def __enter__(self):
+        self.t.start()
+        return self
+
+    def __exit__(self, *a):
+        self._stop.set()
+        self.t.join(timeout=6)
+
+    def summary(self):
+        if not self.rows:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["unavailable"]}
+        sm = sorted(float(r[0]) for r in self.rows)
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = [n for i, n in enumerate(names) if any(r[3 + i].lower().startswith("active") for r in self.rows)]
+        return {"sm_mhz": sm[len(sm) // 2], "sm_max_mhz": float(self.rows[0][1]), "reasons": reasons,
+                "samples": len(self.rows)}
+
+
+# ------------------------------------------------------------------------------------------------------
+def build_workload(name, overrides):
+    from workloads import make_config
+    return make_config(name, with_kv=False, **overrides)
+
+
+def oracle_step_sample(wl, fmt, K0, V0, q0, p):
+    """The oracle's decode layer-step for sequence 0 (select + attend), as it stands.  Returns seconds, budget."""
+    from oracle import attention as OA
+    from oracle import quant as OQ
+    from oracle import selection as OS
+    from oracle.bf16 import bf16_bits_to_f64
+    t0 = time.perf_counter()
+    keys = OQ.quantize_dequantize(fmt, wl.sel_k[0])
+    kw = wl.select_kwargs()
+    kw["p"] = p
+    s_bar, sel = OS.select_decode(bf16_bits_to_f64(wl.sel_q[0]), wl.w[0].astype(np.float64), keys,
+                                  int(wl.seq_len[0]), wl.blk, wl.mode, **kw)
+    OA.sparse_attn_decode(bf16_bits_to_f64(q0), bf16_bits_to_f64(K0).transpose(1, 0, 2),
+                          bf16_bits_to_f64(V0).transpose(1, 0, 2), sel.indices, int(wl.seq_len[0]), wl.blk, wl.sm_scale)
+    return time.perf_counter() - t0, sel.budget
+
+
+def host_kv_for_seq0(wl, seed):
+    """Sequence 0's K/V/q as BF16 bits on the host, N(0,1) (used by the reference arm, which has no GPU copy)."""
+    from workloads import f32_to_bf16_bits
+    rng = np.random.Generator(np.random.Philox(seed + 17))
+    K0 = f32_to_bf16_bits(rng.standard_normal((wl.H_kv, wl.L_cap, wl.D), dtype=np.float32))
+    V0 = f32_to_bf16_bits(rng.standard_normal((wl.H_kv, wl.L_cap, wl.D), dtype=np.float32))
+    return K0, V0, wl.q[0]
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    wl = build_workload(args.workload, {})
+    K0, V0, q0 = host_kv_for_seq0(wl, wl.seed)
+    times = []
+    budget = 0
+    for i in range(args.warmup + args.steps):
+        dt, budget = oracle_step_sample(wl, args.fmt, K0, V0, q0, args.p)
+        if i >= args.warmup:
+            times.append(dt)
+    per_seq = float(np.mean(times))
+    us = per_seq * wl.B * 1e6
+    cores = len(os.sched_getaffinity(0))
+    line = {
+        "impl": "reference", "metric": METRIC, "value": us, "unit": "us/layer-step", "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": us / 1e3, "higher_is_better": False,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": args.workload, "fmt": args.fmt, "p": args.p, "B": wl.B, "L": wl.L_cap},
+        "cpu_baseline": {"value": us, "unit": "us/layer-step", "cores": cores, "kind": "oracle",
+                         "sample": "sequence 0 of %d (select + attend, budget %d blocks), time x B" % (wl.B, budget)},
+        "e2e": {"value": us, "unit": "us/layer-step", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+    }
+    print(json.dumps(line))
+
+
+# ------------------------------------------------------------------------------------------------------
+def run_ours(args):
+    import ctypes as C
+
+    import torch
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local_rank)
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    from paper_2606_22874_b200 import _lib, api
+    from paper_2606_22874_b200 import build as B
+    B.build()
+    _lib.load()                                   # no fallback: raises if the CUDA library is missing
+
+    # every rank runs the same-shaped batch of independent sequences (its own seed): weak scaling, no collective
+    wl = build_workload(args.workload, {})
+    if rank:
+        from workloads import CONFIGS, make_decode_workload
+        kw = dict(CONFIGS[args.workload])
+        kw["seed"] = kw["seed"] + 1000 * rank
+        wl = make_decode_workload(args.workload, with_kv=False, **kw)
+    dev = torch.device("cuda", local_rank)
+    Bn, L, Hq, Hkv, D = wl.B, wl.L_cap, wl.H_q, wl.H_kv, wl.D
+    gen = torch.Generator(device=dev)
+    gen.manual_seed(wl.seed + 17)
+    K = torch.randn((Bn, Hkv, L, D), generator=gen, device=dev, dtype=torch.bfloat16)
+    V = torch.randn((Bn, Hkv, L, D), generator=gen, device=dev, dtype=torch.bfloat16)
+    q = torch.from_numpy(wl.q.view(np.int16)).to(dev)
+    sel_q = torch.from_numpy(wl.sel_q.view(np.int16)).to(dev)
+    w = torch.from_numpy(wl.w).to(dev)
+    seq_len = torch.from_numpy(wl.seq_len).to(dev)
+    sel_k_bf16 = torch.from_numpy(wl.sel_k.view(np.int16)).to(dev)
+    sel_bytes = api.spot_selector_k_bytes(args.fmt, Bn, L, wl.H_idx, wl.d_idx)
+    if args.fmt == "bf16":
+        sel_k = sel_k_bf16
+    else:
+        sel_k = torch.zeros(sel_bytes, dtype=torch.uint8, device=dev)
+        api.spot_quantize_selector_k(sel_k_bf16, sel_k, args.fmt, Bn, L, 0, L, wl.H_idx, wl.d_idx)
+        del sel_k_bf16
+    n_b = -(-L // wl.blk)
+    cap = n_b
+    indices = torch.empty((Bn, cap), dtype=torch.int32, device=dev)
+    budgets = torch.empty((Bn,), dtype=torch.int32, device=dev)
+    out = torch.empty((Bn, Hq, D), dtype=torch.int16, device=dev)
+    sp = api.make_select_params(sel_q, w, sel_k, args.fmt, L, seq_len, L, Bn, 1, wl.H_idx, wl.d_idx, blk=wl.blk,
+                                q_block=1, mode=wl.mode, top_k=wl.top_k, p=args.p, sink_blocks=wl.sink_blocks,
+                                recency_blocks=wl.recency_blocks, kmin_blocks=wl.kmin_blocks,
+                                temperature=wl.temperature, indices=indices, cap=cap, budgets=budgets)
+    ws_sel = torch.empty(max(16, api.spot_select_workspace_bytes(sp)), dtype=torch.uint8, device=dev)
+    sp.workspace, sp.workspace_bytes = ws_sel.data_ptr(), ws_sel.numel()
+    kv_strides = (Hkv * L * D, D, L * D)
+    ap = api.make_attn_params(q, K, V, kv_strides, seq_len, L, indices, budgets, cap, Bn, 1, Hq, Hkv, D, blk=wl.blk,
+                              sm_scale=wl.sm_scale, out=out)
+    ws_att = torch.empty(max(16, api.spot_sparse_attn_decode_workspace_bytes(ap)), dtype=torch.uint8, device=dev)
+    ap.workspace, ap.workspace_bytes = ws_att.data_ptr(), ws_att.numel()
+    apd = api.make_attn_params(q, K, V, kv_strides, seq_len, L, None, None, 0, Bn, 1, Hq, Hkv, D, blk=wl.blk,
+                               sm_scale=wl.sm_scale, out=torch.empty_like(out))
+    ws_den = torch.empty(max(16, api.spot_dense_attn_decode_workspace_bytes(apd)), dtype=torch.uint8, device=dev)
+    apd.workspace, apd.workspace_bytes = ws_den.data_ptr(), ws_den.numel()
+
+    flush = torch.empty(512 << 20, dtype=torch.uint8, device=dev).zero_()
+    stream = torch.cuda.current_stream()
+
+    def flush_l2():
+        flush.view(torch.int64).sum()             # read sweep: leaves the L2 full of clean lines
+
+    def step():
+        api.spot_select(sp, stream)
+        api.spot_sparse_attn_decode(ap, stream)
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            import torch.distributed as dist
+            dist.barrier()
+            torch.cuda.synchronize()
+
+    for _ in range(max(args.warmup, 3)):
+        flush_l2()
+        step()
+    barrier()
+
+    ev = [[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(args.steps)]
+    with ClockSampler(local_rank) as clk:
+        for i in range(args.steps):
+            flush_l2()
+            ev[i][0].record(stream)
+            api.spot_select(sp, stream)
+            ev[i][1].record(stream)
+            api.spot_sparse_attn_decode(ap, stream)
+            ev[i][2].record(stream)
+        barrier()
+    sel_ms = np.array([e[0].elapsed_time(e[1]) for e in ev])
+    att_ms = np.array([e[1].elapsed_time(e[2]) for e in ev])
+    step_ms = np.array([e[0].elapsed_time(e[2]) for e in ev])
+    clocks = clk.summary()
+
+    # dense comparator (same shapes, every block)
+    den = []
+    for i in range(max(3, min(args.steps, 10)) + 2):
+        flush_l2()
+        a, b_ = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record(stream)
+        api.spot_dense_attn_decode(apd, stream)
+        b_.record(stream)
+        torch.cuda.synchronize()
+        if i >= 2:
+            den.append(a.elapsed_time(b_))
+
+    # e2e: host buffers through spot_decode_step_host (H2D of the step's q / q^I / w, D2H of out + budgets)
+    hp = api.DecodeStepHostParams()
+    h_selq = torch.from_numpy(wl.sel_q.view(np.int16)).pin_memory()
+    h_w = torch.from_numpy(wl.w).pin_memory()
+    h_q = torch.from_numpy(wl.q.view(np.int16)).pin_memory()
+    h_out = torch.empty((Bn, Hq, D), dtype=torch.int16).pin_memory()
+    h_bud = torch.empty((Bn,), dtype=torch.int32).pin_memory()
+    hp.sel_q_host, hp.w_host, hp.q_host = h_selq.data_ptr(), h_w.data_ptr(), h_q.data_ptr()
+    hp.out_host, hp.budgets_host = h_out.data_ptr(), h_bud.data_ptr()
+    hp.select, hp.attn = sp, ap
+    h2d = h_selq.numel() * 2 + h_w.numel() * 4 + h_q.numel() * 2
+    d2h = h_out.numel() * 2 + h_bud.numel() * 4
+    e2e = []
+    for i in range(args.steps + 2):
+        flush_l2()
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        api.spot_decode_step_host(hp, stream)
+        torch.cuda.synchronize()
+        if i >= 2:
+            e2e.append((time.perf_counter() - t0) * 1e3)
+    bud_host = h_bud.numpy().copy()
+
+    step_mean = float(step_ms.mean())
+    if world > 1:
+        import torch.distributed as dist
+        t = torch.tensor([step_mean], device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        step_mean = float(t.item())
+    if rank != 0:
+        return
+
+    peak, peak_src = measured_peaks()
+    bytes_per_tok = {"bf16": wl.H_idx * wl.d_idx * 2}.get(args.fmt, wl.H_idx * wl.d_idx // 2 + wl.H_idx * wl.d_idx // 32)
+    sel_alg = float(np.sum(wl.seq_len.astype(np.int64)) * bytes_per_tok)
+    kv_alg = float(np.sum(bud_host.astype(np.int64)) * wl.blk * Hkv * D * 2 * 2)
+    att_s = float(att_ms.mean()) * 1e-3
+    achieved = kv_alg / att_s / 1e9
+    traffic = None
+    tpath = os.path.join(ROOT, "profiles", "traffic.json")
+    if os.path.exists(tpath):
+        with open(tpath) as f:
+            traffic = json.load(f).get("%s/%s/attn_decode_kernel" % (args.workload, args.fmt))
+    us = step_mean * 1e3
+    n_layers = N_LAYERS.get(Hq, 36)
+
+    # oracle on the host cores, bounded sample: sequence 0 (needs its K/V bits back on the host)
+    K0 = K[0].view(torch.int16).cpu().numpy().view(np.uint16)
+    V0 = V[0].view(torch.int16).cpu().numpy().view(np.uint16)
+    cpu_t, cpu_budget = oracle_step_sample(wl, args.fmt, K0, V0, wl.q[0], args.p)
+    line = {
+        "metric": METRIC, "value": us, "unit": "us/layer-step", "n_gpus": world, "steps": args.steps,
+        "warmup": max(args.warmup, 3), "ms_per_step": step_mean, "higher_is_better": False, "scaling": "weak",
+        "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
+        "config": {"workload": args.workload, "B": Bn, "L": L, "H_q": Hq, "H_kv": Hkv, "D": D,
+                   "selector": "%dx%d %s" % (wl.H_idx, wl.d_idx, args.fmt), "blk": wl.blk, "mode": wl.mode,
+                   "p": args.p, "sink/recency/kmin": [wl.sink_blocks, wl.recency_blocks, wl.kmin_blocks],
+                   "budgets": bud_host.tolist(), "l2": "flushed by a 512 MiB read sweep before every timed step",
+                   "kv": "N(0,1) BF16 generated on the device (seeded); selector side from workloads/"},
+        "tokens_per_s": world * Bn / (n_layers * step_mean * 1e-3),
+        "breakdown_us": {"select (score+select kernels)": float(sel_ms.mean()) * 1e3,
+                         "sparse attention (attn+merge kernels)": float(att_ms.mean()) * 1e3,
+                         "dense flash-decode comparator": float(np.mean(den)) * 1e3},
+        "step_roofline": {"bytes": sel_alg + kv_alg, "achieved_gbs": (sel_alg + kv_alg) / (step_mean * 1e-3) / 1e9,
+                          "frac_of_measured": (sel_alg + kv_alg) / (step_mean * 1e-3) / 1e9 / peak,
+                          "frac_of_8TBs": (sel_alg + kv_alg) / (step_mean * 1e-3) / 1e9 / 8000.0,
+                          "selector_bytes": sel_alg, "selected_kv_bytes": kv_alg,
+                          "selector_gbs": sel_alg / (float(sel_ms.mean()) * 1e-3) / 1e9},
+        "roofline": {"bound": "hbm", "kernel": "attn_decode_kernel", "achieved": achieved, "peak": peak, "unit": "GB/s",
+                     "frac": achieved / peak, "traffic": traffic, "peak_source": peak_src,
+                     "algorithmic_bytes": kv_alg},
+        "cpu_baseline": {"value": cpu_t * Bn * 1e6, "unit": "us/layer-step", "cores": len(os.sched_getaffinity(0)),
+                         "kind": "oracle",
+                         "sample": "sequence 0 of %d (select + attend, budget %d blocks), time x B" % (Bn, cpu_budget)},
+        "e2e": {"value": float(np.mean(e2e)) * 1e3, "unit": "us/layer-step", "h2d_bytes_per_step": h2d,
+                "d2h_bytes_per_step": d2h},
+        "gpu_launches": 4 * args.steps,
+        "clocks": clocks,
+        "paper_context": "paper: 3.9x FlashAttention / 1.8x Twilight end-to-end at L=128K, Qwen3-8B, one B200, Triton "
+                         "kernels (PAPER.md:146); other shapes, context only",
+    }
+    print(json.dumps(line))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="cfg3")
+    ap.add_argument("--fmt", default="bf16", choices=["bf16", "mxfp4", "int4_e4m3"])
+    ap.add_argument("--p", type=float, default=0.90)
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()
