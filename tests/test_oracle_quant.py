@@ -6,6 +6,7 @@
   exact rationals -- an independent definition of RNE, against the oracle's threshold chains;
 * exact round trips on grid-valued groups; error bounds; BF16-exactness of dequantised keys.
 """
+import os
 from fractions import Fraction
 
 import numpy as np
@@ -66,7 +67,8 @@ def test_golden_group_int4(golden):
 
 
 def test_e4m3_spot_values(golden):
-    with open(__import__("os").path.join(__import__("conftest").GOLDEN, "e4m3_spot.txt")) as f:
+    here = os.path.dirname(os.path.abspath(__file__))
+    with open(os.path.join(here, "golden", "e4m3_spot.txt")) as f:
         rows = [l.split() for l in f if l.strip() and not l.startswith("#")]
     for val, code in rows:
         got = int(quant.encode_e4m3_rne_satfinite(np.float32(float(val))))
