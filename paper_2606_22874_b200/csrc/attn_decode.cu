@@ -226,28 +226,52 @@ __global__ void __launch_bounds__(ATT_WARPS * 32, 2) attn_decode_kernel(AttnArgs
     }
 }
 
-// merge the chunk partials of one (sequence, query head); 128 threads = 128 output dims
-__global__ void __launch_bounds__(128) attn_merge_kernel(AttnArgs a) {
+// merge the chunk partials of one (sequence, query head): 8 warps take the chunks round-robin (one 512-byte partial
+// row per warp per step, float4 per lane), then the 8 partial sums are combined through shared memory.
+constexpr int MERGE_WARPS = 8;
+__global__ void __launch_bounds__(MERGE_WARPS * 32) attn_merge_kernel(AttnArgs a) {
+    __shared__ float s_m[MERGE_WARPS];
+    __shared__ __align__(16) float s_acc[MERGE_WARPS][ATT_D];
+    __shared__ float s_l[MERGE_WARPS];
     const int h = blockIdx.x, b = blockIdx.y;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int G = a.G, hk = h / G, r = h - hk * G;
     const int L = a.seq_len[b];
     const int budget = a.indices ? min(a.budgets[b], a.cap) : ((L + 63) >> 6);
     const int nch = (budget + a.chunk_blocks - 1) / a.chunk_blocks;
     const int64_t base = ((int64_t)b * a.H_kv + hk) * a.n_chunks;
     float M = -INFINITY;
-    for (int ch = 0; ch < nch; ++ch) M = fmaxf(M, a.part_ml[((base + ch) * G + r) * 2]);
+    for (int ch = threadIdx.x; ch < nch; ch += MERGE_WARPS * 32) M = fmaxf(M, a.part_ml[((base + ch) * G + r) * 2]);
+#pragma unroll
+    for (int o = 16; o; o >>= 1) M = fmaxf(M, __shfl_xor_sync(0xffffffffu, M, o));
+    if (lane == 0) s_m[warp] = M;
+    __syncthreads();
+#pragma unroll
+    for (int w = 0; w < MERGE_WARPS; ++w) M = fmaxf(M, s_m[w]);
     const float Mu = (M == -INFINITY) ? 0.f : M;
-    float acc = 0.f, lsum = 0.f;
-    for (int ch = 0; ch < nch; ++ch) {
+    float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
+    float lsum = 0.f;
+#pragma unroll 4
+    for (int ch = warp; ch < nch; ch += MERGE_WARPS) {
         const int64_t pr = (base + ch) * G + r;
-        float f = fast_exp2(a.part_ml[pr * 2] - Mu);
-        acc += f * a.part_o[pr * ATT_D + threadIdx.x];
-        lsum += f * a.part_ml[pr * 2 + 1];
+        const float2 ml = *reinterpret_cast<const float2*>(a.part_ml + pr * 2);
+        const float4 o = *reinterpret_cast<const float4*>(a.part_o + pr * ATT_D + lane * 4);
+        const float f = fast_exp2(ml.x - Mu);
+        acc.x += f * o.x; acc.y += f * o.y; acc.z += f * o.z; acc.w += f * o.w;
+        lsum += f * ml.y;
     }
-    float outv = (lsum > 0.f) ? acc / lsum : 0.f;
-    a.out[((int64_t)b * a.H_q + h) * ATT_D + threadIdx.x] = __bfloat16_as_ushort(__float2bfloat16_rn(outv));
-    if (a.lse && threadIdx.x == 0)
-        a.lse[(int64_t)b * a.H_q + h] = (lsum > 0.f) ? (M + log2f(lsum)) * 0.6931471805599453f : -INFINITY;
+    *reinterpret_cast<float4*>(&s_acc[warp][lane * 4]) = acc;
+    if (lane == 0) s_l[warp] = lsum;
+    __syncthreads();
+    if (threadIdx.x < ATT_D) {
+        float tot = 0.f, lt = 0.f;
+#pragma unroll
+        for (int w = 0; w < MERGE_WARPS; ++w) { tot += s_acc[w][threadIdx.x]; lt += s_l[w]; }
+        float outv = (lt > 0.f) ? tot / lt : 0.f;
+        a.out[((int64_t)b * a.H_q + h) * ATT_D + threadIdx.x] = __bfloat16_as_ushort(__float2bfloat16_rn(outv));
+        if (a.lse && threadIdx.x == 0)
+            a.lse[(int64_t)b * a.H_q + h] = (lt > 0.f) ? (M + log2f(lt)) * 0.6931471805599453f : -INFINITY;
+    }
 }
 
 int pick_chunk_blocks(const spot_attn_params* p, bool dense) {
@@ -313,7 +337,7 @@ spot_status run_decode(const spot_attn_params* p, bool dense, cudaStream_t s) {
     dim3 grid((unsigned)n_chunks, (unsigned)p->H_kv, (unsigned)p->B);
     attn_decode_kernel<<<grid, ATT_WARPS * 32, ATT_SMEM, s>>>(a);
     SPOT_LAUNCH_CHECK();
-    attn_merge_kernel<<<dim3((unsigned)p->H_q, (unsigned)p->B), 128, 0, s>>>(a);
+    attn_merge_kernel<<<dim3((unsigned)p->H_q, (unsigned)p->B), MERGE_WARPS * 32, 0, s>>>(a);
     SPOT_LAUNCH_CHECK();
     return SPOT_OK;
 }

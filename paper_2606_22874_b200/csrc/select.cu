@@ -1,18 +1,27 @@
 // Step a2 -- block distribution and selection rule, one CTA per selection row:
 // reserved sink/recency tier, residual softmax (Eq. 7), nucleus + K_min floor (Eq. 8) or static top-K (Eq. 6).
 //
-// Latency-bound (<= 8192 scores per row).  The residual blocks are sorted in shared memory by the 64-bit key
-// (~orderable(score), block id) -- ascending key order is (score descending, index ascending), the order R7 fixes.
-// The mass arithmetic (exp, normalisation, prefix sum, threshold test) runs in fp64 so that the only source of
-// disagreement with the fp64 oracle is the fp32 block score itself.
+// Latency-bound (<= 8192 scores per row, 4..16 rows at decode), so the kernel is built around the critical path:
+//   * every thread keeps 8 scores in registers as 32-bit order-preserving keys; element e lives at
+//     (warp w, register r, lane l) with e = 256 w + 32 r + l;
+//   * a bitonic sort of the KEYS ONLY (no payload): strides 1..16 are warp shuffles, strides 32..128 are
+//     register-to-register, strides >= 256 go through shared memory three at a time (a transposed layout makes
+//     three consecutive strides thread-local), i.e. 2 CTA barriers per three cross-warp strides instead of one per
+//     stride;
+//   * the mass of a block is a function of its score, so the sorted keys alone give the sorted masses: exp,
+//     normalisation and the prefix mass run in fp64 on the sorted keys (the only source of disagreement with the
+//     fp64 oracle is then the fp32 block score itself);
+//   * the cut is a key value tau = key of rank n_take-1; blocks with a better key are selected, blocks tied with tau
+//     are taken in ascending block index until n_take is reached -- exactly the (score descending, index
+//     ascending) order R7 fixes -- and the ascending index list falls out of one ballot/popc scan in index order.
 #include "common.cuh"
 
 namespace spot {
 
 namespace {
 
-constexpr int SEL_THREADS = 1024;
 constexpr int SEL_MAX_NB = 8192;
+constexpr uint32_t KEY_PAD = 0xffffffffu;
 
 __device__ __forceinline__ uint32_t orderable(float x) {
     uint32_t u = __float_as_uint(x + 0.0f);   // -0.0 -> +0.0
@@ -22,57 +31,9 @@ __device__ __forceinline__ float from_orderable(uint32_t o) {
     uint32_t u = (o & 0x80000000u) ? (o & 0x7fffffffu) : ~o;
     return __uint_as_float(u);
 }
-
-// inclusive scan of one double per thread across the CTA; `warp_tot` is a 32-entry shared scratch.
-__device__ double block_inclusive_scan(double v, double* warp_tot, double* total) {
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-#pragma unroll
-    for (int o = 1; o < 32; o <<= 1) {
-        double t = __shfl_up_sync(0xffffffffu, v, o);
-        if (lane >= o) v += t;
-    }
-    __syncthreads();
-    if (lane == 31) warp_tot[warp] = v;
-    __syncthreads();
-    if (warp == 0) {
-        double t = warp_tot[lane];
-#pragma unroll
-        for (int o = 1; o < 32; o <<= 1) {
-            double u = __shfl_up_sync(0xffffffffu, t, o);
-            if (lane >= o) t += u;
-        }
-        warp_tot[lane] = t;
-    }
-    __syncthreads();
-    double off = warp ? warp_tot[warp - 1] : 0.0;
-    *total = warp_tot[31];
-    return v + off;
-}
-
-__device__ int block_inclusive_scan_int(int v, int* warp_tot, int* total) {
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-#pragma unroll
-    for (int o = 1; o < 32; o <<= 1) {
-        int t = __shfl_up_sync(0xffffffffu, v, o);
-        if (lane >= o) v += t;
-    }
-    __syncthreads();
-    if (lane == 31) warp_tot[warp] = v;
-    __syncthreads();
-    if (warp == 0) {
-        int t = warp_tot[lane];
-#pragma unroll
-        for (int o = 1; o < 32; o <<= 1) {
-            int u = __shfl_up_sync(0xffffffffu, t, o);
-            if (lane >= o) t += u;
-        }
-        warp_tot[lane] = t;
-    }
-    __syncthreads();
-    int off = warp ? warp_tot[warp - 1] : 0;
-    *total = warp_tot[31];
-    return v + off;
-}
+// sort key: ascending key == descending score
+__device__ __forceinline__ uint32_t score_key(float s) { return ~orderable(s); }
+__device__ __forceinline__ float key_score(uint32_t k) { return from_orderable(~k); }
 
 struct SelectArgs {
     const float* scores;      // [rows][nb_stride]
@@ -89,140 +50,267 @@ struct SelectArgs {
     float* probs;             // optional [rows][nb_stride]
 };
 
-__global__ void __launch_bounds__(SEL_THREADS) select_kernel(SelectArgs a, int n_pow2_max) {
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    uint64_t* key = reinterpret_cast<uint64_t*>(smem_raw);                      // [n_pow2]
-    double* mass = reinterpret_cast<double*>(smem_raw + (size_t)n_pow2_max * 8);   // [n_pow2]
-    uint8_t* flag = reinterpret_cast<uint8_t*>(smem_raw + (size_t)n_pow2_max * 16); // [n_pow2]
-    __shared__ double wtot[32];
-    __shared__ int itot[32];
-    __shared__ int s_nstar;
+__device__ __forceinline__ void cmpx(uint32_t& a, uint32_t& b, bool asc) {
+    const uint32_t lo = min(a, b), hi = max(a, b);
+    a = asc ? lo : hi;
+    b = asc ? hi : lo;
+}
+
+// LT = log2(threads); the CTA sorts NPAD = 8 << LT keys.
+template <int LT>
+__global__ void __launch_bounds__(1 << LT) select_kernel(SelectArgs a) {
+    constexpr int T = 1 << LT;
+    constexpr int NPAD = 8 * T;
+    constexpr int LOGN = LT + 3;
+    constexpr int NSEG = T / 4;                 // 32-element rank segments: (warp, register)
+    static_assert(LT == 5 || LT >= 8, "cross-warp rounds need three register bits above bit 8");
+    __shared__ uint32_t s_key[NPAD];
+    __shared__ double s_seg[NSEG];
+    __shared__ int s_cnt[NSEG][2];
+    __shared__ double s_total;
+    __shared__ uint32_t s_bcast[2];
+    __shared__ int s_below;
+    __shared__ int s_tot[2];
 
     const int row = blockIdx.x;
     const int b = row / a.n_q, i = row - b * a.n_q;
-    const int tid = threadIdx.x;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     int n_b;
     if (a.q_block == 1) n_b = (a.seq_len[b] + a.blk - 1) / a.blk;
     else n_b = (a.q_start + (i + 1) * a.q_block - 1) / a.blk + 1;
-    n_b = min(n_b, SEL_MAX_NB);
+    n_b = min(n_b, NPAD);
     const int sink_end = min(a.sink, n_b);
-    const int rec_beg = max(0, n_b - a.rec);
-    int n_reserved = sink_end + (n_b - max(rec_beg, sink_end));
-    const int n_res = n_b - n_reserved;
-    int n = 1;
-    while (n < n_b) n <<= 1;
+    const int rec_beg = max(sink_end, n_b - a.rec);     // residual blocks: [sink_end, rec_beg)
+    const int n_res = rec_beg - sink_end;
+    const int n_reserved = n_b - n_res;
+    const int ebase = warp * 256 + lane;                // element of register r: ebase + 32 r
 
+    // ---- load: block scores -> keys (pads and reserved blocks sort last)
     const float* srow = a.scores + (int64_t)row * a.nb_stride;
-    for (int j = tid; j < n; j += SEL_THREADS) {
-        uint64_t k = ~0ull;
-        if (j < n_b && j >= sink_end && j < rec_beg) k = ((uint64_t)(~orderable(srow[j])) << 32) | (uint32_t)j;
-        key[j] = k;
-        flag[j] = (j < n_b && !(j >= sink_end && j < rec_beg)) ? 1 : 0;
+    uint32_t okey[8], key[8];
+#pragma unroll
+    for (int r = 0; r < 8; ++r) {
+        const int j = ebase + 32 * r;
+        okey[r] = (j >= sink_end && j < rec_beg) ? score_key(srow[j]) : KEY_PAD;
+        key[r] = okey[r];
     }
-    if (tid == 0) s_nstar = 0;
-    __syncthreads();
+    if (tid == 0) { s_below = 0; }
 
-    // bitonic sort, ascending
-    for (int k = 2; k <= n; k <<= 1) {
-        for (int j = k >> 1; j > 0; j >>= 1) {
-            for (int t = tid; t < (n >> 1); t += SEL_THREADS) {
-                int lo = ((t & ~(j - 1)) << 1) | (t & (j - 1));
-                int hi = lo | j;
-                bool asc = (lo & k) == 0;
-                uint64_t x = key[lo], y = key[hi];
-                if ((x > y) == asc) { key[lo] = y; key[hi] = x; }
+    // ---- bitonic sort, ascending
+#pragma unroll
+    for (int lk = 1; lk <= LOGN; ++lk) {
+        const int k = 1 << lk;
+#pragma unroll
+        for (int lj = lk - 1; lj >= 0; --lj) {
+            if (lj >= 8) {
+                // cross-warp strides, three at a time: the group whose lowest stride bit is ls is thread-local in
+                // the transposed layout idx_m = low + (m << ls) + (high << (ls + 3)).
+                if ((lk - 1 - lj) % 3 == 0) {            // first stride of its group: run the whole group here
+                    const int cnt = (lj - 7) >= 3 ? 3 : (lj - 7);
+                    const int ls = lj - cnt + 1;
+#pragma unroll
+                    for (int r = 0; r < 8; ++r) s_key[ebase + 32 * r] = key[r];
+                    __syncthreads();
+                    const int low = tid & ((1 << ls) - 1), high = tid >> ls;
+                    const int tbase = low + (high << (ls + 3));
+                    uint32_t v[8];
+#pragma unroll
+                    for (int m = 0; m < 8; ++m) v[m] = s_key[tbase + (m << ls)];
+#pragma unroll
+                    for (int bit = cnt - 1; bit >= 0; --bit) {
+#pragma unroll
+                        for (int m = 0; m < 8; ++m) {
+                            // the direction bit lk may itself be a register bit (lk < ls + 3): test it per element
+                            if ((m & (1 << bit)) == 0)
+                                cmpx(v[m], v[m | (1 << bit)], ((tbase + (m << ls)) & k) == 0);
+                        }
+                    }
+#pragma unroll
+                    for (int m = 0; m < 8; ++m) s_key[tbase + (m << ls)] = v[m];
+                    __syncthreads();
+#pragma unroll
+                    for (int r = 0; r < 8; ++r) key[r] = s_key[ebase + 32 * r];
+                }
+            } else if (lj >= 5) {
+                const int rr = 1 << (lj - 5);
+#pragma unroll
+                for (int r = 0; r < 8; ++r)
+                    if ((r & rr) == 0) cmpx(key[r], key[r | rr], ((ebase + 32 * r) & k) == 0);
+            } else {
+                const int j = 1 << lj;
+                const bool lower = (lane & j) == 0;
+#pragma unroll
+                for (int r = 0; r < 8; ++r) {
+                    const uint32_t other = __shfl_xor_sync(0xffffffffu, key[r], j);
+                    const bool asc = ((ebase + 32 * r) & k) == 0;
+                    key[r] = (asc == lower) ? min(key[r], other) : max(key[r], other);
+                }
             }
-            __syncthreads();
         }
     }
+    // key[r] now holds rank ebase + 32 r of the residual blocks (ranks >= n_res are pads).
 
     int n_take = 0;
+    double inv_total = 0.0, zmax = 0.0;
     if (a.mode == SPOT_MODE_TOPK) {
         n_take = min(max(0, a.top_k - n_reserved), n_res);
-        if (a.probs) {
-            for (int j = tid; j < n_b; j += SEL_THREADS) a.probs[(int64_t)row * a.nb_stride + j] = 0.f;
-        }
     } else {
-        // Eq. 7 in fp64 on the sorted residual blocks; z = s_bar / T; m = z of rank 0.
-        const int per = (n + SEL_THREADS - 1) / SEL_THREADS;      // consecutive ranks per thread (<= 8)
-        const int r0 = tid * per;
-        double zmax = 0.0;
-        if (n_res > 0) zmax = (double)from_orderable(~(uint32_t)(key[0] >> 32)) / a.temperature;
-        double e[8];
-        double loc = 0.0;
-#pragma unroll
-        for (int u = 0; u < 8; ++u) {
-            e[u] = 0.0;
-            int r = r0 + u;
-            if (u < per && r < n_res) {
-                double z = (double)from_orderable(~(uint32_t)(key[r] >> 32)) / a.temperature;
-                e[u] = exp(z - zmax);
-            }
-            loc += e[u];
-        }
-        double total;
-        block_inclusive_scan(loc, wtot, &total);
+        // Eq. 7 in fp64 on the sorted keys: z = s_bar / T, m = z of rank 0, e = exp(z - m).
+        if (tid == 0) s_bcast[0] = key[0];
         __syncthreads();
-        // p~ = e / sum, then the prefix mass along the sorted order
-        double pl = 0.0;
+        zmax = (double)key_score(s_bcast[0]) / a.temperature;
+        double inc[8];
 #pragma unroll
-        for (int u = 0; u < 8; ++u) {
-            e[u] = (total > 0.0) ? e[u] / total : 0.0;
-            pl += e[u];
-        }
-        double dummy;
-        double incl = block_inclusive_scan(pl, wtot, &dummy);
-        double run = incl - pl;
-        int below = 0;
+        for (int r = 0; r < 8; ++r) {
+            const int rank = ebase + 32 * r;
+            double e = 0.0;
+            if (rank < n_res) e = exp((double)key_score(key[r]) / a.temperature - zmax);
 #pragma unroll
-        for (int u = 0; u < 8; ++u) {
-            int r = r0 + u;
-            if (u < per && r < n_res) {
-                run += e[u];
-                mass[r] = e[u];
-                if (run < a.p) ++below;              // ranks whose cumulative mass is still < p
+            for (int o = 1; o < 32; o <<= 1) {
+                const double t = __shfl_up_sync(0xffffffffu, e, o);
+                if (lane >= o) e += t;
             }
+            inc[r] = e;                                   // inclusive prefix inside the segment
+            if (lane == 31) s_seg[warp * 8 + r] = e;
         }
-        if (below) atomicAdd(&s_nstar, below);
+        __syncthreads();
+        if (warp == 0) {
+            // exclusive scan of the NSEG segment totals (rank order = segment order)
+            constexpr int PER = (NSEG + 31) / 32;
+            double v[PER], run = 0.0;
+#pragma unroll
+            for (int u = 0; u < PER; ++u) {
+                const int s = lane * PER + u;
+                v[u] = (s < NSEG) ? s_seg[s] : 0.0;
+                run += v[u];
+            }
+            double incl = run;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                const double t = __shfl_up_sync(0xffffffffu, incl, o);
+                if (lane >= o) incl += t;
+            }
+            double off = incl - run;
+#pragma unroll
+            for (int u = 0; u < PER; ++u) {
+                const int s = lane * PER + u;
+                if (s < NSEG) s_seg[s] = off;
+                off += v[u];
+            }
+            if (lane == 31) s_total = incl;
+        }
+        __syncthreads();
+        const double total = s_total;
+        inv_total = total > 0.0 ? 1.0 / total : 0.0;
+        int below = 0;                                    // ranks whose cumulative mass is still < p
+#pragma unroll
+        for (int r = 0; r < 8; ++r) {
+            const int rank = ebase + 32 * r;
+            const double cum = (s_seg[warp * 8 + r] + inc[r]) * inv_total;
+            if (rank < n_res && cum < a.p) ++below;
+        }
+        below = __reduce_add_sync(0xffffffffu, below);
+        if (lane == 0 && below) atomicAdd(&s_below, below);
         __syncthreads();
         int n_star;
         if (n_res == 0) n_star = 0;
         else if (a.p >= 1.0) n_star = n_res;
-        else n_star = min(n_res, s_nstar + 1);
+        else n_star = min(n_res, s_below + 1);
         n_take = n_star;
-        int target = min(a.kmin, n_b);
+        const int target = min(a.kmin, n_b);
         if (n_reserved + n_take < target) n_take = min(n_res, target - n_reserved);
-        if (a.probs) {
-            float* pr = a.probs + (int64_t)row * a.nb_stride;
-            for (int j = tid; j < n_b; j += SEL_THREADS)
-                if (!(j >= sink_end && j < rec_beg)) pr[j] = 0.f;
-            for (int r = tid; r < n_res; r += SEL_THREADS) pr[(uint32_t)key[r]] = (float)mass[r];
-        }
     }
-    for (int r = tid; r < n_take; r += SEL_THREADS) flag[(uint32_t)key[r]] = 1;
-    __syncthreads();
 
-    // ascending compaction of the selected block ids
-    const int per = (n + SEL_THREADS - 1) / SEL_THREADS;
-    const int j0 = tid * per;
-    int cnt = 0;
-    for (int u = 0; u < per; ++u) {
-        int j = j0 + u;
-        if (j < n_b && flag[j]) ++cnt;
+    // ---- the cut as a key value
+    if (n_take > 0) {
+#pragma unroll
+        for (int r = 0; r < 8; ++r)
+            if (ebase + 32 * r == n_take - 1) s_bcast[1] = key[r];
     }
-    int total_sel;
-    int incl = block_inclusive_scan_int(cnt, itot, &total_sel);
-    int pos = incl - cnt;
+    __syncthreads();
+    const uint32_t tau = n_take > 0 ? s_bcast[1] : 0u;
+
+    // ---- index order: A = reserved or strictly better than tau (certainly selected), Tt = tied with tau
+    int prefA[8], prefT[8];
+    uint32_t isA = 0, isT = 0;
+#pragma unroll
+    for (int r = 0; r < 8; ++r) {
+        const int j = ebase + 32 * r;
+        const bool resid = j >= sink_end && j < rec_beg;
+        const bool fa = (j < n_b && !resid) || (resid && n_take > 0 && okey[r] < tau);
+        const bool ft = resid && n_take > 0 && okey[r] == tau;
+        const uint32_t ba = __ballot_sync(0xffffffffu, fa), bt = __ballot_sync(0xffffffffu, ft);
+        const uint32_t lt = (1u << lane) - 1u;
+        prefA[r] = __popc(ba & lt);
+        prefT[r] = __popc(bt & lt);
+        isA |= (uint32_t)fa << r;
+        isT |= (uint32_t)ft << r;
+        if (lane == 0) { s_cnt[warp * 8 + r][0] = __popc(ba); s_cnt[warp * 8 + r][1] = __popc(bt); }
+    }
+    __syncthreads();
+    if (warp == 0) {
+        constexpr int PER = (NSEG + 31) / 32;
+        int va[PER], vt[PER], ra = 0, rt = 0;
+#pragma unroll
+        for (int u = 0; u < PER; ++u) {
+            const int s = lane * PER + u;
+            va[u] = (s < NSEG) ? s_cnt[s][0] : 0;
+            vt[u] = (s < NSEG) ? s_cnt[s][1] : 0;
+            ra += va[u]; rt += vt[u];
+        }
+        int ia = ra, it = rt;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const int ta = __shfl_up_sync(0xffffffffu, ia, o), tt = __shfl_up_sync(0xffffffffu, it, o);
+            if (lane >= o) { ia += ta; it += tt; }
+        }
+        int oa = ia - ra, ot = it - rt;
+#pragma unroll
+        for (int u = 0; u < PER; ++u) {
+            const int s = lane * PER + u;
+            if (s < NSEG) { s_cnt[s][0] = oa; s_cnt[s][1] = ot; }
+            oa += va[u]; ot += vt[u];
+        }
+        if (lane == 31) { s_tot[0] = ia; s_tot[1] = it; }
+    }
+    __syncthreads();
+    const int total_A = s_tot[0], total_T = s_tot[1];
+    const int need = n_take - (total_A - n_reserved);    // ties to take, lowest block index first
+    const int total_sel = total_A + min(total_T, max(need, 0));
     int32_t* out = a.indices + (int64_t)row * a.cap;
-    for (int u = 0; u < per; ++u) {
-        int j = j0 + u;
-        if (j < n_b && flag[j]) {
-            if (pos < a.cap) out[pos] = j;
-            ++pos;
+#pragma unroll
+    for (int r = 0; r < 8; ++r) {
+        const int j = ebase + 32 * r;
+        const int a_before = s_cnt[warp * 8 + r][0] + prefA[r];
+        const int t_before = s_cnt[warp * 8 + r][1] + prefT[r];
+        int pos = -1;
+        if ((isA >> r) & 1u) pos = a_before + min(t_before, need);
+        else if (((isT >> r) & 1u) && t_before < need) pos = a_before + t_before;
+        if (pos >= 0 && pos < a.cap) out[pos] = j;
+    }
+    for (int j = total_sel + tid; j < a.cap; j += T) out[j] = -1;
+    if (tid == 0) a.budgets[row] = min(total_sel, a.cap);
+
+    if (a.probs) {
+        float* pr = a.probs + (int64_t)row * a.nb_stride;
+#pragma unroll
+        for (int r = 0; r < 8; ++r) {
+            const int j = ebase + 32 * r;
+            if (j < n_b) {
+                float pv = 0.f;
+                if (a.mode != SPOT_MODE_TOPK && j >= sink_end && j < rec_beg)
+                    pv = (float)(exp((double)key_score(okey[r]) / a.temperature - zmax) * inv_total);
+                pr[j] = pv;
+            }
         }
     }
-    for (int j = total_sel + tid; j < a.cap; j += SEL_THREADS) out[j] = -1;
-    if (tid == 0) a.budgets[row] = min(total_sel, a.cap);
+}
+
+template <int LT>
+spot_status launch_select(const SelectArgs& a, int rows, cudaStream_t s) {
+    select_kernel<LT><<<(unsigned)rows, 1 << LT, 0, s>>>(a);
+    SPOT_LAUNCH_CHECK();
+    return SPOT_OK;
 }
 
 }  // namespace
@@ -230,23 +318,17 @@ __global__ void __launch_bounds__(SEL_THREADS) select_kernel(SelectArgs a, int n
 spot_status run_select(const spot_select_params* p, const float* scores, int nb_stride, int rows_per_seq,
                        int max_nb, cudaStream_t s) {
     if (max_nb > SEL_MAX_NB) return SPOT_ERR_UNSUPPORTED;
-    int n = 1;
-    while (n < max_nb) n <<= 1;
     SelectArgs a;
     a.scores = scores; a.nb_stride = nb_stride; a.seq_len = p->seq_len; a.n_q = rows_per_seq;
     a.q_start = p->q_start; a.q_block = p->q_block; a.blk = p->blk;
     a.mode = p->mode; a.top_k = p->top_k; a.p = p->p; a.temperature = p->temperature;
     a.sink = p->sink_blocks; a.rec = p->recency_blocks; a.kmin = p->kmin_blocks;
     a.indices = p->indices; a.cap = p->cap; a.budgets = p->budgets; a.probs = p->block_probs;
-    size_t smem = (size_t)n * 17;
-    static bool attr_set = false;
-    if (!attr_set) {
-        SPOT_CUDA_TRY(cudaFuncSetAttribute(select_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, SEL_MAX_NB * 17));
-        attr_set = true;
-    }
-    select_kernel<<<(unsigned)(p->B * rows_per_seq), SEL_THREADS, smem, s>>>(a, n);
-    SPOT_LAUNCH_CHECK();
-    return SPOT_OK;
+    const int rows = p->B * rows_per_seq;
+    if (max_nb <= 256) return launch_select<5>(a, rows, s);
+    if (max_nb <= 2048) return launch_select<8>(a, rows, s);
+    if (max_nb <= 4096) return launch_select<9>(a, rows, s);
+    return launch_select<10>(a, rows, s);
 }
 
 }  // namespace spot
