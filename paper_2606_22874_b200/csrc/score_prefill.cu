@@ -1,4 +1,320 @@
+// Step a1', prefill form -- one score per (64-query block, 64-key block) tile (reading R2):
+//   s_bar[i,j] = max_{q in i} max_{t in j, t <= q}  sum_h w_h[q] ReLU(q^I_h[q] . k^I_{h,t}).
+//
+// This IS a dense contraction (4 heads x [Tq x 64] x [64 x L_visible]), so it runs on the 5th-gen tensor cores:
+//   * work item = (128-query tile = two query blocks, chunk of up to CHUNK key blocks); items are dealt round-robin
+//     to one persistent CTA per SM;
+//   * warp 8 lane 0: TMA producer -- the query tile ([4 heads][128][64] BF16, 64 KiB, double-buffered) and a 3-stage
+//     ring of key blocks ([4][64][64], 32 KiB) land in 128-byte-swizzled shared memory through 4-D tensor maps;
+//   * warp 9 lane 0: issues tcgen05.mma (M = 128, N = 64, K = 16; 4 k-steps x 4 heads per key block) into one of two
+//     TMEM accumulator stages (4 heads x 64 fp32 columns = 256 columns each);
+//   * warps 0-7: epilogue.  Warp w reads TMEM lanes 32 (w & 3) .. +31 (one query per lane) and columns
+//     32 (w >> 2) .. +31 of every head with tcgen05.ld, forms sum_h w_h ReLU(d_h) in fp32 and keeps a running max; the
+//     tile maximum is a REDUX.MAX over an order-preserving integer key plus one shared-memory atomicMax per warp.
+// The epilogue, not the MMA, is the near-co-bound (9 lane-ops per (query, key) pair against 512 tensor flops), so
+// ReLU is split between the two fp32 pipes: heads 0-1 use (w/2)(d + |d|) (FADD with an abs modifier, FMA pipe), heads
+// 2-3 use w max(d, 0) (ALU pipe); both forms give bit-identical products.  The weighted sum uses packed FFMA2.
 #include "common.cuh"
+#include "tc100.cuh"
+
 namespace spot {
-spot_status score_prefill(const spot_select_params*, float*, int, cudaStream_t) { return SPOT_ERR_UNSUPPORTED; }
+
+namespace {
+
+constexpr int PF_H = 4;                 // selector heads
+constexpr int PF_D = 64;                // d_idx (one 128-byte swizzle row)
+constexpr int PF_M = 128;               // queries per tile (two 64-query blocks)
+constexpr int PF_N = 64;                // keys per block
+constexpr int PF_CHUNK = 32;            // key blocks per work item
+constexpr int PF_KSTAGES = 3;
+constexpr int PF_EPI_WARPS = 8;
+constexpr int PF_THREADS = (PF_EPI_WARPS + 2) * 32;
+constexpr uint32_t Q_TILE_BYTES = PF_H * PF_M * PF_D * 2;   // 65536
+constexpr uint32_t K_TILE_BYTES = PF_H * PF_N * PF_D * 2;   // 32768
+constexpr uint32_t PF_SMEM_TILES = 2 * Q_TILE_BYTES + PF_KSTAGES * K_TILE_BYTES;
+constexpr uint32_t PF_SMEM_MISC = 1024;
+constexpr uint32_t PF_SMEM_BYTES = 1024 + PF_SMEM_TILES + PF_SMEM_MISC;   // 1024: manual alignment slack
+
+struct PrefillScoreArgs {
+    const float* w;           // [B][Tq][4]
+    float* scores;            // [B * n_qb][nb_stride]
+    int nb_stride;
+    int B, Tq, n_qb, n_qt;    // query blocks / query tiles per sequence
+    int qb_start;             // q_start / 64
+    int n_chunks_max;
+    int total_ids;
+};
+
+__device__ __forceinline__ uint32_t f32_order_key(float x) {
+    const uint32_t u = __float_as_uint(x);
+    return (u & 0x80000000u) ? ~u : (u | 0x80000000u);
 }
+__device__ __forceinline__ float f32_from_order_key(uint32_t k) {
+    return __uint_as_float((k & 0x80000000u) ? (k & 0x7fffffffu) : ~k);
+}
+
+// id -> (b, chunk c, tile m); false when the chunk lies beyond the tile's causal range
+__device__ __forceinline__ bool decode_item(const PrefillScoreArgs& a, int id, int& b, int& c, int& m, int& nk) {
+    const int per_b = a.n_chunks_max * a.n_qt;
+    b = id / per_b;
+    const int rem = id - b * per_b;
+    c = rem / a.n_qt;
+    m = rem - c * a.n_qt;
+    const int last_qb = min(2 * m + 1, a.n_qb - 1);        // last existing query block of the tile
+    const int n_vis = a.qb_start + last_qb + 1;            // key blocks the tile can see
+    nk = min(PF_CHUNK, n_vis - c * PF_CHUNK);
+    return nk > 0;
+}
+
+__global__ void __launch_bounds__(PF_THREADS, 1) score_prefill_kernel(const __grid_constant__ CUtensorMap tm_q,
+                                                                      const __grid_constant__ CUtensorMap tm_k,
+                                                                      const PrefillScoreArgs a) {
+    extern __shared__ unsigned char smem_raw[];
+    const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
+    unsigned char* smem = smem_raw + (smem_base - smem_u32(smem_raw));
+    const uint32_t q_smem = smem_base;                               // 2 x 64 KiB
+    const uint32_t k_smem = smem_base + 2 * Q_TILE_BYTES;            // 3 x 32 KiB
+    unsigned char* misc = smem + PF_SMEM_TILES;
+    const uint32_t misc_u32 = smem_base + PF_SMEM_TILES;
+    // barriers (8 bytes each)
+    const uint32_t bar_q_full = misc_u32 + 0;      // [2]
+    const uint32_t bar_q_empty = misc_u32 + 16;    // [2]
+    const uint32_t bar_k_full = misc_u32 + 32;     // [3]
+    const uint32_t bar_k_empty = misc_u32 + 56;    // [3]
+    const uint32_t bar_t_full = misc_u32 + 80;     // [2]
+    const uint32_t bar_t_empty = misc_u32 + 96;    // [2]
+    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(misc + 112);
+    uint32_t* s_max = reinterpret_cast<uint32_t*>(misc + 128);       // [2 item buffers][CHUNK][2 query blocks]
+
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+
+    if (threadIdx.x == 0) {
+        for (int i = 0; i < 2; ++i) {
+            mbar_init(bar_q_full + 8 * i, 1);
+            mbar_init(bar_q_empty + 8 * i, 1);
+            mbar_init(bar_t_full + 8 * i, 1);
+            mbar_init(bar_t_empty + 8 * i, PF_EPI_WARPS);
+        }
+        for (int i = 0; i < PF_KSTAGES; ++i) {
+            mbar_init(bar_k_full + 8 * i, 1);
+            mbar_init(bar_k_empty + 8 * i, 1);
+        }
+        mbar_fence_init();
+    }
+    if (threadIdx.x < 2 * PF_CHUNK * 2) s_max[threadIdx.x] = 0u;
+    if (warp == 0) tmem_alloc(misc_u32 + 112, 512);
+    if (warp == PF_EPI_WARPS && lane == 0) {
+        tma_prefetch_desc(&tm_q);
+        tma_prefetch_desc(&tm_k);
+    }
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+    const uint32_t tbase = *tmem_slot;
+
+    if (warp == PF_EPI_WARPS) {
+        // ================================ TMA producer ================================
+        if (lane == 0) {
+            int n_item = 0, kt = 0;
+            for (int id = blockIdx.x; id < a.total_ids; id += gridDim.x) {
+                int b, c, m, nk;
+                if (!decode_item(a, id, b, c, m, nk)) continue;
+                const int qb = n_item & 1;
+                mbar_wait(bar_q_empty + 8 * qb, ((n_item >> 1) & 1) ^ 1);
+                mbar_arrive_expect_tx(bar_q_full + 8 * qb, Q_TILE_BYTES);
+                tma_load_4d(q_smem + qb * Q_TILE_BYTES, &tm_q, bar_q_full + 8 * qb, 0, m * PF_M, 0, b);
+                for (int kb = 0; kb < nk; ++kb, ++kt) {
+                    const int s = kt % PF_KSTAGES;
+                    mbar_wait(bar_k_empty + 8 * s, ((kt / PF_KSTAGES) & 1) ^ 1);
+                    mbar_arrive_expect_tx(bar_k_full + 8 * s, K_TILE_BYTES);
+                    tma_load_4d(k_smem + s * K_TILE_BYTES, &tm_k, bar_k_full + 8 * s, 0, (c * PF_CHUNK + kb) * PF_N, 0, b);
+                }
+                ++n_item;
+            }
+        }
+    } else if (warp == PF_EPI_WARPS + 1) {
+        // ================================ MMA issuer ================================
+        if (lane == 0) {
+            constexpr uint32_t idesc = umma_idesc_bf16(PF_M, PF_N);
+            int n_item = 0, kt = 0;
+            for (int id = blockIdx.x; id < a.total_ids; id += gridDim.x) {
+                int b, c, m, nk;
+                if (!decode_item(a, id, b, c, m, nk)) continue;
+                const int qb = n_item & 1;
+                mbar_wait(bar_q_full + 8 * qb, (n_item >> 1) & 1);
+                const uint32_t qa = q_smem + qb * Q_TILE_BYTES;
+                for (int kb = 0; kb < nk; ++kb, ++kt) {
+                    const int s = kt % PF_KSTAGES, as = kt & 1;
+                    mbar_wait(bar_k_full + 8 * s, (kt / PF_KSTAGES) & 1);
+                    mbar_wait(bar_t_empty + 8 * as, ((kt >> 1) & 1) ^ 1);
+                    tc_fence_after();
+                    const uint32_t ka = k_smem + s * K_TILE_BYTES;
+#pragma unroll
+                    for (int h = 0; h < PF_H; ++h) {
+#pragma unroll
+                        for (int kk = 0; kk < PF_D / 16; ++kk) {
+                            const uint64_t ad = umma_desc_sw128(qa + h * (PF_M * PF_D * 2) + kk * 32);
+                            const uint64_t bd = umma_desc_sw128(ka + h * (PF_N * PF_D * 2) + kk * 32);
+                            umma_bf16_ss(tbase + as * 256 + h * PF_N, ad, bd, idesc, kk > 0);
+                        }
+                    }
+                    umma_commit(bar_k_empty + 8 * s);      // smem slot free once these MMAs have read it
+                    umma_commit(bar_t_full + 8 * as);      // accumulators ready for the epilogue
+                }
+                umma_commit(bar_q_empty + 8 * qb);
+                ++n_item;
+            }
+        }
+    } else {
+        // ================================ epilogue (warps 0-7) ================================
+        const int lq = warp & 3, ch = warp >> 2;
+        const int row = lq * 32 + lane;           // query row of the tile = TMEM lane
+        const int qbl = lq >> 1;                  // which of the tile's two query blocks
+        const uint32_t t_lane = tbase + ((uint32_t)(lq * 32) << 16) + ch * 32;
+        int n_item = 0, kt = 0;
+        for (int id = blockIdx.x; id < a.total_ids; id += gridDim.x) {
+            int b, c, m, nk;
+            if (!decode_item(a, id, b, c, m, nk)) continue;
+            const int ib = n_item & 1;
+            const int q_local = m * PF_M + row;                 // query index inside the chunk of Tq queries
+            const bool q_exists = q_local < a.Tq;
+            float4 wv = make_float4(0.f, 0.f, 0.f, 0.f);
+            if (q_exists) wv = *reinterpret_cast<const float4*>(a.w + ((int64_t)b * a.Tq + q_local) * PF_H);
+            const float wh0 = 0.5f * wv.x, wh1 = 0.5f * wv.y;   // heads 0-1: (w/2)(d + |d|)
+            const int qb_abs = a.qb_start + 2 * m + qbl;        // this row's (absolute) query block = its diagonal
+            const int q_in_blk = row & 63;
+            for (int kb = 0; kb < nk; ++kb, ++kt) {
+                const int as = kt & 1;
+                const int j = c * PF_CHUNK + kb;
+                mbar_wait(bar_t_full + 8 * as, (kt >> 1) & 1);
+                tc_fence_after();
+                const uint32_t ta = t_lane + as * 256;
+                float mx = -INFINITY;
+                const bool diag = (j == qb_abs);
+#pragma unroll
+                for (int half = 0; half < 2; ++half) {
+                    float d0[16], d1[16], d2[16], d3[16];
+                    tmem_ld16(ta + 0 * PF_N + half * 16, d0);
+                    tmem_ld16(ta + 1 * PF_N + half * 16, d1);
+                    tmem_ld16(ta + 2 * PF_N + half * 16, d2);
+                    tmem_ld16(ta + 3 * PF_N + half * 16, d3);
+                    tmem_ld_wait();
+                    if (half == 1) {
+                        tc_fence_before();
+                        __syncwarp();
+                        if (lane == 0) mbar_arrive(bar_t_empty + 8 * as);
+                    }
+                    float sv[16];
+#pragma unroll
+                    for (int i = 0; i < 16; i += 2) {
+                        float s0 = wh0 * (d0[i] + fabsf(d0[i]));
+                        float s1 = wh0 * (d0[i + 1] + fabsf(d0[i + 1]));
+                        ffma2(s0, s1, d1[i] + fabsf(d1[i]), d1[i + 1] + fabsf(d1[i + 1]), wh1, s0, s1);
+                        ffma2(s0, s1, fmaxf(d2[i], 0.f), fmaxf(d2[i + 1], 0.f), wv.z, s0, s1);
+                        ffma2(s0, s1, fmaxf(d3[i], 0.f), fmaxf(d3[i + 1], 0.f), wv.w, s0, s1);
+                        sv[i] = s0; sv[i + 1] = s1;
+                    }
+                    if (diag) {
+                        // causal mask inside the diagonal tile: key t of the block is visible iff t <= q
+#pragma unroll
+                        for (int i = 0; i < 16; ++i)
+                            if (ch * 32 + half * 16 + i > q_in_blk) sv[i] = -INFINITY;
+                    }
+#pragma unroll
+                    for (int i = 0; i < 16; i += 2) mx = fmax3(mx, sv[i], sv[i + 1]);
+                }
+                if (j <= qb_abs && q_exists) {        // warp-uniform: Tq is a multiple of 64, a warp's rows share a block
+                    const uint32_t key = __reduce_max_sync(0xffffffffu, f32_order_key(mx));
+                    if (lane == 0) atomicMax(&s_max[(ib * PF_CHUNK + kb) * 2 + qbl], key);
+                }
+            }
+            // item done: all epilogue warps meet, then the tile maxima go out and the buffer is re-armed
+            asm volatile("bar.sync 1, %0;" :: "n"(PF_EPI_WARPS * 32) : "memory");
+            for (int e = threadIdx.x; e < nk * 2; e += PF_EPI_WARPS * 32) {
+                const int kb = e >> 1, qq = e & 1;
+                const int qblk = 2 * m + qq;
+                const int j = c * PF_CHUNK + kb;
+                const uint32_t key = s_max[(ib * PF_CHUNK + kb) * 2 + qq];
+                s_max[(ib * PF_CHUNK + kb) * 2 + qq] = 0u;
+                if (qblk < a.n_qb && j <= a.qb_start + qblk)
+                    a.scores[((int64_t)b * a.n_qb + qblk) * a.nb_stride + j] = f32_from_order_key(key);
+            }
+            ++n_item;
+        }
+    }
+
+    tc_fence_before();
+    __syncthreads();
+    if (warp == 0) tmem_dealloc(tbase, 512);
+}
+
+}  // namespace
+
+// ---- host ---------------------------------------------------------------------------------------------------
+bool encode_tmap_bf16_sw128(CUtensorMap* out, const void* base, int rank, const uint64_t* dims,
+                            const uint64_t* strides_bytes, const uint32_t* box) {
+    typedef CUresult (*EncodeFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                 const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                 CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+    static EncodeFn fn = nullptr;
+    if (!fn) {
+        void* p = nullptr;
+        cudaDriverEntryPointQueryResult qres;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &qres) != cudaSuccess || !p ||
+            qres != cudaDriverEntryPointSuccess) {
+            cudaGetLastError();
+            return false;
+        }
+        fn = reinterpret_cast<EncodeFn>(p);
+    }
+    cuuint64_t gdim[5], gstr[4];
+    cuuint32_t bx[5], es[5];
+    for (int i = 0; i < rank; ++i) { gdim[i] = dims[i]; bx[i] = box[i]; es[i] = 1; }
+    for (int i = 0; i + 1 < rank; ++i) gstr[i] = strides_bytes[i];
+    CUresult r = fn(out, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, (cuuint32_t)rank, const_cast<void*>(base), gdim, gstr, bx, es,
+                    CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                    CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    return r == CUDA_SUCCESS;
+}
+
+// scores: fp32 [B * Tq/64][nb_stride]; entry (row, j) is written for every key block j the row's query block can see
+spot_status score_prefill(const spot_select_params* p, float* scores, int nb_stride, cudaStream_t s) {
+    if (p->fmt != SPOT_SELK_BF16) return SPOT_ERR_UNSUPPORTED;      // 4-bit prefill scoring: SURVEY 8(f) f2
+    if (p->H_idx != PF_H || p->d_idx != PF_D) return SPOT_ERR_UNSUPPORTED;
+    PrefillScoreArgs a;
+    a.w = p->w; a.scores = scores; a.nb_stride = nb_stride;
+    a.B = p->B; a.Tq = p->Tq; a.n_qb = p->Tq / 64; a.n_qt = (a.n_qb + 1) / 2;
+    a.qb_start = p->q_start / 64;
+    const int n_vis_max = a.qb_start + a.n_qb;
+    a.n_chunks_max = (n_vis_max + PF_CHUNK - 1) / PF_CHUNK;
+    const int64_t total = (int64_t)a.B * a.n_chunks_max * a.n_qt;
+    if (total > 0x7fffffff) return SPOT_ERR_UNSUPPORTED;
+    a.total_ids = (int)total;
+
+    CUtensorMap tm_q, tm_k;
+    const uint64_t row_bytes = (uint64_t)PF_H * PF_D * 2;
+    {
+        const uint64_t dims[4] = {(uint64_t)PF_D, (uint64_t)p->Tq, (uint64_t)PF_H, (uint64_t)p->B};
+        const uint64_t strides[3] = {row_bytes, (uint64_t)PF_D * 2, (uint64_t)p->Tq * row_bytes};
+        const uint32_t box[4] = {(uint32_t)PF_D, (uint32_t)PF_M, (uint32_t)PF_H, 1u};
+        if (!encode_tmap_bf16_sw128(&tm_q, p->sel_q, 4, dims, strides, box)) return SPOT_ERR_CUDA;
+    }
+    {
+        const uint64_t dims[4] = {(uint64_t)PF_D, (uint64_t)p->cache_stride_tokens, (uint64_t)PF_H, (uint64_t)p->B};
+        const uint64_t strides[3] = {row_bytes, (uint64_t)PF_D * 2, (uint64_t)p->cache_stride_tokens * row_bytes};
+        const uint32_t box[4] = {(uint32_t)PF_D, (uint32_t)PF_N, (uint32_t)PF_H, 1u};
+        if (!encode_tmap_bf16_sw128(&tm_k, p->sel_k, 4, dims, strides, box)) return SPOT_ERR_CUDA;
+    }
+    static bool attr_set = false;
+    if (!attr_set) {
+        SPOT_CUDA_TRY(cudaFuncSetAttribute(score_prefill_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                           (int)PF_SMEM_BYTES));
+        attr_set = true;
+    }
+    const int grid = (int)(total < sm_count() ? total : sm_count());
+    score_prefill_kernel<<<grid, PF_THREADS, PF_SMEM_BYTES, s>>>(tm_q, tm_k, a);
+    SPOT_LAUNCH_CHECK();
+    return SPOT_OK;
+}
+
+}  // namespace spot

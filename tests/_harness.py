@@ -143,3 +143,86 @@ def classify_selection(s_bar, sel, gpu_idx, gpu_budget, p=None, rel=1e-6):
         if margin < rel and all(abs(rank_pos.get(b, -99) - (n - 1)) <= 1 for b in diff):
             return "mass-near-cut"
     return "FAIL: sets differ %s (budget %d vs %d)" % (sorted(diff)[:8], gpu_budget, sel.budget)
+
+
+# ------------------------------------------------------------------------------------------------------
+# prefill form
+# ------------------------------------------------------------------------------------------------------
+
+class DevicePrefill:
+    """One or more PrefillWorkloads (same shapes, one per batch entry) resident on the GPU; the chunk of queries
+    [q_start, q_start + Tq) is scored against the BF16 selector K-cache of capacity L."""
+
+    def __init__(self, wls, q_start, Tq, with_kv=True):
+        import torch
+        from paper_2606_22874_b200 import api
+        self.api, self.wls, self.q_start, self.Tq = api, wls, q_start, Tq
+        wl = wls[0]
+        self.wl, self.B, self.L = wl, len(wls), wl.L
+        self.sel_q = dev_u16(np.stack([x.sel_q[q_start:q_start + Tq] for x in wls]))
+        self.w = torch.from_numpy(np.stack([x.w[q_start:q_start + Tq] for x in wls])).cuda()
+        self.sel_k = dev_u16(np.stack([x.sel_k for x in wls]))
+        self.n_q = Tq // wl.q_block
+        self.n_b_max = (q_start + Tq - 1) // wl.blk + 1
+        if with_kv and wl.K is not None:
+            self.Q = dev_u16(np.stack([x.Q[q_start:q_start + Tq] for x in wls]))     # [B][Tq][H_q][D]
+            self.K = dev_u16(np.stack([x.K for x in wls]))                           # [B][H_kv][L][D]
+            self.V = dev_u16(np.stack([x.V for x in wls]))
+            self.kv_strides = (wl.H_kv * wl.L * wl.D, wl.D, wl.L * wl.D)
+
+    def select(self, cap=None, want_scores=True, want_probs=True, **over):
+        import torch
+        wl, api = self.wl, self.api
+        kw = dict(mode=wl.mode, top_k=wl.top_k, p=wl.p, sink_blocks=wl.sink_blocks,
+                  recency_blocks=wl.recency_blocks, kmin_blocks=wl.kmin_blocks, temperature=wl.temperature)
+        kw.update(over)
+        cap = self.n_b_max if cap is None else cap
+        rows = self.B * self.n_q
+        indices = torch.full((rows, cap), -7, dtype=torch.int32, device="cuda")
+        budgets = torch.full((rows,), -7, dtype=torch.int32, device="cuda")
+        nb_stride = (self.n_b_max + 3) & ~3
+        scores = torch.full((rows, nb_stride), float("nan"), device="cuda") if want_scores else None
+        probs = torch.full((rows, nb_stride), float("nan"), device="cuda") if want_probs else None
+        sp = api.make_select_params(self.sel_q, self.w, self.sel_k, "bf16", self.L, None, 0, self.B, self.Tq,
+                                    wl.H_idx, wl.d_idx, q_start=self.q_start, blk=wl.blk, q_block=wl.q_block,
+                                    indices=indices, cap=cap, budgets=budgets, block_scores=scores,
+                                    block_probs=probs, nb_stride=nb_stride, **kw)
+        ws = torch.empty(max(api.spot_select_workspace_bytes(sp), 16), dtype=torch.uint8, device="cuda")
+        sp.workspace, sp.workspace_bytes = ws.data_ptr(), ws.numel()
+        api.spot_select(sp)
+        torch.cuda.synchronize()
+        return (indices.cpu().numpy(), budgets.cpu().numpy(),
+                None if scores is None else scores.cpu().numpy(), None if probs is None else probs.cpu().numpy())
+
+    def attend(self, indices_np, budgets_np, want_lse=False):
+        import torch
+        wl, api = self.wl, self.api
+        out = torch.zeros((self.B, self.Tq, wl.H_q, wl.D), dtype=torch.int16, device="cuda")
+        lse = torch.zeros((self.B, self.Tq, wl.H_q), device="cuda") if want_lse else None
+        idx = torch.from_numpy(np.ascontiguousarray(indices_np, dtype=np.int32)).cuda()
+        bud = torch.from_numpy(np.ascontiguousarray(budgets_np, dtype=np.int32)).cuda()
+        ap = api.make_attn_params(self.Q, self.K, self.V, self.kv_strides, None, 0, idx, bud, idx.shape[1], self.B,
+                                  self.Tq, wl.H_q, wl.H_kv, wl.D, q_start=self.q_start, blk=wl.blk,
+                                  sm_scale=wl.sm_scale, out=out, lse=lse)
+        ws = torch.empty(max(api.spot_sparse_attn_prefill_workspace_bytes(ap), 16), dtype=torch.uint8, device="cuda")
+        ap.workspace, ap.workspace_bytes = ws.data_ptr(), ws.numel()
+        api.spot_sparse_attn_prefill(ap)
+        torch.cuda.synchronize()
+        return bf16_bits_to_f64(to_np_u16(out)), (None if lse is None else lse.cpu().numpy())
+
+
+def oracle_select_prefill(wl, q_start, Tq, **over):
+    """-> list over query blocks of (s_bar_i, Selection_i) for the chunk [q_start, q_start + Tq)."""
+    kw = wl.select_kwargs()
+    kw.update(over)
+    mode = kw.pop("mode", wl.mode)
+    return OS.select_prefill(bf16_bits_to_f64(wl.sel_q[q_start:q_start + Tq]),
+                             wl.w[q_start:q_start + Tq].astype(np.float64), bf16_bits_to_f64(wl.sel_k),
+                             q_start, wl.q_block, wl.blk, mode, **kw)
+
+
+def oracle_attend_prefill(wl, q_start, Tq, block_lists):
+    K = bf16_bits_to_f64(wl.K).transpose(1, 0, 2)
+    V = bf16_bits_to_f64(wl.V).transpose(1, 0, 2)
+    return OA.sparse_attn_prefill(bf16_bits_to_f64(wl.Q[q_start:q_start + Tq]), K, V, block_lists, q_start,
+                                  wl.q_block, wl.blk, wl.sm_scale)
