@@ -220,32 +220,40 @@ def run_ours(args):
         step()
     barrier()
 
-    ev = [[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(args.steps)]
+    # the step: both calls back to back, one event pair around them (the four kernels chain through programmatic
+    # dependent launch, which an event between the calls would break)
+    ev = [[torch.cuda.Event(enable_timing=True) for _ in range(2)] for _ in range(args.steps)]
     with ClockSampler(local_rank) as clk:
         for i in range(args.steps):
             flush_l2()
             ev[i][0].record(stream)
             api.spot_select(sp, stream)
-            ev[i][1].record(stream)
             api.spot_sparse_attn_decode(ap, stream)
-            ev[i][2].record(stream)
+            ev[i][1].record(stream)
         barrier()
-    sel_ms = np.array([e[0].elapsed_time(e[1]) for e in ev])
-    att_ms = np.array([e[1].elapsed_time(e[2]) for e in ev])
-    step_ms = np.array([e[0].elapsed_time(e[2]) for e in ev])
+    step_ms = np.array([e[0].elapsed_time(e[1]) for e in ev])
     clocks = clk.summary()
 
+    def time_alone(fn, n):
+        ts = []
+        for i in range(n + 2):
+            flush_l2()
+            a_, b_ = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a_.record(stream)
+            fn()
+            b_.record(stream)
+            torch.cuda.synchronize()
+            if i >= 2:
+                ts.append(a_.elapsed_time(b_))
+        return np.array(ts)
+
+    # the two calls timed alone (breakdown, and the live duration of the dominant kernel for the roofline object)
+    n_alone = max(3, min(args.steps, 20))
+    sel_ms = time_alone(lambda: api.spot_select(sp, stream), n_alone)
+    att_ms = time_alone(lambda: api.spot_sparse_attn_decode(ap, stream), n_alone)
+
     # dense comparator (same shapes, every block)
-    den = []
-    for i in range(max(3, min(args.steps, 10)) + 2):
-        flush_l2()
-        a, b_ = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        a.record(stream)
-        api.spot_dense_attn_decode(apd, stream)
-        b_.record(stream)
-        torch.cuda.synchronize()
-        if i >= 2:
-            den.append(a.elapsed_time(b_))
+    den = time_alone(lambda: api.spot_dense_attn_decode(apd, stream), max(3, min(args.steps, 10)))
 
     # e2e: host buffers through spot_decode_step_host (H2D of the step's q / q^I / w, D2H of out + budgets)
     hp = api.DecodeStepHostParams()
@@ -323,10 +331,255 @@ def run_ours(args):
                          "sample": "sequence 0 of %d (select + attend, budget %d blocks), time x B" % (Bn, cpu_budget)},
         "e2e": {"value": float(np.mean(e2e)) * 1e3, "unit": "us/layer-step", "h2d_bytes_per_step": h2d,
                 "d2h_bytes_per_step": d2h},
-        "gpu_launches": 4 * args.steps,
+        "gpu_launches": 4 * args.steps,          # score, select, attn, merge per step (timed loop only)
         "clocks": clocks,
         "paper_context": "paper: 3.9x FlashAttention / 1.8x Twilight end-to-end at L=128K, Qwen3-8B, one B200, Triton "
                          "kernels (PAPER.md:146); other shapes, context only",
+    }
+    print(json.dumps(line))
+
+
+# ------------------------------------------------------------------------------------------------------
+# chunked prefill (BASELINE.json config 5): a1' tile scoring on tcgen05 -> a2 per query block -> a3' sparse attention
+# ------------------------------------------------------------------------------------------------------
+PF_METRIC = "prefill ms/layer (selector GEMM + dual top-p + block-sparse causal attn) @L=64K; % of tensor-pipe peak"
+
+
+def tensor_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as f:
+            d = json.load(f)
+        return float(d["bf16_tflops"]), float(d.get("bf16_tflops_sustained", d["bf16_tflops"])), \
+            "measured (MEASURED_PEAKS.json bf16_tflops, burst: the kernel is timed alone)"
+    return 1700.0, 1700.0, "fallback (B200_PROFILING.md)"
+
+
+def oracle_prefill_sample(wl, K, V, Q, blocks, p):
+    """The oracle's prefill layer pass on a few query blocks (scoring, selection, attention).  K/V/Q: BF16 bits on the
+    host.  Returns (seconds, scored tiles, attended (query block, key block) pairs)."""
+    from oracle import attention as OA
+    from oracle import selection as OS
+    from oracle.bf16 import bf16_bits_to_f64
+    t0 = time.perf_counter()
+    tiles = pairs = 0
+    kw = wl.select_kwargs()
+    kw["p"] = p
+    for i in blocks:
+        q0 = i * 64
+        n_tok = q0 + 64
+        res = OS.select_prefill(bf16_bits_to_f64(wl.sel_q[q0:q0 + 64]), wl.w[q0:q0 + 64].astype(np.float64),
+                                bf16_bits_to_f64(wl.sel_k[:n_tok]), q0, wl.q_block, wl.blk, wl.mode, **kw)
+        s_bar, sel = res[0]
+        OA.sparse_attn_prefill(bf16_bits_to_f64(Q[q0:q0 + 64]), bf16_bits_to_f64(K[:, :n_tok]).transpose(1, 0, 2),
+                               bf16_bits_to_f64(V[:, :n_tok]).transpose(1, 0, 2), [sel.indices.tolist()], q0,
+                               wl.q_block, wl.blk, wl.sm_scale)
+        tiles += i + 1
+        pairs += sel.budget
+    return time.perf_counter() - t0, tiles, pairs
+
+
+def run_prefill(args):
+    import torch
+    from workloads import make_prefill_workload, f32_to_bf16_bits
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    L = args.L or 65536
+    wl = make_prefill_workload(seed=5005 + 1000 * rank, L=L, with_kv=False)
+    wl.p = args.p
+    n_qb = L // 64
+    Hq, Hkv, D = wl.H_q, wl.H_kv, wl.D
+
+    if args.impl == "reference":
+        if rank != 0:
+            return
+        rng = np.random.Generator(np.random.Philox(wl.seed + 17))
+        n_tok = min(L, 4096)                       # the sampled query blocks all sit below this position
+        Kh = f32_to_bf16_bits(rng.standard_normal((Hkv, n_tok, D), dtype=np.float32))
+        Vh = f32_to_bf16_bits(rng.standard_normal((Hkv, n_tok, D), dtype=np.float32))
+        Qh = f32_to_bf16_bits(rng.standard_normal((n_tok, Hq, D), dtype=np.float32))
+        blocks = [0, n_tok // 128, n_tok // 64 - 1]
+        ts = []
+        for i in range(args.warmup + args.steps):
+            dt, tiles, pairs = oracle_prefill_sample(wl, Kh, Vh, Qh, blocks, args.p)
+            if i >= args.warmup:
+                ts.append(dt)
+        full_tiles = n_qb * (n_qb + 1) // 2
+        ms = float(np.mean(ts)) / tiles * full_tiles * 1e3
+        cores = len(os.sched_getaffinity(0))
+        sample = ("query blocks %s of %d (score + select + attend; %d tiles, %d attended block pairs), time scaled "
+                  "linearly in scored tiles to the full lower triangle (%d tiles)" % (blocks, n_qb, tiles, pairs, full_tiles))
+        print(json.dumps({
+            "impl": "reference", "metric": PF_METRIC, "value": ms, "unit": "ms/layer", "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": False,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": "cfg5", "L": L, "p": args.p},
+            "cpu_baseline": {"value": ms, "unit": "ms/layer", "cores": cores, "kind": "oracle", "sample": sample},
+            "e2e": {"value": ms, "unit": "ms/layer", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}))
+        return
+
+    torch.cuda.set_device(local_rank)
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    from paper_2606_22874_b200 import _lib, api
+    from paper_2606_22874_b200 import build as B
+    B.build()
+    _lib.load()
+    dev = torch.device("cuda", local_rank)
+    gen = torch.Generator(device=dev)
+    gen.manual_seed(wl.seed + 17)
+    Q = torch.randn((1, L, Hq, D), generator=gen, device=dev, dtype=torch.bfloat16)
+    K = torch.randn((1, Hkv, L, D), generator=gen, device=dev, dtype=torch.bfloat16)
+    V = torch.randn((1, Hkv, L, D), generator=gen, device=dev, dtype=torch.bfloat16)
+    h_selq = torch.from_numpy(wl.sel_q.view(np.int16)).pin_memory()
+    h_w = torch.from_numpy(wl.w).pin_memory()
+    h_selk = torch.from_numpy(wl.sel_k.view(np.int16)).pin_memory()
+    sel_q, w, sel_k = h_selq.to(dev), h_w.to(dev), h_selk.to(dev)
+    cap = n_qb
+    nb_stride = (n_qb + 3) & ~3
+    indices = torch.empty((n_qb, cap), dtype=torch.int32, device=dev)
+    budgets = torch.empty((n_qb,), dtype=torch.int32, device=dev)
+    scores = torch.empty((n_qb, nb_stride), dtype=torch.float32, device=dev)
+    out = torch.empty((1, L, Hq, D), dtype=torch.int16, device=dev)
+    sp = api.make_select_params(sel_q, w, sel_k, "bf16", L, None, 0, 1, L, wl.H_idx, wl.d_idx, q_start=0, blk=64,
+                                q_block=64, mode=wl.mode, top_k=wl.top_k, p=args.p, sink_blocks=wl.sink_blocks,
+                                recency_blocks=wl.recency_blocks, kmin_blocks=wl.kmin_blocks,
+                                temperature=wl.temperature, indices=indices, cap=cap, budgets=budgets,
+                                block_scores=scores, nb_stride=nb_stride)
+    ws = torch.empty(max(16, api.spot_select_workspace_bytes(sp)), dtype=torch.uint8, device=dev)
+    sp.workspace, sp.workspace_bytes = ws.data_ptr(), ws.numel()
+    ap = api.make_attn_params(Q, K, V, (Hkv * L * D, D, L * D), None, 0, indices, budgets, cap, 1, L, Hq, Hkv, D,
+                              q_start=0, blk=64, sm_scale=wl.sm_scale, out=out)
+    stream = torch.cuda.current_stream()
+    flush = torch.empty(512 << 20, dtype=torch.uint8, device=dev).zero_()
+
+    def flush_l2():
+        flush.view(torch.int64).sum()
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            import torch.distributed as dist
+            dist.barrier()
+            torch.cuda.synchronize()
+
+    W = max(args.warmup, 3)
+    for _ in range(W):
+        flush_l2()
+        api.spot_select(sp, stream)
+        api.spot_sparse_attn_prefill(ap, stream)
+    barrier()
+    ev = [[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(args.steps)]
+    with ClockSampler(local_rank) as clk:
+        for i in range(args.steps):
+            flush_l2()
+            ev[i][0].record(stream)
+            api.spot_select(sp, stream)
+            ev[i][1].record(stream)
+            api.spot_sparse_attn_prefill(ap, stream)
+            ev[i][2].record(stream)
+        barrier()
+    sel_ms = np.array([e[0].elapsed_time(e[1]) for e in ev])
+    att_ms = np.array([e[1].elapsed_time(e[2]) for e in ev])
+    step_ms = np.array([e[0].elapsed_time(e[2]) for e in ev])
+    clocks = clk.summary()
+    # the selector GEMM kernel alone (spot_score_blocks = a1' only), live, for the roofline object
+    sc = []
+    for i in range(args.steps + 2):
+        flush_l2()
+        a_, b_ = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a_.record(stream)
+        api.spot_score_blocks(sp, stream)
+        b_.record(stream)
+        torch.cuda.synchronize()
+        if i >= 2:
+            sc.append(a_.elapsed_time(b_))
+    # dense causal comparator (indices NULL) -- a few iterations only
+    apd = api.make_attn_params(Q, K, V, (Hkv * L * D, D, L * D), None, 0, None, None, 0, 1, L, Hq, Hkv, D,
+                               q_start=0, blk=64, sm_scale=wl.sm_scale, out=out)
+    den = []
+    for i in range(3):
+        a_, b_ = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a_.record(stream)
+        api.spot_sparse_attn_prefill(apd, stream)
+        b_.record(stream)
+        torch.cuda.synchronize()
+        if i >= 1:
+            den.append(a_.elapsed_time(b_))
+    api.spot_select(sp, stream)
+    torch.cuda.synchronize()
+    bud_host = budgets.cpu().numpy().astype(np.int64)
+    # e2e: the selector-side inputs of the chunk cross PCIe inside the timed region, budgets come back
+    e2e = []
+    h_bud = torch.empty((n_qb,), dtype=torch.int32).pin_memory()
+    for i in range(min(args.steps, 5) + 1):
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        sel_q.copy_(h_selq, non_blocking=True)
+        w.copy_(h_w, non_blocking=True)
+        sel_k.copy_(h_selk, non_blocking=True)
+        api.spot_select(sp, stream)
+        api.spot_sparse_attn_prefill(ap, stream)
+        h_bud.copy_(budgets, non_blocking=True)
+        torch.cuda.synchronize()
+        if i >= 1:
+            e2e.append((time.perf_counter() - t0) * 1e3)
+
+    step_mean = float(step_ms.mean())
+    if world > 1:
+        import torch.distributed as dist
+        t = torch.tensor([step_mean], device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        step_mean = float(t.item())
+    if rank != 0:
+        return
+    burst, sustained, peak_src = tensor_peaks()
+    tiles = n_qb * (n_qb + 1) // 2
+    gemm_flop = 2.0 * 64 * 64 * wl.d_idx * wl.H_idx * tiles
+    att_flop = 4.0 * 64 * 64 * D * Hq * float(bud_host.sum())
+    score_s = float(np.mean(sc)) * 1e-3
+    achieved = gemm_flop / score_s / 1e12
+    traffic = None
+    tpath = os.path.join(ROOT, "profiles", "traffic.json")
+    if os.path.exists(tpath):
+        with open(tpath) as f:
+            traffic = json.load(f).get("cfg5/bf16/score_prefill_kernel")
+    # oracle on the host cores: three query blocks below position 4096
+    n_tok = min(L, 4096)
+    Kh = K[0, :, :n_tok].contiguous().view(torch.int16).cpu().numpy().view(np.uint16)
+    Vh = V[0, :, :n_tok].contiguous().view(torch.int16).cpu().numpy().view(np.uint16)
+    Qh = Q[0, :n_tok].contiguous().view(torch.int16).cpu().numpy().view(np.uint16)
+    blocks = [0, n_tok // 128, n_tok // 64 - 1]
+    cpu_t, cpu_tiles, cpu_pairs = oracle_prefill_sample(wl, Kh, Vh, Qh, blocks, args.p)
+    line = {
+        "metric": PF_METRIC, "value": step_mean, "unit": "ms/layer", "n_gpus": world, "steps": args.steps,
+        "warmup": W, "ms_per_step": step_mean, "higher_is_better": False, "scaling": "weak", "vs_baseline": None,
+        "dtype": "bf16", "data": "synthetic",
+        "config": {"workload": "cfg5", "B": 1, "L": L, "H_q": Hq, "H_kv": Hkv, "D": D,
+                   "selector": "%dx%d bf16" % (wl.H_idx, wl.d_idx), "blk": 64, "q_block": 64, "mode": wl.mode, "p": args.p,
+                   "sink/recency/kmin": [wl.sink_blocks, wl.recency_blocks, wl.kmin_blocks],
+                   "mean_budget": float(bud_host.mean()), "density": float(bud_host.sum()) / tiles,
+                   "l2": "flushed by a 512 MiB read sweep before every timed step"},
+        "tokens_per_s": world * L / (step_mean * 1e-3),
+        "breakdown_ms": {"select (tile-score GEMM + selection kernels)": float(sel_ms.mean()),
+                         "tile-score GEMM alone (spot_score_blocks)": float(np.mean(sc)),
+                         "sparse causal attention": float(att_ms.mean()),
+                         "dense causal attention (same kernel, every block)": float(np.mean(den))},
+        "attention_tflops": att_flop / (float(att_ms.mean()) * 1e-3) / 1e12,
+        "roofline": {"bound": "tensor", "kernel": "score_prefill_kernel", "achieved": achieved, "peak": burst,
+                     "unit": "TFLOP/s", "frac": achieved / burst, "frac_of_sustained": achieved / sustained,
+                     "traffic": traffic, "peak_source": peak_src, "algorithmic_flops": gemm_flop},
+        "cpu_baseline": {"value": cpu_t / cpu_tiles * tiles * 1e3, "unit": "ms/layer",
+                         "cores": len(os.sched_getaffinity(0)), "kind": "oracle",
+                         "sample": "query blocks %s of %d (score + select + attend; %d tiles, %d attended block pairs), "
+                                   "time scaled linearly in scored tiles to %d" % (blocks, n_qb, cpu_tiles, cpu_pairs, tiles)},
+        "e2e": {"value": float(np.mean(e2e)), "unit": "ms/layer",
+                "h2d_bytes_per_step": h_selq.numel() * 2 + h_w.numel() * 4 + h_selk.numel() * 2,
+                "d2h_bytes_per_step": h_bud.numel() * 4},
+        "gpu_launches": 3 * args.steps,
+        "clocks": clocks,
     }
     print(json.dumps(line))
 
@@ -340,8 +593,11 @@ def main():
     ap.add_argument("--workload", default="cfg3")
     ap.add_argument("--fmt", default="bf16", choices=["bf16", "mxfp4", "int4_e4m3"])
     ap.add_argument("--p", type=float, default=0.90)
+    ap.add_argument("--L", type=int, default=0, help="cfg5 only: prompt length (default 65536)")
     args = ap.parse_args()
-    if args.impl == "reference":
+    if args.workload == "cfg5":
+        run_prefill(args)
+    elif args.impl == "reference":
         run_reference(args)
     else:
         run_ours(args)

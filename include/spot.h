@@ -153,6 +153,12 @@ typedef struct {
 size_t spot_select_workspace_bytes(const spot_select_params* p);
 spot_status spot_select(const spot_select_params* p, void* stream);
 
+/* a1 / a1' alone -- the scoring half of spot_select: writes s_bar into block_scores (required,
+ * row stride nb_stride) and stops; the rule fields, indices, budgets, cap and the workspace are ignored.  Same
+ * argument checks and errors as spot_select otherwise.  Lets a caller (and bench.py) run and time the selector
+ * scoring kernel by itself. */
+spot_status spot_score_blocks(const spot_select_params* p, void* stream);
+
 /* ---------------------------------------------------------------------------------------------------
  * a3 / a3' -- block-sparse GQA attention over the selected KV blocks.
  *

@@ -65,6 +65,7 @@ PROTOTYPES = {
                                              C.c_int64, C.c_int, C.c_int, C.c_void_p]),
     "spot_select_workspace_bytes": (C.c_size_t, [C.POINTER(SelectParams)]),
     "spot_select": (C.c_int, [C.POINTER(SelectParams), C.c_void_p]),
+    "spot_score_blocks": (C.c_int, [C.POINTER(SelectParams), C.c_void_p]),
     "spot_sparse_attn_decode_workspace_bytes": (C.c_size_t, [C.POINTER(AttnParams)]),
     "spot_sparse_attn_decode": (C.c_int, [C.POINTER(AttnParams), C.c_void_p]),
     "spot_sparse_attn_prefill_workspace_bytes": (C.c_size_t, [C.POINTER(AttnParams)]),

@@ -96,6 +96,10 @@ def spot_select(sp, stream=None):
     _check(L.load().spot_select(C.byref(sp), _stream(stream)), "spot_select")
 
 
+def spot_score_blocks(sp, stream=None):
+    _check(L.load().spot_score_blocks(C.byref(sp), _stream(stream)), "spot_score_blocks")
+
+
 def make_attn_params(q, k, v, kv_strides, seq_len, max_seq_len, indices, budgets, cap, B, Tq, H_q, H_kv, D, *,
                      q_start=0, blk=64, sm_scale=None, out=None, lse=None, workspace=None):
     ap = AttnParams()

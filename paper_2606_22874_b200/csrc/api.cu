@@ -47,14 +47,15 @@ struct SelectGeom {
     bool own_scores;  // scores live in the workspace
 };
 
-spot_status select_geometry(const spot_select_params* p, SelectGeom* g) {
+spot_status select_geometry(const spot_select_params* p, SelectGeom* g, bool score_only = false) {
     if (!p) return SPOT_ERR_INVALID_ARG;
-    if (!p->sel_q || !p->w || !p->sel_k || !p->indices || !p->budgets) return SPOT_ERR_INVALID_ARG;
+    if (!p->sel_q || !p->w || !p->sel_k) return SPOT_ERR_INVALID_ARG;
+    if (score_only ? !p->block_scores : (!p->indices || !p->budgets)) return SPOT_ERR_INVALID_ARG;
     if (!aligned16(p->sel_q) || !aligned16(p->sel_k) || !aligned16(p->w)) return SPOT_ERR_INVALID_ARG;
     if (p->fmt != SPOT_SELK_BF16 && p->fmt != SPOT_SELK_INT4_E4M3 && p->fmt != SPOT_SELK_MXFP4) return SPOT_ERR_INVALID_ARG;
     if (p->mode != SPOT_MODE_TOPK && p->mode != SPOT_MODE_DUAL_TOPP) return SPOT_ERR_INVALID_ARG;
     if (p->B <= 0 || p->Tq <= 0 || p->H_idx <= 0 || p->d_idx <= 0 || p->d_idx % 32 != 0) return SPOT_ERR_INVALID_ARG;
-    if (p->blk <= 0 || p->cap <= 0 || p->cache_stride_tokens <= 0) return SPOT_ERR_INVALID_ARG;
+    if (p->blk <= 0 || (!score_only && p->cap <= 0) || p->cache_stride_tokens <= 0) return SPOT_ERR_INVALID_ARG;
     if (p->sink_blocks < 0 || p->recency_blocks < 0 || p->kmin_blocks < 0 || p->top_k < 0) return SPOT_ERR_INVALID_ARG;
     if (p->mode == SPOT_MODE_DUAL_TOPP && !(p->p > 0.0 && p->p <= 1.0)) return SPOT_ERR_INVALID_ARG;
     if (!(p->temperature > 0.0)) return SPOT_ERR_INVALID_ARG;
@@ -77,7 +78,7 @@ spot_status select_geometry(const spot_select_params* p, SelectGeom* g) {
     }
     g->max_nb = (int)ceil_div64(max_tokens, p->blk);
     int need_cap = p->mode == SPOT_MODE_DUAL_TOPP ? g->max_nb : (p->top_k < g->max_nb ? p->top_k : g->max_nb);
-    if (p->cap < need_cap) return SPOT_ERR_INVALID_ARG;
+    if (!score_only && p->cap < need_cap) return SPOT_ERR_INVALID_ARG;
     if (p->block_scores || p->block_probs) {
         if (p->nb_stride < g->max_nb) return SPOT_ERR_INVALID_ARG;
     }
@@ -138,6 +139,16 @@ extern "C" spot_status spot_select(const spot_select_params* p, void* stream) {
     else st = score_prefill(p, scores, g.nb_stride, s);
     if (st != SPOT_OK) return st;
     return run_select(p, scores, g.nb_stride, g.rows_per_seq, g.max_nb, s);
+}
+
+extern "C" spot_status spot_score_blocks(const spot_select_params* p, void* stream) {
+    SelectGeom g;
+    spot_status st = select_geometry(p, &g, true);
+    if (st != SPOT_OK) return st;
+    if ((st = check_device()) != SPOT_OK) return st;
+    cudaStream_t s = (cudaStream_t)stream;
+    return p->q_block == 1 ? score_decode(p, p->block_scores, g.nb_stride, s)
+                           : score_prefill(p, p->block_scores, g.nb_stride, s);
 }
 
 extern "C" spot_status spot_decode_step_host(const spot_decode_step_host_params* p, void* stream) {

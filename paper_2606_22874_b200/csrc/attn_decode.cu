@@ -1,14 +1,18 @@
 // Step a3 -- block-sparse GQA flash-decode over the selected 64-token KV blocks (PAPER.md:47 Fig. 2, :71), and the
 // dense comparator (every block) from the same code.
 //
-// HBM-bound: 32 KiB of K+V per (selected block, KV head), 4-8 flop/B.  Split-K over the index list: CTA
-// (chunk, kv head, sequence) owns up to `chunk_blocks` consecutive entries of the sequence's index list.  Inside the
-// CTA every warp runs its OWN cp.async ring over its 16-token quarter of each block (8 KiB of K+V per stage, zero
-// CTA-wide barriers in the main loop), feeds ldmatrix -> mma.sync m16n8k16 with the G = H_q/H_kv query heads of the
-// group as the (padded) M = 16 rows, and keeps a private online-softmax state.  The warps' states are merged through
-// shared memory at the end and written as an unnormalised partial (m, l, O); a second small kernel merges the
-// partials of all chunks (log-sum-exp) and writes BF16.  M is tiny here, so this is mma.sync territory, not tcgen05:
-// the tensor pipe needs < 15 % of the time the HBM stream takes.
+// HBM-bound: 32 KiB of K+V per (selected block, KV head), 4-8 flop/B.  The work is the flat list of units
+// (sequence, KV head, position in that sequence's index list), U = H_kv * sum_b budget_b of them, and it is cut
+// stream-K style into gridDim.x equal contiguous ranges, one per persistent CTA (2 CTAs per SM): every CTA streams the
+// same number of bytes whatever the budgets are (config 4's 8..512-block mix included) and the whole grid is one wave.
+// A CTA's range touches one segment (sequence, KV head) or a few; for each it keeps a private online-softmax state
+// and writes ONE unnormalised partial (m, l, O) -- <= gridDim.x + B*H_kv partials in total (slot = CTA + segment
+// index, unique because the (CTA, segment) pairs form a staircase), a few hundred KiB instead of one per 8 blocks.
+// Inside the CTA every warp runs its OWN cp.async ring over its 16-token quarter of each block (8 KiB of K+V per
+// stage, zero CTA-wide barriers in the main loop) and feeds ldmatrix -> mma.sync m16n8k16 with the G = H_q/H_kv query
+// heads of the group as the (padded) M = 16 rows.  M is tiny here, so this is mma.sync territory, not tcgen05: the
+// tensor pipe needs < 15 % of the time the HBM stream takes.  A second small kernel merges each (sequence, head)'s
+// partials (log-sum-exp) and writes BF16.
 #include "common.cuh"
 
 namespace spot {
@@ -31,14 +35,19 @@ struct AttnArgs {
     const int32_t* indices;      // nullptr: dense
     const int32_t* budgets;
     int cap;
-    int H_q, H_kv, G;
+    int B, H_q, H_kv, G;
     float scale_log2;            // sm_scale * log2(e)
-    int chunk_blocks, n_chunks;
-    float* part_o;               // [B][H_kv][n_chunks][G][128]
-    float* part_ml;              // [B][H_kv][n_chunks][G][2]
+    int n_ctas;                  // gridDim.x of attn_decode_kernel (the merge kernel recomputes the same cut)
+    float* part_o;               // [n_ctas + B*H_kv][G][128]
+    float* part_ml;              // [n_ctas + B*H_kv][G][2]
     uint16_t* out;
     float* lse;
 };
+
+// blocks of sequence b that are attended
+__device__ __forceinline__ int seq_blocks(const AttnArgs& a, int b) {
+    return a.indices ? max(0, min(a.budgets[b], a.cap)) : ((a.seq_len[b] + 63) >> 6);
+}
 
 // smem sub-tile: [16 rows][256 B], 16-byte chunk index XOR-swizzled with (row & 7)
 __device__ __forceinline__ uint32_t sw_off(int row, int chunk) { return (uint32_t)(row * 256 + ((chunk ^ (row & 7)) << 4)); }
@@ -60,230 +69,256 @@ __device__ __forceinline__ void issue_subtile(uint32_t smem_stage, const uint16_
 
 __global__ void __launch_bounds__(ATT_WARPS * 32, 2) attn_decode_kernel(AttnArgs a) {
     extern __shared__ __align__(128) unsigned char smem[];
-    const int chunk = blockIdx.x, hk = blockIdx.y, b = blockIdx.z;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int g = lane >> 2, c = lane & 3;
-    const int L = a.seq_len[b];
-    const int n_b = (L + 63) >> 6;
-    const int budget = a.indices ? min(a.budgets[b], a.cap) : n_b;
-    const int jbeg = chunk * a.chunk_blocks;
-    const int jend = min(jbeg + a.chunk_blocks, budget);
-    if (jbeg >= jend) return;
     const int G = a.G;
+    pdl_wait();
+    pdl_launch_dependents();
 
-    // Q fragments (A operand): rows = query heads of this KV group, zero-padded to 16.
-    uint32_t qa[8][4];
-    {
-        const uint16_t* qb = a.q + ((int64_t)b * a.H_q + (int64_t)hk * G) * ATT_D;
-#pragma unroll
-        for (int ks = 0; ks < 8; ++ks) {
-            int col = ks * 16 + c * 2;
-            qa[ks][0] = (g < G) ? *reinterpret_cast<const uint32_t*>(qb + g * ATT_D + col) : 0u;
-            qa[ks][1] = (g + 8 < G) ? *reinterpret_cast<const uint32_t*>(qb + (g + 8) * ATT_D + col) : 0u;
-            qa[ks][2] = (g < G) ? *reinterpret_cast<const uint32_t*>(qb + g * ATT_D + col + 8) : 0u;
-            qa[ks][3] = (g + 8 < G) ? *reinterpret_cast<const uint32_t*>(qb + (g + 8) * ATT_D + col + 8) : 0u;
-        }
-    }
-
-    const uint16_t* kbase = a.k + (int64_t)b * a.sb + (int64_t)hk * a.sh;
-    const uint16_t* vbase = a.v + (int64_t)b * a.sb + (int64_t)hk * a.sh;
-    const int32_t* idx = a.indices ? a.indices + (int64_t)b * a.cap : nullptr;
+    // this CTA's range of the flat unit list
+    long long U = 0;
+    for (int bb = 0; bb < a.B; ++bb) U += seq_blocks(a, bb);
+    U *= a.H_kv;
+    const long long u0 = (long long)blockIdx.x * U / gridDim.x, u1 = (long long)(blockIdx.x + 1) * U / gridDim.x;
+    if (u0 >= u1) return;
+    int b = 0, nb = seq_blocks(a, 0);
+    long long base = 0;
+    while (u0 >= base + (long long)a.H_kv * nb) { base += (long long)a.H_kv * nb; ++b; nb = seq_blocks(a, b); }
+    int hk = (int)((u0 - base) / nb);
+    int jbeg = (int)(u0 - base - (long long)hk * nb);
     const uint32_t my_smem = smem_u32(smem) + warp * (ATT_STAGES * STAGE_BYTES);
 
-    float o[16][4];
+    for (long long u = u0; u < u1;) {
+        const int jend = (int)min((long long)nb, (long long)jbeg + (u1 - u));
+        const int n_it = jend - jbeg;
+        if (n_it > 0) {
+            const int L = a.seq_len[b];
+            // Q fragments (A operand): rows = query heads of this KV group, zero-padded to 16.
+            uint32_t qa[8][4];
+            {
+                const uint16_t* qb = a.q + ((int64_t)b * a.H_q + (int64_t)hk * G) * ATT_D;
 #pragma unroll
-    for (int i = 0; i < 16; ++i) o[i][0] = o[i][1] = o[i][2] = o[i][3] = 0.f;
-    float m0 = -INFINITY, m1 = -INFINITY, l0 = 0.f, l1 = 0.f;
-
-    const int n_it = jend - jbeg;
-    // the chunk's block ids, one per lane (chunk_blocks <= 32), broadcast by shuffle when needed
-    const int my_blk = (lane < n_it) ? (idx ? idx[jbeg + lane] : (jbeg + lane)) : 0;
-    // prologue: fill STAGES-1 stages
-#pragma unroll
-    for (int s = 0; s < ATT_STAGES - 1; ++s) {
-        if (s < n_it) {
-            int blk_id = __shfl_sync(0xffffffffu, my_blk, s);
-            issue_subtile(my_smem + s * STAGE_BYTES, kbase, vbase, a.st, blk_id * 64 + warp * SUB_TOK, L, lane);
-        }
-        cp_async_commit();
-    }
-
-    for (int it = 0; it < n_it; ++it) {
-        {
-            int nx = it + ATT_STAGES - 1;
-            if (nx < n_it) {
-                int blk_id = __shfl_sync(0xffffffffu, my_blk, nx);
-                issue_subtile(my_smem + (nx % ATT_STAGES) * STAGE_BYTES, kbase, vbase, a.st,
-                              blk_id * 64 + warp * SUB_TOK, L, lane);
+                for (int ks = 0; ks < 8; ++ks) {
+                    int col = ks * 16 + c * 2;
+                    qa[ks][0] = (g < G) ? *reinterpret_cast<const uint32_t*>(qb + g * ATT_D + col) : 0u;
+                    qa[ks][1] = (g + 8 < G) ? *reinterpret_cast<const uint32_t*>(qb + (g + 8) * ATT_D + col) : 0u;
+                    qa[ks][2] = (g < G) ? *reinterpret_cast<const uint32_t*>(qb + g * ATT_D + col + 8) : 0u;
+                    qa[ks][3] = (g + 8 < G) ? *reinterpret_cast<const uint32_t*>(qb + (g + 8) * ATT_D + col + 8) : 0u;
+                }
             }
-            cp_async_commit();
-        }
-        cp_async_wait<ATT_STAGES - 1>();
-        __syncwarp();
+            const uint16_t* kbase = a.k + (int64_t)b * a.sb + (int64_t)hk * a.sh;
+            const uint16_t* vbase = a.v + (int64_t)b * a.sb + (int64_t)hk * a.sh;
+            const int32_t* idx = a.indices ? a.indices + (int64_t)b * a.cap + jbeg : nullptr;
 
-        const uint32_t ks_base = my_smem + (it % ATT_STAGES) * STAGE_BYTES;
-        const uint32_t vs_base = ks_base + SUB_TOK * 256;
-        const int blk_id = __shfl_sync(0xffffffffu, my_blk, it);
-        const int tok0 = blk_id * 64 + warp * SUB_TOK;
-
-        // S = Q K^T : 16 (heads) x 16 (tokens), k = 128
-        float s[2][4] = {{0.f, 0.f, 0.f, 0.f}, {0.f, 0.f, 0.f, 0.f}};
-        {
-            const int mi = lane >> 3, r8 = lane & 7;
-            const int row = (mi >> 1) * 8 + r8;
+            float o[16][4];
 #pragma unroll
-            for (int ks = 0; ks < 8; ++ks) {
-                uint32_t b0, b1, b2, b3;
-                ldmatrix_x4(b0, b1, b2, b3, ks_base + sw_off(row, 2 * ks + (mi & 1)));
-                mma_bf16_16816(s[0], qa[ks][0], qa[ks][1], qa[ks][2], qa[ks][3], b0, b1);
-                mma_bf16_16816(s[1], qa[ks][0], qa[ks][1], qa[ks][2], qa[ks][3], b2, b3);
+            for (int i = 0; i < 16; ++i) o[i][0] = o[i][1] = o[i][2] = o[i][3] = 0.f;
+            float m0 = -INFINITY, m1 = -INFINITY, l0 = 0.f, l1 = 0.f;
+
+            // block ids of the portion, 32 per window, one per lane; the next window is fetched a window ahead
+            auto load_ids = [&](int w) -> int {
+                const int it = w * 32 + lane;
+                return (it < n_it) ? (idx ? idx[it] : (jbeg + it)) : 0;
+            };
+            int ids_cur = load_ids(0), ids_nxt = load_ids(1), win = 0;
+            auto blk_at = [&](int it) -> int {
+                return __shfl_sync(0xffffffffu, (it >> 5) == win ? ids_cur : ids_nxt, it & 31);
+            };
+            // prologue: fill STAGES-1 stages
+#pragma unroll
+            for (int s = 0; s < ATT_STAGES - 1; ++s) {
+                if (s < n_it)
+                    issue_subtile(my_smem + s * STAGE_BYTES, kbase, vbase, a.st, blk_at(s) * 64 + warp * SUB_TOK, L, lane);
+                cp_async_commit();
             }
-        }
-        // scale to the log2 domain, mask tokens beyond the sequence (only the ragged last block can have any)
+
+            for (int it = 0; it < n_it; ++it) {
+                if ((it >> 5) != win) { win = it >> 5; ids_cur = ids_nxt; ids_nxt = load_ids(win + 1); }
+                {
+                    int nx = it + ATT_STAGES - 1;
+                    if (nx < n_it)
+                        issue_subtile(my_smem + (nx % ATT_STAGES) * STAGE_BYTES, kbase, vbase, a.st,
+                                      blk_at(nx) * 64 + warp * SUB_TOK, L, lane);
+                    cp_async_commit();
+                }
+                cp_async_wait<ATT_STAGES - 1>();
+                __syncwarp();
+
+                const uint32_t ks_base = my_smem + (it % ATT_STAGES) * STAGE_BYTES;
+                const uint32_t vs_base = ks_base + SUB_TOK * 256;
+                const int tok0 = blk_at(it) * 64 + warp * SUB_TOK;
+
+                // S = Q K^T : 16 (heads) x 16 (tokens), k = 128
+                float s[2][4] = {{0.f, 0.f, 0.f, 0.f}, {0.f, 0.f, 0.f, 0.f}};
+                {
+                    const int mi = lane >> 3, r8 = lane & 7;
+                    const int row = (mi >> 1) * 8 + r8;
 #pragma unroll
-        for (int nt = 0; nt < 2; ++nt)
+                    for (int ks = 0; ks < 8; ++ks) {
+                        uint32_t b0, b1, b2, b3;
+                        ldmatrix_x4(b0, b1, b2, b3, ks_base + sw_off(row, 2 * ks + (mi & 1)));
+                        mma_bf16_16816(s[0], qa[ks][0], qa[ks][1], qa[ks][2], qa[ks][3], b0, b1);
+                        mma_bf16_16816(s[1], qa[ks][0], qa[ks][1], qa[ks][2], qa[ks][3], b2, b3);
+                    }
+                }
+                // scale to the log2 domain, mask tokens beyond the sequence (only a ragged last block has any)
 #pragma unroll
-            for (int e = 0; e < 4; ++e) {
-                int tok = tok0 + nt * 8 + c * 2 + (e & 1);
-                s[nt][e] = (tok < L) ? s[nt][e] * a.scale_log2 : -INFINITY;
+                for (int nt = 0; nt < 2; ++nt)
+#pragma unroll
+                    for (int e = 0; e < 4; ++e) {
+                        int tok = tok0 + nt * 8 + c * 2 + (e & 1);
+                        s[nt][e] = (tok < L) ? s[nt][e] * a.scale_log2 : -INFINITY;
+                    }
+                // online softmax, rows g (m0, l0) and g + 8 (m1, l1)
+                float mx0 = fmaxf(fmaxf(s[0][0], s[0][1]), fmaxf(s[1][0], s[1][1]));
+                float mx1 = fmaxf(fmaxf(s[0][2], s[0][3]), fmaxf(s[1][2], s[1][3]));
+                mx0 = fmaxf(mx0, __shfl_xor_sync(0xffffffffu, mx0, 1));
+                mx0 = fmaxf(mx0, __shfl_xor_sync(0xffffffffu, mx0, 2));
+                mx1 = fmaxf(mx1, __shfl_xor_sync(0xffffffffu, mx1, 1));
+                mx1 = fmaxf(mx1, __shfl_xor_sync(0xffffffffu, mx1, 2));
+                const float mn0 = fmaxf(m0, mx0), mn1 = fmaxf(m1, mx1);
+                const float mu0 = (mn0 == -INFINITY) ? 0.f : mn0, mu1 = (mn1 == -INFINITY) ? 0.f : mn1;
+                const float c0 = fast_exp2(m0 - mu0), c1 = fast_exp2(m1 - mu1);
+                m0 = mn0; m1 = mn1;
+                float ps0 = 0.f, ps1 = 0.f;
+#pragma unroll
+                for (int nt = 0; nt < 2; ++nt) {
+                    s[nt][0] = fast_exp2(s[nt][0] - mu0); s[nt][1] = fast_exp2(s[nt][1] - mu0);
+                    s[nt][2] = fast_exp2(s[nt][2] - mu1); s[nt][3] = fast_exp2(s[nt][3] - mu1);
+                    ps0 += s[nt][0] + s[nt][1];
+                    ps1 += s[nt][2] + s[nt][3];
+                }
+                l0 = l0 * c0 + ps0;
+                l1 = l1 * c1 + ps1;
+#pragma unroll
+                for (int i = 0; i < 16; ++i) { o[i][0] *= c0; o[i][1] *= c0; o[i][2] *= c1; o[i][3] *= c1; }
+
+                // O += P V : P (16 x 16 tokens) as A, V (16 tokens x 128) as B through ldmatrix.trans
+                const uint32_t pa0 = pack_bf16x2(s[0][0], s[0][1]), pa1 = pack_bf16x2(s[0][2], s[0][3]);
+                const uint32_t pa2 = pack_bf16x2(s[1][0], s[1][1]), pa3 = pack_bf16x2(s[1][2], s[1][3]);
+                {
+                    const int mi = lane >> 3, r8 = lane & 7;
+                    const int row = (mi & 1) * 8 + r8;
+#pragma unroll
+                    for (int nd = 0; nd < 16; nd += 2) {
+                        uint32_t b0, b1, b2, b3;
+                        ldmatrix_x4_trans(b0, b1, b2, b3, vs_base + sw_off(row, nd + (mi >> 1)));
+                        mma_bf16_16816(o[nd], pa0, pa1, pa2, pa3, b0, b1);
+                        mma_bf16_16816(o[nd + 1], pa0, pa1, pa2, pa3, b2, b3);
+                    }
+                }
+                __syncwarp();   // everyone is done reading this stage before a later iteration refills it
             }
-        // online softmax, rows g (m0, l0) and g + 8 (m1, l1)
-        float mx0 = fmaxf(fmaxf(s[0][0], s[0][1]), fmaxf(s[1][0], s[1][1]));
-        float mx1 = fmaxf(fmaxf(s[0][2], s[0][3]), fmaxf(s[1][2], s[1][3]));
-        mx0 = fmaxf(mx0, __shfl_xor_sync(0xffffffffu, mx0, 1));
-        mx0 = fmaxf(mx0, __shfl_xor_sync(0xffffffffu, mx0, 2));
-        mx1 = fmaxf(mx1, __shfl_xor_sync(0xffffffffu, mx1, 1));
-        mx1 = fmaxf(mx1, __shfl_xor_sync(0xffffffffu, mx1, 2));
-        const float mn0 = fmaxf(m0, mx0), mn1 = fmaxf(m1, mx1);
-        const float mu0 = (mn0 == -INFINITY) ? 0.f : mn0, mu1 = (mn1 == -INFINITY) ? 0.f : mn1;
-        const float c0 = fast_exp2(m0 - mu0), c1 = fast_exp2(m1 - mu1);
-        m0 = mn0; m1 = mn1;
-        float ps0 = 0.f, ps1 = 0.f;
-#pragma unroll
-        for (int nt = 0; nt < 2; ++nt) {
-            s[nt][0] = fast_exp2(s[nt][0] - mu0); s[nt][1] = fast_exp2(s[nt][1] - mu0);
-            s[nt][2] = fast_exp2(s[nt][2] - mu1); s[nt][3] = fast_exp2(s[nt][3] - mu1);
-            ps0 += s[nt][0] + s[nt][1];
-            ps1 += s[nt][2] + s[nt][3];
-        }
-        l0 = l0 * c0 + ps0;
-        l1 = l1 * c1 + ps1;
-#pragma unroll
-        for (int i = 0; i < 16; ++i) { o[i][0] *= c0; o[i][1] *= c0; o[i][2] *= c1; o[i][3] *= c1; }
+            cp_async_wait<0>();
 
-        // O += P V : P (16 x 16 tokens) as A, V (16 tokens x 128) as B through ldmatrix.trans
-        const uint32_t pa0 = pack_bf16x2(s[0][0], s[0][1]), pa1 = pack_bf16x2(s[0][2], s[0][3]);
-        const uint32_t pa2 = pack_bf16x2(s[1][0], s[1][1]), pa3 = pack_bf16x2(s[1][2], s[1][3]);
-        {
-            const int mi = lane >> 3, r8 = lane & 7;
-            const int row = (mi & 1) * 8 + r8;
+            // full row sums
+            l0 += __shfl_xor_sync(0xffffffffu, l0, 1); l0 += __shfl_xor_sync(0xffffffffu, l0, 2);
+            l1 += __shfl_xor_sync(0xffffffffu, l1, 1); l1 += __shfl_xor_sync(0xffffffffu, l1, 2);
+
+            // merge the 4 warps through shared memory (the rings are idle now)
+            __syncthreads();
+            float* so = reinterpret_cast<float*>(smem);                  // [warp][16][128]
+            float* sml = so + ATT_WARPS * 16 * ATT_D;                    // [warp][16][2]
 #pragma unroll
-            for (int nd = 0; nd < 16; nd += 2) {
-                uint32_t b0, b1, b2, b3;
-                ldmatrix_x4_trans(b0, b1, b2, b3, vs_base + sw_off(row, nd + (mi >> 1)));
-                mma_bf16_16816(o[nd], pa0, pa1, pa2, pa3, b0, b1);
-                mma_bf16_16816(o[nd + 1], pa0, pa1, pa2, pa3, b2, b3);
+            for (int nd = 0; nd < 16; ++nd) {
+                int col = nd * 8 + c * 2;
+                *reinterpret_cast<float2*>(so + (warp * 16 + g) * ATT_D + col) = make_float2(o[nd][0], o[nd][1]);
+                *reinterpret_cast<float2*>(so + (warp * 16 + g + 8) * ATT_D + col) = make_float2(o[nd][2], o[nd][3]);
             }
+            if (c == 0) {
+                sml[(warp * 16 + g) * 2] = m0; sml[(warp * 16 + g) * 2 + 1] = l0;
+                sml[(warp * 16 + g + 8) * 2] = m1; sml[(warp * 16 + g + 8) * 2 + 1] = l1;
+            }
+            __syncthreads();
+            const int64_t pbase = ((int64_t)blockIdx.x + (int64_t)b * a.H_kv + hk) * G;   // slot = CTA + segment
+            for (int r = 0; r < G; ++r) {
+                float mw[ATT_WARPS], M = -INFINITY;
+#pragma unroll
+                for (int w = 0; w < ATT_WARPS; ++w) { mw[w] = sml[(w * 16 + r) * 2]; M = fmaxf(M, mw[w]); }
+                const float Mu = (M == -INFINITY) ? 0.f : M;
+                float acc = 0.f, lsum = 0.f;
+#pragma unroll
+                for (int w = 0; w < ATT_WARPS; ++w) {
+                    float f = fast_exp2(mw[w] - Mu);
+                    acc += f * so[(w * 16 + r) * ATT_D + threadIdx.x];
+                    lsum += f * sml[(w * 16 + r) * 2 + 1];
+                }
+                a.part_o[(pbase + r) * ATT_D + threadIdx.x] = acc;
+                if (threadIdx.x == 0) { a.part_ml[(pbase + r) * 2] = M; a.part_ml[(pbase + r) * 2 + 1] = lsum; }
+            }
+            __syncthreads();    // the rings are reused by the next portion
         }
-        __syncwarp();   // everyone is done reading this stage before a later iteration refills it
-    }
-    cp_async_wait<0>();
-
-    // full row sums
-    l0 += __shfl_xor_sync(0xffffffffu, l0, 1); l0 += __shfl_xor_sync(0xffffffffu, l0, 2);
-    l1 += __shfl_xor_sync(0xffffffffu, l1, 1); l1 += __shfl_xor_sync(0xffffffffu, l1, 2);
-
-    // merge the 4 warps through shared memory (the rings are idle now)
-    __syncthreads();
-    float* so = reinterpret_cast<float*>(smem);                  // [warp][16][128]
-    float* sml = so + ATT_WARPS * 16 * ATT_D;                    // [warp][16][2]
-#pragma unroll
-    for (int nd = 0; nd < 16; ++nd) {
-        int col = nd * 8 + c * 2;
-        *reinterpret_cast<float2*>(so + (warp * 16 + g) * ATT_D + col) = make_float2(o[nd][0], o[nd][1]);
-        *reinterpret_cast<float2*>(so + (warp * 16 + g + 8) * ATT_D + col) = make_float2(o[nd][2], o[nd][3]);
-    }
-    if (c == 0) {
-        sml[(warp * 16 + g) * 2] = m0; sml[(warp * 16 + g) * 2 + 1] = l0;
-        sml[(warp * 16 + g + 8) * 2] = m1; sml[(warp * 16 + g + 8) * 2 + 1] = l1;
-    }
-    __syncthreads();
-    const int64_t pbase = (((int64_t)b * a.H_kv + hk) * a.n_chunks + chunk) * G;
-    for (int r = 0; r < G; ++r) {
-        float mw[ATT_WARPS], M = -INFINITY;
-#pragma unroll
-        for (int w = 0; w < ATT_WARPS; ++w) { mw[w] = sml[(w * 16 + r) * 2]; M = fmaxf(M, mw[w]); }
-        const float Mu = (M == -INFINITY) ? 0.f : M;
-        float acc = 0.f, lsum = 0.f;
-#pragma unroll
-        for (int w = 0; w < ATT_WARPS; ++w) {
-            float f = fast_exp2(mw[w] - Mu);
-            acc += f * so[(w * 16 + r) * ATT_D + threadIdx.x];
-            lsum += f * sml[(w * 16 + r) * 2 + 1];
+        u += n_it;
+        jbeg = jend;
+        if (jbeg >= nb) {
+            jbeg = 0;
+            if (++hk == a.H_kv) { hk = 0; ++b; nb = (b < a.B) ? seq_blocks(a, b) : 1; }
         }
-        a.part_o[(pbase + r) * ATT_D + threadIdx.x] = acc;
-        if (threadIdx.x == 0) { a.part_ml[(pbase + r) * 2] = M; a.part_ml[(pbase + r) * 2 + 1] = lsum; }
     }
 }
 
-// merge the chunk partials of one (sequence, query head): 8 warps take the chunks round-robin (one 512-byte partial
-// row per warp per step, float4 per lane), then the 8 partial sums are combined through shared memory.
-constexpr int MERGE_WARPS = 8;
+// merge the partials of one (sequence, query head): one warp each.  The contributors of segment s = (b, hk) are the
+// CTAs whose ranges overlap the segment's units; their slots are CTA + s.
+constexpr int MERGE_WARPS = 4;
 __global__ void __launch_bounds__(MERGE_WARPS * 32) attn_merge_kernel(AttnArgs a) {
-    __shared__ float s_m[MERGE_WARPS];
-    __shared__ __align__(16) float s_acc[MERGE_WARPS][ATT_D];
-    __shared__ float s_l[MERGE_WARPS];
-    const int h = blockIdx.x, b = blockIdx.y;
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int lane = threadIdx.x & 31;
+    const int row = blockIdx.x * MERGE_WARPS + (threadIdx.x >> 5);
+    pdl_wait();
+    pdl_launch_dependents();
+    if (row >= a.B * a.H_q) return;
+    const int b = row / a.H_q, h = row - b * a.H_q;
     const int G = a.G, hk = h / G, r = h - hk * G;
-    const int L = a.seq_len[b];
-    const int budget = a.indices ? min(a.budgets[b], a.cap) : ((L + 63) >> 6);
-    const int nch = (budget + a.chunk_blocks - 1) / a.chunk_blocks;
-    const int64_t base = ((int64_t)b * a.H_kv + hk) * a.n_chunks;
+    long long U = 0, before = 0;
+    for (int bb = 0; bb < a.B; ++bb) {
+        const int n = seq_blocks(a, bb);
+        if (bb < b) before += n;
+        U += n;
+    }
+    U *= a.H_kv;
+    const int nb = seq_blocks(a, b);
+    uint16_t* outp = a.out + ((int64_t)b * a.H_q + h) * ATT_D + lane * 4;
+    if (nb == 0) {
+        *reinterpret_cast<uint2*>(outp) = make_uint2(0u, 0u);
+        if (a.lse && lane == 0) a.lse[(int64_t)b * a.H_q + h] = -INFINITY;
+        return;
+    }
+    const long long us = before * a.H_kv + (long long)hk * nb, ue = us + nb;
+    const int n = a.n_ctas;
+    const int c_first = (int)(((us + 1) * n - 1) / U), c_last = (int)((ue * n - 1) / U);
+    const int64_t seg = (int64_t)b * a.H_kv + hk;
+    // with more CTAs than units some ranges are empty: those CTAs wrote nothing
+    const bool all_live = U >= n;       // (64-bit divisions are slow: only the tiny-problem case pays for them)
+    auto live = [&](int cc) -> bool { return all_live || (long long)cc * U / n < (long long)(cc + 1) * U / n; };
     float M = -INFINITY;
-    for (int ch = threadIdx.x; ch < nch; ch += MERGE_WARPS * 32) M = fmaxf(M, a.part_ml[((base + ch) * G + r) * 2]);
+    for (int cc = c_first + lane; cc <= c_last; cc += 32)
+        if (live(cc)) M = fmaxf(M, a.part_ml[((cc + seg) * G + r) * 2]);
 #pragma unroll
     for (int o = 16; o; o >>= 1) M = fmaxf(M, __shfl_xor_sync(0xffffffffu, M, o));
-    if (lane == 0) s_m[warp] = M;
-    __syncthreads();
-#pragma unroll
-    for (int w = 0; w < MERGE_WARPS; ++w) M = fmaxf(M, s_m[w]);
     const float Mu = (M == -INFINITY) ? 0.f : M;
     float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
     float lsum = 0.f;
 #pragma unroll 4
-    for (int ch = warp; ch < nch; ch += MERGE_WARPS) {
-        const int64_t pr = (base + ch) * G + r;
+    for (int cc = c_first; cc <= c_last; ++cc) {
+        if (!live(cc)) continue;
+        const int64_t pr = (cc + seg) * G + r;
         const float2 ml = *reinterpret_cast<const float2*>(a.part_ml + pr * 2);
         const float4 o = *reinterpret_cast<const float4*>(a.part_o + pr * ATT_D + lane * 4);
         const float f = fast_exp2(ml.x - Mu);
         acc.x += f * o.x; acc.y += f * o.y; acc.z += f * o.z; acc.w += f * o.w;
         lsum += f * ml.y;
     }
-    *reinterpret_cast<float4*>(&s_acc[warp][lane * 4]) = acc;
-    if (lane == 0) s_l[warp] = lsum;
-    __syncthreads();
-    if (threadIdx.x < ATT_D) {
-        float tot = 0.f, lt = 0.f;
-#pragma unroll
-        for (int w = 0; w < MERGE_WARPS; ++w) { tot += s_acc[w][threadIdx.x]; lt += s_l[w]; }
-        float outv = (lt > 0.f) ? tot / lt : 0.f;
-        a.out[((int64_t)b * a.H_q + h) * ATT_D + threadIdx.x] = __bfloat16_as_ushort(__float2bfloat16_rn(outv));
-        if (a.lse && threadIdx.x == 0)
-            a.lse[(int64_t)b * a.H_q + h] = (lt > 0.f) ? (M + log2f(lt)) * 0.6931471805599453f : -INFINITY;
-    }
+    const float inv = lsum > 0.f ? 1.f / lsum : 0.f;
+    *reinterpret_cast<uint2*>(outp) = make_uint2(pack_bf16x2(acc.x * inv, acc.y * inv), pack_bf16x2(acc.z * inv, acc.w * inv));
+    if (a.lse && lane == 0)
+        a.lse[(int64_t)b * a.H_q + h] = (lsum > 0.f) ? (M + log2f(lsum)) * 0.6931471805599453f : -INFINITY;
 }
 
-int pick_chunk_blocks(const spot_attn_params* p, bool dense) {
-    // enough CTAs for ~4 waves of 2 CTAs/SM at the largest possible budget, at most 8 blocks (256 KiB of KV per
-    // head) per CTA so that the partials stay < 2 % of the traffic
+// persistent grid: two CTAs per SM, never more CTAs than units
+int pick_ctas(const spot_attn_params* p, bool dense) {
     int64_t max_blocks = dense ? (p->max_seq_len + 63) / 64 : p->cap;
-    int64_t total = max_blocks * p->H_kv * p->B;
-    int64_t want = (int64_t)sm_count() * 2 * 4;
-    int64_t cb = total / want;
-    if (cb < 1) cb = 1;
-    if (cb > 8) cb = 8;   // must stay <= 32 (one block id per lane)
-    return (int)cb;
+    int64_t units = max_blocks * p->H_kv * p->B;
+    int64_t want = (int64_t)sm_count() * 2;
+    return (int)(units < want ? (units < 1 ? 1 : units) : want);
 }
 
 spot_status check_attn(const spot_attn_params* p, bool dense, bool prefill) {
@@ -303,10 +338,8 @@ spot_status check_attn(const spot_attn_params* p, bool dense, bool prefill) {
 
 size_t decode_ws_bytes(const spot_attn_params* p, bool dense) {
     const bool use_idx = !dense && p->indices;
-    int cb = pick_chunk_blocks(p, !use_idx);
-    int64_t max_blocks = use_idx ? p->cap : (p->max_seq_len + 63) / 64;
-    int64_t n_chunks = (max_blocks + cb - 1) / cb;
-    return (size_t)((int64_t)p->B * p->H_q * n_chunks * (ATT_D + 2) * 4);
+    const int64_t slots = (int64_t)pick_ctas(p, !use_idx) + (int64_t)p->B * p->H_kv;
+    return (size_t)(slots * (p->H_q / p->H_kv) * (ATT_D + 2) * 4);
 }
 
 spot_status run_decode(const spot_attn_params* p, bool dense, cudaStream_t s) {
@@ -314,31 +347,30 @@ spot_status run_decode(const spot_attn_params* p, bool dense, cudaStream_t s) {
     if (stt != SPOT_OK) return stt;
     if ((stt = check_device()) != SPOT_OK) return stt;
     const bool use_idx = !dense && p->indices;
-    int cb = pick_chunk_blocks(p, !use_idx);
-    int64_t max_blocks = use_idx ? p->cap : (p->max_seq_len + 63) / 64;
-    int n_chunks = (int)((max_blocks + cb - 1) / cb);
-    size_t need = (size_t)((int64_t)p->B * p->H_q * n_chunks * (ATT_D + 2) * 4);
+    const int n_ctas = pick_ctas(p, !use_idx);
+    const int G = p->H_q / p->H_kv;
+    const int64_t slots = (int64_t)n_ctas + (int64_t)p->B * p->H_kv;
+    const size_t need = (size_t)(slots * G * (ATT_D + 2) * 4);
     if (!p->workspace || p->workspace_bytes < need) return SPOT_ERR_WORKSPACE_TOO_SMALL;
     AttnArgs a;
     a.q = p->q; a.k = p->k; a.v = p->v;
     a.sb = p->kv_stride_batch; a.st = p->kv_stride_token; a.sh = p->kv_stride_head;
     a.seq_len = p->seq_len; a.indices = use_idx ? p->indices : nullptr; a.budgets = p->budgets; a.cap = p->cap;
-    a.H_q = p->H_q; a.H_kv = p->H_kv; a.G = p->H_q / p->H_kv;
+    a.B = p->B; a.H_q = p->H_q; a.H_kv = p->H_kv; a.G = G;
     a.scale_log2 = p->sm_scale * 1.4426950408889634f;
-    a.chunk_blocks = cb; a.n_chunks = n_chunks;
+    a.n_ctas = n_ctas;
     a.part_o = reinterpret_cast<float*>(p->workspace);
-    a.part_ml = a.part_o + (int64_t)p->B * p->H_q * n_chunks * ATT_D;
+    a.part_ml = a.part_o + slots * G * ATT_D;
     a.out = p->out; a.lse = p->lse;
     static bool attr_set = false;
     if (!attr_set) {
         SPOT_CUDA_TRY(cudaFuncSetAttribute(attn_decode_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, ATT_SMEM));
         attr_set = true;
     }
-    dim3 grid((unsigned)n_chunks, (unsigned)p->H_kv, (unsigned)p->B);
-    attn_decode_kernel<<<grid, ATT_WARPS * 32, ATT_SMEM, s>>>(a);
-    SPOT_LAUNCH_CHECK();
-    attn_merge_kernel<<<dim3((unsigned)p->H_q, (unsigned)p->B), MERGE_WARPS * 32, 0, s>>>(a);
-    SPOT_LAUNCH_CHECK();
+    SPOT_CUDA_TRY(launch_pdl(attn_decode_kernel, dim3((unsigned)n_ctas), dim3(ATT_WARPS * 32), ATT_SMEM, s, a));
+    const int rows = p->B * p->H_q;
+    SPOT_CUDA_TRY(launch_pdl(attn_merge_kernel, dim3((unsigned)((rows + MERGE_WARPS - 1) / MERGE_WARPS)),
+                             dim3(MERGE_WARPS * 32), 0, s, a));
     return SPOT_OK;
 }
 

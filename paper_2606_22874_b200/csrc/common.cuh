@@ -40,6 +40,31 @@ __host__ __device__ inline int64_t selk_tile_bytes(int H, int d) {
     return SELK_TILE * (selk_codes_per_token(H, d) + selk_scales_per_token(H, d));
 }
 
+// ---- programmatic dependent launch (PDL) ------------------------------------------------------------
+// The decode step is a chain of four short kernels (score -> select -> attend -> merge) whose launch latencies sit
+// on the critical path.  Every kernel of the chain is launched with programmaticStreamSerializationAllowed = 1 and
+//   * calls pdl_wait() before its first global read or write (returns once the previous kernel in the stream has
+//     completed and its writes are visible; a no-op under an ordinary launch), on EVERY path, so that completion of
+//     a kernel always implies completion of its predecessors;
+//   * calls pdl_launch_dependents() right after, which lets the next kernel's CTAs become resident (and run their
+//     own prologue up to pdl_wait()) as soon as SM resources allow.  All grids here fit on the chip in one wave, so
+//     early-resident dependents never starve their predecessor.
+#ifdef __CUDACC__
+template <typename... KArgs, typename... Args>
+static inline cudaError_t launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t s,
+                                     Args... args) {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = s;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at; cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, kernel, KArgs(args)...);
+}
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+#endif
+
 // ---- device helpers ------------------------------------------------------------------------------
 #ifdef __CUDACC__
 

@@ -86,6 +86,8 @@ __global__ void __launch_bounds__(SCORE_WARPS * 32) score_decode_bf16_kernel(
     const int b = blockIdx.y;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int g = lane >> 2, c = lane & 3;
+    pdl_wait();
+    pdl_launch_dependents();
     const int L = seq_len[b];
     const int n_b = (L + 63) >> 6;
 
@@ -165,6 +167,8 @@ __global__ void __launch_bounds__(SCORE_WARPS * 32) score_decode_q4_kernel(
     const int b = blockIdx.y;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int g = lane >> 2, c = lane & 3;
+    pdl_wait();
+    pdl_launch_dependents();
     const int L = seq_len[b];
     const int n_b = (L + 63) >> 6;
 
@@ -277,19 +281,26 @@ __global__ void __launch_bounds__(SCORE_WARPS * 32) score_decode_q4_kernel(
 
 template <int H, int D_IDX>
 spot_status launch_score(const spot_select_params* p, float* scores, int nb_stride, cudaStream_t s) {
+    // every warp gets the same number of 64-token tiles: with T tiles per sequence and room for `cap_warps` warps
+    // per sequence (4 CTAs per SM in all), tiles per warp = ceil(T / cap_warps) and just enough warps for that.
+    // (A grid-stride loop over a fixed 4 CTAs/SM grid left 3.46 tiles per warp at L = 128K, B = 4: a quarter of the
+    // warps ran a 4th tile while the others idled -- profiles/r1_decode_cfg3_launches.md.)
     const int n_b_max = (p->max_seq_len + 63) / 64;
-    int per_seq = (n_b_max + SCORE_WARPS - 1) / SCORE_WARPS;
-    int cap_ctas = max(1, (sm_count() * 4) / p->B);
-    dim3 grid((unsigned)min(per_seq, cap_ctas), (unsigned)p->B);
+    const int cap_warps = max(1, (sm_count() * 4 * SCORE_WARPS) / p->B);
+    const int tiles_per_warp = (n_b_max + cap_warps - 1) / cap_warps;
+    const int warps = (n_b_max + tiles_per_warp - 1) / tiles_per_warp;
+    dim3 grid((unsigned)((warps + SCORE_WARPS - 1) / SCORE_WARPS), (unsigned)p->B);
+    const dim3 block(SCORE_WARPS * 32);
     if (p->fmt == SPOT_SELK_BF16) {
-        score_decode_bf16_kernel<H, D_IDX><<<grid, SCORE_WARPS * 32, 0, s>>>(
-            p->sel_q, p->w, (const uint16_t*)p->sel_k, p->cache_stride_tokens, p->seq_len, scores, nb_stride);
+        SPOT_CUDA_TRY(launch_pdl(score_decode_bf16_kernel<H, D_IDX>, grid, block, 0, s, p->sel_q, p->w,
+                                 (const uint16_t*)p->sel_k, p->cache_stride_tokens, p->seq_len, scores, nb_stride));
     } else if (p->fmt == SPOT_SELK_MXFP4) {
-        score_decode_q4_kernel<H, D_IDX, SPOT_SELK_MXFP4><<<grid, SCORE_WARPS * 32, 0, s>>>(
-            p->sel_q, p->w, (const uint8_t*)p->sel_k, p->cache_stride_tokens / 64, p->seq_len, scores, nb_stride);
+        SPOT_CUDA_TRY(launch_pdl(score_decode_q4_kernel<H, D_IDX, SPOT_SELK_MXFP4>, grid, block, 0, s, p->sel_q, p->w,
+                                 (const uint8_t*)p->sel_k, p->cache_stride_tokens / 64, p->seq_len, scores, nb_stride));
     } else {
-        score_decode_q4_kernel<H, D_IDX, SPOT_SELK_INT4_E4M3><<<grid, SCORE_WARPS * 32, 0, s>>>(
-            p->sel_q, p->w, (const uint8_t*)p->sel_k, p->cache_stride_tokens / 64, p->seq_len, scores, nb_stride);
+        SPOT_CUDA_TRY(launch_pdl(score_decode_q4_kernel<H, D_IDX, SPOT_SELK_INT4_E4M3>, grid, block, 0, s, p->sel_q,
+                                 p->w, (const uint8_t*)p->sel_k, p->cache_stride_tokens / 64, p->seq_len, scores,
+                                 nb_stride));
     }
     SPOT_LAUNCH_CHECK();
     return SPOT_OK;

@@ -75,6 +75,8 @@ __global__ void __launch_bounds__(1 << LT) select_kernel(SelectArgs a) {
     const int row = blockIdx.x;
     const int b = row / a.n_q, i = row - b * a.n_q;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    pdl_wait();
+    pdl_launch_dependents();
     int n_b;
     if (a.q_block == 1) n_b = (a.seq_len[b] + a.blk - 1) / a.blk;
     else n_b = (a.q_start + (i + 1) * a.q_block - 1) / a.blk + 1;
@@ -308,8 +310,7 @@ __global__ void __launch_bounds__(1 << LT) select_kernel(SelectArgs a) {
 
 template <int LT>
 spot_status launch_select(const SelectArgs& a, int rows, cudaStream_t s) {
-    select_kernel<LT><<<(unsigned)rows, 1 << LT, 0, s>>>(a);
-    SPOT_LAUNCH_CHECK();
+    SPOT_CUDA_TRY(launch_pdl(select_kernel<LT>, dim3((unsigned)rows), dim3(1 << LT), 0, s, a));
     return SPOT_OK;
 }
 

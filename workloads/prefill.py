@@ -2,8 +2,11 @@
 
 No method arithmetic here.  One sequence of L tokens, causal.  Selector Q and K
 are N(0,1) plus a low-rank "topic" component (n_topics random directions, each
-token assigned one topic, amplitude ``topic_amp``) so that tile scores are
-structured rather than flat; w_h[q] = (1 + 0.25 u) / (H_idx sqrt(d_idx)),
+span of ``topic_span`` consecutive tokens assigned one topic, amplitude
+``topic_amp``) so that tile scores are structured rather than flat: a query
+block's mass concentrates on the earlier spans that share its topic, which at
+the defaults gives per-query-block densities from about 0.15 to 0.85 at
+p = 0.9 (the per-layer K/L range of PAPER.md:166); w_h[q] = (1 + 0.25 u) / (H_idx sqrt(d_idx)),
 u ~ U(-1, 1).  Attention Q, K, V ~ N(0,1).  Layouts:
 
     Q      uint16 [L][H_q][D]           BF16 bits
@@ -53,13 +56,14 @@ class PrefillWorkload:
 
 
 def make_prefill_workload(name="cfg5", seed=5005, L=65536, H_q=32, H_kv=8, D=128, H_idx=4,
-                          d_idx=64, blk=64, q_block=64, n_topics=16, topic_amp=2.0,
+                          d_idx=64, blk=64, q_block=64, n_topics=16, topic_amp=5.5, topic_span=256,
                           mode="dual_topp", top_k=0, p=0.90, sink_blocks=1, recency_blocks=2,
                           kmin_blocks=8, temperature=1.0, with_kv=True):
     rng = np.random.Generator(np.random.Philox(seed))
     topics = rng.standard_normal((n_topics, H_idx, d_idx), dtype=np.float32)
     topics /= np.linalg.norm(topics, axis=-1, keepdims=True)
-    assign = rng.integers(0, n_topics, size=L)
+    n_span = -(-L // topic_span)
+    assign = np.repeat(rng.integers(0, n_topics, size=n_span), topic_span)[:L]
     sq = rng.standard_normal((L, H_idx, d_idx), dtype=np.float32) + topic_amp * topics[assign]
     sk = rng.standard_normal((L, H_idx, d_idx), dtype=np.float32) + topic_amp * topics[assign]
     u = rng.uniform(-1.0, 1.0, size=(L, H_idx)).astype(np.float32)
