@@ -1,25 +1,37 @@
 // Step a1, decode form -- stream the selector K-cache once and emit one score per 64-token block:
 //   s[t] = sum_h w_h ReLU(q_h . k_{h,t}),   s_bar[b] = max_{t in b} s[t].
 //
-// HBM-bound: 512 B (BF16) or 136 B (4-bit) per token, 2 flop/B.  One warp owns one 64-token tile at a time;
-// lanes issue 128-bit streaming loads straight into mma.sync A-fragments (no shared-memory staging: there is no
-// reuse), the query sits in the B fragment (column 0 only -- the tensor pipe is idle otherwise, so the wasted
-// columns are free) and the per-token reduction over d_idx happens inside the MMA instead of in shuffles.
+// HBM-bound: 512 B (BF16) or 136 B (4-bit) per token, 2 flop/B, no reuse.  What limits a kernel like this is the
+// number of bytes it keeps in flight (6.5 TB/s x ~1.5 us of loaded latency = ~10 MB = ~70 KiB per SM), so the loads
+// are taken off the warps' registers: one persistent CTA per SM owns a contiguous range of the flat (sequence, tile)
+// list and a producer lane streams its 64-token tiles through a shared-memory ring with the bulk-copy engine --
+//   BF16 cache : one cp.async.bulk.tensor (TMA) per tile, box [d 64][64 tokens][H*d/64 planes], 128-byte swizzle
+//                (32 KiB per tile at 4 x 64), so that ldmatrix reads of 8 token rows are bank-conflict free;
+//   4-bit cache: one cp.async.bulk per tile; the opaque layout keeps a tile's codes and scales contiguous (8704 B)
+// -- 144..192 KiB in flight per SM, completion on mbarriers.  Consumer warps (each owning its share of the ring's stages) take the tiles round-robin; a tile
+// is 16-token row groups fed to mma.sync m16n8k16 with the query in column 0 of the B fragment (the tensor pipe is
+// idle otherwise, so the 7 wasted columns are free) and the reduction over d_idx happens inside the MMA instead of
+// in shuffles.
 //   BF16 cache : bf16 HMMA, products exact, fp32 accumulate.
 //   4-bit cache: codes are unpacked to fp16 pairs in registers (INT4: magic-number OR + one HFMA2 per pair;
 //                MXFP4: cvt.rn.f16x2.e2m1x2, one instruction per pair), multiplied against an fp16 copy of the
 //                query (pre-scaled per head by a power of two so that the copy is exact for every element
 //                within 2^-29 of the head's largest), and the group scale is applied to the 32-element partial
-//                sum after the MMA (one FMUL per group instead of one per element).
-// The k index of each MMA is a fixed permutation of the d_idx axis applied to both operands, chosen so that
-// every lane's 16-byte load lands directly in fragment registers.
+//                sum after the MMA (one FMUL per group instead of one per element).  The k index of each MMA is a
+//                fixed permutation of the d_idx axis applied to both operands, chosen so that every lane's 16-byte
+//                shared-memory load lands directly in fragment registers.
 #include "common.cuh"
+#include "tc100.cuh"
+
+#include <string.h>
+#include <type_traits>
 
 namespace spot {
 
 namespace {
 
-constexpr int SCORE_WARPS = 4;
+constexpr int SC_SMEM_BUDGET = 196 * 1024;     // ring bytes per CTA (one CTA per SM)
+
 
 // four bytes of E2M1 pairs -> four fp16 pairs; the vector mov lets ptxas use F2FP's byte selectors (.B0-.B3),
 // one instruction per pair and no shift/mask.
@@ -73,67 +85,111 @@ __device__ __forceinline__ float scale_to_f32(uint32_t byte) {
     }
 }
 
-// ---------------------------------------------------------------------------------------------------
-// BF16 cache
-// ---------------------------------------------------------------------------------------------------
-template <int H, int D_IDX>
-__global__ void __launch_bounds__(SCORE_WARPS * 32) score_decode_bf16_kernel(
-    const uint16_t* __restrict__ sel_q, const float* __restrict__ w, const uint16_t* __restrict__ sel_k,
-    int64_t cache_stride_tokens, const int32_t* __restrict__ seq_len, float* __restrict__ scores, int nb_stride) {
-    constexpr int ROW = H * D_IDX;          // elements per token
-    constexpr int NSEG = ROW / 32;          // 64-byte segments per token
-    constexpr int SEG_PER_HEAD = D_IDX / 32;
-    const int b = blockIdx.y;
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const int g = lane >> 2, c = lane & 3;
-    pdl_wait();
-    pdl_launch_dependents();
-    const int L = seq_len[b];
-    const int n_b = (L + 63) >> 6;
 
-    // query fragments: only the lanes that hold column 0 of B (g == 0) carry q; k-permutation as in the header.
-    uint32_t qf[NSEG][4];
-    {
-        const uint4* qp = reinterpret_cast<const uint4*>(sel_q + (int64_t)b * ROW);
-#pragma unroll
-        for (int s = 0; s < NSEG; ++s) {
-            uint4 v = make_uint4(0, 0, 0, 0);
-            if (g == 0) v = qp[s * 4 + c];
-            qf[s][0] = v.x; qf[s][1] = v.y; qf[s][2] = v.z; qf[s][3] = v.w;
-        }
+__device__ __forceinline__ uint4 lds128(uint32_t addr) {
+    uint4 r;
+    asm volatile("ld.shared.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w) : "r"(addr));
+    return r;
+}
+__device__ __forceinline__ uint32_t lds32(uint32_t addr) {
+    uint32_t r;
+    asm volatile("ld.shared.u32 %0, [%1];" : "=r"(r) : "r"(addr));
+    return r;
+}
+// contiguous global -> shared bulk copy (bytes a multiple of 16), completion counted on an mbarrier
+__device__ __forceinline__ void bulk_load(uint32_t smem_dst, const void* gsrc, uint32_t bytes, uint32_t bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 :: "r"(smem_dst), "l"(gsrc), "r"(bytes), "r"(bar) : "memory");
+}
+
+template <int H, int D_IDX, int FMT>
+struct ScoreCfg {
+    static constexpr int ROW = H * D_IDX;                      // elements per token
+    static constexpr int TILE_BYTES = FMT == SPOT_SELK_BF16 ? 64 * ROW * 2 : 64 * (ROW / 2 + ROW / 32);
+    static constexpr int STAGE_BYTES = (TILE_BYTES + 1023) / 1024 * 1024;
+    static constexpr int STAGES_RAW = SC_SMEM_BUDGET / STAGE_BYTES;
+    // Every ring stage belongs to ONE consumer warp (stage s -> warp s % CONSUMERS), so a warp meets the phases of a
+    // stage's barrier strictly in order; with stages shared in rotation a warp could wait for phase k+1 of a barrier
+    // whose phase k (another warp's tile) has not completed yet, and a parity wait cannot tell those apart.
+    // BF16: few big tiles and a light ldmatrix + HMMA body -> as many consumers as stages (6 or 3).
+    // 4-bit: many small tiles and an ALU-heavy unpack -> 8 consumers, 16 or 8 stages.
+    static constexpr int CONSUMERS = FMT == SPOT_SELK_BF16 ? (STAGES_RAW > 6 ? 6 : STAGES_RAW) : 8;
+    static constexpr int STAGES = FMT == SPOT_SELK_BF16 ? CONSUMERS : (STAGES_RAW >= 16 ? 16 : 8);
+    static constexpr int THREADS = (CONSUMERS + 1) * 32;
+    static_assert(STAGES % CONSUMERS == 0 && STAGES * STAGE_BYTES <= SC_SMEM_BUDGET, "ring geometry");
+    static constexpr int Q16_BYTES = FMT == SPOT_SELK_BF16 ? 0 : CONSUMERS * (ROW * 2 + 64);
+    static constexpr int SMEM_BYTES = 1024 + STAGES * STAGE_BYTES + 2 * STAGES * 8 + Q16_BYTES + 64;
+};
+
+struct ScoreArgs {
+    const uint16_t* sel_q;        // [B][H][d]
+    const float* w;               // [B][H]
+    const uint8_t* sel_k;         // 4-bit formats: the cache; BF16: unused (the tensor map carries the address)
+    int64_t tiles_per_seq;        // 4-bit formats: cache_stride_tokens / 64
+    const int32_t* seq_len;
+    int B;
+    float* scores;
+    int nb_stride;
+};
+
+// (sequence, tile) cursor over the flat tile list
+struct TileCursor {
+    int b, t, nb;
+    __device__ __forceinline__ void advance(const ScoreArgs& a, int n) {
+        t += n;
+        while (t >= nb && b + 1 < a.B) { t -= nb; ++b; nb = (a.seq_len[b] + 63) >> 6; }
     }
-    float wh[H];
-#pragma unroll
-    for (int h = 0; h < H; ++h) wh[h] = w[(int64_t)b * H + h];
+};
 
-    const uint16_t* kb = sel_k + (int64_t)b * cache_stride_tokens * ROW;
-    for (int tile = blockIdx.x * SCORE_WARPS + warp; tile < n_b; tile += gridDim.x * SCORE_WARPS) {
-        float m = -INFINITY;
-        const int t0 = tile * 64;
-#pragma unroll 1
-        for (int it = 0; it < 4; ++it) {
-            const int ta = t0 + it * 16 + g, tb = ta + 8;
-            const uint4* ra = reinterpret_cast<const uint4*>(kb + (int64_t)min(ta, L - 1) * ROW) + c;
-            const uint4* rb = reinterpret_cast<const uint4*>(kb + (int64_t)min(tb, L - 1) * ROW) + c;
-            uint4 va[NSEG], vb[NSEG];
+// ---- BF16 tile: planes [H * D_IDX / 64][64 tokens][128 B], 128-byte swizzle --------------------------------
+template <int H, int D_IDX>
+struct Bf16Tile {
+    static constexpr int PPH = D_IDX / 64;       // planes per head
+    static constexpr int NP = H * PPH;
+    uint32_t qf[NP][4][2];
+    float wh[H];
+
+    __device__ __forceinline__ void load_query(const ScoreArgs& a, int b, int lane, uint32_t) {
+        const int g = lane >> 2, c = lane & 3;
+        const uint16_t* q = a.sel_q + (int64_t)b * (H * D_IDX);
 #pragma unroll
-            for (int s = 0; s < NSEG; ++s) {
-                va[s] = ldg_stream_v4(ra + s * 4);
-                vb[s] = ldg_stream_v4(rb + s * 4);
+        for (int pl = 0; pl < NP; ++pl)
+#pragma unroll
+            for (int ks = 0; ks < 4; ++ks) {
+                qf[pl][ks][0] = (g == 0) ? *reinterpret_cast<const uint32_t*>(q + pl * 64 + ks * 16 + 2 * c) : 0u;
+                qf[pl][ks][1] = (g == 0) ? *reinterpret_cast<const uint32_t*>(q + pl * 64 + ks * 16 + 8 + 2 * c) : 0u;
             }
+#pragma unroll
+        for (int h = 0; h < H; ++h) wh[h] = a.w[(int64_t)b * H + h];
+    }
+
+    // max over the tile's valid tokens of s[t]; valid on every lane after the final shuffles
+    __device__ __forceinline__ float tile_max(uint32_t st, int t0, int L, int lane) const {
+        const int g = lane >> 2, c = lane & 3, mi = lane >> 3, r8 = lane & 7;
+        float m = -INFINITY;
+#pragma unroll 1
+        for (int rg = 0; rg < 4; ++rg) {
+            const int row = rg * 16 + (mi & 1) * 8 + r8;
+            const uint32_t rbase = st + row * 128;
+            const int sw = row & 7;
             float sa = 0.f, sb = 0.f;
 #pragma unroll
             for (int h = 0; h < H; ++h) {
                 float acc[4] = {0.f, 0.f, 0.f, 0.f};
 #pragma unroll
-                for (int ss = 0; ss < SEG_PER_HEAD; ++ss) {
-                    const int s = h * SEG_PER_HEAD + ss;
-                    mma_bf16_16816(acc, va[s].x, vb[s].x, va[s].y, vb[s].y, qf[s][0], qf[s][1]);
-                    mma_bf16_16816(acc, va[s].z, vb[s].z, va[s].w, vb[s].w, qf[s][2], qf[s][3]);
+                for (int sub = 0; sub < PPH; ++sub) {
+                    const int pl = h * PPH + sub;
+#pragma unroll
+                    for (int ks = 0; ks < 4; ++ks) {
+                        uint32_t a0, a1, a2, a3;
+                        ldmatrix_x4(a0, a1, a2, a3, rbase + pl * 8192 + (((2 * ks + (mi >> 1)) ^ sw) << 4));
+                        mma_bf16_16816(acc, a0, a1, a2, a3, qf[pl][ks][0], qf[pl][ks][1]);
+                    }
                 }
                 sa = fmaf(wh[h], fmaxf(acc[0], 0.f), sa);   // column 0, row g     (valid on lanes c == 0)
                 sb = fmaf(wh[h], fmaxf(acc[2], 0.f), sb);   // column 0, row g + 8
             }
+            const int ta = t0 + rg * 16 + g, tb = ta + 8;
             if (ta < L) m = fmaxf(m, sa);
             if (tb < L) m = fmaxf(m, sb);
         }
@@ -141,106 +197,87 @@ __global__ void __launch_bounds__(SCORE_WARPS * 32) score_decode_bf16_kernel(
         m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, 4));
         m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, 8));
         m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, 16));
-        if (lane == 0) scores[(int64_t)b * nb_stride + tile] = m;
+        return m;
     }
-}
+};
 
-// ---------------------------------------------------------------------------------------------------
-// 4-bit caches (INT4 + E4M3 scale, MXFP4)
-// ---------------------------------------------------------------------------------------------------
+// ---- 4-bit tile: [64][ROW/2] code bytes, then [64][ROW/32] scale bytes ------------------------------------
 template <int H, int D_IDX, int FMT>
-__global__ void __launch_bounds__(SCORE_WARPS * 32) score_decode_q4_kernel(
-    const uint16_t* __restrict__ sel_q, const float* __restrict__ w, const uint8_t* __restrict__ sel_k,
-    int64_t tiles_per_seq, const int32_t* __restrict__ seq_len, float* __restrict__ scores, int nb_stride) {
-    constexpr int ROW = H * D_IDX;
-    constexpr int CPT = ROW / 2;            // code bytes per token
-    constexpr int NG = ROW / 32;            // groups (= scale bytes) per token
-    constexpr int NQL = NG / 4;             // 64-byte "quad loads" per token: 4 groups, one per lane of a quad
-    constexpr int GPH = D_IDX / 32;         // groups per head (2 or 4)
-    constexpr int64_t TILE_BYTES = 64 * (CPT + NG);
+struct Q4Tile {
+    static constexpr int ROW = H * D_IDX;
+    static constexpr int CPT = ROW / 2;            // code bytes per token
+    static constexpr int NG = ROW / 32;            // groups (= scale bytes) per token
+    static constexpr int NQL = NG / 4;             // 64-byte "quad loads" per token: 4 groups, one per lane of a quad
+    static constexpr int GPH = D_IDX / 32;         // groups per head (2 or 4)
     static_assert(GPH == 2 || GPH == 4, "d_idx must be 64 or 128 for the 4-bit scoring kernels");
     static_assert(NG % 4 == 0, "H_idx * d_idx must be a multiple of 128");
-
-    __shared__ __align__(16) __half q16[ROW];   // fp16 copy of q, pre-scaled per head by 2^sh[h]
-    __shared__ float post[H];                   // 2^-sh[h]
-
-    const int b = blockIdx.y;
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const int g = lane >> 2, c = lane & 3;
-    pdl_wait();
-    pdl_launch_dependents();
-    const int L = seq_len[b];
-    const int n_b = (L + 63) >> 6;
-
-    // prologue: one warp per head finds the head's largest |q| exponent and writes the scaled fp16 copy.
-    for (int h = warp; h < H; h += SCORE_WARPS) {
-        const uint16_t* qh = sel_q + (int64_t)b * ROW + h * D_IDX;
-        float mx = 0.f;
-        for (int i = lane; i < D_IDX; i += 32) mx = fmaxf(mx, fabsf(bf16_bits_to_float(qh[i])));
-#pragma unroll
-        for (int o = 16; o; o >>= 1) mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, o));
-        int sh = 0;
-        if (mx > 0.f) sh = 14 - ilogbf(mx);       // largest element lands in [2^14, 2^15)
-        sh = max(-100, min(100, sh));
-        float up = __uint_as_float((uint32_t)(127 + sh) << 23);
-        for (int i = lane; i < D_IDX; i += 32) q16[h * D_IDX + i] = __float2half_rn(bf16_bits_to_float(qh[i]) * up);
-        if (lane == 0) post[h] = __uint_as_float((uint32_t)(127 - sh) << 23);
-    }
-    __syncthreads();
-
-    // B fragments: column n of the MMA is the group held by quad-lane c == n; only lane (g == n, c == n) is non-zero.
     uint32_t qf[NQL][16];
-#pragma unroll
-    for (int ql = 0; ql < NQL; ++ql) {
-        const uint4* src = reinterpret_cast<const uint4*>(q16 + (ql * 4 + c) * 32);
-#pragma unroll
-        for (int i = 0; i < 4; ++i) {
-            uint4 v = make_uint4(0, 0, 0, 0);
-            if (g == c) v = src[i];
-            qf[ql][4 * i + 0] = v.x; qf[ql][4 * i + 1] = v.y; qf[ql][4 * i + 2] = v.z; qf[ql][4 * i + 3] = v.w;
-        }
-    }
-    // lanes c < 2 read columns 2c, 2c+1 = groups 4ql + 2c (+1); their head, weight and power-of-two post-scale:
     float wq[NQL], ps[NQL];
+
+    // q16: this warp's shared scratch, ROW halfs + H floats
+    __device__ __forceinline__ void load_query(const ScoreArgs& a, int b, int lane, uint32_t q16_addr) {
+        const int g = lane >> 2, c = lane & 3;
+        __half* q16 = reinterpret_cast<__half*>(__cvta_shared_to_generic((size_t)q16_addr));
+        float* post = reinterpret_cast<float*>(q16 + ROW);
+        __syncwarp();
+        for (int h = 0; h < H; ++h) {
+            // fp16 copy of q, pre-scaled per head by 2^sh so that the head's largest element lands in [2^14, 2^15)
+            const uint16_t* qh = a.sel_q + (int64_t)b * ROW + h * D_IDX;
+            float mx = 0.f;
+            for (int i = lane; i < D_IDX; i += 32) mx = fmaxf(mx, fabsf(bf16_bits_to_float(qh[i])));
 #pragma unroll
-    for (int ql = 0; ql < NQL; ++ql) {
-        int head = (4 * ql + 2 * (c & 1)) / GPH;
-        wq[ql] = w[(int64_t)b * H + head];
-        ps[ql] = post[head];
+            for (int o = 16; o; o >>= 1) mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, o));
+            int sh = 0;
+            if (mx > 0.f) sh = 14 - ilogbf(mx);
+            sh = max(-100, min(100, sh));
+            const float up = __uint_as_float((uint32_t)(127 + sh) << 23);
+            for (int i = lane; i < D_IDX; i += 32) q16[h * D_IDX + i] = __float2half_rn(bf16_bits_to_float(qh[i]) * up);
+            if (lane == 0) post[h] = __uint_as_float((uint32_t)(127 - sh) << 23);
+        }
+        __syncwarp();
+        // B fragments: column n of the MMA is the group held by quad-lane c == n; only lane (g == n, c == n) is non-zero
+#pragma unroll
+        for (int ql = 0; ql < NQL; ++ql) {
+            const uint4* src = reinterpret_cast<const uint4*>(q16 + (ql * 4 + c) * 32);
+#pragma unroll
+            for (int i = 0; i < 4; ++i) {
+                uint4 v = make_uint4(0, 0, 0, 0);
+                if (g == c) v = src[i];
+                qf[ql][4 * i + 0] = v.x; qf[ql][4 * i + 1] = v.y; qf[ql][4 * i + 2] = v.z; qf[ql][4 * i + 3] = v.w;
+            }
+        }
+        // lanes c < 2 read columns 2c, 2c+1 = groups 4ql + 2c (+1); their head, weight and power-of-two post-scale
+#pragma unroll
+        for (int ql = 0; ql < NQL; ++ql) {
+            const int head = (4 * ql + 2 * (c & 1)) / GPH;
+            wq[ql] = a.w[(int64_t)b * H + head];
+            ps[ql] = post[head];
+        }
+        __syncwarp();
     }
 
-    const uint8_t* kb = sel_k + (int64_t)b * tiles_per_seq * TILE_BYTES;
-    for (int tile = blockIdx.x * SCORE_WARPS + warp; tile < n_b; tile += gridDim.x * SCORE_WARPS) {
-        const uint8_t* tb = kb + (int64_t)tile * TILE_BYTES;
-        const int t0 = tile * 64;
-        // whole tile in flight: 16 x LDG.128 of codes per lane (8 KiB per warp) + the scale bytes
-        uint4 cd[4][NQL][2];
-#pragma unroll
-        for (int it = 0; it < 4; ++it)
-#pragma unroll
-            for (int ql = 0; ql < NQL; ++ql)
-#pragma unroll
-                for (int hf = 0; hf < 2; ++hf)
-                    cd[it][ql][hf] = ldg_stream_v4(tb + (it * 16 + hf * 8 + g) * CPT + ql * 64 + c * 16);
-        uint32_t scw[4][2][NG / 4];
-#pragma unroll
-        for (int it = 0; it < 4; ++it)
+    __device__ __forceinline__ float tile_max(uint32_t st, int t0, int L, int lane) const {
+        const int g = lane >> 2, c = lane & 3;
+        float m = -INFINITY;
+#pragma unroll 2
+        for (int it = 0; it < 4; ++it) {
+            uint4 cd[NQL][2];
+            uint32_t scw[2][NQL];
 #pragma unroll
             for (int hf = 0; hf < 2; ++hf) {
-                const uint32_t* sp = reinterpret_cast<const uint32_t*>(tb + 64 * CPT + (it * 16 + hf * 8 + g) * NG);
+                const int tok = it * 16 + hf * 8 + g;
 #pragma unroll
-                for (int i = 0; i < NG / 4; ++i) scw[it][hf][i] = __ldg(sp + i);
+                for (int ql = 0; ql < NQL; ++ql) {
+                    cd[ql][hf] = lds128(st + tok * CPT + ql * 64 + c * 16);
+                    scw[hf][ql] = lds32(st + 64 * CPT + tok * NG + ql * 4);
+                }
             }
-
-        float m = -INFINITY;
-#pragma unroll
-        for (int it = 0; it < 4; ++it) {
             float srow[2] = {0.f, 0.f};
 #pragma unroll
             for (int ql = 0; ql < NQL; ++ql) {
                 float acc[4] = {0.f, 0.f, 0.f, 0.f};
-                const uint32_t wa[4] = {cd[it][ql][0].x, cd[it][ql][0].y, cd[it][ql][0].z, cd[it][ql][0].w};
-                const uint32_t wb[4] = {cd[it][ql][1].x, cd[it][ql][1].y, cd[it][ql][1].z, cd[it][ql][1].w};
+                const uint32_t wa[4] = {cd[ql][0].x, cd[ql][0].y, cd[ql][0].z, cd[ql][0].w};
+                const uint32_t wb[4] = {cd[ql][1].x, cd[ql][1].y, cd[ql][1].z, cd[ql][1].w};
 #pragma unroll
                 for (int wd = 0; wd < 4; ++wd) {
                     uint32_t pa[4], pb[4];
@@ -252,10 +289,10 @@ __global__ void __launch_bounds__(SCORE_WARPS * 32) score_decode_q4_kernel(
                 // acc[0], acc[1]: row g, columns 2c, 2c+1; acc[2], acc[3]: row g + 8.  (lanes c >= 2: zeros)
 #pragma unroll
                 for (int hf = 0; hf < 2; ++hf) {
-                    const int gi = 4 * ql + 2 * (c & 1);               // first of this lane's two groups
-                    const uint32_t sw = scw[it][hf][ql];               // scale bytes of groups 4ql .. 4ql+3
-                    float s0 = scale_to_f32<FMT>((sw >> (8 * (gi & 3))) & 0xffu);
-                    float s1 = scale_to_f32<FMT>((sw >> (8 * ((gi & 3) + 1))) & 0xffu);
+                    const int gi = 2 * (c & 1);                        // first of this lane's two groups in the quad load
+                    const uint32_t sw = scw[hf][ql];                   // scale bytes of groups 4ql .. 4ql+3
+                    const float s0 = scale_to_f32<FMT>((sw >> (8 * gi)) & 0xffu);
+                    const float s1 = scale_to_f32<FMT>((sw >> (8 * (gi + 1))) & 0xffu);
                     float d = fmaf(acc[2 * hf], s0, acc[2 * hf + 1] * s1);
                     if (GPH == 4) d += __shfl_xor_sync(0xffffffffu, d, 1);   // the head's other two groups
                     d *= ps[ql];
@@ -265,8 +302,8 @@ __global__ void __launch_bounds__(SCORE_WARPS * 32) score_decode_q4_kernel(
                 }
             }
             // heads are split over quad lanes 0 and 1
-            float sa = srow[0] + __shfl_xor_sync(0xffffffffu, srow[0], 1);
-            float sb = srow[1] + __shfl_xor_sync(0xffffffffu, srow[1], 1);
+            const float sa = srow[0] + __shfl_xor_sync(0xffffffffu, srow[0], 1);
+            const float sb = srow[1] + __shfl_xor_sync(0xffffffffu, srow[1], 1);
             const int ta = t0 + it * 16 + g, tbk = ta + 8;
             if (ta < L) m = fmaxf(m, sa);
             if (tbk < L) m = fmaxf(m, sb);
@@ -275,35 +312,120 @@ __global__ void __launch_bounds__(SCORE_WARPS * 32) score_decode_q4_kernel(
         m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, 4));
         m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, 8));
         m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, 16));
-        if (lane == 0) scores[(int64_t)b * nb_stride + tile] = m;
+        return m;
     }
+};
+
+template <int H, int D_IDX, int FMT>
+__global__ void __launch_bounds__((ScoreCfg<H, D_IDX, FMT>::THREADS), 1) score_decode_kernel(const __grid_constant__ CUtensorMap tm_k,
+                                                                     const ScoreArgs a) {
+    using Cfg = ScoreCfg<H, D_IDX, FMT>;
+    constexpr int NS = Cfg::STAGES;
+    constexpr int SC_CONSUMERS = Cfg::CONSUMERS;
+    extern __shared__ unsigned char smem_raw[];
+    const uint32_t ring = (smem_u32(smem_raw) + 1023u) & ~1023u;
+    const uint32_t bar_full = ring + NS * Cfg::STAGE_BYTES;        // [NS]
+    const uint32_t bar_empty = bar_full + NS * 8;                  // [NS]
+    const uint32_t q16_base = bar_empty + NS * 8;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+
+    if (threadIdx.x == 0) {
+        for (int s = 0; s < NS; ++s) { mbar_init(bar_full + 8 * s, 1); mbar_init(bar_empty + 8 * s, 1); }
+        mbar_fence_init();
+        if (FMT == SPOT_SELK_BF16) tma_prefetch_desc(&tm_k);
+    }
+    __syncthreads();
+    pdl_wait();
+    pdl_launch_dependents();
+
+    // this CTA's range of the flat (sequence, tile) list
+    long long total = 0;
+    for (int bb = 0; bb < a.B; ++bb) total += (a.seq_len[bb] + 63) >> 6;
+    const long long i0 = (long long)blockIdx.x * total / gridDim.x, i1 = (long long)(blockIdx.x + 1) * total / gridDim.x;
+    const int n_my = (int)(i1 - i0);
+    if (n_my <= 0) return;
+    TileCursor cur;
+    cur.b = 0; cur.nb = (a.seq_len[0] + 63) >> 6; cur.t = 0;
+    {
+        long long rem = i0;                       // (64-bit while locating the start only)
+        while (rem >= cur.nb && cur.b + 1 < a.B) { rem -= cur.nb; ++cur.b; cur.nb = (a.seq_len[cur.b] + 63) >> 6; }
+        cur.t = (int)rem;
+    }
+
+    if (warp == SC_CONSUMERS) {
+        // ================================ producer ================================
+        if (lane == 0) {
+            for (int i = 0; i < n_my; ++i) {
+                const int s = i % NS;
+                mbar_wait(bar_empty + 8 * s, ((i / NS) & 1) ^ 1);
+                mbar_arrive_expect_tx(bar_full + 8 * s, Cfg::TILE_BYTES);
+                if (FMT == SPOT_SELK_BF16)
+                    tma_load_4d(ring + s * Cfg::STAGE_BYTES, &tm_k, bar_full + 8 * s, 0, cur.t * 64, 0, cur.b);
+                else
+                    bulk_load(ring + s * Cfg::STAGE_BYTES,
+                              a.sel_k + ((int64_t)cur.b * a.tiles_per_seq + cur.t) * Cfg::TILE_BYTES, Cfg::TILE_BYTES,
+                              bar_full + 8 * s);
+                cur.advance(a, 1);
+            }
+        }
+    } else {
+        // ================================ consumers ================================
+        typename std::conditional<FMT == SPOT_SELK_BF16, Bf16Tile<H, D_IDX>, Q4Tile<H, D_IDX, FMT>>::type tile;
+        cur.advance(a, warp);
+        int cur_b = -1, L = 0;
+        for (int i = warp; i < n_my; i += SC_CONSUMERS) {
+            if (cur.b != cur_b) {
+                cur_b = cur.b;
+                L = a.seq_len[cur_b];
+                tile.load_query(a, cur_b, lane, q16_base + warp * (Cfg::ROW * 2 + 64));
+            }
+            const int s = i % NS;
+            mbar_wait(bar_full + 8 * s, (i / NS) & 1);
+            const float m = tile.tile_max(ring + s * Cfg::STAGE_BYTES, cur.t * 64, L, lane);
+            __syncwarp();
+            if (lane == 0) {
+                mbar_arrive(bar_empty + 8 * s);
+                a.scores[(int64_t)cur_b * a.nb_stride + cur.t] = m;
+            }
+            cur.advance(a, SC_CONSUMERS);
+        }
+    }
+}
+
+template <int H, int D_IDX, int FMT>
+spot_status launch_score_fmt(const spot_select_params* p, float* scores, int nb_stride, cudaStream_t s) {
+    using Cfg = ScoreCfg<H, D_IDX, FMT>;
+    ScoreArgs a;
+    a.sel_q = p->sel_q; a.w = p->w; a.sel_k = (const uint8_t*)p->sel_k; a.tiles_per_seq = p->cache_stride_tokens / 64;
+    a.seq_len = p->seq_len; a.B = p->B; a.scores = scores; a.nb_stride = nb_stride;
+    CUtensorMap tm;
+    memset(&tm, 0, sizeof(tm));
+    if (FMT == SPOT_SELK_BF16) {
+        constexpr int NP = H * D_IDX / 64;
+        const uint64_t row_bytes = (uint64_t)H * D_IDX * 2;
+        const uint64_t dims[4] = {64, (uint64_t)p->cache_stride_tokens, (uint64_t)NP, (uint64_t)p->B};
+        const uint64_t strides[3] = {row_bytes, 128, (uint64_t)p->cache_stride_tokens * row_bytes};
+        const uint32_t box[4] = {64, 64, (uint32_t)NP, 1};
+        if (!encode_tmap_bf16_sw128(&tm, p->sel_k, 4, dims, strides, box)) return SPOT_ERR_CUDA;
+    }
+    static bool attr_set = false;
+    if (!attr_set) {
+        SPOT_CUDA_TRY(cudaFuncSetAttribute(score_decode_kernel<H, D_IDX, FMT>,
+                                           cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg::SMEM_BYTES));
+        attr_set = true;
+    }
+    const int64_t max_tiles = (int64_t)p->B * ((p->max_seq_len + 63) / 64);
+    const int grid = (int)(max_tiles < sm_count() ? max_tiles : sm_count());
+    SPOT_CUDA_TRY(launch_pdl(score_decode_kernel<H, D_IDX, FMT>, dim3((unsigned)grid), dim3(Cfg::THREADS),
+                             (size_t)Cfg::SMEM_BYTES, s, tm, a));
+    return SPOT_OK;
 }
 
 template <int H, int D_IDX>
 spot_status launch_score(const spot_select_params* p, float* scores, int nb_stride, cudaStream_t s) {
-    // every warp gets the same number of 64-token tiles: with T tiles per sequence and room for `cap_warps` warps
-    // per sequence (4 CTAs per SM in all), tiles per warp = ceil(T / cap_warps) and just enough warps for that.
-    // (A grid-stride loop over a fixed 4 CTAs/SM grid left 3.46 tiles per warp at L = 128K, B = 4: a quarter of the
-    // warps ran a 4th tile while the others idled -- profiles/r1_decode_cfg3_launches.md.)
-    const int n_b_max = (p->max_seq_len + 63) / 64;
-    const int cap_warps = max(1, (sm_count() * 4 * SCORE_WARPS) / p->B);
-    const int tiles_per_warp = (n_b_max + cap_warps - 1) / cap_warps;
-    const int warps = (n_b_max + tiles_per_warp - 1) / tiles_per_warp;
-    dim3 grid((unsigned)((warps + SCORE_WARPS - 1) / SCORE_WARPS), (unsigned)p->B);
-    const dim3 block(SCORE_WARPS * 32);
-    if (p->fmt == SPOT_SELK_BF16) {
-        SPOT_CUDA_TRY(launch_pdl(score_decode_bf16_kernel<H, D_IDX>, grid, block, 0, s, p->sel_q, p->w,
-                                 (const uint16_t*)p->sel_k, p->cache_stride_tokens, p->seq_len, scores, nb_stride));
-    } else if (p->fmt == SPOT_SELK_MXFP4) {
-        SPOT_CUDA_TRY(launch_pdl(score_decode_q4_kernel<H, D_IDX, SPOT_SELK_MXFP4>, grid, block, 0, s, p->sel_q, p->w,
-                                 (const uint8_t*)p->sel_k, p->cache_stride_tokens / 64, p->seq_len, scores, nb_stride));
-    } else {
-        SPOT_CUDA_TRY(launch_pdl(score_decode_q4_kernel<H, D_IDX, SPOT_SELK_INT4_E4M3>, grid, block, 0, s, p->sel_q,
-                                 p->w, (const uint8_t*)p->sel_k, p->cache_stride_tokens / 64, p->seq_len, scores,
-                                 nb_stride));
-    }
-    SPOT_LAUNCH_CHECK();
-    return SPOT_OK;
+    if (p->fmt == SPOT_SELK_BF16) return launch_score_fmt<H, D_IDX, SPOT_SELK_BF16>(p, scores, nb_stride, s);
+    if (p->fmt == SPOT_SELK_MXFP4) return launch_score_fmt<H, D_IDX, SPOT_SELK_MXFP4>(p, scores, nb_stride, s);
+    return launch_score_fmt<H, D_IDX, SPOT_SELK_INT4_E4M3>(p, scores, nb_stride, s);
 }
 
 }  // namespace
