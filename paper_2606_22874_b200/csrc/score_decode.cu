@@ -106,18 +106,23 @@ template <int H, int D_IDX, int FMT>
 struct ScoreCfg {
     static constexpr int ROW = H * D_IDX;                      // elements per token
     static constexpr int TILE_BYTES = FMT == SPOT_SELK_BF16 ? 64 * ROW * 2 : 64 * (ROW / 2 + ROW / 32);
-    static constexpr int STAGE_BYTES = (TILE_BYTES + 1023) / 1024 * 1024;
+    static constexpr bool SELF = FMT != SPOT_SELK_BF16;
+    // BF16 (producer ring): few big tiles (32 / 64 KiB, 1024-byte aligned for the 128-byte swizzle) and a light
+    // ldmatrix + HMMA body.  One producer lane feeds the ring; every stage belongs to ONE consumer warp (stage s ->
+    // warp s % CONSUMERS, CONSUMERS == STAGES), so a warp meets the phases of a stage's barrier strictly in order --
+    // with stages shared in rotation a warp could wait for phase k+1 of a barrier whose phase k (another warp's tile)
+    // has not completed yet, and a parity wait cannot tell those apart.
+    // 4-bit (self-serve ring): many small tiles (8.5 / 17 KiB) and an ALU-heavy unpack.  A single producer lane cannot
+    // issue a copy per ~350 cycles, so every consumer warp owns PER_WARP stages and refills a stage itself as soon as
+    // it has consumed it: no producer warp, no empty barriers.
+    static constexpr int STAGE_BYTES = SELF ? TILE_BYTES : (TILE_BYTES + 1023) / 1024 * 1024;
     static constexpr int STAGES_RAW = SC_SMEM_BUDGET / STAGE_BYTES;
-    // Every ring stage belongs to ONE consumer warp (stage s -> warp s % CONSUMERS), so a warp meets the phases of a
-    // stage's barrier strictly in order; with stages shared in rotation a warp could wait for phase k+1 of a barrier
-    // whose phase k (another warp's tile) has not completed yet, and a parity wait cannot tell those apart.
-    // BF16: few big tiles and a light ldmatrix + HMMA body -> as many consumers as stages (6 or 3).
-    // 4-bit: many small tiles and an ALU-heavy unpack -> 8 consumers, 16 or 8 stages.
-    static constexpr int CONSUMERS = FMT == SPOT_SELK_BF16 ? (STAGES_RAW > 6 ? 6 : STAGES_RAW) : 8;
-    static constexpr int STAGES = FMT == SPOT_SELK_BF16 ? CONSUMERS : (STAGES_RAW >= 16 ? 16 : 8);
-    static constexpr int THREADS = (CONSUMERS + 1) * 32;
-    static_assert(STAGES % CONSUMERS == 0 && STAGES * STAGE_BYTES <= SC_SMEM_BUDGET, "ring geometry");
-    static constexpr int Q16_BYTES = FMT == SPOT_SELK_BF16 ? 0 : CONSUMERS * (ROW * 2 + 64);
+    static constexpr int CONSUMERS = SELF ? (TILE_BYTES <= 8704 ? 8 : 6) : (STAGES_RAW > 6 ? 6 : STAGES_RAW);
+    static constexpr int PER_WARP = SELF ? (TILE_BYTES <= 8704 ? 3 : 2) : 1;
+    static constexpr int STAGES = CONSUMERS * PER_WARP;
+    static constexpr int THREADS = (CONSUMERS + (SELF ? 0 : 1)) * 32;
+    static_assert(STAGES * STAGE_BYTES <= 208 * 1024, "ring geometry");
+    static constexpr int Q16_BYTES = SELF ? CONSUMERS * (ROW * 2 + 64) : 0;
     static constexpr int SMEM_BYTES = 1024 + STAGES * STAGE_BYTES + 2 * STAGES * 8 + Q16_BYTES + 64;
 };
 
@@ -219,21 +224,33 @@ struct Q4Tile {
         const int g = lane >> 2, c = lane & 3;
         __half* q16 = reinterpret_cast<__half*>(__cvta_shared_to_generic((size_t)q16_addr));
         float* post = reinterpret_cast<float*>(q16 + ROW);
+        // fp16 copy of q, pre-scaled per head by 2^sh so that the head's largest element lands in [2^14, 2^15).
+        // One coalesced read of the whole query: lane l holds elements [EPL l, EPL l + EPL), 32 / H lanes per head.
+        constexpr int EPL = ROW / 32, LPH = 32 / H;
+        static_assert(EPL % 8 == 0 && LPH * EPL == D_IDX && (LPH & (LPH - 1)) == 0, "query staging geometry");
         __syncwarp();
-        for (int h = 0; h < H; ++h) {
-            // fp16 copy of q, pre-scaled per head by 2^sh so that the head's largest element lands in [2^14, 2^15)
-            const uint16_t* qh = a.sel_q + (int64_t)b * ROW + h * D_IDX;
-            float mx = 0.f;
-            for (int i = lane; i < D_IDX; i += 32) mx = fmaxf(mx, fabsf(bf16_bits_to_float(qh[i])));
+        uint4 raw[EPL / 8];
 #pragma unroll
-            for (int o = 16; o; o >>= 1) mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, o));
-            int sh = 0;
-            if (mx > 0.f) sh = 14 - ilogbf(mx);
-            sh = max(-100, min(100, sh));
-            const float up = __uint_as_float((uint32_t)(127 + sh) << 23);
-            for (int i = lane; i < D_IDX; i += 32) q16[h * D_IDX + i] = __float2half_rn(bf16_bits_to_float(qh[i]) * up);
-            if (lane == 0) post[h] = __uint_as_float((uint32_t)(127 - sh) << 23);
+        for (int i = 0; i < EPL / 8; ++i)
+            raw[i] = *reinterpret_cast<const uint4*>(a.sel_q + (int64_t)b * ROW + lane * EPL + i * 8);
+        float v[EPL], mx = 0.f;
+#pragma unroll
+        for (int i = 0; i < EPL / 8; ++i) {
+            const uint32_t wds[4] = {raw[i].x, raw[i].y, raw[i].z, raw[i].w};
+#pragma unroll
+            for (int j = 0; j < 4; ++j) { v[i * 8 + 2 * j] = bf16lo(wds[j]); v[i * 8 + 2 * j + 1] = bf16hi(wds[j]); }
         }
+#pragma unroll
+        for (int i = 0; i < EPL; ++i) mx = fmaxf(mx, fabsf(v[i]));
+#pragma unroll
+        for (int o = LPH / 2; o; o >>= 1) mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, o));
+        int sh = 0;
+        if (mx > 0.f) sh = 14 - ilogbf(mx);
+        sh = max(-100, min(100, sh));
+        const float up = __uint_as_float((uint32_t)(127 + sh) << 23);
+#pragma unroll
+        for (int i = 0; i < EPL; ++i) q16[lane * EPL + i] = __float2half_rn(v[i] * up);
+        if (lane % LPH == 0) post[lane / LPH] = __uint_as_float((uint32_t)(127 - sh) << 23);
         __syncwarp();
         // B fragments: column n of the MMA is the group held by quad-lane c == n; only lane (g == n, c == n) is non-zero
 #pragma unroll
@@ -352,7 +369,47 @@ __global__ void __launch_bounds__((ScoreCfg<H, D_IDX, FMT>::THREADS), 1) score_d
         cur.t = (int)rem;
     }
 
-    if (warp == SC_CONSUMERS) {
+    if constexpr (Cfg::SELF) {
+        // ================================ self-serve consumers (4-bit) ================================
+        // warp w streams tiles w, w + C, w + 2C, ... through its own stages w*K .. w*K + K-1
+        constexpr int K = Cfg::PER_WARP;
+        Q4Tile<H, D_IDX, FMT> tile;
+        cur.advance(a, warp);
+        TileCursor nxt = cur;                      // the next tile to request
+        auto request = [&](int j) {                // j-th tile of this warp -> stage w*K + j % K   (lane 0 only)
+            const uint32_t s = warp * K + j % K;
+            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // earlier generic reads of the stage
+            mbar_arrive_expect_tx(bar_full + 8 * s, Cfg::TILE_BYTES);
+            bulk_load(ring + s * Cfg::STAGE_BYTES,
+                      a.sel_k + ((int64_t)nxt.b * a.tiles_per_seq + nxt.t) * Cfg::TILE_BYTES, Cfg::TILE_BYTES,
+                      bar_full + 8 * s);
+        };
+        const int n_w = (n_my - warp + SC_CONSUMERS - 1) / SC_CONSUMERS;     // tiles of this warp
+#pragma unroll
+        for (int j = 0; j < K; ++j)
+            if (j < n_w) {
+                if (lane == 0) request(j);
+                nxt.advance(a, SC_CONSUMERS);
+            }
+        int cur_b = -1, L = 0;
+        for (int j = 0; j < n_w; ++j) {
+            if (cur.b != cur_b) {
+                cur_b = cur.b;
+                L = a.seq_len[cur_b];
+                tile.load_query(a, cur_b, lane, q16_base + warp * (Cfg::ROW * 2 + 64));
+            }
+            const uint32_t s = warp * K + j % K;
+            mbar_wait(bar_full + 8 * s, (j / K) & 1);
+            const float m = tile.tile_max(ring + s * Cfg::STAGE_BYTES, cur.t * 64, L, lane);
+            __syncwarp();
+            if (j + K < n_w) {
+                if (lane == 0) request(j + K);
+                nxt.advance(a, SC_CONSUMERS);
+            }
+            if (lane == 0) a.scores[(int64_t)cur_b * a.nb_stride + cur.t] = m;
+            cur.advance(a, SC_CONSUMERS);
+        }
+    } else if (warp == SC_CONSUMERS) {
         // ================================ producer ================================
         if (lane == 0) {
             for (int i = 0; i < n_my; ++i) {
@@ -370,7 +427,7 @@ __global__ void __launch_bounds__((ScoreCfg<H, D_IDX, FMT>::THREADS), 1) score_d
         }
     } else {
         // ================================ consumers ================================
-        typename std::conditional<FMT == SPOT_SELK_BF16, Bf16Tile<H, D_IDX>, Q4Tile<H, D_IDX, FMT>>::type tile;
+        Bf16Tile<H, D_IDX> tile;
         cur.advance(a, warp);
         int cur_b = -1, L = 0;
         for (int i = warp; i < n_my; i += SC_CONSUMERS) {
