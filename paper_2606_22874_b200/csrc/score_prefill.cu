@@ -4,16 +4,20 @@
 // This IS a dense contraction (4 heads x [Tq x 64] x [64 x L_visible]), so it runs on the 5th-gen tensor cores:
 //   * work item = (128-query tile = two query blocks, chunk of up to CHUNK key blocks); items are dealt round-robin
 //     to one persistent CTA per SM;
-//   * warp 8 lane 0: TMA producer -- the query tile ([4 heads][128][64] BF16, 64 KiB, double-buffered) and a 3-stage
-//     ring of key blocks ([4][64][64], 32 KiB) land in 128-byte-swizzled shared memory through 4-D tensor maps;
-//   * warp 9 lane 0: issues tcgen05.mma (M = 128, N = 64, K = 16; 4 k-steps x 4 heads per key block) into one of two
-//     TMEM accumulator stages (4 heads x 64 fp32 columns = 256 columns each);
-//   * warps 0-7: epilogue.  Warp w reads TMEM lanes 32 (w & 3) .. +31 (one query per lane) and columns
-//     32 (w >> 2) .. +31 of every head with tcgen05.ld, forms sum_h w_h ReLU(d_h) in fp32 and keeps a running max; the
-//     tile maximum is a REDUX.MAX over an order-preserving integer key plus one shared-memory atomicMax per warp.
-// The epilogue, not the MMA, is the near-co-bound (9 lane-ops per (query, key) pair against 512 tensor flops), so
-// ReLU is split between the two fp32 pipes: heads 0-1 use (w/2)(d + |d|) (FADD with an abs modifier, FMA pipe), heads
-// 2-3 use w max(d, 0) (ALU pipe); both forms give bit-identical products.  The weighted sum uses packed FFMA2.
+//   * warp 8 lane 0: TMA producer -- the query tile ([4 heads][128][64] BF16, 64 KiB) and a 2-stage ring of key-block
+//     PAIRS ([4 heads][128 keys][64], 64 KiB) land in 128-byte-swizzled shared memory through 4-D tensor maps;
+//   * warp 9 lane 0: issues tcgen05.mma with M = 128 queries, N = 128 keys (two key blocks), K = 16: four k-steps per
+//     head into a 128-column TMEM accumulator.  N = 64 made every MMA read 6 KiB of operands for 16 cycles of math
+//     (384 B/clk) and the tensor pipe sat at 65 % busy for 37 % of peak (profiles/r1_prefill_cfg5.md); N = 128 halves
+//     the A-operand re-reads per flop.  The 512 TMEM columns are a ring of FOUR accumulators, one per (pair, head):
+//     the issuer runs up to three heads ahead of the epilogue;
+//   * warps 0-7: epilogue.  Warp w owns TMEM lanes 32 (w & 3) .. +31 (one query per lane) and the 64 columns of key
+//     block (w >> 2) of the pair.  Head by head it reads the accumulator (tcgen05.ld), releases it, and adds
+//     w_h ReLU(d_h) to a 64-register running sum; after the fourth head the tile maximum is a REDUX.MAX over an
+//     order-preserving integer key plus one shared-memory atomicMax per warp.
+// The epilogue is the near-co-bound (9 lane-ops per (query, key) pair against 512 tensor flops), so ReLU is split
+// between the two fp32 pipes: heads 0-1 use (w/2)(d + |d|) (FADD with an abs modifier, FMA pipe), heads 2-3 use
+// w max(d, 0) (ALU pipe); both forms give bit-identical products.  The weighted sum uses packed FFMA2.
 #include "common.cuh"
 #include "tc100.cuh"
 
@@ -24,14 +28,15 @@ namespace {
 constexpr int PF_H = 4;                 // selector heads
 constexpr int PF_D = 64;                // d_idx (one 128-byte swizzle row)
 constexpr int PF_M = 128;               // queries per tile (two 64-query blocks)
-constexpr int PF_N = 64;                // keys per block
+constexpr int PF_N = 128;               // keys per MMA (two 64-key blocks)
 constexpr int PF_CHUNK = 32;            // key blocks per work item
-constexpr int PF_KSTAGES = 3;
+constexpr int PF_KSTAGES = 2;
+constexpr int PF_TSTAGES = 4;           // TMEM accumulators (128 columns each)
 constexpr int PF_EPI_WARPS = 8;
 constexpr int PF_THREADS = (PF_EPI_WARPS + 2) * 32;
 constexpr uint32_t Q_TILE_BYTES = PF_H * PF_M * PF_D * 2;   // 65536
-constexpr uint32_t K_TILE_BYTES = PF_H * PF_N * PF_D * 2;   // 32768
-constexpr uint32_t PF_SMEM_TILES = 2 * Q_TILE_BYTES + PF_KSTAGES * K_TILE_BYTES;
+constexpr uint32_t K_TILE_BYTES = PF_H * PF_N * PF_D * 2;   // 65536
+constexpr uint32_t PF_SMEM_TILES = Q_TILE_BYTES + PF_KSTAGES * K_TILE_BYTES;
 constexpr uint32_t PF_SMEM_MISC = 1024;
 constexpr uint32_t PF_SMEM_BYTES = 1024 + PF_SMEM_TILES + PF_SMEM_MISC;   // 1024: manual alignment slack
 
@@ -72,32 +77,32 @@ __global__ void __launch_bounds__(PF_THREADS, 1) score_prefill_kernel(const __gr
     extern __shared__ unsigned char smem_raw[];
     const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
     unsigned char* smem = smem_raw + (smem_base - smem_u32(smem_raw));
-    const uint32_t q_smem = smem_base;                               // 2 x 64 KiB
-    const uint32_t k_smem = smem_base + 2 * Q_TILE_BYTES;            // 3 x 32 KiB
+    const uint32_t q_smem = smem_base;                               // 64 KiB
+    const uint32_t k_smem = smem_base + Q_TILE_BYTES;                // 2 x 64 KiB
     unsigned char* misc = smem + PF_SMEM_TILES;
     const uint32_t misc_u32 = smem_base + PF_SMEM_TILES;
     // barriers (8 bytes each)
-    const uint32_t bar_q_full = misc_u32 + 0;      // [2]
-    const uint32_t bar_q_empty = misc_u32 + 16;    // [2]
-    const uint32_t bar_k_full = misc_u32 + 32;     // [3]
-    const uint32_t bar_k_empty = misc_u32 + 56;    // [3]
-    const uint32_t bar_t_full = misc_u32 + 80;     // [2]
-    const uint32_t bar_t_empty = misc_u32 + 96;    // [2]
+    const uint32_t bar_q_full = misc_u32 + 0;
+    const uint32_t bar_q_empty = misc_u32 + 8;
+    const uint32_t bar_k_full = misc_u32 + 16;     // [2]
+    const uint32_t bar_k_empty = misc_u32 + 32;    // [2]
+    const uint32_t bar_t_full = misc_u32 + 48;     // [4]
+    const uint32_t bar_t_empty = misc_u32 + 80;    // [4]
     uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(misc + 112);
     uint32_t* s_max = reinterpret_cast<uint32_t*>(misc + 128);       // [2 item buffers][CHUNK][2 query blocks]
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
 
     if (threadIdx.x == 0) {
-        for (int i = 0; i < 2; ++i) {
-            mbar_init(bar_q_full + 8 * i, 1);
-            mbar_init(bar_q_empty + 8 * i, 1);
-            mbar_init(bar_t_full + 8 * i, 1);
-            mbar_init(bar_t_empty + 8 * i, PF_EPI_WARPS);
-        }
+        mbar_init(bar_q_full, 1);
+        mbar_init(bar_q_empty, 1);
         for (int i = 0; i < PF_KSTAGES; ++i) {
             mbar_init(bar_k_full + 8 * i, 1);
             mbar_init(bar_k_empty + 8 * i, 1);
+        }
+        for (int i = 0; i < PF_TSTAGES; ++i) {
+            mbar_init(bar_t_full + 8 * i, 1);
+            mbar_init(bar_t_empty + 8 * i, PF_EPI_WARPS);
         }
         mbar_fence_init();
     }
@@ -111,23 +116,26 @@ __global__ void __launch_bounds__(PF_THREADS, 1) score_prefill_kernel(const __gr
     __syncthreads();
     tc_fence_after();
     const uint32_t tbase = *tmem_slot;
+    pdl_wait();
+    pdl_launch_dependents();
 
     if (warp == PF_EPI_WARPS) {
         // ================================ TMA producer ================================
         if (lane == 0) {
-            int n_item = 0, kt = 0;
+            int n_item = 0, kp = 0;
             for (int id = blockIdx.x; id < a.total_ids; id += gridDim.x) {
                 int b, c, m, nk;
                 if (!decode_item(a, id, b, c, m, nk)) continue;
-                const int qb = n_item & 1;
-                mbar_wait(bar_q_empty + 8 * qb, ((n_item >> 1) & 1) ^ 1);
-                mbar_arrive_expect_tx(bar_q_full + 8 * qb, Q_TILE_BYTES);
-                tma_load_4d(q_smem + qb * Q_TILE_BYTES, &tm_q, bar_q_full + 8 * qb, 0, m * PF_M, 0, b);
-                for (int kb = 0; kb < nk; ++kb, ++kt) {
-                    const int s = kt % PF_KSTAGES;
-                    mbar_wait(bar_k_empty + 8 * s, ((kt / PF_KSTAGES) & 1) ^ 1);
+                mbar_wait(bar_q_empty, (n_item & 1) ^ 1);
+                mbar_arrive_expect_tx(bar_q_full, Q_TILE_BYTES);
+                tma_load_4d(q_smem, &tm_q, bar_q_full, 0, m * PF_M, 0, b);
+                const int np = (nk + 1) >> 1;
+                for (int pr = 0; pr < np; ++pr, ++kp) {
+                    const int s = kp % PF_KSTAGES;
+                    mbar_wait(bar_k_empty + 8 * s, ((kp / PF_KSTAGES) & 1) ^ 1);
                     mbar_arrive_expect_tx(bar_k_full + 8 * s, K_TILE_BYTES);
-                    tma_load_4d(k_smem + s * K_TILE_BYTES, &tm_k, bar_k_full + 8 * s, 0, (c * PF_CHUNK + kb) * PF_N, 0, b);
+                    // a pair that overhangs the cache is zero-filled by TMA; its second block is never used
+                    tma_load_4d(k_smem + s * K_TILE_BYTES, &tm_k, bar_k_full + 8 * s, 0, (c * PF_CHUNK + 2 * pr) * 64, 0, b);
                 }
                 ++n_item;
             }
@@ -136,32 +144,32 @@ __global__ void __launch_bounds__(PF_THREADS, 1) score_prefill_kernel(const __gr
         // ================================ MMA issuer ================================
         if (lane == 0) {
             constexpr uint32_t idesc = umma_idesc_bf16(PF_M, PF_N);
-            int n_item = 0, kt = 0;
+            int n_item = 0, kp = 0, acc = 0;
             for (int id = blockIdx.x; id < a.total_ids; id += gridDim.x) {
                 int b, c, m, nk;
                 if (!decode_item(a, id, b, c, m, nk)) continue;
-                const int qb = n_item & 1;
-                mbar_wait(bar_q_full + 8 * qb, (n_item >> 1) & 1);
-                const uint32_t qa = q_smem + qb * Q_TILE_BYTES;
-                for (int kb = 0; kb < nk; ++kb, ++kt) {
-                    const int s = kt % PF_KSTAGES, as = kt & 1;
-                    mbar_wait(bar_k_full + 8 * s, (kt / PF_KSTAGES) & 1);
-                    mbar_wait(bar_t_empty + 8 * as, ((kt >> 1) & 1) ^ 1);
-                    tc_fence_after();
+                mbar_wait(bar_q_full, n_item & 1);
+                const int np = (nk + 1) >> 1;
+                for (int pr = 0; pr < np; ++pr, ++kp) {
+                    const int s = kp % PF_KSTAGES;
+                    mbar_wait(bar_k_full + 8 * s, (kp / PF_KSTAGES) & 1);
                     const uint32_t ka = k_smem + s * K_TILE_BYTES;
 #pragma unroll
-                    for (int h = 0; h < PF_H; ++h) {
+                    for (int h = 0; h < PF_H; ++h, ++acc) {
+                        const int ts = acc % PF_TSTAGES;
+                        mbar_wait(bar_t_empty + 8 * ts, ((acc / PF_TSTAGES) & 1) ^ 1);
+                        tc_fence_after();
 #pragma unroll
                         for (int kk = 0; kk < PF_D / 16; ++kk) {
-                            const uint64_t ad = umma_desc_sw128(qa + h * (PF_M * PF_D * 2) + kk * 32);
+                            const uint64_t ad = umma_desc_sw128(q_smem + h * (PF_M * PF_D * 2) + kk * 32);
                             const uint64_t bd = umma_desc_sw128(ka + h * (PF_N * PF_D * 2) + kk * 32);
-                            umma_bf16_ss(tbase + as * 256 + h * PF_N, ad, bd, idesc, kk > 0);
+                            umma_bf16_ss(tbase + ts * PF_N, ad, bd, idesc, kk > 0);
                         }
+                        umma_commit(bar_t_full + 8 * ts);      // this head's accumulator is ready for the epilogue
                     }
-                    umma_commit(bar_k_empty + 8 * s);      // smem slot free once these MMAs have read it
-                    umma_commit(bar_t_full + 8 * as);      // accumulators ready for the epilogue
+                    umma_commit(bar_k_empty + 8 * s);          // smem slot free once these MMAs have read it
                 }
-                umma_commit(bar_q_empty + 8 * qb);
+                umma_commit(bar_q_empty);
                 ++n_item;
             }
         }
@@ -170,8 +178,8 @@ __global__ void __launch_bounds__(PF_THREADS, 1) score_prefill_kernel(const __gr
         const int lq = warp & 3, ch = warp >> 2;
         const int row = lq * 32 + lane;           // query row of the tile = TMEM lane
         const int qbl = lq >> 1;                  // which of the tile's two query blocks
-        const uint32_t t_lane = tbase + ((uint32_t)(lq * 32) << 16) + ch * 32;
-        int n_item = 0, kt = 0;
+        const uint32_t t_lane = tbase + ((uint32_t)(lq * 32) << 16) + ch * 64;
+        int n_item = 0, acc = 0;
         for (int id = blockIdx.x; id < a.total_ids; id += gridDim.x) {
             int b, c, m, nk;
             if (!decode_item(a, id, b, c, m, nk)) continue;
@@ -183,47 +191,50 @@ __global__ void __launch_bounds__(PF_THREADS, 1) score_prefill_kernel(const __gr
             const float wh0 = 0.5f * wv.x, wh1 = 0.5f * wv.y;   // heads 0-1: (w/2)(d + |d|)
             const int qb_abs = a.qb_start + 2 * m + qbl;        // this row's (absolute) query block = its diagonal
             const int q_in_blk = row & 63;
-            for (int kb = 0; kb < nk; ++kb, ++kt) {
-                const int as = kt & 1;
-                const int j = c * PF_CHUNK + kb;
-                mbar_wait(bar_t_full + 8 * as, (kt >> 1) & 1);
-                tc_fence_after();
-                const uint32_t ta = t_lane + as * 256;
-                float mx = -INFINITY;
-                const bool diag = (j == qb_abs);
+            const int np = (nk + 1) >> 1;
+            for (int pr = 0; pr < np; ++pr) {
+                float S[64];
 #pragma unroll
-                for (int half = 0; half < 2; ++half) {
-                    float d0[16], d1[16], d2[16], d3[16];
-                    tmem_ld16(ta + 0 * PF_N + half * 16, d0);
-                    tmem_ld16(ta + 1 * PF_N + half * 16, d1);
-                    tmem_ld16(ta + 2 * PF_N + half * 16, d2);
-                    tmem_ld16(ta + 3 * PF_N + half * 16, d3);
+                for (int h = 0; h < PF_H; ++h, ++acc) {
+                    const int ts = acc % PF_TSTAGES;
+                    mbar_wait(bar_t_full + 8 * ts, (acc / PF_TSTAGES) & 1);
+                    tc_fence_after();
+                    float d[4][16];
+#pragma unroll
+                    for (int q4 = 0; q4 < 4; ++q4) tmem_ld16(t_lane + ts * PF_N + q4 * 16, d[q4]);
                     tmem_ld_wait();
-                    if (half == 1) {
-                        tc_fence_before();
-                        __syncwarp();
-                        if (lane == 0) mbar_arrive(bar_t_empty + 8 * as);
-                    }
-                    float sv[16];
+                    tc_fence_before();
+                    __syncwarp();
+                    if (lane == 0) mbar_arrive(bar_t_empty + 8 * ts);
 #pragma unroll
-                    for (int i = 0; i < 16; i += 2) {
-                        float s0 = wh0 * (d0[i] + fabsf(d0[i]));
-                        float s1 = wh0 * (d0[i + 1] + fabsf(d0[i + 1]));
-                        ffma2(s0, s1, d1[i] + fabsf(d1[i]), d1[i + 1] + fabsf(d1[i + 1]), wh1, s0, s1);
-                        ffma2(s0, s1, fmaxf(d2[i], 0.f), fmaxf(d2[i + 1], 0.f), wv.z, s0, s1);
-                        ffma2(s0, s1, fmaxf(d3[i], 0.f), fmaxf(d3[i + 1], 0.f), wv.w, s0, s1);
-                        sv[i] = s0; sv[i + 1] = s1;
-                    }
-                    if (diag) {
-                        // causal mask inside the diagonal tile: key t of the block is visible iff t <= q
+                    for (int q4 = 0; q4 < 4; ++q4)
 #pragma unroll
-                        for (int i = 0; i < 16; ++i)
-                            if (ch * 32 + half * 16 + i > q_in_blk) sv[i] = -INFINITY;
-                    }
-#pragma unroll
-                    for (int i = 0; i < 16; i += 2) mx = fmax3(mx, sv[i], sv[i + 1]);
+                        for (int i = 0; i < 16; i += 2) {
+                            float& s0 = S[q4 * 16 + i];
+                            float& s1 = S[q4 * 16 + i + 1];
+                            const float d0 = d[q4][i], d1 = d[q4][i + 1];
+                            if (h == 0) {
+                                s0 = wh0 * (d0 + fabsf(d0));
+                                s1 = wh0 * (d1 + fabsf(d1));
+                            } else if (h == 1) {
+                                ffma2(s0, s1, d0 + fabsf(d0), d1 + fabsf(d1), wh1, s0, s1);
+                            } else {
+                                ffma2(s0, s1, fmaxf(d0, 0.f), fmaxf(d1, 0.f), h == 2 ? wv.z : wv.w, s0, s1);
+                            }
+                        }
                 }
-                if (j <= qb_abs && q_exists) {        // warp-uniform: Tq is a multiple of 64, a warp's rows share a block
+                const int kb = 2 * pr + ch;                     // this warp's key block of the pair
+                const int j = c * PF_CHUNK + kb;
+                if (j == qb_abs) {
+                    // causal mask inside the diagonal tile: key t of the block is visible iff t <= q
+#pragma unroll
+                    for (int i = 0; i < 64; ++i)
+                        if (i > q_in_blk) S[i] = -INFINITY;
+                }
+                float mx = -INFINITY;
+#pragma unroll
+                for (int i = 0; i < 64; i += 2) mx = fmax3(mx, S[i], S[i + 1]);
+                if (kb < nk && j <= qb_abs && q_exists) {   // warp-uniform: Tq is a multiple of 64, a warp's rows share a block
                     const uint32_t key = __reduce_max_sync(0xffffffffu, f32_order_key(mx));
                     if (lane == 0) atomicMax(&s_max[(ib * PF_CHUNK + kb) * 2 + qbl], key);
                 }
@@ -302,7 +313,7 @@ spot_status score_prefill(const spot_select_params* p, float* scores, int nb_str
     {
         const uint64_t dims[4] = {(uint64_t)PF_D, (uint64_t)p->cache_stride_tokens, (uint64_t)PF_H, (uint64_t)p->B};
         const uint64_t strides[3] = {row_bytes, (uint64_t)PF_D * 2, (uint64_t)p->cache_stride_tokens * row_bytes};
-        const uint32_t box[4] = {(uint32_t)PF_D, (uint32_t)PF_N, (uint32_t)PF_H, 1u};
+        const uint32_t box[4] = {(uint32_t)PF_D, (uint32_t)PF_N, (uint32_t)PF_H, 1u};   // a pair of key blocks
         if (!encode_tmap_bf16_sw128(&tm_k, p->sel_k, 4, dims, strides, box)) return SPOT_ERR_CUDA;
     }
     static bool attr_set = false;
@@ -312,8 +323,8 @@ spot_status score_prefill(const spot_select_params* p, float* scores, int nb_str
         attr_set = true;
     }
     const int grid = (int)(total < sm_count() ? total : sm_count());
-    score_prefill_kernel<<<grid, PF_THREADS, PF_SMEM_BYTES, s>>>(tm_q, tm_k, a);
-    SPOT_LAUNCH_CHECK();
+    SPOT_CUDA_TRY(launch_pdl(score_prefill_kernel, dim3((unsigned)grid), dim3(PF_THREADS), (size_t)PF_SMEM_BYTES, s, tm_q,
+                             tm_k, a));
     return SPOT_OK;
 }
 
