@@ -135,6 +135,28 @@ def run_reference(args):
     print(json.dumps(line))
 
 
+def rank_workload(name, rank):
+    """Every rank runs the same-shaped batch of independent sequences with its own seed (rank 0: the config's seed):
+    the path shards by sequence, weak scaling, no data-path collective."""
+    if rank == 0:
+        return build_workload(name, {})
+    from workloads import CONFIGS, make_decode_workload
+    kw = dict(CONFIGS[name])
+    kw["seed"] = kw["seed"] + 1000 * rank
+    return make_decode_workload(name, with_kv=False, **kw)
+
+
+def max_over_ranks(value, device, world):
+    """The step time the contract reports: the slowest rank's."""
+    if world <= 1:
+        return float(value)
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([float(value)], device=device, dtype=torch.float64)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
 # ------------------------------------------------------------------------------------------------------
 def run_ours(args):
     import ctypes as C
@@ -152,13 +174,7 @@ def run_ours(args):
     B.build()
     _lib.load()                                   # no fallback: raises if the CUDA library is missing
 
-    # every rank runs the same-shaped batch of independent sequences (its own seed): weak scaling, no collective
-    wl = build_workload(args.workload, {})
-    if rank:
-        from workloads import CONFIGS, make_decode_workload
-        kw = dict(CONFIGS[args.workload])
-        kw["seed"] = kw["seed"] + 1000 * rank
-        wl = make_decode_workload(args.workload, with_kv=False, **kw)
+    wl = rank_workload(args.workload, rank)
     dev = torch.device("cuda", local_rank)
     Bn, L, Hq, Hkv, D = wl.B, wl.L_cap, wl.H_q, wl.H_kv, wl.D
     gen = torch.Generator(device=dev)
@@ -278,12 +294,7 @@ def run_ours(args):
             e2e.append((time.perf_counter() - t0) * 1e3)
     bud_host = h_bud.numpy().copy()
 
-    step_mean = float(step_ms.mean())
-    if world > 1:
-        import torch.distributed as dist
-        t = torch.tensor([step_mean], device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        step_mean = float(t.item())
+    step_mean = max_over_ranks(step_ms.mean(), dev, world)
     if rank != 0:
         return
 
@@ -527,12 +538,7 @@ def run_prefill(args):
         if i >= 1:
             e2e.append((time.perf_counter() - t0) * 1e3)
 
-    step_mean = float(step_ms.mean())
-    if world > 1:
-        import torch.distributed as dist
-        t = torch.tensor([step_mean], device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        step_mean = float(t.item())
+    step_mean = max_over_ranks(step_ms.mean(), dev, world)
     if rank != 0:
         return
     burst, sustained, peak_src = tensor_peaks()
