@@ -14,6 +14,7 @@ namespace spot {
 
 namespace {
 
+constexpr bool PA_USE_TCGEN05 = true;           // attn_prefill_tc.cu; the mma.sync kernel below is the first form
 constexpr int PA_WARPS = 8;
 constexpr int PA_ROWS = PA_WARPS * 16;          // 128 rows per CTA
 constexpr int PA_STAGES = 3;
@@ -232,6 +233,8 @@ spot_status check_prefill(const spot_attn_params* p) {
 
 }  // namespace spot
 
+namespace spot { spot_status attn_prefill_tc(const spot_attn_params* p, cudaStream_t stream); }
+
 using namespace spot;
 
 extern "C" size_t spot_sparse_attn_prefill_workspace_bytes(const spot_attn_params* p) {
@@ -243,6 +246,7 @@ extern "C" spot_status spot_sparse_attn_prefill(const spot_attn_params* p, void*
     spot_status st = check_prefill(p);
     if (st != SPOT_OK) return st;
     if ((st = check_device()) != SPOT_OK) return st;
+    if (PA_USE_TCGEN05) return attn_prefill_tc(p, (cudaStream_t)stream);
     PrefillAttnArgs a;
     a.q = p->q; a.k = p->k; a.v = p->v;
     a.sb = p->kv_stride_batch; a.st = p->kv_stride_token; a.sh = p->kv_stride_head;

@@ -1,0 +1,339 @@
+// Step a3' on the 5th-generation tensor cores -- block-sparse causal GQA flash attention for chunked prefill
+// (Fig. 2): every 64-token query block attends to its own list of selected 64-token key
+// blocks; only the diagonal block needs a token-level mask.
+//
+// Tensor-bound.  Work item = (sequence, query block, KV head, PAIR of 128-row tiles); rows stack the group's query
+// heads: row = head_in_group * 64 + query, so one K/V tile in shared memory feeds every head of the group.
+//   warp 0 lane 0 : TMA producer.  Q (two [2 d-halves][128 rows][64] tiles) once, then a 3-stage ring of K_j and V_j
+//                   ([2 d-halves][64 keys][64], 16 KiB each, 128-byte swizzle) through rank-5 tensor maps built from
+//                   the caller's element strides.
+//   warp 1 lane 0 : tcgen05.mma issuer.  S_t = Q_t K_j^T (M=128, N=64, 8 k-steps, both operands K-major) into TMEM;
+//                   O_t += P_t V_j (M=128, N=128, 4 k-steps) with P_t K-major from shared memory and V_j used as an
+//                   MN-major B operand exactly as TMA wrote it (no transpose).  The two tiles ping-pong: while the
+//                   softmax warps of one tile work, the tensor pipe runs the other tile's MMAs:
+//                       PV0(n)  QK0(n+1)  |  PV1(n)  QK1(n+1)  | ...
+//   warps 4-7, 8-11: softmax of tile 0 / tile 1, one thread per row (TMEM lane = row).  tcgen05.ld of the 64 logits,
+//                   log2-domain online softmax with a LAZY rescale of the TMEM-resident O (only when a row's max
+//                   grows by more than 2^8 since the last rescale: P stays <= 256, l and O use the same stale max, so
+//                   the result is exact), P rounded to BF16 into 128-byte-swizzled shared memory, fence.proxy.async,
+//                   mbarrier hand-off.  Epilogue: O / l -> BF16, 256 B per row, optional LSE.
+// TMEM: S_0 | S_1 | O_0 | O_1 = 64 + 64 + 128 + 128 columns.
+#include "common.cuh"
+#include "tc100.cuh"
+
+namespace spot {
+
+namespace {
+
+constexpr int TA_STAGES = 3;
+constexpr int TA_THREADS = 12 * 32;
+constexpr uint32_t TA_Q_TILE = 2 * 128 * 128;          // 32 KiB: [2 halves][128 rows][128 B]
+constexpr uint32_t TA_KV_TILE = 2 * 64 * 128;          // 16 KiB: [2 halves][64 keys][128 B]
+constexpr uint32_t TA_P_TILE = 128 * 128;              // 16 KiB: [128 rows][64 keys] BF16
+constexpr uint32_t TA_SMEM_TILES = 2 * TA_Q_TILE + TA_STAGES * 2 * TA_KV_TILE + 2 * TA_P_TILE;   // 192 KiB
+constexpr uint32_t TA_SMEM_BYTES = 1024 + TA_SMEM_TILES + 256;
+constexpr float TA_RESCALE_THRESHOLD = 8.0f;           // log2 units
+
+struct TcAttnArgs {
+    const int32_t* indices;      // [B * n_qb][cap]; nullptr: every causally visible block
+    const int32_t* budgets;
+    int cap;
+    int Tq, n_qb, H_q, H_kv, G;
+    int qb_start;                // q_start / 64
+    float scale_log2;
+    uint16_t* out;               // [B][Tq][H_q][128]
+    float* lse;                  // optional [B][Tq][H_q]
+};
+
+__global__ void __launch_bounds__(TA_THREADS, 1) attn_prefill_tc_kernel(const __grid_constant__ CUtensorMap tm_q,
+                                                                        const __grid_constant__ CUtensorMap tm_k,
+                                                                        const __grid_constant__ CUtensorMap tm_v,
+                                                                        const TcAttnArgs a) {
+    extern __shared__ unsigned char smem_raw[];
+    const uint32_t base = (smem_u32(smem_raw) + 1023u) & ~1023u;
+    unsigned char* smem = smem_raw + (base - smem_u32(smem_raw));
+    const uint32_t q_smem = base;                                        // 2 x 32 KiB
+    const uint32_t kv_smem = base + 2 * TA_Q_TILE;                       // stages x (K 16 KiB, V 16 KiB)
+    const uint32_t p_smem = kv_smem + TA_STAGES * 2 * TA_KV_TILE;        // 2 x 16 KiB
+    const uint32_t misc = base + TA_SMEM_TILES;
+    const uint32_t bar_q_full = misc;
+    const uint32_t bar_k_full = misc + 8;                // [3]
+    const uint32_t bar_v_full = misc + 32;               // [3]
+    const uint32_t bar_kv_empty = misc + 56;             // [3]
+    const uint32_t bar_s_full = misc + 80;               // [2]
+    const uint32_t bar_p_full = misc + 96;               // [2]
+    const uint32_t bar_o_done = misc + 112;              // [2]
+    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(smem + TA_SMEM_TILES + 128);
+
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int pair = blockIdx.x, hk = blockIdx.y;
+    const int rowz = (int)gridDim.z - 1 - (int)blockIdx.z;               // heaviest (latest) query blocks first
+    const int b = rowz / a.n_qb, i = rowz - b * a.n_qb;
+    const int G = a.G;
+    const int qb_abs = a.qb_start + i;
+    const bool two = (2 * pair + 1) * 2 < G;                             // does the pair's second tile have live rows?
+
+    if (threadIdx.x == 0) {
+        mbar_init(bar_q_full, 1);
+        for (int s = 0; s < TA_STAGES; ++s) {
+            mbar_init(bar_k_full + 8 * s, 1);
+            mbar_init(bar_v_full + 8 * s, 1);
+            mbar_init(bar_kv_empty + 8 * s, 1);
+        }
+        for (int t = 0; t < 2; ++t) {
+            mbar_init(bar_s_full + 8 * t, 1);
+            mbar_init(bar_p_full + 8 * t, 128);
+            mbar_init(bar_o_done + 8 * t, 1);
+        }
+        mbar_fence_init();
+        tma_prefetch_desc(&tm_q);
+        tma_prefetch_desc(&tm_k);
+        tma_prefetch_desc(&tm_v);
+    }
+    if (warp == 2) tmem_alloc(misc + 128, 512);
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+    const uint32_t tbase = *tmem_slot;
+    pdl_wait();
+    pdl_launch_dependents();
+
+    const int budget = a.indices ? max(0, min(a.budgets[rowz], a.cap)) : qb_abs + 1;
+    const int32_t* idx = a.indices ? a.indices + (int64_t)rowz * a.cap : nullptr;
+    auto block_of = [&](int it) -> int { return idx ? idx[it] : it; };
+    auto visible = [&](int j) -> bool { return j >= 0 && j <= qb_abs; };
+
+    if (warp == 0) {
+        // ================================ TMA producer ================================
+        if (lane == 0) {
+            mbar_arrive_expect_tx(bar_q_full, two ? 2 * TA_Q_TILE : TA_Q_TILE);
+            for (int t = 0; t < (two ? 2 : 1); ++t)
+                tma_load_5d(q_smem + t * TA_Q_TILE, &tm_q, bar_q_full, 0, i * 64, hk * G + (2 * pair + t) * 2, 0, b);
+            int n = 0;
+            for (int it = 0; it < budget; ++it) {
+                const int j = block_of(it);
+                if (!visible(j)) continue;
+                const int s = n % TA_STAGES;
+                mbar_wait(bar_kv_empty + 8 * s, ((n / TA_STAGES) & 1) ^ 1);
+                const uint32_t ks = kv_smem + s * 2 * TA_KV_TILE;
+                mbar_arrive_expect_tx(bar_k_full + 8 * s, TA_KV_TILE);
+                tma_load_5d(ks, &tm_k, bar_k_full + 8 * s, 0, j * 64, 0, hk, b);
+                mbar_arrive_expect_tx(bar_v_full + 8 * s, TA_KV_TILE);
+                tma_load_5d(ks + TA_KV_TILE, &tm_v, bar_v_full + 8 * s, 0, j * 64, 0, hk, b);
+                ++n;
+            }
+        }
+    } else if (warp == 1) {
+        // ================================ MMA issuer ================================
+        if (lane == 0) {
+            constexpr uint32_t idesc_qk = umma_idesc_bf16(128, 64);
+            constexpr uint32_t idesc_pv = umma_idesc_bf16(128, 128) | UMMA_B_MN_MAJOR;
+            int nv = 0;
+            for (int it = 0; it < budget; ++it) nv += visible(block_of(it)) ? 1 : 0;
+            const int nt = two ? 2 : 1;
+            auto qk = [&](int t, uint32_t ks) {           // S_t = Q_t K^T
+#pragma unroll
+                for (int kk = 0; kk < 8; ++kk) {
+                    const uint64_t ad = umma_desc_sw128(q_smem + t * TA_Q_TILE + (kk >> 2) * (128 * 128) + (kk & 3) * 32);
+                    const uint64_t bd = umma_desc_sw128(ks + (kk >> 2) * (64 * 128) + (kk & 3) * 32);
+                    umma_bf16_ss(tbase + t * 64, ad, bd, idesc_qk, kk > 0);
+                }
+                umma_commit(bar_s_full + 8 * t);
+            };
+            auto pv = [&](int t, uint32_t vs, bool acc) { // O_t += P_t V
+#pragma unroll
+                for (int kk = 0; kk < 4; ++kk) {
+                    const uint64_t ad = umma_desc_sw128(p_smem + t * TA_P_TILE + kk * 32);
+                    const uint64_t bd = umma_desc_sw128_mn(vs + kk * 2048, 64 * 128, 1024);
+                    umma_bf16_ss(tbase + 128 + t * 128, ad, bd, idesc_pv, acc || kk > 0);
+                }
+                umma_commit(bar_o_done + 8 * t);
+            };
+            if (nv > 0) {
+                mbar_wait(bar_q_full, 0);
+                mbar_wait(bar_k_full, 0);
+                tc_fence_after();
+                for (int t = 0; t < nt; ++t) qk(t, kv_smem);
+                for (int n = 0; n < nv; ++n) {
+                    const int s = n % TA_STAGES, s1 = (n + 1) % TA_STAGES;
+                    const uint32_t vs = kv_smem + s * 2 * TA_KV_TILE + TA_KV_TILE;
+                    const uint32_t ks1 = kv_smem + s1 * 2 * TA_KV_TILE;
+                    mbar_wait(bar_v_full + 8 * s, (n / TA_STAGES) & 1);
+                    if (n + 1 < nv) mbar_wait(bar_k_full + 8 * s1, ((n + 1) / TA_STAGES) & 1);
+                    for (int t = 0; t < nt; ++t) {
+                        mbar_wait(bar_p_full + 8 * t, n & 1);          // P_t(n) written, S_t consumed, O_t rescaled
+                        tc_fence_after();
+                        pv(t, vs, n > 0);
+                        if (n + 1 < nv) qk(t, ks1);
+                    }
+                    umma_commit(bar_kv_empty + 8 * s);                  // K(n), V(n) no longer read
+                }
+            }
+        }
+    } else if (warp >= 4) {
+        // ================================ softmax + epilogue ================================
+        const int t = (warp - 4) >> 2;                    // tile of the pair
+        const int lq = warp & 3;                          // TMEM lane quarter this warp may access
+        if (t == 0 || two) {
+            const int r = lq * 32 + lane;                 // row of the tile = TMEM lane
+            const int hg = (2 * pair + t) * 2 + (r >> 6); // head in group
+            const int ql = r & 63;                        // query in block
+            const bool live = hg < G;
+            const uint32_t t_s = tbase + ((uint32_t)(lq * 32) << 16) + t * 64;
+            const uint32_t t_o = tbase + ((uint32_t)(lq * 32) << 16) + 128 + t * 128;
+            const uint32_t p_row = p_smem + t * TA_P_TILE + r * 128;
+            float m_used = -INFINITY, l = 0.f;
+            int n = 0;
+            for (int it = 0; it < budget; ++it) {
+                const int j = block_of(it);
+                if (!visible(j)) continue;
+                mbar_wait(bar_s_full + 8 * t, n & 1);
+                tc_fence_after();
+                float x[64];
+                {
+                    float d0[16], d1[16], d2[16], d3[16];
+                    tmem_ld16(t_s, d0); tmem_ld16(t_s + 16, d1); tmem_ld16(t_s + 32, d2); tmem_ld16(t_s + 48, d3);
+                    tmem_ld_wait();
+#pragma unroll
+                    for (int e = 0; e < 16; ++e) { x[e] = d0[e]; x[16 + e] = d1[e]; x[32 + e] = d2[e]; x[48 + e] = d3[e]; }
+                }
+                const bool diag = (j == qb_abs);
+                float mx = -INFINITY;
+#pragma unroll
+                for (int e = 0; e < 64; ++e) {
+                    x[e] = (diag && e > ql) ? -INFINITY : x[e] * a.scale_log2;
+                    mx = fmaxf(mx, x[e]);
+                }
+                // lazy rescale: keep the stale max unless the row max grew by more than 2^8 (warp-uniform decision,
+                // tcgen05.ld/st are warp-collective)
+                const bool need = mx > m_used + TA_RESCALE_THRESHOLD;
+                if (__any_sync(0xffffffffu, need)) {
+                    const float m_new = need ? mx : m_used;
+                    const float alpha = (m_used == -INFINITY) ? 0.f : fast_exp2(m_used - m_new);   // 1 when !need
+                    l *= alpha;
+                    m_used = m_new;
+                    if (n > 0) {
+                        mbar_wait(bar_o_done + 8 * t, (n - 1) & 1);          // PV(n-1) has landed in O_t
+                        tc_fence_after();
+#pragma unroll
+                        for (int cb = 0; cb < 8; ++cb) {
+                            float o[16];
+                            tmem_ld16(t_o + cb * 16, o);
+                            tmem_ld_wait();
+#pragma unroll
+                            for (int e = 0; e < 16; ++e) o[e] *= alpha;
+                            tmem_st16(t_o + cb * 16, o);
+                        }
+                        tmem_st_wait();
+                    }
+                }
+                float ps = 0.f;
+                uint32_t pk[32];
+#pragma unroll
+                for (int e = 0; e < 64; e += 2) {
+                    const float p0 = fast_exp2(x[e] - m_used), p1 = fast_exp2(x[e + 1] - m_used);
+                    ps += p0 + p1;
+                    pk[e >> 1] = pack_bf16x2(p0, p1);
+                }
+                l += ps;
+                if (n > 0) mbar_wait(bar_o_done + 8 * t, (n - 1) & 1);       // PV(n-1) no longer reads P_t
+#pragma unroll
+                for (int c = 0; c < 8; ++c) {
+                    asm volatile("st.shared.v4.u32 [%0], {%1,%2,%3,%4};" :: "r"(p_row + (((uint32_t)c ^ (r & 7)) << 4)),
+                                 "r"(pk[4 * c]), "r"(pk[4 * c + 1]), "r"(pk[4 * c + 2]), "r"(pk[4 * c + 3]) : "memory");
+                }
+                fence_proxy_async_smem();
+                tc_fence_before();
+                mbar_arrive(bar_p_full + 8 * t);
+                ++n;
+            }
+            // epilogue: O / l -> BF16
+            const int q_row = i * 64 + ql;
+            const int h = hk * G + hg;
+            uint16_t* orow = a.out + (((int64_t)b * a.Tq + q_row) * a.H_q + h) * 128;
+            if (n > 0) {
+                mbar_wait(bar_o_done + 8 * t, (n - 1) & 1);
+                tc_fence_after();
+            }
+            const float inv = l > 0.f ? 1.f / l : 0.f;
+#pragma unroll
+            for (int cb = 0; cb < 8; ++cb) {
+                float o[16];
+                if (n > 0) {
+                    tmem_ld16(t_o + cb * 16, o);
+                    tmem_ld_wait();
+                } else {
+#pragma unroll
+                    for (int e = 0; e < 16; ++e) o[e] = 0.f;
+                }
+                if (live) {
+                    uint4 v0, v1;
+                    v0.x = pack_bf16x2(o[0] * inv, o[1] * inv);   v0.y = pack_bf16x2(o[2] * inv, o[3] * inv);
+                    v0.z = pack_bf16x2(o[4] * inv, o[5] * inv);   v0.w = pack_bf16x2(o[6] * inv, o[7] * inv);
+                    v1.x = pack_bf16x2(o[8] * inv, o[9] * inv);   v1.y = pack_bf16x2(o[10] * inv, o[11] * inv);
+                    v1.z = pack_bf16x2(o[12] * inv, o[13] * inv); v1.w = pack_bf16x2(o[14] * inv, o[15] * inv);
+                    *reinterpret_cast<uint4*>(orow + cb * 16) = v0;
+                    *reinterpret_cast<uint4*>(orow + cb * 16 + 8) = v1;
+                }
+            }
+            if (a.lse && live)
+                a.lse[((int64_t)b * a.Tq + q_row) * a.H_q + h] =
+                    l > 0.f ? (m_used + log2f(l)) * 0.6931471805599453f : -INFINITY;
+        }
+    }
+
+    tc_fence_before();
+    __syncthreads();
+    if (warp == 2) tmem_dealloc(tbase, 512);
+}
+
+// rank-5 map of a [..][rows][..][128] BF16 tensor as (64 d, rows, 2 d-halves, dim3, dim4): a box of R rows lands in
+// shared memory as [2 halves][R][128 B] (K-major 128-byte-swizzled operand tiles).
+bool make_map(CUtensorMap* m, const void* base, uint64_t rows, uint64_t row_stride_elems, uint64_t n3,
+              uint64_t stride3_elems, uint64_t n4, uint64_t stride4_elems, uint32_t box_rows, uint32_t box3) {
+    const uint64_t dims[5] = {64, rows, 2, n3, n4};
+    const uint64_t strides[4] = {row_stride_elems * 2, 128, stride3_elems * 2, stride4_elems * 2};
+    const uint32_t box[5] = {64, box_rows, 2, box3, 1};
+    return encode_tmap_bf16_sw128(m, base, 5, dims, strides, box);
+}
+
+}  // namespace
+
+// Q [B][Tq][H_q][128]; K/V with element strides; see attn_prefill.cu for the argument checks (already done).
+spot_status attn_prefill_tc(const spot_attn_params* p, cudaStream_t stream) {
+    TcAttnArgs a;
+    a.indices = p->indices; a.budgets = p->budgets; a.cap = p->cap;
+    a.Tq = p->Tq; a.n_qb = p->Tq / 64; a.H_q = p->H_q; a.H_kv = p->H_kv; a.G = p->H_q / p->H_kv;
+    a.qb_start = p->q_start / 64;
+    a.scale_log2 = p->sm_scale * 1.4426950408889634f;
+    a.out = p->out; a.lse = p->lse;
+    CUtensorMap tm_q, tm_k, tm_v;
+    // Q as (64 d, query, head, d-half, batch): a box of 64 queries x 2 heads x 2 halves lands as
+    // [half][head][query][128 B] = [half][128 rows][128 B], row = head * 64 + query.
+    {
+        const uint64_t dims[5] = {64, (uint64_t)p->Tq, (uint64_t)p->H_q, 2, (uint64_t)p->B};
+        const uint64_t strides[4] = {(uint64_t)p->H_q * 128 * 2, 128 * 2, 128, (uint64_t)p->Tq * p->H_q * 128 * 2};
+        const uint32_t box[5] = {64, 64, 2, 2, 1};       // -> [half][head][query][128 B] = [half][128 rows][128 B]
+        if (!encode_tmap_bf16_sw128(&tm_q, p->q, 5, dims, strides, box)) return SPOT_ERR_CUDA;
+    }
+    const uint64_t n_tok = (uint64_t)p->q_start + p->Tq;
+    if (!make_map(&tm_k, p->k, n_tok, (uint64_t)p->kv_stride_token, (uint64_t)p->H_kv, (uint64_t)p->kv_stride_head,
+                  (uint64_t)p->B, (uint64_t)p->kv_stride_batch, 64, 1))
+        return SPOT_ERR_CUDA;
+    if (!make_map(&tm_v, p->v, n_tok, (uint64_t)p->kv_stride_token, (uint64_t)p->H_kv, (uint64_t)p->kv_stride_head,
+                  (uint64_t)p->B, (uint64_t)p->kv_stride_batch, 64, 1))
+        return SPOT_ERR_CUDA;
+    static bool attr_set = false;
+    if (!attr_set) {
+        SPOT_CUDA_TRY(cudaFuncSetAttribute(attn_prefill_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                           (int)TA_SMEM_BYTES));
+        attr_set = true;
+    }
+    const int n_mt = (a.G * 64 + 127) / 128;
+    dim3 grid((unsigned)((n_mt + 1) / 2), (unsigned)p->H_kv, (unsigned)(p->B * a.n_qb));
+    SPOT_CUDA_TRY(launch_pdl(attn_prefill_tc_kernel, grid, dim3(TA_THREADS), (size_t)TA_SMEM_BYTES, stream, tm_q, tm_k,
+                             tm_v, a));
+    return SPOT_OK;
+}
+
+}  // namespace spot
