@@ -163,3 +163,64 @@ def test_end_to_end_step_matches_oracle(torch_cuda):
         want, _ = H.oracle_attend(wl, b, sel.indices)
         err = np.abs(out[b] - want)
         assert err.max() <= MAX_ABS and err.mean() <= MEAN_ABS
+
+
+@pytest.mark.parametrize("fmt,seqs", [("bf16", (0, 3)), ("mxfp4", (1,))])
+def test_full_size_cfg3_in_the_bench_configuration(torch_cuda, fmt, seqs):
+    """BASELINE.json config 3 at full size (B=4, L=131072, 2048 blocks per sequence), launched exactly as bench.py
+    launches it (scores in the workspace, cap = n_b, K/V [B][H_kv][L][D] drawn on the device).  Sampled outputs the
+    oracle can compute one by one: the whole selection of the sampled sequences (scores, index list, budget), and
+    the attention output of every head of those sequences over the oracle's list (the oracle is run on the gathered
+    selected blocks -- attention is a sum over the selected tokens, so gathering them first changes nothing)."""
+    torch = torch_cuda
+    from oracle import attention as OA
+    from paper_2606_22874_b200 import api
+    wl = make_config("cfg3", with_kv=False)
+    dd = H.DeviceDecode(wl, fmt, with_kv=False)
+    idx, bud, scores, probs = dd.select()
+    assert bud.min() >= 8 and bud.max() <= dd.n_b_max
+    dev = torch.device("cuda")
+    gen = torch.Generator(device=dev)
+    gen.manual_seed(wl.seed + 17)
+    B, L, Hkv, D, Hq = wl.B, wl.L_cap, wl.H_kv, wl.D, wl.H_q
+    K = torch.randn((B, Hkv, L, D), generator=gen, device=dev, dtype=torch.bfloat16)
+    V = torch.randn((B, Hkv, L, D), generator=gen, device=dev, dtype=torch.bfloat16)
+    q = H.dev_u16(wl.q)
+    out = torch.zeros((B, Hq, D), dtype=torch.int16, device=dev)
+    lse = torch.zeros((B, Hq), device=dev)
+    # attention runs over the ORACLE's lists for the sampled sequences (north_star: "computed on the same selected set")
+    idx_use, bud_use = idx.copy(), bud.copy()
+    sels = {}
+    for b in seqs:
+        s_bar, sel = H.oracle_select(wl, fmt, b)
+        np.testing.assert_allclose(scores[b, :len(s_bar)], s_bar, rtol=2e-5, atol=2e-5)
+        cls = H.classify_selection(s_bar, sel, idx[b], int(bud[b]), wl.p)
+        assert not cls.startswith("FAIL"), "seq %d: %s" % (b, cls)
+        print("cfg3 %s seq %d: selection %s, budget %d" % (fmt, b, cls, sel.budget))
+        if cls == "exact":
+            assert np.abs(probs[b, :len(s_bar)] - sel.probs).max() <= PROB_ABS
+        idx_use[b] = -1
+        idx_use[b, :sel.budget] = sel.indices
+        bud_use[b] = sel.budget
+        sels[b] = sel
+    d_idx = torch.from_numpy(idx_use).to(dev)
+    d_bud = torch.from_numpy(bud_use).to(dev)
+    ap = api.make_attn_params(q, K, V, (Hkv * L * D, D, L * D), dd.seq_len, L, d_idx, d_bud, idx.shape[1], B, 1, Hq, Hkv,
+                              D, blk=wl.blk, sm_scale=wl.sm_scale, out=out, lse=lse)
+    ws = torch.empty(max(16, api.spot_sparse_attn_decode_workspace_bytes(ap)), dtype=torch.uint8, device=dev)
+    ap.workspace, ap.workspace_bytes = ws.data_ptr(), ws.numel()
+    api.spot_sparse_attn_decode(ap)
+    torch.cuda.synchronize()
+    got = H.bf16_bits_to_f64(H.to_np_u16(out))
+    for b in seqs:
+        blocks = torch.from_numpy(sels[b].indices.astype(np.int64)).to(dev)
+        n = len(blocks)
+        Kg = K[b].view(Hkv, L // 64, 64, D)[:, blocks].reshape(Hkv, n * 64, D)
+        Vg = V[b].view(Hkv, L // 64, 64, D)[:, blocks].reshape(Hkv, n * 64, D)
+        Kh = H.bf16_bits_to_f64(H.to_np_u16(Kg.contiguous().view(torch.int16))).transpose(1, 0, 2)
+        Vh = H.bf16_bits_to_f64(H.to_np_u16(Vg.contiguous().view(torch.int16))).transpose(1, 0, 2)
+        want, want_lse = OA.sparse_attn_decode(H.bf16_bits_to_f64(wl.q[b]), Kh, Vh, np.arange(n), n * 64, 64, wl.sm_scale)
+        err = np.abs(got[b] - want)
+        assert err.max() <= MAX_ABS and err.mean() <= MEAN_ABS, (b, err.max(), err.mean())
+        assert np.abs(lse[b].cpu().numpy() - want_lse).max() <= 2e-3
+        print("cfg3 %s seq %d: attention over %d blocks, max-abs %.2e mean-abs %.2e" % (fmt, b, n, err.max(), err.mean()))

@@ -165,3 +165,58 @@ def test_prefill_attention_argument_errors(torch_cuda):
         with pytest.raises(api.SpotError) as e:
             api.spot_sparse_attn_prefill(params(**bad))
         assert "INVALID_ARG" in str(e.value)
+
+
+def test_full_size_cfg5_in_the_bench_configuration(torch_cuda):
+    """BASELINE.json config 5 at full size (L=65536, whole prompt as one chunk), launched as bench.py launches it.
+    Sampled outputs the oracle can compute one by one: the selection rows of a few query blocks (first, middle, last)
+    and their attention outputs over the oracle's lists.  For attention the oracle runs on the gathered selected
+    blocks with the query block re-based onto the last of them (all other selected blocks are fully visible, so the
+    causal structure is unchanged)."""
+    torch = torch_cuda
+    from oracle import attention as OA
+    from paper_2606_22874_b200 import api
+    L = 65536
+    wl = make_prefill_workload(seed=5005, L=L, with_kv=False)
+    dp = H.DevicePrefill([wl], 0, L, with_kv=False)
+    idx, bud, scores, probs = dp.select(want_probs=False)
+    sample = [0, 1, 511, 1023]
+    sels = {}
+    for i in sample:
+        (s_bar, sel), = H.oracle_select_prefill(wl, i * 64, 64)
+        np.testing.assert_allclose(scores[i, :len(s_bar)], s_bar, rtol=2e-5, atol=2e-5)
+        cls = H.classify_selection(s_bar, sel, idx[i], int(bud[i]), wl.p)
+        assert not cls.startswith("FAIL"), "query block %d: %s" % (i, cls)
+        print("cfg5 query block %d: selection %s, budget %d of %d" % (i, cls, sel.budget, i + 1))
+        idx[i] = -1
+        idx[i, :sel.budget] = sel.indices
+        bud[i] = sel.budget
+        sels[i] = sel
+    dev = torch.device("cuda")
+    gen = torch.Generator(device=dev)
+    gen.manual_seed(wl.seed + 17)
+    Hq, Hkv, D = wl.H_q, wl.H_kv, wl.D
+    Q = torch.randn((1, L, Hq, D), generator=gen, device=dev, dtype=torch.bfloat16)
+    K = torch.randn((1, Hkv, L, D), generator=gen, device=dev, dtype=torch.bfloat16)
+    V = torch.randn((1, Hkv, L, D), generator=gen, device=dev, dtype=torch.bfloat16)
+    out = torch.zeros((1, L, Hq, D), dtype=torch.int16, device=dev)
+    d_idx, d_bud = torch.from_numpy(idx).to(dev), torch.from_numpy(bud).to(dev)
+    ap = api.make_attn_params(Q, K, V, (Hkv * L * D, D, L * D), None, 0, d_idx, d_bud, idx.shape[1], 1, L, Hq, Hkv, D,
+                              q_start=0, blk=64, sm_scale=wl.sm_scale, out=out)
+    api.spot_sparse_attn_prefill(ap)
+    torch.cuda.synchronize()
+    for i in sample:
+        blocks = sels[i].indices.astype(np.int64)
+        assert blocks[-1] == i                                   # the diagonal block is reserved (recency tier)
+        n = len(blocks)
+        bl = torch.from_numpy(blocks).to(dev)
+        Kg = K[0].view(Hkv, L // 64, 64, D)[:, bl].reshape(Hkv, n * 64, D)
+        Vg = V[0].view(Hkv, L // 64, 64, D)[:, bl].reshape(Hkv, n * 64, D)
+        Kh = H.bf16_bits_to_f64(H.to_np_u16(Kg.contiguous().view(torch.int16))).transpose(1, 0, 2)
+        Vh = H.bf16_bits_to_f64(H.to_np_u16(Vg.contiguous().view(torch.int16))).transpose(1, 0, 2)
+        Qh = H.bf16_bits_to_f64(H.to_np_u16(Q[0, i * 64:(i + 1) * 64].contiguous().view(torch.int16)))
+        want = OA.sparse_attn_prefill(Qh, Kh, Vh, [list(range(n))], (n - 1) * 64, 64, 64, wl.sm_scale)
+        got = H.bf16_bits_to_f64(H.to_np_u16(out[0, i * 64:(i + 1) * 64]))
+        err = np.abs(got - want)
+        assert err.max() <= MAX_ABS and err.mean() <= MEAN_ABS, (i, err.max(), err.mean())
+        print("cfg5 query block %d: attention over %d blocks, max-abs %.2e mean-abs %.2e" % (i, n, err.max(), err.mean()))
