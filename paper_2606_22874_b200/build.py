@@ -11,7 +11,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libspot.so")
-SOURCES = ["api.cu", "quantize.cu", "score_decode.cu", "select.cu", "attn_decode.cu", "score_prefill.cu",
+SOURCES = ["api.cu", "quantize.cu", "score_decode.cu", "select.cu", "select_hist.cu", "attn_decode.cu", "score_prefill.cu",
            "attn_prefill.cu", "attn_prefill_tc.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "--expt-relaxed-constexpr"]

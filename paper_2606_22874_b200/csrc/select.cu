@@ -14,41 +14,11 @@
 //   * the cut is a key value tau = key of rank n_take-1; blocks with a better key are selected, blocks tied with tau
 //     are taken in ascending block index until n_take is reached -- exactly the (score descending, index
 //     ascending) order R7 fixes -- and the ascending index list falls out of one ballot/popc scan in index order.
-#include "common.cuh"
+#include "select_common.cuh"
 
 namespace spot {
 
 namespace {
-
-constexpr int SEL_MAX_NB = 8192;
-constexpr uint32_t KEY_PAD = 0xffffffffu;
-
-__device__ __forceinline__ uint32_t orderable(float x) {
-    uint32_t u = __float_as_uint(x + 0.0f);   // -0.0 -> +0.0
-    return (u & 0x80000000u) ? ~u : (u | 0x80000000u);
-}
-__device__ __forceinline__ float from_orderable(uint32_t o) {
-    uint32_t u = (o & 0x80000000u) ? (o & 0x7fffffffu) : ~o;
-    return __uint_as_float(u);
-}
-// sort key: ascending key == descending score
-__device__ __forceinline__ uint32_t score_key(float s) { return ~orderable(s); }
-__device__ __forceinline__ float key_score(uint32_t k) { return from_orderable(~k); }
-
-struct SelectArgs {
-    const float* scores;      // [rows][nb_stride]
-    int nb_stride;
-    const int32_t* seq_len;   // decode: [B]; prefill: nullptr
-    int n_q;                  // rows per sequence
-    int q_start, q_block, blk;
-    int mode, top_k;
-    double p, temperature;
-    int sink, rec, kmin;
-    int32_t* indices;
-    int cap;
-    int32_t* budgets;
-    float* probs;             // optional [rows][nb_stride]
-};
 
 __device__ __forceinline__ void cmpx(uint32_t& a, uint32_t& b, bool asc) {
     const uint32_t lo = min(a, b), hi = max(a, b);
@@ -316,6 +286,8 @@ spot_status launch_select(const SelectArgs& a, int rows, cudaStream_t s) {
 
 }  // namespace
 
+spot_status launch_select_hist(const SelectArgs& a, int rows, cudaStream_t s);    // select_hist.cu
+
 spot_status run_select(const spot_select_params* p, const float* scores, int nb_stride, int rows_per_seq,
                        int max_nb, cudaStream_t s) {
     if (max_nb > SEL_MAX_NB) return SPOT_ERR_UNSUPPORTED;
@@ -326,8 +298,7 @@ spot_status run_select(const spot_select_params* p, const float* scores, int nb_
     a.sink = p->sink_blocks; a.rec = p->recency_blocks; a.kmin = p->kmin_blocks;
     a.indices = p->indices; a.cap = p->cap; a.budgets = p->budgets; a.probs = p->block_probs;
     const int rows = p->B * rows_per_seq;
-    if (max_nb <= 256) return launch_select<5>(a, rows, s);
-    if (max_nb <= 2048) return launch_select<8>(a, rows, s);
+    if (max_nb <= 2048) return launch_select_hist(a, rows, s);     // histogram-partition form
     if (max_nb <= 4096) return launch_select<9>(a, rows, s);
     return launch_select<10>(a, rows, s);
 }

@@ -1,0 +1,37 @@
+// Shared by the two selection kernels (select.cu: bitonic-sort form; select_hist.cu: histogram-partition form).
+#pragma once
+#include "common.cuh"
+
+namespace spot {
+
+constexpr int SEL_MAX_NB = 8192;
+constexpr uint32_t KEY_PAD = 0xffffffffu;
+
+__device__ __forceinline__ uint32_t orderable(float x) {
+    uint32_t u = __float_as_uint(x + 0.0f);   // -0.0 -> +0.0
+    return (u & 0x80000000u) ? ~u : (u | 0x80000000u);
+}
+__device__ __forceinline__ float from_orderable(uint32_t o) {
+    uint32_t u = (o & 0x80000000u) ? (o & 0x7fffffffu) : ~o;
+    return __uint_as_float(u);
+}
+// sort key: ascending key == descending score
+__device__ __forceinline__ uint32_t score_key(float s) { return ~orderable(s); }
+__device__ __forceinline__ float key_score(uint32_t k) { return from_orderable(~k); }
+
+struct SelectArgs {
+    const float* scores;      // [rows][nb_stride]
+    int nb_stride;
+    const int32_t* seq_len;   // decode: [B]; prefill: nullptr
+    int n_q;                  // rows per sequence
+    int q_start, q_block, blk;
+    int mode, top_k;
+    double p, temperature;
+    int sink, rec, kmin;
+    int32_t* indices;
+    int cap;
+    int32_t* budgets;
+    float* probs;             // optional [rows][nb_stride]
+};
+
+}  // namespace spot

@@ -1,0 +1,407 @@
+// Step a2, histogram-partition form (rows with n_b <= 2048) -- reserved tier, residual softmax (Eq. 7), nucleus +
+// K_min floor (Eq. 8) or static top-K (Eq. 6), one CTA of 256 threads per selection row.
+//
+// The rule only needs (a) the mass in front of the cut and (b) the key value tau at the cut, not a full sort.  So:
+//   1. keys (order-preserving 32-bit images of the scores, ascending key = descending score) go into 2048 bins by a
+//      MONOTONE map of the key range (float multiply + truncate), i.e. bins are contiguous key ranges in rank order;
+//   2. an exclusive scan of the bin counts turns the bins into rank ranges, and a counting-sort scatter groups
+//      (key, exp(z - z_max)) by bin in shared memory -- unordered inside a bin, exactly ordered across bins;
+//   3. a prefix sum of the masses in that grouped order is exact at every bin boundary, so the first position whose
+//      running mass reaches p * total names the bin that holds the cut;
+//   4. only that bin (typically 1-3 blocks) is ranked exactly -- by one warp when it holds <= 32 keys, by a plain
+//      counting pass of the whole CTA otherwise (degenerate inputs such as all-equal scores take an arithmetic
+//      shortcut) -- which gives n* and tau; K_min / top-K ask the same machinery for "the key of rank r";
+//   5. blocks with a better key than tau are selected, blocks tied with tau are taken in ascending block index until
+//      the count is reached (R7), and the ascending index list falls out of a ballot/popc scan in index order.
+// exp, normalisation and the running mass are fp64 (the fp32 block score is then the only source of disagreement
+// with the fp64 oracle).  ~12 CTA barriers and 2300 instructions per warp instead of a 66-step
+// bitonic network and 3400; the launch is 13.9 us against 14.1 us at n_b = 2048 all the same, because a kernel that
+// runs once per step on 4 SMs from cold caches is bound by instruction fetch (stall reason no_instruction 3.6 cycles
+// per issue) and two dependent DRAM misses, not by its instruction count: profiles/r1_decode_cfg3_launches.md, D.
+#include "select_common.cuh"
+
+namespace spot {
+
+namespace {
+
+constexpr int SH_T = 256;
+constexpr int SH_N = 2048;          // keys per row (8 per thread)
+constexpr int SH_NBIN = 2048;
+constexpr int SH_WARPS = SH_T / 32;
+
+struct BinMap {
+    uint32_t kmn;
+    float scale;
+    __device__ __forceinline__ int operator()(uint32_t key) const {
+        const int b = (int)((float)(key - kmn) * scale);      // monotone in key
+        return b < SH_NBIN - 1 ? b : SH_NBIN - 1;
+    }
+};
+
+// Exact ranking of one bin by a single warp (cB <= 32 keys at grouped positions sB ..).  by_mass: returns the number
+// n_in of keys (in rank order) whose running mass base + ... is still < target, clamped to cB - 1; else n_in = want.
+// tau = key of rank n_in inside the bin.  Equal keys are ranked by position (they carry equal mass).
+__device__ __forceinline__ void warp_resolve(const uint32_t* s_k, const double* s_e, int sB, int cB, double base,
+                                             double target, int want, bool by_mass, int lane, int& n_in, uint32_t& tau) {
+    const uint32_t k = lane < cB ? s_k[sB + lane] : KEY_PAD;
+    const double e = (by_mass && lane < cB) ? s_e[sB + lane] : 0.0;
+    int rank = 0;
+    for (int j = 0; j < cB; ++j) {
+        const uint32_t kj = __shfl_sync(0xffffffffu, k, j);
+        rank += (kj < k || (kj == k && j < lane)) ? 1 : 0;
+    }
+    if (lane >= cB) rank = 64 + lane;
+    n_in = want;
+    if (by_mass) {
+        double acc = base, mine = 0.0;
+        for (int r = 0; r < cB; ++r) {
+            const int src = __ffs(__ballot_sync(0xffffffffu, rank == r)) - 1;
+            acc += __shfl_sync(0xffffffffu, e, src);
+            if (rank == r) mine = acc;
+        }
+        n_in = __popc(__ballot_sync(0xffffffffu, lane < cB && mine < target));
+    }
+    n_in = max(0, min(n_in, cB - 1));
+    const int src = __ffs(__ballot_sync(0xffffffffu, rank == n_in)) - 1;
+    tau = __shfl_sync(0xffffffffu, k, src);
+}
+
+__global__ void __launch_bounds__(SH_T) select_hist_kernel(SelectArgs a) {
+    __shared__ uint32_t s_cnt[SH_NBIN];       // bin counts, then exclusive starts
+    __shared__ double s_e[SH_N];              // masses grouped by bin
+    __shared__ uint32_t s_k[SH_N];            // keys grouped by bin
+    __shared__ double s_wd[SH_WARPS];
+    __shared__ uint32_t s_wu[SH_WARPS][2];
+    __shared__ int s_wi[SH_WARPS][2];
+    __shared__ int s_seg[SH_T / 4][2];
+    __shared__ double s_base;
+    __shared__ uint32_t s_tau;
+    __shared__ int s_nin, s_tot[2];
+
+    const int row = blockIdx.x;
+    const int b = row / a.n_q, i = row - b * a.n_q;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    pdl_wait();
+    pdl_launch_dependents();
+    int n_b;
+    if (a.q_block == 1) n_b = (a.seq_len[b] + a.blk - 1) / a.blk;
+    else n_b = (a.q_start + (i + 1) * a.q_block - 1) / a.blk + 1;
+    n_b = min(n_b, SH_N);
+    const int sink_end = min(a.sink, n_b);
+    const int rec_beg = max(sink_end, n_b - a.rec);     // residual blocks: [sink_end, rec_beg)
+    const int n_res = rec_beg - sink_end;
+    const int n_reserved = n_b - n_res;
+    const int ebase = warp * 256 + lane;                // block of register r: ebase + 32 r
+    const bool topp = a.mode != SPOT_MODE_TOPK;
+
+    // ---- load: block scores -> keys; key range of the residual blocks
+    const float* srow = a.scores + (int64_t)row * a.nb_stride;
+    uint32_t okey[8];
+    uint32_t kmn = 0xffffffffu, kmx = 0u;
+#pragma unroll
+    for (int r = 0; r < 8; ++r) {
+        const int j = ebase + 32 * r;
+        const bool resid = j >= sink_end && j < rec_beg;
+        okey[r] = resid ? score_key(srow[j]) : KEY_PAD;
+        if (resid) { kmn = min(kmn, okey[r]); kmx = max(kmx, okey[r]); }
+        s_cnt[tid * 8 + r] = 0u;
+    }
+    kmn = __reduce_min_sync(0xffffffffu, kmn);
+    kmx = __reduce_max_sync(0xffffffffu, kmx);
+    if (lane == 0) { s_wu[warp][0] = kmn; s_wu[warp][1] = kmx; }
+    if (tid == 0) { s_nin = 0; s_tau = 0u; s_base = 0.0; }
+    __syncthreads();
+#pragma unroll
+    for (int w = 0; w < SH_WARPS; ++w) { kmn = min(kmn, s_wu[w][0]); kmx = max(kmx, s_wu[w][1]); }
+
+    int n_take = 0;
+    uint32_t tau = 0u;
+    double e[8], total = 0.0;
+#pragma unroll
+    for (int r = 0; r < 8; ++r) e[r] = 0.0;
+
+    if (n_res > 0) {
+        BinMap bin_of;
+        bin_of.kmn = kmn;
+        bin_of.scale = (float)SH_NBIN / ((float)(kmx - kmn) + 1.0f);
+        // ---- masses (Eq. 7 numerators, fp64), bins, rank inside the bin
+        const double zmax = (double)key_score(kmn) / a.temperature;
+        // (one rolled loop -- the fp64 exp is ~150 instructions and this kernel runs once per step from a cold
+        // instruction cache: code size, not instruction count, is what its latency is made of.  The arrays stay in
+        // registers: every trip works on element 0 and rotates.)
+        uint32_t pk[8];                                   // bin << 12 | rank inside the bin; 0xffffffff: not residual
+        {
+            uint32_t kq[8];
+#pragma unroll
+            for (int r = 0; r < 8; ++r) { kq[r] = okey[r]; pk[r] = 0xffffffffu; }
+#pragma unroll 1
+            for (int r = 0; r < 8; ++r) {
+                const int j = ebase + 32 * r;
+                double ev = 0.0;
+                uint32_t pv = 0xffffffffu;
+                if (j >= sink_end && j < rec_beg) {
+                    if (topp) ev = exp((double)key_score(kq[0]) / a.temperature - zmax);
+                    const int bn = bin_of(kq[0]);
+                    pv = ((uint32_t)bn << 12) | atomicAdd(&s_cnt[bn], 1u);
+                }
+#pragma unroll
+                for (int u = 0; u < 7; ++u) { kq[u] = kq[u + 1]; e[u] = e[u + 1]; pk[u] = pk[u + 1]; }
+                e[7] = ev;
+                pk[7] = pv;
+            }
+        }
+        __syncthreads();
+        // ---- exclusive scan of the bin counts: thread t owns bins 8t .. 8t+7
+        {
+            uint32_t c[8], run = 0;
+#pragma unroll
+            for (int u = 0; u < 8; ++u) { c[u] = s_cnt[tid * 8 + u]; run += c[u]; }
+            uint32_t inc = run;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                const uint32_t t = __shfl_up_sync(0xffffffffu, inc, o);
+                if (lane >= o) inc += t;
+            }
+            if (lane == 31) s_wi[warp][0] = (int)inc;
+            __syncthreads();
+            uint32_t off = inc - run;
+#pragma unroll
+            for (int w = 0; w < SH_WARPS; ++w) off += (w < warp) ? (uint32_t)s_wi[w][0] : 0u;
+#pragma unroll
+            for (int u = 0; u < 8; ++u) { s_cnt[tid * 8 + u] = off; off += c[u]; }
+        }
+        __syncthreads();
+        // ---- counting-sort scatter: grouped by bin, bins in rank order
+#pragma unroll
+        for (int r = 0; r < 8; ++r)
+            if (pk[r] != 0xffffffffu) {
+                const int pos = (int)s_cnt[pk[r] >> 12] + (int)(pk[r] & 0xfffu);
+                s_k[pos] = okey[r];
+                if (topp) s_e[pos] = e[r];
+            }
+        __syncthreads();
+        // ---- what has to be resolved exactly: up to two queries against one bin each, run by ONE copy of the code
+        //      query 0 (dual top-p, p < 1): the bin holding the cut of the running mass -> n*, tau
+        //      query 1 (top-K, K_min floor): the key of rank n_take - 1
+        double target = 0.0, off = 0.0, c[8];
+        int n_lt = 0;
+        if (topp) {
+            // running mass in grouped order: thread t owns positions 8t .. 8t+7
+            double run = 0.0;
+#pragma unroll
+            for (int u = 0; u < 8; ++u) {
+                const int pos = tid * 8 + u;
+                run += pos < n_res ? s_e[pos] : 0.0;
+                c[u] = run;
+            }
+            double inc = run;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                const double t = __shfl_up_sync(0xffffffffu, inc, o);
+                if (lane >= o) inc += t;
+            }
+            if (lane == 31) s_wd[warp] = inc;
+            __syncthreads();
+            off = inc - run;
+#pragma unroll
+            for (int w = 0; w < SH_WARPS; ++w) {
+                if (w < warp) off += s_wd[w];
+                total += s_wd[w];
+            }
+            target = a.p * total;
+            int cnt = 0;
+#pragma unroll
+            for (int u = 0; u < 8; ++u) cnt += (tid * 8 + u < n_res && off + c[u] < target) ? 1 : 0;
+            cnt = __reduce_add_sync(0xffffffffu, cnt);
+            if (lane == 0) s_wi[warp][1] = cnt;
+            __syncthreads();
+#pragma unroll
+            for (int w = 0; w < SH_WARPS; ++w) n_lt += s_wi[w][1];
+            n_take = n_res;                                   // p >= 1: all of B_res by definition (R20)
+        } else {
+#pragma unroll
+            for (int u = 0; u < 8; ++u) c[u] = 0.0;
+            n_take = min(max(0, a.top_k - n_reserved), n_res);
+        }
+        bool have_tau = false;
+#pragma unroll 1
+        for (int query = (topp && a.p < 1.0) ? 0 : 1; query < 2; ++query) {
+            const bool by_mass = query == 0;
+            if (!by_mass) {
+                if (have_tau || n_take <= 0) break;
+                if (n_take == n_res) { tau = kmx; break; }    // everything: the worst key
+            }
+            const int B = bin_of(s_k[by_mass ? min(n_lt, n_res - 1) : n_take - 1]);   // the bin holding that position
+            const int sB = (int)s_cnt[B];
+            const int cB = (B + 1 < SH_NBIN ? (int)s_cnt[B + 1] : n_res) - sB;
+            const int want = n_take - 1 - sB;
+            if (by_mass && sB > 0 && tid == ((sB - 1) >> 3)) {   // running mass in front of the bin: its owner publishes it
+                double v = c[0];
+#pragma unroll
+                for (int u = 1; u < 8; ++u) v = (((sB - 1) & 7) == u) ? c[u] : v;
+                s_base = off + v;
+            }
+            __syncthreads();
+            const double base = (by_mass && sB > 0) ? s_base : 0.0;
+            // exact ranking of the bin (grouped positions sB .. sB + cB - 1): s_nin = keys of the bin in front of the
+            // cut (or `want`), s_tau = the key of that rank
+            if (cB <= 32) {
+                if (warp == 0) {
+                    int n_in;
+                    uint32_t t;
+                    warp_resolve(s_k, s_e, sB, cB, base, target, want, by_mass, lane, n_in, t);
+                    if (lane == 0) { s_nin = n_in; s_tau = t; }
+                }
+            } else {
+                // a crowded bin (degenerate score distributions): whole CTA
+                uint32_t lo = 0xffffffffu, hi = 0u;
+                for (int x = tid; x < cB; x += SH_T) { const uint32_t k = s_k[sB + x]; lo = min(lo, k); hi = max(hi, k); }
+                lo = __reduce_min_sync(0xffffffffu, lo);
+                hi = __reduce_max_sync(0xffffffffu, hi);
+                if (lane == 0) { s_wu[warp][0] = lo; s_wu[warp][1] = hi; }
+                if (tid == 0) s_nin = 0;
+                __syncthreads();
+#pragma unroll
+                for (int w = 0; w < SH_WARPS; ++w) { lo = min(lo, s_wu[w][0]); hi = max(hi, s_wu[w][1]); }
+                if (lo == hi) {
+                    // every key of the bin is the same: equal masses, ranked by position -> arithmetic
+                    if (tid == 0) {
+                        int m = want;
+                        if (by_mass) {
+                            const double e0 = s_e[sB];
+                            m = e0 > 0.0 ? (int)fmin(fmax(ceil((target - base) / e0) - 1.0, 0.0), (double)(cB - 1)) : 0;
+                            while (m > 0 && base + (double)m * e0 >= target) --m;
+                            while (m < cB - 1 && base + (double)(m + 1) * e0 < target) ++m;
+                        }
+                        s_nin = max(0, min(m, cB - 1));
+                        s_tau = lo;
+                    }
+                } else {
+                    // two counting passes: (mass query only) how many keys stay in front of the cut, then the key
+                    // of the wanted rank
+                    int n_in = want;
+                    if (by_mass) {
+                        int cnt = 0;
+#pragma unroll 1
+                        for (int x = tid; x < cB; x += SH_T) {
+                            const uint32_t kx = s_k[sB + x];
+                            double cum = base;
+                            for (int j = 0; j < cB; ++j) {
+                                const uint32_t kj = s_k[sB + j];
+                                if (kj < kx || (kj == kx && j <= x)) cum += s_e[sB + j];
+                            }
+                            if (cum < target) ++cnt;
+                        }
+                        cnt = __reduce_add_sync(0xffffffffu, cnt);
+                        if (lane == 0 && cnt) atomicAdd(&s_nin, cnt);
+                        __syncthreads();
+                        n_in = s_nin;
+                        __syncthreads();
+                    }
+                    n_in = max(0, min(n_in, cB - 1));
+#pragma unroll 1
+                    for (int x = tid; x < cB; x += SH_T) {
+                        const uint32_t kx = s_k[sB + x];
+                        int rank = 0;
+                        for (int j = 0; j < cB; ++j) {
+                            const uint32_t kj = s_k[sB + j];
+                            rank += (kj < kx || (kj == kx && j < x)) ? 1 : 0;
+                        }
+                        if (rank == n_in) { s_tau = kx; s_nin = n_in; }
+                    }
+                }
+            }
+            __syncthreads();
+            tau = s_tau;
+            have_tau = true;
+            if (by_mass) {
+                n_take = sB + s_nin + 1;                      // n*
+                const int floor_cnt = min(a.kmin, n_b);       // K_min floor on the union (R8)
+                if (n_reserved + n_take < floor_cnt) { n_take = min(n_res, floor_cnt - n_reserved); have_tau = false; }
+            }
+            __syncthreads();                                  // s_nin / s_tau may be rewritten by the next query
+        }
+    }
+    __syncthreads();
+
+    // ---- index order: A = reserved or strictly better than tau (certainly selected), Tt = tied with tau
+    constexpr int NSEG = SH_T / 4;                       // 32-block segments: (warp, register)
+    int prefA[8], prefT[8];
+    uint32_t isA = 0, isT = 0;
+#pragma unroll
+    for (int r = 0; r < 8; ++r) {
+        const int j = ebase + 32 * r;
+        const bool resid = j >= sink_end && j < rec_beg;
+        const bool fa = (j < n_b && !resid) || (resid && n_take > 0 && okey[r] < tau);
+        const bool ft = resid && n_take > 0 && okey[r] == tau;
+        const uint32_t ba = __ballot_sync(0xffffffffu, fa), bt = __ballot_sync(0xffffffffu, ft);
+        const uint32_t lt = (1u << lane) - 1u;
+        prefA[r] = __popc(ba & lt);
+        prefT[r] = __popc(bt & lt);
+        isA |= (uint32_t)fa << r;
+        isT |= (uint32_t)ft << r;
+        if (lane == 0) { s_seg[warp * 8 + r][0] = __popc(ba); s_seg[warp * 8 + r][1] = __popc(bt); }
+    }
+    __syncthreads();
+    if (warp == 0) {
+        constexpr int PER = NSEG / 32;
+        int va[PER], vt[PER], ra = 0, rt = 0;
+#pragma unroll
+        for (int u = 0; u < PER; ++u) {
+            const int s = lane * PER + u;
+            va[u] = s_seg[s][0];
+            vt[u] = s_seg[s][1];
+            ra += va[u]; rt += vt[u];
+        }
+        int ia = ra, it = rt;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const int ta = __shfl_up_sync(0xffffffffu, ia, o), tt = __shfl_up_sync(0xffffffffu, it, o);
+            if (lane >= o) { ia += ta; it += tt; }
+        }
+        int oa = ia - ra, ot = it - rt;
+#pragma unroll
+        for (int u = 0; u < PER; ++u) {
+            const int s = lane * PER + u;
+            s_seg[s][0] = oa; s_seg[s][1] = ot;
+            oa += va[u]; ot += vt[u];
+        }
+        if (lane == 31) { s_tot[0] = ia; s_tot[1] = it; }
+    }
+    __syncthreads();
+    const int total_A = s_tot[0], total_T = s_tot[1];
+    const int need = n_take - (total_A - n_reserved);    // ties to take, lowest block index first
+    const int total_sel = total_A + min(total_T, max(need, 0));
+    int32_t* out = a.indices + (int64_t)row * a.cap;
+#pragma unroll
+    for (int r = 0; r < 8; ++r) {
+        const int j = ebase + 32 * r;
+        const int a_before = s_seg[warp * 8 + r][0] + prefA[r];
+        const int t_before = s_seg[warp * 8 + r][1] + prefT[r];
+        int pos = -1;
+        if ((isA >> r) & 1u) pos = a_before + min(t_before, need);
+        else if (((isT >> r) & 1u) && t_before < need) pos = a_before + t_before;
+        if (pos >= 0 && pos < a.cap) out[pos] = j;
+    }
+    for (int j = total_sel + tid; j < a.cap; j += SH_T) out[j] = -1;
+    if (tid == 0) a.budgets[row] = min(total_sel, a.cap);
+
+    if (a.probs) {
+        float* pr = a.probs + (int64_t)row * a.nb_stride;
+        const double inv_total = total > 0.0 ? 1.0 / total : 0.0;
+#pragma unroll
+        for (int r = 0; r < 8; ++r) {
+            const int j = ebase + 32 * r;
+            if (j < n_b) pr[j] = (float)(e[r] * inv_total);      // 0 on reserved blocks and in top-K mode
+        }
+    }
+}
+
+}  // namespace
+
+spot_status launch_select_hist(const SelectArgs& a, int rows, cudaStream_t s) {
+    SPOT_CUDA_TRY(launch_pdl(select_hist_kernel, dim3((unsigned)rows), dim3(SH_T), 0, s, a));
+    return SPOT_OK;
+}
+
+}  // namespace spot

@@ -106,6 +106,42 @@ def test_select_edge_cases(torch_cuda):
                 _check_select(dd, fmt, report, **over)
 
 
+def test_select_crowded_cut_bins_and_ties(torch_cuda):
+    """Score distributions that defeat the histogram partition of the selection kernel: the cut falls into ONE bin
+    holding (a) 40 distinct scores 4e-6 apart, (b) 40 exactly tied scores, (c) every residual block, all tied
+    (all-zero scores), (d) 200 tied blocks among distinct ones.  Scores are planted exactly: head 0 reads k[0] with
+    weight 1, head 1 reads k[0] with weight 4e-6, one live token per block."""
+    from workloads import f32_to_bf16_bits
+    n_b, L = 256, 256 * 64
+    wl = make_decode_workload("crowd", 11, B=4, L=L, kind="gauss", with_kv=False)
+    q = np.zeros((4, wl.H_idx, wl.d_idx), dtype=np.float32)
+    q[:, 0, 0] = 1.0
+    q[:, 1, 0] = 1.0
+    wl.sel_q = f32_to_bf16_bits(q)
+    wl.w = np.tile(np.array([1.0, 4e-6, 0.0, 0.0], dtype=np.float32), (4, 1))
+    k = np.zeros((4, L, wl.H_idx, wl.d_idx), dtype=np.float32)
+    rng = np.random.default_rng(5)
+    tok = np.arange(n_b) * 64 + rng.integers(0, 64, size=n_b)
+    cluster = rng.permutation(np.arange(1, n_b - 2))[:40]
+    k[0, tok, 0, 0] = 2.0 ** -10                  # low background stretches the key range: one bin = 40960 ulps
+    k[0, tok[cluster], 0, 0] = 1.0
+    k[0, tok[cluster], 1, 0] = np.arange(40)      # (a) 1 + 4e-6 m
+    k[1, tok, 0, 0] = 2.0 ** -10
+    k[1, tok[cluster], 0, 0] = 1.0                # (b) 40 exact ties at the cut
+    # (c) sequence 2 stays all zero: every score is exactly 0
+    k[3, tok, 0, 0] = 0.5 + rng.integers(0, 64, size=n_b) / 128.0
+    big = rng.permutation(np.arange(1, n_b - 2))[:200]
+    k[3, tok[big], 0, 0] = 1.25                   # (d) 200 ties
+    wl.sel_k = f32_to_bf16_bits(k)
+    dd = H.DeviceDecode(wl, "bf16", with_kv=False)
+    report = []
+    for over in (dict(p=0.5, kmin_blocks=0), dict(p=0.9), dict(p=0.3, kmin_blocks=30), dict(p=1.0),
+                 dict(mode="topk", top_k=23), dict(mode="topk", top_k=150, sink_blocks=0, recency_blocks=0)):
+        _check_select(dd, "bf16", report, **over)
+    bad = [r for r in report if r[3] != "exact"]  # planted scores are far apart or exactly tied: everything exact
+    assert not bad, bad
+
+
 # ---------------------------------------------------------------- a3
 def _check_attend(dd, idx_lists, dense=False):
     wl = dd.wl
