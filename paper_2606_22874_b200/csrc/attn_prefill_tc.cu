@@ -130,41 +130,49 @@ __global__ void __launch_bounds__(TA_THREADS, 1) attn_prefill_tc_kernel(const __
             constexpr uint32_t idesc_pv = umma_idesc_bf16(128, 128) | UMMA_B_MN_MAJOR;
             int nv = 0;
             for (int it = 0; it < budget; ++it) nv += visible(block_of(it)) ? 1 : 0;
-            const int nt = two ? 2 : 1;
-            auto qk = [&](int t, uint32_t ks) {           // S_t = Q_t K^T
+            // One lone thread issues every MMA, with nobody to hide its instruction latencies: descriptors are built
+            // once and advanced by compile-time constants (the start-address field is the low 14 bits, in 16-byte
+            // units), so each tcgen05.mma costs two integer adds, not a dozen dependent ones.
+            const uint64_t qd[2] = {umma_desc_sw128(q_smem), umma_desc_sw128(q_smem + TA_Q_TILE)};
+            auto qk = [&](int t, uint64_t kd) {           // S_t = Q_t K^T
 #pragma unroll
-                for (int kk = 0; kk < 8; ++kk) {
-                    const uint64_t ad = umma_desc_sw128(q_smem + t * TA_Q_TILE + (kk >> 2) * (128 * 128) + (kk & 3) * 32);
-                    const uint64_t bd = umma_desc_sw128(ks + (kk >> 2) * (64 * 128) + (kk & 3) * 32);
-                    umma_bf16_ss(tbase + t * 64, ad, bd, idesc_qk, kk > 0);
-                }
+                for (int kk = 0; kk < 8; ++kk)
+                    umma_bf16_ss(tbase + t * 64, qd[t] + (uint64_t)(((kk >> 2) * (128 * 128) + (kk & 3) * 32) >> 4),
+                                 kd + (uint64_t)(((kk >> 2) * (64 * 128) + (kk & 3) * 32) >> 4), idesc_qk, kk > 0);
                 umma_commit(bar_s_full + 8 * t);
             };
-            auto pv = [&](int t, uint32_t vs, bool acc) { // O_t += P_t V
+            auto pv = [&](int t, uint64_t vd, bool acc) { // O_t += P_t V, P_t packed BF16 in the first 32 columns of S_t
 #pragma unroll
-                for (int kk = 0; kk < 4; ++kk) {
-                    const uint64_t ad = umma_desc_sw128(p_smem + t * TA_P_TILE + kk * 32);
-                    const uint64_t bd = umma_desc_sw128_mn(vs + kk * 2048, 64 * 128, 1024);
-                    umma_bf16_ss(tbase + 128 + t * 128, ad, bd, idesc_pv, acc || kk > 0);
-                }
+                for (int kk = 0; kk < 4; ++kk)
+                    umma_bf16_ts(tbase + 128 + t * 128, tbase + t * 64 + kk * 8, vd + (uint64_t)((kk * 2048) >> 4), idesc_pv,
+                                 acc || kk > 0);
                 umma_commit(bar_o_done + 8 * t);
             };
             if (nv > 0) {
                 mbar_wait(bar_q_full, 0);
                 mbar_wait(bar_k_full, 0);
                 tc_fence_after();
-                for (int t = 0; t < nt; ++t) qk(t, kv_smem);
+                {
+                    const uint64_t kd0 = umma_desc_sw128(kv_smem);
+                    qk(0, kd0);
+                    if (two) qk(1, kd0);
+                }
                 for (int n = 0; n < nv; ++n) {
                     const int s = n % TA_STAGES, s1 = (n + 1) % TA_STAGES;
-                    const uint32_t vs = kv_smem + s * 2 * TA_KV_TILE + TA_KV_TILE;
-                    const uint32_t ks1 = kv_smem + s1 * 2 * TA_KV_TILE;
+                    const uint64_t vd = umma_desc_sw128_mn(kv_smem + s * 2 * TA_KV_TILE + TA_KV_TILE, 64 * 128, 1024);
+                    const uint64_t kd1 = umma_desc_sw128(kv_smem + s1 * 2 * TA_KV_TILE);
+                    const bool more = n + 1 < nv;
                     mbar_wait(bar_v_full + 8 * s, (n / TA_STAGES) & 1);
-                    if (n + 1 < nv) mbar_wait(bar_k_full + 8 * s1, ((n + 1) / TA_STAGES) & 1);
-                    for (int t = 0; t < nt; ++t) {
-                        mbar_wait(bar_p_full + 8 * t, n & 1);          // P_t(n) written, S_t consumed, O_t rescaled
+                    if (more) mbar_wait(bar_k_full + 8 * s1, ((n + 1) / TA_STAGES) & 1);
+                    mbar_wait(bar_p_full, n & 1);                       // P_0(n) written, S_0 consumed, O_0 rescaled
+                    tc_fence_after();
+                    pv(0, vd, n > 0);
+                    if (more) qk(0, kd1);
+                    if (two) {
+                        mbar_wait(bar_p_full + 8, n & 1);
                         tc_fence_after();
-                        pv(t, vs, n > 0);
-                        if (n + 1 < nv) qk(t, ks1);
+                        pv(1, vd, n > 0);
+                        if (more) qk(1, kd1);
                     }
                     umma_commit(bar_kv_empty + 8 * s);                  // K(n), V(n) no longer read
                 }
@@ -183,7 +191,13 @@ __global__ void __launch_bounds__(TA_THREADS, 1) attn_prefill_tc_kernel(const __
             const uint32_t t_o = tbase + ((uint32_t)(lq * 32) << 16) + 128 + t * 128;
             const uint32_t p_row = p_smem + t * TA_P_TILE + r * 128;
             float m_used = -INFINITY, l = 0.f;
-            int n = 0;
+            int n = 0, nv = 0;
+            for (int it = 0; it < budget; ++it) nv += visible(block_of(it)) ? 1 : 0;
+            // The two tiles must run in ANTI-phase (softmax of one while the tensor pipe works for the other).  Left
+            // alone they fall into phase -- both S tiles are ready together, both softmaxes share the MUFU, both
+            // hand back together -- and MUFU time and tensor time add up instead of overlapping (ncu: XU 37 % +
+            // tensor 60 %).  Named barriers 2 / 3 make the exp sections alternate: tile 0, tile 1, tile 0, ...
+            if (two && t == 1) asm volatile("bar.arrive 2, 256;" ::: "memory");
             for (int it = 0; it < budget; ++it) {
                 const int j = block_of(it);
                 if (!visible(j)) continue;
@@ -197,13 +211,21 @@ __global__ void __launch_bounds__(TA_THREADS, 1) attn_prefill_tc_kernel(const __
 #pragma unroll
                     for (int e = 0; e < 16; ++e) { x[e] = d0[e]; x[16 + e] = d1[e]; x[32 + e] = d2[e]; x[48 + e] = d3[e]; }
                 }
-                const bool diag = (j == qb_abs);
-                float mx = -INFINITY;
-#pragma unroll
-                for (int e = 0; e < 64; ++e) {
-                    x[e] = (diag && e > ql) ? -INFINITY : x[e] * a.scale_log2;
-                    mx = fmaxf(mx, x[e]);
+                if (two) {
+                    if (t == 0) asm volatile("bar.sync 2, 256;" ::: "memory");
+                    else asm volatile("bar.sync 3, 256;" ::: "memory");
                 }
+                // causal mask inside the diagonal block only (CTA-uniform branch); the row max is taken on the raw
+                // logits (sm_scale > 0) so that scale and max-subtraction fuse into one FFMA per element below
+                if (j == qb_abs) {
+#pragma unroll
+                    for (int e = 0; e < 64; ++e)
+                        if (e > ql) x[e] = -INFINITY;
+                }
+                float mxa = fmax3(x[0], x[1], x[2]), mxb = fmax3(x[3], x[4], x[5]);
+#pragma unroll
+                for (int e = 6; e < 62; e += 4) { mxa = fmax3(mxa, x[e], x[e + 1]); mxb = fmax3(mxb, x[e + 2], x[e + 3]); }
+                const float mx = fmax3(fmaxf(mxa, mxb), x[62], x[63]) * a.scale_log2;
                 // lazy rescale: keep the stale max unless the row max grew by more than 2^8 (warp-uniform decision,
                 // tcgen05.ld/st are warp-collective)
                 const bool need = mx > m_used + TA_RESCALE_THRESHOLD;
@@ -227,22 +249,28 @@ __global__ void __launch_bounds__(TA_THREADS, 1) attn_prefill_tc_kernel(const __
                         tmem_st_wait();
                     }
                 }
-                float ps = 0.f;
+                float ps0 = 0.f, ps1 = 0.f;
                 uint32_t pk[32];
+                const float neg_m = -m_used;
 #pragma unroll
                 for (int e = 0; e < 64; e += 2) {
-                    const float p0 = fast_exp2(x[e] - m_used), p1 = fast_exp2(x[e + 1] - m_used);
-                    ps += p0 + p1;
+                    const float p0 = fast_exp2(fmaf(x[e], a.scale_log2, neg_m));
+                    const float p1 = fast_exp2(fmaf(x[e + 1], a.scale_log2, neg_m));
+                    ps0 += p0;
+                    ps1 += p1;
                     pk[e >> 1] = pack_bf16x2(p0, p1);
                 }
-                l += ps;
-                if (n > 0) mbar_wait(bar_o_done + 8 * t, (n - 1) & 1);       // PV(n-1) no longer reads P_t
-#pragma unroll
-                for (int c = 0; c < 8; ++c) {
-                    asm volatile("st.shared.v4.u32 [%0], {%1,%2,%3,%4};" :: "r"(p_row + (((uint32_t)c ^ (r & 7)) << 4)),
-                                 "r"(pk[4 * c]), "r"(pk[4 * c + 1]), "r"(pk[4 * c + 2]), "r"(pk[4 * c + 3]) : "memory");
+                const float ps = ps0 + ps1;
+                if (two) {
+                    if (t == 0) asm volatile("bar.arrive 3, 256;" ::: "memory");
+                    else if (n + 1 < nv) asm volatile("bar.arrive 2, 256;" ::: "memory");
                 }
-                fence_proxy_async_smem();
+                l += ps;
+                // P_t overwrites the first half of S_t (the logits are in registers; QK_t(n+1), which rewrites S_t, is
+                // issued after PV_t(n) and the tensor pipe runs them in order)
+                tmem_st16u(t_s, pk);
+                tmem_st16u(t_s + 16, pk + 16);
+                tmem_st_wait();
                 tc_fence_before();
                 mbar_arrive(bar_p_full + 8 * t);
                 ++n;
