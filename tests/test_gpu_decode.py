@@ -212,9 +212,11 @@ def test_end_to_end_step_matches_oracle(torch_cuda):
         assert err.max() <= MAX_ABS and err.mean() <= MEAN_ABS
 
 
-@pytest.mark.parametrize("fmt,seqs", [("bf16", (0, 3)), ("mxfp4", (1,))])
-def test_full_size_cfg3_in_the_bench_configuration(torch_cuda, fmt, seqs):
-    """BASELINE.json config 3 at full size (B=4, L=131072, 2048 blocks per sequence), launched exactly as bench.py
+@pytest.mark.parametrize("cfg,fmt,seqs", [("cfg3", "bf16", (0, 3)), ("cfg3", "mxfp4", (1,)), ("cfg3", "int4_e4m3", (2,)),
+                                          ("cfg2", "bf16", (0, 7)), ("cfg4_b4", "mxfp4", (0, 1, 2, 3))])
+def test_full_size_configs_in_the_bench_configuration(torch_cuda, cfg, fmt, seqs):
+    """BASELINE.json configs 2, 3 and 4 (batch 4) at full size (config 3: B=4, L=131072, 2048 blocks per sequence;
+    config 4: H_q=64 and per-query budgets from the K_min floor to hundreds of blocks), launched exactly as bench.py
     launches it (scores in the workspace, cap = n_b, K/V [B][H_kv][L][D] drawn on the device).  Sampled outputs the
     oracle can compute one by one: the whole selection of the sampled sequences (scores, index list, budget), and
     the attention output of every head of those sequences over the oracle's list (the oracle is run on the gathered
@@ -222,10 +224,11 @@ def test_full_size_cfg3_in_the_bench_configuration(torch_cuda, fmt, seqs):
     torch = torch_cuda
     from oracle import attention as OA
     from paper_2606_22874_b200 import api
-    wl = make_config("cfg3", with_kv=False)
+    wl = make_config(cfg, with_kv=False)
     dd = H.DeviceDecode(wl, fmt, with_kv=False)
     idx, bud, scores, probs = dd.select()
     assert bud.min() >= 8 and bud.max() <= dd.n_b_max
+    print("%s %s budgets %s" % (cfg, fmt, bud.tolist()))
     dev = torch.device("cuda")
     gen = torch.Generator(device=dev)
     gen.manual_seed(wl.seed + 17)
@@ -243,7 +246,7 @@ def test_full_size_cfg3_in_the_bench_configuration(torch_cuda, fmt, seqs):
         np.testing.assert_allclose(scores[b, :len(s_bar)], s_bar, rtol=2e-5, atol=2e-5)
         cls = H.classify_selection(s_bar, sel, idx[b], int(bud[b]), wl.p)
         assert not cls.startswith("FAIL"), "seq %d: %s" % (b, cls)
-        print("cfg3 %s seq %d: selection %s, budget %d" % (fmt, b, cls, sel.budget))
+        print("%s %s seq %d: selection %s, budget %d" % (cfg, fmt, b, cls, sel.budget))
         if cls == "exact":
             assert np.abs(probs[b, :len(s_bar)] - sel.probs).max() <= PROB_ABS
         idx_use[b] = -1
@@ -270,4 +273,4 @@ def test_full_size_cfg3_in_the_bench_configuration(torch_cuda, fmt, seqs):
         err = np.abs(got[b] - want)
         assert err.max() <= MAX_ABS and err.mean() <= MEAN_ABS, (b, err.max(), err.mean())
         assert np.abs(lse[b].cpu().numpy() - want_lse).max() <= 2e-3
-        print("cfg3 %s seq %d: attention over %d blocks, max-abs %.2e mean-abs %.2e" % (fmt, b, n, err.max(), err.mean()))
+        print("%s %s seq %d: attention over %d blocks, max-abs %.2e mean-abs %.2e" % (cfg, fmt, b, n, err.max(), err.mean()))
