@@ -4,20 +4,25 @@
 //
 // Tensor-bound.  Work item = (sequence, query block, KV head, PAIR of 128-row tiles); rows stack the group's query
 // heads: row = head_in_group * 64 + query, so one K/V tile in shared memory feeds every head of the group.
-//   warp 0 lane 0 : TMA producer.  Q (two [2 d-halves][128 rows][64] tiles) once, then a 3-stage ring of K_j and V_j
+//   warp 0 lane 0 : TMA producer.  Q (two [2 d-halves][128 rows][64] tiles) once, then a 4-stage ring of K_j and V_j
 //                   ([2 d-halves][64 keys][64], 16 KiB each, 128-byte swizzle) through rank-5 tensor maps built from
 //                   the caller's element strides.
-//   warp 1 lane 0 : tcgen05.mma issuer.  S_t = Q_t K_j^T (M=128, N=64, 8 k-steps, both operands K-major) into TMEM;
-//                   O_t += P_t V_j (M=128, N=128, 4 k-steps) with P_t K-major from shared memory and V_j used as an
-//                   MN-major B operand exactly as TMA wrote it (no transpose).  The two tiles ping-pong: while the
-//                   softmax warps of one tile work, the tensor pipe runs the other tile's MMAs:
+//   warp 1 lane 0 : tcgen05.mma issuer.  S_t = Q_t K_j^T (M=128, N=64, 8 k-steps, both operands K-major in shared
+//                   memory) into TMEM; O_t += P_t V_j (M=128, N=128, 4 k-steps) with P_t read from TENSOR MEMORY
+//                   (packed BF16 over the first half of S_t) and V_j used as an MN-major B operand exactly as TMA
+//                   wrote it (no transpose).  Descriptors are built once and advanced by constants: the lone issuing
+//                   thread has nobody to hide its instruction latencies.  The two tiles ping-pong:
 //                       PV0(n)  QK0(n+1)  |  PV1(n)  QK1(n+1)  | ...
 //   warps 4-7, 8-11: softmax of tile 0 / tile 1, one thread per row (TMEM lane = row).  tcgen05.ld of the 64 logits,
-//                   log2-domain online softmax with a LAZY rescale of the TMEM-resident O (only when a row's max
-//                   grows by more than 2^8 since the last rescale: P stays <= 256, l and O use the same stale max, so
-//                   the result is exact), P rounded to BF16 into 128-byte-swizzled shared memory, fence.proxy.async,
-//                   mbarrier hand-off.  Epilogue: O / l -> BF16, 256 B per row, optional LSE.
-// TMEM: S_0 | S_1 | O_0 | O_1 = 64 + 64 + 128 + 128 columns.
+//                   log2-domain online softmax (scale and max-subtraction fused into one FFMA per element) with a
+//                   LAZY rescale of the TMEM-resident O (only when a row's max grows by more than 2^8 since the last
+//                   rescale: P stays <= 256, l and O use the same stale max, so the result is exact), P rounded to
+//                   BF16 and stored back to TMEM (tcgen05.st), mbarrier hand-off.  Named barriers keep the two tiles'
+//                   exp sections alternating.  Epilogue: O / l -> BF16, 256 B per row, optional LSE.
+// TMEM: S_0 | S_1 | O_0 | O_1 = 64 + 64 + 128 + 128 columns.  Grid: (tile pair, query block heaviest-first, KV head) with
+// the KV head slowest, so the CTAs in flight share one head's K/V in L2 (DRAM traffic 25 GB -> see profiles/).
+// History (cfg5, TFLOP/s): mma.sync 328 -> tcgen05 SS 789 -> fused FFMA 805 -> P in TMEM 826 -> hoisted descriptors
+// 887 -> head-slowest grid 982.
 #include "common.cuh"
 #include "tc100.cuh"
 
@@ -25,12 +30,11 @@ namespace spot {
 
 namespace {
 
-constexpr int TA_STAGES = 3;
+constexpr int TA_STAGES = 4;
 constexpr int TA_THREADS = 12 * 32;
 constexpr uint32_t TA_Q_TILE = 2 * 128 * 128;          // 32 KiB: [2 halves][128 rows][128 B]
 constexpr uint32_t TA_KV_TILE = 2 * 64 * 128;          // 16 KiB: [2 halves][64 keys][128 B]
-constexpr uint32_t TA_P_TILE = 128 * 128;              // 16 KiB: [128 rows][64 keys] BF16
-constexpr uint32_t TA_SMEM_TILES = 2 * TA_Q_TILE + TA_STAGES * 2 * TA_KV_TILE + 2 * TA_P_TILE;   // 192 KiB
+constexpr uint32_t TA_SMEM_TILES = 2 * TA_Q_TILE + TA_STAGES * 2 * TA_KV_TILE;   // 192 KiB
 constexpr uint32_t TA_SMEM_BYTES = 1024 + TA_SMEM_TILES + 256;
 constexpr float TA_RESCALE_THRESHOLD = 8.0f;           // log2 units
 
@@ -54,20 +58,21 @@ __global__ void __launch_bounds__(TA_THREADS, 1) attn_prefill_tc_kernel(const __
     unsigned char* smem = smem_raw + (base - smem_u32(smem_raw));
     const uint32_t q_smem = base;                                        // 2 x 32 KiB
     const uint32_t kv_smem = base + 2 * TA_Q_TILE;                       // stages x (K 16 KiB, V 16 KiB)
-    const uint32_t p_smem = kv_smem + TA_STAGES * 2 * TA_KV_TILE;        // 2 x 16 KiB
     const uint32_t misc = base + TA_SMEM_TILES;
     const uint32_t bar_q_full = misc;
-    const uint32_t bar_k_full = misc + 8;                // [3]
-    const uint32_t bar_v_full = misc + 32;               // [3]
-    const uint32_t bar_kv_empty = misc + 56;             // [3]
-    const uint32_t bar_s_full = misc + 80;               // [2]
-    const uint32_t bar_p_full = misc + 96;               // [2]
-    const uint32_t bar_o_done = misc + 112;              // [2]
-    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(smem + TA_SMEM_TILES + 128);
+    const uint32_t bar_k_full = misc + 8;                // [TA_STAGES]
+    const uint32_t bar_v_full = misc + 40;               // [TA_STAGES]
+    const uint32_t bar_kv_empty = misc + 72;             // [TA_STAGES]
+    const uint32_t bar_s_full = misc + 104;              // [2]
+    const uint32_t bar_p_full = misc + 120;              // [2]
+    const uint32_t bar_o_done = misc + 136;              // [2]
+    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(smem + TA_SMEM_TILES + 160);
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int pair = blockIdx.x, hk = blockIdx.y;
-    const int rowz = (int)gridDim.z - 1 - (int)blockIdx.z;               // heaviest (latest) query blocks first
+    // launch order: x (tile pair) fastest, then y (query block, heaviest = latest first), KV head slowest -- the CTAs in
+    // flight at any time share ONE head's K/V (32 MiB at L = 64K, L2-resident) instead of all eight heads' (256 MiB)
+    const int pair = blockIdx.x, hk = blockIdx.z;
+    const int rowz = (int)gridDim.y - 1 - (int)blockIdx.y;
     const int b = rowz / a.n_qb, i = rowz - b * a.n_qb;
     const int G = a.G;
     const int qb_abs = a.qb_start + i;
@@ -90,7 +95,7 @@ __global__ void __launch_bounds__(TA_THREADS, 1) attn_prefill_tc_kernel(const __
         tma_prefetch_desc(&tm_k);
         tma_prefetch_desc(&tm_v);
     }
-    if (warp == 2) tmem_alloc(misc + 128, 512);
+    if (warp == 2) tmem_alloc(misc + 160, 512);
     tc_fence_before();
     __syncthreads();
     tc_fence_after();
@@ -189,7 +194,6 @@ __global__ void __launch_bounds__(TA_THREADS, 1) attn_prefill_tc_kernel(const __
             const bool live = hg < G;
             const uint32_t t_s = tbase + ((uint32_t)(lq * 32) << 16) + t * 64;
             const uint32_t t_o = tbase + ((uint32_t)(lq * 32) << 16) + 128 + t * 128;
-            const uint32_t p_row = p_smem + t * TA_P_TILE + r * 128;
             float m_used = -INFINITY, l = 0.f;
             int n = 0, nv = 0;
             for (int it = 0; it < budget; ++it) nv += visible(block_of(it)) ? 1 : 0;
@@ -358,7 +362,7 @@ spot_status attn_prefill_tc(const spot_attn_params* p, cudaStream_t stream) {
         attr_set = true;
     }
     const int n_mt = (a.G * 64 + 127) / 128;
-    dim3 grid((unsigned)((n_mt + 1) / 2), (unsigned)p->H_kv, (unsigned)(p->B * a.n_qb));
+    dim3 grid((unsigned)((n_mt + 1) / 2), (unsigned)(p->B * a.n_qb), (unsigned)p->H_kv);
     SPOT_CUDA_TRY(launch_pdl(attn_prefill_tc_kernel, grid, dim3(TA_THREADS), (size_t)TA_SMEM_BYTES, stream, tm_q, tm_k,
                              tm_v, a));
     return SPOT_OK;
