@@ -482,6 +482,19 @@ def run_prefill(args):
         api.spot_select(sp, stream)
         api.spot_sparse_attn_prefill(ap, stream)
     barrier()
+    # the selector GEMM kernel alone (spot_score_blocks = a1' only), live, for the roofline object -- timed BEFORE the
+    # long step loop: its denominator is the burst peak of a kernel timed alone (B200_PROFILING.md), and tens of ms of
+    # attention per step push the part into its power cap
+    sc = []
+    for i in range(args.steps + 2):
+        flush_l2()
+        a_, b_ = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a_.record(stream)
+        api.spot_score_blocks(sp, stream)
+        b_.record(stream)
+        torch.cuda.synchronize()
+        if i >= 2:
+            sc.append(a_.elapsed_time(b_))
     ev = [[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(args.steps)]
     with ClockSampler(local_rank) as clk:
         for i in range(args.steps):
@@ -496,17 +509,6 @@ def run_prefill(args):
     att_ms = np.array([e[1].elapsed_time(e[2]) for e in ev])
     step_ms = np.array([e[0].elapsed_time(e[2]) for e in ev])
     clocks = clk.summary()
-    # the selector GEMM kernel alone (spot_score_blocks = a1' only), live, for the roofline object
-    sc = []
-    for i in range(args.steps + 2):
-        flush_l2()
-        a_, b_ = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        a_.record(stream)
-        api.spot_score_blocks(sp, stream)
-        b_.record(stream)
-        torch.cuda.synchronize()
-        if i >= 2:
-            sc.append(a_.elapsed_time(b_))
     # dense causal comparator (indices NULL) -- a few iterations only
     apd = api.make_attn_params(Q, K, V, (Hkv * L * D, D, L * D), None, 0, None, None, 0, 1, L, Hq, Hkv, D,
                                q_start=0, blk=64, sm_scale=wl.sm_scale, out=out)
