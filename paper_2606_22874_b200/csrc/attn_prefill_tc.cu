@@ -4,25 +4,27 @@
 //
 // Tensor-bound.  Work item = (sequence, query block, KV head, PAIR of 128-row tiles); rows stack the group's query
 // heads: row = head_in_group * 64 + query, so one K/V tile in shared memory feeds every head of the group.
-//   warp 0 lane 0 : TMA producer.  Q (two [2 d-halves][128 rows][64] tiles) once, then a 4-stage ring of K_j and V_j
-//                   ([2 d-halves][64 keys][64], 16 KiB each, 128-byte swizzle) through rank-5 tensor maps built from
-//                   the caller's element strides.
-//   warp 1 lane 0 : tcgen05.mma issuer.  S_t = Q_t K_j^T (M=128, N=64, 8 k-steps, both operands K-major in shared
-//                   memory) into TMEM; O_t += P_t V_j (M=128, N=128, 4 k-steps) with P_t read from TENSOR MEMORY
-//                   (packed BF16 over the first half of S_t) and V_j used as an MN-major B operand exactly as TMA
-//                   wrote it (no transpose).  Descriptors are built once and advanced by constants: the lone issuing
-//                   thread has nobody to hide its instruction latencies.  The two tiles ping-pong:
+// One iteration covers a PAIR of selected key blocks (128 keys; any two blocks of the list, the last pair may be single).
+//   warp 0 lane 0 : TMA producer.  Q (two [2 d-halves][128 rows][64] tiles) once, then a 2-stage ring of K pairs and V
+//                   pairs ([2 d-halves][128 keys][64], 32 KiB each, 128-byte swizzle; a block is four 8 KiB boxes)
+//                   through rank-5 tensor maps built from the caller's element strides.
+//   warp 1 lane 0 : tcgen05.mma issuer.  S_t = Q_t K^T (M=128, N=128, 8 k-steps, both operands K-major in shared
+//                   memory) into TMEM; O_t += P_t V (M=128, N=128, 8 k-steps) with P_t read from TENSOR MEMORY (packed
+//                   BF16 over the start of S_t) and V used as an MN-major B operand exactly as TMA wrote it (no
+//                   transpose).  Descriptors are built once and advanced by constants: the lone issuing thread has
+//                   nobody to hide its instruction latencies.  The two tiles ping-pong:
 //                       PV0(n)  QK0(n+1)  |  PV1(n)  QK1(n+1)  | ...
-//   warps 4-7, 8-11: softmax of tile 0 / tile 1, one thread per row (TMEM lane = row).  tcgen05.ld of the 64 logits,
-//                   log2-domain online softmax (scale and max-subtraction fused into one FFMA per element) with a
-//                   LAZY rescale of the TMEM-resident O (only when a row's max grows by more than 2^8 since the last
-//                   rescale: P stays <= 256, l and O use the same stale max, so the result is exact), P rounded to
-//                   BF16 and stored back to TMEM (tcgen05.st), mbarrier hand-off.  Named barriers keep the two tiles'
-//                   exp sections alternating.  Epilogue: O / l -> BF16, 256 B per row, optional LSE.
-// TMEM: S_0 | S_1 | O_0 | O_1 = 64 + 64 + 128 + 128 columns.  Grid: (tile pair, query block heaviest-first, KV head) with
-// the KV head slowest, so the CTAs in flight share one head's K/V in L2 (DRAM traffic 25 GB -> see profiles/).
+//   warps 4-7, 8-11: softmax of tile 0 / tile 1, one thread per row (TMEM lane = row).  Two passes of tcgen05.ld over
+//                   the 128 logits (row max, then exp), log2-domain online softmax (scale and max-subtraction fused
+//                   into one FFMA per element) with a LAZY rescale of the TMEM-resident O (only when a row's max grows
+//                   by more than 2^8 since the last rescale: P stays <= 256, l and O use the same stale max, so the
+//                   result is exact), P rounded to BF16 and stored back to TMEM (tcgen05.st), mbarrier hand-off.
+//                   Named barriers keep the two tiles' exp sections alternating.  Epilogue: O / l -> BF16, 256 B per
+//                   row, optional LSE.
+// TMEM: S_0 | S_1 | O_0 | O_1 = 128 + 128 + 128 + 128 columns (all 512).  Grid: (tile pair, query block heaviest-first,
+// KV head) with the KV head slowest, so the CTAs in flight share one head's K/V in L2 (DRAM reads 25 GB -> 0.8 GB).
 // History (cfg5, TFLOP/s): mma.sync 328 -> tcgen05 SS 789 -> fused FFMA 805 -> P in TMEM 826 -> hoisted descriptors
-// 887 -> head-slowest grid 982.
+// 887 -> head-slowest grid 982 -> 128 keys per iteration 1016.
 #include "common.cuh"
 #include "tc100.cuh"
 
@@ -30,10 +32,11 @@ namespace spot {
 
 namespace {
 
-constexpr int TA_STAGES = 4;
+constexpr int TA_STAGES = 2;
 constexpr int TA_THREADS = 12 * 32;
 constexpr uint32_t TA_Q_TILE = 2 * 128 * 128;          // 32 KiB: [2 halves][128 rows][128 B]
-constexpr uint32_t TA_KV_TILE = 2 * 64 * 128;          // 16 KiB: [2 halves][64 keys][128 B]
+constexpr uint32_t TA_KV_TILE = 2 * 128 * 128;         // 32 KiB: [2 halves][128 keys = a PAIR of key blocks][128 B]
+constexpr uint32_t TA_BLK_BYTES = 2 * 64 * 128;        // 16 KiB of K (or V) per 64-key block
 constexpr uint32_t TA_SMEM_TILES = 2 * TA_Q_TILE + TA_STAGES * 2 * TA_KV_TILE;   // 192 KiB
 constexpr uint32_t TA_SMEM_BYTES = 1024 + TA_SMEM_TILES + 256;
 constexpr float TA_RESCALE_THRESHOLD = 8.0f;           // log2 units
@@ -114,70 +117,85 @@ __global__ void __launch_bounds__(TA_THREADS, 1) attn_prefill_tc_kernel(const __
             mbar_arrive_expect_tx(bar_q_full, two ? 2 * TA_Q_TILE : TA_Q_TILE);
             for (int t = 0; t < (two ? 2 : 1); ++t)
                 tma_load_5d(q_smem + t * TA_Q_TILE, &tm_q, bar_q_full, 0, i * 64, hk * G + (2 * pair + t) * 2, 0, b);
-            int n = 0;
-            for (int it = 0; it < budget; ++it) {
-                const int j = block_of(it);
-                if (!visible(j)) continue;
+            // one ring stage = a PAIR of visible key blocks (any two, they need not be adjacent): K pair, then V pair,
+            // each [2 d-halves][128 keys][128 B]; a block is four 8 KiB boxes (K/V x d-half)
+            int n = 0, it = 0;
+            while (true) {
+                int jA = -1, jB = -1;
+                for (; it < budget && jA < 0; ++it) { const int j = block_of(it); if (visible(j)) jA = j; }
+                if (jA < 0) break;
+                for (; it < budget && jB < 0; ++it) { const int j = block_of(it); if (visible(j)) jB = j; }
                 const int s = n % TA_STAGES;
                 mbar_wait(bar_kv_empty + 8 * s, ((n / TA_STAGES) & 1) ^ 1);
                 const uint32_t ks = kv_smem + s * 2 * TA_KV_TILE;
-                mbar_arrive_expect_tx(bar_k_full + 8 * s, TA_KV_TILE);
-                tma_load_5d(ks, &tm_k, bar_k_full + 8 * s, 0, j * 64, 0, hk, b);
-                mbar_arrive_expect_tx(bar_v_full + 8 * s, TA_KV_TILE);
-                tma_load_5d(ks + TA_KV_TILE, &tm_v, bar_v_full + 8 * s, 0, j * 64, 0, hk, b);
+                const uint32_t bytes = (jB >= 0 ? 2 : 1) * TA_BLK_BYTES;
+                mbar_arrive_expect_tx(bar_k_full + 8 * s, bytes);
+                for (int u = 0; u < (jB >= 0 ? 2 : 1); ++u)
+                    for (int hf = 0; hf < 2; ++hf)
+                        tma_load_5d(ks + hf * (128 * 128) + u * (64 * 128), &tm_k, bar_k_full + 8 * s, 0, (u ? jB : jA) * 64,
+                                    hf, hk, b);
+                mbar_arrive_expect_tx(bar_v_full + 8 * s, bytes);
+                for (int u = 0; u < (jB >= 0 ? 2 : 1); ++u)
+                    for (int hf = 0; hf < 2; ++hf)
+                        tma_load_5d(ks + TA_KV_TILE + hf * (128 * 128) + u * (64 * 128), &tm_v, bar_v_full + 8 * s, 0,
+                                    (u ? jB : jA) * 64, hf, hk, b);
                 ++n;
             }
         }
     } else if (warp == 1) {
         // ================================ MMA issuer ================================
         if (lane == 0) {
-            constexpr uint32_t idesc_qk = umma_idesc_bf16(128, 64);
+            constexpr uint32_t idesc_qk128 = umma_idesc_bf16(128, 128), idesc_qk64 = umma_idesc_bf16(128, 64);
             constexpr uint32_t idesc_pv = umma_idesc_bf16(128, 128) | UMMA_B_MN_MAJOR;
             int nv = 0;
             for (int it = 0; it < budget; ++it) nv += visible(block_of(it)) ? 1 : 0;
+            const int np = (nv + 1) >> 1;                 // iterations: pairs of key blocks (the last may be single)
             // One lone thread issues every MMA, with nobody to hide its instruction latencies: descriptors are built
             // once and advanced by compile-time constants (the start-address field is the low 14 bits, in 16-byte
             // units), so each tcgen05.mma costs two integer adds, not a dozen dependent ones.
             const uint64_t qd[2] = {umma_desc_sw128(q_smem), umma_desc_sw128(q_smem + TA_Q_TILE)};
-            auto qk = [&](int t, uint64_t kd) {           // S_t = Q_t K^T
+            auto qk = [&](int t, uint64_t kd, bool full) {     // S_t = Q_t K^T over 128 (or 64) keys
+                const uint32_t idesc = full ? idesc_qk128 : idesc_qk64;
 #pragma unroll
                 for (int kk = 0; kk < 8; ++kk)
-                    umma_bf16_ss(tbase + t * 64, qd[t] + (uint64_t)(((kk >> 2) * (128 * 128) + (kk & 3) * 32) >> 4),
-                                 kd + (uint64_t)(((kk >> 2) * (64 * 128) + (kk & 3) * 32) >> 4), idesc_qk, kk > 0);
+                    umma_bf16_ss(tbase + t * 128, qd[t] + (uint64_t)(((kk >> 2) * (128 * 128) + (kk & 3) * 32) >> 4),
+                                 kd + (uint64_t)(((kk >> 2) * (128 * 128) + (kk & 3) * 32) >> 4), idesc, kk > 0);
                 umma_commit(bar_s_full + 8 * t);
             };
-            auto pv = [&](int t, uint64_t vd, bool acc) { // O_t += P_t V, P_t packed BF16 in the first 32 columns of S_t
+            auto pv = [&](int t, uint64_t vd, bool acc, bool full) {   // O_t += P_t V; P_t packed BF16 over the start of S_t
 #pragma unroll
-                for (int kk = 0; kk < 4; ++kk)
-                    umma_bf16_ts(tbase + 128 + t * 128, tbase + t * 64 + kk * 8, vd + (uint64_t)((kk * 2048) >> 4), idesc_pv,
-                                 acc || kk > 0);
+                for (int kk = 0; kk < 8; ++kk)
+                    if (kk < 4 || full)
+                        umma_bf16_ts(tbase + 256 + t * 128, tbase + t * 128 + kk * 8, vd + (uint64_t)((kk * 2048) >> 4),
+                                     idesc_pv, acc || kk > 0);
                 umma_commit(bar_o_done + 8 * t);
             };
-            if (nv > 0) {
+            if (np > 0) {
                 mbar_wait(bar_q_full, 0);
                 mbar_wait(bar_k_full, 0);
                 tc_fence_after();
                 {
                     const uint64_t kd0 = umma_desc_sw128(kv_smem);
-                    qk(0, kd0);
-                    if (two) qk(1, kd0);
+                    qk(0, kd0, nv >= 2);
+                    if (two) qk(1, kd0, nv >= 2);
                 }
-                for (int n = 0; n < nv; ++n) {
+                for (int n = 0; n < np; ++n) {
                     const int s = n % TA_STAGES, s1 = (n + 1) % TA_STAGES;
-                    const uint64_t vd = umma_desc_sw128_mn(kv_smem + s * 2 * TA_KV_TILE + TA_KV_TILE, 64 * 128, 1024);
+                    const uint64_t vd = umma_desc_sw128_mn(kv_smem + s * 2 * TA_KV_TILE + TA_KV_TILE, 128 * 128, 1024);
                     const uint64_t kd1 = umma_desc_sw128(kv_smem + s1 * 2 * TA_KV_TILE);
-                    const bool more = n + 1 < nv;
+                    const bool more = n + 1 < np;
+                    const bool full = 2 * n + 1 < nv, full1 = 2 * n + 3 < nv;
                     mbar_wait(bar_v_full + 8 * s, (n / TA_STAGES) & 1);
                     if (more) mbar_wait(bar_k_full + 8 * s1, ((n + 1) / TA_STAGES) & 1);
                     mbar_wait(bar_p_full, n & 1);                       // P_0(n) written, S_0 consumed, O_0 rescaled
                     tc_fence_after();
-                    pv(0, vd, n > 0);
-                    if (more) qk(0, kd1);
+                    pv(0, vd, n > 0, full);
+                    if (more) qk(0, kd1, full1);
                     if (two) {
                         mbar_wait(bar_p_full + 8, n & 1);
                         tc_fence_after();
-                        pv(1, vd, n > 0);
-                        if (more) qk(1, kd1);
+                        pv(1, vd, n > 0, full);
+                        if (more) qk(1, kd1, full1);
                     }
                     umma_commit(bar_kv_empty + 8 * s);                  // K(n), V(n) no longer read
                 }
@@ -192,44 +210,53 @@ __global__ void __launch_bounds__(TA_THREADS, 1) attn_prefill_tc_kernel(const __
             const int hg = (2 * pair + t) * 2 + (r >> 6); // head in group
             const int ql = r & 63;                        // query in block
             const bool live = hg < G;
-            const uint32_t t_s = tbase + ((uint32_t)(lq * 32) << 16) + t * 64;
-            const uint32_t t_o = tbase + ((uint32_t)(lq * 32) << 16) + 128 + t * 128;
+            const uint32_t t_s = tbase + ((uint32_t)(lq * 32) << 16) + t * 128;
+            const uint32_t t_o = tbase + ((uint32_t)(lq * 32) << 16) + 256 + t * 128;
             float m_used = -INFINITY, l = 0.f;
-            int n = 0, nv = 0;
-            for (int it = 0; it < budget; ++it) nv += visible(block_of(it)) ? 1 : 0;
-            // The two tiles must run in ANTI-phase (softmax of one while the tensor pipe works for the other).  Left
-            // alone they fall into phase -- both S tiles are ready together, both softmaxes share the MUFU, both
-            // hand back together -- and MUFU time and tensor time add up instead of overlapping (ncu: XU 37 % +
-            // tensor 60 %).  Named barriers 2 / 3 make the exp sections alternate: tile 0, tile 1, tile 0, ...
+            int n = 0, it = 0, np = 0;
+            for (int q = 0; q < budget; ++q) np += visible(block_of(q)) ? 1 : 0;
+            np = (np + 1) >> 1;
+            // The two tiles should run in ANTI-phase (softmax of one while the tensor pipe works for the other); named
+            // barriers 2 / 3 make their exp sections alternate: tile 0, tile 1, tile 0, ...
             if (two && t == 1) asm volatile("bar.arrive 2, 256;" ::: "memory");
-            for (int it = 0; it < budget; ++it) {
-                const int j = block_of(it);
-                if (!visible(j)) continue;
+            while (true) {
+                // this iteration's pair of visible key blocks (the last pair may be single)
+                int jA = -1, jB = -1;
+                for (; it < budget && jA < 0; ++it) { const int j = block_of(it); if (visible(j)) jA = j; }
+                if (jA < 0) break;
+                for (; it < budget && jB < 0; ++it) { const int j = block_of(it); if (visible(j)) jB = j; }
+                const int nh = jB >= 0 ? 2 : 1;
                 mbar_wait(bar_s_full + 8 * t, n & 1);
                 tc_fence_after();
-                float x[64];
-                {
-                    float d0[16], d1[16], d2[16], d3[16];
-                    tmem_ld16(t_s, d0); tmem_ld16(t_s + 16, d1); tmem_ld16(t_s + 32, d2); tmem_ld16(t_s + 48, d3);
-                    tmem_ld_wait();
-#pragma unroll
-                    for (int e = 0; e < 16; ++e) { x[e] = d0[e]; x[16 + e] = d1[e]; x[32 + e] = d2[e]; x[48 + e] = d3[e]; }
-                }
                 if (two) {
                     if (t == 0) asm volatile("bar.sync 2, 256;" ::: "memory");
                     else asm volatile("bar.sync 3, 256;" ::: "memory");
                 }
-                // causal mask inside the diagonal block only (CTA-uniform branch); the row max is taken on the raw
-                // logits (sm_scale > 0) so that scale and max-subtraction fuse into one FFMA per element below
-                if (j == qb_abs) {
+                // pass A: row max of the raw logits (sm_scale > 0), 64 columns at a time; the causal mask applies inside
+                // the diagonal block only
+                float mx = -INFINITY;
+#pragma unroll 1
+                for (int hf = 0; hf < nh; ++hf) {
+                    float x[64];
+                    {
+                        float d0[16], d1[16], d2[16], d3[16];
+                        const uint32_t ta = t_s + hf * 64;
+                        tmem_ld16(ta, d0); tmem_ld16(ta + 16, d1); tmem_ld16(ta + 32, d2); tmem_ld16(ta + 48, d3);
+                        tmem_ld_wait();
 #pragma unroll
-                    for (int e = 0; e < 64; ++e)
-                        if (e > ql) x[e] = -INFINITY;
+                        for (int e = 0; e < 16; ++e) { x[e] = d0[e]; x[16 + e] = d1[e]; x[32 + e] = d2[e]; x[48 + e] = d3[e]; }
+                    }
+                    if ((hf ? jB : jA) == qb_abs) {
+#pragma unroll
+                        for (int e = 0; e < 64; ++e)
+                            if (e > ql) x[e] = -INFINITY;
+                    }
+                    float mxa = fmax3(x[0], x[1], x[2]), mxb = fmax3(x[3], x[4], x[5]);
+#pragma unroll
+                    for (int e = 6; e < 62; e += 4) { mxa = fmax3(mxa, x[e], x[e + 1]); mxb = fmax3(mxb, x[e + 2], x[e + 3]); }
+                    mx = fmaxf(mx, fmax3(fmaxf(mxa, mxb), x[62], x[63]));
                 }
-                float mxa = fmax3(x[0], x[1], x[2]), mxb = fmax3(x[3], x[4], x[5]);
-#pragma unroll
-                for (int e = 6; e < 62; e += 4) { mxa = fmax3(mxa, x[e], x[e + 1]); mxb = fmax3(mxb, x[e + 2], x[e + 3]); }
-                const float mx = fmax3(fmaxf(mxa, mxb), x[62], x[63]) * a.scale_log2;
+                mx *= a.scale_log2;
                 // lazy rescale: keep the stale max unless the row max grew by more than 2^8 (warp-uniform decision,
                 // tcgen05.ld/st are warp-collective)
                 const bool need = mx > m_used + TA_RESCALE_THRESHOLD;
@@ -253,27 +280,45 @@ __global__ void __launch_bounds__(TA_THREADS, 1) attn_prefill_tc_kernel(const __
                         tmem_st_wait();
                     }
                 }
+                // pass B: P = exp2(scale * x - m) (scale and max-subtraction in one FFMA), rounded to BF16 and stored
+                // back to tensor memory over the start of S_t: columns 32 hf .. +31 hold the 64 keys of block hf (the
+                // logits they overwrite have been read; QK_t(n+1), which rewrites S_t, is issued after PV_t(n) and the
+                // tensor pipe runs them in order)
                 float ps0 = 0.f, ps1 = 0.f;
-                uint32_t pk[32];
                 const float neg_m = -m_used;
+#pragma unroll 1
+                for (int hf = 0; hf < nh; ++hf) {
+                    float x[64];
+                    {
+                        float d0[16], d1[16], d2[16], d3[16];
+                        const uint32_t ta = t_s + hf * 64;
+                        tmem_ld16(ta, d0); tmem_ld16(ta + 16, d1); tmem_ld16(ta + 32, d2); tmem_ld16(ta + 48, d3);
+                        tmem_ld_wait();
 #pragma unroll
-                for (int e = 0; e < 64; e += 2) {
-                    const float p0 = fast_exp2(fmaf(x[e], a.scale_log2, neg_m));
-                    const float p1 = fast_exp2(fmaf(x[e + 1], a.scale_log2, neg_m));
-                    ps0 += p0;
-                    ps1 += p1;
-                    pk[e >> 1] = pack_bf16x2(p0, p1);
+                        for (int e = 0; e < 16; ++e) { x[e] = d0[e]; x[16 + e] = d1[e]; x[32 + e] = d2[e]; x[48 + e] = d3[e]; }
+                    }
+                    if ((hf ? jB : jA) == qb_abs) {
+#pragma unroll
+                        for (int e = 0; e < 64; ++e)
+                            if (e > ql) x[e] = -INFINITY;
+                    }
+                    uint32_t pk[32];
+#pragma unroll
+                    for (int e = 0; e < 64; e += 2) {
+                        const float p0 = fast_exp2(fmaf(x[e], a.scale_log2, neg_m));
+                        const float p1 = fast_exp2(fmaf(x[e + 1], a.scale_log2, neg_m));
+                        ps0 += p0;
+                        ps1 += p1;
+                        pk[e >> 1] = pack_bf16x2(p0, p1);
+                    }
+                    tmem_st16u(t_s + hf * 32, pk);
+                    tmem_st16u(t_s + hf * 32 + 16, pk + 16);
                 }
-                const float ps = ps0 + ps1;
                 if (two) {
                     if (t == 0) asm volatile("bar.arrive 3, 256;" ::: "memory");
-                    else if (n + 1 < nv) asm volatile("bar.arrive 2, 256;" ::: "memory");
+                    else if (n + 1 < np) asm volatile("bar.arrive 2, 256;" ::: "memory");
                 }
-                l += ps;
-                // P_t overwrites the first half of S_t (the logits are in registers; QK_t(n+1), which rewrites S_t, is
-                // issued after PV_t(n) and the tensor pipe runs them in order)
-                tmem_st16u(t_s, pk);
-                tmem_st16u(t_s + 16, pk + 16);
+                l += ps0 + ps1;
                 tmem_st_wait();
                 tc_fence_before();
                 mbar_arrive(bar_p_full + 8 * t);
@@ -325,7 +370,7 @@ bool make_map(CUtensorMap* m, const void* base, uint64_t rows, uint64_t row_stri
               uint64_t stride3_elems, uint64_t n4, uint64_t stride4_elems, uint32_t box_rows, uint32_t box3) {
     const uint64_t dims[5] = {64, rows, 2, n3, n4};
     const uint64_t strides[4] = {row_stride_elems * 2, 128, stride3_elems * 2, stride4_elems * 2};
-    const uint32_t box[5] = {64, box_rows, 2, box3, 1};
+    const uint32_t box[5] = {64, box_rows, 1, box3, 1};          // one d-half per box
     return encode_tmap_bf16_sw128(m, base, 5, dims, strides, box);
 }
 
