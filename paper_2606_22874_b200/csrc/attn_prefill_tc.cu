@@ -14,8 +14,9 @@
 //                   transpose).  Descriptors are built once and advanced by constants: the lone issuing thread has
 //                   nobody to hide its instruction latencies.  The two tiles ping-pong:
 //                       PV0(n)  QK0(n+1)  |  PV1(n)  QK1(n+1)  | ...
-//   warps 4-7, 8-11: softmax of tile 0 / tile 1, one thread per row (TMEM lane = row).  Two passes of tcgen05.ld over
-//                   the 128 logits (row max, then exp), log2-domain online softmax (scale and max-subtraction fused
+//   warps 4-7, 8-11: softmax of tile 0 / tile 1, one thread per row (TMEM lane = row).  One optimistic pass over the 128
+//                   logits (exp against the stale max while the new max is found; redone only when a rescale is
+//                   due), log2-domain online softmax (scale and max-subtraction fused
 //                   into one FFMA per element) with a LAZY rescale of the TMEM-resident O (only when a row's max grows
 //                   by more than 2^8 since the last rescale: P stays <= 256, l and O use the same stale max, so the
 //                   result is exact), P rounded to BF16 and stored back to TMEM (tcgen05.st), mbarrier hand-off.
@@ -24,7 +25,7 @@
 // TMEM: S_0 | S_1 | O_0 | O_1 = 128 + 128 + 128 + 128 columns (all 512).  Grid: (tile pair, query block heaviest-first,
 // KV head) with the KV head slowest, so the CTAs in flight share one head's K/V in L2 (DRAM reads 25 GB -> 0.8 GB).
 // History (cfg5, TFLOP/s): mma.sync 328 -> tcgen05 SS 789 -> fused FFMA 805 -> P in TMEM 826 -> hoisted descriptors
-// 887 -> head-slowest grid 982 -> 128 keys per iteration 1016.
+// 887 -> head-slowest grid 982 -> 128 keys per iteration 1016 -> optimistic single-pass softmax 1069.
 #include "common.cuh"
 #include "tc100.cuh"
 
@@ -232,35 +233,51 @@ __global__ void __launch_bounds__(TA_THREADS, 1) attn_prefill_tc_kernel(const __
                     if (t == 0) asm volatile("bar.sync 2, 256;" ::: "memory");
                     else asm volatile("bar.sync 3, 256;" ::: "memory");
                 }
-                // pass A: row max of the raw logits (sm_scale > 0), 64 columns at a time; the causal mask applies inside
-                // the diagonal block only
-                float mx = -INFINITY;
-#pragma unroll 1
-                for (int hf = 0; hf < nh; ++hf) {
-                    float x[64];
-                    {
-                        float d0[16], d1[16], d2[16], d3[16];
-                        const uint32_t ta = t_s + hf * 64;
-                        tmem_ld16(ta, d0); tmem_ld16(ta + 16, d1); tmem_ld16(ta + 32, d2); tmem_ld16(ta + 48, d3);
-                        tmem_ld_wait();
+                // Optimistic single pass: exp2 against the STALE max while the row max of this pair is being found (sm_scale
+                // > 0: max on the raw logits; scale and max-subtraction are one FFMA).  P = exp2(scale x - m) rounded to
+                // BF16 waits in registers.  Only if some row's max grew by more than 2^8 since its last rescale (always
+                // in the first iteration, rarely later) is the pair redone after rescaling O -- P stays <= 256, and l
+                // and O always use the same max, so the result is exact.  The causal mask applies inside the diagonal
+                // block only.
+                uint32_t pk[64];
+                float ps0 = 0.f, ps1 = 0.f, mx = -INFINITY;
+                {
+                    const float neg_m = -m_used;
 #pragma unroll
-                        for (int e = 0; e < 16; ++e) { x[e] = d0[e]; x[16 + e] = d1[e]; x[32 + e] = d2[e]; x[48 + e] = d3[e]; }
+                    for (int hf = 0; hf < 2; ++hf) {
+                        if (hf < nh) {
+                            float x[64];
+                            {
+                                float d0[16], d1[16], d2[16], d3[16];
+                                const uint32_t ta = t_s + hf * 64;
+                                tmem_ld16(ta, d0); tmem_ld16(ta + 16, d1); tmem_ld16(ta + 32, d2); tmem_ld16(ta + 48, d3);
+                                tmem_ld_wait();
+#pragma unroll
+                                for (int e = 0; e < 16; ++e) { x[e] = d0[e]; x[16 + e] = d1[e]; x[32 + e] = d2[e]; x[48 + e] = d3[e]; }
+                            }
+                            if ((hf ? jB : jA) == qb_abs) {
+#pragma unroll
+                                for (int e = 0; e < 64; ++e)
+                                    if (e > ql) x[e] = -INFINITY;
+                            }
+                            float mxa = fmax3(x[0], x[1], x[2]), mxb = fmax3(x[3], x[4], x[5]);
+#pragma unroll
+                            for (int e = 6; e < 62; e += 4) { mxa = fmax3(mxa, x[e], x[e + 1]); mxb = fmax3(mxb, x[e + 2], x[e + 3]); }
+                            mx = fmaxf(mx, fmax3(fmaxf(mxa, mxb), x[62], x[63]));
+#pragma unroll
+                            for (int e = 0; e < 64; e += 2) {
+                                const float p0 = fast_exp2(fmaf(x[e], a.scale_log2, neg_m));
+                                const float p1 = fast_exp2(fmaf(x[e + 1], a.scale_log2, neg_m));
+                                ps0 += p0;
+                                ps1 += p1;
+                                pk[hf * 32 + (e >> 1)] = pack_bf16x2(p0, p1);
+                            }
+                        }
                     }
-                    if ((hf ? jB : jA) == qb_abs) {
-#pragma unroll
-                        for (int e = 0; e < 64; ++e)
-                            if (e > ql) x[e] = -INFINITY;
-                    }
-                    float mxa = fmax3(x[0], x[1], x[2]), mxb = fmax3(x[3], x[4], x[5]);
-#pragma unroll
-                    for (int e = 6; e < 62; e += 4) { mxa = fmax3(mxa, x[e], x[e + 1]); mxb = fmax3(mxb, x[e + 2], x[e + 3]); }
-                    mx = fmaxf(mx, fmax3(fmaxf(mxa, mxb), x[62], x[63]));
                 }
                 mx *= a.scale_log2;
-                // lazy rescale: keep the stale max unless the row max grew by more than 2^8 (warp-uniform decision,
-                // tcgen05.ld/st are warp-collective)
-                const bool need = mx > m_used + TA_RESCALE_THRESHOLD;
-                if (__any_sync(0xffffffffu, need)) {
+                const bool need = mx > m_used + TA_RESCALE_THRESHOLD;       // (true for every row while m_used = -inf)
+                if (__any_sync(0xffffffffu, need)) {                         // warp-uniform: tcgen05.ld/st are collective
                     const float m_new = need ? mx : m_used;
                     const float alpha = (m_used == -INFINITY) ? 0.f : fast_exp2(m_used - m_new);   // 1 when !need
                     l *= alpha;
@@ -279,40 +296,43 @@ __global__ void __launch_bounds__(TA_THREADS, 1) attn_prefill_tc_kernel(const __
                         }
                         tmem_st_wait();
                     }
-                }
-                // pass B: P = exp2(scale * x - m) (scale and max-subtraction in one FFMA), rounded to BF16 and stored
-                // back to tensor memory over the start of S_t: columns 32 hf .. +31 hold the 64 keys of block hf (the
-                // logits they overwrite have been read; QK_t(n+1), which rewrites S_t, is issued after PV_t(n) and the
-                // tensor pipe runs them in order)
-                float ps0 = 0.f, ps1 = 0.f;
-                const float neg_m = -m_used;
+                    // redo the pair against the new max (S_t is still intact: P has not been stored yet)
+                    ps0 = ps1 = 0.f;
+                    const float neg_m = -m_used;
+#pragma unroll
+                    for (int hf = 0; hf < 2; ++hf) {
+                        if (hf < nh) {
+                            const bool dg = (hf ? jB : jA) == qb_abs;
 #pragma unroll 1
-                for (int hf = 0; hf < nh; ++hf) {
-                    float x[64];
-                    {
-                        float d0[16], d1[16], d2[16], d3[16];
-                        const uint32_t ta = t_s + hf * 64;
-                        tmem_ld16(ta, d0); tmem_ld16(ta + 16, d1); tmem_ld16(ta + 32, d2); tmem_ld16(ta + 48, d3);
-                        tmem_ld_wait();
+                            for (int c16 = 0; c16 < 4; ++c16) {
+                                float d[16];
+                                tmem_ld16(t_s + hf * 64 + c16 * 16, d);
+                                tmem_ld_wait();
 #pragma unroll
-                        for (int e = 0; e < 16; ++e) { x[e] = d0[e]; x[16 + e] = d1[e]; x[32 + e] = d2[e]; x[48 + e] = d3[e]; }
-                    }
-                    if ((hf ? jB : jA) == qb_abs) {
+                                for (int e = 0; e < 16; e += 2) {
+                                    const float x0 = (dg && c16 * 16 + e > ql) ? -INFINITY : d[e];
+                                    const float x1 = (dg && c16 * 16 + e + 1 > ql) ? -INFINITY : d[e + 1];
+                                    const float p0 = fast_exp2(fmaf(x0, a.scale_log2, neg_m));
+                                    const float p1 = fast_exp2(fmaf(x1, a.scale_log2, neg_m));
+                                    ps0 += p0;
+                                    ps1 += p1;
+                                    const uint32_t w = pack_bf16x2(p0, p1);
+                                    // pk[hf * 32 + c16 * 8 + e / 2] with c16 a loop variable: select statically
 #pragma unroll
-                        for (int e = 0; e < 64; ++e)
-                            if (e > ql) x[e] = -INFINITY;
+                                    for (int q = 0; q < 4; ++q)
+                                        if (q == c16) pk[hf * 32 + q * 8 + (e >> 1)] = w;
+                                }
+                            }
+                        }
                     }
-                    uint32_t pk[32];
-#pragma unroll
-                    for (int e = 0; e < 64; e += 2) {
-                        const float p0 = fast_exp2(fmaf(x[e], a.scale_log2, neg_m));
-                        const float p1 = fast_exp2(fmaf(x[e + 1], a.scale_log2, neg_m));
-                        ps0 += p0;
-                        ps1 += p1;
-                        pk[e >> 1] = pack_bf16x2(p0, p1);
-                    }
-                    tmem_st16u(t_s + hf * 32, pk);
-                    tmem_st16u(t_s + hf * 32 + 16, pk + 16);
+                }
+                // P goes back to tensor memory over the start of S_t: columns 32 hf .. +31 hold the 64 keys of block hf
+                // (QK_t(n+1), which rewrites S_t, is issued after PV_t(n) and the tensor pipe runs them in order)
+                tmem_st16u(t_s, pk);
+                tmem_st16u(t_s + 16, pk + 16);
+                if (nh == 2) {
+                    tmem_st16u(t_s + 32, pk + 32);
+                    tmem_st16u(t_s + 48, pk + 48);
                 }
                 if (two) {
                     if (t == 0) asm volatile("bar.arrive 3, 256;" ::: "memory");
