@@ -20,12 +20,12 @@
 //                   into one FFMA per element) with a LAZY rescale of the TMEM-resident O (only when a row's max grows
 //                   by more than 2^8 since the last rescale: P stays <= 256, l and O use the same stale max, so the
 //                   result is exact), P rounded to BF16 and stored back to TMEM (tcgen05.st), mbarrier hand-off.
-//                   Named barriers keep the two tiles' exp sections alternating.  Epilogue: O / l -> BF16, 256 B per
-//                   row, optional LSE.
+//                   Epilogue: O / l -> BF16, 256 B per row, optional LSE.  (Named barriers that forced the two tiles'
+//                   exp sections to alternate were measured and dropped: 1069 vs 1096 TFLOP/s without.)
 // TMEM: S_0 | S_1 | O_0 | O_1 = 128 + 128 + 128 + 128 columns (all 512).  Grid: (tile pair, query block heaviest-first,
 // KV head) with the KV head slowest, so the CTAs in flight share one head's K/V in L2 (DRAM reads 25 GB -> 0.8 GB).
 // History (cfg5, TFLOP/s): mma.sync 328 -> tcgen05 SS 789 -> fused FFMA 805 -> P in TMEM 826 -> hoisted descriptors
-// 887 -> head-slowest grid 982 -> 128 keys per iteration 1016 -> optimistic single-pass softmax 1069.
+// 887 -> head-slowest grid 982 -> 128 keys per iteration 1016 -> optimistic single-pass softmax 1069 -> no ordering barriers 1096.
 #include "common.cuh"
 #include "tc100.cuh"
 
@@ -214,12 +214,7 @@ __global__ void __launch_bounds__(TA_THREADS, 1) attn_prefill_tc_kernel(const __
             const uint32_t t_s = tbase + ((uint32_t)(lq * 32) << 16) + t * 128;
             const uint32_t t_o = tbase + ((uint32_t)(lq * 32) << 16) + 256 + t * 128;
             float m_used = -INFINITY, l = 0.f;
-            int n = 0, it = 0, np = 0;
-            for (int q = 0; q < budget; ++q) np += visible(block_of(q)) ? 1 : 0;
-            np = (np + 1) >> 1;
-            // The two tiles should run in ANTI-phase (softmax of one while the tensor pipe works for the other); named
-            // barriers 2 / 3 make their exp sections alternate: tile 0, tile 1, tile 0, ...
-            if (two && t == 1) asm volatile("bar.arrive 2, 256;" ::: "memory");
+            int n = 0, it = 0;
             while (true) {
                 // this iteration's pair of visible key blocks (the last pair may be single)
                 int jA = -1, jB = -1;
@@ -229,10 +224,6 @@ __global__ void __launch_bounds__(TA_THREADS, 1) attn_prefill_tc_kernel(const __
                 const int nh = jB >= 0 ? 2 : 1;
                 mbar_wait(bar_s_full + 8 * t, n & 1);
                 tc_fence_after();
-                if (two) {
-                    if (t == 0) asm volatile("bar.sync 2, 256;" ::: "memory");
-                    else asm volatile("bar.sync 3, 256;" ::: "memory");
-                }
                 // Optimistic single pass: exp2 against the STALE max while the row max of this pair is being found (sm_scale
                 // > 0: max on the raw logits; scale and max-subtraction are one FFMA).  P = exp2(scale x - m) rounded to
                 // BF16 waits in registers.  Only if some row's max grew by more than 2^8 since its last rescale (always
@@ -333,10 +324,6 @@ __global__ void __launch_bounds__(TA_THREADS, 1) attn_prefill_tc_kernel(const __
                 if (nh == 2) {
                     tmem_st16u(t_s + 32, pk + 32);
                     tmem_st16u(t_s + 48, pk + 48);
-                }
-                if (two) {
-                    if (t == 0) asm volatile("bar.arrive 3, 256;" ::: "memory");
-                    else if (n + 1 < np) asm volatile("bar.arrive 2, 256;" ::: "memory");
                 }
                 l += ps0 + ps1;
                 tmem_st_wait();
