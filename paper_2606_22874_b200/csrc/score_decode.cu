@@ -114,11 +114,12 @@ struct ScoreCfg {
     // has not completed yet, and a parity wait cannot tell those apart.
     // 4-bit (self-serve ring): many small tiles (8.5 / 17 KiB) and an ALU-heavy unpack.  A single producer lane cannot
     // issue a copy per ~350 cycles, so every consumer warp owns PER_WARP stages and refills a stage itself as soon as
-    // it has consumed it: no producer warp, no empty barriers.
+    // it has consumed it: no producer warp, no empty barriers.  The unpack's dependent chains want warps more than
+    // ring depth: 12 warps x 2 stages beat 8 x 3 (MXFP4 20 -> 17 us); 16 warps x 3 half-tile stages were slower again.
     static constexpr int STAGE_BYTES = SELF ? TILE_BYTES : (TILE_BYTES + 1023) / 1024 * 1024;
     static constexpr int STAGES_RAW = SC_SMEM_BUDGET / STAGE_BYTES;
-    static constexpr int CONSUMERS = SELF ? (TILE_BYTES <= 8704 ? 8 : 6) : (STAGES_RAW > 6 ? 6 : STAGES_RAW);
-    static constexpr int PER_WARP = SELF ? (TILE_BYTES <= 8704 ? 3 : 2) : 1;
+    static constexpr int CONSUMERS = SELF ? (TILE_BYTES <= 8704 ? 12 : 6) : (STAGES_RAW > 6 ? 6 : STAGES_RAW);
+    static constexpr int PER_WARP = SELF ? 2 : 1;
     static constexpr int STAGES = CONSUMERS * PER_WARP;
     static constexpr int THREADS = (CONSUMERS + (SELF ? 0 : 1)) * 32;
     static_assert(STAGES * STAGE_BYTES <= 208 * 1024, "ring geometry");
