@@ -79,7 +79,11 @@ __global__ void __launch_bounds__(ATT_WARPS * 32, 2) attn_decode_kernel(AttnArgs
     long long U = 0;
     for (int bb = 0; bb < a.B; ++bb) U += seq_blocks(a, bb);
     U *= a.H_kv;
-    const long long u0 = (long long)blockIdx.x * U / gridDim.x, u1 = (long long)(blockIdx.x + 1) * U / gridDim.x;
+    // with fewer units than CTAs only the first U CTAs work (one unit each): every working CTA owns >= 1 unit, which
+    // is what lets the merge kernel skip per-CTA emptiness checks
+    const long long n_eff = U < (long long)gridDim.x ? U : (long long)gridDim.x;
+    if ((long long)blockIdx.x >= n_eff) return;
+    const long long u0 = (long long)blockIdx.x * U / n_eff, u1 = (long long)(blockIdx.x + 1) * U / n_eff;
     if (u0 >= u1) return;
     int b = 0, nb = seq_blocks(a, 0);
     long long base = 0;
@@ -283,15 +287,11 @@ __global__ void __launch_bounds__(MERGE_WARPS * 32) attn_merge_kernel(AttnArgs a
         return;
     }
     const long long us = before * a.H_kv + (long long)hk * nb, ue = us + nb;
-    const int n = a.n_ctas;
+    const long long n = U < (long long)a.n_ctas ? U : (long long)a.n_ctas;     // working CTAs (same rule as the kernel)
     const int c_first = (int)(((us + 1) * n - 1) / U), c_last = (int)((ue * n - 1) / U);
     const int64_t seg = (int64_t)b * a.H_kv + hk;
-    // with more CTAs than units some ranges are empty: those CTAs wrote nothing
-    const bool all_live = U >= n;       // (64-bit divisions are slow: only the tiny-problem case pays for them)
-    auto live = [&](int cc) -> bool { return all_live || (long long)cc * U / n < (long long)(cc + 1) * U / n; };
     float M = -INFINITY;
-    for (int cc = c_first + lane; cc <= c_last; cc += 32)
-        if (live(cc)) M = fmaxf(M, a.part_ml[((cc + seg) * G + r) * 2]);
+    for (int cc = c_first + lane; cc <= c_last; cc += 32) M = fmaxf(M, a.part_ml[((cc + seg) * G + r) * 2]);
 #pragma unroll
     for (int o = 16; o; o >>= 1) M = fmaxf(M, __shfl_xor_sync(0xffffffffu, M, o));
     const float Mu = (M == -INFINITY) ? 0.f : M;
@@ -299,7 +299,6 @@ __global__ void __launch_bounds__(MERGE_WARPS * 32) attn_merge_kernel(AttnArgs a
     float lsum = 0.f;
 #pragma unroll 4
     for (int cc = c_first; cc <= c_last; ++cc) {
-        if (!live(cc)) continue;
         const int64_t pr = (cc + seg) * G + r;
         const float2 ml = *reinterpret_cast<const float2*>(a.part_ml + pr * 2);
         const float4 o = *reinterpret_cast<const float4*>(a.part_o + pr * ATT_D + lane * 4);
