@@ -1,5 +1,5 @@
 // Step a2, histogram-partition form (rows with n_b <= 2048) -- reserved tier, residual softmax (Eq. 7), nucleus +
-// K_min floor (Eq. 8) or static top-K (Eq. 6), one CTA of 256 threads per selection row.
+// K_min floor (Eq. 8) or static top-K (Eq. 6), one CTA of 1024 threads x 2 keys (decode) or 256 threads x 8 keys (prefill) per selection row.
 //
 // The rule only needs (a) the mass in front of the cut and (b) the key value tau at the cut, not a full sort.  So:
 //   1. keys (order-preserving 32-bit images of the scores, ascending key = descending score) go into 2048 bins by a
@@ -15,19 +15,18 @@
 //      the count is reached (R7), and the ascending index list falls out of a ballot/popc scan in index order.
 // exp, normalisation and the running mass are fp64 (the fp32 block score is then the only source of disagreement
 // with the fp64 oracle).  ~12 CTA barriers and 2300 instructions per warp instead of a 66-step
-// bitonic network and 3400; the launch is 13.9 us against 14.1 us at n_b = 2048 all the same, because a kernel that
-// runs once per step on 4 SMs from cold caches is bound by instruction fetch (stall reason no_instruction 3.6 cycles
-// per issue) and two dependent DRAM misses, not by its instruction count: profiles/r1_decode_cfg3_launches.md, D.
+// bitonic network and 3400.  With 256 threads x 8 keys the launch was 13.9 us against 14.1 us at n_b = 2048 all the same:
+// a kernel that runs once per step on 4 SMs from cold caches is a chain of latencies (instruction fetch, two dependent
+// DRAM misses, eight sequential fp64 exps per thread), not of work.  1024 threads x 2 keys shorten every per-thread
+// section: decode step 172.6 -> 169 us (profiles/r1_decode_cfg3_launches.md, D).
 #include "select_common.cuh"
 
 namespace spot {
 
 namespace {
 
-constexpr int SH_T = 256;
-constexpr int SH_N = 2048;          // keys per row (8 per thread)
+constexpr int SH_N = 2048;          // keys per row
 constexpr int SH_NBIN = 2048;
-constexpr int SH_WARPS = SH_T / 32;
 
 struct BinMap {
     uint32_t kmn;
@@ -66,14 +65,19 @@ __device__ __forceinline__ void warp_resolve(const uint32_t* s_k, const double* 
     tau = __shfl_sync(0xffffffffu, k, src);
 }
 
-__global__ void __launch_bounds__(SH_T) select_hist_kernel(SelectArgs a) {
+// E keys per thread, SH_N / E threads: decode rows (a handful of CTAs, pure latency) run 1024 threads x 2 keys so that
+// every per-thread section (two fp64 exps instead of eight, ...) is short; prefill rows (a thousand CTAs, throughput) run
+// 256 threads x 8 keys.
+template <int SH_E>
+__global__ void __launch_bounds__(SH_N / SH_E) select_hist_kernel(SelectArgs a) {
+    constexpr int SH_T = SH_N / SH_E, SH_WARPS = SH_T / 32;
     __shared__ uint32_t s_cnt[SH_NBIN];       // bin counts, then exclusive starts
     __shared__ double s_e[SH_N];              // masses grouped by bin
     __shared__ uint32_t s_k[SH_N];            // keys grouped by bin
     __shared__ double s_wd[SH_WARPS];
     __shared__ uint32_t s_wu[SH_WARPS][2];
     __shared__ int s_wi[SH_WARPS][2];
-    __shared__ int s_seg[SH_T / 4][2];
+    __shared__ int s_seg[SH_N / 32][2];
     __shared__ double s_base;
     __shared__ uint32_t s_tau;
     __shared__ int s_nin, s_tot[2];
@@ -91,20 +95,20 @@ __global__ void __launch_bounds__(SH_T) select_hist_kernel(SelectArgs a) {
     const int rec_beg = max(sink_end, n_b - a.rec);     // residual blocks: [sink_end, rec_beg)
     const int n_res = rec_beg - sink_end;
     const int n_reserved = n_b - n_res;
-    const int ebase = warp * 256 + lane;                // block of register r: ebase + 32 r
+    const int ebase = warp * (32 * SH_E) + lane;                // block of register r: ebase + 32 r
     const bool topp = a.mode != SPOT_MODE_TOPK;
 
     // ---- load: block scores -> keys; key range of the residual blocks
     const float* srow = a.scores + (int64_t)row * a.nb_stride;
-    uint32_t okey[8];
+    uint32_t okey[SH_E];
     uint32_t kmn = 0xffffffffu, kmx = 0u;
 #pragma unroll
-    for (int r = 0; r < 8; ++r) {
+    for (int r = 0; r < SH_E; ++r) {
         const int j = ebase + 32 * r;
         const bool resid = j >= sink_end && j < rec_beg;
         okey[r] = resid ? score_key(srow[j]) : KEY_PAD;
         if (resid) { kmn = min(kmn, okey[r]); kmx = max(kmx, okey[r]); }
-        s_cnt[tid * 8 + r] = 0u;
+        s_cnt[tid * SH_E + r] = 0u;
     }
     kmn = __reduce_min_sync(0xffffffffu, kmn);
     kmx = __reduce_max_sync(0xffffffffu, kmx);
@@ -116,9 +120,9 @@ __global__ void __launch_bounds__(SH_T) select_hist_kernel(SelectArgs a) {
 
     int n_take = 0;
     uint32_t tau = 0u;
-    double e[8], total = 0.0;
+    double e[SH_E], total = 0.0;
 #pragma unroll
-    for (int r = 0; r < 8; ++r) e[r] = 0.0;
+    for (int r = 0; r < SH_E; ++r) e[r] = 0.0;
 
     if (n_res > 0) {
         BinMap bin_of;
@@ -129,13 +133,13 @@ __global__ void __launch_bounds__(SH_T) select_hist_kernel(SelectArgs a) {
         // (one rolled loop -- the fp64 exp is ~150 instructions and this kernel runs once per step from a cold
         // instruction cache: code size, not instruction count, is what its latency is made of.  The arrays stay in
         // registers: every trip works on element 0 and rotates.)
-        uint32_t pk[8];                                   // bin << 12 | rank inside the bin; 0xffffffff: not residual
+        uint32_t pk[SH_E];                                   // bin << 12 | rank inside the bin; 0xffffffff: not residual
         {
-            uint32_t kq[8];
+            uint32_t kq[SH_E];
 #pragma unroll
-            for (int r = 0; r < 8; ++r) { kq[r] = okey[r]; pk[r] = 0xffffffffu; }
+            for (int r = 0; r < SH_E; ++r) { kq[r] = okey[r]; pk[r] = 0xffffffffu; }
 #pragma unroll 1
-            for (int r = 0; r < 8; ++r) {
+            for (int r = 0; r < SH_E; ++r) {
                 const int j = ebase + 32 * r;
                 double ev = 0.0;
                 uint32_t pv = 0xffffffffu;
@@ -145,17 +149,17 @@ __global__ void __launch_bounds__(SH_T) select_hist_kernel(SelectArgs a) {
                     pv = ((uint32_t)bn << 12) | atomicAdd(&s_cnt[bn], 1u);
                 }
 #pragma unroll
-                for (int u = 0; u < 7; ++u) { kq[u] = kq[u + 1]; e[u] = e[u + 1]; pk[u] = pk[u + 1]; }
-                e[7] = ev;
-                pk[7] = pv;
+                for (int u = 0; u < SH_E - 1; ++u) { kq[u] = kq[u + 1]; e[u] = e[u + 1]; pk[u] = pk[u + 1]; }
+                e[SH_E - 1] = ev;
+                pk[SH_E - 1] = pv;
             }
         }
         __syncthreads();
         // ---- exclusive scan of the bin counts: thread t owns bins 8t .. 8t+7
         {
-            uint32_t c[8], run = 0;
+            uint32_t c[SH_E], run = 0;
 #pragma unroll
-            for (int u = 0; u < 8; ++u) { c[u] = s_cnt[tid * 8 + u]; run += c[u]; }
+            for (int u = 0; u < SH_E; ++u) { c[u] = s_cnt[tid * SH_E + u]; run += c[u]; }
             uint32_t inc = run;
 #pragma unroll
             for (int o = 1; o < 32; o <<= 1) {
@@ -168,12 +172,12 @@ __global__ void __launch_bounds__(SH_T) select_hist_kernel(SelectArgs a) {
 #pragma unroll
             for (int w = 0; w < SH_WARPS; ++w) off += (w < warp) ? (uint32_t)s_wi[w][0] : 0u;
 #pragma unroll
-            for (int u = 0; u < 8; ++u) { s_cnt[tid * 8 + u] = off; off += c[u]; }
+            for (int u = 0; u < SH_E; ++u) { s_cnt[tid * SH_E + u] = off; off += c[u]; }
         }
         __syncthreads();
         // ---- counting-sort scatter: grouped by bin, bins in rank order
 #pragma unroll
-        for (int r = 0; r < 8; ++r)
+        for (int r = 0; r < SH_E; ++r)
             if (pk[r] != 0xffffffffu) {
                 const int pos = (int)s_cnt[pk[r] >> 12] + (int)(pk[r] & 0xfffu);
                 s_k[pos] = okey[r];
@@ -183,14 +187,14 @@ __global__ void __launch_bounds__(SH_T) select_hist_kernel(SelectArgs a) {
         // ---- what has to be resolved exactly: up to two queries against one bin each, run by ONE copy of the code
         //      query 0 (dual top-p, p < 1): the bin holding the cut of the running mass -> n*, tau
         //      query 1 (top-K, K_min floor): the key of rank n_take - 1
-        double target = 0.0, off = 0.0, c[8];
+        double target = 0.0, off = 0.0, c[SH_E];
         int n_lt = 0;
         if (topp) {
             // running mass in grouped order: thread t owns positions 8t .. 8t+7
             double run = 0.0;
 #pragma unroll
-            for (int u = 0; u < 8; ++u) {
-                const int pos = tid * 8 + u;
+            for (int u = 0; u < SH_E; ++u) {
+                const int pos = tid * SH_E + u;
                 run += pos < n_res ? s_e[pos] : 0.0;
                 c[u] = run;
             }
@@ -211,7 +215,7 @@ __global__ void __launch_bounds__(SH_T) select_hist_kernel(SelectArgs a) {
             target = a.p * total;
             int cnt = 0;
 #pragma unroll
-            for (int u = 0; u < 8; ++u) cnt += (tid * 8 + u < n_res && off + c[u] < target) ? 1 : 0;
+            for (int u = 0; u < SH_E; ++u) cnt += (tid * SH_E + u < n_res && off + c[u] < target) ? 1 : 0;
             cnt = __reduce_add_sync(0xffffffffu, cnt);
             if (lane == 0) s_wi[warp][1] = cnt;
             __syncthreads();
@@ -220,7 +224,7 @@ __global__ void __launch_bounds__(SH_T) select_hist_kernel(SelectArgs a) {
             n_take = n_res;                                   // p >= 1: all of B_res by definition (R20)
         } else {
 #pragma unroll
-            for (int u = 0; u < 8; ++u) c[u] = 0.0;
+            for (int u = 0; u < SH_E; ++u) c[u] = 0.0;
             n_take = min(max(0, a.top_k - n_reserved), n_res);
         }
         bool have_tau = false;
@@ -235,10 +239,10 @@ __global__ void __launch_bounds__(SH_T) select_hist_kernel(SelectArgs a) {
             const int sB = (int)s_cnt[B];
             const int cB = (B + 1 < SH_NBIN ? (int)s_cnt[B + 1] : n_res) - sB;
             const int want = n_take - 1 - sB;
-            if (by_mass && sB > 0 && tid == ((sB - 1) >> 3)) {   // running mass in front of the bin: its owner publishes it
+            if (by_mass && sB > 0 && tid == ((sB - 1) / SH_E)) {   // running mass in front of the bin: its owner publishes it
                 double v = c[0];
 #pragma unroll
-                for (int u = 1; u < 8; ++u) v = (((sB - 1) & 7) == u) ? c[u] : v;
+                for (int u = 1; u < SH_E; ++u) v = (((sB - 1) % SH_E) == u) ? c[u] : v;
                 s_base = off + v;
             }
             __syncthreads();
@@ -325,11 +329,11 @@ __global__ void __launch_bounds__(SH_T) select_hist_kernel(SelectArgs a) {
     __syncthreads();
 
     // ---- index order: A = reserved or strictly better than tau (certainly selected), Tt = tied with tau
-    constexpr int NSEG = SH_T / 4;                       // 32-block segments: (warp, register)
-    int prefA[8], prefT[8];
+    constexpr int NSEG = SH_N / 32;                       // 32-block segments: (warp, register)
+    int prefA[SH_E], prefT[SH_E];
     uint32_t isA = 0, isT = 0;
 #pragma unroll
-    for (int r = 0; r < 8; ++r) {
+    for (int r = 0; r < SH_E; ++r) {
         const int j = ebase + 32 * r;
         const bool resid = j >= sink_end && j < rec_beg;
         const bool fa = (j < n_b && !resid) || (resid && n_take > 0 && okey[r] < tau);
@@ -340,7 +344,7 @@ __global__ void __launch_bounds__(SH_T) select_hist_kernel(SelectArgs a) {
         prefT[r] = __popc(bt & lt);
         isA |= (uint32_t)fa << r;
         isT |= (uint32_t)ft << r;
-        if (lane == 0) { s_seg[warp * 8 + r][0] = __popc(ba); s_seg[warp * 8 + r][1] = __popc(bt); }
+        if (lane == 0) { s_seg[warp * SH_E + r][0] = __popc(ba); s_seg[warp * SH_E + r][1] = __popc(bt); }
     }
     __syncthreads();
     if (warp == 0) {
@@ -374,10 +378,10 @@ __global__ void __launch_bounds__(SH_T) select_hist_kernel(SelectArgs a) {
     const int total_sel = total_A + min(total_T, max(need, 0));
     int32_t* out = a.indices + (int64_t)row * a.cap;
 #pragma unroll
-    for (int r = 0; r < 8; ++r) {
+    for (int r = 0; r < SH_E; ++r) {
         const int j = ebase + 32 * r;
-        const int a_before = s_seg[warp * 8 + r][0] + prefA[r];
-        const int t_before = s_seg[warp * 8 + r][1] + prefT[r];
+        const int a_before = s_seg[warp * SH_E + r][0] + prefA[r];
+        const int t_before = s_seg[warp * SH_E + r][1] + prefT[r];
         int pos = -1;
         if ((isA >> r) & 1u) pos = a_before + min(t_before, need);
         else if (((isT >> r) & 1u) && t_before < need) pos = a_before + t_before;
@@ -390,7 +394,7 @@ __global__ void __launch_bounds__(SH_T) select_hist_kernel(SelectArgs a) {
         float* pr = a.probs + (int64_t)row * a.nb_stride;
         const double inv_total = total > 0.0 ? 1.0 / total : 0.0;
 #pragma unroll
-        for (int r = 0; r < 8; ++r) {
+        for (int r = 0; r < SH_E; ++r) {
             const int j = ebase + 32 * r;
             if (j < n_b) pr[j] = (float)(e[r] * inv_total);      // 0 on reserved blocks and in top-K mode
         }
@@ -400,7 +404,8 @@ __global__ void __launch_bounds__(SH_T) select_hist_kernel(SelectArgs a) {
 }  // namespace
 
 spot_status launch_select_hist(const SelectArgs& a, int rows, cudaStream_t s) {
-    SPOT_CUDA_TRY(launch_pdl(select_hist_kernel, dim3((unsigned)rows), dim3(SH_T), 0, s, a));
+    if (rows <= 32) SPOT_CUDA_TRY(launch_pdl(select_hist_kernel<2>, dim3((unsigned)rows), dim3(SH_N / 2), 0, s, a));
+    else SPOT_CUDA_TRY(launch_pdl(select_hist_kernel<8>, dim3((unsigned)rows), dim3(SH_N / 8), 0, s, a));
     return SPOT_OK;
 }
 
