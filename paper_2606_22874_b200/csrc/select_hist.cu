@@ -87,6 +87,14 @@ __global__ void __launch_bounds__(SH_N / SH_E) select_hist_kernel(SelectArgs a) 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     pdl_wait();
     pdl_launch_dependents();
+    // the row's scores are requested before seq_len is known (two independent DRAM misses instead of a chain)
+    const float* srow = a.scores + (int64_t)row * a.nb_stride;
+    float sraw[SH_E];
+#pragma unroll
+    for (int r = 0; r < SH_E; ++r) {
+        const int j = warp * (32 * SH_E) + lane + 32 * r;
+        sraw[r] = j < a.nb_stride ? srow[j] : 0.f;
+    }
     int n_b;
     if (a.q_block == 1) n_b = (a.seq_len[b] + a.blk - 1) / a.blk;
     else n_b = (a.q_start + (i + 1) * a.q_block - 1) / a.blk + 1;
@@ -99,14 +107,13 @@ __global__ void __launch_bounds__(SH_N / SH_E) select_hist_kernel(SelectArgs a) 
     const bool topp = a.mode != SPOT_MODE_TOPK;
 
     // ---- load: block scores -> keys; key range of the residual blocks
-    const float* srow = a.scores + (int64_t)row * a.nb_stride;
     uint32_t okey[SH_E];
     uint32_t kmn = 0xffffffffu, kmx = 0u;
 #pragma unroll
     for (int r = 0; r < SH_E; ++r) {
         const int j = ebase + 32 * r;
         const bool resid = j >= sink_end && j < rec_beg;
-        okey[r] = resid ? score_key(srow[j]) : KEY_PAD;
+        okey[r] = resid ? score_key(sraw[r]) : KEY_PAD;
         if (resid) { kmn = min(kmn, okey[r]); kmx = max(kmx, okey[r]); }
         s_cnt[tid * SH_E + r] = 0u;
     }
