@@ -272,17 +272,29 @@ def run_ours(args):
     den = time_alone(lambda: api.spot_dense_attn_decode(apd, stream), max(3, min(args.steps, 10)))
 
     # e2e: host buffers through spot_decode_step_host (H2D of the step's q / q^I / w, D2H of out + budgets)
+    # The step's inputs sit back to back in one pinned buffer (sel_q | w | q) and so do their device staging areas, the
+    # outputs likewise (out | budgets): spot_decode_step_host then moves each group in a single transfer.
     hp = api.DecodeStepHostParams()
-    h_selq = torch.from_numpy(wl.sel_q.view(np.int16)).pin_memory()
-    h_w = torch.from_numpy(wl.w).pin_memory()
-    h_q = torch.from_numpy(wl.q.view(np.int16)).pin_memory()
-    h_out = torch.empty((Bn, Hq, D), dtype=torch.int16).pin_memory()
-    h_bud = torch.empty((Bn,), dtype=torch.int32).pin_memory()
-    hp.sel_q_host, hp.w_host, hp.q_host = h_selq.data_ptr(), h_w.data_ptr(), h_q.data_ptr()
-    hp.out_host, hp.budgets_host = h_out.data_ptr(), h_bud.data_ptr()
-    hp.select, hp.attn = sp, ap
-    h2d = h_selq.numel() * 2 + h_w.numel() * 4 + h_q.numel() * 2
-    d2h = h_out.numel() * 2 + h_bud.numel() * 4
+    n_selq, n_w, n_q = wl.sel_q.nbytes, wl.w.nbytes, wl.q.nbytes
+    n_out, n_bud = Bn * Hq * D * 2, Bn * 4
+    h_in = torch.empty(n_selq + n_w + n_q, dtype=torch.uint8).pin_memory()
+    h_in[:n_selq] = torch.from_numpy(wl.sel_q.view(np.uint8).reshape(-1))
+    h_in[n_selq:n_selq + n_w] = torch.from_numpy(wl.w.view(np.uint8).reshape(-1))
+    h_in[n_selq + n_w:] = torch.from_numpy(wl.q.view(np.uint8).reshape(-1))
+    h_res = torch.empty(n_out + n_bud, dtype=torch.uint8).pin_memory()
+    d_in = torch.empty(n_selq + n_w + n_q, dtype=torch.uint8, device=dev)
+    d_res = torch.empty(n_out + n_bud, dtype=torch.uint8, device=dev)
+    sp_e = type(sp).from_buffer_copy(sp)
+    ap_e = type(ap).from_buffer_copy(ap)
+    sp_e.sel_q, sp_e.w = d_in.data_ptr(), d_in.data_ptr() + n_selq
+    ap_e.q = d_in.data_ptr() + n_selq + n_w
+    ap_e.out, sp_e.budgets, ap_e.budgets = d_res.data_ptr(), d_res.data_ptr() + n_out, d_res.data_ptr() + n_out
+    hp.sel_q_host, hp.w_host, hp.q_host = h_in.data_ptr(), h_in.data_ptr() + n_selq, h_in.data_ptr() + n_selq + n_w
+    hp.out_host, hp.budgets_host = h_res.data_ptr(), h_res.data_ptr() + n_out
+    hp.select, hp.attn = sp_e, ap_e
+    h_bud = h_res[n_out:].view(torch.int32)
+    h2d = n_selq + n_w + n_q
+    d2h = n_out + n_bud
     e2e = []
     for i in range(args.steps + 2):
         flush_l2()

@@ -210,6 +210,8 @@ spot_status spot_dense_attn_decode(const spot_attn_params* p, void* stream);
  * Host-buffer convenience (the "e2e" path of bench.py): one decode layer-step with every tensor in HOST
  * memory.  Copies inputs host->device into caller-provided device staging buffers, runs
  * spot_select + spot_sparse_attn_decode, copies out/indices/budgets back, all on `stream`, no sync.
+ * When the host inputs are laid out back to back (sel_q | w | q) and so are their device staging areas, they go up as
+ * ONE transfer; likewise out | budgets come back as one (each small copy costs microseconds of stream time).
  * (Declared here so that the end-to-end measurement also crosses the C ABI.)
  * --------------------------------------------------------------------------------------------------- */
 typedef struct {

@@ -157,15 +157,35 @@ extern "C" spot_status spot_decode_step_host(const spot_decode_step_host_params*
     const spot_attn_params& ap = p->attn;
     if (sp.q_block != 1 || sp.B != ap.B) return SPOT_ERR_INVALID_ARG;
     cudaStream_t s = (cudaStream_t)stream;
-    SPOT_CUDA_TRY(cudaMemcpyAsync((void*)sp.sel_q, p->sel_q_host, (size_t)sp.B * sp.H_idx * sp.d_idx * 2,
-                                  cudaMemcpyHostToDevice, s));
-    SPOT_CUDA_TRY(cudaMemcpyAsync((void*)sp.w, p->w_host, (size_t)sp.B * sp.H_idx * 4, cudaMemcpyHostToDevice, s));
-    SPOT_CUDA_TRY(cudaMemcpyAsync((void*)ap.q, p->q_host, (size_t)ap.B * ap.H_q * ap.D * 2, cudaMemcpyHostToDevice, s));
+    const size_t n_selq = (size_t)sp.B * sp.H_idx * sp.d_idx * 2, n_w = (size_t)sp.B * sp.H_idx * 4;
+    const size_t n_q = (size_t)ap.B * ap.H_q * ap.D * 2;
+    // every small copy costs a few microseconds of stream time: inputs laid out back to back on both sides
+    // (sel_q | w | q) go up as one transfer
+    const char* h0 = reinterpret_cast<const char*>(p->sel_q_host);
+    const char* d0 = reinterpret_cast<const char*>(sp.sel_q);
+    const bool in_packed = reinterpret_cast<const char*>(p->w_host) == h0 + n_selq &&
+                           reinterpret_cast<const char*>(p->q_host) == h0 + n_selq + n_w &&
+                           reinterpret_cast<const char*>(sp.w) == d0 + n_selq &&
+                           reinterpret_cast<const char*>(ap.q) == d0 + n_selq + n_w;
+    if (in_packed) {
+        SPOT_CUDA_TRY(cudaMemcpyAsync((void*)sp.sel_q, p->sel_q_host, n_selq + n_w + n_q, cudaMemcpyHostToDevice, s));
+    } else {
+        SPOT_CUDA_TRY(cudaMemcpyAsync((void*)sp.sel_q, p->sel_q_host, n_selq, cudaMemcpyHostToDevice, s));
+        SPOT_CUDA_TRY(cudaMemcpyAsync((void*)sp.w, p->w_host, n_w, cudaMemcpyHostToDevice, s));
+        SPOT_CUDA_TRY(cudaMemcpyAsync((void*)ap.q, p->q_host, n_q, cudaMemcpyHostToDevice, s));
+    }
     spot_status st = spot_select(&sp, stream);
     if (st != SPOT_OK) return st;
     st = spot_sparse_attn_decode(&ap, stream);
     if (st != SPOT_OK) return st;
-    SPOT_CUDA_TRY(cudaMemcpyAsync(p->out_host, ap.out, (size_t)ap.B * ap.H_q * ap.D * 2, cudaMemcpyDeviceToHost, s));
-    SPOT_CUDA_TRY(cudaMemcpyAsync(p->budgets_host, sp.budgets, (size_t)sp.B * 4, cudaMemcpyDeviceToHost, s));
+    const size_t n_out = (size_t)ap.B * ap.H_q * ap.D * 2, n_bud = (size_t)sp.B * 4;
+    const bool out_packed = reinterpret_cast<char*>(p->budgets_host) == reinterpret_cast<char*>(p->out_host) + n_out &&
+                            reinterpret_cast<char*>(sp.budgets) == reinterpret_cast<char*>(ap.out) + n_out;
+    if (out_packed) {
+        SPOT_CUDA_TRY(cudaMemcpyAsync(p->out_host, ap.out, n_out + n_bud, cudaMemcpyDeviceToHost, s));
+    } else {
+        SPOT_CUDA_TRY(cudaMemcpyAsync(p->out_host, ap.out, n_out, cudaMemcpyDeviceToHost, s));
+        SPOT_CUDA_TRY(cudaMemcpyAsync(p->budgets_host, sp.budgets, n_bud, cudaMemcpyDeviceToHost, s));
+    }
     return SPOT_OK;
 }

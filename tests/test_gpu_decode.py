@@ -274,3 +274,60 @@ def test_full_size_configs_in_the_bench_configuration(torch_cuda, cfg, fmt, seqs
         assert err.max() <= MAX_ABS and err.mean() <= MEAN_ABS, (b, err.max(), err.mean())
         assert np.abs(lse[b].cpu().numpy() - want_lse).max() <= 2e-3
         print("%s %s seq %d: attention over %d blocks, max-abs %.2e mean-abs %.2e" % (cfg, fmt, b, n, err.max(), err.mean()))
+
+
+@pytest.mark.parametrize("packed", [False, True])
+def test_decode_step_from_host_buffers(torch_cuda, packed):
+    """spot_decode_step_host (the e2e entry of bench.py): inputs in pinned HOST memory, H2D copies + spot_select +
+    spot_sparse_attn_decode + D2H copies on one stream.  Checked against the oracle, with the inputs / outputs either in
+    separate buffers (three + two copies) or laid out back to back (one + one copy)."""
+    torch = torch_cuda
+    from paper_2606_22874_b200 import api
+    wl = make_config("mini2")
+    dd = H.DeviceDecode(wl, "bf16")
+    B, Hq, D, nb = wl.B, wl.H_q, wl.D, dd.n_b_max
+    n_selq, n_w, n_q, n_out, n_bud = wl.sel_q.nbytes, wl.w.nbytes, wl.q.nbytes, B * Hq * D * 2, B * 4
+    if packed:
+        h_in = torch.empty(n_selq + n_w + n_q, dtype=torch.uint8).pin_memory()
+        h_res = torch.zeros(n_out + n_bud, dtype=torch.uint8).pin_memory()
+        d_in = torch.zeros(n_selq + n_w + n_q, dtype=torch.uint8, device="cuda")
+        d_res = torch.zeros(n_out + n_bud, dtype=torch.uint8, device="cuda")
+        off_in, off_res = (0, n_selq, n_selq + n_w), (0, n_out)
+    else:
+        pad = 256                                   # separate regions: the copies cannot be merged
+        h_in = torch.empty(n_selq + n_w + n_q + 2 * pad, dtype=torch.uint8).pin_memory()
+        h_res = torch.zeros(n_out + n_bud + pad, dtype=torch.uint8).pin_memory()
+        d_in = torch.zeros(n_selq + n_w + n_q + 2 * pad, dtype=torch.uint8, device="cuda")
+        d_res = torch.zeros(n_out + n_bud + pad, dtype=torch.uint8, device="cuda")
+        off_in, off_res = (0, n_selq + pad, n_selq + n_w + 2 * pad), (0, n_out + pad)
+    for off, arr in zip(off_in, (wl.sel_q, wl.w, wl.q)):
+        h_in[off:off + arr.nbytes] = torch.from_numpy(arr.view(np.uint8).reshape(-1))
+    indices = torch.full((B, nb), -7, dtype=torch.int32, device="cuda")
+    sp = api.make_select_params(d_in, d_in, dd.sel_k, "bf16", dd.L_cap, dd.seq_len, dd.max_seq_len, B, 1, wl.H_idx,
+                                wl.d_idx, blk=wl.blk, q_block=1, mode=wl.mode, top_k=wl.top_k, p=wl.p,
+                                sink_blocks=wl.sink_blocks, recency_blocks=wl.recency_blocks,
+                                kmin_blocks=wl.kmin_blocks, temperature=wl.temperature, indices=indices, cap=nb,
+                                budgets=d_res)
+    sp.sel_q, sp.w, sp.budgets = d_in.data_ptr() + off_in[0], d_in.data_ptr() + off_in[1], d_res.data_ptr() + off_res[1]
+    ws1 = torch.empty(max(16, api.spot_select_workspace_bytes(sp)), dtype=torch.uint8, device="cuda")
+    sp.workspace, sp.workspace_bytes = ws1.data_ptr(), ws1.numel()
+    ap = api.make_attn_params(d_in, dd.K, dd.V, dd.kv_strides, dd.seq_len, dd.max_seq_len, indices, d_res, nb, B, 1, Hq,
+                              wl.H_kv, D, blk=wl.blk, sm_scale=wl.sm_scale, out=d_res)
+    ap.q, ap.out, ap.budgets = d_in.data_ptr() + off_in[2], d_res.data_ptr() + off_res[0], d_res.data_ptr() + off_res[1]
+    ws2 = torch.empty(max(16, api.spot_sparse_attn_decode_workspace_bytes(ap)), dtype=torch.uint8, device="cuda")
+    ap.workspace, ap.workspace_bytes = ws2.data_ptr(), ws2.numel()
+    hp = api.DecodeStepHostParams()
+    hp.sel_q_host, hp.w_host, hp.q_host = (h_in.data_ptr() + o for o in off_in)
+    hp.out_host, hp.budgets_host = h_res.data_ptr() + off_res[0], h_res.data_ptr() + off_res[1]
+    hp.select, hp.attn = sp, ap
+    api.spot_decode_step_host(hp)
+    torch.cuda.synchronize()
+    out = bf16_bits_to_f64(h_res[off_res[0]:off_res[0] + n_out].numpy().view(np.uint16).reshape(B, Hq, D))
+    bud = h_res[off_res[1]:off_res[1] + n_bud].numpy().view(np.int32)
+    idx = indices.cpu().numpy()
+    for b in range(B):
+        s_bar, sel = H.oracle_select(wl, "bf16", b)
+        assert int(bud[b]) == sel.budget and idx[b, :bud[b]].tolist() == sel.indices.tolist()
+        want, _ = H.oracle_attend(wl, b, sel.indices)
+        err = np.abs(out[b] - want)
+        assert err.max() <= MAX_ABS and err.mean() <= MEAN_ABS
