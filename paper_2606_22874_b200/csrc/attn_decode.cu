@@ -361,11 +361,8 @@ spot_status run_decode(const spot_attn_params* p, bool dense, cudaStream_t s) {
     a.part_o = reinterpret_cast<float*>(p->workspace);
     a.part_ml = a.part_o + slots * G * ATT_D;
     a.out = p->out; a.lse = p->lse;
-    static bool attr_set = false;
-    if (!attr_set) {
-        SPOT_CUDA_TRY(cudaFuncSetAttribute(attn_decode_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, ATT_SMEM));
-        attr_set = true;
-    }
+    static unsigned long long smem_attr_done = 0;
+    SPOT_CUDA_TRY(set_max_smem_once(attn_decode_kernel, ATT_SMEM, smem_attr_done));
     SPOT_CUDA_TRY(launch_pdl(attn_decode_kernel, dim3((unsigned)n_ctas), dim3(ATT_WARPS * 32), ATT_SMEM, s, a));
     const int rows = p->B * p->H_q;
     SPOT_CUDA_TRY(launch_pdl(attn_merge_kernel, dim3((unsigned)((rows + MERGE_WARPS - 1) / MERGE_WARPS)),

@@ -407,12 +407,8 @@ spot_status attn_prefill_tc(const spot_attn_params* p, cudaStream_t stream) {
     if (!make_map(&tm_v, p->v, n_tok, (uint64_t)p->kv_stride_token, (uint64_t)p->H_kv, (uint64_t)p->kv_stride_head,
                   (uint64_t)p->B, (uint64_t)p->kv_stride_batch, 64, 1))
         return SPOT_ERR_CUDA;
-    static bool attr_set = false;
-    if (!attr_set) {
-        SPOT_CUDA_TRY(cudaFuncSetAttribute(attn_prefill_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                           (int)TA_SMEM_BYTES));
-        attr_set = true;
-    }
+    static unsigned long long smem_attr_done = 0;
+    SPOT_CUDA_TRY(set_max_smem_once(attn_prefill_tc_kernel, (int)TA_SMEM_BYTES, smem_attr_done));
     const int n_mt = (a.G * 64 + 127) / 128;
     dim3 grid((unsigned)((n_mt + 1) / 2), (unsigned)(p->B * a.n_qb), (unsigned)p->H_kv);
     SPOT_CUDA_TRY(launch_pdl(attn_prefill_tc_kernel, grid, dim3(TA_THREADS), (size_t)TA_SMEM_BYTES, stream, tm_q, tm_k,

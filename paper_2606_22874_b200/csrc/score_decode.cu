@@ -466,12 +466,8 @@ spot_status launch_score_fmt(const spot_select_params* p, float* scores, int nb_
         const uint32_t box[4] = {64, 64, (uint32_t)NP, 1};
         if (!encode_tmap_bf16_sw128(&tm, p->sel_k, 4, dims, strides, box)) return SPOT_ERR_CUDA;
     }
-    static bool attr_set = false;
-    if (!attr_set) {
-        SPOT_CUDA_TRY(cudaFuncSetAttribute(score_decode_kernel<H, D_IDX, FMT>,
-                                           cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg::SMEM_BYTES));
-        attr_set = true;
-    }
+    static unsigned long long smem_attr_done = 0;
+    SPOT_CUDA_TRY(set_max_smem_once(score_decode_kernel<H, D_IDX, FMT>, Cfg::SMEM_BYTES, smem_attr_done));
     const int64_t max_tiles = (int64_t)p->B * ((p->max_seq_len + 63) / 64);
     const int grid = (int)(max_tiles < sm_count() ? max_tiles : sm_count());
     SPOT_CUDA_TRY(launch_pdl(score_decode_kernel<H, D_IDX, FMT>, dim3((unsigned)grid), dim3(Cfg::THREADS),

@@ -316,12 +316,8 @@ spot_status score_prefill(const spot_select_params* p, float* scores, int nb_str
         const uint32_t box[4] = {(uint32_t)PF_D, (uint32_t)PF_N, (uint32_t)PF_H, 1u};   // a pair of key blocks
         if (!encode_tmap_bf16_sw128(&tm_k, p->sel_k, 4, dims, strides, box)) return SPOT_ERR_CUDA;
     }
-    static bool attr_set = false;
-    if (!attr_set) {
-        SPOT_CUDA_TRY(cudaFuncSetAttribute(score_prefill_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                           (int)PF_SMEM_BYTES));
-        attr_set = true;
-    }
+    static unsigned long long smem_attr_done = 0;
+    SPOT_CUDA_TRY(set_max_smem_once(score_prefill_kernel, (int)PF_SMEM_BYTES, smem_attr_done));
     const int grid = (int)(total < sm_count() ? total : sm_count());
     SPOT_CUDA_TRY(launch_pdl(score_prefill_kernel, dim3((unsigned)grid), dim3(PF_THREADS), (size_t)PF_SMEM_BYTES, s, tm_q,
                              tm_k, a));
