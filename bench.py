@@ -112,7 +112,7 @@ def run_reference(args):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
-    wl = build_workload(args.workload, {})
+    wl = build_workload(args.workload, dict(D_IDX_OVERRIDE))
     K0, V0, q0 = host_kv_for_seq0(wl, wl.seed)
     times = []
     budget = 0
@@ -135,13 +135,17 @@ def run_reference(args):
     print(json.dumps(line))
 
 
+D_IDX_OVERRIDE = {}
+
+
 def rank_workload(name, rank):
     """Every rank runs the same-shaped batch of independent sequences with its own seed (rank 0: the config's seed):
     the path shards by sequence, weak scaling, no data-path collective."""
     if rank == 0:
-        return build_workload(name, {})
+        return build_workload(name, dict(D_IDX_OVERRIDE))
     from workloads import CONFIGS, make_decode_workload
     kw = dict(CONFIGS[name])
+    kw.update(D_IDX_OVERRIDE)
     kw["seed"] = kw["seed"] + 1000 * rank
     return make_decode_workload(name, with_kv=False, **kw)
 
@@ -614,7 +618,11 @@ def main():
     ap.add_argument("--fmt", default="bf16", choices=["bf16", "mxfp4", "int4_e4m3"])
     ap.add_argument("--p", type=float, default=0.90)
     ap.add_argument("--L", type=int, default=0, help="cfg5 only: prompt length (default 65536)")
+    ap.add_argument("--d-idx", type=int, default=0, choices=[0, 64, 128],
+                    help="decode only: selector head dim (default: the config's 64; 128 = the paper's geometry, PAPER.md:363)")
     args = ap.parse_args()
+    if args.d_idx:
+        D_IDX_OVERRIDE["d_idx"] = args.d_idx
     if args.workload == "cfg5":
         run_prefill(args)
     elif args.impl == "reference":

@@ -213,7 +213,8 @@ def test_end_to_end_step_matches_oracle(torch_cuda):
 
 
 @pytest.mark.parametrize("cfg,fmt,seqs", [("cfg3", "bf16", (0, 3)), ("cfg3", "mxfp4", (1,)), ("cfg3", "int4_e4m3", (2,)),
-                                          ("cfg2", "bf16", (0, 7)), ("cfg4_b4", "mxfp4", (0, 1, 2, 3))])
+                                          ("cfg2", "bf16", (0, 7)), ("cfg4_b4", "mxfp4", (0, 1, 2, 3)),
+                                          ("cfg3/d128", "bf16", (1,)), ("cfg3/d128", "mxfp4", (2,))])
 def test_full_size_configs_in_the_bench_configuration(torch_cuda, cfg, fmt, seqs):
     """BASELINE.json configs 2, 3 and 4 (batch 4) at full size (config 3: B=4, L=131072, 2048 blocks per sequence;
     config 4: H_q=64 and per-query budgets from the K_min floor to hundreds of blocks), launched exactly as bench.py
@@ -224,7 +225,8 @@ def test_full_size_configs_in_the_bench_configuration(torch_cuda, cfg, fmt, seqs
     torch = torch_cuda
     from oracle import attention as OA
     from paper_2606_22874_b200 import api
-    wl = make_config(cfg, with_kv=False)
+    # "/d128": the paper's selector geometry, 4 heads x 128, instead of BASELINE.json's 4 x 64
+    wl = make_config(cfg.split("/")[0], with_kv=False, **({"d_idx": 128} if cfg.endswith("/d128") else {}))
     dd = H.DeviceDecode(wl, fmt, with_kv=False)
     idx, bud, scores, probs = dd.select()
     assert bud.min() >= 8 and bud.max() <= dd.n_b_max
