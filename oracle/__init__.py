@@ -22,6 +22,9 @@ Modules (each function cites the PAPER.md passage it restates):
                    selected blocks (PAPER.md:47 Fig. 2, :71), GQA, decode form
                    and causal chunked-prefill form; a second, independent
                    mask-form coding; plain dense attention.
+* ``projection`` - upstream step f1: selector projections W_q h, W_k h, W_w h and
+                   the rotary embedding of q^I / k^I (PAPER.md:39, :362-364;
+                   DESIGN.md readings R27-R29).
 * ``brute``      - exhaustive enumeration used to pin the nucleus rule on tiny
                    inputs.
 
