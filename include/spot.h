@@ -61,7 +61,7 @@ int spot_last_cuda_error(void);
 /* Library version, "major.minor". */
 const char* spot_version(void);
 /* sizeof() of the parameter blocks as this library was compiled (which: 0 = spot_select_params,
- * 1 = spot_attn_params, 2 = spot_decode_step_host_params; anything else: 0) -- lets a binding verify its layout. */
+ * 1 = spot_attn_params, 2 = spot_decode_step_host_params, 3 = spot_project_params; anything else: 0) -- lets a binding verify its layout. */
 size_t spot_struct_size(int which);
 
 /* ---------------------------------------------------------------------------------------------------
@@ -93,6 +93,40 @@ spot_status spot_quantize_selector_k(const uint16_t* k_bf16, void* k_cache, spot
 spot_status spot_dequantize_selector_k(const void* k_cache, uint16_t* k_bf16_out, spot_selk_format fmt,
                                        int64_t B, int64_t n_tokens, int64_t token_offset,
                                        int64_t cache_stride_tokens, int H_idx, int d_idx, void* stream);
+
+/* ---------------------------------------------------------------------------------------------------
+ * f1 -- the step right before the path (decode form): selector projections, RoPE, mixing weights, and the
+ * append of the new token's selector key to the (quantised) cache, PAPER.md:39 ("q^I_h, k^I_{h,t} are the
+ * per-head query/key projections and W_w a small linear map producing the per-query mixing weights w_h from
+ * the hidden state h_q"), PAPER.md:362-364 (4 heads, "RoPE head dim 64").  Readings R27-R29 of DESIGN.md:
+ *   q^I = W_q h, k^I = W_k h, w = W_w h (no bias, no activation; BF16 inputs, fp32 accumulation);
+ *   rotary embedding on the first rope_dims dims of every selector head of q^I and k^I, rotate-half pairing
+ *   (i, i + rope_dims/2), angle = pos * rope_base^(-2 i / rope_dims); the other dims pass through;
+ *   q^I and k^I are rounded once to BF16 after the rotation; the cache entry of token pos[b] of sequence b is
+ *   that BF16 k^I in format fmt (quantised exactly as spot_quantize_selector_k would quantise it).
+ * One token per sequence.  A sequence whose pos[b] lies outside [0, cache_stride_tokens) gets sel_q and w but no
+ * cache write.  Requires d_model % 256 == 0, d_idx % 32 == 0, rope_dims even and <= d_idx, H_idx * d_idx % 2 == 0.
+ * workspace: >= spot_selector_project_append_workspace_bytes (the BF16 k^I of the new tokens, B * H_idx * d_idx * 2).
+ * --------------------------------------------------------------------------------------------------- */
+typedef struct {
+    const uint16_t* hidden;      /* [B][d_model] BF16 hidden state h of the current token                */
+    const uint16_t* w_q;         /* [H_idx*d_idx][d_model] BF16, row r = head r / d_idx, dim r % d_idx   */
+    const uint16_t* w_k;         /* [H_idx*d_idx][d_model] BF16                                           */
+    const uint16_t* w_w;         /* [H_idx][d_model] BF16                                                 */
+    const int32_t* pos;          /* [B] device: absolute position of the token = its slot in the cache    */
+    int32_t B, d_model, H_idx, d_idx, rope_dims;
+    float rope_base;
+    uint16_t* sel_q;             /* out [B][H_idx][d_idx] BF16                                            */
+    float* w;                    /* out [B][H_idx] fp32                                                   */
+    void* sel_k;                 /* selector K-cache, format fmt                                          */
+    int32_t fmt;                 /* spot_selk_format                                                      */
+    int64_t cache_stride_tokens;
+    void* workspace;
+    size_t workspace_bytes;
+} spot_project_params;
+
+size_t spot_selector_project_append_workspace_bytes(const spot_project_params* p);
+spot_status spot_selector_project_append(const spot_project_params* p, void* stream);
 
 /* ---------------------------------------------------------------------------------------------------
  * a1 + a2 -- spot_select: scores, block distribution, selection, index list + per-query budget.

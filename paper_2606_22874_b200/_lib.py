@@ -52,6 +52,17 @@ class DecodeStepHostParams(C.Structure):
     ]
 
 
+class ProjectParams(C.Structure):
+    _fields_ = [
+        ("hidden", C.c_void_p), ("w_q", C.c_void_p), ("w_k", C.c_void_p), ("w_w", C.c_void_p), ("pos", C.c_void_p),
+        ("B", C.c_int32), ("d_model", C.c_int32), ("H_idx", C.c_int32), ("d_idx", C.c_int32), ("rope_dims", C.c_int32),
+        ("rope_base", C.c_float),
+        ("sel_q", C.c_void_p), ("w", C.c_void_p), ("sel_k", C.c_void_p), ("fmt", C.c_int32),
+        ("cache_stride_tokens", C.c_int64),
+        ("workspace", C.c_void_p), ("workspace_bytes", C.c_size_t),
+    ]
+
+
 # every symbol include/spot.h declares: name -> (restype, argtypes)
 PROTOTYPES = {
     "spot_status_string": (C.c_char_p, [C.c_int]),
@@ -73,6 +84,8 @@ PROTOTYPES = {
     "spot_dense_attn_decode_workspace_bytes": (C.c_size_t, [C.POINTER(AttnParams)]),
     "spot_dense_attn_decode": (C.c_int, [C.POINTER(AttnParams), C.c_void_p]),
     "spot_decode_step_host": (C.c_int, [C.POINTER(DecodeStepHostParams), C.c_void_p]),
+    "spot_selector_project_append_workspace_bytes": (C.c_size_t, [C.POINTER(ProjectParams)]),
+    "spot_selector_project_append": (C.c_int, [C.POINTER(ProjectParams), C.c_void_p]),
 }
 
 _lib = None
@@ -91,7 +104,7 @@ def load():
             fn = getattr(lib, name)
             fn.restype = res
             fn.argtypes = args
-        for which, st in enumerate((SelectParams, AttnParams, DecodeStepHostParams)):
+        for which, st in enumerate((SelectParams, AttnParams, DecodeStepHostParams, ProjectParams)):
             if lib.spot_struct_size(which) != C.sizeof(st):
                 raise RuntimeError("ABI mismatch: %s is %d bytes in libspot.so, %d in the binding"
                                    % (st.__name__, lib.spot_struct_size(which), C.sizeof(st)))

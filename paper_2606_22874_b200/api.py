@@ -7,7 +7,7 @@ import ctypes as C
 import torch
 
 from . import _lib as L
-from ._lib import AttnParams, DecodeStepHostParams, SelectParams, FORMATS, MODES  # noqa: F401
+from ._lib import AttnParams, DecodeStepHostParams, ProjectParams, SelectParams, FORMATS, MODES  # noqa: F401
 
 
 class SpotError(RuntimeError):
@@ -146,3 +146,25 @@ def spot_sparse_attn_prefill(ap, stream=None):
 
 def spot_decode_step_host(hp, stream=None):
     _check(L.load().spot_decode_step_host(C.byref(hp), _stream(stream)), "spot_decode_step_host")
+
+
+def make_project_params(hidden, w_q, w_k, w_w, pos, B, d_model, H_idx, d_idx, *, rope_dims=64, rope_base=1.0e6,
+                        sel_q=None, w=None, sel_k=None, fmt="bf16", cache_stride_tokens=0, workspace=None):
+    pp = ProjectParams()
+    pp.hidden, pp.w_q, pp.w_k, pp.w_w, pp.pos = (t.data_ptr() for t in (hidden, w_q, w_k, w_w, pos))
+    pp.B, pp.d_model, pp.H_idx, pp.d_idx, pp.rope_dims = B, d_model, H_idx, d_idx, rope_dims
+    pp.rope_base = float(rope_base)
+    pp.sel_q, pp.w, pp.sel_k = sel_q.data_ptr(), w.data_ptr(), sel_k.data_ptr()
+    pp.fmt = _fmt(fmt)
+    pp.cache_stride_tokens = cache_stride_tokens
+    if workspace is not None:
+        pp.workspace, pp.workspace_bytes = workspace.data_ptr(), workspace.numel() * workspace.element_size()
+    return pp
+
+
+def spot_selector_project_append_workspace_bytes(pp):
+    return int(L.load().spot_selector_project_append_workspace_bytes(C.byref(pp)))
+
+
+def spot_selector_project_append(pp, stream=None):
+    _check(L.load().spot_selector_project_append(C.byref(pp), _stream(stream)), "spot_selector_project_append")

@@ -111,6 +111,7 @@ extern "C" size_t spot_struct_size(int which) {
         case 0: return sizeof(spot_select_params);
         case 1: return sizeof(spot_attn_params);
         case 2: return sizeof(spot_decode_step_host_params);
+        case 3: return sizeof(spot_project_params);
     }
     return 0;
 }

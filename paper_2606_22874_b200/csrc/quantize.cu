@@ -33,13 +33,19 @@ __device__ __forceinline__ float e4m3_to_f32(uint32_t code) {
 template <int FMT>
 __global__ void __launch_bounds__(256) quantize_kernel(const uint16_t* __restrict__ k_in, uint8_t* __restrict__ cache,
                                                        int64_t n_tokens, int64_t token_offset, int64_t tiles_per_seq,
-                                                       int groups_per_token, int64_t total_groups) {
+                                                       int groups_per_token, int64_t total_groups,
+                                                       const int32_t* __restrict__ pos) {
+    pdl_wait();
     int64_t gid = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (gid >= total_groups) return;
     int gi = (int)(gid % groups_per_token);
     int64_t tok_lin = gid / groups_per_token;            // b * n_tokens + t
     int64_t b = tok_lin / n_tokens;
     int64_t t = token_offset + (tok_lin - b * n_tokens);
+    if (pos) {                                           // append form: one token per sequence at its own slot
+        t = pos[b];
+        if (t < 0 || t >= tiles_per_seq * SELK_TILE) return;
+    }
 
     const uint4* src = reinterpret_cast<const uint4*>(k_in + gid * 32);
     uint32_t wv[16];
@@ -169,11 +175,17 @@ __global__ void __launch_bounds__(256) dequantize_kernel(const uint8_t* __restri
 __global__ void __launch_bounds__(256) copy_rows_kernel(const uint4* __restrict__ src, uint4* __restrict__ dst,
                                                         int64_t n_tokens, int64_t vec_per_token,
                                                         int64_t src_stride_tokens, int64_t src_offset,
-                                                        int64_t dst_stride_tokens, int64_t dst_offset, int64_t total) {
+                                                        int64_t dst_stride_tokens, int64_t dst_offset, int64_t total,
+                                                        const int32_t* __restrict__ pos) {
+    pdl_wait();
     int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= total) return;
     int64_t per_seq = n_tokens * vec_per_token;
     int64_t b = i / per_seq, r = i - b * per_seq;
+    if (pos) {
+        dst_offset = pos[b];
+        if (dst_offset < 0 || dst_offset >= dst_stride_tokens) return;
+    }
     dst[(b * dst_stride_tokens + dst_offset) * vec_per_token + r] =
         src[(b * src_stride_tokens + src_offset) * vec_per_token + r];
 }
@@ -189,6 +201,29 @@ spot_status check_quant_args(const void* a, const void* b, int fmt, int64_t B, i
 }
 
 }  // namespace
+
+// f1: write one new token per sequence (k_new [B][H*d] BF16) into the cache at slot pos[b] (device array), in format fmt.
+// Same quantisers, same layout; launched with the PDL attribute so that it chains behind the projection kernel.
+spot_status append_selector_k(const uint16_t* k_new, void* cache, int fmt, int B, const int32_t* pos, int64_t stride,
+                              int H, int d, cudaStream_t s) {
+    if (fmt == SPOT_SELK_BF16) {
+        const int64_t vpt = (int64_t)H * d / 8, total = (int64_t)B * vpt;
+        SPOT_CUDA_TRY(launch_pdl(copy_rows_kernel, dim3((unsigned)ceil_div64(total, 256)), dim3(256), 0, s,
+                                 (const uint4*)k_new, (uint4*)cache, (int64_t)1, vpt, (int64_t)1, (int64_t)0, stride,
+                                 (int64_t)0, total, pos));
+        return SPOT_OK;
+    }
+    const int gpt = H * d / 32;
+    const int64_t total = (int64_t)B * gpt, tiles = stride / SELK_TILE;
+    const dim3 grid((unsigned)ceil_div64(total, 256));
+    if (fmt == SPOT_SELK_MXFP4)
+        SPOT_CUDA_TRY(launch_pdl(quantize_kernel<SPOT_SELK_MXFP4>, grid, dim3(256), 0, s, k_new, (uint8_t*)cache, (int64_t)1,
+                                 (int64_t)0, tiles, gpt, total, pos));
+    else
+        SPOT_CUDA_TRY(launch_pdl(quantize_kernel<SPOT_SELK_INT4_E4M3>, grid, dim3(256), 0, s, k_new, (uint8_t*)cache,
+                                 (int64_t)1, (int64_t)0, tiles, gpt, total, pos));
+    return SPOT_OK;
+}
 
 }  // namespace spot
 
@@ -215,7 +250,7 @@ extern "C" spot_status spot_quantize_selector_k(const uint16_t* k_bf16, void* k_
     if (fmt == SPOT_SELK_BF16) {
         int64_t vpt = (int64_t)H_idx * d_idx / 8, total = B * n_tokens * vpt;
         copy_rows_kernel<<<(unsigned)ceil_div64(total, 256), 256, 0, s>>>(
-            (const uint4*)k_bf16, (uint4*)k_cache, n_tokens, vpt, n_tokens, 0, cache_stride_tokens, token_offset, total);
+            (const uint4*)k_bf16, (uint4*)k_cache, n_tokens, vpt, n_tokens, 0, cache_stride_tokens, token_offset, total, nullptr);
         SPOT_LAUNCH_CHECK();
         return SPOT_OK;
     }
@@ -224,9 +259,9 @@ extern "C" spot_status spot_quantize_selector_k(const uint16_t* k_bf16, void* k_
     int64_t tiles = cache_stride_tokens / SELK_TILE;
     unsigned grid = (unsigned)ceil_div64(total, 256);
     if (fmt == SPOT_SELK_MXFP4)
-        quantize_kernel<SPOT_SELK_MXFP4><<<grid, 256, 0, s>>>(k_bf16, (uint8_t*)k_cache, n_tokens, token_offset, tiles, gpt, total);
+        quantize_kernel<SPOT_SELK_MXFP4><<<grid, 256, 0, s>>>(k_bf16, (uint8_t*)k_cache, n_tokens, token_offset, tiles, gpt, total, nullptr);
     else
-        quantize_kernel<SPOT_SELK_INT4_E4M3><<<grid, 256, 0, s>>>(k_bf16, (uint8_t*)k_cache, n_tokens, token_offset, tiles, gpt, total);
+        quantize_kernel<SPOT_SELK_INT4_E4M3><<<grid, 256, 0, s>>>(k_bf16, (uint8_t*)k_cache, n_tokens, token_offset, tiles, gpt, total, nullptr);
     SPOT_LAUNCH_CHECK();
     return SPOT_OK;
 }
@@ -241,7 +276,7 @@ extern "C" spot_status spot_dequantize_selector_k(const void* k_cache, uint16_t*
     if (fmt == SPOT_SELK_BF16) {
         int64_t vpt = (int64_t)H_idx * d_idx / 8, total = B * n_tokens * vpt;
         copy_rows_kernel<<<(unsigned)ceil_div64(total, 256), 256, 0, s>>>(
-            (const uint4*)k_cache, (uint4*)k_bf16_out, n_tokens, vpt, cache_stride_tokens, token_offset, n_tokens, 0, total);
+            (const uint4*)k_cache, (uint4*)k_bf16_out, n_tokens, vpt, cache_stride_tokens, token_offset, n_tokens, 0, total, nullptr);
         SPOT_LAUNCH_CHECK();
         return SPOT_OK;
     }

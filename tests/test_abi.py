@@ -43,7 +43,8 @@ def test_struct_layout_and_strings(lib):
     assert lib.spot_struct_size(0) == C.sizeof(_lib.SelectParams)
     assert lib.spot_struct_size(1) == C.sizeof(_lib.AttnParams)
     assert lib.spot_struct_size(2) == C.sizeof(_lib.DecodeStepHostParams)
-    assert lib.spot_struct_size(3) == 0
+    assert lib.spot_struct_size(3) == C.sizeof(_lib.ProjectParams)
+    assert lib.spot_struct_size(4) == 0
     assert [lib.spot_status_string(i) for i in range(5)] == [
         b"SPOT_OK", b"SPOT_ERR_INVALID_ARG", b"SPOT_ERR_UNSUPPORTED", b"SPOT_ERR_WORKSPACE_TOO_SMALL", b"SPOT_ERR_CUDA"]
     assert re.match(rb"\d+\.\d+$", lib.spot_version())
@@ -136,6 +137,28 @@ def test_quantize_argument_errors(lib):
     assert f(0x1000, 0x2000, 2, 1, 64, 64, 64, 4, 64, None) == INVALID          # past the capacity
     assert f(0x1000, 0x2000, 5, 1, 64, 0, 64, 4, 64, None) == INVALID           # unknown format
     assert lib.spot_dequantize_selector_k(0x1000, None, 2, 1, 64, 0, 64, 4, 64, None) == INVALID
+
+
+def test_project_argument_errors(lib):
+    from paper_2606_22874_b200 import _lib
+    INVALID, WS = 1, 3
+
+    def params(**over):
+        pp = _lib.ProjectParams()
+        pp.hidden, pp.w_q, pp.w_k, pp.w_w, pp.pos = 0x1000, 0x2000, 0x3000, 0x4000, 0x5000
+        pp.B, pp.d_model, pp.H_idx, pp.d_idx, pp.rope_dims, pp.rope_base = 4, 4096, 4, 64, 64, 1e6
+        pp.sel_q, pp.w, pp.sel_k, pp.fmt, pp.cache_stride_tokens = 0x6000, 0x7000, 0x8000, 2, 4096
+        for k, v in over.items():
+            setattr(pp, k, v)
+        return pp
+    assert lib.spot_selector_project_append_workspace_bytes(C.byref(params())) >= 4 * 4 * 64 * 2
+    for o in (dict(hidden=None), dict(w_w=None), dict(pos=None), dict(sel_k=None), dict(w_q=0x2004), dict(B=0),
+              dict(d_model=4000), dict(d_idx=48), dict(rope_dims=33), dict(rope_dims=128), dict(rope_base=0.0),
+              dict(fmt=7), dict(cache_stride_tokens=100)):
+        pp = params(**o)
+        assert lib.spot_selector_project_append(C.byref(pp), None) == INVALID, o
+        assert lib.spot_selector_project_append_workspace_bytes(C.byref(pp)) == 0, o
+    assert lib.spot_selector_project_append(None, None) == INVALID
 
 
 def test_binding_fails_loudly_without_the_library(monkeypatch):

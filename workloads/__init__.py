@@ -10,3 +10,4 @@ patterns, so the oracle and the GPU library read the very same bits.
 from .bf16 import f32_to_bf16_bits, bf16_bits_to_f32  # noqa: F401
 from .decode import DecodeWorkload, make_decode_workload, CONFIGS, make_config  # noqa: F401
 from .prefill import PrefillWorkload, make_prefill_workload  # noqa: F401
+from .project import make_project_workload  # noqa: F401
