@@ -275,6 +275,26 @@ def run_ours(args):
     # dense comparator (same shapes, every block)
     den = time_alone(lambda: api.spot_dense_attn_decode(apd, stream), max(3, min(args.steps, 10)))
 
+    # the step right before the path, timed alone and reported beside the step, not inside it: selector
+    # projections + RoPE + mixing weights + append of the new token's key to the cache (synthetic Qwen3-8B-sized weights)
+    from workloads import make_project_workload
+    d_model = 4096 if Hq == 32 else 5120
+    pw = make_project_workload(seed=wl.seed + 29, B=Bn, d_model=d_model, H_idx=wl.H_idx, d_idx=wl.d_idx, L=L)
+    p_dev = {k: torch.from_numpy(pw[k].view(np.int16)).to(dev) for k in ("hidden", "w_q", "w_k", "w_w")}
+    p_pos = torch.full((Bn,), 63, dtype=torch.int32, device=dev)
+    p_q = torch.empty_like(sel_q)
+    p_w = torch.empty_like(w)
+    # (a 64-token scratch cache of the same format: the append touches one slot per sequence whatever the cache size,
+    # and the step's real cache stays as the generator made it)
+    p_cache = torch.zeros(api.spot_selector_k_bytes(args.fmt, Bn, 64, wl.H_idx, wl.d_idx), dtype=torch.uint8, device=dev)
+    pp = api.make_project_params(p_dev["hidden"], p_dev["w_q"], p_dev["w_k"], p_dev["w_w"], p_pos, Bn, d_model, wl.H_idx,
+                                 wl.d_idx, rope_dims=min(64, wl.d_idx), rope_base=1.0e6, sel_q=p_q, w=p_w, sel_k=p_cache,
+                                 fmt=args.fmt, cache_stride_tokens=64)
+    ws_p = torch.empty(api.spot_selector_project_append_workspace_bytes(pp), dtype=torch.uint8, device=dev)
+    pp.workspace, pp.workspace_bytes = ws_p.data_ptr(), ws_p.numel()
+    f1_ms = time_alone(lambda: api.spot_selector_project_append(pp, stream), max(3, min(args.steps, 10)))
+    f1_bytes = (2 * wl.H_idx * wl.d_idx + wl.H_idx + Bn) * d_model * 2
+
     # e2e: host buffers through spot_decode_step_host (H2D of the step's q / q^I / w, D2H of out + budgets)
     # The step's inputs sit back to back in one pinned buffer (sel_q | w | q) and so do their device staging areas, the
     # outputs likewise (out | budgets): spot_decode_step_host then moves each group in a single transfer.
@@ -344,7 +364,11 @@ def run_ours(args):
         "tokens_per_s": world * Bn / (n_layers * step_mean * 1e-3),
         "breakdown_us": {"select (score+select kernels)": float(sel_ms.mean()) * 1e3,
                          "sparse attention (attn+merge kernels)": float(att_ms.mean()) * 1e3,
-                         "dense flash-decode comparator": float(np.mean(den)) * 1e3},
+                         "dense flash-decode comparator": float(np.mean(den)) * 1e3,
+                         "upstream f1 alone (projection + RoPE + append; not in the step)": float(np.mean(f1_ms)) * 1e3},
+        "upstream_f1": {"us": float(np.mean(f1_ms)) * 1e3, "weight_bytes": f1_bytes, "d_model": d_model,
+                        "note": "latency-bound: %.1f MiB of weights = %.2f us at the measured copy peak"
+                                % (f1_bytes / 2 ** 20, f1_bytes / peak / 1e3)},
         "step_roofline": {"bytes": sel_alg + kv_alg, "achieved_gbs": (sel_alg + kv_alg) / (step_mean * 1e-3) / 1e9,
                           "frac_of_measured": (sel_alg + kv_alg) / (step_mean * 1e-3) / 1e9 / peak,
                           "frac_of_8TBs": (sel_alg + kv_alg) / (step_mean * 1e-3) / 1e9 / 8000.0,

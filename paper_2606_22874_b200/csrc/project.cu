@@ -3,9 +3,10 @@
 // DESIGN.md readings R27-R29):  q^I = RoPE(W_q h), k^I = RoPE(W_k h), w = W_w h.
 //
 // A matrix-vector product shared by the B sequences of the step: (2 H d + H) x d_model BF16 weights (4.2 MiB at
-// 4 x 64 x 4096) are read once -- HBM-bound, ~1 us of traffic, so the kernel is shaped for latency: one warp per PAIR
-// of output rows (the two rows a rotary pair needs, so the rotation happens in registers), 16-byte loads of both weight
-// rows and of the hidden vectors, fp32 FMAs, butterfly reduction, fp64 sincos for the angle (positions reach 2^17).
+// 4 x 64 x 4096) are read once -- HBM-bound, ~1 us of traffic, so the kernel is shaped for latency: one CTA per PAIR
+// of output rows (the two rows a rotary pair needs, so the rotation happens in registers), its four warps splitting
+// d_model, eight 16-byte weight loads in flight per thread before the first FMA, fp32 FMAs, butterfly + shared-memory
+// reduction, fp64 sincos for the angle (positions reach 2^17).
 // The new k^I goes to a small BF16 staging row and is appended by quantize.cu's kernels in the cache's own format
 // (programmatic dependent launch), so that a0's bit-exact quantiser definition has a single implementation.
 #include "common.cuh"
@@ -44,11 +45,11 @@ __device__ __forceinline__ float dot8(uint4 a, uint4 b, float acc) {
 }
 
 __global__ void __launch_bounds__(PJ_WARPS * 32) project_rope_kernel(ProjectArgs a) {
-    const int lane = threadIdx.x & 31;
-    const int unit = blockIdx.x * PJ_WARPS + (threadIdx.x >> 5);
+    __shared__ float part[PJ_WARPS][2 * PJ_BC];
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int unit = blockIdx.x;                     // one CTA per pair of output rows; its 4 warps split d_model
     pdl_wait();
     pdl_launch_dependents();
-    if (unit >= a.n_units) return;
     // unit -> (matrix, two output rows, rotary pair index or -1)
     const uint16_t* W;
     int r0, r1, pair_i = -1, kind;                   // kind 0: q, 1: k, 2: w
@@ -73,14 +74,29 @@ __global__ void __launch_bounds__(PJ_WARPS * 32) project_rope_kernel(ProjectArgs
         float acc0[PJ_BC], acc1[PJ_BC];
 #pragma unroll
         for (int j = 0; j < PJ_BC; ++j) acc0[j] = acc1[j] = 0.f;
-        for (int v = lane; v < n_vec; v += 32) {
-            const uint4 x0 = ldg_stream_v4(w0 + v), x1 = ldg_stream_v4(w1 + v);
+        // four vectors of each weight row per thread and trip, all eight loads in flight before the first FMA: the
+        // kernel is a chain of DRAM latencies, not of bytes
+        for (int v0 = tid; v0 < n_vec; v0 += 4 * PJ_WARPS * 32) {
+            uint4 xa[4], xb[4];
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+                const int v = v0 + u * PJ_WARPS * 32;
+                xa[u] = v < n_vec ? ldg_stream_v4(w0 + v) : make_uint4(0, 0, 0, 0);
+                xb[u] = v < n_vec ? ldg_stream_v4(w1 + v) : make_uint4(0, 0, 0, 0);
+            }
 #pragma unroll
             for (int j = 0; j < PJ_BC; ++j) {
                 if (b0 + j < a.B) {
-                    const uint4 hv = __ldg(reinterpret_cast<const uint4*>(a.hidden + (int64_t)(b0 + j) * a.d_model) + v);
-                    acc0[j] = dot8(x0, hv, acc0[j]);
-                    acc1[j] = dot8(x1, hv, acc1[j]);
+                    const uint4* hp = reinterpret_cast<const uint4*>(a.hidden + (int64_t)(b0 + j) * a.d_model);
+#pragma unroll
+                    for (int u = 0; u < 4; ++u) {
+                        const int v = v0 + u * PJ_WARPS * 32;
+                        if (v < n_vec) {
+                            const uint4 hv = __ldg(hp + v);
+                            acc0[j] = dot8(xa[u], hv, acc0[j]);
+                            acc1[j] = dot8(xb[u], hv, acc1[j]);
+                        }
+                    }
                 }
             }
         }
@@ -91,13 +107,18 @@ __global__ void __launch_bounds__(PJ_WARPS * 32) project_rope_kernel(ProjectArgs
                 acc0[j] += __shfl_xor_sync(0xffffffffu, acc0[j], o);
                 acc1[j] += __shfl_xor_sync(0xffffffffu, acc1[j], o);
             }
-        // lane j finishes sequence b0 + j
-        float x0 = 0.f, x1 = 0.f;
+        __syncthreads();                             // (the previous pass has read `part`)
+        if (lane == 0) {
 #pragma unroll
-        for (int j = 0; j < PJ_BC; ++j)
-            if (lane == j) { x0 = acc0[j]; x1 = acc1[j]; }
-        const int b = b0 + lane;
-        if (lane < PJ_BC && b < a.B) {
+            for (int j = 0; j < PJ_BC; ++j) { part[warp][2 * j] = acc0[j]; part[warp][2 * j + 1] = acc1[j]; }
+        }
+        __syncthreads();
+        // thread j of warp 0 finishes sequence b0 + j
+        const int b = b0 + tid;
+        if (tid < PJ_BC && b < a.B) {
+            float x0 = 0.f, x1 = 0.f;
+#pragma unroll
+            for (int w = 0; w < PJ_WARPS; ++w) { x0 += part[w][2 * tid]; x1 += part[w][2 * tid + 1]; }
             if (kind == 2) {
                 a.w[(int64_t)b * a.H + r0] = x0;
                 if (r1 != r0) a.w[(int64_t)b * a.H + r1] = x1;
@@ -160,7 +181,6 @@ extern "C" spot_status spot_selector_project_append(const spot_project_params* p
     a.n_qk_units = p->H_idx * p->d_idx / 2;
     a.n_units = 2 * a.n_qk_units + (p->H_idx + 1) / 2;
     cudaStream_t s = (cudaStream_t)stream;
-    SPOT_CUDA_TRY(launch_pdl(project_rope_kernel, dim3((unsigned)((a.n_units + PJ_WARPS - 1) / PJ_WARPS)), dim3(PJ_WARPS * 32),
-                             0, s, a));
+    SPOT_CUDA_TRY(launch_pdl(project_rope_kernel, dim3((unsigned)a.n_units), dim3(PJ_WARPS * 32), 0, s, a));
     return append_selector_k(a.k_new, p->sel_k, p->fmt, p->B, p->pos, p->cache_stride_tokens, p->H_idx, p->d_idx, s);
 }
