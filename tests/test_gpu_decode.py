@@ -142,9 +142,10 @@ def test_select_crowded_cut_bins_and_ties(torch_cuda):
     assert not bad, bad
 
 
-@pytest.mark.parametrize("L", [200000, 300000])
+@pytest.mark.parametrize("L", [200000, 300000, 524288])
 def test_select_rows_longer_than_2048_blocks(torch_cuda, L):
-    """n_b = 3125 / 4688: rows beyond the histogram kernel's 2048 blocks take the bitonic-sort kernel (LT = 9 / 10)."""
+    """n_b = 3125 / 4688 / 8192 (the maximum row the library accepts, L = 512K as in PAPER.md:144): rows beyond the
+    histogram kernel's 2048 blocks take the bitonic-sort kernel (LT = 9 / 10)."""
     wl = make_decode_workload("long", 77 + L, B=1, L=L, kind="zipf", zipf_s=1.1, with_kv=False)
     dd = H.DeviceDecode(wl, "bf16", with_kv=False)
     report = []
