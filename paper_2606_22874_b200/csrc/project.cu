@@ -9,6 +9,8 @@
 // reduction, fp64 sincos for the angle (positions reach 2^17).
 // The new k^I goes to a small BF16 staging row and is appended by quantize.cu's kernels in the cache's own format
 // (programmatic dependent launch), so that a0's bit-exact quantiser definition has a single implementation.
+#include <math.h>
+
 #include "common.cuh"
 
 namespace spot {
@@ -20,6 +22,7 @@ namespace {
 
 constexpr int PJ_WARPS = 4;
 constexpr int PJ_BC = 8;            // sequences per pass over a pair of weight rows
+constexpr int PJ_MAX_ROPE = 256;
 
 struct ProjectArgs {
     const uint16_t* hidden;
@@ -34,6 +37,7 @@ struct ProjectArgs {
     float* w;
     int n_qk_units;       // H*d/2 pair units per projection
     int n_units;          // 2 * n_qk_units + ceil(H/2)
+    double inv_freq[PJ_MAX_ROPE / 2];   // base^(-2 i / rope), computed on the host in fp64 (keeps pow() off the device path)
 };
 
 __device__ __forceinline__ float dot8(uint4 a, uint4 b, float acc) {
@@ -126,7 +130,7 @@ __global__ void __launch_bounds__(PJ_WARPS * 32) project_rope_kernel(ProjectArgs
                 float y0 = x0, y1 = x1;
                 if (pair_i >= 0) {
                     // angle = pos * base^(-2 i / rope); fp64: positions reach 2^17 and the angle must be good to ~1e-7
-                    const double ang = (double)a.pos[b] * exp2(-2.0 * (double)pair_i / (double)a.rope * log2((double)a.rope_base));
+                    const double ang = (double)a.pos[b] * a.inv_freq[pair_i];
                     double sn, cs;
                     sincos(ang, &sn, &cs);
                     y0 = (float)((double)x0 * cs - (double)x1 * sn);
@@ -150,6 +154,7 @@ spot_status check_project(const spot_project_params* p) {
         return SPOT_ERR_INVALID_ARG;
     if (p->rope_dims < 0 || p->rope_dims % 2 != 0 || p->rope_dims > p->d_idx || !(p->rope_base > 0.f))
         return SPOT_ERR_INVALID_ARG;
+    if (p->rope_dims > PJ_MAX_ROPE) return SPOT_ERR_UNSUPPORTED;
     if (p->fmt != SPOT_SELK_BF16 && p->fmt != SPOT_SELK_INT4_E4M3 && p->fmt != SPOT_SELK_MXFP4) return SPOT_ERR_INVALID_ARG;
     if (p->cache_stride_tokens <= 0) return SPOT_ERR_INVALID_ARG;
     if (p->fmt != SPOT_SELK_BF16 && p->cache_stride_tokens % SELK_TILE != 0) return SPOT_ERR_INVALID_ARG;
@@ -178,6 +183,8 @@ extern "C" spot_status spot_selector_project_append(const spot_project_params* p
     a.B = p->B; a.d_model = p->d_model; a.H = p->H_idx; a.d = p->d_idx; a.rope = p->rope_dims; a.rope_base = p->rope_base;
     a.sel_q = p->sel_q; a.w = p->w;
     a.k_new = reinterpret_cast<uint16_t*>((reinterpret_cast<uintptr_t>(p->workspace) + 255) & ~(uintptr_t)255);
+    for (int i = 0; i < p->rope_dims / 2; ++i)
+        a.inv_freq[i] = pow((double)p->rope_base, -2.0 * (double)i / (double)p->rope_dims);
     a.n_qk_units = p->H_idx * p->d_idx / 2;
     a.n_units = 2 * a.n_qk_units + (p->H_idx + 1) / 2;
     cudaStream_t s = (cudaStream_t)stream;
