@@ -167,3 +167,18 @@ def test_binding_fails_loudly_without_the_library(monkeypatch):
     monkeypatch.setattr(_lib, "LIB_PATH", os.path.join(ROOT, "no_such_dir", "libspot.so"))
     with pytest.raises(RuntimeError, match="no CPU fallback"):
         _lib.load()
+
+
+def test_header_is_plain_c99():
+    """include/spot.h is the boundary: it must compile as C99 (no C++, no torch, no CUDA types in the signatures)."""
+    import shutil
+    import subprocess
+    gcc = shutil.which("gcc")
+    if gcc is None:
+        pytest.skip("no gcc on this machine")
+    hdr = os.path.join(ROOT, "include", "spot.h")
+    r = subprocess.run([gcc, "-std=c99", "-Wall", "-Wextra", "-Werror", "-fsyntax-only", "-x", "c", hdr],
+                       capture_output=True, text=True)
+    assert r.returncode == 0, r.stderr
+    src = open(hdr).read()
+    assert "torch" not in src and "cuda_runtime" not in src and "cudaStream_t stream" not in src
