@@ -272,6 +272,18 @@ def run_ours(args):
     sel_ms = time_alone(lambda: api.spot_select(sp, stream), n_alone)
     att_ms = time_alone(lambda: api.spot_sparse_attn_decode(ap, stream), n_alone)
 
+    # the same step replayed from a CUDA graph (the calls never synchronise, so a caller may capture them)
+    graph_us = None
+    try:
+        cap_stream = torch.cuda.Stream()
+        gph = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(gph, stream=cap_stream):
+            api.spot_select(sp, torch.cuda.current_stream())
+            api.spot_sparse_attn_decode(ap, torch.cuda.current_stream())
+        graph_us = float(time_alone(gph.replay, n_alone).mean()) * 1e3
+    except Exception as e:                                    # reported, never fatal for the headline number
+        graph_us = "capture failed: %s" % (str(e).splitlines()[0] if str(e) else type(e).__name__)
+
     # dense comparator (same shapes, every block)
     den = time_alone(lambda: api.spot_dense_attn_decode(apd, stream), max(3, min(args.steps, 10)))
 
@@ -365,6 +377,7 @@ def run_ours(args):
         "breakdown_us": {"select (score+select kernels)": float(sel_ms.mean()) * 1e3,
                          "sparse attention (attn+merge kernels)": float(att_ms.mean()) * 1e3,
                          "dense flash-decode comparator": float(np.mean(den)) * 1e3,
+                         "step replayed from a CUDA graph": graph_us,
                          "upstream f1 alone (projection + RoPE + append; not in the step)": float(np.mean(f1_ms)) * 1e3},
         "upstream_f1": {"us": float(np.mean(f1_ms)) * 1e3, "weight_bytes": f1_bytes, "d_model": d_model,
                         "note": "latency-bound: %.1f MiB of weights = %.2f us at the measured copy peak"

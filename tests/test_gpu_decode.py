@@ -357,3 +357,43 @@ def test_many_short_sequences(torch_cuda):
             err = np.abs(out[b] - want)
             assert err.max() <= MAX_ABS and err.mean() <= MEAN_ABS, (b, err.max(), err.mean())
             assert np.abs(lse[b] - want_lse).max() <= 1e-3
+
+
+def test_decode_step_is_capturable_in_a_cuda_graph(torch_cuda):
+    """Every call is asynchronous on the caller's stream and never synchronises (include/spot.h), so a decode step
+    (spot_select + spot_sparse_attn_decode, four kernels chained by programmatic dependent launch) can be captured in a
+    CUDA graph; the replay gives the same bits as the eager step."""
+    torch = torch_cuda
+    from paper_2606_22874_b200 import api
+    wl = make_config("mini2")
+    dd = H.DeviceDecode(wl, "mxfp4")
+    B, nb = wl.B, dd.n_b_max
+    idx = torch.zeros((B, nb), dtype=torch.int32, device="cuda")
+    bud = torch.zeros((B,), dtype=torch.int32, device="cuda")
+    out = torch.zeros((B, wl.H_q, wl.D), dtype=torch.int16, device="cuda")
+    sp = api.make_select_params(dd.sel_q, dd.w, dd.sel_k, "mxfp4", dd.L_cap, dd.seq_len, dd.max_seq_len, B, 1, wl.H_idx,
+                                wl.d_idx, indices=idx, cap=nb, budgets=bud)
+    ws1 = torch.empty(max(16, api.spot_select_workspace_bytes(sp)), dtype=torch.uint8, device="cuda")
+    sp.workspace, sp.workspace_bytes = ws1.data_ptr(), ws1.numel()
+    ap = api.make_attn_params(dd.q, dd.K, dd.V, dd.kv_strides, dd.seq_len, dd.max_seq_len, idx, bud, nb, B, 1, wl.H_q,
+                              wl.H_kv, wl.D, sm_scale=wl.sm_scale, out=out)
+    ws2 = torch.empty(max(16, api.spot_sparse_attn_decode_workspace_bytes(ap)), dtype=torch.uint8, device="cuda")
+    ap.workspace, ap.workspace_bytes = ws2.data_ptr(), ws2.numel()
+    s = torch.cuda.Stream()
+    with torch.cuda.stream(s):
+        api.spot_select(sp, s)
+        api.spot_sparse_attn_decode(ap, s)
+    s.synchronize()
+    ref_out, ref_bud, ref_idx = out.clone(), bud.clone(), idx.clone()
+    out.zero_(); bud.zero_(); idx.zero_()
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g, stream=s):
+        api.spot_select(sp, torch.cuda.current_stream())
+        api.spot_sparse_attn_decode(ap, torch.cuda.current_stream())
+    out.zero_(); bud.zero_(); idx.zero_()
+    g.replay()
+    torch.cuda.synchronize()
+    assert torch.equal(bud, ref_bud) and torch.equal(idx, ref_idx) and torch.equal(out, ref_out)
+    for b in range(B):
+        s_bar, sel = H.oracle_select(wl, "mxfp4", b)
+        assert idx[b, :bud[b]].tolist() == sel.indices.tolist()
