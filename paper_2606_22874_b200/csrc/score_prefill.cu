@@ -199,9 +199,8 @@ __global__ void __launch_bounds__(PF_THREADS, 1) score_prefill_kernel(const __gr
                     const int ts = acc % PF_TSTAGES;
                     mbar_wait(bar_t_full + 8 * ts, (acc / PF_TSTAGES) & 1);
                     tc_fence_after();
-                    float d[4][16];
-#pragma unroll
-                    for (int q4 = 0; q4 < 4; ++q4) tmem_ld16(t_lane + ts * PF_N + q4 * 16, d[q4]);
+                    float dd[64];
+                    tmem_ld64(t_lane + ts * PF_N, dd);
                     tmem_ld_wait();
                     tc_fence_before();
                     __syncwarp();
@@ -212,7 +211,7 @@ __global__ void __launch_bounds__(PF_THREADS, 1) score_prefill_kernel(const __gr
                         for (int i = 0; i < 16; i += 2) {
                             float& s0 = S[q4 * 16 + i];
                             float& s1 = S[q4 * 16 + i + 1];
-                            const float d0 = d[q4][i], d1 = d[q4][i + 1];
+                            const float d0 = dd[q4 * 16 + i], d1 = dd[q4 * 16 + i + 1];
                             if (h == 0) {
                                 s0 = wh0 * (d0 + fabsf(d0));
                                 s1 = wh0 * (d1 + fabsf(d1));
