@@ -38,6 +38,8 @@ def selector_k_bytes(fmt, n_elements):
         return 2 * n_elements
     if fmt in ("mxfp4", "int4_e4m3"):
         return n_elements // 2 + n_elements // GROUP
+    if fmt == "fp8_e4m3":                # f2: one E4M3 byte per element, no scale (the paper's "0.5x" variants)
+        return n_elements
     if fmt == "int4_scale16":            # the paper's 4.5 bit/elt accounting
         return n_elements // 2 + 2 * (n_elements // GROUP)
     raise ValueError(fmt)
@@ -175,6 +177,27 @@ def dequantize_int4_e4m3(q, scale_code):
     return out.reshape(q.shape)
 
 
+# --------------------------------------------------------------------------
+# FP8-E4M3 per element (R30): the paper lists FP8 among the selector-cache precisions
+# (Table 9) at half the BF16 footprint and says nothing else.
+# --------------------------------------------------------------------------
+
+def quantize_fp8_e4m3(k_bits):
+    """BF16 bits [..., d] -> uint8 codes [..., d]: sign bit | RNE-satfinite E4M3 of |v| (no scale, saturating at 448,
+    subnormals down to 2^-9, a zero keeps its sign)."""
+    k_bits = np.asarray(k_bits, dtype=np.uint16)
+    v = bf16_bits_to_f32(k_bits)
+    sign = (k_bits >> np.uint16(15)).astype(np.uint8)
+    return (sign << np.uint8(7)) | encode_e4m3_rne_satfinite(np.abs(v))
+
+
+def dequantize_fp8_e4m3(codes):
+    """-> float64 [..., d]; 4 significant bits, so exact in BF16."""
+    codes = np.asarray(codes, dtype=np.uint8)
+    mag = e4m3_value(codes & np.uint8(0x7F))
+    return np.where(codes >> np.uint8(7), -mag, mag)
+
+
 def quantize_dequantize(fmt, k_bits):
     """Convenience: BF16 bits -> float64 dequantised keys for a format name."""
     if fmt == "bf16":
@@ -184,4 +207,6 @@ def quantize_dequantize(fmt, k_bits):
         return dequantize_mxfp4(*quantize_mxfp4(k_bits))
     if fmt == "int4_e4m3":
         return dequantize_int4_e4m3(*quantize_int4_e4m3(k_bits))
+    if fmt == "fp8_e4m3":
+        return dequantize_fp8_e4m3(quantize_fp8_e4m3(k_bits))
     raise ValueError(fmt)

@@ -242,3 +242,29 @@ def test_dequantised_keys_are_bf16_exact_and_sign_of_zero():
     X = np.ldexp(1.0, scale.astype(int) - 127)
     err = np.abs(quant.dequantize_mxfp4(codes, scale) - bf16_bits_to_f64(bits)).reshape(64, 4, 2, 32)
     assert np.all(err < 2 * X[..., None])
+
+
+def test_fp8_cache_is_nearest_e4m3_value_per_element():
+    """f2 (R30): every element goes to the nearest of the 253 finite E4M3 values (ties to the even code),
+    saturating at +-448 -- brute force over the value table; every finite code round-trips; half the BF16 footprint."""
+    table = quant.e4m3_value(np.arange(0x7F))                            # 0 .. 448, increasing
+    assert table[0] == 0.0 and table[-1] == 448.0 and np.all(np.diff(table) > 0)
+    rng = np.random.default_rng(8)
+    x = np.concatenate([rng.standard_normal(4000) * 3, rng.standard_normal(500) * 300, rng.standard_normal(500) * 1e-3,
+                        [0.0, -0.0, 448.0, -448.0, 460.0, 1e9, -1e9, 2.0 ** -9, 2.0 ** -10, 3 * 2.0 ** -10]]).astype(np.float32)
+    bits = f32_to_bf16_bits(x)
+    v = bf16_bits_to_f64(bits)
+    codes = quant.quantize_fp8_e4m3(bits)
+    got = quant.dequantize_fp8_e4m3(codes)
+    for vi, ci, gi in zip(v, codes, got):
+        a = min(abs(vi), 448.0)
+        d = np.abs(table - a)
+        best = np.flatnonzero(d == d.min())
+        want_code = best[0] if len(best) == 1 else [c for c in best if c % 2 == 0][0]
+        assert int(ci & 0x7F) == want_code, (vi, ci, want_code)
+        assert (ci >> 7) == (1 if np.signbit(vi) else 0)
+        assert gi == (-table[want_code] if np.signbit(vi) else table[want_code])
+    all_codes = np.concatenate([np.arange(0x7F), 0x80 + np.arange(0x7F)]).astype(np.uint8)
+    vals = quant.dequantize_fp8_e4m3(all_codes)
+    assert np.array_equal(quant.quantize_fp8_e4m3(f32_to_bf16_bits(vals.astype(np.float32))) & 0x7F, all_codes & 0x7F)
+    assert quant.selector_k_bytes("fp8_e4m3", 131072 * 36 * 512) * 2 == quant.selector_k_bytes("bf16", 131072 * 36 * 512)
