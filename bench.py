@@ -351,7 +351,8 @@ def run_ours(args):
         return
 
     peak, peak_src = measured_peaks()
-    bytes_per_tok = {"bf16": wl.H_idx * wl.d_idx * 2}.get(args.fmt, wl.H_idx * wl.d_idx // 2 + wl.H_idx * wl.d_idx // 32)
+    bytes_per_tok = {"bf16": wl.H_idx * wl.d_idx * 2, "fp8_e4m3": wl.H_idx * wl.d_idx}.get(
+        args.fmt, wl.H_idx * wl.d_idx // 2 + wl.H_idx * wl.d_idx // 32)
     sel_alg = float(np.sum(wl.seq_len.astype(np.int64)) * bytes_per_tok)
     kv_alg = float(np.sum(bud_host.astype(np.int64)) * wl.blk * Hkv * D * 2 * 2)
     att_s = float(att_ms.mean()) * 1e-3
@@ -658,7 +659,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="cfg3")
-    ap.add_argument("--fmt", default="bf16", choices=["bf16", "mxfp4", "int4_e4m3"])
+    ap.add_argument("--fmt", default="bf16", choices=["bf16", "mxfp4", "int4_e4m3", "fp8_e4m3"])
     ap.add_argument("--p", type=float, default=0.90)
     ap.add_argument("--L", type=int, default=0, help="cfg5 only: prompt length (default 65536)")
     ap.add_argument("--d-idx", type=int, default=0, choices=[0, 64, 128],

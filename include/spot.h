@@ -47,7 +47,8 @@ typedef enum {
 typedef enum {
     SPOT_SELK_BF16 = 0,      /* [B][cache_stride_tokens][H_idx][d_idx] BF16                              */
     SPOT_SELK_INT4_E4M3 = 1, /* signed 4-bit codes, group 32 along d_idx, one FP8-E4M3 scale per group   */
-    SPOT_SELK_MXFP4 = 2      /* E2M1 codes, group 32 along d_idx, one E8M0 scale per group (OCP MX)      */
+    SPOT_SELK_MXFP4 = 2,     /* E2M1 codes, group 32 along d_idx, one E8M0 scale per group (OCP MX)      */
+    SPOT_SELK_FP8_E4M3 = 3   /* f2: one FP8-E4M3 byte per element, no scale, [B][tokens][H_idx][d_idx]   */
 } spot_selk_format;
 
 typedef enum {
@@ -73,7 +74,8 @@ size_t spot_struct_size(int which);
  *
  * Bytes of a cache holding B sequences of cache_stride_tokens tokens each (a multiple of 64 for the 4-bit
  * formats): BF16 2*n, 4-bit formats n/2 + n/32 with n = B*tokens*H_idx*d_idx (16 -> 4.25
- * bit/element).  Returns 0 on invalid arguments.
+ * bit/element), FP8-E4M3 n (the paper's "FP8" precision; R30: RNE-satfinite cast of every
+ * element, no scale).  Returns 0 on invalid arguments.
  * --------------------------------------------------------------------------------------------------- */
 size_t spot_selector_k_bytes(spot_selk_format fmt, int64_t B, int64_t cache_stride_tokens, int H_idx, int d_idx);
 

@@ -129,7 +129,7 @@ def encode_e4m3_rne_satfinite(x):
     code = np.zeros(x.shape, dtype=np.int64)
     # subnormal range: multiples of 2^-9 below 2^-6
     sub = x < 2.0 ** -6
-    rs = np.rint(x / 2.0 ** -9).astype(np.int64)      # 0..8, half-to-even; 8 == min normal 0x08
+    rs = np.rint(np.where(sub, x, 0.0) / 2.0 ** -9).astype(np.int64)   # 0..8, half-to-even; 8 == min normal 0x08
     code = np.where(sub, rs, code)
     # normal range
     _, ex = np.frexp(np.where(sub, 1.0, x))

@@ -52,7 +52,8 @@ spot_status select_geometry(const spot_select_params* p, SelectGeom* g, bool sco
     if (!p->sel_q || !p->w || !p->sel_k) return SPOT_ERR_INVALID_ARG;
     if (score_only ? !p->block_scores : (!p->indices || !p->budgets)) return SPOT_ERR_INVALID_ARG;
     if (!aligned16(p->sel_q) || !aligned16(p->sel_k) || !aligned16(p->w)) return SPOT_ERR_INVALID_ARG;
-    if (p->fmt != SPOT_SELK_BF16 && p->fmt != SPOT_SELK_INT4_E4M3 && p->fmt != SPOT_SELK_MXFP4) return SPOT_ERR_INVALID_ARG;
+    if (p->fmt != SPOT_SELK_BF16 && p->fmt != SPOT_SELK_INT4_E4M3 && p->fmt != SPOT_SELK_MXFP4 &&
+        p->fmt != SPOT_SELK_FP8_E4M3) return SPOT_ERR_INVALID_ARG;
     if (p->mode != SPOT_MODE_TOPK && p->mode != SPOT_MODE_DUAL_TOPP) return SPOT_ERR_INVALID_ARG;
     if (p->B <= 0 || p->Tq <= 0 || p->H_idx <= 0 || p->d_idx <= 0 || p->d_idx % 32 != 0) return SPOT_ERR_INVALID_ARG;
     if (p->blk <= 0 || (!score_only && p->cap <= 0) || p->cache_stride_tokens <= 0) return SPOT_ERR_INVALID_ARG;
@@ -60,7 +61,8 @@ spot_status select_geometry(const spot_select_params* p, SelectGeom* g, bool sco
     if (p->mode == SPOT_MODE_DUAL_TOPP && !(p->p > 0.0 && p->p <= 1.0)) return SPOT_ERR_INVALID_ARG;
     if (!(p->temperature > 0.0)) return SPOT_ERR_INVALID_ARG;
     if (p->mode == SPOT_MODE_TOPK && p->top_k < p->sink_blocks + p->recency_blocks) return SPOT_ERR_INVALID_ARG;
-    if (p->fmt != SPOT_SELK_BF16 && p->cache_stride_tokens % SELK_TILE != 0) return SPOT_ERR_INVALID_ARG;
+    if (p->fmt != SPOT_SELK_BF16 && p->cache_stride_tokens % SELK_TILE != 0)
+        return SPOT_ERR_INVALID_ARG;
     if (p->blk != 64) return SPOT_ERR_UNSUPPORTED;
     int64_t max_tokens;
     if (p->q_block == 1) {

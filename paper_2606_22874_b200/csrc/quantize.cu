@@ -171,6 +171,58 @@ __global__ void __launch_bounds__(256) dequantize_kernel(const uint8_t* __restri
     for (int i = 0; i < 4; ++i) dst[i] = make_uint4(o[4 * i], o[4 * i + 1], o[4 * i + 2], o[4 * i + 3]);
 }
 
+// f2 -- FP8-E4M3 per element (R30): cache [B][tokens][H*d] bytes, byte = cvt.rn.satfinite.e4m3x2.f32 of
+// the element (RNE onto the E4M3 grid, saturating at +-448, sign of zero kept); 16 elements per thread.
+__global__ void __launch_bounds__(256) fp8_quantize_kernel(const uint16_t* __restrict__ k_in, uint8_t* __restrict__ cache,
+                                                           int64_t n_tokens, int64_t token_offset, int64_t stride_tokens,
+                                                           int64_t vec_per_token, int64_t total,
+                                                           const int32_t* __restrict__ pos) {
+    pdl_wait();
+    int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= total) return;
+    const int64_t per_seq = n_tokens * vec_per_token;
+    const int64_t b = i / per_seq, r = i - b * per_seq;
+    int64_t t = token_offset + r / vec_per_token;
+    if (pos) {
+        t = pos[b];
+        if (t < 0 || t >= stride_tokens) return;
+    }
+    const uint4* src = reinterpret_cast<const uint4*>(k_in + i * 16);
+    const uint4 x0 = ldg_stream_v4(src), x1 = ldg_stream_v4(src + 1);
+    const uint32_t w[8] = {x0.x, x0.y, x0.z, x0.w, x1.x, x1.y, x1.z, x1.w};
+    uint32_t o[4];
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+        const uint32_t lo = __nv_cvt_float2_to_fp8x2(make_float2(bf16lo(w[2 * j]), bf16hi(w[2 * j])), __NV_SATFINITE, __NV_E4M3);
+        const uint32_t hi = __nv_cvt_float2_to_fp8x2(make_float2(bf16lo(w[2 * j + 1]), bf16hi(w[2 * j + 1])), __NV_SATFINITE, __NV_E4M3);
+        o[j] = (lo & 0xffffu) | (hi << 16);
+    }
+    *reinterpret_cast<uint4*>(cache + ((b * stride_tokens + t) * vec_per_token + r % vec_per_token) * 16) =
+        make_uint4(o[0], o[1], o[2], o[3]);
+}
+
+__global__ void __launch_bounds__(256) fp8_dequantize_kernel(const uint8_t* __restrict__ cache, uint16_t* __restrict__ k_out,
+                                                             int64_t n_tokens, int64_t token_offset, int64_t stride_tokens,
+                                                             int64_t vec_per_token, int64_t total) {
+    int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= total) return;
+    const int64_t per_seq = n_tokens * vec_per_token;
+    const int64_t b = i / per_seq, r = i - b * per_seq;
+    const int64_t t = token_offset + r / vec_per_token;
+    const uint4 c = *reinterpret_cast<const uint4*>(cache + ((b * stride_tokens + t) * vec_per_token + r % vec_per_token) * 16);
+    const uint32_t cw[4] = {c.x, c.y, c.z, c.w};
+    uint32_t o[8];
+#pragma unroll
+    for (int j = 0; j < 8; ++j) {
+        const __half2_raw h = __nv_cvt_fp8x2_to_halfraw2((__nv_fp8x2_storage_t)((cw[j >> 1] >> (16 * (j & 1))) & 0xffffu), __NV_E4M3);
+        const float lo = __half2float(__ushort_as_half(h.x)), hi = __half2float(__ushort_as_half(h.y));
+        o[j] = pack_bf16x2(lo, hi);                       // exact: E4M3 values have 4 significant bits
+    }
+    uint4* dst = reinterpret_cast<uint4*>(k_out + i * 16);
+    dst[0] = make_uint4(o[0], o[1], o[2], o[3]);
+    dst[1] = make_uint4(o[4], o[5], o[6], o[7]);
+}
+
 // BF16 "format": plain row copy into / out of the cache (16 B per thread).
 __global__ void __launch_bounds__(256) copy_rows_kernel(const uint4* __restrict__ src, uint4* __restrict__ dst,
                                                         int64_t n_tokens, int64_t vec_per_token,
@@ -193,7 +245,8 @@ __global__ void __launch_bounds__(256) copy_rows_kernel(const uint4* __restrict_
 spot_status check_quant_args(const void* a, const void* b, int fmt, int64_t B, int64_t n_tokens, int64_t token_offset,
                              int64_t stride, int H, int d) {
     if (!a || !b || !aligned16(a) || !aligned16(b)) return SPOT_ERR_INVALID_ARG;
-    if (fmt != SPOT_SELK_BF16 && fmt != SPOT_SELK_INT4_E4M3 && fmt != SPOT_SELK_MXFP4) return SPOT_ERR_INVALID_ARG;
+    if (fmt != SPOT_SELK_BF16 && fmt != SPOT_SELK_INT4_E4M3 && fmt != SPOT_SELK_MXFP4 && fmt != SPOT_SELK_FP8_E4M3)
+        return SPOT_ERR_INVALID_ARG;
     if (B <= 0 || n_tokens <= 0 || token_offset < 0 || H <= 0 || d <= 0 || d % 32 != 0) return SPOT_ERR_INVALID_ARG;
     if (token_offset + n_tokens > stride) return SPOT_ERR_INVALID_ARG;
     if (fmt != SPOT_SELK_BF16 && stride % SELK_TILE != 0) return SPOT_ERR_INVALID_ARG;
@@ -211,6 +264,12 @@ spot_status append_selector_k(const uint16_t* k_new, void* cache, int fmt, int B
         SPOT_CUDA_TRY(launch_pdl(copy_rows_kernel, dim3((unsigned)ceil_div64(total, 256)), dim3(256), 0, s,
                                  (const uint4*)k_new, (uint4*)cache, (int64_t)1, vpt, (int64_t)1, (int64_t)0, stride,
                                  (int64_t)0, total, pos));
+        return SPOT_OK;
+    }
+    if (fmt == SPOT_SELK_FP8_E4M3) {
+        const int64_t vpt = (int64_t)H * d / 16, total = (int64_t)B * vpt;
+        SPOT_CUDA_TRY(launch_pdl(fp8_quantize_kernel, dim3((unsigned)ceil_div64(total, 256)), dim3(256), 0, s, k_new,
+                                 (uint8_t*)cache, (int64_t)1, (int64_t)0, stride, vpt, total, pos));
         return SPOT_OK;
     }
     const int gpt = H * d / 32;
@@ -237,6 +296,7 @@ extern "C" size_t spot_selector_k_bytes(spot_selk_format fmt, int64_t B, int64_t
         if (tokens % SELK_TILE != 0) return 0;
         return (size_t)(n / 2 + n / 32);
     }
+    if (fmt == SPOT_SELK_FP8_E4M3) return tokens % SELK_TILE != 0 ? 0 : (size_t)n;
     return 0;
 }
 
@@ -251,6 +311,13 @@ extern "C" spot_status spot_quantize_selector_k(const uint16_t* k_bf16, void* k_
         int64_t vpt = (int64_t)H_idx * d_idx / 8, total = B * n_tokens * vpt;
         copy_rows_kernel<<<(unsigned)ceil_div64(total, 256), 256, 0, s>>>(
             (const uint4*)k_bf16, (uint4*)k_cache, n_tokens, vpt, n_tokens, 0, cache_stride_tokens, token_offset, total, nullptr);
+        SPOT_LAUNCH_CHECK();
+        return SPOT_OK;
+    }
+    if (fmt == SPOT_SELK_FP8_E4M3) {
+        const int64_t vpt = (int64_t)H_idx * d_idx / 16, total = B * n_tokens * vpt;
+        fp8_quantize_kernel<<<(unsigned)ceil_div64(total, 256), 256, 0, s>>>(k_bf16, (uint8_t*)k_cache, n_tokens, token_offset,
+                                                                             cache_stride_tokens, vpt, total, nullptr);
         SPOT_LAUNCH_CHECK();
         return SPOT_OK;
     }
@@ -277,6 +344,13 @@ extern "C" spot_status spot_dequantize_selector_k(const void* k_cache, uint16_t*
         int64_t vpt = (int64_t)H_idx * d_idx / 8, total = B * n_tokens * vpt;
         copy_rows_kernel<<<(unsigned)ceil_div64(total, 256), 256, 0, s>>>(
             (const uint4*)k_cache, (uint4*)k_bf16_out, n_tokens, vpt, cache_stride_tokens, token_offset, n_tokens, 0, total, nullptr);
+        SPOT_LAUNCH_CHECK();
+        return SPOT_OK;
+    }
+    if (fmt == SPOT_SELK_FP8_E4M3) {
+        const int64_t vpt = (int64_t)H_idx * d_idx / 16, total = B * n_tokens * vpt;
+        fp8_dequantize_kernel<<<(unsigned)ceil_div64(total, 256), 256, 0, s>>>((const uint8_t*)k_cache, k_bf16_out, n_tokens,
+                                                                               token_offset, cache_stride_tokens, vpt, total);
         SPOT_LAUNCH_CHECK();
         return SPOT_OK;
     }

@@ -105,7 +105,8 @@ __device__ __forceinline__ void bulk_load(uint32_t smem_dst, const void* gsrc, u
 template <int H, int D_IDX, int FMT>
 struct ScoreCfg {
     static constexpr int ROW = H * D_IDX;                      // elements per token
-    static constexpr int TILE_BYTES = FMT == SPOT_SELK_BF16 ? 64 * ROW * 2 : 64 * (ROW / 2 + ROW / 32);
+    static constexpr int TILE_BYTES = FMT == SPOT_SELK_BF16 ? 64 * ROW * 2
+                                      : FMT == SPOT_SELK_FP8_E4M3 ? 64 * ROW : 64 * (ROW / 2 + ROW / 32);
     static constexpr bool SELF = FMT != SPOT_SELK_BF16;
     // BF16 (producer ring): few big tiles (32 / 64 KiB, 1024-byte aligned for the 128-byte swizzle) and a light
     // ldmatrix + HMMA body.  One producer lane feeds the ring; every stage belongs to ONE consumer warp (stage s ->
@@ -118,7 +119,8 @@ struct ScoreCfg {
     // ring depth: 12 warps x 2 stages beat 8 x 3 (MXFP4 20 -> 17 us); 16 warps x 3 half-tile stages were slower again.
     static constexpr int STAGE_BYTES = SELF ? TILE_BYTES : (TILE_BYTES + 1023) / 1024 * 1024;
     static constexpr int STAGES_RAW = SC_SMEM_BUDGET / STAGE_BYTES;
-    static constexpr int CONSUMERS = SELF ? (TILE_BYTES <= 8704 ? 12 : 6) : (STAGES_RAW > 6 ? 6 : STAGES_RAW);
+    static constexpr int SELF_MAX = (208 * 1024 / STAGE_BYTES) / 2;           // warps that fit with 2 stages each
+    static constexpr int CONSUMERS = SELF ? (SELF_MAX > 12 ? 12 : SELF_MAX) : (STAGES_RAW > 6 ? 6 : STAGES_RAW);
     static constexpr int PER_WARP = SELF ? 2 : 1;
     static constexpr int STAGES = CONSUMERS * PER_WARP;
     static constexpr int THREADS = (CONSUMERS + (SELF ? 0 : 1)) * 32;
@@ -334,6 +336,111 @@ struct Q4Tile {
     }
 };
 
+// ---- FP8-E4M3 tile (f2): [64 tokens][ROW] bytes, one byte per element, no scales ---------------------------
+// Same scheme as the 4-bit tiles -- fp16 HMMA against the power-of-two pre-scaled fp16 query, the k index a fixed
+// permutation so that a lane's 16-byte load lands in fragment registers -- with one cvt.rn.f16x2.e4m3x2 per pair and
+// the query in column 0 only (no per-group scales to keep apart).
+template <int H, int D_IDX>
+struct Fp8Tile {
+    static constexpr int ROW = H * D_IDX;          // bytes per token
+    static constexpr int NQL = ROW / 64;           // 64-byte quad loads per token (16 B per lane of a quad)
+    static constexpr int QPH = D_IDX / 64;         // quad loads per head
+    static_assert(D_IDX % 64 == 0, "d_idx must be a multiple of 64 for the FP8 scoring kernel");
+    uint32_t qf[NQL][8];
+    float wq[H], ps[H];
+
+    __device__ __forceinline__ void load_query(const ScoreArgs& a, int b, int lane, uint32_t q16_addr) {
+        const int g = lane >> 2, c = lane & 3;
+        __half* q16 = reinterpret_cast<__half*>(__cvta_shared_to_generic((size_t)q16_addr));
+        float* post = reinterpret_cast<float*>(q16 + ROW);
+        constexpr int EPL = ROW / 32, LPH = 32 / H;
+        static_assert(EPL % 8 == 0 && LPH * EPL == D_IDX && (LPH & (LPH - 1)) == 0, "query staging geometry");
+        __syncwarp();
+        uint4 raw[EPL / 8];
+#pragma unroll
+        for (int i = 0; i < EPL / 8; ++i)
+            raw[i] = *reinterpret_cast<const uint4*>(a.sel_q + (int64_t)b * ROW + lane * EPL + i * 8);
+        float v[EPL], mx = 0.f;
+#pragma unroll
+        for (int i = 0; i < EPL / 8; ++i) {
+            const uint32_t wds[4] = {raw[i].x, raw[i].y, raw[i].z, raw[i].w};
+#pragma unroll
+            for (int j = 0; j < 4; ++j) { v[i * 8 + 2 * j] = bf16lo(wds[j]); v[i * 8 + 2 * j + 1] = bf16hi(wds[j]); }
+        }
+#pragma unroll
+        for (int i = 0; i < EPL; ++i) mx = fmaxf(mx, fabsf(v[i]));
+#pragma unroll
+        for (int o = LPH / 2; o; o >>= 1) mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, o));
+        int sh = 0;
+        if (mx > 0.f) sh = 14 - ilogbf(mx);       // E4M3 magnitudes reach 448 = 2^8.8: products stay below 2^24
+        sh = max(-100, min(100, sh));
+        sh -= 9;                                   // keep |q16| * 448 * d_idx inside fp32-exact accumulation range
+        const float up = __uint_as_float((uint32_t)(127 + sh) << 23);
+#pragma unroll
+        for (int i = 0; i < EPL; ++i) q16[lane * EPL + i] = __float2half_rn(v[i] * up);
+        if (lane % LPH == 0) post[lane / LPH] = __uint_as_float((uint32_t)(127 - sh) << 23);
+        __syncwarp();
+#pragma unroll
+        for (int ql = 0; ql < NQL; ++ql)
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+                const uint32_t* src = reinterpret_cast<const uint32_t*>(q16 + ql * 64 + 16 * c + 4 * j);
+                qf[ql][2 * j] = (g == 0) ? src[0] : 0u;
+                qf[ql][2 * j + 1] = (g == 0) ? src[1] : 0u;
+            }
+#pragma unroll
+        for (int h = 0; h < H; ++h) { wq[h] = a.w[(int64_t)b * H + h]; ps[h] = post[h]; }
+        __syncwarp();
+    }
+
+    static __device__ __forceinline__ void e4m3x4_to_f16x2x2(uint32_t w, uint32_t& lo, uint32_t& hi) {
+        asm("{ .reg .b16 l, h; mov.b32 {l, h}, %2; cvt.rn.f16x2.e4m3x2 %0, l; cvt.rn.f16x2.e4m3x2 %1, h; }"
+            : "=r"(lo), "=r"(hi) : "r"(w));
+    }
+
+    __device__ __forceinline__ float tile_max(uint32_t st, int t0, int L, int lane) const {
+        const int g = lane >> 2, c = lane & 3;
+        float m = -INFINITY;
+#pragma unroll 2
+        for (int it = 0; it < 4; ++it) {
+            uint4 ca[NQL], cb[NQL];
+#pragma unroll
+            for (int ql = 0; ql < NQL; ++ql) {
+                ca[ql] = lds128(st + (it * 16 + g) * ROW + ql * 64 + c * 16);
+                cb[ql] = lds128(st + (it * 16 + 8 + g) * ROW + ql * 64 + c * 16);
+            }
+            float sa = 0.f, sb = 0.f;
+#pragma unroll
+            for (int h = 0; h < H; ++h) {
+                float acc[4] = {0.f, 0.f, 0.f, 0.f};
+#pragma unroll
+                for (int qq = 0; qq < QPH; ++qq) {
+                    const int ql = h * QPH + qq;
+                    const uint32_t wa[4] = {ca[ql].x, ca[ql].y, ca[ql].z, ca[ql].w};
+                    const uint32_t wb[4] = {cb[ql].x, cb[ql].y, cb[ql].z, cb[ql].w};
+#pragma unroll
+                    for (int j = 0; j < 4; ++j) {
+                        uint32_t a0, a2, a1, a3;
+                        e4m3x4_to_f16x2x2(wa[j], a0, a2);
+                        e4m3x4_to_f16x2x2(wb[j], a1, a3);
+                        mma_f16_16816(acc, a0, a1, a2, a3, qf[ql][2 * j], qf[ql][2 * j + 1]);
+                    }
+                }
+                sa = fmaf(wq[h], fmaxf(acc[0] * ps[h], 0.f), sa);     // column 0, row g     (valid on lanes c == 0)
+                sb = fmaf(wq[h], fmaxf(acc[2] * ps[h], 0.f), sb);     // column 0, row g + 8
+            }
+            const int ta = t0 + it * 16 + g, tb = ta + 8;
+            if (ta < L) m = fmaxf(m, sa);
+            if (tb < L) m = fmaxf(m, sb);
+        }
+        if (c != 0) m = -INFINITY;
+        m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, 4));
+        m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, 8));
+        m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, 16));
+        return m;
+    }
+};
+
 template <int H, int D_IDX, int FMT>
 __global__ void __launch_bounds__((ScoreCfg<H, D_IDX, FMT>::THREADS), 1) score_decode_kernel(const __grid_constant__ CUtensorMap tm_k,
                                                                      const ScoreArgs a) {
@@ -374,7 +481,7 @@ __global__ void __launch_bounds__((ScoreCfg<H, D_IDX, FMT>::THREADS), 1) score_d
         // ================================ self-serve consumers (4-bit) ================================
         // warp w streams tiles w, w + C, w + 2C, ... through its own stages w*K .. w*K + K-1
         constexpr int K = Cfg::PER_WARP;
-        Q4Tile<H, D_IDX, FMT> tile;
+        typename std::conditional<FMT == SPOT_SELK_FP8_E4M3, Fp8Tile<H, D_IDX>, Q4Tile<H, D_IDX, FMT>>::type tile;
         cur.advance(a, warp);
         TileCursor nxt = cur;                      // the next tile to request
         auto request = [&](int j) {                // j-th tile of this warp -> stage w*K + j % K   (lane 0 only)
@@ -479,6 +586,7 @@ template <int H, int D_IDX>
 spot_status launch_score(const spot_select_params* p, float* scores, int nb_stride, cudaStream_t s) {
     if (p->fmt == SPOT_SELK_BF16) return launch_score_fmt<H, D_IDX, SPOT_SELK_BF16>(p, scores, nb_stride, s);
     if (p->fmt == SPOT_SELK_MXFP4) return launch_score_fmt<H, D_IDX, SPOT_SELK_MXFP4>(p, scores, nb_stride, s);
+    if (p->fmt == SPOT_SELK_FP8_E4M3) return launch_score_fmt<H, D_IDX, SPOT_SELK_FP8_E4M3>(p, scores, nb_stride, s);
     return launch_score_fmt<H, D_IDX, SPOT_SELK_INT4_E4M3>(p, scores, nb_stride, s);
 }
 

@@ -62,6 +62,7 @@ def test_selector_k_bytes_matches_the_papers_footprint(lib):
     assert round(fp4 / 2 ** 30, 2) == 1.20
     # the measured geometry: 4 x 64, 136 B per token
     assert api.spot_selector_k_bytes("mxfp4", 4, 131072, 4, 64) == 4 * 131072 * 136
+    assert api.spot_selector_k_bytes("fp8_e4m3", 1, n_tok, 4, 128) * 2 == bf16           # f2: the paper's 0.5x
     # invalid: unknown format, d_idx not a multiple of 32, capacity not a multiple of the 64-token tile
     assert lib.spot_selector_k_bytes(7, 1, 64, 4, 64) == 0
     assert api.spot_selector_k_bytes("mxfp4", 1, 64, 4, 48) == 0

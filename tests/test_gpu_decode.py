@@ -26,7 +26,7 @@ def torch_cuda():
 
 
 # ---------------------------------------------------------------- a0 quantisers
-@pytest.mark.parametrize("fmt", ["mxfp4", "int4_e4m3"])
+@pytest.mark.parametrize("fmt", ["mxfp4", "int4_e4m3", "fp8_e4m3"])
 def test_quantise_dequantise_bit_exact(torch_cuda, fmt):
     torch = torch_cuda
     from paper_2606_22874_b200 import api
@@ -74,7 +74,7 @@ def _check_select(dd, fmt, report, **over):
     return idx, bud
 
 
-@pytest.mark.parametrize("fmt", ["bf16", "mxfp4", "int4_e4m3"])
+@pytest.mark.parametrize("fmt", ["bf16", "mxfp4", "int4_e4m3", "fp8_e4m3"])
 @pytest.mark.parametrize("cfg", ["cfg1", "mini2", "mini3", "mini4"])
 def test_select_matches_oracle(torch_cuda, cfg, fmt):
     wl = make_config(cfg, with_kv=False)
@@ -98,7 +98,7 @@ def test_select_edge_cases(torch_cuda):
                                   with_kv=False)
         if seed == 2:
             wl.sel_k[2, 64:128] = wl.sel_k[2, 128:192]      # blocks 1 and 2 tie exactly -> index tie-break (R7)
-        for fmt in ("bf16", "mxfp4", "int4_e4m3"):
+        for fmt in ("bf16", "mxfp4", "int4_e4m3", "fp8_e4m3"):
             dd = H.DeviceDecode(wl, fmt, with_kv=False)
             report = []
             for over in (dict(), dict(p=0.5, kmin_blocks=0), dict(sink_blocks=0, recency_blocks=0, kmin_blocks=0),
@@ -215,7 +215,8 @@ def test_end_to_end_step_matches_oracle(torch_cuda):
 
 @pytest.mark.parametrize("cfg,fmt,seqs", [("cfg3", "bf16", (0, 3)), ("cfg3", "mxfp4", (1,)), ("cfg3", "int4_e4m3", (2,)),
                                           ("cfg2", "bf16", (0, 7)), ("cfg4_b4", "mxfp4", (0, 1, 2, 3)),
-                                          ("cfg3/d128", "bf16", (1,)), ("cfg3/d128", "mxfp4", (2,))])
+                                          ("cfg3/d128", "bf16", (1,)), ("cfg3/d128", "mxfp4", (2,)),
+                                          ("cfg3", "fp8_e4m3", (3,)), ("cfg3/d128", "fp8_e4m3", (0,))])
 def test_full_size_configs_in_the_bench_configuration(torch_cuda, cfg, fmt, seqs):
     """BASELINE.json configs 2, 3 and 4 (batch 4) at full size (config 3: B=4, L=131072, 2048 blocks per sequence;
     config 4: H_q=64 and per-query budgets from the K_min floor to hundreds of blocks), launched exactly as bench.py

@@ -63,7 +63,7 @@ def test_project_rope_append(torch_cuda, B, d_model, d_idx, rope_dims):
     cache_init = f32_to_bf16_bits(rng.standard_normal((B, stride, Hh, d_idx), dtype=np.float32))
     # the kernel takes ONE position per sequence (rotation angle and cache slot); run it per role
     res = {}
-    for fmt in ("bf16", "mxfp4", "int4_e4m3"):
+    for fmt in ("bf16", "mxfp4", "int4_e4m3", "fp8_e4m3"):
         wl_f = dict(wl)
         wl_f["pos"] = slot.astype(np.int32)
         res[fmt] = _run(torch, wl_f, fmt, stride, rope_dims, base, cache_init)
@@ -79,7 +79,7 @@ def test_project_rope_append(torch_cuda, B, d_model, d_idx, rope_dims):
             exact += int(np.sum(got == bf16_bits_to_f64(f32_to_bf16_bits(ref.astype(np.float32)))))
             total += ref.size
         assert np.allclose(w_gpu[b], w_ref, rtol=1e-5, atol=1e-6)
-        for fmt in ("bf16", "mxfp4", "int4_e4m3"):
+        for fmt in ("bf16", "mxfp4", "int4_e4m3", "fp8_e4m3"):
             q_f, w_f, back = res[fmt]
             assert np.array_equal(q_f, q_gpu) and np.array_equal(w_f, w_gpu)          # format-independent outputs
             want_slot = OQ.quantize_dequantize(fmt, k_gpu_bits)
