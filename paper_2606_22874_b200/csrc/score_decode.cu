@@ -117,7 +117,11 @@ struct ScoreCfg {
     // issue a copy per ~350 cycles, so every consumer warp owns PER_WARP stages and refills a stage itself as soon as
     // it has consumed it: no producer warp, no empty barriers.  The unpack's dependent chains want warps more than
     // ring depth: 12 warps x 2 stages beat 8 x 3 (MXFP4 20 -> 17 us); 16 warps x 3 half-tile stages were slower again.
-    static constexpr int STAGE_BYTES = SELF ? TILE_BYTES : (TILE_BYTES + 1023) / 1024 * 1024;
+    // FP8 (self-serve ring, split tiles): a 16 / 32 KiB tile would leave room for 6 / 3 warps only, so a stage holds
+    // an 8 KiB slice (32 / 16 tokens) and a warp walks the SPLIT slices of its tile through its two stages, keeping
+    // the running block maximum in registers.
+    static constexpr int SPLIT = FMT == SPOT_SELK_FP8_E4M3 ? TILE_BYTES / 8192 : 1;
+    static constexpr int STAGE_BYTES = SELF ? TILE_BYTES / SPLIT : (TILE_BYTES + 1023) / 1024 * 1024;
     static constexpr int STAGES_RAW = SC_SMEM_BUDGET / STAGE_BYTES;
     static constexpr int SELF_MAX = (208 * 1024 / STAGE_BYTES) / 2;           // warps that fit with 2 stages each
     static constexpr int CONSUMERS = SELF ? (SELF_MAX > 12 ? 12 : SELF_MAX) : (STAGES_RAW > 6 ? 6 : STAGES_RAW);
@@ -398,11 +402,13 @@ struct Fp8Tile {
             : "=r"(lo), "=r"(hi) : "r"(w));
     }
 
-    __device__ __forceinline__ float tile_max(uint32_t st, int t0, int L, int lane) const {
+    // maximum over NIT * 16 tokens starting at token t0, whose codes start at shared address st
+    template <int NIT>
+    __device__ __forceinline__ float part_max(uint32_t st, int t0, int L, int lane) const {
         const int g = lane >> 2, c = lane & 3;
         float m = -INFINITY;
 #pragma unroll 2
-        for (int it = 0; it < 4; ++it) {
+        for (int it = 0; it < NIT; ++it) {
             uint4 ca[NQL], cb[NQL];
 #pragma unroll
             for (int ql = 0; ql < NQL; ++ql) {
@@ -480,25 +486,30 @@ __global__ void __launch_bounds__((ScoreCfg<H, D_IDX, FMT>::THREADS), 1) score_d
     if constexpr (Cfg::SELF) {
         // ================================ self-serve consumers (4-bit) ================================
         // warp w streams tiles w, w + C, w + 2C, ... through its own stages w*K .. w*K + K-1
-        constexpr int K = Cfg::PER_WARP;
+        // (a stage holds one of the SP slices of a tile; SP == 1 for the 4-bit formats)
+        constexpr int K = Cfg::PER_WARP, SP = Cfg::SPLIT;
         typename std::conditional<FMT == SPOT_SELK_FP8_E4M3, Fp8Tile<H, D_IDX>, Q4Tile<H, D_IDX, FMT>>::type tile;
         cur.advance(a, warp);
-        TileCursor nxt = cur;                      // the next tile to request
-        auto request = [&](int j) {                // j-th tile of this warp -> stage w*K + j % K   (lane 0 only)
-            const uint32_t s = warp * K + j % K;
-            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // earlier generic reads of the stage
-            mbar_arrive_expect_tx(bar_full + 8 * s, Cfg::TILE_BYTES);
-            bulk_load(ring + s * Cfg::STAGE_BYTES,
-                      a.sel_k + ((int64_t)nxt.b * a.tiles_per_seq + nxt.t) * Cfg::TILE_BYTES, Cfg::TILE_BYTES,
-                      bar_full + 8 * s);
-        };
+        TileCursor nxt = cur;                      // the tile of the next slice to request
         const int n_w = (n_my - warp + SC_CONSUMERS - 1) / SC_CONSUMERS;     // tiles of this warp
-#pragma unroll
-        for (int j = 0; j < K; ++j)
-            if (j < n_w) {
-                if (lane == 0) request(j);
-                nxt.advance(a, SC_CONSUMERS);
+        const int n_q = n_w * SP;                  // slices of this warp
+        int rq = 0;                                // next slice to request: slice q -> stage w*K + q % K
+        auto request_next = [&]() {
+            if (rq >= n_q) return;
+            if (lane == 0) {
+                const uint32_t s = warp * K + rq % K;
+                asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // earlier generic reads of the stage
+                mbar_arrive_expect_tx(bar_full + 8 * s, Cfg::STAGE_BYTES);
+                bulk_load(ring + s * Cfg::STAGE_BYTES,
+                          a.sel_k + ((int64_t)nxt.b * a.tiles_per_seq + nxt.t) * Cfg::TILE_BYTES
+                              + (rq % SP) * Cfg::STAGE_BYTES,
+                          Cfg::STAGE_BYTES, bar_full + 8 * s);
             }
+            if (rq % SP == SP - 1) nxt.advance(a, SC_CONSUMERS);
+            ++rq;
+        };
+#pragma unroll
+        for (int j = 0; j < K; ++j) request_next();
         int cur_b = -1, L = 0;
         for (int j = 0; j < n_w; ++j) {
             if (cur.b != cur_b) {
@@ -506,13 +517,19 @@ __global__ void __launch_bounds__((ScoreCfg<H, D_IDX, FMT>::THREADS), 1) score_d
                 L = a.seq_len[cur_b];
                 tile.load_query(a, cur_b, lane, q16_base + warp * (Cfg::ROW * 2 + 64));
             }
-            const uint32_t s = warp * K + j % K;
-            mbar_wait(bar_full + 8 * s, (j / K) & 1);
-            const float m = tile.tile_max(ring + s * Cfg::STAGE_BYTES, cur.t * 64, L, lane);
-            __syncwarp();
-            if (j + K < n_w) {
-                if (lane == 0) request(j + K);
-                nxt.advance(a, SC_CONSUMERS);
+            float m = -INFINITY;
+#pragma unroll
+            for (int part = 0; part < SP; ++part) {
+                const int q = j * SP + part;
+                const uint32_t s = warp * K + q % K;
+                mbar_wait(bar_full + 8 * s, (q / K) & 1);
+                if constexpr (FMT == SPOT_SELK_FP8_E4M3)
+                    m = fmaxf(m, tile.template part_max<4 / SP>(ring + s * Cfg::STAGE_BYTES,
+                                                                cur.t * 64 + part * (64 / SP), L, lane));
+                else
+                    m = tile.tile_max(ring + s * Cfg::STAGE_BYTES, cur.t * 64, L, lane);
+                __syncwarp();
+                request_next();
             }
             if (lane == 0) a.scores[(int64_t)cur_b * a.nb_stride + cur.t] = m;
             cur.advance(a, SC_CONSUMERS);
