@@ -664,9 +664,14 @@ def main():
     ap.add_argument("--L", type=int, default=0, help="cfg5 only: prompt length (default 65536)")
     ap.add_argument("--d-idx", type=int, default=0, choices=[0, 64, 128],
                     help="decode only: selector head dim (default: the config's 64; 128 = the paper's geometry, PAPER.md:363)")
+    ap.add_argument("--blk", type=int, default=64, choices=[64, 16],
+                    help="decode only: selection block size (16 = the paper's geometry with its 8/16/32 reserved "
+                         "sink/recency/K_min blocks, PAPER.md:362-365, :400-402)")
     args = ap.parse_args()
     if args.d_idx:
         D_IDX_OVERRIDE["d_idx"] = args.d_idx
+    if args.blk == 16:
+        D_IDX_OVERRIDE.update(blk=16, sink_blocks=8, recency_blocks=16, kmin_blocks=32)
     if args.workload == "cfg5":
         run_prefill(args)
     elif args.impl == "reference":

@@ -35,6 +35,7 @@ struct AttnArgs {
     const int32_t* indices;      // nullptr: dense
     const int32_t* budgets;
     int cap;
+    int fine;                    // 16-token blocks (f3): a unit is four consecutive list entries, one per warp
     int B, H_q, H_kv, G;
     float scale_log2;            // sm_scale * log2(e)
     int n_ctas;                  // gridDim.x of attn_decode_kernel (the merge kernel recomputes the same cut)
@@ -44,9 +45,14 @@ struct AttnArgs {
     float* lse;
 };
 
-// blocks of sequence b that are attended
+// list entries of sequence b (sparse form)
+__device__ __forceinline__ int seq_entries(const AttnArgs& a, int b) { return max(0, min(a.budgets[b], a.cap)); }
+// units of sequence b per KV head: 64 tokens each -- a selected 64-token block, four selected 16-token blocks (the
+// last unit of a list may be short), or a 64-token stretch of the whole sequence (dense)
 __device__ __forceinline__ int seq_blocks(const AttnArgs& a, int b) {
-    return a.indices ? max(0, min(a.budgets[b], a.cap)) : ((a.seq_len[b] + 63) >> 6);
+    if (!a.indices) return (a.seq_len[b] + 63) >> 6;
+    const int n = seq_entries(a, b);
+    return a.fine ? (n + 3) >> 2 : n;
 }
 
 // smem sub-tile: [16 rows][256 B], 16-byte chunk index XOR-swizzled with (row & 7)
@@ -112,27 +118,35 @@ __global__ void __launch_bounds__(ATT_WARPS * 32, 2) attn_decode_kernel(AttnArgs
             }
             const uint16_t* kbase = a.k + (int64_t)b * a.sb + (int64_t)hk * a.sh;
             const uint16_t* vbase = a.v + (int64_t)b * a.sb + (int64_t)hk * a.sh;
-            const int32_t* idx = a.indices ? a.indices + (int64_t)b * a.cap + jbeg : nullptr;
+            const bool fine = a.fine != 0;
+            const int n_ent = fine ? seq_entries(a, b) : 0;
+            const int32_t* idx = a.indices ? a.indices + (int64_t)b * a.cap + (fine ? 0 : jbeg) : nullptr;
 
             float o[16][4];
 #pragma unroll
             for (int i = 0; i < 16; ++i) o[i][0] = o[i][1] = o[i][2] = o[i][3] = 0.f;
             float m0 = -INFINITY, m1 = -INFINITY, l0 = 0.f, l1 = 0.f;
 
-            // block ids of the portion, 32 per window, one per lane; the next window is fetched a window ahead
+            // first token of this warp's 16-token sub-tile of every unit of the portion, 32 units per window, one per
+            // lane; the next window is fetched a window ahead.  (A list entry past the budget: a token past L, masked.)
             auto load_ids = [&](int w) -> int {
                 const int it = w * 32 + lane;
-                return (it < n_it) ? (idx ? idx[it] : (jbeg + it)) : 0;
+                if (it >= n_it) return 0;
+                if (fine) {
+                    const int e = (jbeg + it) * 4 + warp;
+                    return e < n_ent ? idx[e] * 16 : 0x3fffff00;
+                }
+                return (idx ? idx[it] : (jbeg + it)) * 64 + warp * SUB_TOK;
             };
             int ids_cur = load_ids(0), ids_nxt = load_ids(1), win = 0;
-            auto blk_at = [&](int it) -> int {
+            auto tok_at = [&](int it) -> int {
                 return __shfl_sync(0xffffffffu, (it >> 5) == win ? ids_cur : ids_nxt, it & 31);
             };
             // prologue: fill STAGES-1 stages
 #pragma unroll
             for (int s = 0; s < ATT_STAGES - 1; ++s) {
                 if (s < n_it)
-                    issue_subtile(my_smem + s * STAGE_BYTES, kbase, vbase, a.st, blk_at(s) * 64 + warp * SUB_TOK, L, lane);
+                    issue_subtile(my_smem + s * STAGE_BYTES, kbase, vbase, a.st, tok_at(s), L, lane);
                 cp_async_commit();
             }
 
@@ -142,7 +156,7 @@ __global__ void __launch_bounds__(ATT_WARPS * 32, 2) attn_decode_kernel(AttnArgs
                     int nx = it + ATT_STAGES - 1;
                     if (nx < n_it)
                         issue_subtile(my_smem + (nx % ATT_STAGES) * STAGE_BYTES, kbase, vbase, a.st,
-                                      blk_at(nx) * 64 + warp * SUB_TOK, L, lane);
+                                      tok_at(nx), L, lane);
                     cp_async_commit();
                 }
                 cp_async_wait<ATT_STAGES - 1>();
@@ -150,7 +164,7 @@ __global__ void __launch_bounds__(ATT_WARPS * 32, 2) attn_decode_kernel(AttnArgs
 
                 const uint32_t ks_base = my_smem + (it % ATT_STAGES) * STAGE_BYTES;
                 const uint32_t vs_base = ks_base + SUB_TOK * 256;
-                const int tok0 = blk_at(it) * 64 + warp * SUB_TOK;
+                const int tok0 = tok_at(it);
 
                 // S = Q K^T : 16 (heads) x 16 (tokens), k = 128
                 float s[2][4] = {{0.f, 0.f, 0.f, 0.f}, {0.f, 0.f, 0.f, 0.f}};
@@ -325,7 +339,7 @@ spot_status check_attn(const spot_attn_params* p, bool dense, bool prefill) {
     if (!aligned16(p->q) || !aligned16(p->k) || !aligned16(p->v) || !aligned16(p->out)) return SPOT_ERR_INVALID_ARG;
     if (p->B <= 0 || p->H_q <= 0 || p->H_kv <= 0 || p->H_q % p->H_kv != 0) return SPOT_ERR_INVALID_ARG;
     if (p->H_q / p->H_kv > 16) return SPOT_ERR_UNSUPPORTED;
-    if (p->D != 128 || p->blk != 64) return SPOT_ERR_UNSUPPORTED;
+    if (p->D != 128 || (p->blk != 64 && !(p->blk == 16 && !prefill))) return SPOT_ERR_UNSUPPORTED;
     if (p->kv_stride_token < p->D || p->kv_stride_token % 8 || p->kv_stride_head % 8 || p->kv_stride_batch % 8)
         return SPOT_ERR_INVALID_ARG;
     if (!dense && p->indices && (!p->budgets || p->cap <= 0)) return SPOT_ERR_INVALID_ARG;
@@ -355,6 +369,7 @@ spot_status run_decode(const spot_attn_params* p, bool dense, cudaStream_t s) {
     a.q = p->q; a.k = p->k; a.v = p->v;
     a.sb = p->kv_stride_batch; a.st = p->kv_stride_token; a.sh = p->kv_stride_head;
     a.seq_len = p->seq_len; a.indices = use_idx ? p->indices : nullptr; a.budgets = p->budgets; a.cap = p->cap;
+    a.fine = use_idx && p->blk == 16;
     a.B = p->B; a.H_q = p->H_q; a.H_kv = p->H_kv; a.G = G;
     a.scale_log2 = p->sm_scale * 1.4426950408889634f;
     a.n_ctas = n_ctas;

@@ -142,6 +142,7 @@ struct ScoreArgs {
     int B;
     float* scores;
     int nb_stride;
+    int fine;                     // blk == 16: four block maxima per 64-token tile (f3)
 };
 
 // (sequence, tile) cursor over the flat tile list
@@ -152,6 +153,24 @@ struct TileCursor {
         while (t >= nb && b + 1 < a.B) { t -= nb; ++b; nb = (a.seq_len[b] + 63) >> 6; }
     }
 };
+
+// Column 0 of the accumulators lives on lanes c == 0: the maximum over the 8 row lanes.
+__device__ __forceinline__ float rows_max(float m, int lane) {
+    if ((lane & 3) != 0) m = -INFINITY;
+    m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, 4));
+    m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, 8));
+    m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, 16));
+    return m;
+}
+// One 16-token group (rows g and g + 8 of an MMA) has been scored.  Coarse (blk 64): fold it into the lane's running
+// maximum, reduced over lanes once per tile.  Fine (blk 16, f3): reduce now and leave the group's maximum on lane 4 * grp.
+__device__ __forceinline__ float group_update(float m, float sa, float sb, bool va, bool vb, int grp, int lane, bool fine) {
+    float mi = va ? sa : -INFINITY;
+    if (vb) mi = fmaxf(mi, sb);
+    if (!fine) return fmaxf(m, mi);
+    mi = rows_max(mi, lane);               // valid on lanes c == 0
+    return lane == 4 * grp ? mi : m;
+}
 
 // ---- BF16 tile: planes [H * D_IDX / 64][64 tokens][128 B], 128-byte swizzle --------------------------------
 template <int H, int D_IDX>
@@ -176,7 +195,8 @@ struct Bf16Tile {
     }
 
     // max over the tile's valid tokens of s[t]; valid on every lane after the final shuffles
-    __device__ __forceinline__ float tile_max(uint32_t st, int t0, int L, int lane) const {
+    // (fine: lane 4 i, i < 4, returns the maximum over tokens [16 i, 16 i + 16) of the tile instead)
+    __device__ __forceinline__ float tile_max(uint32_t st, int t0, int L, int lane, bool fine) const {
         const int g = lane >> 2, c = lane & 3, mi = lane >> 3, r8 = lane & 7;
         float m = -INFINITY;
 #pragma unroll 1
@@ -202,14 +222,9 @@ struct Bf16Tile {
                 sb = fmaf(wh[h], fmaxf(acc[2], 0.f), sb);   // column 0, row g + 8
             }
             const int ta = t0 + rg * 16 + g, tb = ta + 8;
-            if (ta < L) m = fmaxf(m, sa);
-            if (tb < L) m = fmaxf(m, sb);
+            m = group_update(m, sa, sb, ta < L, tb < L, rg, lane, fine);
         }
-        if (c != 0) m = -INFINITY;
-        m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, 4));
-        m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, 8));
-        m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, 16));
-        return m;
+        return fine ? m : rows_max(m, lane);
     }
 };
 
@@ -280,7 +295,7 @@ struct Q4Tile {
         __syncwarp();
     }
 
-    __device__ __forceinline__ float tile_max(uint32_t st, int t0, int L, int lane) const {
+    __device__ __forceinline__ float tile_max(uint32_t st, int t0, int L, int lane, bool fine) const {
         const int g = lane >> 2, c = lane & 3;
         float m = -INFINITY;
 #pragma unroll 2
@@ -329,14 +344,9 @@ struct Q4Tile {
             const float sa = srow[0] + __shfl_xor_sync(0xffffffffu, srow[0], 1);
             const float sb = srow[1] + __shfl_xor_sync(0xffffffffu, srow[1], 1);
             const int ta = t0 + it * 16 + g, tbk = ta + 8;
-            if (ta < L) m = fmaxf(m, sa);
-            if (tbk < L) m = fmaxf(m, sb);
+            m = group_update(m, sa, sb, ta < L, tbk < L, it, lane, fine);
         }
-        if (c != 0) m = -INFINITY;
-        m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, 4));
-        m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, 8));
-        m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, 16));
-        return m;
+        return fine ? m : rows_max(m, lane);
     }
 };
 
@@ -403,8 +413,9 @@ struct Fp8Tile {
     }
 
     // maximum over NIT * 16 tokens starting at token t0, whose codes start at shared address st
+    // (it0: index of the slice's first 16-token group inside its tile, for the fine form)
     template <int NIT>
-    __device__ __forceinline__ float part_max(uint32_t st, int t0, int L, int lane) const {
+    __device__ __forceinline__ float part_max(uint32_t st, int t0, int L, int lane, bool fine, int it0) const {
         const int g = lane >> 2, c = lane & 3;
         float m = -INFINITY;
 #pragma unroll 2
@@ -436,16 +447,21 @@ struct Fp8Tile {
                 sb = fmaf(wq[h], fmaxf(acc[2] * ps[h], 0.f), sb);     // column 0, row g + 8
             }
             const int ta = t0 + it * 16 + g, tb = ta + 8;
-            if (ta < L) m = fmaxf(m, sa);
-            if (tb < L) m = fmaxf(m, sb);
+            m = group_update(m, sa, sb, ta < L, tb < L, it0 + it, lane, fine);
         }
-        if (c != 0) m = -INFINITY;
-        m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, 4));
-        m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, 8));
-        m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, 16));
-        return m;
+        return fine ? m : rows_max(m, lane);
     }
 };
+
+// block scores of tile t of sequence b: one (lane 0) or, with 16-token blocks, up to four (lanes 0, 4, 8, 12)
+__device__ __forceinline__ void store_scores(const ScoreArgs& a, int b, int t, int L, int lane, float m) {
+    if (a.fine) {
+        const int grp = lane >> 2;
+        if ((lane & 3) == 0 && grp < 4 && t * 64 + grp * 16 < L) a.scores[(int64_t)b * a.nb_stride + t * 4 + grp] = m;
+    } else if (lane == 0) {
+        a.scores[(int64_t)b * a.nb_stride + t] = m;
+    }
+}
 
 template <int H, int D_IDX, int FMT>
 __global__ void __launch_bounds__((ScoreCfg<H, D_IDX, FMT>::THREADS), 1) score_decode_kernel(const __grid_constant__ CUtensorMap tm_k,
@@ -459,6 +475,7 @@ __global__ void __launch_bounds__((ScoreCfg<H, D_IDX, FMT>::THREADS), 1) score_d
     const uint32_t bar_empty = bar_full + NS * 8;                  // [NS]
     const uint32_t q16_base = bar_empty + NS * 8;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const bool fine = a.fine != 0;
 
     if (threadIdx.x == 0) {
         for (int s = 0; s < NS; ++s) { mbar_init(bar_full + 8 * s, 1); mbar_init(bar_empty + 8 * s, 1); }
@@ -525,13 +542,14 @@ __global__ void __launch_bounds__((ScoreCfg<H, D_IDX, FMT>::THREADS), 1) score_d
                 mbar_wait(bar_full + 8 * s, (q / K) & 1);
                 if constexpr (FMT == SPOT_SELK_FP8_E4M3)
                     m = fmaxf(m, tile.template part_max<4 / SP>(ring + s * Cfg::STAGE_BYTES,
-                                                                cur.t * 64 + part * (64 / SP), L, lane));
+                                                                cur.t * 64 + part * (64 / SP), L, lane, fine,
+                                                                part * (4 / SP)));
                 else
-                    m = tile.tile_max(ring + s * Cfg::STAGE_BYTES, cur.t * 64, L, lane);
+                    m = tile.tile_max(ring + s * Cfg::STAGE_BYTES, cur.t * 64, L, lane, fine);
                 __syncwarp();
                 request_next();
             }
-            if (lane == 0) a.scores[(int64_t)cur_b * a.nb_stride + cur.t] = m;
+            store_scores(a, cur_b, cur.t, L, lane, m);
             cur.advance(a, SC_CONSUMERS);
         }
     } else if (warp == SC_CONSUMERS) {
@@ -563,12 +581,10 @@ __global__ void __launch_bounds__((ScoreCfg<H, D_IDX, FMT>::THREADS), 1) score_d
             }
             const int s = i % NS;
             mbar_wait(bar_full + 8 * s, (i / NS) & 1);
-            const float m = tile.tile_max(ring + s * Cfg::STAGE_BYTES, cur.t * 64, L, lane);
+            const float m = tile.tile_max(ring + s * Cfg::STAGE_BYTES, cur.t * 64, L, lane, fine);
             __syncwarp();
-            if (lane == 0) {
-                mbar_arrive(bar_empty + 8 * s);
-                a.scores[(int64_t)cur_b * a.nb_stride + cur.t] = m;
-            }
+            if (lane == 0) mbar_arrive(bar_empty + 8 * s);
+            store_scores(a, cur_b, cur.t, L, lane, m);
             cur.advance(a, SC_CONSUMERS);
         }
     }
@@ -579,7 +595,7 @@ spot_status launch_score_fmt(const spot_select_params* p, float* scores, int nb_
     using Cfg = ScoreCfg<H, D_IDX, FMT>;
     ScoreArgs a;
     a.sel_q = p->sel_q; a.w = p->w; a.sel_k = (const uint8_t*)p->sel_k; a.tiles_per_seq = p->cache_stride_tokens / 64;
-    a.seq_len = p->seq_len; a.B = p->B; a.scores = scores; a.nb_stride = nb_stride;
+    a.seq_len = p->seq_len; a.B = p->B; a.scores = scores; a.nb_stride = nb_stride; a.fine = p->blk == 16;
     CUtensorMap tm;
     memset(&tm, 0, sizeof(tm));
     if (FMT == SPOT_SELK_BF16) {

@@ -1,8 +1,8 @@
-// Step a2, histogram-partition form (rows with n_b <= 2048) -- reserved tier, residual softmax (Eq. 7), nucleus +
+// Step a2, histogram partition (rows of up to 2048 blocks; up to 8192 with 1024 threads x 8 keys) -- reserved tier, residual softmax (Eq. 7), nucleus +
 // K_min floor (Eq. 8) or static top-K (Eq. 6), one CTA of 1024 threads x 2 keys (decode) or 256 threads x 8 keys (prefill) per selection row.
 //
 // The rule only needs (a) the mass in front of the cut and (b) the key value tau at the cut, not a full sort.  So:
-//   1. keys (order-preserving 32-bit images of the scores, ascending key = descending score) go into 2048 bins by a
+//   1. keys (order-preserving 32-bit images of the scores, ascending key = descending score) go into as many bins as the row has slots by a
 //      MONOTONE map of the key range (float multiply + truncate), i.e. bins are contiguous key ranges in rank order;
 //   2. an exclusive scan of the bin counts turns the bins into rank ranges, and a counting-sort scatter groups
 //      (key, exp(z - z_max)) by bin in shared memory -- unordered inside a bin, exactly ordered across bins;
@@ -25,9 +25,8 @@ namespace spot {
 
 namespace {
 
-constexpr int SH_N = 2048;          // keys per row
-constexpr int SH_NBIN = 2048;
-
+// SH_N keys per row (2048, or 8192 for the long rows of 16-token blocks / L > 128K) and as many bins
+template <int SH_NBIN>
 struct BinMap {
     uint32_t kmn;
     float scale;
@@ -68,12 +67,19 @@ __device__ __forceinline__ void warp_resolve(const uint32_t* s_k, const double* 
 // E keys per thread, SH_N / E threads: decode rows (a handful of CTAs, pure latency) run 1024 threads x 2 keys so that
 // every per-thread section (two fp64 exps instead of eight, ...) is short; prefill rows (a thousand CTAs, throughput) run
 // 256 threads x 8 keys.
-template <int SH_E>
+// (rows of up to 2048 keys keep their 32 KiB of arrays static; the 8192-key form takes 128 KiB of dynamic shared memory)
+template <int SH_N, int SH_E>
 __global__ void __launch_bounds__(SH_N / SH_E) select_hist_kernel(SelectArgs a) {
-    constexpr int SH_T = SH_N / SH_E, SH_WARPS = SH_T / 32;
-    __shared__ uint32_t s_cnt[SH_NBIN];       // bin counts, then exclusive starts
-    __shared__ double s_e[SH_N];              // masses grouped by bin
-    __shared__ uint32_t s_k[SH_N];            // keys grouped by bin
+    constexpr int SH_T = SH_N / SH_E, SH_WARPS = SH_T / 32, SH_NBIN = SH_N;
+    constexpr bool STATIC = SH_N <= 2048;
+    constexpr int PK_SHIFT = SH_N > 4096 ? 13 : 12;           // bin << PK_SHIFT | rank inside the bin
+    __shared__ uint32_t st_cnt[STATIC ? SH_NBIN : 1];
+    __shared__ double st_e[STATIC ? SH_N : 1];
+    __shared__ uint32_t st_k[STATIC ? SH_N : 1];
+    extern __shared__ __align__(16) unsigned char sh_dyn[];
+    double* const s_e = STATIC ? st_e : reinterpret_cast<double*>(sh_dyn);                           // masses grouped by bin
+    uint32_t* const s_k = STATIC ? st_k : reinterpret_cast<uint32_t*>(sh_dyn + SH_N * 8);            // keys grouped by bin
+    uint32_t* const s_cnt = STATIC ? st_cnt : reinterpret_cast<uint32_t*>(sh_dyn + SH_N * 12);       // bin counts, then exclusive starts
     __shared__ double s_wd[SH_WARPS];
     __shared__ uint32_t s_wu[SH_WARPS][2];
     __shared__ int s_wi[SH_WARPS][2];
@@ -132,7 +138,7 @@ __global__ void __launch_bounds__(SH_N / SH_E) select_hist_kernel(SelectArgs a) 
     for (int r = 0; r < SH_E; ++r) e[r] = 0.0;
 
     if (n_res > 0) {
-        BinMap bin_of;
+        BinMap<SH_NBIN> bin_of;
         bin_of.kmn = kmn;
         bin_of.scale = (float)SH_NBIN / ((float)(kmx - kmn) + 1.0f);
         // ---- masses (Eq. 7 numerators, fp64), bins, rank inside the bin
@@ -140,7 +146,7 @@ __global__ void __launch_bounds__(SH_N / SH_E) select_hist_kernel(SelectArgs a) 
         // (one rolled loop -- the fp64 exp is ~150 instructions and this kernel runs once per step from a cold
         // instruction cache: code size, not instruction count, is what its latency is made of.  The arrays stay in
         // registers: every trip works on element 0 and rotates.)
-        uint32_t pk[SH_E];                                   // bin << 12 | rank inside the bin; 0xffffffff: not residual
+        uint32_t pk[SH_E];                                   // bin << PK_SHIFT | rank inside the bin; 0xffffffff: not residual
         {
             uint32_t kq[SH_E];
 #pragma unroll
@@ -153,7 +159,7 @@ __global__ void __launch_bounds__(SH_N / SH_E) select_hist_kernel(SelectArgs a) 
                 if (j >= sink_end && j < rec_beg) {
                     if (topp) ev = exp((double)key_score(kq[0]) / a.temperature - zmax);
                     const int bn = bin_of(kq[0]);
-                    pv = ((uint32_t)bn << 12) | atomicAdd(&s_cnt[bn], 1u);
+                    pv = ((uint32_t)bn << PK_SHIFT) | atomicAdd(&s_cnt[bn], 1u);
                 }
 #pragma unroll
                 for (int u = 0; u < SH_E - 1; ++u) { kq[u] = kq[u + 1]; e[u] = e[u + 1]; pk[u] = pk[u + 1]; }
@@ -186,7 +192,7 @@ __global__ void __launch_bounds__(SH_N / SH_E) select_hist_kernel(SelectArgs a) 
 #pragma unroll
         for (int r = 0; r < SH_E; ++r)
             if (pk[r] != 0xffffffffu) {
-                const int pos = (int)s_cnt[pk[r] >> 12] + (int)(pk[r] & 0xfffu);
+                const int pos = (int)s_cnt[pk[r] >> PK_SHIFT] + (int)(pk[r] & ((1u << PK_SHIFT) - 1u));
                 s_k[pos] = okey[r];
                 if (topp) s_e[pos] = e[r];
             }
@@ -410,9 +416,17 @@ __global__ void __launch_bounds__(SH_N / SH_E) select_hist_kernel(SelectArgs a) 
 
 }  // namespace
 
-spot_status launch_select_hist(const SelectArgs& a, int rows, cudaStream_t s) {
-    if (rows <= 32) SPOT_CUDA_TRY(launch_pdl(select_hist_kernel<2>, dim3((unsigned)rows), dim3(SH_N / 2), 0, s, a));
-    else SPOT_CUDA_TRY(launch_pdl(select_hist_kernel<8>, dim3((unsigned)rows), dim3(SH_N / 8), 0, s, a));
+spot_status launch_select_hist(const SelectArgs& a, int rows, int max_nb, cudaStream_t s) {
+    if (max_nb > 2048) {
+        constexpr int BIG = 8192, BIG_SMEM = BIG * 16;
+        static unsigned long long smem_attr_done = 0;
+        SPOT_CUDA_TRY(set_max_smem_once(select_hist_kernel<BIG, 8>, BIG_SMEM, smem_attr_done));
+        SPOT_CUDA_TRY(launch_pdl(select_hist_kernel<BIG, 8>, dim3((unsigned)rows), dim3(BIG / 8), BIG_SMEM, s, a));
+    } else if (rows <= 32) {
+        SPOT_CUDA_TRY(launch_pdl(select_hist_kernel<2048, 2>, dim3((unsigned)rows), dim3(2048 / 2), 0, s, a));
+    } else {
+        SPOT_CUDA_TRY(launch_pdl(select_hist_kernel<2048, 8>, dim3((unsigned)rows), dim3(2048 / 8), 0, s, a));
+    }
     return SPOT_OK;
 }
 

@@ -97,7 +97,10 @@ def test_select_argument_errors_are_caught_on_the_host(lib):
         sp = _select_params(**o)
         assert lib.spot_select(C.byref(sp), None) == INVALID, o
         assert lib.spot_select_workspace_bytes(C.byref(sp)) == 0, o
-    assert lib.spot_select(C.byref(_select_params(blk=16)), None) == UNSUPPORTED
+    assert lib.spot_select(C.byref(_select_params(blk=32)), None) == UNSUPPORTED
+    # 16-token blocks (f3) are a decode geometry: accepted there (4x the blocks), not for 64-query prefill rows
+    assert lib.spot_select_workspace_bytes(C.byref(_select_params(blk=16, cap=256, nb_stride=256))) >= 2 * 256 * 4
+    assert lib.spot_select(C.byref(_select_params(blk=16, cap=256, q_block=64, Tq=64, seq_len=None)), None) == UNSUPPORTED
     assert lib.spot_select(None, None) == INVALID
     assert lib.spot_score_blocks(C.byref(_select_params()), None) == INVALID        # block_scores is required
 
@@ -122,11 +125,13 @@ def test_attention_argument_errors_are_caught_on_the_host(lib):
         ap = _attn_params(**o)
         assert lib.spot_sparse_attn_decode(C.byref(ap), None) == INVALID, o
         assert lib.spot_sparse_attn_decode_workspace_bytes(C.byref(ap)) == 0, o
-    for o in (dict(D=64), dict(blk=16), dict(H_q=8 * 17)):
+    for o in (dict(D=64), dict(blk=32), dict(H_q=8 * 17)):
         assert lib.spot_sparse_attn_decode(C.byref(_attn_params(**o)), None) == UNSUPPORTED, o
     # prefill: chunk alignment (R26)
     for o in (dict(Tq=96), dict(Tq=128, q_start=32), dict(Tq=0)):
         assert lib.spot_sparse_attn_prefill(C.byref(_attn_params(**o)), None) == INVALID, o
+    assert lib.spot_sparse_attn_decode_workspace_bytes(C.byref(_attn_params(blk=16))) > 0          # f3
+    assert lib.spot_sparse_attn_prefill(C.byref(_attn_params(Tq=64, blk=16)), None) == UNSUPPORTED
     assert lib.spot_decode_step_host(None, None) == INVALID
 
 

@@ -106,14 +106,15 @@ def test_select_edge_cases(torch_cuda):
                 _check_select(dd, fmt, report, **over)
 
 
-def test_select_crowded_cut_bins_and_ties(torch_cuda):
-    """Score distributions that defeat the histogram partition of the selection kernel: the cut falls into ONE bin
+@pytest.mark.parametrize("n_b,blk", [(256, 64), (2304, 16)])
+def test_select_crowded_cut_bins_and_ties(torch_cuda, n_b, blk):
+    """(n_b = 2304: the 8192-key form of the kernel.)  Score distributions that defeat the histogram partition of the selection kernel: the cut falls into ONE bin
     holding (a) 40 distinct scores 4e-6 apart, (b) 40 exactly tied scores, (c) every residual block, all tied
     (all-zero scores), (d) 200 tied blocks among distinct ones.  Scores are planted exactly: head 0 reads k[0] with
     weight 1, head 1 reads k[0] with weight 4e-6, one live token per block."""
     from workloads import f32_to_bf16_bits
-    n_b, L = 256, 256 * 64
-    wl = make_decode_workload("crowd", 11, B=4, L=L, kind="gauss", with_kv=False)
+    L = n_b * blk
+    wl = make_decode_workload("crowd", 11, B=4, L=L, kind="gauss", with_kv=False, blk=blk)
     q = np.zeros((4, wl.H_idx, wl.d_idx), dtype=np.float32)
     q[:, 0, 0] = 1.0
     q[:, 1, 0] = 1.0
@@ -121,7 +122,7 @@ def test_select_crowded_cut_bins_and_ties(torch_cuda):
     wl.w = np.tile(np.array([1.0, 4e-6, 0.0, 0.0], dtype=np.float32), (4, 1))
     k = np.zeros((4, L, wl.H_idx, wl.d_idx), dtype=np.float32)
     rng = np.random.default_rng(5)
-    tok = np.arange(n_b) * 64 + rng.integers(0, 64, size=n_b)
+    tok = np.arange(n_b) * blk + rng.integers(0, blk, size=n_b)
     cluster = rng.permutation(np.arange(1, n_b - 2))[:40]
     k[0, tok, 0, 0] = 2.0 ** -10                  # low background stretches the key range: one bin = 40960 ulps
     k[0, tok[cluster], 0, 0] = 1.0
@@ -398,3 +399,70 @@ def test_decode_step_is_capturable_in_a_cuda_graph(torch_cuda):
     for b in range(B):
         s_bar, sel = H.oracle_select(wl, "mxfp4", b)
         assert idx[b, :bud[b]].tolist() == sel.indices.tolist()
+
+
+# ---------------------------------------------------------------- f3: the paper's 16-token blocks at decode
+F3 = dict(blk=16, sink_blocks=8, recency_blocks=16, kmin_blocks=32)
+
+
+@pytest.mark.parametrize("fmt", ["bf16", "mxfp4", "int4_e4m3", "fp8_e4m3"])
+@pytest.mark.parametrize("cfg", ["mini2", "mini4"])
+def test_block16_select_matches_oracle(torch_cuda, cfg, fmt):
+    """Four block maxima per 64-token tile, 4x the blocks per row (512 here), the paper's reserved tiers."""
+    wl = make_config(cfg, with_kv=False, **F3)
+    dd = H.DeviceDecode(wl, fmt, with_kv=False)
+    report = []
+    _check_select(dd, fmt, report)
+    _check_select(dd, fmt, report, p=0.7)
+    _check_select(dd, fmt, report, mode="topk", top_k=64)
+    non_exact = [r for r in report if r[3] != "exact"]
+    print("near-tie report:", non_exact)
+    assert len(non_exact) <= max(1, len(report) // 10)
+
+
+def test_block16_select_edge_cases_and_long_rows(torch_cuda):
+    # ragged tails inside a tile (L % 64 in 1..63, L % 16 != 0), contexts smaller than the reserved tiers, d_idx = 128,
+    # and rows beyond 2048 blocks (L = 40000 -> 2500 blocks, 131072 -> 8192: the bitonic kernels)
+    for seed, L, seqs, d_idx in [(11, 64, [1, 17, 64], 64), (12, 320, [65, 129, 307], 64), (13, 2048, [2048, 1999, 777], 128)]:
+        wl = make_decode_workload("e16_%d" % seed, seed, B=3, L=L, kind="gauss", seq_lens=seqs, d_idx=d_idx,
+                                  with_kv=False, blk=16)
+        for fmt in ("bf16", "mxfp4", "fp8_e4m3"):
+            dd = H.DeviceDecode(wl, fmt, with_kv=False)
+            report = []
+            for over in (dict(), dict(sink_blocks=8, recency_blocks=16, kmin_blocks=32), dict(mode="topk", top_k=5)):
+                _check_select(dd, fmt, report, **over)
+    for L, seqs in ((40000 + 24, [40000, 33333]), (131072, [131072, 100001])):
+        wl = make_decode_workload("long16", 90 + L, B=2, L=L, kind="zipf", zipf_s=1.1, seq_lens=seqs, with_kv=False, **F3)
+        dd = H.DeviceDecode(wl, "bf16", with_kv=False)
+        report = []
+        _check_select(dd, "bf16", report)
+        print("long rows (blk 16):", report)
+
+
+def test_block16_attention(torch_cuda):
+    wl = make_config("mini2", **F3)
+    dd = H.DeviceDecode(wl, "bf16")
+    lists = [H.oracle_select(wl, "bf16", b)[1].indices.tolist() for b in range(wl.B)]
+    _check_attend(dd, lists)
+    # hand-made lists: lengths 1, 2, 3, 5 (a short last unit), the ragged last block alone, an empty list
+    n_b = [-(-int(L) // 16) for L in wl.seq_len]
+    _check_attend(dd, [[0], [3, n_b[1] - 1], [1, 2, n_b[2] - 1]])
+    _check_attend(dd, [[0, 5, 6, 7, 400], [n_b[1] - 1], list(range(n_b[2]))])       # p = 1 on the last sequence
+    out, lse = dd.attend(np.full((wl.B, 4), -1, dtype=np.int32), np.zeros(wl.B, dtype=np.int32))
+    assert np.all(out == 0) and np.all(np.isneginf(lse))
+    # dense comparator is geometry-free
+    all64 = [list(range(-(-int(L) // 16))) for L in wl.seq_len]
+    _check_attend(dd, all64, dense=True)
+
+
+def test_block16_end_to_end_step(torch_cuda):
+    wl = make_config("mini4", **F3)
+    dd = H.DeviceDecode(wl, "mxfp4")
+    idx, bud, _, _ = dd.select()
+    out, _ = dd.attend(idx, bud)
+    for b in range(wl.B):
+        s_bar, sel = H.oracle_select(wl, "mxfp4", b)
+        assert idx[b, :bud[b]].tolist() == sel.indices.tolist()
+        want, _ = H.oracle_attend(wl, b, sel.indices)
+        err = np.abs(out[b] - want)
+        assert err.max() <= MAX_ABS and err.mean() <= MEAN_ABS
