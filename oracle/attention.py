@@ -114,3 +114,19 @@ def sparse_attn_prefill(Q, K, V, block_lists, q_start, q_block, blk, sm_scale):
                 e = np.exp(logits - logits.max())
                 out[qq, h] = (e[:, None] * V[toks, g, :]).sum(axis=0) / e.sum()
     return out
+
+
+def gather_paged_kv(pool, page_table, L, page_tokens):
+    """f3 (R32) -- a paged K or V cache read back as the logical tensor.
+
+    pool [n_pages][page_tokens][H_kv][D], page_table [ceil(L / page_tokens)] physical page of every logical
+    page of ONE sequence -> [L][H_kv][D]: logical token t is row t % page_tokens of page
+    page_table[t // page_tokens].  Paging is a storage layout, not arithmetic: attention over a paged cache
+    is, by definition, attention over this tensor ("attention runs only over the gathered
+    K_I, V_I", says nothing about where the rows live).  Written as the loop it is.
+    """
+    pool = np.asarray(pool)
+    out = np.empty((L,) + pool.shape[2:], dtype=pool.dtype)
+    for t in range(L):
+        out[t] = pool[int(page_table[t // page_tokens]), t % page_tokens]
+    return out

@@ -115,3 +115,28 @@ def test_prefill_form_against_torch_block_sparse_causal_mask_and_decode_form():
         pos = q_start + qq
         o, _ = A.sparse_attn_decode(Q[qq], K, V, lists[qq // 64], pos + 1, blk, sc)
         assert np.allclose(out[qq], o, atol=1e-13)
+
+
+def test_paged_gather_round_trip_and_identity():
+    """f3 / R32: scattering a logical cache into randomly placed pages and gathering it back is the identity (also with
+    a ragged last page and pages shared with another sequence's allocation); the identity table is a plain reshape."""
+    rng = np.random.default_rng(12)
+    L, pt, H_kv, D = 1000, 64, 2, 8
+    logical = rng.standard_normal((L, H_kv, D))
+    n_log = -(-L // pt)
+    n_pages = 40
+    table = rng.permutation(n_pages)[:n_log]
+    pool = rng.standard_normal((n_pages, pt, H_kv, D))                 # other sequences' pages: garbage to us
+    for lp in range(n_log):
+        t0, t1 = lp * pt, min((lp + 1) * pt, L)
+        pool[table[lp], :t1 - t0] = logical[t0:t1]
+    got = A.gather_paged_kv(pool, table, L, pt)
+    assert np.array_equal(got, logical)
+    ident = A.gather_paged_kv(logical[:960].reshape(15, pt, H_kv, D), np.arange(15), 960, pt)
+    assert np.array_equal(ident, logical[:960])
+    # a wrong table entry is visible: swapping two pages moves exactly those 128 tokens
+    t2 = table.copy()
+    t2[[3, 7]] = t2[[7, 3]]
+    bad = A.gather_paged_kv(pool, t2, L, pt)
+    diff = np.flatnonzero(np.any(bad != logical, axis=(1, 2)))
+    assert set(diff // pt) == {3, 7}
