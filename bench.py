@@ -209,12 +209,20 @@ def run_ours(args):
     ws_sel = torch.empty(max(16, api.spot_select_workspace_bytes(sp)), dtype=torch.uint8, device=dev)
     sp.workspace, sp.workspace_bytes = ws_sel.data_ptr(), ws_sel.numel()
     kv_strides = (Hkv * L * D, D, L * D)
+    paging = {}
+    if args.paged:
+        # the same bytes read as a page pool [page][H_kv][page_tokens][D] behind a random page table (f3, R32)
+        pt = args.paged
+        n_log = -(-L // pt)
+        table = torch.randperm(Bn * n_log, generator=gen, device=dev).to(torch.int32).reshape(Bn, n_log)
+        kv_strides = (Hkv * pt * D, D, pt * D)
+        paging = dict(page_table=table, page_tokens=pt)
     ap = api.make_attn_params(q, K, V, kv_strides, seq_len, L, indices, budgets, cap, Bn, 1, Hq, Hkv, D, blk=wl.blk,
-                              sm_scale=wl.sm_scale, out=out)
+                              sm_scale=wl.sm_scale, out=out, **paging)
     ws_att = torch.empty(max(16, api.spot_sparse_attn_decode_workspace_bytes(ap)), dtype=torch.uint8, device=dev)
     ap.workspace, ap.workspace_bytes = ws_att.data_ptr(), ws_att.numel()
     apd = api.make_attn_params(q, K, V, kv_strides, seq_len, L, None, None, 0, Bn, 1, Hq, Hkv, D, blk=wl.blk,
-                               sm_scale=wl.sm_scale, out=torch.empty_like(out))
+                               sm_scale=wl.sm_scale, out=torch.empty_like(out), **paging)
     ws_den = torch.empty(max(16, api.spot_dense_attn_decode_workspace_bytes(apd)), dtype=torch.uint8, device=dev)
     apd.workspace, apd.workspace_bytes = ws_den.data_ptr(), ws_den.numel()
 
@@ -374,7 +382,9 @@ def run_ours(args):
         "warmup": max(args.warmup, 3), "ms_per_step": step_mean, "higher_is_better": False, "scaling": "weak",
         "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
         "config": {"workload": args.workload, "B": Bn, "L": L, "H_q": Hq, "H_kv": Hkv, "D": D,
-                   "selector": "%dx%d %s" % (wl.H_idx, wl.d_idx, args.fmt), "blk": wl.blk, "mode": wl.mode,
+                   "selector": "%dx%d %s" % (wl.H_idx, wl.d_idx, args.fmt), "blk": wl.blk,
+                   "kv_layout": ("paged, %d tokens per page, random table" % args.paged) if args.paged else "[B][H_kv][L][D]",
+                   "mode": wl.mode,
                    "p": args.p, "sink/recency/kmin": [wl.sink_blocks, wl.recency_blocks, wl.kmin_blocks],
                    "budgets": bud_host.tolist(), "l2": "flushed by a 512 MiB read sweep before every timed step",
                    "kv": "N(0,1) BF16 generated on the device (seeded); selector side from workloads/"},
@@ -664,6 +674,8 @@ def main():
     ap.add_argument("--L", type=int, default=0, help="cfg5 only: prompt length (default 65536)")
     ap.add_argument("--d-idx", type=int, default=0, choices=[0, 64, 128],
                     help="decode only: selector head dim (default: the config's 64; 128 = the paper's geometry, PAPER.md:363)")
+    ap.add_argument("--paged", type=int, default=0, choices=[0, 16, 64, 256],
+                    help="decode only: K/V as a page pool of this many tokens per page behind a random page table")
     ap.add_argument("--blk", type=int, default=64, choices=[64, 16],
                     help="decode only: selection block size (16 = the paper's geometry with its 8/16/32 reserved "
                          "sink/recency/K_min blocks, PAPER.md:362-365, :400-402)")

@@ -42,6 +42,7 @@ class AttnParams(C.Structure):
         ("q_start", C.c_int32), ("blk", C.c_int32), ("sm_scale", C.c_float),
         ("out", C.c_void_p), ("lse", C.c_void_p),
         ("workspace", C.c_void_p), ("workspace_bytes", C.c_size_t),
+        ("page_table", C.c_void_p), ("page_table_stride", C.c_int32), ("page_tokens", C.c_int32),
     ]
 
 

@@ -101,7 +101,8 @@ def spot_score_blocks(sp, stream=None):
 
 
 def make_attn_params(q, k, v, kv_strides, seq_len, max_seq_len, indices, budgets, cap, B, Tq, H_q, H_kv, D, *,
-                     q_start=0, blk=64, sm_scale=None, out=None, lse=None, workspace=None):
+                     q_start=0, blk=64, sm_scale=None, out=None, lse=None, workspace=None, page_table=None,
+                     page_tokens=0):
     ap = AttnParams()
     ap.q, ap.k, ap.v = q.data_ptr(), k.data_ptr(), v.data_ptr()
     ap.kv_stride_batch, ap.kv_stride_token, ap.kv_stride_head = kv_strides
@@ -117,6 +118,8 @@ def make_attn_params(q, k, v, kv_strides, seq_len, max_seq_len, indices, budgets
     ap.lse = lse.data_ptr() if lse is not None else None
     if workspace is not None:
         ap.workspace, ap.workspace_bytes = workspace.data_ptr(), workspace.numel() * workspace.element_size()
+    if page_table is not None:
+        ap.page_table, ap.page_table_stride, ap.page_tokens = page_table.data_ptr(), page_table.shape[1], page_tokens
     return ap
 
 

@@ -36,6 +36,8 @@ struct AttnArgs {
     const int32_t* budgets;
     int cap;
     int fine;                    // 16-token blocks (f3): a unit is four consecutive list entries, one per warp
+    const int32_t* page_table;   // nullptr: contiguous caches; else k / v are page pools (f3, R32)
+    int pt_stride, page_tokens, page_vtok;   // page_vtok = page stride in units of the token stride
     int B, H_q, H_kv, G;
     float scale_log2;            // sm_scale * log2(e)
     int n_ctas;                  // gridDim.x of attn_decode_kernel (the merge kernel recomputes the same cut)
@@ -58,16 +60,17 @@ __device__ __forceinline__ int seq_blocks(const AttnArgs& a, int b) {
 // smem sub-tile: [16 rows][256 B], 16-byte chunk index XOR-swizzled with (row & 7)
 __device__ __forceinline__ uint32_t sw_off(int row, int chunk) { return (uint32_t)(row * 256 + ((chunk ^ (row & 7)) << 4)); }
 
+// tok0: the sub-tile's first LOGICAL token (rows at or past L are zero-filled); vtok0: where it lives, in units of
+// the token stride from kbase / vbase (== tok0 unless the cache is paged)
 __device__ __forceinline__ void issue_subtile(uint32_t smem_stage, const uint16_t* kbase, const uint16_t* vbase,
-                                              int64_t st, int tok0, int L, int lane) {
+                                              int64_t st, int tok0, int vtok0, int L, int lane) {
     // 16 rows x 16 chunks of 16 B for K and again for V: 8 + 8 cp.async per lane
 #pragma unroll
     for (int i = 0; i < 8; ++i) {
         int id = i * 32 + lane;
         int row = id >> 4, ch = id & 15;
-        int tok = tok0 + row;
-        bool ok = tok < L;
-        int64_t off = (int64_t)(ok ? tok : (L - 1)) * st + ch * 8;
+        bool ok = tok0 + row < L;
+        int64_t off = (int64_t)(ok ? vtok0 + row : 0) * st + ch * 8;
         cp_async16(smem_stage + sw_off(row, ch), kbase + off, ok);
         cp_async16(smem_stage + SUB_TOK * 256 + sw_off(row, ch), vbase + off, ok);
     }
@@ -116,8 +119,11 @@ __global__ void __launch_bounds__(ATT_WARPS * 32, 2) attn_decode_kernel(AttnArgs
                     qa[ks][3] = (g + 8 < G) ? *reinterpret_cast<const uint32_t*>(qb + (g + 8) * ATT_D + col + 8) : 0u;
                 }
             }
-            const uint16_t* kbase = a.k + (int64_t)b * a.sb + (int64_t)hk * a.sh;
-            const uint16_t* vbase = a.v + (int64_t)b * a.sb + (int64_t)hk * a.sh;
+            const bool paged = a.page_table != nullptr;
+            const int64_t hbase = (paged ? 0 : (int64_t)b * a.sb) + (int64_t)hk * a.sh;
+            const uint16_t* kbase = a.k + hbase;
+            const uint16_t* vbase = a.v + hbase;
+            const int32_t* ptab = paged ? a.page_table + (int64_t)b * a.pt_stride : nullptr;
             const bool fine = a.fine != 0;
             const int n_ent = fine ? seq_entries(a, b) : 0;
             const int32_t* idx = a.indices ? a.indices + (int64_t)b * a.cap + (fine ? 0 : jbeg) : nullptr;
@@ -138,25 +144,43 @@ __global__ void __launch_bounds__(ATT_WARPS * 32, 2) attn_decode_kernel(AttnArgs
                 }
                 return (idx ? idx[it] : (jbeg + it)) * 64 + warp * SUB_TOK;
             };
+            // paged: the sub-tile's place in the pool (a sub-tile never straddles a page: page_tokens % 16 == 0)
+            auto place = [&](int tok) -> int {
+                if (!paged || tok >= L) return tok;
+                const int lp = tok / a.page_tokens;
+                return ptab[lp] * a.page_vtok + (tok - lp * a.page_tokens);
+            };
             int ids_cur = load_ids(0), ids_nxt = load_ids(1), win = 0;
+            int vid_cur = place(ids_cur), vid_nxt = place(ids_nxt);
             auto tok_at = [&](int it) -> int {
                 return __shfl_sync(0xffffffffu, (it >> 5) == win ? ids_cur : ids_nxt, it & 31);
+            };
+            auto vtok_at = [&](int it, int tok) -> int {
+                return paged ? __shfl_sync(0xffffffffu, (it >> 5) == win ? vid_cur : vid_nxt, it & 31) : tok;
             };
             // prologue: fill STAGES-1 stages
 #pragma unroll
             for (int s = 0; s < ATT_STAGES - 1; ++s) {
-                if (s < n_it)
-                    issue_subtile(my_smem + s * STAGE_BYTES, kbase, vbase, a.st, tok_at(s), L, lane);
+                if (s < n_it) {
+                    const int t = tok_at(s);
+                    issue_subtile(my_smem + s * STAGE_BYTES, kbase, vbase, a.st, t, vtok_at(s, t), L, lane);
+                }
                 cp_async_commit();
             }
 
             for (int it = 0; it < n_it; ++it) {
-                if ((it >> 5) != win) { win = it >> 5; ids_cur = ids_nxt; ids_nxt = load_ids(win + 1); }
+                if ((it >> 5) != win) {
+                    win = it >> 5;
+                    ids_cur = ids_nxt; ids_nxt = load_ids(win + 1);
+                    vid_cur = vid_nxt; vid_nxt = place(ids_nxt);
+                }
                 {
                     int nx = it + ATT_STAGES - 1;
-                    if (nx < n_it)
-                        issue_subtile(my_smem + (nx % ATT_STAGES) * STAGE_BYTES, kbase, vbase, a.st,
-                                      tok_at(nx), L, lane);
+                    if (nx < n_it) {
+                        const int t = tok_at(nx);
+                        issue_subtile(my_smem + (nx % ATT_STAGES) * STAGE_BYTES, kbase, vbase, a.st, t, vtok_at(nx, t),
+                                      L, lane);
+                    }
                     cp_async_commit();
                 }
                 cp_async_wait<ATT_STAGES - 1>();
@@ -346,6 +370,12 @@ spot_status check_attn(const spot_attn_params* p, bool dense, bool prefill) {
     if (!prefill) {
         if (!p->seq_len || p->max_seq_len <= 0) return SPOT_ERR_INVALID_ARG;
     }
+    if (p->page_table) {
+        if (prefill) return SPOT_ERR_UNSUPPORTED;
+        if (p->page_tokens <= 0 || p->page_tokens % 16 != 0) return SPOT_ERR_INVALID_ARG;
+        if ((int64_t)p->page_table_stride * p->page_tokens < p->max_seq_len) return SPOT_ERR_INVALID_ARG;
+        if (p->kv_stride_batch <= 0 || p->kv_stride_batch % p->kv_stride_token != 0) return SPOT_ERR_INVALID_ARG;
+    }
     return SPOT_OK;
 }
 
@@ -370,6 +400,8 @@ spot_status run_decode(const spot_attn_params* p, bool dense, cudaStream_t s) {
     a.sb = p->kv_stride_batch; a.st = p->kv_stride_token; a.sh = p->kv_stride_head;
     a.seq_len = p->seq_len; a.indices = use_idx ? p->indices : nullptr; a.budgets = p->budgets; a.cap = p->cap;
     a.fine = use_idx && p->blk == 16;
+    a.page_table = p->page_table; a.pt_stride = p->page_table_stride; a.page_tokens = p->page_tokens;
+    a.page_vtok = p->page_table ? (int)(p->kv_stride_batch / p->kv_stride_token) : 0;
     a.B = p->B; a.H_q = p->H_q; a.H_kv = p->H_kv; a.G = G;
     a.scale_log2 = p->sm_scale * 1.4426950408889634f;
     a.n_ctas = n_ctas;

@@ -82,7 +82,8 @@ class DeviceDecode:
             cap = idx.shape[1]
         ap = api.make_attn_params(self.q, self.K, self.V, self.kv_strides, self.seq_len, self.max_seq_len, idx, bud,
                                   cap, wl.B, 1, wl.H_q, wl.H_kv, wl.D, blk=wl.blk, sm_scale=wl.sm_scale, out=out,
-                                  lse=lse)
+                                  lse=lse, page_table=getattr(self, "page_table", None),
+                                  page_tokens=getattr(self, "page_tokens", 0))
         fn_ws = api.spot_dense_attn_decode_workspace_bytes if dense else api.spot_sparse_attn_decode_workspace_bytes
         ws = torch.empty(max(fn_ws(ap), 16), dtype=torch.uint8, device="cuda")
         ap.workspace, ap.workspace_bytes = ws.data_ptr(), ws.numel()

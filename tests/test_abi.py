@@ -132,6 +132,13 @@ def test_attention_argument_errors_are_caught_on_the_host(lib):
         assert lib.spot_sparse_attn_prefill(C.byref(_attn_params(**o)), None) == INVALID, o
     assert lib.spot_sparse_attn_decode_workspace_bytes(C.byref(_attn_params(blk=16))) > 0          # f3
     assert lib.spot_sparse_attn_prefill(C.byref(_attn_params(Tq=64, blk=16)), None) == UNSUPPORTED
+    # paged K/V (f3): decode only; page size a multiple of 16, the table must cover max_seq_len, page stride a multiple
+    # of the token stride
+    paged = dict(page_table=0x8000, page_table_stride=64, page_tokens=64, kv_stride_batch=8 * 64 * 128)
+    assert lib.spot_sparse_attn_decode_workspace_bytes(C.byref(_attn_params(**paged))) > 0
+    for o in (dict(page_tokens=0), dict(page_tokens=40), dict(page_table_stride=63), dict(kv_stride_batch=8 * 64 * 128 + 8)):
+        assert lib.spot_sparse_attn_decode(C.byref(_attn_params(**dict(paged, **o))), None) == INVALID, o
+    assert lib.spot_sparse_attn_prefill(C.byref(_attn_params(Tq=64, **paged)), None) == UNSUPPORTED
     assert lib.spot_decode_step_host(None, None) == INVALID
 
 

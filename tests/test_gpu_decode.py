@@ -466,3 +466,44 @@ def test_block16_end_to_end_step(torch_cuda):
         want, _ = H.oracle_attend(wl, b, sel.indices)
         err = np.abs(out[b] - want)
         assert err.max() <= MAX_ABS and err.mean() <= MEAN_ABS
+
+
+# ---------------------------------------------------------------- f3: paged K/V
+@pytest.mark.parametrize("blk,page_tokens,layout", [(64, 64, "phd"), (64, 128, "pthd"), (16, 16, "phd"), (16, 64, "pthd")])
+def test_paged_kv_decode_attention(torch_cuda, blk, page_tokens, layout):
+    """K/V live in a page pool shared by the batch, pages placed at random (and garbage in the unused ones); the
+    oracle reads the pool back through its page table (oracle.attention.gather_paged_kv) and attends as usual."""
+    torch = torch_cuda
+    from oracle import attention as OA
+    over = F3 if blk == 16 else {}
+    wl = make_config("mini2", **over)
+    dd = H.DeviceDecode(wl, "bf16")
+    pt, B, Hkv, D, Lc = page_tokens, wl.B, wl.H_kv, wl.D, wl.L_cap
+    n_log = -(-Lc // pt)
+    rng = np.random.default_rng(31)
+    n_pages = B * n_log + 7
+    table = rng.permutation(n_pages)[:B * n_log].reshape(B, n_log).astype(np.int32)
+    poolK = rng.integers(0, 1 << 16, size=(n_pages, pt, Hkv, D), dtype=np.uint16) & 0x3fff      # finite garbage
+    poolV = rng.integers(0, 1 << 16, size=(n_pages, pt, Hkv, D), dtype=np.uint16) & 0x3fff
+    for b in range(B):
+        Kb, Vb = wl.K[b].transpose(1, 0, 2), wl.V[b].transpose(1, 0, 2)             # [L][H_kv][D]
+        for lp in range(n_log):
+            t0, t1 = lp * pt, min((lp + 1) * pt, Lc)
+            poolK[table[b, lp], :t1 - t0] = Kb[t0:t1]
+            poolV[table[b, lp], :t1 - t0] = Vb[t0:t1]
+        Lb = int(wl.seq_len[b])
+        assert np.array_equal(OA.gather_paged_kv(poolK, table[b], Lb, pt), Kb[:Lb])  # the oracle's reading of the pool
+        assert np.array_equal(OA.gather_paged_kv(poolV, table[b], Lb, pt), Vb[:Lb])
+    if layout == "phd":          # [page][H_kv][page_tokens][D]
+        dd.K, dd.V = H.dev_u16(np.ascontiguousarray(poolK.transpose(0, 2, 1, 3))), H.dev_u16(np.ascontiguousarray(poolV.transpose(0, 2, 1, 3)))
+        dd.kv_strides = (Hkv * pt * D, D, pt * D)
+    else:                        # [page][page_tokens][H_kv][D]
+        dd.K, dd.V = H.dev_u16(poolK), H.dev_u16(poolV)
+        dd.kv_strides = (pt * Hkv * D, Hkv * D, D)
+    dd.page_table = torch.from_numpy(table).cuda()
+    dd.page_tokens = pt
+    lists = [H.oracle_select(wl, "bf16", b)[1].indices.tolist() for b in range(B)]
+    _check_attend(dd, lists)
+    n_b = [-(-int(L) // blk) for L in wl.seq_len]
+    _check_attend(dd, [[0], [3, n_b[1] - 1], [1, 2, n_b[2] - 1]])
+    _check_attend(dd, [list(range(n)) for n in n_b], dense=True)
