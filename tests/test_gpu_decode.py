@@ -507,3 +507,33 @@ def test_paged_kv_decode_attention(torch_cuda, blk, page_tokens, layout):
     n_b = [-(-int(L) // blk) for L in wl.seq_len]
     _check_attend(dd, [[0], [3, n_b[1] - 1], [1, 2, n_b[2] - 1]])
     _check_attend(dd, [list(range(n)) for n in n_b], dense=True)
+
+
+# ---------------------------------------------------------------- f2: quantised selector queries (decode)
+@pytest.mark.parametrize("fmt", ["mxfp4", "int4_e4m3", "fp8_e4m3"])
+def test_quantised_query_through_the_cache_quantiser(torch_cuda, fmt):
+    """PAPER.md:115 / :186 quantise the selector's queries as well as its key cache.  Every value these quantisers
+    produce is exactly a BF16 number, so a quantised query is the BF16 query passed through spot_quantize_selector_k /
+    spot_dequantize_selector_k (a one-token-per-sequence scratch cache) and then scored by the unchanged kernels:
+    (a) the round trip equals the oracle's quantiser on the query bit for bit, (b) selection with it matches the
+    oracle run on (quantised q, quantised K)."""
+    torch = torch_cuda
+    from paper_2606_22874_b200 import api
+    wl = make_config("mini2", with_kv=False)
+    dd = H.DeviceDecode(wl, fmt, with_kv=False)
+    B, Hh, d = wl.B, wl.H_idx, wl.d_idx
+    scratch = torch.zeros(api.spot_selector_k_bytes(fmt, B, 64, Hh, d), dtype=torch.uint8, device="cuda")
+    qq = torch.zeros((B, 1, Hh, d), dtype=torch.int16, device="cuda")
+    api.spot_quantize_selector_k(dd.sel_q, scratch, fmt, B, 1, 0, 64, Hh, d)
+    api.spot_dequantize_selector_k(scratch, qq, fmt, B, 1, 0, 64, Hh, d)
+    torch.cuda.synchronize()
+    got_bits = H.to_np_u16(qq).reshape(B, Hh, d)
+    want = OQ.quantize_dequantize(fmt, wl.sel_q)                        # fp64 values
+    assert np.array_equal(bf16_bits_to_f64(got_bits), want)
+    from workloads import f32_to_bf16_bits
+    assert np.array_equal(bf16_bits_to_f64(f32_to_bf16_bits(want.astype(np.float32))), want)   # exactly BF16
+    wl.sel_q = got_bits.copy()                                          # the oracle now sees the quantised query too
+    dd.sel_q = qq.reshape(B, Hh, d)
+    report = []
+    _check_select(dd, fmt, report)
+    _check_select(dd, fmt, report, mode="topk", top_k=16)
