@@ -434,13 +434,15 @@ def tensor_peaks():
     return 1700.0, 1700.0, "fallback (B200_PROFILING.md)"
 
 
-def oracle_prefill_sample(wl, K, V, Q, blocks, p):
+def oracle_prefill_sample(wl, K, V, Q, blocks, p, fmt="bf16"):
     """The oracle's prefill layer pass on a few query blocks (scoring, selection, attention).  K/V/Q: BF16 bits on the
     host.  Returns (seconds, scored tiles, attended (query block, key block) pairs)."""
     from oracle import attention as OA
+    from oracle import quant as OQ
     from oracle import selection as OS
     from oracle.bf16 import bf16_bits_to_f64
     t0 = time.perf_counter()
+    keys = OQ.quantize_dequantize(fmt, wl.sel_k[:(max(blocks) + 1) * 64])        # fp64, as the cache format stores them
     tiles = pairs = 0
     kw = wl.select_kwargs()
     kw["p"] = p
@@ -448,7 +450,7 @@ def oracle_prefill_sample(wl, K, V, Q, blocks, p):
         q0 = i * 64
         n_tok = q0 + 64
         res = OS.select_prefill(bf16_bits_to_f64(wl.sel_q[q0:q0 + 64]), wl.w[q0:q0 + 64].astype(np.float64),
-                                bf16_bits_to_f64(wl.sel_k[:n_tok]), q0, wl.q_block, wl.blk, wl.mode, **kw)
+                                keys[:n_tok], q0, wl.q_block, wl.blk, wl.mode, **kw)
         s_bar, sel = res[0]
         OA.sparse_attn_prefill(bf16_bits_to_f64(Q[q0:q0 + 64]), bf16_bits_to_f64(K[:, :n_tok]).transpose(1, 0, 2),
                                bf16_bits_to_f64(V[:, :n_tok]).transpose(1, 0, 2), [sel.indices.tolist()], q0,
@@ -481,7 +483,7 @@ def run_prefill(args):
         blocks = [0, n_tok // 128, n_tok // 64 - 1]
         ts = []
         for i in range(args.warmup + args.steps):
-            dt, tiles, pairs = oracle_prefill_sample(wl, Kh, Vh, Qh, blocks, args.p)
+            dt, tiles, pairs = oracle_prefill_sample(wl, Kh, Vh, Qh, blocks, args.p, args.fmt)
             if i >= args.warmup:
                 ts.append(dt)
         full_tiles = n_qb * (n_qb + 1) // 2
@@ -516,13 +518,18 @@ def run_prefill(args):
     h_w = torch.from_numpy(wl.w).pin_memory()
     h_selk = torch.from_numpy(wl.sel_k.view(np.int16)).pin_memory()
     sel_q, w, sel_k = h_selq.to(dev), h_w.to(dev), h_selk.to(dev)
+    sel_k_bf16 = sel_k
+    if args.fmt != "bf16":
+        # f2: the selector cache in a quantised format; spot_select dequantises the visible prefix into its workspace
+        sel_k = torch.zeros(api.spot_selector_k_bytes(args.fmt, 1, L, wl.H_idx, wl.d_idx), dtype=torch.uint8, device=dev)
+        api.spot_quantize_selector_k(sel_k_bf16, sel_k, args.fmt, 1, L, 0, L, wl.H_idx, wl.d_idx)
     cap = n_qb
     nb_stride = (n_qb + 3) & ~3
     indices = torch.empty((n_qb, cap), dtype=torch.int32, device=dev)
     budgets = torch.empty((n_qb,), dtype=torch.int32, device=dev)
     scores = torch.empty((n_qb, nb_stride), dtype=torch.float32, device=dev)
     out = torch.empty((1, L, Hq, D), dtype=torch.int16, device=dev)
-    sp = api.make_select_params(sel_q, w, sel_k, "bf16", L, None, 0, 1, L, wl.H_idx, wl.d_idx, q_start=0, blk=64,
+    sp = api.make_select_params(sel_q, w, sel_k, args.fmt, L, None, 0, 1, L, wl.H_idx, wl.d_idx, q_start=0, blk=64,
                                 q_block=64, mode=wl.mode, top_k=wl.top_k, p=args.p, sink_blocks=wl.sink_blocks,
                                 recency_blocks=wl.recency_blocks, kmin_blocks=wl.kmin_blocks,
                                 temperature=wl.temperature, indices=indices, cap=cap, budgets=budgets,
@@ -600,7 +607,9 @@ def run_prefill(args):
         t0 = time.perf_counter()
         sel_q.copy_(h_selq, non_blocking=True)
         w.copy_(h_w, non_blocking=True)
-        sel_k.copy_(h_selk, non_blocking=True)
+        sel_k_bf16.copy_(h_selk, non_blocking=True)
+        if args.fmt != "bf16":             # the cache is produced from the fresh keys inside the step
+            api.spot_quantize_selector_k(sel_k_bf16, sel_k, args.fmt, 1, L, 0, L, wl.H_idx, wl.d_idx, stream)
         api.spot_select(sp, stream)
         api.spot_sparse_attn_prefill(ap, stream)
         h_bud.copy_(budgets, non_blocking=True)
@@ -630,13 +639,13 @@ def run_prefill(args):
     Vh = V[0, :, :n_tok].contiguous().view(torch.int16).cpu().numpy().view(np.uint16)
     Qh = Q[0, :n_tok].contiguous().view(torch.int16).cpu().numpy().view(np.uint16)
     blocks = [0, n_tok // 128, n_tok // 64 - 1]
-    cpu_t, cpu_tiles, cpu_pairs = oracle_prefill_sample(wl, Kh, Vh, Qh, blocks, args.p)
+    cpu_t, cpu_tiles, cpu_pairs = oracle_prefill_sample(wl, Kh, Vh, Qh, blocks, args.p, args.fmt)
     line = {
         "metric": PF_METRIC, "value": step_mean, "unit": "ms/layer", "n_gpus": world, "steps": args.steps,
         "warmup": W, "ms_per_step": step_mean, "higher_is_better": False, "scaling": "weak", "vs_baseline": None,
         "dtype": "bf16", "data": "synthetic",
         "config": {"workload": "cfg5", "B": 1, "L": L, "H_q": Hq, "H_kv": Hkv, "D": D,
-                   "selector": "%dx%d bf16" % (wl.H_idx, wl.d_idx), "blk": 64, "q_block": 64, "mode": wl.mode, "p": args.p,
+                   "selector": "%dx%d %s" % (wl.H_idx, wl.d_idx, args.fmt), "blk": 64, "q_block": 64, "mode": wl.mode, "p": args.p,
                    "sink/recency/kmin": [wl.sink_blocks, wl.recency_blocks, wl.kmin_blocks],
                    "mean_budget": float(bud_host.mean()), "density": float(bud_host.sum()) / tiles,
                    "l2": "flushed by a 512 MiB read sweep before every timed step"},

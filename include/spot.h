@@ -194,7 +194,8 @@ spot_status spot_select(const spot_select_params* p, void* stream);
 
 /* a1 / a1' alone -- the scoring half of spot_select: writes s_bar into block_scores (required,
  * row stride nb_stride) and stops; the rule fields, indices, budgets, cap and the workspace are ignored.  Same
- * argument checks and errors as spot_select otherwise.  Lets a caller (and bench.py) run and time the selector
+ * argument checks and errors as spot_select otherwise (one exception: prefill rows over a quantised cache need
+ * spot_select_workspace_bytes of workspace for the dequantised prefix).  Lets a caller (and bench.py) run and time the selector
  * scoring kernel by itself. */
 spot_status spot_score_blocks(const spot_select_params* p, void* stream);
 

@@ -90,6 +90,27 @@ spot_status select_geometry(const spot_select_params* p, SelectGeom* g, bool sco
     return SPOT_OK;
 }
 
+// Prefill scoring of a quantised cache (f2): the visible prefix is dequantised into a BF16 scratch in the workspace and
+// the BF16 tile-score GEMM runs on that (every dequantised value is exactly a BF16 number).  What the paper's own
+// kernels do ("dequantisation overhead"); a fused unpack inside the GEMM's operand path is the next form.
+size_t prefill_scratch_bytes(const spot_select_params* p) {
+    if (p->q_block == 1 || p->fmt == SPOT_SELK_BF16) return 0;
+    return 256 + (size_t)p->B * ((size_t)p->q_start + p->Tq) * p->H_idx * p->d_idx * 2;
+}
+
+spot_status score_any(const spot_select_params* p, float* scores, int nb_stride, void* scratch_area, cudaStream_t s) {
+    if (p->q_block == 1) return score_decode(p, scores, nb_stride, s);
+    if (p->fmt == SPOT_SELK_BF16) return score_prefill(p, scores, nb_stride, s);
+    uint16_t* deq = reinterpret_cast<uint16_t*>((reinterpret_cast<uintptr_t>(scratch_area) + 255) & ~(uintptr_t)255);
+    const int tok = p->q_start + p->Tq;
+    spot_status st = spot_dequantize_selector_k(p->sel_k, deq, (spot_selk_format)p->fmt, p->B, tok, 0, p->cache_stride_tokens, p->H_idx,
+                                                p->d_idx, (void*)s);
+    if (st != SPOT_OK) return st;
+    spot_select_params q = *p;
+    q.sel_k = deq; q.fmt = SPOT_SELK_BF16; q.cache_stride_tokens = tok;
+    return score_prefill(&q, scores, nb_stride, s);
+}
+
 }  // namespace
 
 }  // namespace spot
@@ -124,7 +145,7 @@ extern "C" size_t spot_select_workspace_bytes(const spot_select_params* p) {
     if (select_geometry(p, &g) != SPOT_OK) return 0;
     size_t bytes = 256;
     if (g.own_scores) bytes += (size_t)p->B * g.rows_per_seq * g.nb_stride * sizeof(float);
-    return bytes;
+    return bytes + prefill_scratch_bytes(p);
 }
 
 extern "C" spot_status spot_select(const spot_select_params* p, void* stream) {
@@ -133,14 +154,13 @@ extern "C" spot_status spot_select(const spot_select_params* p, void* stream) {
     if (st != SPOT_OK) return st;
     if ((st = check_device()) != SPOT_OK) return st;
     float* scores = p->block_scores;
-    if (g.own_scores) {
-        size_t need = 256 + (size_t)p->B * g.rows_per_seq * g.nb_stride * sizeof(float);
-        if (!p->workspace || p->workspace_bytes < need) return SPOT_ERR_WORKSPACE_TOO_SMALL;
+    const size_t own = g.own_scores ? 256 + (size_t)p->B * g.rows_per_seq * g.nb_stride * sizeof(float) : 0;
+    const size_t need = own + prefill_scratch_bytes(p);
+    if (need && (!p->workspace || p->workspace_bytes < need)) return SPOT_ERR_WORKSPACE_TOO_SMALL;
+    if (g.own_scores)
         scores = reinterpret_cast<float*>(reinterpret_cast<uintptr_t>(p->workspace) + 255 & ~(uintptr_t)255);
-    }
     cudaStream_t s = (cudaStream_t)stream;
-    if (p->q_block == 1) st = score_decode(p, scores, g.nb_stride, s);
-    else st = score_prefill(p, scores, g.nb_stride, s);
+    st = score_any(p, scores, g.nb_stride, reinterpret_cast<char*>(p->workspace) + own, s);
     if (st != SPOT_OK) return st;
     return run_select(p, scores, g.nb_stride, g.rows_per_seq, g.max_nb, s);
 }
@@ -151,8 +171,9 @@ extern "C" spot_status spot_score_blocks(const spot_select_params* p, void* stre
     if (st != SPOT_OK) return st;
     if ((st = check_device()) != SPOT_OK) return st;
     cudaStream_t s = (cudaStream_t)stream;
-    return p->q_block == 1 ? score_decode(p, p->block_scores, g.nb_stride, s)
-                           : score_prefill(p, p->block_scores, g.nb_stride, s);
+    const size_t need = prefill_scratch_bytes(p);        // quantised cache in prefill: the one case that needs the workspace
+    if (need && (!p->workspace || p->workspace_bytes < need)) return SPOT_ERR_WORKSPACE_TOO_SMALL;
+    return score_any(p, p->block_scores, g.nb_stride, p->workspace, s);
 }
 
 extern "C" spot_status spot_decode_step_host(const spot_decode_step_host_params* p, void* stream) {

@@ -184,7 +184,8 @@ class DevicePrefill:
         nb_stride = (self.n_b_max + 3) & ~3
         scores = torch.full((rows, nb_stride), float("nan"), device="cuda") if want_scores else None
         probs = torch.full((rows, nb_stride), float("nan"), device="cuda") if want_probs else None
-        sp = api.make_select_params(self.sel_q, self.w, self.sel_k, "bf16", self.L, None, 0, self.B, self.Tq,
+        sp = api.make_select_params(self.sel_q, self.w, self.sel_k, getattr(self, "fmt", "bf16"), self.L, None, 0,
+                                    self.B, self.Tq,
                                     wl.H_idx, wl.d_idx, q_start=self.q_start, blk=wl.blk, q_block=wl.q_block,
                                     indices=indices, cap=cap, budgets=budgets, block_scores=scores,
                                     block_probs=probs, nb_stride=nb_stride, **kw)
@@ -194,6 +195,20 @@ class DevicePrefill:
         torch.cuda.synchronize()
         return (indices.cpu().numpy(), budgets.cpu().numpy(),
                 None if scores is None else scores.cpu().numpy(), None if probs is None else probs.cpu().numpy())
+
+    def set_cache_format(self, fmt):
+        """Re-store the selector cache in a quantised format (f2); the workloads' BF16 keys are replaced by the ORACLE
+        quantiser's image of them (exactly BF16 numbers), so the oracle side needs no other change."""
+        import torch
+        from workloads import f32_to_bf16_bits
+        wl, api = self.wl, self.api
+        bf16 = self.sel_k
+        self.sel_k = torch.zeros(api.spot_selector_k_bytes(fmt, self.B, self.L, wl.H_idx, wl.d_idx), dtype=torch.uint8,
+                                 device="cuda")
+        api.spot_quantize_selector_k(bf16, self.sel_k, fmt, self.B, self.L, 0, self.L, wl.H_idx, wl.d_idx)
+        self.fmt = fmt
+        for x in self.wls:
+            x.sel_k = f32_to_bf16_bits(OQ.quantize_dequantize(fmt, x.sel_k).astype(np.float32))
 
     def attend(self, indices_np, budgets_np, want_lse=False):
         import torch

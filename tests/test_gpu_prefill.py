@@ -69,6 +69,39 @@ def test_prefill_scores_and_selection(torch_cuda, L, q_start, Tq, B, over):
     print("prefill select L=%d q_start=%d Tq=%d: %d near-tie rows %s" % (L, q_start, Tq, len(report), report[:4]))
 
 
+@pytest.mark.parametrize("fmt", ["mxfp4", "int4_e4m3", "fp8_e4m3"])
+def test_prefill_selection_over_a_quantised_cache(torch_cuda, fmt):
+    """f2: a later chunk (batch of 2, odd number of query blocks) scored against a quantised selector cache -- the
+    library dequantises the visible prefix into its workspace and runs the BF16 tile-score GEMM; the oracle scores the
+    oracle-quantised keys.  spot_score_blocks takes the same path and needs the same workspace."""
+    torch = torch_cuda
+    from paper_2606_22874_b200 import api
+    wls = [_neg_weights(make_prefill_workload(seed=6006 + 7 * b, L=1024, with_kv=False), 70 + b) for b in range(2)]
+    dp = H.DevicePrefill(wls, 512, 320, with_kv=False)
+    dp.set_cache_format(fmt)
+    report = []
+    idx, bud = _check_select_prefill(dp, report)
+    _check_select_prefill(dp, report, mode="topk", top_k=6)
+    print("quantised prefill select (%s): near-tie rows %s" % (fmt, report[:4]))
+    # score-only entry: same scores; too small a workspace is reported, not overrun
+    wl = dp.wl
+    nb_stride = (dp.n_b_max + 3) & ~3
+    scores = torch.full((dp.B * dp.n_q, nb_stride), float("nan"), device="cuda")
+    sp = api.make_select_params(dp.sel_q, dp.w, dp.sel_k, fmt, dp.L, None, 0, dp.B, dp.Tq, wl.H_idx, wl.d_idx,
+                                q_start=dp.q_start, blk=wl.blk, q_block=wl.q_block, block_scores=scores,
+                                nb_stride=nb_stride)
+    with pytest.raises(RuntimeError, match="WORKSPACE"):
+        api.spot_score_blocks(sp)
+    ws = torch.empty(256 + dp.B * (dp.q_start + dp.Tq) * wl.H_idx * wl.d_idx * 2, dtype=torch.uint8, device="cuda")
+    sp.workspace, sp.workspace_bytes = ws.data_ptr(), ws.numel()
+    api.spot_score_blocks(sp)
+    torch.cuda.synchronize()
+    got = scores.cpu().numpy()
+    for b, w in enumerate(dp.wls):
+        for i, (s_bar, _) in enumerate(H.oracle_select_prefill(w, dp.q_start, dp.Tq)):
+            np.testing.assert_allclose(got[b * dp.n_q + i, :len(s_bar)], s_bar, rtol=2e-5, atol=2e-5)
+
+
 def _check_attn_prefill(dp, lists_per_seq, want_lse=False):
     """lists_per_seq[b][i] = selected key blocks of query block i of sequence b (the oracle's lists on both sides)."""
     wl = dp.wl
