@@ -217,7 +217,8 @@ def test_end_to_end_step_matches_oracle(torch_cuda):
 @pytest.mark.parametrize("cfg,fmt,seqs", [("cfg3", "bf16", (0, 3)), ("cfg3", "mxfp4", (1,)), ("cfg3", "int4_e4m3", (2,)),
                                           ("cfg2", "bf16", (0, 7)), ("cfg4_b4", "mxfp4", (0, 1, 2, 3)),
                                           ("cfg3/d128", "bf16", (1,)), ("cfg3/d128", "mxfp4", (2,)),
-                                          ("cfg3", "fp8_e4m3", (3,)), ("cfg3/d128", "fp8_e4m3", (0,))])
+                                          ("cfg3", "fp8_e4m3", (3,)), ("cfg3/d128", "fp8_e4m3", (0,)),
+                                          ("cfg3/blk16", "bf16", (2,)), ("cfg3/blk16/d128", "mxfp4", (0,))])
 def test_full_size_configs_in_the_bench_configuration(torch_cuda, cfg, fmt, seqs):
     """BASELINE.json configs 2, 3 and 4 (batch 4) at full size (config 3: B=4, L=131072, 2048 blocks per sequence;
     config 4: H_q=64 and per-query budgets from the K_min floor to hundreds of blocks), launched exactly as bench.py
@@ -229,7 +230,13 @@ def test_full_size_configs_in_the_bench_configuration(torch_cuda, cfg, fmt, seqs
     from oracle import attention as OA
     from paper_2606_22874_b200 import api
     # "/d128": the paper's selector geometry, 4 heads x 128, instead of BASELINE.json's 4 x 64
-    wl = make_config(cfg.split("/")[0], with_kv=False, **({"d_idx": 128} if cfg.endswith("/d128") else {}))
+    # "/blk16": the paper's 16-token blocks with its 8 / 16 / 32 reserved blocks (f3): 8192 blocks per sequence
+    parts = cfg.split("/")
+    over = {"d_idx": 128} if "d128" in parts else {}
+    if "blk16" in parts:
+        over.update(blk=16, sink_blocks=8, recency_blocks=16, kmin_blocks=32)
+    wl = make_config(parts[0], with_kv=False, **over)
+    blk = wl.blk
     dd = H.DeviceDecode(wl, fmt, with_kv=False)
     idx, bud, scores, probs = dd.select()
     assert bud.min() >= 8 and bud.max() <= dd.n_b_max
@@ -270,11 +277,11 @@ def test_full_size_configs_in_the_bench_configuration(torch_cuda, cfg, fmt, seqs
     for b in seqs:
         blocks = torch.from_numpy(sels[b].indices.astype(np.int64)).to(dev)
         n = len(blocks)
-        Kg = K[b].view(Hkv, L // 64, 64, D)[:, blocks].reshape(Hkv, n * 64, D)
-        Vg = V[b].view(Hkv, L // 64, 64, D)[:, blocks].reshape(Hkv, n * 64, D)
+        Kg = K[b].view(Hkv, L // blk, blk, D)[:, blocks].reshape(Hkv, n * blk, D)
+        Vg = V[b].view(Hkv, L // blk, blk, D)[:, blocks].reshape(Hkv, n * blk, D)
         Kh = H.bf16_bits_to_f64(H.to_np_u16(Kg.contiguous().view(torch.int16))).transpose(1, 0, 2)
         Vh = H.bf16_bits_to_f64(H.to_np_u16(Vg.contiguous().view(torch.int16))).transpose(1, 0, 2)
-        want, want_lse = OA.sparse_attn_decode(H.bf16_bits_to_f64(wl.q[b]), Kh, Vh, np.arange(n), n * 64, 64, wl.sm_scale)
+        want, want_lse = OA.sparse_attn_decode(H.bf16_bits_to_f64(wl.q[b]), Kh, Vh, np.arange(n), n * blk, blk, wl.sm_scale)
         err = np.abs(got[b] - want)
         assert err.max() <= MAX_ABS and err.mean() <= MEAN_ABS, (b, err.max(), err.mean())
         assert np.abs(lse[b].cpu().numpy() - want_lse).max() <= 2e-3
