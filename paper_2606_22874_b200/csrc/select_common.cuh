@@ -1,4 +1,4 @@
-// Shared by the two selection kernels (select.cu: bitonic-sort form; select_hist.cu: histogram-partition form).
+// Shared by select.cu (argument marshalling) and select_hist.cu (the selection kernel).
 #pragma once
 #include "common.cuh"
 

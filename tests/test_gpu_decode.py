@@ -146,7 +146,7 @@ def test_select_crowded_cut_bins_and_ties(torch_cuda, n_b, blk):
 @pytest.mark.parametrize("L", [200000, 300000, 524288])
 def test_select_rows_longer_than_2048_blocks(torch_cuda, L):
     """n_b = 3125 / 4688 / 8192 (the maximum row the library accepts, L = 512K as in PAPER.md:144): rows beyond the
-    histogram kernel's 2048 blocks take the bitonic-sort kernel (LT = 9 / 10)."""
+    2048 blocks take the 8192-key form of the histogram kernel (1024 threads x 8 keys, 128 KiB of shared memory)."""
     wl = make_decode_workload("long", 77 + L, B=1, L=L, kind="zipf", zipf_s=1.1, with_kv=False)
     dd = H.DeviceDecode(wl, "bf16", with_kv=False)
     report = []
@@ -429,7 +429,7 @@ def test_block16_select_matches_oracle(torch_cuda, cfg, fmt):
 
 def test_block16_select_edge_cases_and_long_rows(torch_cuda):
     # ragged tails inside a tile (L % 64 in 1..63, L % 16 != 0), contexts smaller than the reserved tiers, d_idx = 128,
-    # and rows beyond 2048 blocks (L = 40000 -> 2500 blocks, 131072 -> 8192: the bitonic kernels)
+    # and rows beyond 2048 blocks (L = 40000 -> 2500 blocks, 131072 -> 8192: the 8192-key form of the selection kernel)
     for seed, L, seqs, d_idx in [(11, 64, [1, 17, 64], 64), (12, 320, [65, 129, 307], 64), (13, 2048, [2048, 1999, 777], 128)]:
         wl = make_decode_workload("e16_%d" % seed, seed, B=3, L=L, kind="gauss", seq_lens=seqs, d_idx=d_idx,
                                   with_kv=False, blk=16)
