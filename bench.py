@@ -552,24 +552,25 @@ def run_prefill(args):
             torch.cuda.synchronize()
 
     W = max(args.warmup, 3)
-    for _ in range(W):
-        flush_l2()
-        api.spot_select(sp, stream)
-        api.spot_sparse_attn_prefill(ap, stream)
-    barrier()
-    # the selector GEMM kernel alone (spot_score_blocks = a1' only), live, for the roofline object -- timed BEFORE the
-    # long step loop: its denominator is the burst peak of a kernel timed alone (B200_PROFILING.md), and tens of ms of
-    # attention per step push the part into its power cap
+    # the selector GEMM kernel alone (spot_score_blocks = a1' only), live, for the roofline object -- timed FIRST, after
+    # W warm-up launches of its own and before any attention pass: its denominator is the burst peak of a kernel timed
+    # alone (B200_PROFILING.md), and tens of ms of attention per step push the part into its power cap (SM clock
+    # 1800 instead of 1965 MHz: the same kernel then takes 1.28 instead of 1.17 ms)
     sc = []
-    for i in range(args.steps + 2):
+    for i in range(args.steps + W):
         flush_l2()
         a_, b_ = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         a_.record(stream)
         api.spot_score_blocks(sp, stream)
         b_.record(stream)
         torch.cuda.synchronize()
-        if i >= 2:
+        if i >= W:
             sc.append(a_.elapsed_time(b_))
+    for _ in range(W):
+        flush_l2()
+        api.spot_select(sp, stream)
+        api.spot_sparse_attn_prefill(ap, stream)
+    barrier()
     ev = [[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(args.steps)]
     clk = ClockSampler(local_rank)
     clk.__enter__()
