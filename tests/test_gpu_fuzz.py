@@ -83,3 +83,34 @@ def test_fuzz_attention(torch_cuda, chunk):
         lists = [x if x else [0] for x in lists]
         _check_attend(dd, lists)
         _check_attend(dd, [list(range(-(-int(L) // blk))) for L in wl.seq_len], dense=True)
+
+
+@pytest.mark.parametrize("chunk", range(2))
+def test_fuzz_prefill(torch_cuda, chunk):
+    """Chunked prefill: random prompt length, chunk position and size, batch, GQA group, selector head dim, rule
+    parameters and cache format; selection against the oracle, attention over the oracle's lists."""
+    from tests.test_gpu_prefill import _check_attn_prefill, _check_select_prefill
+    from workloads import make_prefill_workload
+    rng = np.random.default_rng(31337 + chunk)
+    for case in range(chunk * 6, chunk * 6 + 6):
+        L = int(rng.choice([256, 640, 1024, 1536]))
+        n_blk = L // 64
+        qb0 = int(rng.integers(0, n_blk))
+        nqb = int(rng.integers(1, min(n_blk - qb0, 6) + 1))
+        B = int(rng.integers(1, 3))
+        over = dict(p=float(rng.choice([0.5, 0.9, 1.0])), sink_blocks=int(rng.integers(0, 3)),
+                    recency_blocks=int(rng.integers(0, 4)), kmin_blocks=int(rng.integers(0, 10)))
+        if rng.random() < 0.25:
+            over = dict(mode="topk", top_k=int(rng.integers(3, 12)), sink_blocks=1, recency_blocks=2)
+        H_q = int(rng.choice([8, 32, 64]))
+        wls = [make_prefill_workload(seed=8000 + 13 * case + b, L=L, H_q=H_q, topic_span=int(rng.choice([64, 128, 256])))
+               for b in range(B)]
+        dp = H.DevicePrefill(wls, qb0 * 64, nqb * 64)
+        fmt = str(rng.choice(["bf16", "bf16", "mxfp4", "fp8_e4m3"]))
+        if fmt != "bf16":
+            dp.set_cache_format(fmt)
+        report = []
+        _check_select_prefill(dp, report, **over)
+        lists = [[sel.indices.tolist() for _, sel in H.oracle_select_prefill(w, dp.q_start, dp.Tq, **over)] for w in wls]
+        _check_attn_prefill(dp, lists)
+        print("fuzz prefill case %d: L=%d q_start=%d Tq=%d B=%d H_q=%d %s near-ties %s" % (case, L, dp.q_start, dp.Tq, B, H_q, fmt, report))
