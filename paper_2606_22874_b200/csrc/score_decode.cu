@@ -120,7 +120,9 @@ struct ScoreCfg {
     // FP8 (self-serve ring, split tiles): a 16 / 32 KiB tile would leave room for 6 / 3 warps only, so a stage holds
     // an 8 KiB slice (32 / 16 tokens) and a warp walks the SPLIT slices of its tile through its two stages, keeping
     // the running block maximum in registers.  (4 KiB slices x 4 stages per warp: no faster, 39.9 vs 38.0 us score + select.)
-    static constexpr int SPLIT = FMT == SPOT_SELK_FP8_E4M3 ? TILE_BYTES / 8192 : 1;
+    // The 17 KiB 4-bit tiles of d_idx = 128 get the same treatment (12 warps instead of 6): a slice is 32 tokens' codes
+    // plus their scale bytes, two bulk copies on one barrier.
+    static constexpr int SPLIT = FMT == SPOT_SELK_FP8_E4M3 ? TILE_BYTES / 8192 : (SELF && TILE_BYTES > 12288 ? 2 : 1);
     static constexpr int STAGE_BYTES = SELF ? TILE_BYTES / SPLIT : (TILE_BYTES + 1023) / 1024 * 1024;
     static constexpr int STAGES_RAW = SC_SMEM_BUDGET / STAGE_BYTES;
     static constexpr int SELF_MAX = (208 * 1024 / STAGE_BYTES) / 2;           // warps that fit with 2 stages each
@@ -295,11 +297,14 @@ struct Q4Tile {
         __syncwarp();
     }
 
-    __device__ __forceinline__ float tile_max(uint32_t st, int t0, int L, int lane, bool fine) const {
+    // maximum over the NIT * 16 tokens of a slice whose codes start at shared address st and whose scale bytes follow
+    // them ([NIT*16][CPT] then [NIT*16][NG]); it0 = the slice's first 16-token group inside its tile (fine form)
+    template <int NIT>
+    __device__ __forceinline__ float part_max(uint32_t st, int t0, int L, int lane, bool fine, int it0) const {
         const int g = lane >> 2, c = lane & 3;
         float m = -INFINITY;
 #pragma unroll 2
-        for (int it = 0; it < 4; ++it) {
+        for (int it = 0; it < NIT; ++it) {
             uint4 cd[NQL][2];
             uint32_t scw[2][NQL];
 #pragma unroll
@@ -308,7 +313,7 @@ struct Q4Tile {
 #pragma unroll
                 for (int ql = 0; ql < NQL; ++ql) {
                     cd[ql][hf] = lds128(st + tok * CPT + ql * 64 + c * 16);
-                    scw[hf][ql] = lds32(st + 64 * CPT + tok * NG + ql * 4);
+                    scw[hf][ql] = lds32(st + NIT * 16 * CPT + tok * NG + ql * 4);
                 }
             }
             float srow[2] = {0.f, 0.f};
@@ -344,7 +349,7 @@ struct Q4Tile {
             const float sa = srow[0] + __shfl_xor_sync(0xffffffffu, srow[0], 1);
             const float sb = srow[1] + __shfl_xor_sync(0xffffffffu, srow[1], 1);
             const int ta = t0 + it * 16 + g, tbk = ta + 8;
-            m = group_update(m, sa, sb, ta < L, tbk < L, it, lane, fine);
+            m = group_update(m, sa, sb, ta < L, tbk < L, it0 + it, lane, fine);
         }
         return fine ? m : rows_max(m, lane);
     }
@@ -517,10 +522,18 @@ __global__ void __launch_bounds__((ScoreCfg<H, D_IDX, FMT>::THREADS), 1) score_d
                 const uint32_t s = warp * K + rq % K;
                 asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // earlier generic reads of the stage
                 mbar_arrive_expect_tx(bar_full + 8 * s, Cfg::STAGE_BYTES);
-                bulk_load(ring + s * Cfg::STAGE_BYTES,
-                          a.sel_k + ((int64_t)nxt.b * a.tiles_per_seq + nxt.t) * Cfg::TILE_BYTES
-                              + (rq % SP) * Cfg::STAGE_BYTES,
-                          Cfg::STAGE_BYTES, bar_full + 8 * s);
+                const uint8_t* tile_src = a.sel_k + ((int64_t)nxt.b * a.tiles_per_seq + nxt.t) * Cfg::TILE_BYTES;
+                if constexpr (FMT == SPOT_SELK_FP8_E4M3 || SP == 1) {
+                    bulk_load(ring + s * Cfg::STAGE_BYTES, tile_src + (rq % SP) * Cfg::STAGE_BYTES, Cfg::STAGE_BYTES,
+                              bar_full + 8 * s);
+                } else {
+                    // 4-bit slice: the slice's code rows, then its scale rows (they sit behind all 64 code rows)
+                    constexpr int NTOK = 64 / SP, CODES = NTOK * (Cfg::ROW / 2), SCALES = NTOK * (Cfg::ROW / 32);
+                    static_assert(CODES + SCALES == Cfg::STAGE_BYTES && SCALES % 16 == 0, "4-bit slice geometry");
+                    bulk_load(ring + s * Cfg::STAGE_BYTES, tile_src + (rq % SP) * CODES, CODES, bar_full + 8 * s);
+                    bulk_load(ring + s * Cfg::STAGE_BYTES + CODES, tile_src + SP * CODES + (rq % SP) * SCALES, SCALES,
+                              bar_full + 8 * s);
+                }
             }
             if (rq % SP == SP - 1) nxt.advance(a, SC_CONSUMERS);
             ++rq;
@@ -540,12 +553,8 @@ __global__ void __launch_bounds__((ScoreCfg<H, D_IDX, FMT>::THREADS), 1) score_d
                 const int q = j * SP + part;
                 const uint32_t s = warp * K + q % K;
                 mbar_wait(bar_full + 8 * s, (q / K) & 1);
-                if constexpr (FMT == SPOT_SELK_FP8_E4M3)
-                    m = fmaxf(m, tile.template part_max<4 / SP>(ring + s * Cfg::STAGE_BYTES,
-                                                                cur.t * 64 + part * (64 / SP), L, lane, fine,
-                                                                part * (4 / SP)));
-                else
-                    m = tile.tile_max(ring + s * Cfg::STAGE_BYTES, cur.t * 64, L, lane, fine);
+                m = fmaxf(m, tile.template part_max<4 / SP>(ring + s * Cfg::STAGE_BYTES, cur.t * 64 + part * (64 / SP),
+                                                            L, lane, fine, part * (4 / SP)));
                 __syncwarp();
                 request_next();
             }
