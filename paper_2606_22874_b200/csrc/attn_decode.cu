@@ -13,6 +13,11 @@
 // heads of the group as the (padded) M = 16 rows.  M is tiny here, so this is mma.sync territory, not tcgen05: the
 // tensor pipe needs < 15 % of the time the HBM stream takes.  A second small kernel merges each (sequence, head)'s
 // partials (log-sum-exp) and writes BF16.
+//
+// Two next-row options ride on the same loop: with 16-token blocks (blk == 16) a unit is four
+// consecutive entries of the index list, one per warp (a short last unit is masked like tokens past the sequence end);
+// with a page table the K/V caches are page pools and every 16-token sub-tile is placed through one table lookup,
+// fetched with the index window a window of 32 units ahead (page_tokens % 16 == 0: a sub-tile never straddles pages).
 #include "common.cuh"
 
 namespace spot {

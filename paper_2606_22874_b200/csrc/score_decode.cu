@@ -20,6 +20,8 @@
 //                sum after the MMA (one FMUL per group instead of one per element).  The k index of each MMA is a
 //                fixed permutation of the d_idx axis applied to both operands, chosen so that every lane's 16-byte
 //                shared-memory load lands directly in fragment registers.
+//   FP8 cache  : (f2) one cvt.rn.f16x2.e4m3x2 per pair, no scales, the same fp16 HMMA.
+// With 16-token blocks (f3, blk == 16) a tile yields its four 16-token maxima instead of one.
 #include "common.cuh"
 #include "tc100.cuh"
 
