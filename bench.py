@@ -467,7 +467,7 @@ def run_prefill(args):
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
     L = args.L or 65536
-    wl = make_prefill_workload(seed=5005 + 1000 * rank, L=L, with_kv=False)
+    wl = make_prefill_workload(seed=5005 + 1000 * rank, L=L, with_kv=False, **D_IDX_OVERRIDE)
     wl.p = args.p
     n_qb = L // 64
     Hq, Hkv, D = wl.H_q, wl.H_kv, wl.D
@@ -683,7 +683,7 @@ def main():
     ap.add_argument("--p", type=float, default=0.90)
     ap.add_argument("--L", type=int, default=0, help="cfg5 only: prompt length (default 65536)")
     ap.add_argument("--d-idx", type=int, default=0, choices=[0, 64, 128],
-                    help="decode only: selector head dim (default: the config's 64; 128 = the paper's geometry, PAPER.md:363)")
+                    help="selector head dim (default: the config's 64; 128 = the paper's geometry, PAPER.md:363)")
     ap.add_argument("--paged", type=int, default=0, choices=[0, 16, 64, 256],
                     help="decode only: K/V as a page pool of this many tokens per page behind a random page table")
     ap.add_argument("--blk", type=int, default=64, choices=[64, 16],
@@ -692,7 +692,7 @@ def main():
     args = ap.parse_args()
     if args.d_idx:
         D_IDX_OVERRIDE["d_idx"] = args.d_idx
-    if args.blk == 16:
+    if args.blk == 16 and args.workload != "cfg5":
         D_IDX_OVERRIDE.update(blk=16, sink_blocks=8, recency_blocks=16, kmin_blocks=32)
     if args.workload == "cfg5":
         run_prefill(args)

@@ -26,19 +26,31 @@ namespace spot {
 namespace {
 
 constexpr int PF_H = 4;                 // selector heads
-constexpr int PF_D = 64;                // d_idx (one 128-byte swizzle row)
 constexpr int PF_M = 128;               // queries per tile (two 64-query blocks)
 constexpr int PF_N = 128;               // keys per MMA (two 64-key blocks)
 constexpr int PF_CHUNK = 32;            // key blocks per work item
-constexpr int PF_KSTAGES = 2;
 constexpr int PF_TSTAGES = 4;           // TMEM accumulators (128 columns each)
 constexpr int PF_EPI_WARPS = 8;
 constexpr int PF_THREADS = (PF_EPI_WARPS + 2) * 32;
-constexpr uint32_t Q_TILE_BYTES = PF_H * PF_M * PF_D * 2;   // 65536
-constexpr uint32_t K_TILE_BYTES = PF_H * PF_N * PF_D * 2;   // 65536
-constexpr uint32_t PF_SMEM_TILES = Q_TILE_BYTES + PF_KSTAGES * K_TILE_BYTES;
+constexpr uint32_t PF_PLANE_BYTES = 128 * 64 * 2;          // [128 rows][64 d] BF16: one 128-byte swizzle row per token
 constexpr uint32_t PF_SMEM_MISC = 1024;
-constexpr uint32_t PF_SMEM_BYTES = 1024 + PF_SMEM_TILES + PF_SMEM_MISC;   // 1024: manual alignment slack
+
+// d_idx = 64: a head is one plane; the query tile is 64 KiB and a K stage holds all four heads of a key-block pair
+// (64 KiB, 2 stages).  d_idx = 128 (the paper's selector width): a head is two planes (the cache row
+// [H][128] read as [2H][64]); the query tile is 128 KiB, so a K stage holds ONE head of a pair (32 KiB, 3 stages) and
+// the issuer accumulates both planes (8 k-steps) into the head's accumulator.
+template <int D>
+struct PfCfg {
+    static_assert(D == 64 || D == 128, "d_idx must be 64 or 128");
+    static constexpr int NSUB = D / 64;                                   // planes per head
+    static constexpr bool PER_HEAD = D == 128;                            // K ring granularity
+    static constexpr int KSTAGES = PER_HEAD ? 3 : 2;
+    static constexpr uint32_t Q_TILE_BYTES = PF_H * NSUB * PF_PLANE_BYTES;
+    static constexpr uint32_t K_STAGE_BYTES = (PER_HEAD ? NSUB : PF_H * NSUB) * PF_PLANE_BYTES;
+    static constexpr uint32_t SMEM_TILES = Q_TILE_BYTES + KSTAGES * K_STAGE_BYTES;
+    static constexpr uint32_t SMEM_BYTES = 1024 + SMEM_TILES + PF_SMEM_MISC;   // 1024: manual alignment slack
+    static_assert(SMEM_BYTES <= 227 * 1024, "shared memory");
+};
 
 struct PrefillScoreArgs {
     const float* w;           // [B][Tq][4]
@@ -71,25 +83,29 @@ __device__ __forceinline__ bool decode_item(const PrefillScoreArgs& a, int id, i
     return nk > 0;
 }
 
+template <int D>
 __global__ void __launch_bounds__(PF_THREADS, 1) score_prefill_kernel(const __grid_constant__ CUtensorMap tm_q,
                                                                       const __grid_constant__ CUtensorMap tm_k,
                                                                       const PrefillScoreArgs a) {
+    using Cfg = PfCfg<D>;
+    constexpr int PF_KSTAGES = Cfg::KSTAGES, NSUB = Cfg::NSUB;
+    constexpr uint32_t Q_TILE_BYTES = Cfg::Q_TILE_BYTES, K_TILE_BYTES = Cfg::K_STAGE_BYTES;
     extern __shared__ unsigned char smem_raw[];
     const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
     unsigned char* smem = smem_raw + (smem_base - smem_u32(smem_raw));
-    const uint32_t q_smem = smem_base;                               // 64 KiB
-    const uint32_t k_smem = smem_base + Q_TILE_BYTES;                // 2 x 64 KiB
-    unsigned char* misc = smem + PF_SMEM_TILES;
-    const uint32_t misc_u32 = smem_base + PF_SMEM_TILES;
+    const uint32_t q_smem = smem_base;                               // 64 / 128 KiB
+    const uint32_t k_smem = smem_base + Q_TILE_BYTES;                // 2 x 64 KiB / 3 x 32 KiB
+    unsigned char* misc = smem + Cfg::SMEM_TILES;
+    const uint32_t misc_u32 = smem_base + Cfg::SMEM_TILES;
     // barriers (8 bytes each)
     const uint32_t bar_q_full = misc_u32 + 0;
     const uint32_t bar_q_empty = misc_u32 + 8;
-    const uint32_t bar_k_full = misc_u32 + 16;     // [2]
-    const uint32_t bar_k_empty = misc_u32 + 32;    // [2]
-    const uint32_t bar_t_full = misc_u32 + 48;     // [4]
-    const uint32_t bar_t_empty = misc_u32 + 80;    // [4]
-    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(misc + 112);
-    uint32_t* s_max = reinterpret_cast<uint32_t*>(misc + 128);       // [2 item buffers][CHUNK][2 query blocks]
+    const uint32_t bar_k_full = misc_u32 + 16;     // [<= 4]
+    const uint32_t bar_k_empty = misc_u32 + 48;    // [<= 4]
+    const uint32_t bar_t_full = misc_u32 + 80;     // [4]
+    const uint32_t bar_t_empty = misc_u32 + 112;   // [4]
+    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(misc + 144);
+    uint32_t* s_max = reinterpret_cast<uint32_t*>(misc + 160);       // [2 item buffers][CHUNK][2 query blocks]
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
 
@@ -107,7 +123,7 @@ __global__ void __launch_bounds__(PF_THREADS, 1) score_prefill_kernel(const __gr
         mbar_fence_init();
     }
     if (threadIdx.x < 2 * PF_CHUNK * 2) s_max[threadIdx.x] = 0u;
-    if (warp == 0) tmem_alloc(misc_u32 + 112, 512);
+    if (warp == 0) tmem_alloc(misc_u32 + 144, 512);
     if (warp == PF_EPI_WARPS && lane == 0) {
         tma_prefetch_desc(&tm_q);
         tma_prefetch_desc(&tm_k);
@@ -130,13 +146,16 @@ __global__ void __launch_bounds__(PF_THREADS, 1) score_prefill_kernel(const __gr
                 mbar_arrive_expect_tx(bar_q_full, Q_TILE_BYTES);
                 tma_load_4d(q_smem, &tm_q, bar_q_full, 0, m * PF_M, 0, b);
                 const int np = (nk + 1) >> 1;
-                for (int pr = 0; pr < np; ++pr, ++kp) {
-                    const int s = kp % PF_KSTAGES;
-                    mbar_wait(bar_k_empty + 8 * s, ((kp / PF_KSTAGES) & 1) ^ 1);
-                    mbar_arrive_expect_tx(bar_k_full + 8 * s, K_TILE_BYTES);
-                    // a pair that overhangs the cache is zero-filled by TMA; its second block is never used
-                    tma_load_4d(k_smem + s * K_TILE_BYTES, &tm_k, bar_k_full + 8 * s, 0, (c * PF_CHUNK + 2 * pr) * 64, 0, b);
-                }
+                // (kp counts ring slots: one per pair at d_idx 64, one per (pair, head) at d_idx 128)
+                for (int pr = 0; pr < np; ++pr)
+                    for (int hh = 0; hh < (Cfg::PER_HEAD ? PF_H : 1); ++hh, ++kp) {
+                        const int s = kp % PF_KSTAGES;
+                        mbar_wait(bar_k_empty + 8 * s, ((kp / PF_KSTAGES) & 1) ^ 1);
+                        mbar_arrive_expect_tx(bar_k_full + 8 * s, K_TILE_BYTES);
+                        // a pair that overhangs the cache is zero-filled by TMA; its second block is never used
+                        tma_load_4d(k_smem + s * K_TILE_BYTES, &tm_k, bar_k_full + 8 * s, 0, (c * PF_CHUNK + 2 * pr) * 64,
+                                    hh * NSUB, b);
+                    }
                 ++n_item;
             }
         }
@@ -150,24 +169,39 @@ __global__ void __launch_bounds__(PF_THREADS, 1) score_prefill_kernel(const __gr
                 if (!decode_item(a, id, b, c, m, nk)) continue;
                 mbar_wait(bar_q_full, n_item & 1);
                 const int np = (nk + 1) >> 1;
-                for (int pr = 0; pr < np; ++pr, ++kp) {
-                    const int s = kp % PF_KSTAGES;
-                    mbar_wait(bar_k_full + 8 * s, (kp / PF_KSTAGES) & 1);
-                    const uint32_t ka = k_smem + s * K_TILE_BYTES;
+                for (int pr = 0; pr < np; ++pr) {
+                    int s = 0;
+                    uint32_t ka = 0;
+                    if constexpr (!Cfg::PER_HEAD) {
+                        s = kp % PF_KSTAGES;
+                        mbar_wait(bar_k_full + 8 * s, (kp / PF_KSTAGES) & 1);
+                        ka = k_smem + s * K_TILE_BYTES;
+                        ++kp;
+                    }
 #pragma unroll
                     for (int h = 0; h < PF_H; ++h, ++acc) {
+                        if constexpr (Cfg::PER_HEAD) {
+                            s = kp % PF_KSTAGES;
+                            mbar_wait(bar_k_full + 8 * s, (kp / PF_KSTAGES) & 1);
+                            ka = k_smem + s * K_TILE_BYTES;
+                            ++kp;
+                        }
                         const int ts = acc % PF_TSTAGES;
                         mbar_wait(bar_t_empty + 8 * ts, ((acc / PF_TSTAGES) & 1) ^ 1);
                         tc_fence_after();
 #pragma unroll
-                        for (int kk = 0; kk < PF_D / 16; ++kk) {
-                            const uint64_t ad = umma_desc_sw128(q_smem + h * (PF_M * PF_D * 2) + kk * 32);
-                            const uint64_t bd = umma_desc_sw128(ka + h * (PF_N * PF_D * 2) + kk * 32);
-                            umma_bf16_ss(tbase + ts * PF_N, ad, bd, idesc, kk > 0);
-                        }
+                        for (int sub = 0; sub < NSUB; ++sub)
+#pragma unroll
+                            for (int kk = 0; kk < 4; ++kk) {
+                                const uint64_t ad = umma_desc_sw128(q_smem + (h * NSUB + sub) * PF_PLANE_BYTES + kk * 32);
+                                const uint64_t bd = umma_desc_sw128(ka + ((Cfg::PER_HEAD ? 0 : h * NSUB) + sub) * PF_PLANE_BYTES
+                                                                    + kk * 32);
+                                umma_bf16_ss(tbase + ts * PF_N, ad, bd, idesc, (sub | kk) > 0);
+                            }
                         umma_commit(bar_t_full + 8 * ts);      // this head's accumulator is ready for the epilogue
+                        if constexpr (Cfg::PER_HEAD) umma_commit(bar_k_empty + 8 * s);
                     }
-                    umma_commit(bar_k_empty + 8 * s);          // smem slot free once these MMAs have read it
+                    if constexpr (!Cfg::PER_HEAD) umma_commit(bar_k_empty + 8 * s);   // slot free once these MMAs have read it
                 }
                 umma_commit(bar_q_empty);
                 ++n_item;
@@ -288,9 +322,11 @@ bool encode_tmap_bf16_sw128(CUtensorMap* out, const void* base, int rank, const 
 }
 
 // scores: fp32 [B * Tq/64][nb_stride]; entry (row, j) is written for every key block j the row's query block can see
-spot_status score_prefill(const spot_select_params* p, float* scores, int nb_stride, cudaStream_t s) {
-    if (p->fmt != SPOT_SELK_BF16) return SPOT_ERR_UNSUPPORTED;      // 4-bit prefill scoring: SURVEY 8(f) f2
-    if (p->H_idx != PF_H || p->d_idx != PF_D) return SPOT_ERR_UNSUPPORTED;
+template <int D>
+static spot_status score_prefill_d(const spot_select_params* p, float* scores, int nb_stride, cudaStream_t s) {
+    using Cfg = PfCfg<D>;
+    constexpr int PF_D = 64;                                        // plane width
+    constexpr int PLANES = PF_H * Cfg::NSUB;
     PrefillScoreArgs a;
     a.w = p->w; a.scores = scores; a.nb_stride = nb_stride;
     a.B = p->B; a.Tq = p->Tq; a.n_qb = p->Tq / 64; a.n_qt = (a.n_qb + 1) / 2;
@@ -302,25 +338,34 @@ spot_status score_prefill(const spot_select_params* p, float* scores, int nb_str
     a.total_ids = (int)total;
 
     CUtensorMap tm_q, tm_k;
-    const uint64_t row_bytes = (uint64_t)PF_H * PF_D * 2;
+    const uint64_t row_bytes = (uint64_t)PLANES * PF_D * 2;          // one token: [H][d_idx] = [PLANES][64]
     {
-        const uint64_t dims[4] = {(uint64_t)PF_D, (uint64_t)p->Tq, (uint64_t)PF_H, (uint64_t)p->B};
+        const uint64_t dims[4] = {(uint64_t)PF_D, (uint64_t)p->Tq, (uint64_t)PLANES, (uint64_t)p->B};
         const uint64_t strides[3] = {row_bytes, (uint64_t)PF_D * 2, (uint64_t)p->Tq * row_bytes};
-        const uint32_t box[4] = {(uint32_t)PF_D, (uint32_t)PF_M, (uint32_t)PF_H, 1u};
+        const uint32_t box[4] = {(uint32_t)PF_D, (uint32_t)PF_M, (uint32_t)PLANES, 1u};
         if (!encode_tmap_bf16_sw128(&tm_q, p->sel_q, 4, dims, strides, box)) return SPOT_ERR_CUDA;
     }
     {
-        const uint64_t dims[4] = {(uint64_t)PF_D, (uint64_t)p->cache_stride_tokens, (uint64_t)PF_H, (uint64_t)p->B};
+        const uint64_t dims[4] = {(uint64_t)PF_D, (uint64_t)p->cache_stride_tokens, (uint64_t)PLANES, (uint64_t)p->B};
         const uint64_t strides[3] = {row_bytes, (uint64_t)PF_D * 2, (uint64_t)p->cache_stride_tokens * row_bytes};
-        const uint32_t box[4] = {(uint32_t)PF_D, (uint32_t)PF_N, (uint32_t)PF_H, 1u};   // a pair of key blocks
+        // a pair of key blocks: every head's planes (d_idx 64) or one head's two planes (d_idx 128)
+        const uint32_t box[4] = {(uint32_t)PF_D, (uint32_t)PF_N, (uint32_t)(Cfg::PER_HEAD ? Cfg::NSUB : PLANES), 1u};
         if (!encode_tmap_bf16_sw128(&tm_k, p->sel_k, 4, dims, strides, box)) return SPOT_ERR_CUDA;
     }
     static unsigned long long smem_attr_done = 0;
-    SPOT_CUDA_TRY(set_max_smem_once(score_prefill_kernel, (int)PF_SMEM_BYTES, smem_attr_done));
+    SPOT_CUDA_TRY(set_max_smem_once(score_prefill_kernel<D>, (int)Cfg::SMEM_BYTES, smem_attr_done));
     const int grid = (int)(total < sm_count() ? total : sm_count());
-    SPOT_CUDA_TRY(launch_pdl(score_prefill_kernel, dim3((unsigned)grid), dim3(PF_THREADS), (size_t)PF_SMEM_BYTES, s, tm_q,
-                             tm_k, a));
+    SPOT_CUDA_TRY(launch_pdl(score_prefill_kernel<D>, dim3((unsigned)grid), dim3(PF_THREADS), (size_t)Cfg::SMEM_BYTES, s,
+                             tm_q, tm_k, a));
     return SPOT_OK;
+}
+
+spot_status score_prefill(const spot_select_params* p, float* scores, int nb_stride, cudaStream_t s) {
+    if (p->fmt != SPOT_SELK_BF16) return SPOT_ERR_UNSUPPORTED;      // quantised caches: dequantised by the caller (api.cu)
+    if (p->H_idx != PF_H) return SPOT_ERR_UNSUPPORTED;
+    if (p->d_idx == 64) return score_prefill_d<64>(p, scores, nb_stride, s);
+    if (p->d_idx == 128) return score_prefill_d<128>(p, scores, nb_stride, s);
+    return SPOT_ERR_UNSUPPORTED;
 }
 
 }  // namespace spot

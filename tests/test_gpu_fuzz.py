@@ -103,7 +103,9 @@ def test_fuzz_prefill(torch_cuda, chunk):
         if rng.random() < 0.25:
             over = dict(mode="topk", top_k=int(rng.integers(3, 12)), sink_blocks=1, recency_blocks=2)
         H_q = int(rng.choice([8, 32, 64]))
-        wls = [make_prefill_workload(seed=8000 + 13 * case + b, L=L, H_q=H_q, topic_span=int(rng.choice([64, 128, 256])))
+        d_idx = int(rng.choice([64, 128]))
+        wls = [make_prefill_workload(seed=8000 + 13 * case + b, L=L, H_q=H_q, d_idx=d_idx,
+                                     topic_span=int(rng.choice([64, 128, 256])))
                for b in range(B)]
         dp = H.DevicePrefill(wls, qb0 * 64, nqb * 64)
         fmt = str(rng.choice(["bf16", "bf16", "mxfp4", "fp8_e4m3"]))

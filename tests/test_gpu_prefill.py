@@ -102,6 +102,18 @@ def test_prefill_selection_over_a_quantised_cache(torch_cuda, fmt):
             np.testing.assert_allclose(got[b * dp.n_q + i, :len(s_bar)], s_bar, rtol=2e-5, atol=2e-5)
 
 
+@pytest.mark.parametrize("L,q_start,Tq,B", [(1024, 0, 1024, 1), (1024, 512, 320, 2), (4608, 0, 4608, 1), (1024, 256, 64, 1)])
+def test_prefill_selection_with_the_papers_selector_width(torch_cuda, L, q_start, Tq, B):
+    """d_idx = 128: a head is two 64-wide planes, the K ring is staged per head (4608 tokens: three
+    32-block chunks per query tile, many trips around the 3-stage ring)."""
+    wls = [_neg_weights(make_prefill_workload(seed=7007 + 7 * b, L=L, d_idx=128, with_kv=False), 50 + b) for b in range(B)]
+    dp = H.DevicePrefill(wls, q_start, Tq, with_kv=False)
+    report = []
+    _check_select_prefill(dp, report)
+    _check_select_prefill(dp, report, mode="topk", top_k=6)
+    print("prefill select d_idx=128 L=%d q_start=%d Tq=%d: near-tie rows %s" % (L, q_start, Tq, report[:4]))
+
+
 def _check_attn_prefill(dp, lists_per_seq, want_lse=False):
     """lists_per_seq[b][i] = selected key blocks of query block i of sequence b (the oracle's lists on both sides)."""
     wl = dp.wl
