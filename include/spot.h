@@ -157,6 +157,10 @@ spot_status spot_selector_project_append(const spot_project_params* p, void* str
  * cap must be >= the largest budget any row can reach (>= min(n_b, what the mode allows)); a row whose
  * budget would exceed cap makes the call fail up front when detectable on the host (cap < max n_b for
  * DUAL_TOPP, cap < min(top_k, max n_b) for TOPK) with SPOT_ERR_INVALID_ARG.
+ *
+ * Supported selector geometries: H_idx == 4 with d_idx == 64 or 128 (anything else: SPOT_ERR_UNSUPPORTED), every cache
+ * format in both row forms.  Prefill rows over a quantised cache dequantise the visible prefix into the workspace
+ * first (spot_select_workspace_bytes accounts for it).
  * --------------------------------------------------------------------------------------------------- */
 typedef struct {
     /* inputs */

@@ -129,7 +129,7 @@ extern "C" const char* spot_status_string(spot_status s) {
 }
 
 extern "C" int spot_last_cuda_error(void) { return g_last_cuda_error; }
-extern "C" const char* spot_version(void) { return "0.1"; }
+extern "C" const char* spot_version(void) { return "0.2"; }
 extern "C" size_t spot_struct_size(int which) {
     switch (which) {
         case 0: return sizeof(spot_select_params);
