@@ -536,8 +536,16 @@ def run_prefill(args):
                                 block_scores=scores, nb_stride=nb_stride)
     ws = torch.empty(max(16, api.spot_select_workspace_bytes(sp)), dtype=torch.uint8, device=dev)
     sp.workspace, sp.workspace_bytes = ws.data_ptr(), ws.numel()
-    ap = api.make_attn_params(Q, K, V, (Hkv * L * D, D, L * D), None, 0, indices, budgets, cap, 1, L, Hq, Hkv, D,
-                              q_start=0, blk=64, sm_scale=wl.sm_scale, out=out)
+    kv_strides, paging = (Hkv * L * D, D, L * D), {}
+    if args.paged:
+        # the same bytes read as a page pool [page][H_kv][page_tokens][D] behind a random page table (f3, R32)
+        pt = max(args.paged, 64)
+        gen_t = torch.Generator(device=dev)
+        gen_t.manual_seed(wl.seed + 23)
+        table = torch.randperm(L // pt, generator=gen_t, device=dev).to(torch.int32).reshape(1, L // pt)
+        kv_strides, paging = (Hkv * pt * D, D, pt * D), dict(page_table=table, page_tokens=pt)
+    ap = api.make_attn_params(Q, K, V, kv_strides, None, 0, indices, budgets, cap, 1, L, Hq, Hkv, D,
+                              q_start=0, blk=64, sm_scale=wl.sm_scale, out=out, **paging)
     stream = torch.cuda.current_stream()
     flush = torch.empty(512 << 20, dtype=torch.uint8, device=dev).zero_()
 
@@ -586,8 +594,8 @@ def run_prefill(args):
     att_ms = np.array([e[1].elapsed_time(e[2]) for e in ev])
     step_ms = np.array([e[0].elapsed_time(e[2]) for e in ev])
     # dense causal comparator (indices NULL) -- a few iterations only
-    apd = api.make_attn_params(Q, K, V, (Hkv * L * D, D, L * D), None, 0, None, None, 0, 1, L, Hq, Hkv, D,
-                               q_start=0, blk=64, sm_scale=wl.sm_scale, out=out)
+    apd = api.make_attn_params(Q, K, V, kv_strides, None, 0, None, None, 0, 1, L, Hq, Hkv, D,
+                               q_start=0, blk=64, sm_scale=wl.sm_scale, out=out, **paging)
     den = []
     for i in range(3):
         a_, b_ = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
@@ -646,7 +654,8 @@ def run_prefill(args):
         "warmup": W, "ms_per_step": step_mean, "higher_is_better": False, "scaling": "weak", "vs_baseline": None,
         "dtype": "bf16", "data": "synthetic",
         "config": {"workload": "cfg5", "B": 1, "L": L, "H_q": Hq, "H_kv": Hkv, "D": D,
-                   "selector": "%dx%d %s" % (wl.H_idx, wl.d_idx, args.fmt), "blk": 64, "q_block": 64, "mode": wl.mode, "p": args.p,
+                   "selector": "%dx%d %s" % (wl.H_idx, wl.d_idx, args.fmt), "blk": 64, "q_block": 64,
+                   "kv_layout": ("paged, %d tokens per page, random table" % max(args.paged, 64)) if args.paged else "[B][H_kv][L][D]", "mode": wl.mode, "p": args.p,
                    "sink/recency/kmin": [wl.sink_blocks, wl.recency_blocks, wl.kmin_blocks],
                    "mean_budget": float(bud_host.mean()), "density": float(bud_host.sum()) / tiles,
                    "l2": "flushed by a 512 MiB read sweep before every timed step"},
@@ -685,7 +694,7 @@ def main():
     ap.add_argument("--d-idx", type=int, default=0, choices=[0, 64, 128],
                     help="selector head dim (default: the config's 64; 128 = the paper's geometry, PAPER.md:363)")
     ap.add_argument("--paged", type=int, default=0, choices=[0, 16, 64, 256],
-                    help="decode only: K/V as a page pool of this many tokens per page behind a random page table")
+                    help="K/V as a page pool of this many tokens per page behind a random page table (prefill: >= 64)")
     ap.add_argument("--blk", type=int, default=64, choices=[64, 16],
                     help="decode only: selection block size (16 = the paper's geometry with its 8/16/32 reserved "
                          "sink/recency/K_min blocks, PAPER.md:362-365, :400-402)")

@@ -237,12 +237,12 @@ typedef struct {
     float* lse;                  /* optional                                                              */
     void* workspace;
     size_t workspace_bytes;
-    /* Paged K/V (decode calls only; f3, R32).  page_table == NULL: contiguous caches as described above.
+    /* Paged K/V (f3, R32).  page_table == NULL: contiguous caches as described above.
      * Otherwise k and v are page POOLS: logical token t of sequence b is row t % page_tokens of physical page
      * page_table[b * page_table_stride + t / page_tokens]; kv_stride_batch is then the element stride between
      * PAGES (a multiple of kv_stride_token), kv_stride_token / kv_stride_head apply inside a page.  page_tokens is a
-     * multiple of 16.  Entries for logical pages at or past ceil(seq_len[b] / page_tokens) are never read.  The
-     * prefill call returns SPOT_ERR_UNSUPPORTED when page_table is set. */
+     * multiple of 16 (prefill: of 64, a key block must sit inside one page; SPOT_ERR_UNSUPPORTED otherwise).  Entries
+     * for logical pages at or past ceil(seq_len[b] / page_tokens) (prefill: past q_start + Tq) are never read. */
     const int32_t* page_table;   /* device, int32 [B][page_table_stride]                                  */
     int32_t page_table_stride;
     int32_t page_tokens;

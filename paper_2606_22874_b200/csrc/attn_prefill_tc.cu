@@ -44,6 +44,8 @@ constexpr float TA_RESCALE_THRESHOLD = 8.0f;           // log2 units
 
 struct TcAttnArgs {
     const int32_t* indices;      // [B * n_qb][cap]; nullptr: every causally visible block
+    const int32_t* page_table;   // nullptr: contiguous K/V; else page pools (f3, R32): [B][pt_stride] physical pages
+    int pt_stride, page_tokens;  // page_tokens % 64 == 0: a 64-token block never straddles pages
     const int32_t* budgets;
     int cap;
     int Tq, n_qb, H_q, H_kv, G;
@@ -111,6 +113,18 @@ __global__ void __launch_bounds__(TA_THREADS, 1) attn_prefill_tc_kernel(const __
     const int32_t* idx = a.indices ? a.indices + (int64_t)rowz * a.cap : nullptr;
     auto block_of = [&](int it) -> int { return idx ? idx[it] : it; };
     auto visible = [&](int j) -> bool { return j >= 0 && j <= qb_abs; };
+    // where key block j lives: (token coordinate, outermost coordinate) of the K / V tensor maps -- (64 j, b) for
+    // contiguous caches, (offset inside the page, physical page) for page pools
+    const int32_t* ptab = a.page_table ? a.page_table + (int64_t)b * a.pt_stride : nullptr;
+    auto place = [&](int j, int& tok, int& outer) {
+        tok = j * 64;
+        outer = b;
+        if (ptab) {
+            const int lp = tok / a.page_tokens;
+            outer = ptab[lp];
+            tok -= lp * a.page_tokens;
+        }
+    };
 
     if (warp == 0) {
         // ================================ TMA producer ================================
@@ -126,6 +140,10 @@ __global__ void __launch_bounds__(TA_THREADS, 1) attn_prefill_tc_kernel(const __
                 for (; it < budget && jA < 0; ++it) { const int j = block_of(it); if (visible(j)) jA = j; }
                 if (jA < 0) break;
                 for (; it < budget && jB < 0; ++it) { const int j = block_of(it); if (visible(j)) jB = j; }
+                // (the page-table lookups are issued before the wait for the ring slot, which hides them)
+                int tok[2] = {0, 0}, outer[2] = {0, 0};
+                place(jA, tok[0], outer[0]);
+                if (jB >= 0) place(jB, tok[1], outer[1]);
                 const int s = n % TA_STAGES;
                 mbar_wait(bar_kv_empty + 8 * s, ((n / TA_STAGES) & 1) ^ 1);
                 const uint32_t ks = kv_smem + s * 2 * TA_KV_TILE;
@@ -133,13 +151,13 @@ __global__ void __launch_bounds__(TA_THREADS, 1) attn_prefill_tc_kernel(const __
                 mbar_arrive_expect_tx(bar_k_full + 8 * s, bytes);
                 for (int u = 0; u < (jB >= 0 ? 2 : 1); ++u)
                     for (int hf = 0; hf < 2; ++hf)
-                        tma_load_5d(ks + hf * (128 * 128) + u * (64 * 128), &tm_k, bar_k_full + 8 * s, 0, (u ? jB : jA) * 64,
-                                    hf, hk, b);
+                        tma_load_5d(ks + hf * (128 * 128) + u * (64 * 128), &tm_k, bar_k_full + 8 * s, 0, tok[u], hf, hk,
+                                    outer[u]);
                 mbar_arrive_expect_tx(bar_v_full + 8 * s, bytes);
                 for (int u = 0; u < (jB >= 0 ? 2 : 1); ++u)
                     for (int hf = 0; hf < 2; ++hf)
                         tma_load_5d(ks + TA_KV_TILE + hf * (128 * 128) + u * (64 * 128), &tm_v, bar_v_full + 8 * s, 0,
-                                    (u ? jB : jA) * 64, hf, hk, b);
+                                    tok[u], hf, hk, outer[u]);
                 ++n;
             }
         }
@@ -400,12 +418,16 @@ spot_status attn_prefill_tc(const spot_attn_params* p, cudaStream_t stream) {
         const uint32_t box[5] = {64, 64, 2, 2, 1};       // -> [half][head][query][128 B] = [half][128 rows][128 B]
         if (!encode_tmap_bf16_sw128(&tm_q, p->q, 5, dims, strides, box)) return SPOT_ERR_CUDA;
     }
-    const uint64_t n_tok = (uint64_t)p->q_start + p->Tq;
+    // contiguous caches: (.., token < q_start + Tq, .., head, batch); page pools: (.., token inside a page, .., head,
+    // page) -- the pool's size is not part of the ABI, the page coordinate is bounded by what 2^22 pages would hold
+    a.page_table = p->page_table; a.pt_stride = p->page_table_stride; a.page_tokens = p->page_tokens;
+    const uint64_t n_tok = p->page_table ? (uint64_t)p->page_tokens : (uint64_t)p->q_start + p->Tq;
+    const uint64_t n_outer = p->page_table ? ((uint64_t)1 << 22) : (uint64_t)p->B;
     if (!make_map(&tm_k, p->k, n_tok, (uint64_t)p->kv_stride_token, (uint64_t)p->H_kv, (uint64_t)p->kv_stride_head,
-                  (uint64_t)p->B, (uint64_t)p->kv_stride_batch, 64, 1))
+                  n_outer, (uint64_t)p->kv_stride_batch, 64, 1))
         return SPOT_ERR_CUDA;
     if (!make_map(&tm_v, p->v, n_tok, (uint64_t)p->kv_stride_token, (uint64_t)p->H_kv, (uint64_t)p->kv_stride_head,
-                  (uint64_t)p->B, (uint64_t)p->kv_stride_batch, 64, 1))
+                  n_outer, (uint64_t)p->kv_stride_batch, 64, 1))
         return SPOT_ERR_CUDA;
     static unsigned long long smem_attr_done = 0;
     SPOT_CUDA_TRY(set_max_smem_once(attn_prefill_tc_kernel, (int)TA_SMEM_BYTES, smem_attr_done));

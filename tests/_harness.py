@@ -219,7 +219,8 @@ class DevicePrefill:
         bud = torch.from_numpy(np.ascontiguousarray(budgets_np, dtype=np.int32)).cuda()
         ap = api.make_attn_params(self.Q, self.K, self.V, self.kv_strides, None, 0, idx, bud, idx.shape[1], self.B,
                                   self.Tq, wl.H_q, wl.H_kv, wl.D, q_start=self.q_start, blk=wl.blk,
-                                  sm_scale=wl.sm_scale, out=out, lse=lse)
+                                  sm_scale=wl.sm_scale, out=out, lse=lse, page_table=getattr(self, "page_table", None),
+                                  page_tokens=getattr(self, "page_tokens", 0))
         ws = torch.empty(max(api.spot_sparse_attn_prefill_workspace_bytes(ap), 16), dtype=torch.uint8, device="cuda")
         ap.workspace, ap.workspace_bytes = ws.data_ptr(), ws.numel()
         api.spot_sparse_attn_prefill(ap)

@@ -138,7 +138,9 @@ def test_attention_argument_errors_are_caught_on_the_host(lib):
     assert lib.spot_sparse_attn_decode_workspace_bytes(C.byref(_attn_params(**paged))) > 0
     for o in (dict(page_tokens=0), dict(page_tokens=40), dict(page_table_stride=63), dict(kv_stride_batch=8 * 64 * 128 + 8)):
         assert lib.spot_sparse_attn_decode(C.byref(_attn_params(**dict(paged, **o))), None) == INVALID, o
-    assert lib.spot_sparse_attn_prefill(C.byref(_attn_params(Tq=64, **paged)), None) == UNSUPPORTED
+    assert lib.spot_sparse_attn_prefill_workspace_bytes(C.byref(_attn_params(Tq=64, **paged))) >= 0
+    assert lib.spot_sparse_attn_prefill(C.byref(_attn_params(Tq=64, **dict(paged, page_tokens=32))), None) == UNSUPPORTED
+    assert lib.spot_sparse_attn_prefill(C.byref(_attn_params(Tq=128, q_start=4096, **paged)), None) == INVALID   # table too short
     assert lib.spot_decode_step_host(None, None) == INVALID
 
 

@@ -265,3 +265,42 @@ def test_full_size_cfg5_in_the_bench_configuration(torch_cuda):
         err = np.abs(got - want)
         assert err.max() <= MAX_ABS and err.mean() <= MEAN_ABS, (i, err.max(), err.mean())
         print("cfg5 query block %d: attention over %d blocks, max-abs %.2e mean-abs %.2e" % (i, n, err.max(), err.mean()))
+
+
+@pytest.mark.parametrize("page_tokens,layout", [(64, "phd"), (128, "pthd"), (256, "phd")])
+def test_prefill_attention_over_paged_kv(torch_cuda, page_tokens, layout):
+    """f3 / R32: K/V in a page pool shared by the batch behind a per-sequence page table (pages placed at random,
+    finite garbage in the unused ones); the oracle reads the pool back through the table and attends as usual."""
+    torch = torch_cuda
+    from oracle import attention as OA
+    L, q_start, Tq, B = 1024, 512, 320, 2
+    wls = [make_prefill_workload(seed=9100 + 11 * b, L=L) for b in range(B)]
+    dp = H.DevicePrefill(wls, q_start, Tq)
+    wl = dp.wl
+    pt, Hkv, D = page_tokens, wl.H_kv, wl.D
+    n_log = L // pt
+    rng = np.random.default_rng(41)
+    n_pages = B * n_log + 5
+    table = rng.permutation(n_pages)[:B * n_log].reshape(B, n_log).astype(np.int32)
+    poolK = rng.integers(0, 1 << 16, size=(n_pages, pt, Hkv, D), dtype=np.uint16) & 0x3fff
+    poolV = rng.integers(0, 1 << 16, size=(n_pages, pt, Hkv, D), dtype=np.uint16) & 0x3fff
+    for b, w in enumerate(wls):
+        Kb, Vb = w.K.transpose(1, 0, 2), w.V.transpose(1, 0, 2)                      # [L][H_kv][D]
+        for lp in range(n_log):
+            poolK[table[b, lp]] = Kb[lp * pt:(lp + 1) * pt]
+            poolV[table[b, lp]] = Vb[lp * pt:(lp + 1) * pt]
+        assert np.array_equal(OA.gather_paged_kv(poolK, table[b], L, pt), Kb)
+        assert np.array_equal(OA.gather_paged_kv(poolV, table[b], L, pt), Vb)
+    if layout == "phd":          # [page][H_kv][page_tokens][D]
+        dp.K = H.dev_u16(np.ascontiguousarray(poolK.transpose(0, 2, 1, 3)))
+        dp.V = H.dev_u16(np.ascontiguousarray(poolV.transpose(0, 2, 1, 3)))
+        dp.kv_strides = (Hkv * pt * D, D, pt * D)
+    else:                        # [page][page_tokens][H_kv][D]
+        dp.K, dp.V = H.dev_u16(poolK), H.dev_u16(poolV)
+        dp.kv_strides = (pt * Hkv * D, Hkv * D, D)
+    dp.page_table = torch.from_numpy(table).cuda()
+    dp.page_tokens = pt
+    lists = [[sel.indices.tolist() for _, sel in H.oracle_select_prefill(w, q_start, Tq)] for w in wls]
+    _check_attn_prefill(dp, lists)
+    dense = [[list(range((q_start + 64 * i) // 64 + 1)) for i in range(Tq // 64)] for _ in wls]
+    _check_attn_prefill(dp, dense)
