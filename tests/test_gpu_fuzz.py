@@ -114,5 +114,22 @@ def test_fuzz_prefill(torch_cuda, chunk):
         report = []
         _check_select_prefill(dp, report, **over)
         lists = [[sel.indices.tolist() for _, sel in H.oracle_select_prefill(w, dp.q_start, dp.Tq, **over)] for w in wls]
+        paged = rng.random() < 0.4
+        if paged:                                        # K/V as a page pool [page][H_kv][page_tokens][D]
+            import torch
+            pt = int(rng.choice([64, 128]))
+            n_log = L // pt
+            table = rng.permutation(B * n_log + 2)[:B * n_log].reshape(B, n_log).astype(np.int32)
+            wl0 = wls[0]
+            poolK = np.zeros((B * n_log + 2, wl0.H_kv, pt, wl0.D), dtype=np.uint16)
+            poolV = np.zeros_like(poolK)
+            for b, w in enumerate(wls):
+                for lp in range(n_log):
+                    poolK[table[b, lp]] = w.K[:, lp * pt:(lp + 1) * pt]
+                    poolV[table[b, lp]] = w.V[:, lp * pt:(lp + 1) * pt]
+            dp.K, dp.V = H.dev_u16(poolK), H.dev_u16(poolV)
+            dp.kv_strides = (wl0.H_kv * pt * wl0.D, wl0.D, pt * wl0.D)
+            dp.page_table, dp.page_tokens = torch.from_numpy(table).cuda(), pt
         _check_attn_prefill(dp, lists)
-        print("fuzz prefill case %d: L=%d q_start=%d Tq=%d B=%d H_q=%d %s near-ties %s" % (case, L, dp.q_start, dp.Tq, B, H_q, fmt, report))
+        print("fuzz prefill case %d: L=%d q_start=%d Tq=%d B=%d H_q=%d d_idx=%d %s%s near-ties %s"
+              % (case, L, dp.q_start, dp.Tq, B, H_q, d_idx, fmt, " paged" if paged else "", report))
