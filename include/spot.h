@@ -242,7 +242,8 @@ typedef struct {
      * page_table[b * page_table_stride + t / page_tokens]; kv_stride_batch is then the element stride between
      * PAGES (a multiple of kv_stride_token), kv_stride_token / kv_stride_head apply inside a page.  page_tokens is a
      * multiple of 16 (prefill: of 64, a key block must sit inside one page; SPOT_ERR_UNSUPPORTED otherwise).  Entries
-     * for logical pages at or past ceil(seq_len[b] / page_tokens) (prefill: past q_start + Tq) are never read. */
+     * for logical pages at or past ceil(seq_len[b] / page_tokens) (prefill: past q_start + Tq) are never read.  Page
+     * numbers are < 2^22. */
     const int32_t* page_table;   /* device, int32 [B][page_table_stride]                                  */
     int32_t page_table_stride;
     int32_t page_tokens;
