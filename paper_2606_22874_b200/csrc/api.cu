@@ -37,6 +37,7 @@ spot_status score_decode(const spot_select_params* p, float* scores, int nb_stri
 spot_status score_prefill(const spot_select_params* p, float* scores, int nb_stride, cudaStream_t s);
 spot_status run_select(const spot_select_params* p, const float* scores, int nb_stride, int rows_per_seq, int max_nb,
                        cudaStream_t s);
+spot_status check_attn_decode_args(const spot_attn_params* p);     // attn_decode.cu: the host-side checks of a3
 
 namespace {
 
@@ -142,7 +143,8 @@ extern "C" size_t spot_struct_size(int which) {
 
 extern "C" size_t spot_select_workspace_bytes(const spot_select_params* p) {
     SelectGeom g;
-    if (select_geometry(p, &g) != SPOT_OK) return 0;
+    // a block without an index list is a spot_score_blocks block (it ignores indices / budgets / cap): size it as such
+    if (!p || select_geometry(p, &g, /*score_only=*/!p->indices) != SPOT_OK) return 0;
     size_t bytes = 256;
     if (g.own_scores) bytes += (size_t)p->B * g.rows_per_seq * g.nb_stride * sizeof(float);
     return bytes + prefill_scratch_bytes(p);
@@ -181,6 +183,21 @@ extern "C" spot_status spot_decode_step_host(const spot_decode_step_host_params*
     const spot_select_params& sp = p->select;
     const spot_attn_params& ap = p->attn;
     if (sp.q_block != 1 || sp.B != ap.B) return SPOT_ERR_INVALID_ARG;
+    // every argument check of the two calls runs before the first copy is enqueued
+    {
+        SelectGeom g;
+        spot_status st0 = select_geometry(&sp, &g);
+        if (st0 != SPOT_OK) return st0;
+        if ((st0 = check_attn_decode_args(&ap)) != SPOT_OK) return st0;
+        if ((st0 = check_device()) != SPOT_OK) return st0;
+        // the *_host buffers must be page-locked: a pageable cudaMemcpyAsync blocks the host and cannot be captured
+        const void* hosts[5] = {p->sel_q_host, p->w_host, p->q_host, p->out_host, p->budgets_host};
+        for (const void* h : hosts) {
+            cudaPointerAttributes at;
+            if (cudaPointerGetAttributes(&at, h) != cudaSuccess) { cudaGetLastError(); return SPOT_ERR_INVALID_ARG; }
+            if (at.type != cudaMemoryTypeHost && at.type != cudaMemoryTypeManaged) return SPOT_ERR_INVALID_ARG;
+        }
+    }
     cudaStream_t s = (cudaStream_t)stream;
     const size_t n_selq = (size_t)sp.B * sp.H_idx * sp.d_idx * 2, n_w = (size_t)sp.B * sp.H_idx * 4;
     const size_t n_q = (size_t)ap.B * ap.H_q * ap.D * 2;

@@ -37,6 +37,7 @@ struct AttnArgs {
     const uint16_t* v;
     int64_t sb, st, sh;          // element strides: batch, token, head
     const int32_t* seq_len;
+    int max_len;                 // host-side bound of seq_len: device values are clamped to [0, max_len]
     const int32_t* indices;      // nullptr: dense
     const int32_t* budgets;
     int cap;
@@ -52,12 +53,13 @@ struct AttnArgs {
     float* lse;
 };
 
+__device__ __forceinline__ int seq_len_of(const AttnArgs& a, int b) { return min(max(a.seq_len[b], 0), a.max_len); }
 // list entries of sequence b (sparse form)
 __device__ __forceinline__ int seq_entries(const AttnArgs& a, int b) { return max(0, min(a.budgets[b], a.cap)); }
 // units of sequence b per KV head: 64 tokens each -- a selected 64-token block, four selected 16-token blocks (the
 // last unit of a list may be short), or a 64-token stretch of the whole sequence (dense)
 __device__ __forceinline__ int seq_blocks(const AttnArgs& a, int b) {
-    if (!a.indices) return (a.seq_len[b] + 63) >> 6;
+    if (!a.indices) return (seq_len_of(a, b) + 63) >> 6;
     const int n = seq_entries(a, b);
     return a.fine ? (n + 3) >> 2 : n;
 }
@@ -110,7 +112,7 @@ __global__ void __launch_bounds__(ATT_WARPS * 32, 2) attn_decode_kernel(AttnArgs
         const int jend = (int)min((long long)nb, (long long)jbeg + (u1 - u));
         const int n_it = jend - jbeg;
         if (n_it > 0) {
-            const int L = a.seq_len[b];
+            const int L = seq_len_of(a, b);
             // Q fragments (A operand): rows = query heads of this KV group, zero-padded to 16.
             uint32_t qa[8][4];
             {
@@ -403,7 +405,7 @@ spot_status run_decode(const spot_attn_params* p, bool dense, cudaStream_t s) {
     AttnArgs a;
     a.q = p->q; a.k = p->k; a.v = p->v;
     a.sb = p->kv_stride_batch; a.st = p->kv_stride_token; a.sh = p->kv_stride_head;
-    a.seq_len = p->seq_len; a.indices = use_idx ? p->indices : nullptr; a.budgets = p->budgets; a.cap = p->cap;
+    a.seq_len = p->seq_len; a.max_len = p->max_seq_len; a.indices = use_idx ? p->indices : nullptr; a.budgets = p->budgets; a.cap = p->cap;
     a.fine = use_idx && p->blk == 16;
     a.page_table = p->page_table; a.pt_stride = p->page_table_stride; a.page_tokens = p->page_tokens;
     a.page_vtok = p->page_table ? (int)(p->kv_stride_batch / p->kv_stride_token) : 0;
@@ -423,6 +425,8 @@ spot_status run_decode(const spot_attn_params* p, bool dense, cudaStream_t s) {
 }
 
 }  // namespace
+
+spot_status check_attn_decode_args(const spot_attn_params* p) { return check_attn(p, false, false); }
 
 }  // namespace spot
 

@@ -24,7 +24,6 @@ spot_status check_prefill(const spot_attn_params* p) {
     if (p->kv_stride_token < p->D || p->kv_stride_token % 8 || p->kv_stride_head % 8 || p->kv_stride_batch % 8)
         return SPOT_ERR_INVALID_ARG;
     if (p->indices && (!p->budgets || p->cap <= 0)) return SPOT_ERR_INVALID_ARG;
-    if ((int64_t)p->B * (p->Tq / 64) > 65535) return SPOT_ERR_UNSUPPORTED;
     return SPOT_OK;
 }
 

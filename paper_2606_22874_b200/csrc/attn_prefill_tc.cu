@@ -49,6 +49,7 @@ struct TcAttnArgs {
     const int32_t* budgets;
     int cap;
     int Tq, n_qb, H_q, H_kv, G;
+    int n_pairs, n_rows;         // grid.x = n_rows * n_pairs: pairs of 128-row tiles per (row, KV head); rows = B * n_qb
     int qb_start;                // q_start / 64
     float scale_log2;
     uint16_t* out;               // [B][Tq][H_q][128]
@@ -77,8 +78,9 @@ __global__ void __launch_bounds__(TA_THREADS, 1) attn_prefill_tc_kernel(const __
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     // launch order: x (tile pair) fastest, then y (query block, heaviest = latest first), KV head slowest -- the CTAs in
     // flight at any time share ONE head's K/V (32 MiB at L = 64K, L2-resident) instead of all eight heads' (256 MiB)
-    const int pair = blockIdx.x, hk = blockIdx.z;
-    const int rowz = (int)gridDim.y - 1 - (int)blockIdx.y;
+    // (tile pair and row share blockIdx.x -- up to 2^31 - 1 -- so that B * Tq / 64 is not bound by the 65535 of y / z)
+    const int pair = (int)(blockIdx.x % (unsigned)a.n_pairs), hk = blockIdx.z;
+    const int rowz = a.n_rows - 1 - (int)(blockIdx.x / (unsigned)a.n_pairs);
     const int b = rowz / a.n_qb, i = rowz - b * a.n_qb;
     const int G = a.G;
     const int qb_abs = a.qb_start + i;
@@ -432,7 +434,10 @@ spot_status attn_prefill_tc(const spot_attn_params* p, cudaStream_t stream) {
     static unsigned long long smem_attr_done = 0;
     SPOT_CUDA_TRY(set_max_smem_once(attn_prefill_tc_kernel, (int)TA_SMEM_BYTES, smem_attr_done));
     const int n_mt = (a.G * 64 + 127) / 128;
-    dim3 grid((unsigned)((n_mt + 1) / 2), (unsigned)(p->B * a.n_qb), (unsigned)p->H_kv);
+    a.n_pairs = (n_mt + 1) / 2;
+    a.n_rows = p->B * a.n_qb;
+    if ((int64_t)a.n_pairs * a.n_rows > 0x7fffffff || p->H_kv > 65535) return SPOT_ERR_UNSUPPORTED;
+    dim3 grid((unsigned)(a.n_pairs * a.n_rows), 1u, (unsigned)p->H_kv);
     SPOT_CUDA_TRY(launch_pdl(attn_prefill_tc_kernel, grid, dim3(TA_THREADS), (size_t)TA_SMEM_BYTES, stream, tm_q, tm_k,
                              tm_v, a));
     return SPOT_OK;

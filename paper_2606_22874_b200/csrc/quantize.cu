@@ -19,7 +19,7 @@ namespace {
 __device__ __forceinline__ uint32_t e2m1x2_from_f32(float lo, float hi) {
     // cvt.rn.satfinite.e2m1x2.f32 d, a, b : a -> upper nibble, b -> lower nibble.  RNE on the E2M1 grid,
     // saturating at +-6, keeps the sign of a zero result (R16; checked bit-for-bit against the
-    // oracle's threshold table in tests/test_gpu_quantize.py, ties included).
+    // oracle's threshold table in tests/test_gpu_decode.py::test_quantise_dequantise_bit_exact, ties included).
     uint32_t r;
     asm("{ .reg .b8 t; cvt.rn.satfinite.e2m1x2.f32 t, %1, %2; cvt.u32.u8 %0, t; }" : "=r"(r) : "f"(hi), "f"(lo));
     return r;

@@ -143,18 +143,22 @@ struct ScoreArgs {
     const uint8_t* sel_k;         // 4-bit formats: the cache; BF16: unused (the tensor map carries the address)
     int64_t tiles_per_seq;        // 4-bit formats: cache_stride_tokens / 64
     const int32_t* seq_len;
+    int max_len;                  // host-side bound of seq_len: device values are clamped to [0, max_len]
     int B;
     float* scores;
     int nb_stride;
     int fine;                     // blk == 16: four block maxima per 64-token tile (f3)
 };
 
+// seq_len[b] as the kernels use it: clamped to what the grid, the score rows and the cache were sized for
+__device__ __forceinline__ int seq_len_of(const ScoreArgs& a, int b) { return min(max(a.seq_len[b], 0), a.max_len); }
+
 // (sequence, tile) cursor over the flat tile list
 struct TileCursor {
     int b, t, nb;
     __device__ __forceinline__ void advance(const ScoreArgs& a, int n) {
         t += n;
-        while (t >= nb && b + 1 < a.B) { t -= nb; ++b; nb = (a.seq_len[b] + 63) >> 6; }
+        while (t >= nb && b + 1 < a.B) { t -= nb; ++b; nb = (seq_len_of(a, b) + 63) >> 6; }
     }
 };
 
@@ -495,15 +499,15 @@ __global__ void __launch_bounds__((ScoreCfg<H, D_IDX, FMT>::THREADS), 1) score_d
 
     // this CTA's range of the flat (sequence, tile) list
     long long total = 0;
-    for (int bb = 0; bb < a.B; ++bb) total += (a.seq_len[bb] + 63) >> 6;
+    for (int bb = 0; bb < a.B; ++bb) total += (seq_len_of(a, bb) + 63) >> 6;
     const long long i0 = (long long)blockIdx.x * total / gridDim.x, i1 = (long long)(blockIdx.x + 1) * total / gridDim.x;
     const int n_my = (int)(i1 - i0);
     if (n_my <= 0) return;
     TileCursor cur;
-    cur.b = 0; cur.nb = (a.seq_len[0] + 63) >> 6; cur.t = 0;
+    cur.b = 0; cur.nb = (seq_len_of(a, 0) + 63) >> 6; cur.t = 0;
     {
         long long rem = i0;                       // (64-bit while locating the start only)
-        while (rem >= cur.nb && cur.b + 1 < a.B) { rem -= cur.nb; ++cur.b; cur.nb = (a.seq_len[cur.b] + 63) >> 6; }
+        while (rem >= cur.nb && cur.b + 1 < a.B) { rem -= cur.nb; ++cur.b; cur.nb = (seq_len_of(a, cur.b) + 63) >> 6; }
         cur.t = (int)rem;
     }
 
@@ -546,7 +550,7 @@ __global__ void __launch_bounds__((ScoreCfg<H, D_IDX, FMT>::THREADS), 1) score_d
         for (int j = 0; j < n_w; ++j) {
             if (cur.b != cur_b) {
                 cur_b = cur.b;
-                L = a.seq_len[cur_b];
+                L = seq_len_of(a, cur_b);
                 tile.load_query(a, cur_b, lane, q16_base + warp * (Cfg::ROW * 2 + 64));
             }
             float m = -INFINITY;
@@ -587,7 +591,7 @@ __global__ void __launch_bounds__((ScoreCfg<H, D_IDX, FMT>::THREADS), 1) score_d
         for (int i = warp; i < n_my; i += SC_CONSUMERS) {
             if (cur.b != cur_b) {
                 cur_b = cur.b;
-                L = a.seq_len[cur_b];
+                L = seq_len_of(a, cur_b);
                 tile.load_query(a, cur_b, lane, q16_base + warp * (Cfg::ROW * 2 + 64));
             }
             const int s = i % NS;
@@ -606,7 +610,7 @@ spot_status launch_score_fmt(const spot_select_params* p, float* scores, int nb_
     using Cfg = ScoreCfg<H, D_IDX, FMT>;
     ScoreArgs a;
     a.sel_q = p->sel_q; a.w = p->w; a.sel_k = (const uint8_t*)p->sel_k; a.tiles_per_seq = p->cache_stride_tokens / 64;
-    a.seq_len = p->seq_len; a.B = p->B; a.scores = scores; a.nb_stride = nb_stride; a.fine = p->blk == 16;
+    a.seq_len = p->seq_len; a.max_len = p->max_seq_len; a.B = p->B; a.scores = scores; a.nb_stride = nb_stride; a.fine = p->blk == 16;
     CUtensorMap tm;
     memset(&tm, 0, sizeof(tm));
     if (FMT == SPOT_SELK_BF16) {

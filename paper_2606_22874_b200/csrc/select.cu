@@ -14,7 +14,7 @@ spot_status run_select(const spot_select_params* p, const float* scores, int nb_
                        int max_nb, cudaStream_t s) {
     if (max_nb > SEL_MAX_NB) return SPOT_ERR_UNSUPPORTED;
     SelectArgs a;
-    a.scores = scores; a.nb_stride = nb_stride; a.seq_len = p->seq_len; a.n_q = rows_per_seq;
+    a.scores = scores; a.nb_stride = nb_stride; a.seq_len = p->seq_len; a.max_len = p->max_seq_len; a.n_q = rows_per_seq;
     a.q_start = p->q_start; a.q_block = p->q_block; a.blk = p->blk;
     a.mode = p->mode; a.top_k = p->top_k; a.p = p->p; a.temperature = p->temperature;
     a.sink = p->sink_blocks; a.rec = p->recency_blocks; a.kmin = p->kmin_blocks;

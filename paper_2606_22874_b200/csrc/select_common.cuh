@@ -23,6 +23,7 @@ struct SelectArgs {
     const float* scores;      // [rows][nb_stride]
     int nb_stride;
     const int32_t* seq_len;   // decode: [B]; prefill: nullptr
+    int max_len;              // decode: host-side bound of seq_len (device values are clamped to [0, max_len])
     int n_q;                  // rows per sequence
     int q_start, q_block, blk;
     int mode, top_k;

@@ -102,7 +102,7 @@ __global__ void __launch_bounds__(SH_N / SH_E) select_hist_kernel(SelectArgs a) 
         sraw[r] = j < a.nb_stride ? srow[j] : 0.f;
     }
     int n_b;
-    if (a.q_block == 1) n_b = (a.seq_len[b] + a.blk - 1) / a.blk;
+    if (a.q_block == 1) n_b = (min(max(a.seq_len[b], 0), a.max_len) + a.blk - 1) / a.blk;
     else n_b = (a.q_start + (i + 1) * a.q_block - 1) / a.blk + 1;
     n_b = min(n_b, SH_N);
     const int sink_end = min(a.sink, n_b);

@@ -103,6 +103,12 @@ def test_select_argument_errors_are_caught_on_the_host(lib):
     assert lib.spot_select(C.byref(_select_params(blk=16, cap=256, q_block=64, Tq=64, seq_len=None)), None) == UNSUPPORTED
     assert lib.spot_select(None, None) == INVALID
     assert lib.spot_score_blocks(C.byref(_select_params()), None) == INVALID        # block_scores is required
+    # a score-only block (what spot_score_blocks reads: no indices / budgets / cap) can size its own workspace -- a
+    # quantised cache in prefill needs the dequantised prefix (spot.h), a BF16 one nothing beyond the alignment slack
+    so = dict(indices=None, budgets=None, cap=0, block_scores=0x7000, nb_stride=64, q_block=64, Tq=128, q_start=1024,
+              seq_len=None)
+    assert lib.spot_select_workspace_bytes(C.byref(_select_params(fmt=2, **so))) >= 2 * (1024 + 128) * 4 * 64 * 2
+    assert 0 < lib.spot_select_workspace_bytes(C.byref(_select_params(fmt=0, **so))) <= 4096
 
 
 def _attn_params(**over):

@@ -87,7 +87,7 @@ def test_select_matches_oracle(torch_cuda, cfg, fmt):
         _check_select(dd, fmt, report, mode="topk", top_k=16)
     non_exact = [r for r in report if r[3] != "exact"]
     print("near-tie report:", non_exact)
-    assert len(non_exact) <= max(1, len(report) // 10)
+    assert len(non_exact) <= 1          # the observed bound: planted logits leave no near-ties
 
 
 def test_select_edge_cases(torch_cuda):
@@ -216,12 +216,14 @@ def test_end_to_end_step_matches_oracle(torch_cuda):
 
 @pytest.mark.parametrize("cfg,fmt,seqs", [("cfg3", "bf16", (0, 3)), ("cfg3", "mxfp4", (1,)), ("cfg3", "int4_e4m3", (2,)),
                                           ("cfg2", "bf16", (0, 7)), ("cfg4_b4", "mxfp4", (0, 1, 2, 3)),
+                                          ("cfg4_b1", "mxfp4", (0,)), ("cfg4_b16", "mxfp4", (0, 5, 10, 15)),
                                           ("cfg3/d128", "bf16", (1,)), ("cfg3/d128", "mxfp4", (2,)),
                                           ("cfg3", "fp8_e4m3", (3,)), ("cfg3/d128", "fp8_e4m3", (0,)),
                                           ("cfg3/blk16", "bf16", (2,)), ("cfg3/blk16/d128", "mxfp4", (0,))])
 def test_full_size_configs_in_the_bench_configuration(torch_cuda, cfg, fmt, seqs):
-    """BASELINE.json configs 2, 3 and 4 (batch 4) at full size (config 3: B=4, L=131072, 2048 blocks per sequence;
-    config 4: H_q=64 and per-query budgets from the K_min floor to hundreds of blocks), launched exactly as bench.py
+    """BASELINE.json configs 2, 3 and 4 (its whole batch sweep 1 / 4 / 16) at full size (config 3: B=4, L=131072, 2048
+    blocks per sequence; config 4: H_q=64 and per-query budgets from the K_min floor to hundreds of blocks; batch 1 runs
+    the attention kernel's "fewer units than CTAs" cut, batch 16 the 16-row selection grid), launched exactly as bench.py
     launches it (scores in the workspace, cap = n_b, K/V [B][H_kv][L][D] drawn on the device).  Sampled outputs the
     oracle can compute one by one: the whole selection of the sampled sequences (scores, index list, budget), and
     the attention output of every head of those sequences over the oracle's list (the oracle is run on the gathered
@@ -424,7 +426,7 @@ def test_block16_select_matches_oracle(torch_cuda, cfg, fmt):
     _check_select(dd, fmt, report, mode="topk", top_k=64)
     non_exact = [r for r in report if r[3] != "exact"]
     print("near-tie report:", non_exact)
-    assert len(non_exact) <= max(1, len(report) // 10)
+    assert len(non_exact) <= 1          # the observed bound
 
 
 def test_block16_select_edge_cases_and_long_rows(torch_cuda):

@@ -92,7 +92,10 @@ def test_prefill_selection_over_a_quantised_cache(torch_cuda, fmt):
                                 nb_stride=nb_stride)
     with pytest.raises(RuntimeError, match="WORKSPACE"):
         api.spot_score_blocks(sp)
-    ws = torch.empty(256 + dp.B * (dp.q_start + dp.Tq) * wl.H_idx * wl.d_idx * 2, dtype=torch.uint8, device="cuda")
+    # a score-only block (no indices / budgets / cap) sizes its own workspace: the dequantised prefix
+    need = api.spot_select_workspace_bytes(sp)
+    assert need >= dp.B * (dp.q_start + dp.Tq) * wl.H_idx * wl.d_idx * 2
+    ws = torch.empty(need, dtype=torch.uint8, device="cuda")
     sp.workspace, sp.workspace_bytes = ws.data_ptr(), ws.numel()
     api.spot_score_blocks(sp)
     torch.cuda.synchronize()
@@ -214,29 +217,40 @@ def test_prefill_attention_argument_errors(torch_cuda):
 
 def test_full_size_cfg5_in_the_bench_configuration(torch_cuda):
     """BASELINE.json config 5 at full size (L=65536, whole prompt as one chunk), launched as bench.py launches it.
-    Sampled outputs the oracle can compute one by one: the selection rows of a few query blocks (first, middle, last)
-    and their attention outputs over the oracle's lists.  For attention the oracle runs on the gathered selected
-    blocks with the query block re-based onto the last of them (all other selected blocks are fully visible, so the
-    causal structure is unchanged)."""
+    Sampled outputs the oracle can compute one by one: a seeded sample of 32 query blocks plus
+    the first and the last -- for each, the whole selection row (tile scores, index list, budget) and the attention
+    output over the oracle's list.  For attention the oracle runs on the gathered selected blocks with the query re-based
+    onto the last of them (all other selected blocks are fully visible, so the causal structure is unchanged); the
+    oracle's prefill attention costs ~1.5 s per (query, 32 heads) at a budget of 500 blocks, so the first two query blocks
+    are checked on every query row and the others on four rows each (the block's first and last row -- the two ends of
+    the diagonal mask -- and two seeded ones; eight rows for the last block), every head of each."""
     torch = torch_cuda
     from oracle import attention as OA
     from paper_2606_22874_b200 import api
     L = 65536
+    n_qb = L // 64
     wl = make_prefill_workload(seed=5005, L=L, with_kv=False)
     dp = H.DevicePrefill([wl], 0, L, with_kv=False)
     idx, bud, scores, probs = dp.select(want_probs=False)
-    sample = [0, 1, 511, 1023]
-    sels = {}
+    rng = np.random.Generator(np.random.Philox(55005))
+    sample = sorted(set([0, 1, n_qb - 1]) | set(rng.choice(np.arange(2, n_qb - 1), size=32, replace=False).tolist()))
+    assert len(sample) >= 34
+    full_rows = {0, 1}
+    sels, near = {}, []
     for i in sample:
         (s_bar, sel), = H.oracle_select_prefill(wl, i * 64, 64)
         np.testing.assert_allclose(scores[i, :len(s_bar)], s_bar, rtol=2e-5, atol=2e-5)
         cls = H.classify_selection(s_bar, sel, idx[i], int(bud[i]), wl.p)
         assert not cls.startswith("FAIL"), "query block %d: %s" % (i, cls)
-        print("cfg5 query block %d: selection %s, budget %d of %d" % (i, cls, sel.budget, i + 1))
+        if cls != "exact":
+            near.append((i, cls))
         idx[i] = -1
         idx[i, :sel.budget] = sel.indices
         bud[i] = sel.budget
         sels[i] = sel
+    print("cfg5: %d sampled query blocks, budgets %s, near-tie rows %s"
+          % (len(sample), [sels[i].budget for i in sample], near))
+    assert len(near) <= 1
     dev = torch.device("cuda")
     gen = torch.Generator(device=dev)
     gen.manual_seed(wl.seed + 17)
@@ -250,6 +264,7 @@ def test_full_size_cfg5_in_the_bench_configuration(torch_cuda):
                               q_start=0, blk=64, sm_scale=wl.sm_scale, out=out)
     api.spot_sparse_attn_prefill(ap)
     torch.cuda.synchronize()
+    worst = (0.0, 0.0)
     for i in sample:
         blocks = sels[i].indices.astype(np.int64)
         assert blocks[-1] == i                                   # the diagonal block is reserved (recency tier)
@@ -260,11 +275,21 @@ def test_full_size_cfg5_in_the_bench_configuration(torch_cuda):
         Kh = H.bf16_bits_to_f64(H.to_np_u16(Kg.contiguous().view(torch.int16))).transpose(1, 0, 2)
         Vh = H.bf16_bits_to_f64(H.to_np_u16(Vg.contiguous().view(torch.int16))).transpose(1, 0, 2)
         Qh = H.bf16_bits_to_f64(H.to_np_u16(Q[0, i * 64:(i + 1) * 64].contiguous().view(torch.int16)))
-        want = OA.sparse_attn_prefill(Qh, Kh, Vh, [list(range(n))], (n - 1) * 64, 64, 64, wl.sm_scale)
         got = H.bf16_bits_to_f64(H.to_np_u16(out[0, i * 64:(i + 1) * 64]))
-        err = np.abs(got - want)
+        if i in full_rows:
+            want = OA.sparse_attn_prefill(Qh, Kh, Vh, [list(range(n))], (n - 1) * 64, 64, 64, wl.sm_scale)
+            err = np.abs(got - want)
+        else:
+            extra = 6 if i == n_qb - 1 else 2
+            rows = sorted({0, 63} | set(rng.choice(np.arange(1, 63), size=extra, replace=False).tolist()))
+            # one query at a time: the oracle's prefill form with q_block = 1 at the query's (re-based) position
+            want = np.stack([OA.sparse_attn_prefill(Qh[r:r + 1], Kh, Vh, [list(range(n))], (n - 1) * 64 + r, 1, 64,
+                                                    wl.sm_scale)[0] for r in rows])
+            err = np.abs(got[rows] - want)
         assert err.max() <= MAX_ABS and err.mean() <= MEAN_ABS, (i, err.max(), err.mean())
-        print("cfg5 query block %d: attention over %d blocks, max-abs %.2e mean-abs %.2e" % (i, n, err.max(), err.mean()))
+        worst = (max(worst[0], err.max()), max(worst[1], err.mean()))
+    print("cfg5: attention over the oracle's lists of %d query blocks, worst max-abs %.2e mean-abs %.2e"
+          % (len(sample), worst[0], worst[1]))
 
 
 @pytest.mark.parametrize("page_tokens,layout", [(64, "phd"), (128, "pthd"), (256, "phd")])
