@@ -5,8 +5,8 @@ GQA attention) on synthetic Qwen3-shaped inputs, through the C ABI of include/sp
     python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg3] [--fmt bf16|mxfp4|int4_e4m3] [--p 0.9]
     python bench.py --impl reference ...       # the fp64 CPU oracle on a bounded sample (rank 0 only)
 
-Prints ONE JSON line (rank 0).  A "step" = spot_select + spot_sparse_attn_decode over one batch (all of SURVEY.md
-section 8(a)'s decode rows: a1 score + block max, a2 distribution + selection, a3 sparse attention; a0 runs once, before
+Prints ONE JSON line (rank 0).  A "step" = spot_decode_step (= spot_select + spot_sparse_attn_decode in one call) over
+one batch (all of SURVEY.md section 8(a)'s decode rows: a1 score + block max, a2 distribution + selection, a3 sparse attention; a0 runs once, before
 the timed region, because the cache is quantised when tokens are appended, not per step).  The L2 is flushed (a
 read sweep over a 512 MiB buffer) before every timed step; each step is timed with its own CUDA-event pair on the
 launching stream and the flush sits outside the pairs.  DESIGN.md section 7 states the byte accounting."""
@@ -226,6 +226,12 @@ def run_ours(args):
     ws_den = torch.empty(max(16, api.spot_dense_attn_decode_workspace_bytes(apd)), dtype=torch.uint8, device=dev)
     apd.workspace, apd.workspace_bytes = ws_den.data_ptr(), ws_den.numel()
 
+    # the step: a1 + a2 + a3 in ONE call (spot_decode_step: the same kernels as spot_select + spot_sparse_attn_decode,
+    # launched so that they overlap -- include/spot.h)
+    dp = api.make_decode_step_params(sp, ap)
+    ws_step = torch.empty(max(16, api.spot_decode_step_workspace_bytes(dp)), dtype=torch.uint8, device=dev)
+    dp.workspace, dp.workspace_bytes = ws_step.data_ptr(), ws_step.numel()
+
     flush = torch.empty(512 << 20, dtype=torch.uint8, device=dev).zero_()
     stream = torch.cuda.current_stream()
 
@@ -233,8 +239,7 @@ def run_ours(args):
         flush.view(torch.int64).sum()             # read sweep: leaves the L2 full of clean lines
 
     def step():
-        api.spot_select(sp, stream)
-        api.spot_sparse_attn_decode(ap, stream)
+        api.spot_decode_step(dp, stream)
 
     def barrier():
         torch.cuda.synchronize()
@@ -258,8 +263,7 @@ def run_ours(args):
     for i in range(args.steps):
         flush_l2()
         ev[i][0].record(stream)
-        api.spot_select(sp, stream)
-        api.spot_sparse_attn_decode(ap, stream)
+        api.spot_decode_step(dp, stream)
         ev[i][1].record(stream)
     barrier()
     step_ms = np.array([e[0].elapsed_time(e[1]) for e in ev])
@@ -277,10 +281,12 @@ def run_ours(args):
                 ts.append(a_.elapsed_time(b_))
         return np.array(ts)
 
-    # the two calls timed alone (breakdown, and the live duration of the dominant kernel for the roofline object)
+    # the two calls timed alone (breakdown, and the live duration of the dominant kernel for the roofline object), and
+    # back to back as separate calls (what the one-call step is compared with)
     n_alone = max(3, min(args.steps, 20))
     sel_ms = time_alone(lambda: api.spot_select(sp, stream), n_alone)
     att_ms = time_alone(lambda: api.spot_sparse_attn_decode(ap, stream), n_alone)
+    sep_ms = time_alone(lambda: (api.spot_select(sp, stream), api.spot_sparse_attn_decode(ap, stream)), n_alone)
 
     # the same step replayed from a CUDA graph (the calls never synchronise, so a caller may capture them)
     graph_us = None
@@ -288,8 +294,7 @@ def run_ours(args):
         cap_stream = torch.cuda.Stream()
         gph = torch.cuda.CUDAGraph()
         with torch.cuda.graph(gph, stream=cap_stream):
-            api.spot_select(sp, torch.cuda.current_stream())
-            api.spot_sparse_attn_decode(ap, torch.cuda.current_stream())
+            api.spot_decode_step(dp, torch.cuda.current_stream())
         graph_us = float(time_alone(gph.replay, n_alone).mean()) * 1e3
     except Exception as e:                                    # reported, never fatal for the headline number
         graph_us = "capture failed: %s" % (str(e).splitlines()[0] if str(e) else type(e).__name__)
@@ -338,6 +343,8 @@ def run_ours(args):
     hp.sel_q_host, hp.w_host, hp.q_host = h_in.data_ptr(), h_in.data_ptr() + n_selq, h_in.data_ptr() + n_selq + n_w
     hp.out_host, hp.budgets_host = h_res.data_ptr(), h_res.data_ptr() + n_out
     hp.select, hp.attn = sp_e, ap_e
+    ws_step_e = torch.empty(ws_step.numel(), dtype=torch.uint8, device=dev)
+    hp.step_workspace, hp.step_workspace_bytes = ws_step_e.data_ptr(), ws_step_e.numel()
     h_bud = h_res[n_out:].view(torch.int32)
     h2d = n_selq + n_w + n_q
     d2h = n_out + n_bud
@@ -391,6 +398,7 @@ def run_ours(args):
         "tokens_per_s": world * Bn / (n_layers * step_mean * 1e-3),
         "breakdown_us": {"select (score+select kernels)": float(sel_ms.mean()) * 1e3,
                          "sparse attention (attn+merge kernels)": float(att_ms.mean()) * 1e3,
+                         "spot_select + spot_sparse_attn_decode as two calls": float(sep_ms.mean()) * 1e3,
                          "dense flash-decode comparator": float(np.mean(den)) * 1e3,
                          "step replayed from a CUDA graph": graph_us,
                          "upstream f1 alone (projection + RoPE + append; not in the step)": float(np.mean(f1_ms)) * 1e3},

@@ -18,6 +18,8 @@
  *     library never allocates, frees or keeps a pointer after the call returns.
  *   - Every call is asynchronous on the caller's stream (a cudaStream_t passed as void*; NULL = legacy
  *     default stream) and never synchronises.  All argument checks run on the host before any launch.
+ *   - Device lengths are clamped: a seq_len[b] outside [0, max_seq_len] is read as the nearer bound (grids, score rows
+ *     and workspaces are sized from max_seq_len, so a stale length cannot make a kernel leave its buffers).
  *   - Return value: spot_status.  SPOT_ERR_CUDA means a CUDA runtime call failed; the code is kept
  *     per thread and returned by spot_last_cuda_error().
  *   - BF16 tensors are passed as uint16_t bit patterns.  Pointers must be 16-byte aligned.
@@ -65,7 +67,8 @@ int spot_last_cuda_error(void);
 /* Library version, "major.minor". */
 const char* spot_version(void);
 /* sizeof() of the parameter blocks as this library was compiled (which: 0 = spot_select_params,
- * 1 = spot_attn_params, 2 = spot_decode_step_host_params, 3 = spot_project_params; anything else: 0) -- lets a binding verify its layout. */
+ * 1 = spot_attn_params, 2 = spot_decode_step_host_params, 3 = spot_project_params, 4 = spot_decode_step_params; anything
+ * else: 0) -- lets a binding verify its layout. */
 size_t spot_struct_size(int which);
 
 /* ---------------------------------------------------------------------------------------------------
@@ -261,9 +264,35 @@ size_t spot_dense_attn_decode_workspace_bytes(const spot_attn_params* p);
 spot_status spot_dense_attn_decode(const spot_attn_params* p, void* stream);
 
 /* ---------------------------------------------------------------------------------------------------
- * Host-buffer convenience (the "e2e" path of bench.py): one decode layer-step with every tensor in HOST
- * memory.  Copies inputs host->device into caller-provided device staging buffers, runs
- * spot_select + spot_sparse_attn_decode, copies out/indices/budgets back, all on `stream`, no sync.
+ * One decode layer-step in ONE call: a1 + a2 + a3 (spot_select followed by spot_sparse_attn_decode over the lists it
+ * wrote), same arithmetic, same outputs, same parameter blocks -- but launched as kernels that overlap (DESIGN.md
+ * section 7): the scoring kernel walks the sequences in order, the selection of sequence b runs (on SMs left to it) while
+ * sequences b + 1.. are still being scored, and the attention kernel, resident as soon as the scoring CTAs retire,
+ * starts on the sequences whose lists are ready and takes the last sequence last, so that no selection latency sits
+ * between the two HBM streams.  The hand-offs are a few words in `workspace` (flags and counters; the workspace need not
+ * be initialised and may be reused by the next call on the same stream; two calls in flight on different streams need
+ * two workspaces).
+ *   select / attn: as for the separate calls, with the SAME indices / budgets / cap / seq_len / max_seq_len / blk / B in
+ *   both (SPOT_ERR_INVALID_ARG otherwise), q_block == 1; each still carries its own workspace.
+ * Like every call: asynchronous on `stream`, never synchronises, capturable in a CUDA graph.
+ * --------------------------------------------------------------------------------------------------- */
+typedef struct {
+    spot_select_params select;
+    spot_attn_params attn;
+    void* workspace;
+    size_t workspace_bytes;      /* >= spot_decode_step_workspace_bytes(&params)                          */
+} spot_decode_step_params;
+
+size_t spot_decode_step_workspace_bytes(const spot_decode_step_params* p);
+spot_status spot_decode_step(const spot_decode_step_params* p, void* stream);
+
+/* ---------------------------------------------------------------------------------------------------
+ * Host-buffer convenience (the "e2e" path of bench.py): one decode layer-step with every per-step tensor in HOST
+ * memory.  Copies the step's inputs host->device into caller-provided device staging buffers, runs spot_decode_step,
+ * copies the attention output and the budgets back (the index lists stay on the device: `out | budgets` is all that
+ * returns), all on `stream`, no sync.
+ * The *_host buffers must be PAGE-LOCKED (cudaHostAlloc / cudaHostRegister; SPOT_ERR_INVALID_ARG otherwise): a copy from
+ * pageable memory would block the host and could not be captured.  Every argument check runs before the first copy.
  * When the host inputs are laid out back to back (sel_q | w | q) and so are their device staging areas, they go up as
  * ONE transfer; likewise out | budgets come back as one (each small copy costs microseconds of stream time).
  * (Declared here so that the end-to-end measurement also crosses the C ABI.)
@@ -279,6 +308,8 @@ typedef struct {
     /* device-resident state and staging; select/attn hold the device pointers of everything else */
     spot_select_params select;   /* sel_q / w point at device staging */
     spot_attn_params attn;       /* q / out point at device staging   */
+    void* step_workspace;        /* device, >= spot_decode_step_workspace_bytes of the same select / attn  */
+    size_t step_workspace_bytes;
 } spot_decode_step_host_params;
 
 spot_status spot_decode_step_host(const spot_decode_step_host_params* p, void* stream);

@@ -51,6 +51,14 @@ class DecodeStepHostParams(C.Structure):
         ("sel_q_host", C.c_void_p), ("w_host", C.c_void_p), ("q_host", C.c_void_p),
         ("out_host", C.c_void_p), ("budgets_host", C.c_void_p),
         ("select", SelectParams), ("attn", AttnParams),
+        ("step_workspace", C.c_void_p), ("step_workspace_bytes", C.c_size_t),
+    ]
+
+
+class DecodeStepParams(C.Structure):
+    _fields_ = [
+        ("select", SelectParams), ("attn", AttnParams),
+        ("workspace", C.c_void_p), ("workspace_bytes", C.c_size_t),
     ]
 
 
@@ -86,6 +94,8 @@ PROTOTYPES = {
     "spot_dense_attn_decode_workspace_bytes": (C.c_size_t, [C.POINTER(AttnParams)]),
     "spot_dense_attn_decode": (C.c_int, [C.POINTER(AttnParams), C.c_void_p]),
     "spot_decode_step_host": (C.c_int, [C.POINTER(DecodeStepHostParams), C.c_void_p]),
+    "spot_decode_step_workspace_bytes": (C.c_size_t, [C.POINTER(DecodeStepParams)]),
+    "spot_decode_step": (C.c_int, [C.POINTER(DecodeStepParams), C.c_void_p]),
     "spot_selector_project_append_workspace_bytes": (C.c_size_t, [C.POINTER(ProjectParams)]),
     "spot_selector_project_append": (C.c_int, [C.POINTER(ProjectParams), C.c_void_p]),
 }
@@ -106,7 +116,7 @@ def load():
             fn = getattr(lib, name)
             fn.restype = res
             fn.argtypes = args
-        for which, st in enumerate((SelectParams, AttnParams, DecodeStepHostParams, ProjectParams)):
+        for which, st in enumerate((SelectParams, AttnParams, DecodeStepHostParams, ProjectParams, DecodeStepParams)):
             if lib.spot_struct_size(which) != C.sizeof(st):
                 raise RuntimeError("ABI mismatch: %s is %d bytes in libspot.so, %d in the binding"
                                    % (st.__name__, lib.spot_struct_size(which), C.sizeof(st)))

@@ -7,7 +7,7 @@ import ctypes as C
 import torch
 
 from . import _lib as L
-from ._lib import AttnParams, DecodeStepHostParams, ProjectParams, SelectParams, FORMATS, MODES  # noqa: F401
+from ._lib import AttnParams, DecodeStepHostParams, DecodeStepParams, ProjectParams, SelectParams, FORMATS, MODES  # noqa: F401
 
 
 class SpotError(RuntimeError):
@@ -145,6 +145,22 @@ def spot_sparse_attn_prefill_workspace_bytes(ap):
 
 def spot_sparse_attn_prefill(ap, stream=None):
     _check(L.load().spot_sparse_attn_prefill(C.byref(ap), _stream(stream)), "spot_sparse_attn_prefill")
+
+
+def make_decode_step_params(sp, ap, workspace=None):
+    dp = DecodeStepParams()
+    dp.select, dp.attn = sp, ap
+    if workspace is not None:
+        dp.workspace, dp.workspace_bytes = workspace.data_ptr(), workspace.numel() * workspace.element_size()
+    return dp
+
+
+def spot_decode_step_workspace_bytes(dp):
+    return int(L.load().spot_decode_step_workspace_bytes(C.byref(dp)))
+
+
+def spot_decode_step(dp, stream=None):
+    _check(L.load().spot_decode_step(C.byref(dp), _stream(stream)), "spot_decode_step")
 
 
 def spot_decode_step_host(hp, stream=None):

@@ -2,6 +2,9 @@
 // host-buffer decode step.  All argument validation happens here, on the host, before any launch.
 #include "common.cuh"
 
+#include <chrono>
+#include <string.h>
+
 namespace spot {
 
 static thread_local int g_last_cuda_error = 0;
@@ -33,10 +36,12 @@ int sm_count() {
 }
 
 // kernels implemented in the other translation units
-spot_status score_decode(const spot_select_params* p, float* scores, int nb_stride, cudaStream_t s);
+spot_status score_decode(const spot_select_params* p, float* scores, int nb_stride, const StepSync* sync, int reserve_sms,
+                         cudaStream_t s);
 spot_status score_prefill(const spot_select_params* p, float* scores, int nb_stride, cudaStream_t s);
 spot_status run_select(const spot_select_params* p, const float* scores, int nb_stride, int rows_per_seq, int max_nb,
-                       cudaStream_t s);
+                       const StepSync* sync, cudaStream_t s);
+spot_status attn_decode_piped(const spot_attn_params* p, const StepSync* sync, cudaStream_t s);     // attn_decode.cu
 spot_status check_attn_decode_args(const spot_attn_params* p);     // attn_decode.cu: the host-side checks of a3
 
 namespace {
@@ -99,8 +104,42 @@ size_t prefill_scratch_bytes(const spot_select_params* p) {
     return 256 + (size_t)p->B * ((size_t)p->q_start + p->Tq) * p->H_idx * p->d_idx * 2;
 }
 
-spot_status score_any(const spot_select_params* p, float* scores, int nb_stride, void* scratch_area, cudaStream_t s) {
-    if (p->q_block == 1) return score_decode(p, scores, nb_stride, s);
+#ifdef SPOT_TRACE
+unsigned long long* g_trace = nullptr;     // development builds only: where the kernels of a step stamp %globaltimer
+#endif
+
+// a token unlike the previous call's on the same workspace (common.cuh, StepSync): host clock in ns, salted per thread
+unsigned long long fresh_token() {
+    static thread_local unsigned long long salt = 0;
+    const unsigned long long ns =
+        (unsigned long long)std::chrono::steady_clock::now().time_since_epoch().count();
+    return ((ns << 8) ^ (++salt & 0xffull)) | 1ull;
+}
+
+// the hand-off words of a pipelined call (common.cuh, StepSync): ready[B] laid over `area` (nullptr: no ready words)
+StepSync make_sync(void* area, bool with_ready) {
+    StepSync y;
+    memset(&y, 0, sizeof(y));
+    const unsigned long long t = fresh_token();
+    y.tag = (uint32_t)(t ^ (t >> 32)) | 1u;
+    y.ready = with_ready ? reinterpret_cast<uint32_t*>((reinterpret_cast<uintptr_t>(area) + 63) & ~(uintptr_t)63) : nullptr;
+#ifdef SPOT_TRACE
+    y.trace = g_trace;
+#endif
+    return y;
+}
+size_t sync_area_bytes(int B) { return 64 + step_sync_bytes(B); }   // 64: alignment slack
+
+// decode rows of spot_select / spot_decode_step: the scoring kernel hands its block scores over as 64-bit tagged words
+int tagged_stride(const SelectGeom& g) { return (g.max_nb + 3) & ~3; }
+size_t tagged_bytes(const spot_select_params* p, const SelectGeom& g) { return (size_t)p->B * tagged_stride(g) * 8; }
+
+// SMs the scoring grid leaves to the selection CTAs that run beside it
+int reserve_for_select(int B) { return B < 8 ? B : 8; }
+
+spot_status score_any(const spot_select_params* p, float* scores, int nb_stride, void* scratch_area, const StepSync* sync,
+                      cudaStream_t s) {
+    if (p->q_block == 1) return score_decode(p, scores, nb_stride, sync, sync ? reserve_for_select(p->B) : 0, s);
     if (p->fmt == SPOT_SELK_BF16) return score_prefill(p, scores, nb_stride, s);
     uint16_t* deq = reinterpret_cast<uint16_t*>((reinterpret_cast<uintptr_t>(scratch_area) + 255) & ~(uintptr_t)255);
     const int tok = p->q_start + p->Tq;
@@ -137,6 +176,7 @@ extern "C" size_t spot_struct_size(int which) {
         case 1: return sizeof(spot_attn_params);
         case 2: return sizeof(spot_decode_step_host_params);
         case 3: return sizeof(spot_project_params);
+        case 4: return sizeof(spot_decode_step_params);
     }
     return 0;
 }
@@ -146,25 +186,46 @@ extern "C" size_t spot_select_workspace_bytes(const spot_select_params* p) {
     // a block without an index list is a spot_score_blocks block (it ignores indices / budgets / cap): size it as such
     if (!p || select_geometry(p, &g, /*score_only=*/!p->indices) != SPOT_OK) return 0;
     size_t bytes = 256;
-    if (g.own_scores) bytes += (size_t)p->B * g.rows_per_seq * g.nb_stride * sizeof(float);
+    if (p->q_block == 1 && p->indices) bytes += tagged_bytes(p, g);          // decode rows: block scores as tagged words
+    else if (g.own_scores) bytes += (size_t)p->B * g.rows_per_seq * g.nb_stride * sizeof(float);
     return bytes + prefill_scratch_bytes(p);
 }
 
-extern "C" spot_status spot_select(const spot_select_params* p, void* stream) {
+namespace spot {
+namespace {
+
+// a1 + a2.  ext: the hand-offs of a whole step (spot_decode_step; its `ready` words are what the attention kernel waits
+// for); nullptr: the call's own, in its workspace, when the rows are decode rows.
+spot_status select_impl(const spot_select_params* p, const StepSync* ext, cudaStream_t s) {
     SelectGeom g;
     spot_status st = select_geometry(p, &g);
     if (st != SPOT_OK) return st;
     if ((st = check_device()) != SPOT_OK) return st;
+    const bool piped = p->q_block == 1;
     float* scores = p->block_scores;
-    const size_t own = g.own_scores ? 256 + (size_t)p->B * g.rows_per_seq * g.nb_stride * sizeof(float) : 0;
+    int stride = g.nb_stride;
+    size_t own = 0;
+    if (piped) { own = 256 + tagged_bytes(p, g); stride = tagged_stride(g); }
+    else if (g.own_scores) own = 256 + (size_t)p->B * g.rows_per_seq * g.nb_stride * sizeof(float);
     const size_t need = own + prefill_scratch_bytes(p);
     if (need && (!p->workspace || p->workspace_bytes < need)) return SPOT_ERR_WORKSPACE_TOO_SMALL;
-    if (g.own_scores)
-        scores = reinterpret_cast<float*>(reinterpret_cast<uintptr_t>(p->workspace) + 255 & ~(uintptr_t)255);
-    cudaStream_t s = (cudaStream_t)stream;
-    st = score_any(p, scores, g.nb_stride, reinterpret_cast<char*>(p->workspace) + own, s);
+    if (own) scores = reinterpret_cast<float*>(reinterpret_cast<uintptr_t>(p->workspace) + 255 & ~(uintptr_t)255);
+    StepSync mine;
+    const StepSync* sync = nullptr;
+    if (piped) {
+        if (ext) sync = ext;
+        else { mine = make_sync(nullptr, false); sync = &mine; }
+    }
+    st = score_any(p, scores, stride, reinterpret_cast<char*>(p->workspace) + own, sync, s);
     if (st != SPOT_OK) return st;
-    return run_select(p, scores, g.nb_stride, g.rows_per_seq, g.max_nb, s);
+    return run_select(p, scores, stride, g.rows_per_seq, g.max_nb, sync, s);
+}
+
+}  // namespace
+}  // namespace spot
+
+extern "C" spot_status spot_select(const spot_select_params* p, void* stream) {
+    return select_impl(p, nullptr, (cudaStream_t)stream);
 }
 
 extern "C" spot_status spot_score_blocks(const spot_select_params* p, void* stream) {
@@ -175,20 +236,57 @@ extern "C" spot_status spot_score_blocks(const spot_select_params* p, void* stre
     cudaStream_t s = (cudaStream_t)stream;
     const size_t need = prefill_scratch_bytes(p);        // quantised cache in prefill: the one case that needs the workspace
     if (need && (!p->workspace || p->workspace_bytes < need)) return SPOT_ERR_WORKSPACE_TOO_SMALL;
-    return score_any(p, p->block_scores, g.nb_stride, p->workspace, s);
+    return score_any(p, p->block_scores, g.nb_stride, p->workspace, nullptr, s);
+}
+
+namespace spot {
+namespace {
+
+// the two parameter blocks of a step must describe ONE step: same batch, same lists, same lengths
+spot_status check_step(const spot_select_params& sp, const spot_attn_params& ap) {
+    SelectGeom g;
+    spot_status st = select_geometry(&sp, &g);
+    if (st != SPOT_OK) return st;
+    if ((st = check_attn_decode_args(&ap)) != SPOT_OK) return st;
+    if (sp.q_block != 1 || sp.B != ap.B || sp.blk != ap.blk) return SPOT_ERR_INVALID_ARG;
+    if (ap.indices != sp.indices || ap.budgets != sp.budgets || ap.cap != sp.cap) return SPOT_ERR_INVALID_ARG;
+    if (ap.seq_len != sp.seq_len || ap.max_seq_len != sp.max_seq_len) return SPOT_ERR_INVALID_ARG;
+    return SPOT_OK;
+}
+
+spot_status step_impl(const spot_select_params& sp, const spot_attn_params& ap, void* ws, size_t ws_bytes, cudaStream_t s) {
+    if (!ws || ws_bytes < sync_area_bytes(sp.B)) return SPOT_ERR_WORKSPACE_TOO_SMALL;
+    const StepSync sync = make_sync(ws, true);
+    spot_status st = select_impl(&sp, &sync, s);
+    if (st != SPOT_OK) return st;
+    return attn_decode_piped(&ap, &sync, s);
+}
+
+}  // namespace
+}  // namespace spot
+
+extern "C" size_t spot_decode_step_workspace_bytes(const spot_decode_step_params* p) {
+    if (!p || check_step(p->select, p->attn) != SPOT_OK) return 0;
+    return sync_area_bytes(p->select.B);
+}
+
+extern "C" spot_status spot_decode_step(const spot_decode_step_params* p, void* stream) {
+    if (!p) return SPOT_ERR_INVALID_ARG;
+    spot_status st = check_step(p->select, p->attn);
+    if (st != SPOT_OK) return st;
+    if ((st = check_device()) != SPOT_OK) return st;
+    return step_impl(p->select, p->attn, p->workspace, p->workspace_bytes, (cudaStream_t)stream);
 }
 
 extern "C" spot_status spot_decode_step_host(const spot_decode_step_host_params* p, void* stream) {
     if (!p || !p->sel_q_host || !p->w_host || !p->q_host || !p->out_host || !p->budgets_host) return SPOT_ERR_INVALID_ARG;
     const spot_select_params& sp = p->select;
     const spot_attn_params& ap = p->attn;
-    if (sp.q_block != 1 || sp.B != ap.B) return SPOT_ERR_INVALID_ARG;
-    // every argument check of the two calls runs before the first copy is enqueued
+    // every argument check of the step runs before the first copy is enqueued
     {
-        SelectGeom g;
-        spot_status st0 = select_geometry(&sp, &g);
+        spot_status st0 = check_step(sp, ap);
         if (st0 != SPOT_OK) return st0;
-        if ((st0 = check_attn_decode_args(&ap)) != SPOT_OK) return st0;
+        if (!p->step_workspace || p->step_workspace_bytes < sync_area_bytes(sp.B)) return SPOT_ERR_WORKSPACE_TOO_SMALL;
         if ((st0 = check_device()) != SPOT_OK) return st0;
         // the *_host buffers must be page-locked: a pageable cudaMemcpyAsync blocks the host and cannot be captured
         const void* hosts[5] = {p->sel_q_host, p->w_host, p->q_host, p->out_host, p->budgets_host};
@@ -216,9 +314,7 @@ extern "C" spot_status spot_decode_step_host(const spot_decode_step_host_params*
         SPOT_CUDA_TRY(cudaMemcpyAsync((void*)sp.w, p->w_host, n_w, cudaMemcpyHostToDevice, s));
         SPOT_CUDA_TRY(cudaMemcpyAsync((void*)ap.q, p->q_host, n_q, cudaMemcpyHostToDevice, s));
     }
-    spot_status st = spot_select(&sp, stream);
-    if (st != SPOT_OK) return st;
-    st = spot_sparse_attn_decode(&ap, stream);
+    spot_status st = step_impl(sp, ap, p->step_workspace, p->step_workspace_bytes, s);
     if (st != SPOT_OK) return st;
     const size_t n_out = (size_t)ap.B * ap.H_q * ap.D * 2, n_bud = (size_t)sp.B * 4;
     const bool out_packed = reinterpret_cast<char*>(p->budgets_host) == reinterpret_cast<char*>(p->out_host) + n_out &&
@@ -231,3 +327,7 @@ extern "C" spot_status spot_decode_step_host(const spot_decode_step_host_params*
     }
     return SPOT_OK;
 }
+
+#ifdef SPOT_TRACE
+extern "C" void spot_debug_set_trace(void* dev_buf) { spot::g_trace = (unsigned long long*)dev_buf; }
+#endif

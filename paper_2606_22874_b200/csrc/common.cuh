@@ -53,6 +53,33 @@ __host__ __device__ inline int64_t selk_tile_bytes(int H, int d) {
     return SELK_TILE * (selk_codes_per_token(H, d) + selk_scales_per_token(H, d));
 }
 
+// ---- pipelined decode step: cross-kernel hand-offs through global memory ---------------------------------------
+// spot_select and spot_decode_step run score -> select (-> attend) as kernels that are resident TOGETHER: the scoring
+// kernel walks the sequences in order on all of its CTAs; the selection CTA of a sequence waits for that sequence's block
+// scores only, not for the end of the scoring grid, so the selection of sequence b overlaps the scoring of b + 1, ..; it
+// then publishes ready[b], which is all an attention CTA waits for before it reads that sequence's index list.  Later
+// kernels only ever wait on earlier ones (which are resident, or done, before a later one can start: programmatic
+// dependent launch), never the other way round.
+//
+// No fence in the streaming kernel: a block score travels as ONE 64-bit word {tag, fp32 bits} (a naturally aligned
+// 64-bit store is single-copy atomic), and the selection CTA simply re-reads an entry until it carries this call's tag
+// -- a gpu-scope fence in a warp of the scoring kernel waits for the SM's bulk copies in flight (4-5 us each time,
+// measured).  Only the selection kernel (one release per sequence) and the attention kernel (acquire loads) use
+// ordered accesses.
+//
+// The words live in caller-owned workspace that need NOT be initialised: the tag is derived from a per-call token unlike
+// the previous call's, and every reader clears what it has consumed (score tags: the selection CTA; ready words: the
+// merge kernel, which runs when the attention grid has completed), so a finished call leaves no live tag behind -- which
+// is what lets the replay of a captured graph (same token every time) start clean.
+struct StepSync {
+    uint32_t tag;                 // 0: no hand-offs (plain stream order through griddepcontrol.wait)
+    uint32_t* ready;              // [B] == tag once the selection of sequence b is in global memory; nullptr: nobody waits
+#ifdef SPOT_TRACE
+    unsigned long long* trace;    // development builds only (-DSPOT_TRACE): [kernel][CTA < 512][4] %globaltimer stamps
+#endif
+};
+static inline size_t step_sync_bytes(int B) { return (((size_t)B * 4 + 63) & ~(size_t)63); }
+
 // ---- programmatic dependent launch (PDL) ------------------------------------------------------------
 // The decode step is a chain of four short kernels (score -> select -> attend -> merge) whose launch latencies sit
 // on the critical path.  Every kernel of the chain is launched with programmaticStreamSerializationAllowed = 1 and
@@ -116,6 +143,54 @@ __device__ __forceinline__ void mma_f16_16816(float (&d)[4], uint32_t a0, uint32
     asm volatile("mma.sync.aligned.m16n8k16.row.col.f32.f16.f16.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};"
                  : "+f"(d[0]), "+f"(d[1]), "+f"(d[2]), "+f"(d[3])
                  : "r"(a0), "r"(a1), "r"(a2), "r"(a3), "r"(b0), "r"(b1));
+}
+
+// ---- gpu-scope acquire / release on global words (the hand-offs of the pipelined decode step) --------------------
+__device__ __forceinline__ unsigned long long ld_acquire_u64(const unsigned long long* p) {
+    unsigned long long v;
+    asm volatile("ld.acquire.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
+    return v;
+}
+__device__ __forceinline__ void st_release_u64(unsigned long long* p, unsigned long long v) {
+    asm volatile("st.release.gpu.global.u64 [%0], %1;" :: "l"(p), "l"(v) : "memory");
+}
+__device__ __forceinline__ uint32_t ld_acquire_u32(const uint32_t* p) {
+    uint32_t v;
+    asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    return v;
+}
+__device__ __forceinline__ void st_release_u32(uint32_t* p, uint32_t v) {
+    asm volatile("st.release.gpu.global.u32 [%0], %1;" :: "l"(p), "r"(v) : "memory");
+}
+__device__ __forceinline__ void red_release_add_u32(uint32_t* p, uint32_t v) {
+    asm volatile("red.release.gpu.global.add.u32 [%0], %1;" :: "l"(p), "r"(v) : "memory");
+}
+#ifdef SPOT_TRACE
+__device__ __forceinline__ void trace_stamp(const StepSync& y, int kernel, int slot) {
+    if (y.trace && threadIdx.x == 0 && blockIdx.x < 512) {
+        unsigned long long t;
+        asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+        y.trace[((size_t)kernel * 512 + blockIdx.x) * 4 + slot] = t;
+    }
+}
+#define SPOT_STAMP(y, k, slot) trace_stamp(y, k, slot)
+#else
+#define SPOT_STAMP(y, k, slot) ((void)0)
+#endif
+
+// one thread waits (with back-off) until *p == value
+__device__ __forceinline__ void spin_until_eq(const uint32_t* p, uint32_t value) {
+    while (ld_acquire_u32(p) != value) __nanosleep(64);
+}
+// tagged block scores (see StepSync): one 64-bit word {tag, fp32 bits}
+__device__ __forceinline__ void st_tagged_score(unsigned long long* p, uint32_t tag, float s) {
+    const unsigned long long v = ((unsigned long long)tag << 32) | (unsigned long long)__float_as_uint(s);
+    asm volatile("st.relaxed.gpu.global.u64 [%0], %1;" :: "l"(p), "l"(v) : "memory");
+}
+__device__ __forceinline__ unsigned long long ld_tagged_score(const unsigned long long* p) {
+    unsigned long long v;
+    asm volatile("ld.relaxed.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
+    return v;
 }
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }

@@ -148,17 +148,41 @@ struct ScoreArgs {
     float* scores;
     int nb_stride;
     int fine;                     // blk == 16: four block maxima per 64-token tile (f3)
+    unsigned long long* tagged;   // pipelined step: block scores go out as {tag, fp32 bits} words, [B][nb_stride]
+    uint32_t tag;                 //   (nullptr: plain fp32 into `scores`)
+#ifdef SPOT_TRACE
+    StepSync sync;
+#endif
 };
 
 // seq_len[b] as the kernels use it: clamped to what the grid, the score rows and the cache were sized for
 __device__ __forceinline__ int seq_len_of(const ScoreArgs& a, int b) { return min(max(a.seq_len[b], 0), a.max_len); }
 
-// (sequence, tile) cursor over the flat tile list
+__device__ __forceinline__ int tiles_of(const ScoreArgs& a, int b) { return (seq_len_of(a, b) + 63) >> 6; }
+
+// Work assignment: CTA c of n owns an n-th of EVERY sequence's tiles and walks its slices sequence by sequence -- so
+// the whole grid finishes sequence 0 first, then 1, ..: the selection of a sequence (another kernel, resident beside
+// this one) overlaps the scoring of the next ones.  Sequence b's tiles are cut into n slices [c' nb_b / n,
+// (c' + 1) nb_b / n) and slice c' goes to CTA (c' + off_b) mod n with off_b the number of tiles in front of the sequence:
+// with sequences shorter than n tiles the non-empty slices of consecutive sequences then land on consecutive CTAs instead
+// of on the same few.  The CTA's work list is the concatenation of its slices; the cursor names a position in it.
 struct TileCursor {
-    int b, t, nb;
+    int b, t, end;                // tile t of sequence b; this CTA's slice of sequence b ends at `end`
+    int rot;                      // (blockIdx.x - off_b) mod n: which slice of sequence b is this CTA's
+    __device__ __forceinline__ void slice(const ScoreArgs& a) {
+        const long long nb = tiles_of(a, b);
+        t = (int)((long long)rot * nb / gridDim.x);
+        end = (int)((long long)(rot + 1) * nb / gridDim.x);
+    }
+    __device__ __forceinline__ void first(const ScoreArgs& a) { b = 0; rot = blockIdx.x; slice(a); }
+    __device__ __forceinline__ void next_seq(const ScoreArgs& a) {
+        rot = (int)((rot + (long long)gridDim.x - tiles_of(a, b) % (int)gridDim.x) % gridDim.x);
+        ++b;
+        slice(a);
+    }
     __device__ __forceinline__ void advance(const ScoreArgs& a, int n) {
         t += n;
-        while (t >= nb && b + 1 < a.B) { t -= nb; ++b; nb = (seq_len_of(a, b) + 63) >> 6; }
+        while (t >= end && b + 1 < a.B) { const int over = t - end; next_seq(a); t += over; }
     }
 };
 
@@ -466,11 +490,16 @@ struct Fp8Tile {
 
 // block scores of tile t of sequence b: one (lane 0) or, with 16-token blocks, up to four (lanes 0, 4, 8, 12)
 __device__ __forceinline__ void store_scores(const ScoreArgs& a, int b, int t, int L, int lane, float m) {
+    int j = -1;
     if (a.fine) {
         const int grp = lane >> 2;
-        if ((lane & 3) == 0 && grp < 4 && t * 64 + grp * 16 < L) a.scores[(int64_t)b * a.nb_stride + t * 4 + grp] = m;
+        if ((lane & 3) == 0 && grp < 4 && t * 64 + grp * 16 < L) j = t * 4 + grp;
     } else if (lane == 0) {
-        a.scores[(int64_t)b * a.nb_stride + t] = m;
+        j = t;
+    }
+    if (j >= 0) {
+        if (a.tagged) st_tagged_score(a.tagged + (int64_t)b * a.nb_stride + j, a.tag, m);
+        else a.scores[(int64_t)b * a.nb_stride + j] = m;
     }
 }
 
@@ -494,22 +523,23 @@ __global__ void __launch_bounds__((ScoreCfg<H, D_IDX, FMT>::THREADS), 1) score_d
         if (FMT == SPOT_SELK_BF16) tma_prefetch_desc(&tm_k);
     }
     __syncthreads();
+#ifdef SPOT_TRACE
+    SPOT_STAMP(a.sync, 0, 0);
+#endif
     pdl_wait();
     pdl_launch_dependents();
 
-    // this CTA's range of the flat (sequence, tile) list
-    long long total = 0;
-    for (int bb = 0; bb < a.B; ++bb) total += (seq_len_of(a, bb) + 63) >> 6;
-    const long long i0 = (long long)blockIdx.x * total / gridDim.x, i1 = (long long)(blockIdx.x + 1) * total / gridDim.x;
-    const int n_my = (int)(i1 - i0);
+    // this CTA's work list: its slice of every sequence, in sequence order
+    int n_my = 0;
+    {
+        TileCursor c;
+        c.first(a);
+        n_my = c.end - c.t;
+        while (c.b + 1 < a.B) { c.next_seq(a); n_my += c.end - c.t; }
+    }
     if (n_my <= 0) return;
     TileCursor cur;
-    cur.b = 0; cur.nb = (seq_len_of(a, 0) + 63) >> 6; cur.t = 0;
-    {
-        long long rem = i0;                       // (64-bit while locating the start only)
-        while (rem >= cur.nb && cur.b + 1 < a.B) { rem -= cur.nb; ++cur.b; cur.nb = (seq_len_of(a, cur.b) + 63) >> 6; }
-        cur.t = (int)rem;
-    }
+    cur.first(a);
 
     if constexpr (Cfg::SELF) {
         // ================================ self-serve consumers (4-bit) ================================
@@ -570,6 +600,7 @@ __global__ void __launch_bounds__((ScoreCfg<H, D_IDX, FMT>::THREADS), 1) score_d
     } else if (warp == SC_CONSUMERS) {
         // ================================ producer ================================
         if (lane == 0) {
+            cur.advance(a, 0);
             for (int i = 0; i < n_my; ++i) {
                 const int s = i % NS;
                 mbar_wait(bar_empty + 8 * s, ((i / NS) & 1) ^ 1);
@@ -595,7 +626,13 @@ __global__ void __launch_bounds__((ScoreCfg<H, D_IDX, FMT>::THREADS), 1) score_d
                 tile.load_query(a, cur_b, lane, q16_base + warp * (Cfg::ROW * 2 + 64));
             }
             const int s = i % NS;
+#ifdef SPOT_TRACE
+            if (warp == 0 && i == 0) SPOT_STAMP(a.sync, 6, 0);
+#endif
             mbar_wait(bar_full + 8 * s, (i / NS) & 1);
+#ifdef SPOT_TRACE
+            if (warp == 0 && i < 3 * SC_CONSUMERS) SPOT_STAMP(a.sync, 6, 1 + i / SC_CONSUMERS);
+#endif
             const float m = tile.tile_max(ring + s * Cfg::STAGE_BYTES, cur.t * 64, L, lane, fine);
             __syncwarp();
             if (lane == 0) mbar_arrive(bar_empty + 8 * s);
@@ -603,10 +640,17 @@ __global__ void __launch_bounds__((ScoreCfg<H, D_IDX, FMT>::THREADS), 1) score_d
             cur.advance(a, SC_CONSUMERS);
         }
     }
+#ifdef SPOT_TRACE
+    __syncthreads();
+    SPOT_STAMP(a.sync, 0, 2);
+#endif
 }
 
+// sync: hand-offs of a pipelined step (nullptr: none) -- `scores` is then the [B][nb_stride] array of tagged 64-bit words.
+// reserve_sms: SMs left to the selection CTAs that run beside this kernel.
 template <int H, int D_IDX, int FMT>
-spot_status launch_score_fmt(const spot_select_params* p, float* scores, int nb_stride, cudaStream_t s) {
+spot_status launch_score_fmt(const spot_select_params* p, float* scores, int nb_stride, const StepSync* sync, int reserve_sms,
+                             cudaStream_t s) {
     using Cfg = ScoreCfg<H, D_IDX, FMT>;
     ScoreArgs a;
     a.sel_q = p->sel_q; a.w = p->w; a.sel_k = (const uint8_t*)p->sel_k; a.tiles_per_seq = p->cache_stride_tokens / 64;
@@ -624,26 +668,36 @@ spot_status launch_score_fmt(const spot_select_params* p, float* scores, int nb_
     static unsigned long long smem_attr_done = 0;
     SPOT_CUDA_TRY(set_max_smem_once(score_decode_kernel<H, D_IDX, FMT>, Cfg::SMEM_BYTES, smem_attr_done));
     const int64_t max_tiles = (int64_t)p->B * ((p->max_seq_len + 63) / 64);
-    const int grid = (int)(max_tiles < sm_count() ? max_tiles : sm_count());
+    const int sms = sm_count() - reserve_sms > 0 ? sm_count() - reserve_sms : 1;
+    const int grid = (int)(max_tiles < sms ? max_tiles : sms);
+    a.tagged = nullptr; a.tag = 0;
+    if (sync && sync->tag) { a.tagged = reinterpret_cast<unsigned long long*>(scores); a.tag = sync->tag; a.scores = nullptr; }
+#ifdef SPOT_TRACE
+    memset(&a.sync, 0, sizeof(a.sync));
+    if (sync) a.sync = *sync;
+#endif
     SPOT_CUDA_TRY(launch_pdl(score_decode_kernel<H, D_IDX, FMT>, dim3((unsigned)grid), dim3(Cfg::THREADS),
                              (size_t)Cfg::SMEM_BYTES, s, tm, a));
     return SPOT_OK;
 }
 
 template <int H, int D_IDX>
-spot_status launch_score(const spot_select_params* p, float* scores, int nb_stride, cudaStream_t s) {
-    if (p->fmt == SPOT_SELK_BF16) return launch_score_fmt<H, D_IDX, SPOT_SELK_BF16>(p, scores, nb_stride, s);
-    if (p->fmt == SPOT_SELK_MXFP4) return launch_score_fmt<H, D_IDX, SPOT_SELK_MXFP4>(p, scores, nb_stride, s);
-    if (p->fmt == SPOT_SELK_FP8_E4M3) return launch_score_fmt<H, D_IDX, SPOT_SELK_FP8_E4M3>(p, scores, nb_stride, s);
-    return launch_score_fmt<H, D_IDX, SPOT_SELK_INT4_E4M3>(p, scores, nb_stride, s);
+spot_status launch_score(const spot_select_params* p, float* scores, int nb_stride, const StepSync* sync, int reserve_sms,
+                         cudaStream_t s) {
+    if (p->fmt == SPOT_SELK_BF16) return launch_score_fmt<H, D_IDX, SPOT_SELK_BF16>(p, scores, nb_stride, sync, reserve_sms, s);
+    if (p->fmt == SPOT_SELK_MXFP4) return launch_score_fmt<H, D_IDX, SPOT_SELK_MXFP4>(p, scores, nb_stride, sync, reserve_sms, s);
+    if (p->fmt == SPOT_SELK_FP8_E4M3)
+        return launch_score_fmt<H, D_IDX, SPOT_SELK_FP8_E4M3>(p, scores, nb_stride, sync, reserve_sms, s);
+    return launch_score_fmt<H, D_IDX, SPOT_SELK_INT4_E4M3>(p, scores, nb_stride, sync, reserve_sms, s);
 }
 
 }  // namespace
 
 // scores: fp32 [B][nb_stride]
-spot_status score_decode(const spot_select_params* p, float* scores, int nb_stride, cudaStream_t s) {
-    if (p->H_idx == 4 && p->d_idx == 64) return launch_score<4, 64>(p, scores, nb_stride, s);
-    if (p->H_idx == 4 && p->d_idx == 128) return launch_score<4, 128>(p, scores, nb_stride, s);
+spot_status score_decode(const spot_select_params* p, float* scores, int nb_stride, const StepSync* sync, int reserve_sms,
+                         cudaStream_t s) {
+    if (p->H_idx == 4 && p->d_idx == 64) return launch_score<4, 64>(p, scores, nb_stride, sync, reserve_sms, s);
+    if (p->H_idx == 4 && p->d_idx == 128) return launch_score<4, 128>(p, scores, nb_stride, sync, reserve_sms, s);
     return SPOT_ERR_UNSUPPORTED;
 }
 

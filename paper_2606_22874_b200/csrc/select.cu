@@ -6,14 +6,28 @@
 // at 8192 blocks per row went from 168.9 to 158.8 us; it is gone.)
 #include "select_common.cuh"
 
+#include <string.h>
+
 namespace spot {
 
 spot_status launch_select_hist(const SelectArgs& a, int rows, int max_nb, cudaStream_t s);    // select_hist.cu
 
+// sync (decode rows of a pipelined call): `scores` is then the scoring kernel's array of tagged 64-bit words, row stride
+// nb_stride, and the plain block scores go to p->block_scores (row stride p->nb_stride) if the caller wants them.
 spot_status run_select(const spot_select_params* p, const float* scores, int nb_stride, int rows_per_seq,
-                       int max_nb, cudaStream_t s) {
+                       int max_nb, const StepSync* sync, cudaStream_t s) {
     if (max_nb > SEL_MAX_NB) return SPOT_ERR_UNSUPPORTED;
     SelectArgs a;
+    memset(&a.sync, 0, sizeof(a.sync));
+    a.tagged = nullptr; a.tagged_stride = 0; a.scores_out = nullptr;
+    if (sync && sync->tag && p->q_block == 1) {
+        a.sync = *sync;
+        a.tagged = reinterpret_cast<unsigned long long*>(const_cast<float*>(scores));
+        a.tagged_stride = nb_stride;
+        a.scores_out = p->block_scores;
+        scores = nullptr;
+        nb_stride = p->nb_stride;              // rows of block_scores / block_probs
+    }
     a.scores = scores; a.nb_stride = nb_stride; a.seq_len = p->seq_len; a.max_len = p->max_seq_len; a.n_q = rows_per_seq;
     a.q_start = p->q_start; a.q_block = p->q_block; a.blk = p->blk;
     a.mode = p->mode; a.top_k = p->top_k; a.p = p->p; a.temperature = p->temperature;

@@ -33,6 +33,10 @@ struct SelectArgs {
     int cap;
     int32_t* budgets;
     float* probs;             // optional [rows][nb_stride]
+    StepSync sync;            // pipelined step (decode rows): publish ready[b]; tag == 0: plain stream order
+    unsigned long long* tagged;   // pipelined step: the scoring kernel's {tag, fp32 bits} words [rows][tagged_stride] (read
+    int tagged_stride;            //   until tagged, then cleared); block scores are copied to scores_out when it is set
+    float* scores_out;            // [rows][nb_stride] or nullptr
 };
 
 }  // namespace spot

@@ -91,19 +91,61 @@ __global__ void __launch_bounds__(SH_N / SH_E) select_hist_kernel(SelectArgs a) 
     const int row = blockIdx.x;
     const int b = row / a.n_q, i = row - b * a.n_q;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    pdl_wait();
-    pdl_launch_dependents();
-    // the row's scores are requested before seq_len is known (two independent DRAM misses instead of a chain)
-    const float* srow = a.scores + (int64_t)row * a.nb_stride;
+    const bool piped = a.sync.tag != 0u;
+    SPOT_STAMP(a.sync, 1, 0);
+    if (piped) pdl_launch_dependents();
+    // A pipelined call runs the body twice: first DRY, on a synthetic row with every global store off, while the row's
+    // block scores are still being produced -- this kernel's 45 KB of code (and the constants of the fp64 exp) come from
+    // DRAM, behind an HBM stream at full rate (the bench flushes L2 before every step), and a cold pass costs 15-20 us
+    // there against ~5 us from warm caches.  The selection CTA has its SM to itself and nothing else to do.
+#pragma unroll 1
+  for (int pass = piped ? 0 : 1; pass < 2; ++pass) {
+    const bool dry = pass == 0;
     float sraw[SH_E];
-#pragma unroll
-    for (int r = 0; r < SH_E; ++r) {
-        const int j = warp * (32 * SH_E) + lane + 32 * r;
-        sraw[r] = j < a.nb_stride ? srow[j] : 0.f;
-    }
     int n_b;
-    if (a.q_block == 1) n_b = (min(max(a.seq_len[b], 0), a.max_len) + a.blk - 1) / a.blk;
-    else n_b = (a.q_start + (i + 1) * a.q_block - 1) / a.blk + 1;
+    if (dry) {
+        n_b = min(SH_N, a.tagged_stride);
+#pragma unroll
+        for (int r = 0; r < SH_E; ++r) {
+            const uint32_t j = (uint32_t)(warp * (32 * SH_E) + lane + 32 * r);
+            sraw[r] = (float)((j * 2654435761u) >> 8) * (8.0f / 16777216.0f);      // scores spread over [0, 8)
+        }
+    } else if (piped) {
+        // pipelined step (decode rows): this CTA is resident BESIDE the scoring kernel and waits for its own sequence only
+        // -- every block score arrives as one {tag, fp32 bits} word; an entry is re-read until it carries this call's tag,
+        // then cleared (common.cuh, StepSync)
+        n_b = min((min(max(a.seq_len[b], 0), a.max_len) + a.blk - 1) / a.blk, SH_N);
+        unsigned long long* trow = a.tagged + (int64_t)row * a.tagged_stride;
+        unsigned long long v[SH_E];
+#pragma unroll
+        for (int r = 0; r < SH_E; ++r) {
+            const int j = warp * (32 * SH_E) + lane + 32 * r;
+            v[r] = j < n_b ? ld_tagged_score(trow + j) : ((unsigned long long)a.sync.tag << 32);
+        }
+#pragma unroll
+        for (int r = 0; r < SH_E; ++r) {
+            const int j = warp * (32 * SH_E) + lane + 32 * r;
+            while ((uint32_t)(v[r] >> 32) != a.sync.tag) { __nanosleep(256); v[r] = ld_tagged_score(trow + j); }
+            sraw[r] = __uint_as_float((uint32_t)v[r]);
+            if (j < n_b) {
+                trow[j] = (unsigned long long)(uint32_t)v[r];           // tag cleared: consumed
+                if (a.scores_out) a.scores_out[(int64_t)row * a.nb_stride + j] = sraw[r];
+            }
+        }
+        SPOT_STAMP(a.sync, 1, 1);
+    } else {
+        pdl_wait();
+        pdl_launch_dependents();
+        // the row's scores are requested before seq_len is known (two independent DRAM misses instead of a chain)
+        const float* srow = a.scores + (int64_t)row * a.nb_stride;
+#pragma unroll
+        for (int r = 0; r < SH_E; ++r) {
+            const int j = warp * (32 * SH_E) + lane + 32 * r;
+            sraw[r] = j < a.nb_stride ? srow[j] : 0.f;
+        }
+        if (a.q_block == 1) n_b = (min(max(a.seq_len[b], 0), a.max_len) + a.blk - 1) / a.blk;
+        else n_b = (a.q_start + (i + 1) * a.q_block - 1) / a.blk + 1;
+    }
     n_b = min(n_b, SH_N);
     const int sink_end = min(a.sink, n_b);
     const int rec_beg = max(sink_end, n_b - a.rec);     // residual blocks: [sink_end, rec_beg)
@@ -128,6 +170,7 @@ __global__ void __launch_bounds__(SH_N / SH_E) select_hist_kernel(SelectArgs a) 
     if (lane == 0) { s_wu[warp][0] = kmn; s_wu[warp][1] = kmx; }
     if (tid == 0) { s_nin = 0; s_tau = 0u; s_base = 0.0; }
     __syncthreads();
+    SPOT_STAMP(a.sync, 4, 0);
 #pragma unroll
     for (int w = 0; w < SH_WARPS; ++w) { kmn = min(kmn, s_wu[w][0]); kmx = max(kmx, s_wu[w][1]); }
 
@@ -168,6 +211,7 @@ __global__ void __launch_bounds__(SH_N / SH_E) select_hist_kernel(SelectArgs a) 
             }
         }
         __syncthreads();
+        SPOT_STAMP(a.sync, 4, 1);
         // ---- exclusive scan of the bin counts: thread t owns bins 8t .. 8t+7
         {
             uint32_t c[SH_E], run = 0;
@@ -197,6 +241,7 @@ __global__ void __launch_bounds__(SH_N / SH_E) select_hist_kernel(SelectArgs a) 
                 if (topp) s_e[pos] = e[r];
             }
         __syncthreads();
+        SPOT_STAMP(a.sync, 4, 2);
         // ---- what has to be resolved exactly: up to two queries against one bin each, run by ONE copy of the code
         //      query 0 (dual top-p, p < 1): the bin holding the cut of the running mass -> n*, tau
         //      query 1 (top-K, K_min floor): the key of rank n_take - 1
@@ -340,6 +385,7 @@ __global__ void __launch_bounds__(SH_N / SH_E) select_hist_kernel(SelectArgs a) 
         }
     }
     __syncthreads();
+    SPOT_STAMP(a.sync, 4, 3);
 
     // ---- index order: A = reserved or strictly better than tau (certainly selected), Tt = tied with tau
     constexpr int NSEG = SH_N / 32;                       // 32-block segments: (warp, register)
@@ -398,18 +444,30 @@ __global__ void __launch_bounds__(SH_N / SH_E) select_hist_kernel(SelectArgs a) 
         int pos = -1;
         if ((isA >> r) & 1u) pos = a_before + min(t_before, need);
         else if (((isT >> r) & 1u) && t_before < need) pos = a_before + t_before;
-        if (pos >= 0 && pos < a.cap) out[pos] = j;
+        if (pos >= 0 && pos < a.cap && !dry) out[pos] = j;
     }
-    for (int j = total_sel + tid; j < a.cap; j += SH_T) out[j] = -1;
-    if (tid == 0) a.budgets[row] = min(total_sel, a.cap);
+    if (!dry) {
+        for (int j = total_sel + tid; j < a.cap; j += SH_T) out[j] = -1;
+        if (tid == 0) a.budgets[row] = min(total_sel, a.cap);
+    }
 
-    if (a.probs) {
+    if (a.probs && !dry) {
         float* pr = a.probs + (int64_t)row * a.nb_stride;
         const double inv_total = total > 0.0 ? 1.0 / total : 0.0;
 #pragma unroll
         for (int r = 0; r < SH_E; ++r) {
             const int j = ebase + 32 * r;
             if (j < n_b) pr[j] = (float)(e[r] * inv_total);      // 0 on reserved blocks and in top-K mode
+        }
+    }
+    __syncthreads();                                  // (the shared arrays are reused by the next pass)
+  }
+    if (piped) {
+        __syncthreads();                              // the row's list, budget and probabilities are written
+        SPOT_STAMP(a.sync, 1, 2);
+        if (tid == 0) {
+            if (a.sync.ready) { __threadfence(); st_release_u32(a.sync.ready + b, a.sync.tag); }
+            pdl_wait();                               // completion of this grid implies completion of the scoring grid
         }
     }
 }

@@ -92,6 +92,50 @@ class DeviceDecode:
         return bf16_bits_to_f64(to_np_u16(out)), (None if lse is None else lse.cpu().numpy())
 
 
+    def step_params(self, cap=None, garbage=None, want_lse=True, **over):
+        """Parameter block of spot_decode_step (a1 + a2 + a3 in one call) over this workload, with every buffer it
+        needs kept alive on `self`.  garbage: byte value the workspaces are filled with first (they need not be
+        initialised)."""
+        import torch
+        wl, api = self.wl, self.api
+        kw = dict(mode=wl.mode, top_k=wl.top_k, p=wl.p, sink_blocks=wl.sink_blocks,
+                  recency_blocks=wl.recency_blocks, kmin_blocks=wl.kmin_blocks, temperature=wl.temperature)
+        kw.update(over)
+        cap = self.n_b_max if cap is None else cap
+        self.cap = cap
+        self.indices = torch.full((wl.B, cap), -7, dtype=torch.int32, device="cuda")
+        self.budgets = torch.full((wl.B,), -7, dtype=torch.int32, device="cuda")
+        self.out = torch.zeros((wl.B, wl.H_q, wl.D), dtype=torch.int16, device="cuda")
+        self.lse = torch.zeros((wl.B, wl.H_q), device="cuda") if want_lse else None
+
+        def ws(n):
+            t = torch.empty(max(n, 16), dtype=torch.uint8, device="cuda")
+            if garbage is not None:
+                t.fill_(garbage)
+            return t
+        sp = api.make_select_params(self.sel_q, self.w, self.sel_k, self.fmt, self.L_cap, self.seq_len,
+                                    self.max_seq_len, wl.B, 1, wl.H_idx, wl.d_idx, blk=wl.blk, q_block=1,
+                                    indices=self.indices, cap=cap, budgets=self.budgets, **kw)
+        self.ws_sel = ws(api.spot_select_workspace_bytes(sp))
+        sp.workspace, sp.workspace_bytes = self.ws_sel.data_ptr(), self.ws_sel.numel()
+        ap = api.make_attn_params(self.q, self.K, self.V, self.kv_strides, self.seq_len, self.max_seq_len, self.indices,
+                                  self.budgets, cap, wl.B, 1, wl.H_q, wl.H_kv, wl.D, blk=wl.blk, sm_scale=wl.sm_scale,
+                                  out=self.out, lse=self.lse, page_table=getattr(self, "page_table", None),
+                                  page_tokens=getattr(self, "page_tokens", 0))
+        self.ws_att = ws(api.spot_sparse_attn_decode_workspace_bytes(ap))
+        ap.workspace, ap.workspace_bytes = self.ws_att.data_ptr(), self.ws_att.numel()
+        dp = api.make_decode_step_params(sp, ap)
+        self.ws_step = ws(api.spot_decode_step_workspace_bytes(dp))
+        dp.workspace, dp.workspace_bytes = self.ws_step.data_ptr(), self.ws_step.numel()
+        return dp
+
+    def step_results(self):
+        import torch
+        torch.cuda.synchronize()
+        return (self.indices.cpu().numpy(), self.budgets.cpu().numpy(), bf16_bits_to_f64(to_np_u16(self.out)),
+                None if self.lse is None else self.lse.cpu().numpy())
+
+
 # ------------------------------------------------------------------------------------------------------
 # oracle side
 # ------------------------------------------------------------------------------------------------------

@@ -334,6 +334,8 @@ def test_decode_step_from_host_buffers(torch_cuda, packed):
     hp.sel_q_host, hp.w_host, hp.q_host = (h_in.data_ptr() + o for o in off_in)
     hp.out_host, hp.budgets_host = h_res.data_ptr() + off_res[0], h_res.data_ptr() + off_res[1]
     hp.select, hp.attn = sp, ap
+    ws3 = torch.empty(api.spot_decode_step_workspace_bytes(api.make_decode_step_params(sp, ap)), dtype=torch.uint8, device="cuda")
+    hp.step_workspace, hp.step_workspace_bytes = ws3.data_ptr(), ws3.numel()
     api.spot_decode_step_host(hp)
     torch.cuda.synchronize()
     out = bf16_bits_to_f64(h_res[off_res[0]:off_res[0] + n_out].numpy().view(np.uint16).reshape(B, Hq, D))
