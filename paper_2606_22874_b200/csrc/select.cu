@@ -19,7 +19,7 @@ spot_status run_select(const spot_select_params* p, const float* scores, int nb_
     if (max_nb > SEL_MAX_NB) return SPOT_ERR_UNSUPPORTED;
     SelectArgs a;
     memset(&a.sync, 0, sizeof(a.sync));
-    a.tagged = nullptr; a.tagged_stride = 0; a.scores_out = nullptr;
+    a.tagged = nullptr; a.tagged_stride = 0; a.scores_out = nullptr; a.dry_from_row = 0;
     if (sync && sync->tag && p->q_block == 1) {
         a.sync = *sync;
         a.tagged = reinterpret_cast<unsigned long long*>(const_cast<float*>(scores));
@@ -27,6 +27,12 @@ spot_status run_select(const spot_select_params* p, const float* scores, int nb_
         a.scores_out = p->block_scores;
         scores = nullptr;
         nb_stride = p->nb_stride;              // rows of block_scores / block_probs
+        // when do the scores of sequence b arrive?  ~4 us of ramp, then the cache streams at ~6.5 GB/ms; a dry pass
+        // takes ~12 us, so only rows that arrive later than that gain from one
+        const double bytes_per_seq = (double)p->max_seq_len * (double)spot_selector_k_bytes((spot_selk_format)p->fmt, 1, 64, p->H_idx, p->d_idx) / 64.0;
+        a.dry_from_row = p->B;
+        for (int b = 0; b < p->B; ++b)
+            if (4.0 + (b + 1) * bytes_per_seq / 6.5e6 >= 16.0) { a.dry_from_row = b; break; }
     }
     a.scores = scores; a.nb_stride = nb_stride; a.seq_len = p->seq_len; a.max_len = p->max_seq_len; a.n_q = rows_per_seq;
     a.q_start = p->q_start; a.q_block = p->q_block; a.blk = p->blk;

@@ -37,6 +37,7 @@ struct SelectArgs {
     unsigned long long* tagged;   // pipelined step: the scoring kernel's {tag, fp32 bits} words [rows][tagged_stride] (read
     int tagged_stride;            //   until tagged, then cleared); block scores are copied to scores_out when it is set
     float* scores_out;            // [rows][nb_stride] or nullptr
+    int dry_from_row;             // pipelined step: sequences >= this one warm the kernel's code with a dry pass first
 };
 
 }  // namespace spot

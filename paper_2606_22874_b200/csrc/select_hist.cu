@@ -96,10 +96,12 @@ __global__ void __launch_bounds__(SH_N / SH_E) select_hist_kernel(SelectArgs a) 
     if (piped) pdl_launch_dependents();
     // A pipelined call runs the body twice: first DRY, on a synthetic row with every global store off, while the row's
     // block scores are still being produced -- this kernel's 45 KB of code (and the constants of the fp64 exp) come from
-    // DRAM, behind an HBM stream at full rate (the bench flushes L2 before every step), and a cold pass costs 15-20 us
-    // there against ~5 us from warm caches.  The selection CTA has its SM to itself and nothing else to do.
+    // DRAM, behind an HBM stream at full rate (the bench flushes L2 before every step), and a cold pass costs 10-13 us
+    // there against 8-10 us from warm caches.  The selection CTA has its SM to itself and nothing else to do -- but only
+    // rows whose scores are still far off (dry_from_row, estimated on the host from the bytes in front of them) take it:
+    // a row that is ready before the dry pass ends would only wait for it.
 #pragma unroll 1
-  for (int pass = piped ? 0 : 1; pass < 2; ++pass) {
+  for (int pass = (piped && b >= a.dry_from_row) ? 0 : 1; pass < 2; ++pass) {
     const bool dry = pass == 0;
     float sraw[SH_E];
     int n_b;
@@ -171,8 +173,10 @@ __global__ void __launch_bounds__(SH_N / SH_E) select_hist_kernel(SelectArgs a) 
     if (tid == 0) { s_nin = 0; s_tau = 0u; s_base = 0.0; }
     __syncthreads();
     SPOT_STAMP(a.sync, 4, 0);
-#pragma unroll
-    for (int w = 0; w < SH_WARPS; ++w) { kmn = min(kmn, s_wu[w][0]); kmx = max(kmx, s_wu[w][1]); }
+    // (cross-warp combines: lane w reads warp w's word and the warp reduces -- a loop over the 32 warps in every thread
+    // was 40 % of this kernel's instructions, and with 32 warps per SM the kernel is issue-bound)
+    kmn = __reduce_min_sync(0xffffffffu, lane < SH_WARPS ? s_wu[lane][0] : 0xffffffffu);
+    kmx = __reduce_max_sync(0xffffffffu, lane < SH_WARPS ? s_wu[lane][1] : 0u);
 
     int n_take = 0;
     uint32_t tau = 0u;
@@ -185,7 +189,9 @@ __global__ void __launch_bounds__(SH_N / SH_E) select_hist_kernel(SelectArgs a) 
         bin_of.kmn = kmn;
         bin_of.scale = (float)SH_NBIN / ((float)(kmx - kmn) + 1.0f);
         // ---- masses (Eq. 7 numerators, fp64), bins, rank inside the bin
-        const double zmax = (double)key_score(kmn) / a.temperature;
+        // (x / 1.0 == x exactly: the default temperature, skips three fp64 divisions per thread)
+        const bool t_one = a.temperature == 1.0;
+        const double zmax = t_one ? (double)key_score(kmn) : (double)key_score(kmn) / a.temperature;
         // (one rolled loop -- the fp64 exp is ~150 instructions and this kernel runs once per step from a cold
         // instruction cache: code size, not instruction count, is what its latency is made of.  The arrays stay in
         // registers: every trip works on element 0 and rotates.)
@@ -200,7 +206,10 @@ __global__ void __launch_bounds__(SH_N / SH_E) select_hist_kernel(SelectArgs a) 
                 double ev = 0.0;
                 uint32_t pv = 0xffffffffu;
                 if (j >= sink_end && j < rec_beg) {
-                    if (topp) ev = exp((double)key_score(kq[0]) / a.temperature - zmax);
+                    if (topp) {
+                        const double x = (double)key_score(kq[0]);
+                        ev = exp((t_one ? x : x / a.temperature) - zmax);
+                    }
                     const int bn = bin_of(kq[0]);
                     pv = ((uint32_t)bn << PK_SHIFT) | atomicAdd(&s_cnt[bn], 1u);
                 }
@@ -226,8 +235,7 @@ __global__ void __launch_bounds__(SH_N / SH_E) select_hist_kernel(SelectArgs a) 
             if (lane == 31) s_wi[warp][0] = (int)inc;
             __syncthreads();
             uint32_t off = inc - run;
-#pragma unroll
-            for (int w = 0; w < SH_WARPS; ++w) off += (w < warp) ? (uint32_t)s_wi[w][0] : 0u;
+            off += __reduce_add_sync(0xffffffffu, (lane < SH_WARPS && lane < warp) ? (uint32_t)s_wi[lane][0] : 0u);
 #pragma unroll
             for (int u = 0; u < SH_E; ++u) { s_cnt[tid * SH_E + u] = off; off += c[u]; }
         }
@@ -265,10 +273,16 @@ __global__ void __launch_bounds__(SH_N / SH_E) select_hist_kernel(SelectArgs a) 
             if (lane == 31) s_wd[warp] = inc;
             __syncthreads();
             off = inc - run;
+            {
+                const double wv = lane < SH_WARPS ? s_wd[lane] : 0.0;
+                double before = lane < warp ? wv : 0.0, all = wv;
 #pragma unroll
-            for (int w = 0; w < SH_WARPS; ++w) {
-                if (w < warp) off += s_wd[w];
-                total += s_wd[w];
+                for (int o = 16; o; o >>= 1) {
+                    before += __shfl_xor_sync(0xffffffffu, before, o);
+                    all += __shfl_xor_sync(0xffffffffu, all, o);
+                }
+                off += before;
+                total = all;
             }
             target = a.p * total;
             int cnt = 0;
@@ -277,8 +291,7 @@ __global__ void __launch_bounds__(SH_N / SH_E) select_hist_kernel(SelectArgs a) 
             cnt = __reduce_add_sync(0xffffffffu, cnt);
             if (lane == 0) s_wi[warp][1] = cnt;
             __syncthreads();
-#pragma unroll
-            for (int w = 0; w < SH_WARPS; ++w) n_lt += s_wi[w][1];
+            n_lt = __reduce_add_sync(0xffffffffu, lane < SH_WARPS ? s_wi[lane][1] : 0);
             n_take = n_res;                                   // p >= 1: all of B_res by definition (R20)
         } else {
 #pragma unroll
@@ -323,8 +336,8 @@ __global__ void __launch_bounds__(SH_N / SH_E) select_hist_kernel(SelectArgs a) 
                 if (lane == 0) { s_wu[warp][0] = lo; s_wu[warp][1] = hi; }
                 if (tid == 0) s_nin = 0;
                 __syncthreads();
-#pragma unroll
-                for (int w = 0; w < SH_WARPS; ++w) { lo = min(lo, s_wu[w][0]); hi = max(hi, s_wu[w][1]); }
+                lo = __reduce_min_sync(0xffffffffu, lane < SH_WARPS ? s_wu[lane][0] : 0xffffffffu);
+                hi = __reduce_max_sync(0xffffffffu, lane < SH_WARPS ? s_wu[lane][1] : 0u);
                 if (lo == hi) {
                     // every key of the bin is the same: equal masses, ranked by position -> arithmetic
                     if (tid == 0) {
@@ -467,7 +480,9 @@ __global__ void __launch_bounds__(SH_N / SH_E) select_hist_kernel(SelectArgs a) 
         SPOT_STAMP(a.sync, 1, 2);
         if (tid == 0) {
             if (a.sync.ready) { __threadfence(); st_release_u32(a.sync.ready + b, a.sync.tag); }
-            pdl_wait();                               // completion of this grid implies completion of the scoring grid
+            // completion of this grid implies completion of the scoring grid -- through its LAST CTA alone: the others
+            // must leave their SM to the selection CTAs queued behind them (B > SMs left to this kernel)
+            if (blockIdx.x == gridDim.x - 1) pdl_wait();
         }
     }
 }
