@@ -108,6 +108,13 @@ __global__ void __launch_bounds__(ATT_WARPS * 32, 2) attn_decode_kernel(AttnArgs
     const int G = a.G;
     const bool piped = a.sync.tag != 0u;
     SPOT_STAMP(a.sync, 2, 0);
+#ifdef SPOT_TRACE
+    if (a.sync.trace && threadIdx.x == 0 && blockIdx.x < 512) {
+        unsigned sm;
+        asm volatile("mov.u32 %0, %%smid;" : "=r"(sm));
+        a.sync.trace[((size_t)7 * 512 + blockIdx.x) * 4] = sm;
+    }
+#endif
     if (piped) {
         pdl_launch_dependents();                     // (the index lists are awaited sequence by sequence below)
     } else {

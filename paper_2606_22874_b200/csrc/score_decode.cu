@@ -133,8 +133,13 @@ struct ScoreCfg {
     static constexpr int STAGES = CONSUMERS * PER_WARP;
     static constexpr int THREADS = (CONSUMERS + (SELF ? 0 : 1)) * 32;
     static_assert(STAGES * STAGE_BYTES <= 208 * 1024, "ring geometry");
-    static constexpr int Q16_BYTES = SELF ? CONSUMERS * (ROW * 2 + 64) : 0;
-    static constexpr int SMEM_BYTES = 1024 + STAGES * STAGE_BYTES + 2 * STAGES * 8 + Q16_BYTES + 64;
+    // query slots: one per sequence when the batch has at most Q_SLOTS of them (staged once, at kernel start), else one
+    // per consumer warp (restaged whenever the warp changes sequence)
+    static constexpr int Q_SLOTS = 16;
+    static constexpr int Q_SLOT_BYTES = ROW * 2 + 64;
+    static constexpr int Q16_BYTES = Q_SLOTS * Q_SLOT_BYTES;
+    static_assert(CONSUMERS <= Q_SLOTS, "a slot per consumer warp");
+    static constexpr int SMEM_BYTES = 256 + 1024 + STAGES * STAGE_BYTES + 2 * STAGES * 8 + Q16_BYTES + 64;
 };
 
 struct ScoreArgs {
@@ -148,6 +153,7 @@ struct ScoreArgs {
     float* scores;
     int nb_stride;
     int fine;                     // blk == 16: four block maxima per 64-token tile (f3)
+    int n_groups;                 // the batch is scored in this many groups of consecutive sequences (TileCursor)
     unsigned long long* tagged;   // pipelined step: block scores go out as {tag, fp32 bits} words, [B][nb_stride]
     uint32_t tag;                 //   (nullptr: plain fp32 into `scores`)
 #ifdef SPOT_TRACE
@@ -158,31 +164,71 @@ struct ScoreArgs {
 // seq_len[b] as the kernels use it: clamped to what the grid, the score rows and the cache were sized for
 __device__ __forceinline__ int seq_len_of(const ScoreArgs& a, int b) { return min(max(a.seq_len[b], 0), a.max_len); }
 
-__device__ __forceinline__ int tiles_of(const ScoreArgs& a, int b) { return (seq_len_of(a, b) + 63) >> 6; }
+// tiles of sequence b.  The kernel copies the (clamped) tile counts of the first SC_NB_CACHE sequences into shared memory
+// once, in one coalesced load: the cursors below consult them on every change of sequence, and a chain of dependent
+// global loads in front of the first tile request is what a short kernel cannot afford.
+constexpr int SC_NB_CACHE = 64;
+__device__ __forceinline__ int tiles_of(const ScoreArgs& a, int b) {
+    extern __shared__ unsigned char smem_raw[];
+    if (b < SC_NB_CACHE) return reinterpret_cast<const int*>(smem_raw)[b];
+    return (seq_len_of(a, b) + 63) >> 6;
+}
 
-// Work assignment: CTA c of n owns an n-th of EVERY sequence's tiles and walks its slices sequence by sequence -- so
-// the whole grid finishes sequence 0 first, then 1, ..: the selection of a sequence (another kernel, resident beside
-// this one) overlaps the scoring of the next ones.  Sequence b's tiles are cut into n slices [c' nb_b / n,
-// (c' + 1) nb_b / n) and slice c' goes to CTA (c' + off_b) mod n with off_b the number of tiles in front of the sequence:
-// with sequences shorter than n tiles the non-empty slices of consecutive sequences then land on consecutive CTAs instead
-// of on the same few.  The CTA's work list is the concatenation of its slices; the cursor names a position in it.
+// Work assignment.  The batch is cut into n_groups groups of consecutive sequences (4, or B if smaller) and the whole grid
+// walks them group by group -- so the block scores of group 0 are complete a quarter into the kernel, and the selection
+// of its sequences (another kernel, resident beside this one) overlaps the scoring of the later groups.  Inside a group
+// the CTAs split the flat (sequence, tile) list into equal CONTIGUOUS ranges, so a warp changes sequence (and reloads
+// its query fragments: expensive for the quantised formats) about once per group, not once per tile.  Range c' of group
+// g goes to CTA (c' + off_g) mod n with off_g the number of tiles in front of the group: with groups shorter than n tiles
+// the non-empty ranges of consecutive groups land on consecutive CTAs instead of on the same few.
+// The CTA's work list is the concatenation of its ranges; the cursor names a position in it.  The ranges (64-bit
+// divisions) are worked out once per CTA into shared memory -- walking them costs a few integer instructions per tile,
+// in kernels whose 4-bit forms are issue-bound.
+constexpr int SC_MAX_GROUPS = 4;
+struct CtaRange { int b0, t0, len; };             // first sequence, first tile of it, tiles in the range
+// (thread g works out group g; 32-bit arithmetic -- a 64-bit division is a ~100-instruction dependent chain, and this
+// sits in front of the first tile request: floor(rot T / n) = rot (T / n) + floor(rot (T % n) / n), all below 2^32 for
+// n < 65536 CTAs and fewer than 2^32 / n tiles per group... the batch total is what must stay below 2^32 tiles)
+__device__ __forceinline__ void cta_range_of_group(const ScoreArgs& a, int g, CtaRange* out) {
+    const uint32_t n = gridDim.x;
+    const int b0 = (int)((long long)g * a.B / a.n_groups), b1 = (int)((long long)(g + 1) * a.B / a.n_groups);
+    uint32_t before = 0, T = 0;
+    for (int bb = 0; bb < b0; ++bb) before += (uint32_t)tiles_of(a, bb);
+    for (int bb = b0; bb < b1; ++bb) T += (uint32_t)tiles_of(a, bb);
+    const uint32_t rot = (blockIdx.x + n - before % n) % n;          // which range of the group is this CTA's
+    const uint32_t q = T / n, r = T - q * n;
+    uint32_t i0 = rot * q + rot * r / n;
+    const uint32_t i1 = (rot + 1) * q + (rot + 1) * r / n;
+    out[g].len = (int)(i1 - i0);
+    int b = b0;
+    if (i1 > i0) {
+        uint32_t nb = (uint32_t)tiles_of(a, b);
+        while (i0 >= nb) { i0 -= nb; ++b; nb = (uint32_t)tiles_of(a, b); }
+    }
+    out[g].b0 = b;
+    out[g].t0 = (int)i0;
+}
 struct TileCursor {
-    int b, t, end;                // tile t of sequence b; this CTA's slice of sequence b ends at `end`
-    int rot;                      // (blockIdx.x - off_b) mod n: which slice of sequence b is this CTA's
-    __device__ __forceinline__ void slice(const ScoreArgs& a) {
-        const long long nb = tiles_of(a, b);
-        t = (int)((long long)rot * nb / gridDim.x);
-        end = (int)((long long)(rot + 1) * nb / gridDim.x);
+    int b, t, nb;                 // tile t of sequence b, which has nb tiles
+    int left;                     // tiles of this CTA's range of group g at or after the cursor (<= 0: past the end)
+    int g;
+    // place the cursor `skip` tiles past the start of group gg's range, moving on to later groups as needed
+    __device__ __forceinline__ void enter(const ScoreArgs& a, const CtaRange* rng, int gg, int skip) {
+        g = gg;
+        while (g < a.n_groups && skip >= rng[g].len) { skip -= rng[g].len; ++g; }
+        if (g >= a.n_groups) { left = 0; return; }
+        left = rng[g].len - skip;
+        b = rng[g].b0; t = rng[g].t0 + skip; nb = tiles_of(a, b);
+        while (t >= nb) { t -= nb; ++b; nb = tiles_of(a, b); }
     }
-    __device__ __forceinline__ void first(const ScoreArgs& a) { b = 0; rot = blockIdx.x; slice(a); }
-    __device__ __forceinline__ void next_seq(const ScoreArgs& a) {
-        rot = (int)((rot + (long long)gridDim.x - tiles_of(a, b) % (int)gridDim.x) % gridDim.x);
-        ++b;
-        slice(a);
-    }
-    __device__ __forceinline__ void advance(const ScoreArgs& a, int n) {
-        t += n;
-        while (t >= end && b + 1 < a.B) { const int over = t - end; next_seq(a); t += over; }
+    __device__ __forceinline__ void first(const ScoreArgs& a, const CtaRange* rng) { enter(a, rng, 0, 0); }
+    __device__ __forceinline__ void advance(const ScoreArgs& a, const CtaRange* rng, int n) {
+        if (n < left) {
+            left -= n; t += n;
+            while (t >= nb) { t -= nb; ++b; nb = tiles_of(a, b); }
+            return;
+        }
+        if (left > 0) enter(a, rng, g + 1, n - left);
     }
 };
 
@@ -212,9 +258,19 @@ struct Bf16Tile {
     uint32_t qf[NP][4][2];
     float wh[H];
 
-    __device__ __forceinline__ void load_query(const ScoreArgs& a, int b, int lane, uint32_t) {
+    // slot: ROW BF16 (the query as it is) + H floats (w)
+    static __device__ __forceinline__ void stage(const ScoreArgs& a, int b, int lane, uint32_t slot) {
+        constexpr int ROW = H * D_IDX;
+        uint16_t* dst = reinterpret_cast<uint16_t*>(__cvta_shared_to_generic((size_t)slot));
+        const uint4* src = reinterpret_cast<const uint4*>(a.sel_q + (int64_t)b * ROW);
+        for (int i = lane; i < ROW / 8; i += 32) reinterpret_cast<uint4*>(dst)[i] = src[i];
+        if (lane < H) reinterpret_cast<float*>(dst + ROW)[lane] = a.w[(int64_t)b * H + lane];
+        __syncwarp();
+    }
+    __device__ __forceinline__ void fetch(int lane, uint32_t slot) {
+        constexpr int ROW = H * D_IDX;
         const int g = lane >> 2, c = lane & 3;
-        const uint16_t* q = a.sel_q + (int64_t)b * (H * D_IDX);
+        const uint16_t* q = reinterpret_cast<const uint16_t*>(__cvta_shared_to_generic((size_t)slot));
 #pragma unroll
         for (int pl = 0; pl < NP; ++pl)
 #pragma unroll
@@ -223,7 +279,7 @@ struct Bf16Tile {
                 qf[pl][ks][1] = (g == 0) ? *reinterpret_cast<const uint32_t*>(q + pl * 64 + ks * 16 + 8 + 2 * c) : 0u;
             }
 #pragma unroll
-        for (int h = 0; h < H; ++h) wh[h] = a.w[(int64_t)b * H + h];
+        for (int h = 0; h < H; ++h) wh[h] = reinterpret_cast<const float*>(q + ROW)[h];
     }
 
     // max over the tile's valid tokens of s[t]; valid on every lane after the final shuffles
@@ -273,9 +329,8 @@ struct Q4Tile {
     uint32_t qf[NQL][16];
     float wq[NQL], ps[NQL];
 
-    // q16: this warp's shared scratch, ROW halfs + H floats
-    __device__ __forceinline__ void load_query(const ScoreArgs& a, int b, int lane, uint32_t q16_addr) {
-        const int g = lane >> 2, c = lane & 3;
+    // slot: ROW halfs (the pre-scaled fp16 query) + H floats (power-of-two post-scales) + H floats (w)
+    static __device__ __forceinline__ void stage(const ScoreArgs& a, int b, int lane, uint32_t q16_addr) {
         __half* q16 = reinterpret_cast<__half*>(__cvta_shared_to_generic((size_t)q16_addr));
         float* post = reinterpret_cast<float*>(q16 + ROW);
         // fp16 copy of q, pre-scaled per head by 2^sh so that the head's largest element lands in [2^14, 2^15).
@@ -305,7 +360,13 @@ struct Q4Tile {
 #pragma unroll
         for (int i = 0; i < EPL; ++i) q16[lane * EPL + i] = __float2half_rn(v[i] * up);
         if (lane % LPH == 0) post[lane / LPH] = __uint_as_float((uint32_t)(127 - sh) << 23);
+        if (lane < H) post[H + lane] = a.w[(int64_t)b * H + lane];
         __syncwarp();
+    }
+    __device__ __forceinline__ void fetch(int lane, uint32_t q16_addr) {
+        const int g = lane >> 2, c = lane & 3;
+        const __half* q16 = reinterpret_cast<const __half*>(__cvta_shared_to_generic((size_t)q16_addr));
+        const float* post = reinterpret_cast<const float*>(q16 + ROW);
         // B fragments: column n of the MMA is the group held by quad-lane c == n; only lane (g == n, c == n) is non-zero
 #pragma unroll
         for (int ql = 0; ql < NQL; ++ql) {
@@ -321,10 +382,9 @@ struct Q4Tile {
 #pragma unroll
         for (int ql = 0; ql < NQL; ++ql) {
             const int head = (4 * ql + 2 * (c & 1)) / GPH;
-            wq[ql] = a.w[(int64_t)b * H + head];
+            wq[ql] = post[H + head];
             ps[ql] = post[head];
         }
-        __syncwarp();
     }
 
     // maximum over the NIT * 16 tokens of a slice whose codes start at shared address st and whose scale bytes follow
@@ -398,8 +458,7 @@ struct Fp8Tile {
     uint32_t qf[NQL][8];
     float wq[H], ps[H];
 
-    __device__ __forceinline__ void load_query(const ScoreArgs& a, int b, int lane, uint32_t q16_addr) {
-        const int g = lane >> 2, c = lane & 3;
+    static __device__ __forceinline__ void stage(const ScoreArgs& a, int b, int lane, uint32_t q16_addr) {
         __half* q16 = reinterpret_cast<__half*>(__cvta_shared_to_generic((size_t)q16_addr));
         float* post = reinterpret_cast<float*>(q16 + ROW);
         constexpr int EPL = ROW / 32, LPH = 32 / H;
@@ -428,7 +487,13 @@ struct Fp8Tile {
 #pragma unroll
         for (int i = 0; i < EPL; ++i) q16[lane * EPL + i] = __float2half_rn(v[i] * up);
         if (lane % LPH == 0) post[lane / LPH] = __uint_as_float((uint32_t)(127 - sh) << 23);
+        if (lane < H) post[H + lane] = a.w[(int64_t)b * H + lane];
         __syncwarp();
+    }
+    __device__ __forceinline__ void fetch(int lane, uint32_t q16_addr) {
+        const int g = lane >> 2, c = lane & 3;
+        const __half* q16 = reinterpret_cast<const __half*>(__cvta_shared_to_generic((size_t)q16_addr));
+        const float* post = reinterpret_cast<const float*>(q16 + ROW);
 #pragma unroll
         for (int ql = 0; ql < NQL; ++ql)
 #pragma unroll
@@ -438,8 +503,7 @@ struct Fp8Tile {
                 qf[ql][2 * j + 1] = (g == 0) ? src[1] : 0u;
             }
 #pragma unroll
-        for (int h = 0; h < H; ++h) { wq[h] = a.w[(int64_t)b * H + h]; ps[h] = post[h]; }
-        __syncwarp();
+        for (int h = 0; h < H; ++h) { wq[h] = post[H + h]; ps[h] = post[h]; }
     }
 
     static __device__ __forceinline__ void e4m3x4_to_f16x2x2(uint32_t w, uint32_t& lo, uint32_t& hi) {
@@ -510,7 +574,8 @@ __global__ void __launch_bounds__((ScoreCfg<H, D_IDX, FMT>::THREADS), 1) score_d
     constexpr int NS = Cfg::STAGES;
     constexpr int SC_CONSUMERS = Cfg::CONSUMERS;
     extern __shared__ unsigned char smem_raw[];
-    const uint32_t ring = (smem_u32(smem_raw) + 1023u) & ~1023u;
+    // [0, 256): tile counts of the first 64 sequences (tiles_of); then the ring, 1024-byte aligned
+    const uint32_t ring = (smem_u32(smem_raw) + 256u + 1023u) & ~1023u;
     const uint32_t bar_full = ring + NS * Cfg::STAGE_BYTES;        // [NS]
     const uint32_t bar_empty = bar_full + NS * 8;                  // [NS]
     const uint32_t q16_base = bar_empty + NS * 8;
@@ -529,25 +594,43 @@ __global__ void __launch_bounds__((ScoreCfg<H, D_IDX, FMT>::THREADS), 1) score_d
     pdl_wait();
     pdl_launch_dependents();
 
-    // this CTA's work list: its slice of every sequence, in sequence order
+    // this CTA's work list: its range of every group, in group order
+    __shared__ CtaRange s_rng[SC_MAX_GROUPS];
+    if (threadIdx.x < SC_NB_CACHE && (int)threadIdx.x < a.B)
+        reinterpret_cast<int*>(smem_raw)[threadIdx.x] = (seq_len_of(a, threadIdx.x) + 63) >> 6;
+    __syncthreads();
+    if ((int)threadIdx.x < a.n_groups) cta_range_of_group(a, threadIdx.x, s_rng);
+    __syncthreads();
     int n_my = 0;
-    {
-        TileCursor c;
-        c.first(a);
-        n_my = c.end - c.t;
-        while (c.b + 1 < a.B) { c.next_seq(a); n_my += c.end - c.t; }
-    }
+    for (int gg = 0; gg < a.n_groups; ++gg) n_my += s_rng[gg].len;
     if (n_my <= 0) return;
     TileCursor cur;
-    cur.first(a);
+    cur.first(a, s_rng);
+    // queries: staged once per CTA when every sequence has a slot (ScoreCfg), else per warp on every change of sequence.
+    // The staging runs AFTER the first tile requests are out (below) and ends on a barrier of the consumer warps only.
+    using TileT = typename std::conditional<FMT == SPOT_SELK_BF16, Bf16Tile<H, D_IDX>,
+                  typename std::conditional<FMT == SPOT_SELK_FP8_E4M3, Fp8Tile<H, D_IDX>, Q4Tile<H, D_IDX, FMT>>::type>::type;
+    const bool q_staged = a.B <= Cfg::Q_SLOTS;
+    auto stage_queries = [&]() {
+        if (!q_staged) return;
+        for (int bb = warp; bb < a.B; bb += SC_CONSUMERS) TileT::stage(a, bb, lane, q16_base + bb * Cfg::Q_SLOT_BYTES);
+        asm volatile("bar.sync 1, %0;" :: "n"(SC_CONSUMERS * 32) : "memory");
+    };
+    auto take_query = [&](TileT& tile, int bb) {
+        if (q_staged) { tile.fetch(lane, q16_base + bb * Cfg::Q_SLOT_BYTES); return; }
+        __syncwarp();
+        TileT::stage(a, bb, lane, q16_base + warp * Cfg::Q_SLOT_BYTES);
+        tile.fetch(lane, q16_base + warp * Cfg::Q_SLOT_BYTES);
+        __syncwarp();
+    };
 
     if constexpr (Cfg::SELF) {
         // ================================ self-serve consumers (4-bit) ================================
         // warp w streams tiles w, w + C, w + 2C, ... through its own stages w*K .. w*K + K-1
         // (a stage holds one of the SP slices of a tile; SP == 1 for the 4-bit formats)
         constexpr int K = Cfg::PER_WARP, SP = Cfg::SPLIT;
-        typename std::conditional<FMT == SPOT_SELK_FP8_E4M3, Fp8Tile<H, D_IDX>, Q4Tile<H, D_IDX, FMT>>::type tile;
-        cur.advance(a, warp);
+        TileT tile;
+        cur.advance(a, s_rng, warp);
         TileCursor nxt = cur;                      // the tile of the next slice to request
         const int n_w = (n_my - warp + SC_CONSUMERS - 1) / SC_CONSUMERS;     // tiles of this warp
         const int n_q = n_w * SP;                  // slices of this warp
@@ -571,17 +654,18 @@ __global__ void __launch_bounds__((ScoreCfg<H, D_IDX, FMT>::THREADS), 1) score_d
                               bar_full + 8 * s);
                 }
             }
-            if (rq % SP == SP - 1) nxt.advance(a, SC_CONSUMERS);
+            if (rq % SP == SP - 1) nxt.advance(a, s_rng, SC_CONSUMERS);
             ++rq;
         };
 #pragma unroll
         for (int j = 0; j < K; ++j) request_next();
+        stage_queries();
         int cur_b = -1, L = 0;
         for (int j = 0; j < n_w; ++j) {
             if (cur.b != cur_b) {
                 cur_b = cur.b;
                 L = seq_len_of(a, cur_b);
-                tile.load_query(a, cur_b, lane, q16_base + warp * (Cfg::ROW * 2 + 64));
+                take_query(tile, cur_b);
             }
             float m = -INFINITY;
 #pragma unroll
@@ -595,12 +679,11 @@ __global__ void __launch_bounds__((ScoreCfg<H, D_IDX, FMT>::THREADS), 1) score_d
                 request_next();
             }
             store_scores(a, cur_b, cur.t, L, lane, m);
-            cur.advance(a, SC_CONSUMERS);
+            cur.advance(a, s_rng, SC_CONSUMERS);
         }
     } else if (warp == SC_CONSUMERS) {
         // ================================ producer ================================
         if (lane == 0) {
-            cur.advance(a, 0);
             for (int i = 0; i < n_my; ++i) {
                 const int s = i % NS;
                 mbar_wait(bar_empty + 8 * s, ((i / NS) & 1) ^ 1);
@@ -611,19 +694,20 @@ __global__ void __launch_bounds__((ScoreCfg<H, D_IDX, FMT>::THREADS), 1) score_d
                     bulk_load(ring + s * Cfg::STAGE_BYTES,
                               a.sel_k + ((int64_t)cur.b * a.tiles_per_seq + cur.t) * Cfg::TILE_BYTES, Cfg::TILE_BYTES,
                               bar_full + 8 * s);
-                cur.advance(a, 1);
+                cur.advance(a, s_rng, 1);
             }
         }
     } else {
         // ================================ consumers ================================
-        Bf16Tile<H, D_IDX> tile;
-        cur.advance(a, warp);
+        TileT tile;
+        cur.advance(a, s_rng, warp);
+        stage_queries();
         int cur_b = -1, L = 0;
         for (int i = warp; i < n_my; i += SC_CONSUMERS) {
             if (cur.b != cur_b) {
                 cur_b = cur.b;
                 L = seq_len_of(a, cur_b);
-                tile.load_query(a, cur_b, lane, q16_base + warp * (Cfg::ROW * 2 + 64));
+                take_query(tile, cur_b);
             }
             const int s = i % NS;
 #ifdef SPOT_TRACE
@@ -637,7 +721,7 @@ __global__ void __launch_bounds__((ScoreCfg<H, D_IDX, FMT>::THREADS), 1) score_d
             __syncwarp();
             if (lane == 0) mbar_arrive(bar_empty + 8 * s);
             store_scores(a, cur_b, cur.t, L, lane, m);
-            cur.advance(a, SC_CONSUMERS);
+            cur.advance(a, s_rng, SC_CONSUMERS);
         }
     }
 #ifdef SPOT_TRACE
@@ -654,7 +738,7 @@ spot_status launch_score_fmt(const spot_select_params* p, float* scores, int nb_
     using Cfg = ScoreCfg<H, D_IDX, FMT>;
     ScoreArgs a;
     a.sel_q = p->sel_q; a.w = p->w; a.sel_k = (const uint8_t*)p->sel_k; a.tiles_per_seq = p->cache_stride_tokens / 64;
-    a.seq_len = p->seq_len; a.max_len = p->max_seq_len; a.B = p->B; a.scores = scores; a.nb_stride = nb_stride; a.fine = p->blk == 16;
+    a.seq_len = p->seq_len; a.max_len = p->max_seq_len; a.B = p->B; a.n_groups = p->B < 4 ? p->B : 4; a.scores = scores; a.nb_stride = nb_stride; a.fine = p->blk == 16;
     CUtensorMap tm;
     memset(&tm, 0, sizeof(tm));
     if (FMT == SPOT_SELK_BF16) {

@@ -30,9 +30,14 @@ spot_status run_select(const spot_select_params* p, const float* scores, int nb_
         // when do the scores of sequence b arrive?  ~4 us of ramp, then the cache streams at ~6.5 GB/ms; a dry pass
         // takes ~12 us, so only rows that arrive later than that gain from one
         const double bytes_per_seq = (double)p->max_seq_len * (double)spot_selector_k_bytes((spot_selk_format)p->fmt, 1, 64, p->H_idx, p->d_idx) / 64.0;
+        // (the scoring grid walks the batch in min(B, 4) groups of consecutive sequences; a group's scores are complete
+        // when the grid leaves it)
+        const int n_groups = p->B < 4 ? p->B : 4;
         a.dry_from_row = p->B;
-        for (int b = 0; b < p->B; ++b)
-            if (4.0 + (b + 1) * bytes_per_seq / 6.5e6 >= 16.0) { a.dry_from_row = b; break; }
+        for (int g = 0; g < n_groups; ++g) {
+            const int b_end = (int)((long long)(g + 1) * p->B / n_groups);
+            if (4.0 + b_end * bytes_per_seq / 6.5e6 >= 16.0) { a.dry_from_row = (int)((long long)g * p->B / n_groups); break; }
+        }
     }
     a.scores = scores; a.nb_stride = nb_stride; a.seq_len = p->seq_len; a.max_len = p->max_seq_len; a.n_q = rows_per_seq;
     a.q_start = p->q_start; a.q_block = p->q_block; a.blk = p->blk;
