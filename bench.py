@@ -161,6 +161,57 @@ def max_over_ranks(value, device, world):
     return float(t.item())
 
 
+
+def traffic_entry(key):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch from profiles/traffic.json (ncu --set full captures named in
+    profiles/traffic.json.md), or None when that kernel / workload has not been captured."""
+    tpath = os.path.join(ROOT, "profiles", "traffic.json")
+    if os.path.exists(tpath):
+        with open(tpath) as f:
+            return json.load(f).get(key)
+    return None
+
+
+def prefill_gemm_roofline(dev, steps, warmup, clocks_index):
+    """BASELINE.json's second target, in the default run: the chunked-prefill selector GEMM of config 5 (a1', L = 65536,
+    one chunk, BF16 4 x 64) timed ALONE through spot_score_blocks -> fraction of the measured BF16 tensor peak."""
+    import torch
+    from paper_2606_22874_b200 import api
+    from workloads import make_prefill_workload
+    L = 65536
+    wl = make_prefill_workload(seed=5005, L=L, with_kv=False)
+    n_qb = L // 64
+    sel_q = torch.from_numpy(wl.sel_q.view(np.int16)).to(dev)
+    w = torch.from_numpy(wl.w).to(dev)
+    sel_k = torch.from_numpy(wl.sel_k.view(np.int16)).to(dev)
+    nb_stride = (n_qb + 3) & ~3
+    scores = torch.empty((n_qb, nb_stride), dtype=torch.float32, device=dev)
+    sp = api.make_select_params(sel_q, w, sel_k, "bf16", L, None, 0, 1, L, wl.H_idx, wl.d_idx, q_start=0, blk=64,
+                                q_block=64, block_scores=scores, nb_stride=nb_stride)
+    stream = torch.cuda.current_stream()
+    flush = torch.empty(512 << 20, dtype=torch.uint8, device=dev).zero_()
+    ts = []
+    with ClockSampler(clocks_index) as clk:
+        for i in range(steps + warmup):
+            flush.view(torch.int64).sum()
+            a_, b_ = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a_.record(stream)
+            api.spot_score_blocks(sp, stream)
+            b_.record(stream)
+            torch.cuda.synchronize()
+            if i >= warmup:
+                ts.append(a_.elapsed_time(b_))
+    burst, sustained, peak_src = tensor_peaks()
+    tiles = n_qb * (n_qb + 1) // 2
+    flop = 2.0 * 64 * 64 * wl.d_idx * wl.H_idx * tiles
+    achieved = flop / (float(np.mean(ts)) * 1e-3) / 1e12
+    return {"bound": "tensor", "kernel": "score_prefill_kernel", "workload": "cfg5 (L=65536, one chunk, selector 4x64 bf16)",
+            "ms": float(np.mean(ts)), "achieved": achieved, "peak": burst, "unit": "TFLOP/s", "frac": achieved / burst,
+            "frac_of_sustained": achieved / sustained, "algorithmic_flops": flop,
+            "traffic": traffic_entry("cfg5/bf16/score_prefill_kernel"), "peak_source": peak_src,
+            "launches": steps, "clocks": clk.summary()}
+
+
 # ------------------------------------------------------------------------------------------------------
 def run_ours(args):
     import ctypes as C
@@ -366,17 +417,64 @@ def run_ours(args):
         return
 
     peak, peak_src = measured_peaks()
-    bytes_per_tok = {"bf16": wl.H_idx * wl.d_idx * 2, "fp8_e4m3": wl.H_idx * wl.d_idx}.get(
-        args.fmt, wl.H_idx * wl.d_idx // 2 + wl.H_idx * wl.d_idx // 32)
+
+    def bytes_per_token(fmt):
+        return {"bf16": wl.H_idx * wl.d_idx * 2, "fp8_e4m3": wl.H_idx * wl.d_idx}.get(
+            fmt, wl.H_idx * wl.d_idx // 2 + wl.H_idx * wl.d_idx // 32)
+
+    # config 3's own subject, in the default run: the same step with the selector K-cache quantised (INT4 + E4M3 scale,
+    # MXFP4), beside the BF16 control above; and BASELINE.json's second target, the prefill selector GEMM, timed alone
+    formats, prefill_roofline = None, None
+    if args.extras and args.fmt == "bf16" and args.workload == "cfg3" and not args.paged and wl.blk == 64:
+        formats = {"bf16": {"us": step_mean * 1e3, "selector_cache_bytes": int(sel_bytes), "bytes_per_token": bytes_per_token("bf16")}}
+        for fmt in ("mxfp4", "int4_e4m3"):
+            n_f = max(3, min(args.steps, 10))
+            sel_k_f = torch.zeros(api.spot_selector_k_bytes(fmt, Bn, L, wl.H_idx, wl.d_idx), dtype=torch.uint8, device=dev)
+            api.spot_quantize_selector_k(sel_k, sel_k_f, fmt, Bn, L, 0, L, wl.H_idx, wl.d_idx)
+            sp_f = type(sp).from_buffer_copy(sp)
+            sp_f.sel_k, sp_f.fmt = sel_k_f.data_ptr(), api.FORMATS[fmt]
+            ws_f = torch.empty(max(16, api.spot_select_workspace_bytes(sp_f)), dtype=torch.uint8, device=dev)
+            sp_f.workspace, sp_f.workspace_bytes = ws_f.data_ptr(), ws_f.numel()
+            dp_f = api.make_decode_step_params(sp_f, ap)
+            dp_f.workspace, dp_f.workspace_bytes = ws_step.data_ptr(), ws_step.numel()
+            for _ in range(3):
+                flush_l2()
+                api.spot_decode_step(dp_f, stream)
+            torch.cuda.synchronize()
+            ev_f = [[torch.cuda.Event(enable_timing=True) for _ in range(2)] for _ in range(n_f)]
+            for i in range(n_f):
+                flush_l2()
+                ev_f[i][0].record(stream)
+                api.spot_decode_step(dp_f, stream)
+                ev_f[i][1].record(stream)
+            torch.cuda.synchronize()
+            us_f = float(np.mean([e[0].elapsed_time(e[1]) for e in ev_f])) * 1e3
+            sel_ms_f = time_alone(lambda: api.spot_select(sp_f, stream), max(3, min(args.steps, 10)))
+            bud_f = budgets.cpu().numpy().astype(np.int64)
+            sel_alg_f = float(np.sum(wl.seq_len.astype(np.int64)) * bytes_per_token(fmt))
+            kv_alg_f = float(bud_f.sum() * wl.blk * Hkv * D * 2 * 2)
+            formats[fmt] = {
+                "us": us_f, "steps": n_f, "budgets": bud_f.tolist(),
+                "selector_cache_bytes": int(sel_k_f.numel()), "bytes_per_token": bytes_per_token(fmt),
+                "shrink_vs_bf16": float(sel_bytes) / float(sel_k_f.numel()),
+                "select_call_us": float(sel_ms_f.mean()) * 1e3,
+                "selector_gbs": sel_alg_f / (float(sel_ms_f.mean()) * 1e-3) / 1e9,
+                "step_bytes": sel_alg_f + kv_alg_f,
+                "step_frac": (sel_alg_f + kv_alg_f) / (us_f * 1e-6) / 1e9 / peak,
+                "step_frac_of_8TBs": (sel_alg_f + kv_alg_f) / (us_f * 1e-6) / 1e9 / 8000.0,
+                "selector_kernel_traffic": traffic_entry("%s/%s/score_decode_kernel" % (args.workload, fmt)),
+            }
+            del sel_k_f, ws_f
+        api.spot_decode_step(dp, stream)            # leave indices / budgets as the BF16 control selected them
+        torch.cuda.synchronize()
+        prefill_roofline = prefill_gemm_roofline(dev, max(3, min(args.steps, 10)), 3, local_rank)
+
+    bytes_per_tok = bytes_per_token(args.fmt)
     sel_alg = float(np.sum(wl.seq_len.astype(np.int64)) * bytes_per_tok)
     kv_alg = float(np.sum(bud_host.astype(np.int64)) * wl.blk * Hkv * D * 2 * 2)
     att_s = float(att_ms.mean()) * 1e-3
     achieved = kv_alg / att_s / 1e9
-    traffic = None
-    tpath = os.path.join(ROOT, "profiles", "traffic.json")
-    if os.path.exists(tpath):
-        with open(tpath) as f:
-            traffic = json.load(f).get("%s/%s/attn_decode_kernel" % (args.workload, args.fmt))
+    traffic = traffic_entry("%s/%s/attn_decode_kernel" % (args.workload, args.fmt))
     us = step_mean * 1e3
     n_layers = N_LAYERS.get(Hq, 36)
 
@@ -420,6 +518,10 @@ def run_ours(args):
                 "d2h_bytes_per_step": d2h},
         "gpu_launches": 4 * args.steps,          # score, select, attn, merge per step (timed loop only)
         "clocks": clocks,
+        "formats": formats,
+        "prefill_roofline": prefill_roofline,
+        "traffic_source": "profiles/traffic.json: dram__bytes_read.sum + dram__bytes_write.sum per launch from the ncu --set full "
+                          "captures named in profiles/traffic.json.md (null: that kernel / format has no capture there)",
         "paper_context": "paper: 3.9x FlashAttention / 1.8x Twilight end-to-end at L=128K, Qwen3-8B, one B200, Triton "
                          "kernels (PAPER.md:146); other shapes, context only",
     }
@@ -645,11 +747,7 @@ def run_prefill(args):
     att_flop = 4.0 * 64 * 64 * D * Hq * float(bud_host.sum())
     score_s = float(np.mean(sc)) * 1e-3
     achieved = gemm_flop / score_s / 1e12
-    traffic = None
-    tpath = os.path.join(ROOT, "profiles", "traffic.json")
-    if os.path.exists(tpath):
-        with open(tpath) as f:
-            traffic = json.load(f).get("cfg5/bf16/score_prefill_kernel")
+    traffic = traffic_entry("cfg5/%s/score_prefill_kernel" % args.fmt)
     # oracle on the host cores: three query blocks below position 4096
     n_tok = min(L, 4096)
     Kh = K[0, :, :n_tok].contiguous().view(torch.int16).cpu().numpy().view(np.uint16)
@@ -706,6 +804,9 @@ def main():
     ap.add_argument("--blk", type=int, default=64, choices=[64, 16],
                     help="decode only: selection block size (16 = the paper's geometry with its 8/16/32 reserved "
                          "sink/recency/K_min blocks, PAPER.md:362-365, :400-402)")
+    ap.add_argument("--no-extras", dest="extras", action="store_false",
+                    help="skip the quantised-cache steps and the prefill selector GEMM that the default cfg3 / bf16 run "
+                         "reports beside the headline (keys formats, prefill_roofline)")
     args = ap.parse_args()
     if args.d_idx:
         D_IDX_OVERRIDE["d_idx"] = args.d_idx
