@@ -577,9 +577,14 @@ def run_prefill(args):
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
     L = args.L or 65536
-    wl = make_prefill_workload(seed=5005 + 1000 * rank, L=L, with_kv=False, **D_IDX_OVERRIDE)
+    geo = dict(D_IDX_OVERRIDE)
+    if args.blk == 16:                # the paper's 16-token key blocks with its 8 / 16 / 32 reserved blocks (f3)
+        geo.update(blk=16, sink_blocks=8, recency_blocks=16, kmin_blocks=32)
+    wl = make_prefill_workload(seed=5005 + 1000 * rank, L=L, with_kv=False, **geo)
     wl.p = args.p
     n_qb = L // 64
+    blk = wl.blk
+    n_kb = L // blk
     Hq, Hkv, D = wl.H_q, wl.H_kv, wl.D
 
     if args.impl == "reference":
@@ -633,13 +638,13 @@ def run_prefill(args):
         # f2: the selector cache in a quantised format; spot_select dequantises the visible prefix into its workspace
         sel_k = torch.zeros(api.spot_selector_k_bytes(args.fmt, 1, L, wl.H_idx, wl.d_idx), dtype=torch.uint8, device=dev)
         api.spot_quantize_selector_k(sel_k_bf16, sel_k, args.fmt, 1, L, 0, L, wl.H_idx, wl.d_idx)
-    cap = n_qb
-    nb_stride = (n_qb + 3) & ~3
+    cap = n_kb
+    nb_stride = (n_kb + 3) & ~3
     indices = torch.empty((n_qb, cap), dtype=torch.int32, device=dev)
     budgets = torch.empty((n_qb,), dtype=torch.int32, device=dev)
     scores = torch.empty((n_qb, nb_stride), dtype=torch.float32, device=dev)
     out = torch.empty((1, L, Hq, D), dtype=torch.int16, device=dev)
-    sp = api.make_select_params(sel_q, w, sel_k, args.fmt, L, None, 0, 1, L, wl.H_idx, wl.d_idx, q_start=0, blk=64,
+    sp = api.make_select_params(sel_q, w, sel_k, args.fmt, L, None, 0, 1, L, wl.H_idx, wl.d_idx, q_start=0, blk=blk,
                                 q_block=64, mode=wl.mode, top_k=wl.top_k, p=args.p, sink_blocks=wl.sink_blocks,
                                 recency_blocks=wl.recency_blocks, kmin_blocks=wl.kmin_blocks,
                                 temperature=wl.temperature, indices=indices, cap=cap, budgets=budgets,
@@ -655,7 +660,7 @@ def run_prefill(args):
         table = torch.randperm(L // pt, generator=gen_t, device=dev).to(torch.int32).reshape(1, L // pt)
         kv_strides, paging = (Hkv * pt * D, D, pt * D), dict(page_table=table, page_tokens=pt)
     ap = api.make_attn_params(Q, K, V, kv_strides, None, 0, indices, budgets, cap, 1, L, Hq, Hkv, D,
-                              q_start=0, blk=64, sm_scale=wl.sm_scale, out=out, **paging)
+                              q_start=0, blk=blk, sm_scale=wl.sm_scale, out=out, **paging)
     stream = torch.cuda.current_stream()
     flush = torch.empty(512 << 20, dtype=torch.uint8, device=dev).zero_()
 
@@ -705,7 +710,7 @@ def run_prefill(args):
     step_ms = np.array([e[0].elapsed_time(e[2]) for e in ev])
     # dense causal comparator (indices NULL) -- a few iterations only
     apd = api.make_attn_params(Q, K, V, kv_strides, None, 0, None, None, 0, 1, L, Hq, Hkv, D,
-                               q_start=0, blk=64, sm_scale=wl.sm_scale, out=out, **paging)
+                               q_start=0, blk=blk, sm_scale=wl.sm_scale, out=out, **paging)
     den = []
     for i in range(3):
         a_, b_ = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
@@ -744,7 +749,7 @@ def run_prefill(args):
     burst, sustained, peak_src = tensor_peaks()
     tiles = n_qb * (n_qb + 1) // 2
     gemm_flop = 2.0 * 64 * 64 * wl.d_idx * wl.H_idx * tiles
-    att_flop = 4.0 * 64 * 64 * D * Hq * float(bud_host.sum())
+    att_flop = 4.0 * 64 * blk * D * Hq * float(bud_host.sum())
     score_s = float(np.mean(sc)) * 1e-3
     achieved = gemm_flop / score_s / 1e12
     traffic = traffic_entry("cfg5/%s/score_prefill_kernel" % args.fmt)
@@ -760,10 +765,10 @@ def run_prefill(args):
         "warmup": W, "ms_per_step": step_mean, "higher_is_better": False, "scaling": "weak", "vs_baseline": None,
         "dtype": "bf16", "data": "synthetic",
         "config": {"workload": "cfg5", "B": 1, "L": L, "H_q": Hq, "H_kv": Hkv, "D": D,
-                   "selector": "%dx%d %s" % (wl.H_idx, wl.d_idx, args.fmt), "blk": 64, "q_block": 64,
+                   "selector": "%dx%d %s" % (wl.H_idx, wl.d_idx, args.fmt), "blk": blk, "q_block": 64,
                    "kv_layout": ("paged, %d tokens per page, random table" % max(args.paged, 64)) if args.paged else "[B][H_kv][L][D]", "mode": wl.mode, "p": args.p,
                    "sink/recency/kmin": [wl.sink_blocks, wl.recency_blocks, wl.kmin_blocks],
-                   "mean_budget": float(bud_host.mean()), "density": float(bud_host.sum()) / tiles,
+                   "mean_budget": float(bud_host.mean()), "density": float(bud_host.sum()) * blk / 64.0 / tiles,
                    "l2": "flushed by a 512 MiB read sweep before every timed step"},
         "tokens_per_s": world * L / (step_mean * 1e-3),
         "breakdown_ms": {"select (tile-score GEMM + selection kernels)": float(sel_ms.mean()),

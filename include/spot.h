@@ -23,10 +23,9 @@
  *   - Return value: spot_status.  SPOT_ERR_CUDA means a CUDA runtime call failed; the code is kept
  *     per thread and returned by spot_last_cuda_error().
  *   - BF16 tensors are passed as uint16_t bit patterns.  Pointers must be 16-byte aligned.
- *   - "block" = blk consecutive key tokens (the selection granularity).  This build supports blk == 64 everywhere
- *     and blk == 16 (the paper's own granularity) in the decode calls: spot_select / spot_score_blocks
- *     with q_block == 1 and spot_sparse_attn_decode; the prefill calls return SPOT_ERR_UNSUPPORTED for it.
- *     A row may hold at most 8192 blocks (L <= 512K at blk 64, L <= 128K at blk 16).
+ *   - "block" = blk consecutive key tokens (the selection granularity): blk == 64 (BASELINE.json's configurations) or
+ *     blk == 16 (the paper's own granularity) in every call, decode and prefill; a prefill query block is
+ *     always 64 tokens.  A row may hold at most 8192 blocks (L <= 512K at blk 64, L <= 128K at blk 16).
  *   - No global state, no environment variables, no CPU fallback: on a device that is not compute
  *     capability 10.x every launching call returns SPOT_ERR_UNSUPPORTED.
  */
@@ -176,7 +175,7 @@ typedef struct {
     int32_t max_seq_len;         /* host-side upper bound of seq_len (decode) -- sizes the grid           */
     int32_t B, Tq, H_idx, d_idx;
     int32_t q_start;             /* prefill: absolute position of the first query (multiple of 64)        */
-    int32_t blk;                 /* key block size: 64, or 16 with q_block == 1                           */
+    int32_t blk;                 /* key block size: 64 or 16                                              */
     int32_t q_block;             /* 1 = decode form, 64 = prefill form                                    */
     /* rule */
     int32_t mode;                /* spot_select_mode                                                      */
@@ -220,7 +219,9 @@ spot_status spot_score_blocks(const spot_select_params* p, void* stream);
  *          indices [B*Tq/64][cap], budgets [B*Tq/64]; seq_len unused (keys up to q_start+Tq-1 must exist).
  * indices == NULL means "every block" (the dense comparator); budgets is then ignored.
  * lse (optional, fp32 [B][H_q] decode / [B][Tq][H_q] prefill): natural-log sum-exp of the scaled logits.
- * Requires H_q % H_kv == 0, H_q/H_kv <= 16, D == 128, blk == 64 (decode: or 16).
+ * Requires H_q % H_kv == 0, H_q/H_kv <= 16, D == 128, blk == 64 or 16 (prefill with blk == 16: a list entry is a
+ * 16-token block; a query token attends to the entry's tokens at or before its own position, so an entry may be wholly
+ * invisible to the first rows of the query block that selected it).
  * --------------------------------------------------------------------------------------------------- */
 typedef struct {
     const uint16_t* q;

@@ -69,8 +69,8 @@ spot_status select_geometry(const spot_select_params* p, SelectGeom* g, bool sco
     if (p->mode == SPOT_MODE_TOPK && p->top_k < p->sink_blocks + p->recency_blocks) return SPOT_ERR_INVALID_ARG;
     if (p->fmt != SPOT_SELK_BF16 && p->cache_stride_tokens % SELK_TILE != 0)
         return SPOT_ERR_INVALID_ARG;
-    // 64-token blocks everywhere; the paper's own 16-token blocks (f3) at decode only
-    if (p->blk != 64 && !(p->blk == 16 && p->q_block == 1)) return SPOT_ERR_UNSUPPORTED;
+    // 64-token blocks, or the paper's own 16-token blocks (f3), in both row forms
+    if (p->blk != 64 && p->blk != 16) return SPOT_ERR_UNSUPPORTED;
     int64_t max_tokens;
     if (p->q_block == 1) {
         if (p->Tq != 1 || !p->seq_len || p->max_seq_len <= 0) return SPOT_ERR_INVALID_ARG;

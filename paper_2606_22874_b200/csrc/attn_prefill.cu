@@ -15,7 +15,7 @@ spot_status check_prefill(const spot_attn_params* p) {
     if (p->B <= 0 || p->H_q <= 0 || p->H_kv <= 0 || p->H_q % p->H_kv != 0) return SPOT_ERR_INVALID_ARG;
     if (p->Tq <= 0 || p->Tq % 64 != 0 || p->q_start < 0 || p->q_start % 64 != 0) return SPOT_ERR_INVALID_ARG;   // R26
     if (p->H_q / p->H_kv > 16) return SPOT_ERR_UNSUPPORTED;
-    if (p->D != 128 || p->blk != 64) return SPOT_ERR_UNSUPPORTED;
+    if (p->D != 128 || (p->blk != 64 && p->blk != 16)) return SPOT_ERR_UNSUPPORTED;
     if (p->page_table) {          // f3 / R32: a 64-token block must sit inside one page
         if (p->page_tokens <= 0 || p->page_tokens % 16 != 0 || p->kv_stride_batch <= 0) return SPOT_ERR_INVALID_ARG;
         if (p->page_tokens % 64 != 0) return SPOT_ERR_UNSUPPORTED;

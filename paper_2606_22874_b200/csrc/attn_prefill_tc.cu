@@ -51,11 +51,14 @@ struct TcAttnArgs {
     int Tq, n_qb, H_q, H_kv, G;
     int n_pairs, n_rows;         // grid.x = n_rows * n_pairs: pairs of 128-row tiles per (row, KV head); rows = B * n_qb
     int qb_start;                // q_start / 64
+    int blk;                     // key block size of the index lists: 64, or 16 (f3: a 128-key tile gathers 8 list entries)
     float scale_log2;
     uint16_t* out;               // [B][Tq][H_q][128]
     float* lse;                  // optional [B][Tq][H_q]
 };
 
+template <int BLK>       // key block size of the index lists: 64, or 16 (f3) -- a compile-time constant: the softmax warps are a
+                         // co-bound of this kernel and the 64-token form must not pay for the per-16-key causal limits
 __global__ void __launch_bounds__(TA_THREADS, 1) attn_prefill_tc_kernel(const __grid_constant__ CUtensorMap tm_q,
                                                                         const __grid_constant__ CUtensorMap tm_k,
                                                                         const __grid_constant__ CUtensorMap tm_v,
@@ -111,15 +114,18 @@ __global__ void __launch_bounds__(TA_THREADS, 1) attn_prefill_tc_kernel(const __
     pdl_wait();
     pdl_launch_dependents();
 
-    const int budget = a.indices ? max(0, min(a.budgets[rowz], a.cap)) : qb_abs + 1;
+    const int budget = a.indices ? max(0, min(a.budgets[rowz], a.cap)) : (qb_abs + 1) * (64 / BLK);
     const int32_t* idx = a.indices ? a.indices + (int64_t)rowz * a.cap : nullptr;
+    // one tile of the loop = up to GROUP visible list entries = up to 128 keys (2 x 64 or 8 x 16)
+    constexpr int blk = BLK, GROUP = 128 / BLK;
+    constexpr int blk_shift = BLK == 16 ? 2 : 0;         // list entry -> 64-token block: j >> blk_shift
     auto block_of = [&](int it) -> int { return idx ? idx[it] : it; };
-    auto visible = [&](int j) -> bool { return j >= 0 && j <= qb_abs; };
+    auto visible = [&](int j) -> bool { return j >= 0 && (j >> blk_shift) <= qb_abs; };
     // where key block j lives: (token coordinate, outermost coordinate) of the K / V tensor maps -- (64 j, b) for
     // contiguous caches, (offset inside the page, physical page) for page pools
     const int32_t* ptab = a.page_table ? a.page_table + (int64_t)b * a.pt_stride : nullptr;
     auto place = [&](int j, int& tok, int& outer) {
-        tok = j * 64;
+        tok = j * blk;
         outer = b;
         if (ptab) {
             const int lp = tok / a.page_tokens;
@@ -137,56 +143,65 @@ __global__ void __launch_bounds__(TA_THREADS, 1) attn_prefill_tc_kernel(const __
             // one ring stage = a PAIR of visible key blocks (any two, they need not be adjacent): K pair, then V pair,
             // each [2 d-halves][128 keys][128 B]; a block is four 8 KiB boxes (K/V x d-half)
             int n = 0, it = 0;
+            const uint32_t ent_bytes = (uint32_t)blk * 128u;                  // one d-half of one list entry
             while (true) {
-                int jA = -1, jB = -1;
-                for (; it < budget && jA < 0; ++it) { const int j = block_of(it); if (visible(j)) jA = j; }
-                if (jA < 0) break;
-                for (; it < budget && jB < 0; ++it) { const int j = block_of(it); if (visible(j)) jB = j; }
                 // (the page-table lookups are issued before the wait for the ring slot, which hides them)
-                int tok[2] = {0, 0}, outer[2] = {0, 0};
-                place(jA, tok[0], outer[0]);
-                if (jB >= 0) place(jB, tok[1], outer[1]);
+                int tok[8], outer[8], ne = 0;
+#pragma unroll
+                for (int u = 0; u < 8; ++u) {
+                    tok[u] = outer[u] = 0;
+                    if (u < GROUP)
+                        while (it < budget) {
+                            const int j = block_of(it++);
+                            if (visible(j)) { place(j, tok[u], outer[u]); ++ne; break; }
+                        }
+                }
+                if (ne == 0) break;
                 const int s = n % TA_STAGES;
                 mbar_wait(bar_kv_empty + 8 * s, ((n / TA_STAGES) & 1) ^ 1);
                 const uint32_t ks = kv_smem + s * 2 * TA_KV_TILE;
-                const uint32_t bytes = (jB >= 0 ? 2 : 1) * TA_BLK_BYTES;
+                const uint32_t bytes = (uint32_t)ne * 2u * ent_bytes;
                 mbar_arrive_expect_tx(bar_k_full + 8 * s, bytes);
-                for (int u = 0; u < (jB >= 0 ? 2 : 1); ++u)
-                    for (int hf = 0; hf < 2; ++hf)
-                        tma_load_5d(ks + hf * (128 * 128) + u * (64 * 128), &tm_k, bar_k_full + 8 * s, 0, tok[u], hf, hk,
-                                    outer[u]);
+#pragma unroll
+                for (int u = 0; u < 8; ++u)
+                    if (u < ne)
+                        for (int hf = 0; hf < 2; ++hf)
+                            tma_load_5d(ks + hf * (128 * 128) + u * ent_bytes, &tm_k, bar_k_full + 8 * s, 0, tok[u], hf, hk,
+                                        outer[u]);
                 mbar_arrive_expect_tx(bar_v_full + 8 * s, bytes);
-                for (int u = 0; u < (jB >= 0 ? 2 : 1); ++u)
-                    for (int hf = 0; hf < 2; ++hf)
-                        tma_load_5d(ks + TA_KV_TILE + hf * (128 * 128) + u * (64 * 128), &tm_v, bar_v_full + 8 * s, 0,
-                                    tok[u], hf, hk, outer[u]);
+#pragma unroll
+                for (int u = 0; u < 8; ++u)
+                    if (u < ne)
+                        for (int hf = 0; hf < 2; ++hf)
+                            tma_load_5d(ks + TA_KV_TILE + hf * (128 * 128) + u * ent_bytes, &tm_v, bar_v_full + 8 * s, 0,
+                                        tok[u], hf, hk, outer[u]);
                 ++n;
             }
         }
     } else if (warp == 1) {
         // ================================ MMA issuer ================================
         if (lane == 0) {
-            constexpr uint32_t idesc_qk128 = umma_idesc_bf16(128, 128), idesc_qk64 = umma_idesc_bf16(128, 64);
             constexpr uint32_t idesc_pv = umma_idesc_bf16(128, 128) | UMMA_B_MN_MAJOR;
             int nv = 0;
             for (int it = 0; it < budget; ++it) nv += visible(block_of(it)) ? 1 : 0;
-            const int np = (nv + 1) >> 1;                 // iterations: pairs of key blocks (the last may be single)
+            const int np = (nv + GROUP - 1) / GROUP;     // iterations: tiles of up to 128 keys (the last may be short)
+            auto keys_of = [&](int n) -> int { return min(GROUP, nv - n * GROUP) * blk; };   // keys of tile n: a multiple of 16
             // One lone thread issues every MMA, with nobody to hide its instruction latencies: descriptors are built
             // once and advanced by compile-time constants (the start-address field is the low 14 bits, in 16-byte
             // units), so each tcgen05.mma costs two integer adds, not a dozen dependent ones.
             const uint64_t qd[2] = {umma_desc_sw128(q_smem), umma_desc_sw128(q_smem + TA_Q_TILE)};
-            auto qk = [&](int t, uint64_t kd, bool full) {     // S_t = Q_t K^T over 128 (or 64) keys
-                const uint32_t idesc = full ? idesc_qk128 : idesc_qk64;
+            auto qk = [&](int t, uint64_t kd, int nkeys) {     // S_t = Q_t K^T over nkeys keys (N = nkeys)
+                const uint32_t idesc = umma_idesc_bf16(128, nkeys);
 #pragma unroll
                 for (int kk = 0; kk < 8; ++kk)
                     umma_bf16_ss(tbase + t * 128, qd[t] + (uint64_t)(((kk >> 2) * (128 * 128) + (kk & 3) * 32) >> 4),
                                  kd + (uint64_t)(((kk >> 2) * (128 * 128) + (kk & 3) * 32) >> 4), idesc, kk > 0);
                 umma_commit(bar_s_full + 8 * t);
             };
-            auto pv = [&](int t, uint64_t vd, bool acc, bool full) {   // O_t += P_t V; P_t packed BF16 over the start of S_t
+            auto pv = [&](int t, uint64_t vd, bool acc, int nkeys) {   // O_t += P_t V over nkeys keys: one k-step per 16 keys
 #pragma unroll
                 for (int kk = 0; kk < 8; ++kk)
-                    if (kk < 4 || full)
+                    if (kk * 16 < nkeys)
                         umma_bf16_ts(tbase + 256 + t * 128, tbase + t * 128 + kk * 8, vd + (uint64_t)((kk * 2048) >> 4),
                                      idesc_pv, acc || kk > 0);
                 umma_commit(bar_o_done + 8 * t);
@@ -197,26 +212,26 @@ __global__ void __launch_bounds__(TA_THREADS, 1) attn_prefill_tc_kernel(const __
                 tc_fence_after();
                 {
                     const uint64_t kd0 = umma_desc_sw128(kv_smem);
-                    qk(0, kd0, nv >= 2);
-                    if (two) qk(1, kd0, nv >= 2);
+                    qk(0, kd0, keys_of(0));
+                    if (two) qk(1, kd0, keys_of(0));
                 }
                 for (int n = 0; n < np; ++n) {
                     const int s = n % TA_STAGES, s1 = (n + 1) % TA_STAGES;
                     const uint64_t vd = umma_desc_sw128_mn(kv_smem + s * 2 * TA_KV_TILE + TA_KV_TILE, 128 * 128, 1024);
                     const uint64_t kd1 = umma_desc_sw128(kv_smem + s1 * 2 * TA_KV_TILE);
                     const bool more = n + 1 < np;
-                    const bool full = 2 * n + 1 < nv, full1 = 2 * n + 3 < nv;
+                    const int nk0 = keys_of(n), nk1 = more ? keys_of(n + 1) : 0;
                     mbar_wait(bar_v_full + 8 * s, (n / TA_STAGES) & 1);
                     if (more) mbar_wait(bar_k_full + 8 * s1, ((n + 1) / TA_STAGES) & 1);
                     mbar_wait(bar_p_full, n & 1);                       // P_0(n) written, S_0 consumed, O_0 rescaled
                     tc_fence_after();
-                    pv(0, vd, n > 0, full);
-                    if (more) qk(0, kd1, full1);
+                    pv(0, vd, n > 0, nk0);
+                    if (more) qk(0, kd1, nk1);
                     if (two) {
                         mbar_wait(bar_p_full + 8, n & 1);
                         tc_fence_after();
-                        pv(1, vd, n > 0, full);
-                        if (more) qk(1, kd1, full1);
+                        pv(1, vd, n > 0, nk0);
+                        if (more) qk(1, kd1, nk1);
                     }
                     umma_commit(bar_kv_empty + 8 * s);                  // K(n), V(n) no longer read
                 }
@@ -236,24 +251,46 @@ __global__ void __launch_bounds__(TA_THREADS, 1) attn_prefill_tc_kernel(const __
             float m_used = -INFINITY, l = 0.f;
             int n = 0, it = 0;
             while (true) {
-                // this iteration's pair of visible key blocks (the last pair may be single)
-                int jA = -1, jB = -1;
-                for (; it < budget && jA < 0; ++it) { const int j = block_of(it); if (visible(j)) jA = j; }
-                if (jA < 0) break;
-                for (; it < budget && jB < 0; ++it) { const int j = block_of(it); if (visible(j)) jB = j; }
-                const int nh = jB >= 0 ? 2 : 1;
+                // this iteration's tile: up to GROUP visible list entries (the last tile may be short)
+                int jj[8], ne = 0;
+#pragma unroll
+                for (int u = 0; u < 8; ++u) {                   // (static indices: jj[] stays in registers)
+                    jj[u] = -1;
+                    if (u < GROUP)
+                        while (it < budget) {
+                            const int j = block_of(it++);
+                            if (visible(j)) { jj[u] = j; ++ne; break; }
+                        }
+                }
+                if (ne == 0) break;
+                const int nkeys = ne * blk, nh = (nkeys + 63) >> 6;
+                // 16-token blocks: causal limit of every 16-key group u of the tile -- key e of the group is visible iff
+                // e <= lim(u) (15: the whole group, the usual case; -1: none -- a group past the end of a short tile, or a
+                // block that lies wholly in this row's future although the query block as a whole may see it); packed, byte
+                // u of lim_pk = lim(u) + 1, so that a loop variable can pick its group without indexing jj[].
+                // 64-token blocks: only the diagonal block needs a mask (key e visible iff e <= ql).
+                unsigned long long lim_pk = 0ull;
+                if constexpr (BLK == 16) {
+                    const int q_tok = qb_abs * 64 + ql;
+#pragma unroll
+                    for (int u = 0; u < 8; ++u) {
+                        int lim = -1;
+                        if (u < ne) lim = max(min(15, q_tok - jj[u] * 16), -1);
+                        lim_pk |= (unsigned long long)(lim + 1) << (8 * u);
+                    }
+                }
+                auto lim_of = [&](int u) -> int { return (int)((lim_pk >> (8 * u)) & 0xffull) - 1; };
                 mbar_wait(bar_s_full + 8 * t, n & 1);
                 tc_fence_after();
-                // Optimistic single pass: exp2 against the STALE max while the row max of this pair is being found (sm_scale
+                // Optimistic single pass: exp2 against the STALE max while the row max of this tile is being found (sm_scale
                 // > 0: max on the raw logits; scale and max-subtraction are one FFMA).  P = exp2(scale x - m) rounded to
                 // BF16 waits in registers.  Only if some row's max grew by more than 2^8 since its last rescale (always
-                // in the first iteration, rarely later) is the pair redone after rescaling O -- P stays <= 256, and l
-                // and O always use the same max, so the result is exact.  The causal mask applies inside the diagonal
-                // block only.
+                // in the first iteration, rarely later) is the tile redone after rescaling O -- P stays <= 256, and l
+                // and O always use the same max, so the result is exact.
                 uint32_t pk[64];
                 float ps0 = 0.f, ps1 = 0.f, mx = -INFINITY;
                 {
-                    const float neg_m = -m_used;
+                    const float neg_m = (m_used == -INFINITY) ? 0.f : -m_used;    // (a row that has seen no key yet)
 #pragma unroll
                     for (int hf = 0; hf < 2; ++hf) {
                         if (hf < nh) {
@@ -266,7 +303,17 @@ __global__ void __launch_bounds__(TA_THREADS, 1) attn_prefill_tc_kernel(const __
 #pragma unroll
                                 for (int e = 0; e < 16; ++e) { x[e] = d0[e]; x[16 + e] = d1[e]; x[32 + e] = d2[e]; x[48 + e] = d3[e]; }
                             }
-                            if ((hf ? jB : jA) == qb_abs) {
+                            if constexpr (BLK == 16) {
+#pragma unroll
+                                for (int g4 = 0; g4 < 4; ++g4) {
+                                    const int lim = lim_of(hf * 4 + g4);
+                                    if (lim < 15) {
+#pragma unroll
+                                        for (int e = 0; e < 16; ++e)
+                                            if (e > lim) x[g4 * 16 + e] = -INFINITY;
+                                    }
+                                }
+                            } else if (jj[hf] == qb_abs) {
 #pragma unroll
                                 for (int e = 0; e < 64; ++e)
                                     if (e > ql) x[e] = -INFINITY;
@@ -287,7 +334,7 @@ __global__ void __launch_bounds__(TA_THREADS, 1) attn_prefill_tc_kernel(const __
                     }
                 }
                 mx *= a.scale_log2;
-                const bool need = mx > m_used + TA_RESCALE_THRESHOLD;       // (true for every row while m_used = -inf)
+                const bool need = mx > m_used + TA_RESCALE_THRESHOLD;       // (true for a row's first visible key: m_used = -inf)
                 if (__any_sync(0xffffffffu, need)) {                         // warp-uniform: tcgen05.ld/st are collective
                     const float m_new = need ? mx : m_used;
                     const float alpha = (m_used == -INFINITY) ? 0.f : fast_exp2(m_used - m_new);   // 1 when !need
@@ -307,22 +354,22 @@ __global__ void __launch_bounds__(TA_THREADS, 1) attn_prefill_tc_kernel(const __
                         }
                         tmem_st_wait();
                     }
-                    // redo the pair against the new max (S_t is still intact: P has not been stored yet)
+                    // redo the tile against the new max (S_t is still intact: P has not been stored yet)
                     ps0 = ps1 = 0.f;
-                    const float neg_m = -m_used;
+                    const float neg_m = (m_used == -INFINITY) ? 0.f : -m_used;
 #pragma unroll
                     for (int hf = 0; hf < 2; ++hf) {
                         if (hf < nh) {
-                            const bool dg = (hf ? jB : jA) == qb_abs;
 #pragma unroll 1
                             for (int c16 = 0; c16 < 4; ++c16) {
                                 float d[16];
                                 tmem_ld16(t_s + hf * 64 + c16 * 16, d);
                                 tmem_ld_wait();
+                                const int lim = BLK == 16 ? lim_of(hf * 4 + c16) : (jj[hf] == qb_abs ? ql - c16 * 16 : 15);
 #pragma unroll
                                 for (int e = 0; e < 16; e += 2) {
-                                    const float x0 = (dg && c16 * 16 + e > ql) ? -INFINITY : d[e];
-                                    const float x1 = (dg && c16 * 16 + e + 1 > ql) ? -INFINITY : d[e + 1];
+                                    const float x0 = (e > lim) ? -INFINITY : d[e];
+                                    const float x1 = (e + 1 > lim) ? -INFINITY : d[e + 1];
                                     const float p0 = fast_exp2(fmaf(x0, a.scale_log2, neg_m));
                                     const float p1 = fast_exp2(fmaf(x1, a.scale_log2, neg_m));
                                     ps0 += p0;
@@ -339,12 +386,11 @@ __global__ void __launch_bounds__(TA_THREADS, 1) attn_prefill_tc_kernel(const __
                 }
                 // P goes back to tensor memory over the start of S_t: columns 32 hf .. +31 hold the 64 keys of block hf
                 // (QK_t(n+1), which rewrites S_t, is issued after PV_t(n) and the tensor pipe runs them in order)
+                // (16 columns = 32 keys per store; a short tile stores only what PV will read)
                 tmem_st16u(t_s, pk);
-                tmem_st16u(t_s + 16, pk + 16);
-                if (nh == 2) {
-                    tmem_st16u(t_s + 32, pk + 32);
-                    tmem_st16u(t_s + 48, pk + 48);
-                }
+                if (nkeys > 32) tmem_st16u(t_s + 16, pk + 16);
+                if (nkeys > 64) tmem_st16u(t_s + 32, pk + 32);
+                if (nkeys > 96) tmem_st16u(t_s + 48, pk + 48);
                 l += ps0 + ps1;
                 tmem_st_wait();
                 tc_fence_before();
@@ -409,6 +455,7 @@ spot_status attn_prefill_tc(const spot_attn_params* p, cudaStream_t stream) {
     a.indices = p->indices; a.budgets = p->budgets; a.cap = p->cap;
     a.Tq = p->Tq; a.n_qb = p->Tq / 64; a.H_q = p->H_q; a.H_kv = p->H_kv; a.G = p->H_q / p->H_kv;
     a.qb_start = p->q_start / 64;
+    a.blk = p->blk;
     a.scale_log2 = p->sm_scale * 1.4426950408889634f;
     a.out = p->out; a.lse = p->lse;
     CUtensorMap tm_q, tm_k, tm_v;
@@ -426,20 +473,20 @@ spot_status attn_prefill_tc(const spot_attn_params* p, cudaStream_t stream) {
     const uint64_t n_tok = p->page_table ? (uint64_t)p->page_tokens : (uint64_t)p->q_start + p->Tq;
     const uint64_t n_outer = p->page_table ? ((uint64_t)1 << 22) : (uint64_t)p->B;
     if (!make_map(&tm_k, p->k, n_tok, (uint64_t)p->kv_stride_token, (uint64_t)p->H_kv, (uint64_t)p->kv_stride_head,
-                  n_outer, (uint64_t)p->kv_stride_batch, 64, 1))
+                  n_outer, (uint64_t)p->kv_stride_batch, (uint32_t)p->blk, 1))
         return SPOT_ERR_CUDA;
     if (!make_map(&tm_v, p->v, n_tok, (uint64_t)p->kv_stride_token, (uint64_t)p->H_kv, (uint64_t)p->kv_stride_head,
-                  n_outer, (uint64_t)p->kv_stride_batch, 64, 1))
+                  n_outer, (uint64_t)p->kv_stride_batch, (uint32_t)p->blk, 1))
         return SPOT_ERR_CUDA;
-    static unsigned long long smem_attr_done = 0;
-    SPOT_CUDA_TRY(set_max_smem_once(attn_prefill_tc_kernel, (int)TA_SMEM_BYTES, smem_attr_done));
+    static unsigned long long smem_attr_done[2] = {0, 0};
+    auto kernel = p->blk == 16 ? attn_prefill_tc_kernel<16> : attn_prefill_tc_kernel<64>;
+    SPOT_CUDA_TRY(set_max_smem_once(kernel, (int)TA_SMEM_BYTES, smem_attr_done[p->blk == 16]));
     const int n_mt = (a.G * 64 + 127) / 128;
     a.n_pairs = (n_mt + 1) / 2;
     a.n_rows = p->B * a.n_qb;
     if ((int64_t)a.n_pairs * a.n_rows > 0x7fffffff || p->H_kv > 65535) return SPOT_ERR_UNSUPPORTED;
     dim3 grid((unsigned)(a.n_pairs * a.n_rows), 1u, (unsigned)p->H_kv);
-    SPOT_CUDA_TRY(launch_pdl(attn_prefill_tc_kernel, grid, dim3(TA_THREADS), (size_t)TA_SMEM_BYTES, stream, tm_q, tm_k,
-                             tm_v, a));
+    SPOT_CUDA_TRY(launch_pdl(kernel, grid, dim3(TA_THREADS), (size_t)TA_SMEM_BYTES, stream, tm_q, tm_k, tm_v, a));
     return SPOT_OK;
 }
 

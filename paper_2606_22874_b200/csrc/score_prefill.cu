@@ -33,7 +33,7 @@ constexpr int PF_TSTAGES = 4;           // TMEM accumulators (128 columns each)
 constexpr int PF_EPI_WARPS = 8;
 constexpr int PF_THREADS = (PF_EPI_WARPS + 2) * 32;
 constexpr uint32_t PF_PLANE_BYTES = 128 * 64 * 2;          // [128 rows][64 d] BF16: one 128-byte swizzle row per token
-constexpr uint32_t PF_SMEM_MISC = 1024;
+constexpr uint32_t PF_SMEM_MISC = 2048;        // barriers, TMEM slot, tile maxima [CHUNK][4 quarters][2 query blocks]
 
 // d_idx = 64: a head is one plane; the query tile is 64 KiB and a K stage holds all four heads of a key-block pair
 // (64 KiB, 2 stages).  d_idx = 128 (the paper's selector width): a head is two planes (the cache row
@@ -60,6 +60,7 @@ struct PrefillScoreArgs {
     int qb_start;             // q_start / 64
     int n_chunks_max;
     int total_ids;
+    int fine;                 // blk == 16 (f3): four scores per 64-key block, one per 16-token quarter
 };
 
 __device__ __forceinline__ uint32_t f32_order_key(float x) {
@@ -105,7 +106,7 @@ __global__ void __launch_bounds__(PF_THREADS, 1) score_prefill_kernel(const __gr
     const uint32_t bar_t_full = misc_u32 + 80;     // [4]
     const uint32_t bar_t_empty = misc_u32 + 112;   // [4]
     uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(misc + 144);
-    uint32_t* s_max = reinterpret_cast<uint32_t*>(misc + 160);       // [2 item buffers][CHUNK][2 query blocks]
+    uint32_t* s_max = reinterpret_cast<uint32_t*>(misc + 160);       // [CHUNK][4 quarters][2 query blocks]
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
 
@@ -122,7 +123,7 @@ __global__ void __launch_bounds__(PF_THREADS, 1) score_prefill_kernel(const __gr
         }
         mbar_fence_init();
     }
-    if (threadIdx.x < 2 * PF_CHUNK * 2) s_max[threadIdx.x] = 0u;
+    for (int e = threadIdx.x; e < PF_CHUNK * 4 * 2; e += PF_THREADS) s_max[e] = 0u;
     if (warp == 0) tmem_alloc(misc_u32 + 144, 512);
     if (warp == PF_EPI_WARPS && lane == 0) {
         tma_prefetch_desc(&tm_q);
@@ -217,7 +218,6 @@ __global__ void __launch_bounds__(PF_THREADS, 1) score_prefill_kernel(const __gr
         for (int id = blockIdx.x; id < a.total_ids; id += gridDim.x) {
             int b, c, m, nk;
             if (!decode_item(a, id, b, c, m, nk)) continue;
-            const int ib = n_item & 1;
             const int q_local = m * PF_M + row;                 // query index inside the chunk of Tq queries
             const bool q_exists = q_local < a.Tq;
             float4 wv = make_float4(0.f, 0.f, 0.f, 0.f);
@@ -264,25 +264,43 @@ __global__ void __launch_bounds__(PF_THREADS, 1) score_prefill_kernel(const __gr
                     for (int i = 0; i < 64; ++i)
                         if (i > q_in_blk) S[i] = -INFINITY;
                 }
-                float mx = -INFINITY;
+                const bool live = kb < nk && j <= qb_abs && q_exists;   // warp-uniform: Tq is a multiple of 64, a warp's rows share a block
+                if (!a.fine) {
+                    float mx = -INFINITY;
 #pragma unroll
-                for (int i = 0; i < 64; i += 2) mx = fmax3(mx, S[i], S[i + 1]);
-                if (kb < nk && j <= qb_abs && q_exists) {   // warp-uniform: Tq is a multiple of 64, a warp's rows share a block
-                    const uint32_t key = __reduce_max_sync(0xffffffffu, f32_order_key(mx));
-                    if (lane == 0) atomicMax(&s_max[(ib * PF_CHUNK + kb) * 2 + qbl], key);
+                    for (int i = 0; i < 64; i += 2) mx = fmax3(mx, S[i], S[i + 1]);
+                    if (live) {
+                        const uint32_t key = __reduce_max_sync(0xffffffffu, f32_order_key(mx));
+                        if (lane == 0) atomicMax(&s_max[(kb * 4) * 2 + qbl], key);
+                    }
+                } else {
+                    // 16-token blocks (f3): one maximum per quarter of the 64-key block
+#pragma unroll
+                    for (int q4 = 0; q4 < 4; ++q4) {
+                        float mx = -INFINITY;
+#pragma unroll
+                        for (int i = 0; i < 16; i += 2) mx = fmax3(mx, S[q4 * 16 + i], S[q4 * 16 + i + 1]);
+                        if (live) {
+                            const uint32_t key = __reduce_max_sync(0xffffffffu, f32_order_key(mx));
+                            if (lane == 0) atomicMax(&s_max[(kb * 4 + q4) * 2 + qbl], key);
+                        }
+                    }
                 }
             }
             // item done: all epilogue warps meet, then the tile maxima go out and the buffer is re-armed
             asm volatile("bar.sync 1, %0;" :: "n"(PF_EPI_WARPS * 32) : "memory");
-            for (int e = threadIdx.x; e < nk * 2; e += PF_EPI_WARPS * 32) {
-                const int kb = e >> 1, qq = e & 1;
+            const int nq4 = a.fine ? 4 : 1;
+            for (int e = threadIdx.x; e < nk * nq4 * 2; e += PF_EPI_WARPS * 32) {
+                const int qq = e & 1, q4 = (e >> 1) % nq4, kb = (e >> 1) / nq4;
                 const int qblk = 2 * m + qq;
                 const int j = c * PF_CHUNK + kb;
-                const uint32_t key = s_max[(ib * PF_CHUNK + kb) * 2 + qq];
-                s_max[(ib * PF_CHUNK + kb) * 2 + qq] = 0u;
+                const int slot = (kb * 4 + q4) * 2 + qq;
+                const uint32_t key = s_max[slot];
+                s_max[slot] = 0u;
                 if (qblk < a.n_qb && j <= a.qb_start + qblk)
-                    a.scores[((int64_t)b * a.n_qb + qblk) * a.nb_stride + j] = f32_from_order_key(key);
+                    a.scores[((int64_t)b * a.n_qb + qblk) * a.nb_stride + j * nq4 + q4] = f32_from_order_key(key);
             }
+            asm volatile("bar.sync 1, %0;" :: "n"(PF_EPI_WARPS * 32) : "memory");   // re-armed before the next item's maxima
             ++n_item;
         }
     }
@@ -331,6 +349,7 @@ static spot_status score_prefill_d(const spot_select_params* p, float* scores, i
     a.w = p->w; a.scores = scores; a.nb_stride = nb_stride;
     a.B = p->B; a.Tq = p->Tq; a.n_qb = p->Tq / 64; a.n_qt = (a.n_qb + 1) / 2;
     a.qb_start = p->q_start / 64;
+    a.fine = p->blk == 16;
     const int n_vis_max = a.qb_start + a.n_qb;
     a.n_chunks_max = (n_vis_max + PF_CHUNK - 1) / PF_CHUNK;
     const int64_t total = (int64_t)a.B * a.n_chunks_max * a.n_qt;

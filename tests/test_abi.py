@@ -101,7 +101,8 @@ def test_select_argument_errors_are_caught_on_the_host(lib):
     assert lib.spot_select(C.byref(_select_params(blk=32)), None) == UNSUPPORTED
     # 16-token blocks (f3) are a decode geometry: accepted there (4x the blocks), not for 64-query prefill rows
     assert lib.spot_select_workspace_bytes(C.byref(_select_params(blk=16, cap=256, nb_stride=256))) >= 2 * 256 * 4
-    assert lib.spot_select(C.byref(_select_params(blk=16, cap=256, q_block=64, Tq=64, seq_len=None)), None) == UNSUPPORTED
+    assert lib.spot_select_workspace_bytes(C.byref(_select_params(blk=16, cap=256, nb_stride=256, q_block=64, Tq=64,
+                                                                  seq_len=None))) > 0            # f3: prefill rows too
     assert lib.spot_select(None, None) == INVALID
     assert lib.spot_score_blocks(C.byref(_select_params()), None) == INVALID        # block_scores is required
     # a score-only block (what spot_score_blocks reads: no indices / budgets / cap) can size its own workspace -- a
@@ -138,7 +139,7 @@ def test_attention_argument_errors_are_caught_on_the_host(lib):
     for o in (dict(Tq=96), dict(Tq=128, q_start=32), dict(Tq=0)):
         assert lib.spot_sparse_attn_prefill(C.byref(_attn_params(**o)), None) == INVALID, o
     assert lib.spot_sparse_attn_decode_workspace_bytes(C.byref(_attn_params(blk=16))) > 0          # f3
-    assert lib.spot_sparse_attn_prefill(C.byref(_attn_params(Tq=64, blk=16)), None) == UNSUPPORTED
+    assert lib.spot_sparse_attn_prefill(C.byref(_attn_params(Tq=64, blk=32)), None) == UNSUPPORTED
     # paged K/V (f3): decode only; page size a multiple of 16, the table must cover max_seq_len, page stride a multiple
     # of the token stride
     paged = dict(page_table=0x8000, page_table_stride=64, page_tokens=64, kv_stride_batch=8 * 64 * 128)

@@ -329,3 +329,101 @@ def test_prefill_attention_over_paged_kv(torch_cuda, page_tokens, layout):
     _check_attn_prefill(dp, lists)
     dense = [[list(range((q_start + 64 * i) // 64 + 1)) for i in range(Tq // 64)] for _ in wls]
     _check_attn_prefill(dp, dense)
+
+
+# ---------------------------------------------------------------- f3: the paper's 16-token key blocks in prefill
+F3 = dict(blk=16, sink_blocks=8, recency_blocks=16, kmin_blocks=32)
+
+
+@pytest.mark.parametrize("L,q_start,Tq,B,d_idx,over", [
+    (1024, 0, 1024, 1, 64, {}),
+    (1024, 512, 320, 2, 64, {}),
+    (4608, 0, 4608, 1, 64, {}),                                # 288 blocks per 64-key chunk boundary, three chunks
+    (1024, 256, 256, 1, 128, {}),
+    (1024, 256, 256, 1, 64, {"recency_blocks": 0, "sink_blocks": 0, "kmin_blocks": 0}),   # diagonal quarters residual
+    (1024, 0, 512, 1, 64, {"mode": "topk", "top_k": 40}),
+])
+def test_prefill_block16_scores_and_selection(torch_cuda, L, q_start, Tq, B, d_idx, over):
+    """Four tile scores per 64-key block (one per 16-token quarter, the causal mask applied token-wise inside the
+    diagonal block), selection rows of 4x the entries, the paper's 8 / 16 / 32 reserved blocks."""
+    wls = [_neg_weights(make_prefill_workload(seed=8008 + 7 * b, L=L, d_idx=d_idx, with_kv=False, **F3), 30 + b)
+           for b in range(B)]
+    dp = H.DevicePrefill(wls, q_start, Tq, with_kv=False)
+    report = []
+    _check_select_prefill(dp, report, **over)
+    print("prefill blk16 select L=%d q_start=%d Tq=%d d_idx=%d: near-tie rows %s" % (L, q_start, Tq, d_idx, report[:4]))
+    assert len(report) <= 1
+
+
+def test_prefill_block16_selection_over_a_quantised_cache(torch_cuda):
+    wls = [_neg_weights(make_prefill_workload(seed=8108, L=1024, with_kv=False, **F3), 31)]
+    dp = H.DevicePrefill(wls, 512, 320, with_kv=False)
+    dp.set_cache_format("mxfp4")
+    report = []
+    _check_select_prefill(dp, report)
+    assert len(report) <= 1
+
+
+def test_prefill_block16_attention(torch_cuda):
+    """Block-sparse causal attention over lists of 16-token blocks: the oracle's lists (a later chunk, batch of 2), dense
+    (indices NULL), and hand-made lists -- tiles that are not full (lists of 1, 3, 9, 17 entries), entries that lie wholly
+    in the future of the first rows of the query block (quarters 1-3 of the diagonal block without quarter 0), a list
+    whose only past block is the sink."""
+    L, q_start, Tq, B = 1024, 512, 320, 2
+    wls = [make_prefill_workload(seed=8208 + 11 * b, L=L, **F3) for b in range(B)]
+    dp = H.DevicePrefill(wls, q_start, Tq)
+    lists = [[sel.indices.tolist() for _, sel in H.oracle_select_prefill(w, q_start, Tq)] for w in wls]
+    _check_attn_prefill(dp, lists, want_lse=True)
+    n_q = Tq // 64
+    dense = [[list(range(((q_start + 64 * (i + 1)) // 16))) for i in range(n_q)] for _ in wls]
+    _check_attn_prefill(dp, dense)
+    out_dense, _, _ = _check_attn_prefill_indices_none(dp, dense)
+    d0 = lambda i: (q_start + 64 * i) // 16                     # first 16-token block of query block i's diagonal
+    hand = [[[0], [0, 5, d0(1) + 1], [0, 1, 2, 3, 9, 10, 11, d0(2) + 1, d0(2) + 3],
+             [0] + list(range(17, 32)) + [d0(3) + 2], [0, d0(4), d0(4) + 1, d0(4) + 2, d0(4) + 3]] for _ in wls]
+    _check_attn_prefill(dp, hand)
+
+
+def _check_attn_prefill_indices_none(dp, dense_lists):
+    """indices == NULL (every causally visible block) must equal the explicit dense lists bit for bit."""
+    import torch
+    wl, api = dp.wl, dp.api
+    out = torch.zeros((dp.B, dp.Tq, wl.H_q, wl.D), dtype=torch.int16, device="cuda")
+    ap = api.make_attn_params(dp.Q, dp.K, dp.V, dp.kv_strides, None, 0, None, None, 0, dp.B, dp.Tq, wl.H_q, wl.H_kv, wl.D,
+                              q_start=dp.q_start, blk=wl.blk, sm_scale=wl.sm_scale, out=out)
+    api.spot_sparse_attn_prefill(ap)
+    torch.cuda.synchronize()
+    rows = dp.B * dp.n_q
+    cap = max(max(len(l) for l in ls) for ls in dense_lists)
+    idx = np.full((rows, cap), -1, dtype=np.int32)
+    bud = np.zeros(rows, dtype=np.int32)
+    for b, ls in enumerate(dense_lists):
+        for i, l in enumerate(ls):
+            idx[b * dp.n_q + i, :len(l)] = l
+            bud[b * dp.n_q + i] = len(l)
+    want, _ = dp.attend(idx, bud)
+    got = H.bf16_bits_to_f64(H.to_np_u16(out))
+    assert np.array_equal(got, want)
+    return got, None, None
+
+
+def test_prefill_block16_attention_over_paged_kv(torch_cuda):
+    torch = torch_cuda
+    L, q_start, Tq = 1024, 256, 256
+    wl = make_prefill_workload(seed=8308, L=L, **F3)
+    dp = H.DevicePrefill([wl], q_start, Tq)
+    lists = [[sel.indices.tolist() for _, sel in H.oracle_select_prefill(wl, q_start, Tq)]]
+    _check_attn_prefill(dp, lists)
+    pt, Hkv, D = 64, wl.H_kv, wl.D
+    n_log = L // pt
+    rng = np.random.default_rng(43)
+    table = rng.permutation(n_log + 3)[:n_log].reshape(1, n_log).astype(np.int32)
+    poolK = rng.integers(0, 1 << 16, size=(n_log + 3, Hkv, pt, D), dtype=np.uint16) & 0x3fff
+    poolV = rng.integers(0, 1 << 16, size=(n_log + 3, Hkv, pt, D), dtype=np.uint16) & 0x3fff
+    for lp in range(n_log):
+        poolK[table[0, lp]] = wl.K[:, lp * pt:(lp + 1) * pt]
+        poolV[table[0, lp]] = wl.V[:, lp * pt:(lp + 1) * pt]
+    dp.K, dp.V = H.dev_u16(poolK), H.dev_u16(poolV)
+    dp.kv_strides = (Hkv * pt * D, D, pt * D)
+    dp.page_table, dp.page_tokens = torch.from_numpy(table).cuda(), pt
+    _check_attn_prefill(dp, lists)
