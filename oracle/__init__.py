@@ -25,6 +25,10 @@ Modules (each function cites the PAPER.md passage it restates):
 * ``projection`` - upstream step f1: selector projections W_q h, W_k h, W_w h and
                    the rotary embedding of q^I / k^I (PAPER.md:39, :362-364;
                    DESIGN.md readings R27-R29).
+* ``training``   - f4: the training-side reductions -- head-averaged teacher
+                   distribution (Eq. 1), student softmax (Eq. 2), DenseKL (Eq. 3)
+                   and SparseKL renormalised on the selector's own top-K set
+                   (Eq. 4); readings R34-R36.
 * ``brute``      - exhaustive enumeration used to pin the nucleus rule on tiny
                    inputs.
 

@@ -133,3 +133,53 @@ def test_fuzz_prefill(torch_cuda, chunk):
         _check_attn_prefill(dp, lists)
         print("fuzz prefill case %d: L=%d q_start=%d Tq=%d B=%d H_q=%d d_idx=%d %s%s near-ties %s"
               % (case, L, dp.q_start, dp.Tq, B, H_q, d_idx, fmt, " paged" if paged else "", report))
+
+
+def test_fuzz_prefill_block16(torch_cuda):
+    """f3: chunked prefill over 16-token key blocks -- random chunk geometries, reserved tiers, selector widths, cache
+    formats, contiguous and paged K/V (recency >= 4 blocks keeps the whole diagonal 64 tokens in every list, so every
+    query row sees at least itself)."""
+    from tests.test_gpu_prefill import _check_attn_prefill, _check_select_prefill
+    from workloads import make_prefill_workload
+    rng = np.random.default_rng(1616)
+    for case in range(8):
+        L = int(rng.choice([256, 640, 1024, 1536]))
+        n_blk = L // 64
+        qb0 = int(rng.integers(0, n_blk))
+        nqb = int(rng.integers(1, min(n_blk - qb0, 6) + 1))
+        B = int(rng.integers(1, 3))
+        over = dict(p=float(rng.choice([0.5, 0.9, 1.0])), sink_blocks=int(rng.integers(0, 9)),
+                    recency_blocks=int(rng.integers(4, 17)), kmin_blocks=int(rng.integers(0, 40)))
+        if rng.random() < 0.25:
+            over = dict(mode="topk", top_k=int(rng.integers(24, 60)), sink_blocks=8, recency_blocks=16)
+        H_q = int(rng.choice([8, 32, 64]))
+        d_idx = int(rng.choice([64, 128]))
+        wls = [make_prefill_workload(seed=16000 + 13 * case + b, L=L, H_q=H_q, d_idx=d_idx, blk=16,
+                                     topic_span=int(rng.choice([64, 128, 256])))
+               for b in range(B)]
+        dp = H.DevicePrefill(wls, qb0 * 64, nqb * 64)
+        fmt = str(rng.choice(["bf16", "bf16", "mxfp4", "fp8_e4m3"]))
+        if fmt != "bf16":
+            dp.set_cache_format(fmt)
+        report = []
+        _check_select_prefill(dp, report, **over)
+        lists = [[sel.indices.tolist() for _, sel in H.oracle_select_prefill(w, dp.q_start, dp.Tq, **over)] for w in wls]
+        paged = rng.random() < 0.4
+        if paged:
+            import torch
+            pt = int(rng.choice([64, 128]))
+            n_log = L // pt
+            table = rng.permutation(B * n_log + 2)[:B * n_log].reshape(B, n_log).astype(np.int32)
+            wl0 = wls[0]
+            poolK = np.zeros((B * n_log + 2, wl0.H_kv, pt, wl0.D), dtype=np.uint16)
+            poolV = np.zeros_like(poolK)
+            for b, w in enumerate(wls):
+                for lp in range(n_log):
+                    poolK[table[b, lp]] = w.K[:, lp * pt:(lp + 1) * pt]
+                    poolV[table[b, lp]] = w.V[:, lp * pt:(lp + 1) * pt]
+            dp.K, dp.V = H.dev_u16(poolK), H.dev_u16(poolV)
+            dp.kv_strides = (wl0.H_kv * pt * wl0.D, wl0.D, pt * wl0.D)
+            dp.page_table, dp.page_tokens = torch.from_numpy(table).cuda(), pt
+        _check_attn_prefill(dp, lists)
+        print("fuzz prefill blk16 case %d: L=%d q_start=%d Tq=%d B=%d H_q=%d d_idx=%d %s%s near-ties %s"
+              % (case, L, dp.q_start, dp.Tq, B, H_q, d_idx, fmt, " paged" if paged else "", report))
