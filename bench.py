@@ -792,6 +792,126 @@ def run_prefill(args):
     print(json.dumps(line))
 
 
+
+# ------------------------------------------------------------------------------------------------------
+# f4: the training-side reductions at the paper's training length (L = 16384, K_train = 8192 tokens = 512 blocks
+# of 16) on the synthetic prefill workload's tensors
+# ------------------------------------------------------------------------------------------------------
+TR_METRIC = "training reductions ms/layer (teacher Eq.1 + DenseKL Eq.3 + SparseKL Eq.4) @L=16K; % of tensor-pipe peak"
+
+
+def oracle_train_sample(wl, n):
+    from oracle import training as OT
+    from oracle.bf16 import bf16_bits_to_f64
+    t0 = time.perf_counter()
+    OT.training_reductions(bf16_bits_to_f64(wl.Q[:n]), bf16_bits_to_f64(wl.K[:, :n]).transpose(1, 0, 2), wl.sm_scale,
+                           bf16_bits_to_f64(wl.sel_q[:n]), wl.w[:n].astype(np.float64), bf16_bits_to_f64(wl.sel_k[:n]),
+                           wl.blk, max(1, n // 32))
+    return time.perf_counter() - t0
+
+
+def run_train(args):
+    from workloads import make_prefill_workload
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    L = args.L or 16384
+    top_k = max(1, L // 32)                      # K_train = 0.5 L tokens = L / 32 blocks of 16 (Table 3)
+    wl = make_prefill_workload(seed=7007 + 1000 * rank, L=L, blk=16, **{k: v for k, v in D_IDX_OVERRIDE.items() if k == "d_idx"})
+    cores = len(os.sched_getaffinity(0))
+    n_cpu = 384
+    pairs_full, pairs_cpu = L * (L + 1) / 2, n_cpu * (n_cpu + 1) / 2
+    if args.impl == "reference":
+        if rank != 0:
+            return
+        ts = [oracle_train_sample(wl, n_cpu) for _ in range(args.warmup + args.steps)][args.warmup:]
+        ms = float(np.mean(ts)) * pairs_full / pairs_cpu * 1e3
+        sample = "the first %d tokens of the sequence (%d of %d causal pairs), time scaled by the pair count" % (n_cpu, pairs_cpu, pairs_full)
+        print(json.dumps({"impl": "reference", "metric": TR_METRIC, "value": ms, "unit": "ms/layer", "n_gpus": args.gpus,
+                          "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": False,
+                          "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+                          "config": {"workload": "train", "L": L, "top_k_blocks": top_k},
+                          "cpu_baseline": {"value": ms, "unit": "ms/layer", "cores": cores, "kind": "oracle", "sample": sample},
+                          "e2e": {"value": ms, "unit": "ms/layer", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}))
+        return
+    import torch
+    torch.cuda.set_device(local_rank)
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    from paper_2606_22874_b200 import _lib, api
+    from paper_2606_22874_b200 import build as B
+    B.build()
+    _lib.load()
+    dev = torch.device("cuda", local_rank)
+    pin = lambda a_: torch.from_numpy(np.ascontiguousarray(a_).view(np.int16)).pin_memory()
+    h = {k: pin(getattr(wl, k)) for k in ("Q", "K", "sel_q", "sel_k")}
+    h_w = torch.from_numpy(wl.w).pin_memory()
+    d = {k: v.to(dev) for k, v in h.items()}
+    w = h_w.to(dev)
+    dkl = torch.empty((L,), device=dev)
+    skl = torch.empty((L,), device=dev)
+    tp = api.make_train_params(d["Q"], d["K"], (wl.D, L * wl.D), d["sel_q"], w, d["sel_k"], L, wl.H_q, wl.H_kv, wl.D,
+                               wl.H_idx, wl.d_idx, blk=16, top_k=top_k, sm_scale=wl.sm_scale, dense_kl=dkl, sparse_kl=skl)
+    ws = torch.empty(api.spot_train_kl_workspace_bytes(tp), dtype=torch.uint8, device=dev)
+    tp.workspace, tp.workspace_bytes = ws.data_ptr(), ws.numel()
+    stream = torch.cuda.current_stream()
+    flush = torch.empty(512 << 20, dtype=torch.uint8, device=dev).zero_()
+    W = max(args.warmup, 3)
+    for _ in range(W):
+        api.spot_train_kl(tp, stream)
+    torch.cuda.synchronize()
+    if world > 1:
+        import torch.distributed as dist
+        dist.barrier()
+    ev = [[torch.cuda.Event(enable_timing=True) for _ in range(2)] for _ in range(args.steps)]
+    with ClockSampler(local_rank) as clk:
+        for i in range(args.steps):
+            flush.view(torch.int64).sum()
+            ev[i][0].record(stream)
+            api.spot_train_kl(tp, stream)
+            ev[i][1].record(stream)
+        torch.cuda.synchronize()
+        e2e = []
+        h_out = torch.empty((2, L), dtype=torch.float32).pin_memory()
+        for i in range(min(args.steps, 5) + 1):
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            for k_ in h:
+                d[k_].copy_(h[k_], non_blocking=True)
+            w.copy_(h_w, non_blocking=True)
+            api.spot_train_kl(tp, stream)
+            h_out[0].copy_(dkl, non_blocking=True)
+            h_out[1].copy_(skl, non_blocking=True)
+            torch.cuda.synchronize()
+            if i >= 1:
+                e2e.append((time.perf_counter() - t0) * 1e3)
+    ms = max_over_ranks(float(np.mean([e[0].elapsed_time(e[1]) for e in ev])), dev, world)
+    if rank != 0:
+        return
+    burst, sustained, peak_src = tensor_peaks()
+    flop = 2.0 * (2.0 * pairs_full * wl.H_q * wl.D) + 2.0 * (2.0 * pairs_full * wl.H_idx * wl.d_idx)   # two passes: teacher + selector
+    achieved = flop / (ms * 1e-3) / 1e12
+    cpu_t = oracle_train_sample(wl, n_cpu)
+    print(json.dumps({
+        "metric": TR_METRIC, "value": ms, "unit": "ms/layer", "n_gpus": world, "steps": args.steps, "warmup": W,
+        "ms_per_step": ms, "higher_is_better": False, "scaling": "weak", "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
+        "config": {"workload": "train", "L": L, "H_q": wl.H_q, "H_kv": wl.H_kv, "D": wl.D,
+                   "selector": "%dx%d bf16" % (wl.H_idx, wl.d_idx), "blk": 16, "top_k_blocks": top_k,
+                   "l2": "flushed by a 512 MiB read sweep before every timed step"},
+        "losses": {"dense_kl_mean": float(dkl.mean()), "sparse_kl_mean": float(skl.mean())},
+        "tokens_per_s": world * L / (ms * 1e-3),
+        "roofline": {"bound": "tensor", "kernel": "train_pass_kernel (mma.sync; both passes)", "achieved": achieved,
+                     "peak": sustained, "unit": "TFLOP/s", "frac": achieved / sustained, "traffic": None,
+                     "peak_source": peak_src + "; sustained figure: the two passes run for milliseconds",
+                     "algorithmic_flops": flop},
+        "cpu_baseline": {"value": cpu_t * pairs_full / pairs_cpu * 1e3, "unit": "ms/layer", "cores": cores, "kind": "oracle",
+                         "sample": "the first %d tokens of the sequence, time scaled by the causal pair count" % n_cpu},
+        "e2e": {"value": float(np.mean(e2e)), "unit": "ms/layer",
+                "h2d_bytes_per_step": int(sum(v.numel() * 2 for v in h.values()) + h_w.numel() * 4), "d2h_bytes_per_step": 8 * L},
+        "gpu_launches": 6 * args.steps, "clocks": clk.summary()}))
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -817,7 +937,9 @@ def main():
         D_IDX_OVERRIDE["d_idx"] = args.d_idx
     if args.blk == 16 and args.workload != "cfg5":
         D_IDX_OVERRIDE.update(blk=16, sink_blocks=8, recency_blocks=16, kmin_blocks=32)
-    if args.workload == "cfg5":
+    if args.workload == "train":
+        run_train(args)
+    elif args.workload == "cfg5":
         run_prefill(args)
     elif args.impl == "reference":
         run_reference(args)

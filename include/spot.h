@@ -66,8 +66,8 @@ int spot_last_cuda_error(void);
 /* Library version, "major.minor". */
 const char* spot_version(void);
 /* sizeof() of the parameter blocks as this library was compiled (which: 0 = spot_select_params,
- * 1 = spot_attn_params, 2 = spot_decode_step_host_params, 3 = spot_project_params, 4 = spot_decode_step_params; anything
- * else: 0) -- lets a binding verify its layout. */
+ * 1 = spot_attn_params, 2 = spot_decode_step_host_params, 3 = spot_project_params, 4 = spot_decode_step_params,
+ * 5 = spot_train_params; anything else: 0) -- lets a binding verify its layout. */
 size_t spot_struct_size(int which);
 
 /* ---------------------------------------------------------------------------------------------------
@@ -314,6 +314,48 @@ typedef struct {
 } spot_decode_step_host_params;
 
 spot_status spot_decode_step_host(const spot_decode_step_host_params* p, void* stream);
+
+/* ---------------------------------------------------------------------------------------------------
+ * f4 -- the training-side reductions of ONE sequence (the other half of the method), on synthetic or real
+ * tensors alike; no L x L matrix is stored.
+ *   teacher  p^tau[q,t]   = (1/H_q) sum_h softmax_t(sm_scale q_h . k_{g(h),t})  over t <= q   (Eq. 1: softmax, then mean)
+ *   student  p^sigma[q,t] = softmax_t(s_s[q,t]) over t <= q, s_s as in spot_select              (Eq. 2)
+ *   dense_kl[q]  = sum_t p^tau log(p^tau / p^sigma)                                             (Eq. 3; the loss is its mean)
+ *   sparse_kl[q] = the same over S_q with both distributions renormalised there                 (Eq. 4)
+ * S_q (R35) = the tokens t <= q of the top_k best key blocks of query q by block-max score -- Eq. 6 applied per
+ * query, reserved sink / recency blocks counted inside top_k as in spot_select; the paper's K_train = 8192 tokens at
+ * blk = 16 is top_k = 512.  0 log 0 = 0; a query whose S_q carries no teacher mass gets 0.
+ *   q      [L][H_q][D] BF16          k  BF16 with element strides (token, head), D contiguous (no V: nothing here needs it)
+ *   sel_q  [L][H_idx][d_idx] BF16    w  [L][H_idx] fp32      sel_k  [L][H_idx][d_idx] BF16 (the BF16 cache layout)
+ *   dense_kl, sparse_kl  out fp32 [L];  teacher_lse  optional out fp32 [L][H_q], natural-log sum-exp of the scaled logits
+ *   indices / budgets    optional out (both or neither): the block lists of S_q, int32 [L][cap] ascending, -1 padded, and
+ *                        their lengths; cap >= min(top_k, ceil(L / blk))
+ * Requires D == 128, H_kv <= 8, H_q / H_kv in {2, 4, 8, 16}, H_idx <= 4, d_idx % 16 == 0 and <= 128, blk in {16, 32, 64},
+ * ceil(L / blk) <= 8192 (SPOT_ERR_UNSUPPORTED otherwise).  fp32 softmax statistics and sums; the logits are exact BF16
+ * products accumulated in fp32.
+ * --------------------------------------------------------------------------------------------------- */
+typedef struct {
+    const uint16_t* q;
+    const uint16_t* k;
+    int64_t k_stride_token, k_stride_head;   /* in elements */
+    const uint16_t* sel_q;
+    const float* w;
+    const uint16_t* sel_k;
+    int32_t L, H_q, H_kv, D, H_idx, d_idx;
+    int32_t blk, top_k, sink_blocks, recency_blocks;
+    float sm_scale;
+    float* dense_kl;
+    float* sparse_kl;
+    float* teacher_lse;          /* optional */
+    int32_t* indices;            /* optional */
+    int32_t* budgets;            /* optional */
+    int32_t cap;
+    void* workspace;
+    size_t workspace_bytes;      /* >= spot_train_kl_workspace_bytes(&params)                             */
+} spot_train_params;
+
+size_t spot_train_kl_workspace_bytes(const spot_train_params* p);
+spot_status spot_train_kl(const spot_train_params* p, void* stream);
 
 #ifdef __cplusplus
 }

@@ -73,6 +73,19 @@ class ProjectParams(C.Structure):
     ]
 
 
+class TrainParams(C.Structure):
+    _fields_ = [
+        ("q", C.c_void_p), ("k", C.c_void_p), ("k_stride_token", C.c_int64), ("k_stride_head", C.c_int64),
+        ("sel_q", C.c_void_p), ("w", C.c_void_p), ("sel_k", C.c_void_p),
+        ("L", C.c_int32), ("H_q", C.c_int32), ("H_kv", C.c_int32), ("D", C.c_int32), ("H_idx", C.c_int32), ("d_idx", C.c_int32),
+        ("blk", C.c_int32), ("top_k", C.c_int32), ("sink_blocks", C.c_int32), ("recency_blocks", C.c_int32),
+        ("sm_scale", C.c_float),
+        ("dense_kl", C.c_void_p), ("sparse_kl", C.c_void_p), ("teacher_lse", C.c_void_p),
+        ("indices", C.c_void_p), ("budgets", C.c_void_p), ("cap", C.c_int32),
+        ("workspace", C.c_void_p), ("workspace_bytes", C.c_size_t),
+    ]
+
+
 # every symbol include/spot.h declares: name -> (restype, argtypes)
 PROTOTYPES = {
     "spot_status_string": (C.c_char_p, [C.c_int]),
@@ -98,6 +111,8 @@ PROTOTYPES = {
     "spot_decode_step": (C.c_int, [C.POINTER(DecodeStepParams), C.c_void_p]),
     "spot_selector_project_append_workspace_bytes": (C.c_size_t, [C.POINTER(ProjectParams)]),
     "spot_selector_project_append": (C.c_int, [C.POINTER(ProjectParams), C.c_void_p]),
+    "spot_train_kl_workspace_bytes": (C.c_size_t, [C.POINTER(TrainParams)]),
+    "spot_train_kl": (C.c_int, [C.POINTER(TrainParams), C.c_void_p]),
 }
 
 _lib = None
@@ -116,7 +131,7 @@ def load():
             fn = getattr(lib, name)
             fn.restype = res
             fn.argtypes = args
-        for which, st in enumerate((SelectParams, AttnParams, DecodeStepHostParams, ProjectParams, DecodeStepParams)):
+        for which, st in enumerate((SelectParams, AttnParams, DecodeStepHostParams, ProjectParams, DecodeStepParams, TrainParams)):
             if lib.spot_struct_size(which) != C.sizeof(st):
                 raise RuntimeError("ABI mismatch: %s is %d bytes in libspot.so, %d in the binding"
                                    % (st.__name__, lib.spot_struct_size(which), C.sizeof(st)))

@@ -7,7 +7,8 @@ import ctypes as C
 import torch
 
 from . import _lib as L
-from ._lib import AttnParams, DecodeStepHostParams, DecodeStepParams, ProjectParams, SelectParams, FORMATS, MODES  # noqa: F401
+from ._lib import (AttnParams, DecodeStepHostParams, DecodeStepParams, ProjectParams, SelectParams, TrainParams,  # noqa: F401
+                   FORMATS, MODES)
 
 
 class SpotError(RuntimeError):
@@ -187,3 +188,31 @@ def spot_selector_project_append_workspace_bytes(pp):
 
 def spot_selector_project_append(pp, stream=None):
     _check(L.load().spot_selector_project_append(C.byref(pp), _stream(stream)), "spot_selector_project_append")
+
+
+def make_train_params(q, k, k_strides, sel_q, w, sel_k, L, H_q, H_kv, D, H_idx, d_idx, *, blk=16, top_k=512, sink_blocks=0,
+                      recency_blocks=0, sm_scale=None, dense_kl=None, sparse_kl=None, teacher_lse=None, indices=None,
+                      budgets=None, cap=0, workspace=None):
+    tp = TrainParams()
+    tp.q, tp.k = q.data_ptr(), k.data_ptr()
+    tp.k_stride_token, tp.k_stride_head = k_strides
+    tp.sel_q, tp.w, tp.sel_k = sel_q.data_ptr(), w.data_ptr(), sel_k.data_ptr()
+    tp.L, tp.H_q, tp.H_kv, tp.D, tp.H_idx, tp.d_idx = L, H_q, H_kv, D, H_idx, d_idx
+    tp.blk, tp.top_k, tp.sink_blocks, tp.recency_blocks = blk, top_k, sink_blocks, recency_blocks
+    tp.sm_scale = float(D ** -0.5 if sm_scale is None else sm_scale)
+    tp.dense_kl, tp.sparse_kl = dense_kl.data_ptr(), sparse_kl.data_ptr()
+    tp.teacher_lse = teacher_lse.data_ptr() if teacher_lse is not None else None
+    tp.indices = indices.data_ptr() if indices is not None else None
+    tp.budgets = budgets.data_ptr() if budgets is not None else None
+    tp.cap = cap
+    if workspace is not None:
+        tp.workspace, tp.workspace_bytes = workspace.data_ptr(), workspace.numel() * workspace.element_size()
+    return tp
+
+
+def spot_train_kl_workspace_bytes(tp):
+    return int(L.load().spot_train_kl_workspace_bytes(C.byref(tp)))
+
+
+def spot_train_kl(tp, stream=None):
+    _check(L.load().spot_train_kl(C.byref(tp), _stream(stream)), "spot_train_kl")

@@ -12,7 +12,7 @@ CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libspot.so")
 SOURCES = ["api.cu", "quantize.cu", "score_decode.cu", "select.cu", "select_hist.cu", "attn_decode.cu", "score_prefill.cu",
-           "attn_prefill.cu", "attn_prefill_tc.cu", "project.cu"]
+           "attn_prefill.cu", "attn_prefill_tc.cu", "project.cu", "train_kl.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "--expt-relaxed-constexpr"]
 

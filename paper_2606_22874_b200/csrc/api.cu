@@ -177,6 +177,7 @@ extern "C" size_t spot_struct_size(int which) {
         case 2: return sizeof(spot_decode_step_host_params);
         case 3: return sizeof(spot_project_params);
         case 4: return sizeof(spot_decode_step_params);
+        case 5: return sizeof(spot_train_params);
     }
     return 0;
 }

@@ -1,0 +1,539 @@
+// f4 -- the training-side reductions of one sequence (readings R34-R36):
+//   teacher  p^tau[q,t]   = (1/H_q) sum_h softmax_t(sm_scale q_h . k_{g(h),t})      (Eq. 1: softmax, THEN mean over heads)
+//   student  p^sigma[q,t] = softmax_t(s_s[q,t]),  s_s = sum_h w_h ReLU(q^I_h . k^I_{h,t})          (Eq. 2)
+//   DenseKL[q]  = sum_{t<=q} p^tau log(p^tau / p^sigma)                                                        (Eq. 3)
+//   SparseKL[q] = the same over S_q, both distributions renormalised there                                    (Eq. 4)
+// with S_q the tokens of the top_k best blocks of query q by block-max score (Eq. 6 applied per query, R35).
+//
+// No L x L matrix is ever stored.  Two passes over the causal (query, key) plane, the selection kernel in between:
+//   pass 1  per (query, head) the log-sum-exp of the teacher logits; per query the log-sum-exp of the student scores and
+//           its block maxima s_bar[q, b]                                          -> workspace
+//   select  select_hist_kernel in its decode form on L rows (row q sees q + 1 tokens), top-K -> block lists -> bit masks
+//   pass 2  per (query, key): p^tau from the stored log-sum-exps (a sum over ALL heads: the one cross-warp step), the
+//           student log-probability, membership of the key's block in S_q; per query the four running sums the two KLs
+//           are made of.
+// A CTA owns 32 / G queries (G = H_q / H_kv) and walks its visible keys in tiles of 32.  Warps 0-7: one KV head each,
+// rows of the MMA = (query, head of the group), query-major, so that the head sum of Eq. 1 is a shuffle over row lanes;
+// warp 8: the selector scores of the same tile.  Every warp streams its own operand through a private cp.async ring (as
+// in attn_decode.cu); mma.sync m16n8k16, fp32 accumulate.  (A dense contraction: a tcgen05 form -- S in TMEM, rows =
+// (head, query) as in attn_prefill_tc.cu -- is the next step; this first form is correctness and a measured baseline.)
+#include "select_common.cuh"
+
+#include <string.h>
+
+namespace spot {
+
+spot_status run_select(const spot_select_params* p, const float* scores, int nb_stride, int rows_per_seq, int max_nb,
+                       const StepSync* sync, cudaStream_t s);                                   // select.cu
+
+namespace {
+
+constexpr int TR_KT = 32;                       // keys per tile
+constexpr int TR_TW = 8;                        // teacher warps = KV heads per CTA
+constexpr int TR_THREADS = (TR_TW + 1) * 32;
+constexpr int TR_STAGES = 2;
+constexpr int TR_D = 128;
+constexpr int TR_KSTAGE = TR_KT * TR_D * 2;     // 8 KiB: one K sub-tile of one KV head
+constexpr int TR_QMAX = 16;                     // queries per CTA at most (G = 2)
+
+struct TrainArgs {
+    const uint16_t* q;           // [L][H_q][128]
+    const uint16_t* k;           // token / head strides in elements
+    int64_t k_st, k_sh;
+    const uint16_t* sel_q;       // [L][H][d]
+    const float* w;              // [L][H]
+    const uint16_t* sel_k;       // [L][H][d]
+    int L, H_q, H_kv, G, H_idx, d_idx, blk;
+    float scale_log2;
+    float* t_lse2;               // [L][H_q] log2-domain log-sum-exp of the scaled teacher logits
+    float* s_lse;                // [L] natural-log log-sum-exp of the student scores
+    float* blk_scores;           // [L][nb_stride]
+    int nb_stride;
+    const uint32_t* mask;        // [L][mask_stride] bit b: block b is in S_q
+    int mask_stride;
+    float* dense_kl;
+    float* sparse_kl;
+    float* teacher_lse;          // optional, natural log
+};
+
+__device__ __forceinline__ uint32_t tr_sw(int row, int chunk, int row_bytes) {
+    return (uint32_t)(row * row_bytes + ((chunk ^ (row & 7)) << 4));
+}
+
+// rows x row_bytes from global (row stride in elements) into a swizzled stage; rows at or past n_valid are zero-filled
+__device__ __forceinline__ void tr_issue(uint32_t stage, const uint16_t* base, int64_t stride, int row0, int n_rows_total,
+                                         int row_bytes, int lane) {
+    const int chunks = row_bytes >> 4;
+    for (int id = lane; id < TR_KT * chunks; id += 32) {
+        const int row = id / chunks, ch = id - row * chunks;
+        const bool ok = row0 + row < n_rows_total;
+        cp_async16(stage + tr_sw(row, ch, row_bytes), base + (int64_t)(ok ? row0 + row : 0) * stride + ch * 8, ok);
+    }
+}
+
+template <int PASS>
+__global__ void __launch_bounds__(TR_THREADS, 1) train_pass_kernel(TrainArgs a) {
+    extern __shared__ __align__(128) unsigned char smem[];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int g = lane >> 2, c = lane & 3;
+    const int G = a.G, QPT = 16 / G, QPC = 2 * QPT;
+    const int n_tiles_q = (a.L + QPC - 1) / QPC;
+    const int q0 = (n_tiles_q - 1 - (int)blockIdx.x) * QPC;            // heaviest (latest) queries first
+    const int q_end = min(q0 + QPC, a.L);                              // one past the CTA's last query
+    const int n_kt = (q_end + TR_KT - 1) / TR_KT;                      // key tiles: keys 0 .. q_end - 1
+    const int srow_bytes = a.H_idx * a.d_idx * 2;                      // one token of the selector cache
+    // shared memory: [8 warps][2 stages][8 KiB] K | [2 stages][32 x srow_bytes] selector K | sP[2][16][32] | sS[2][16][32]
+    const uint32_t k_ring = smem_u32(smem) + warp * (TR_STAGES * TR_KSTAGE);
+    const uint32_t s_ring = smem_u32(smem) + TR_TW * TR_STAGES * TR_KSTAGE;
+    float* sP = reinterpret_cast<float*>(smem + TR_TW * TR_STAGES * TR_KSTAGE + TR_STAGES * TR_KT * srow_bytes);
+    float* sS = sP + 2 * TR_QMAX * TR_KT;
+    const uint32_t sQ = smem_u32(sS + 2 * TR_QMAX * TR_KT);            // student: its 16 query rows, swizzled like a key tile
+    if (PASS == 2) {
+        for (int e = threadIdx.x; e < 2 * TR_QMAX * TR_KT; e += TR_THREADS) sP[e] = 0.f;
+        __syncthreads();
+    }
+
+    // ------------------------------------------------------------------------------------------------------------
+    // per-warp state
+    // ------------------------------------------------------------------------------------------------------------
+    const bool teacher = warp < TR_TW && warp < a.H_kv;
+    const bool student = warp == TR_TW;
+    uint32_t qf[2][8][4];                       // teacher: Q fragments of the two m-tiles
+    float swt[4][2];                            // student: w_h of rows g and g + 8
+    float st_m[2][2], st_l[2][2];               // pass 1: online (max, sum) of rows (m-tile j, half)
+    float row_lse[2][2];                        // pass 2 (teacher): log2-domain LSE of the rows
+    float bm[2] = {-INFINITY, -INFINITY};       // pass 1 (student): running maximum of the current key block
+    const int ks_sel = a.d_idx >> 4;            // k-steps per selector head
+#pragma unroll
+    for (int j = 0; j < 2; ++j)
+#pragma unroll
+        for (int hf = 0; hf < 2; ++hf) { st_m[j][hf] = -INFINITY; st_l[j][hf] = 0.f; row_lse[j][hf] = 0.f; }
+
+    // row r of m-tile j: query q0 + j QPT + r / G, head hk G + r % G (query-major: the heads of a query sit on
+    // consecutive row lanes)
+    auto row_query = [&](int j, int r) -> int { return q0 + j * QPT + r / G; };
+    if (teacher) {
+        const int hk = warp;
+#pragma unroll
+        for (int j = 0; j < 2; ++j) {
+            const int ra = g, rb = g + 8;
+            const int qa = row_query(j, ra), qb = row_query(j, rb);
+            const uint16_t* pa = a.q + ((int64_t)qa * a.H_q + hk * G + ra % G) * TR_D;
+            const uint16_t* pb = a.q + ((int64_t)qb * a.H_q + hk * G + rb % G) * TR_D;
+#pragma unroll
+            for (int ks = 0; ks < 8; ++ks) {
+                const int col = ks * 16 + c * 2;
+                qf[j][ks][0] = qa < a.L ? *reinterpret_cast<const uint32_t*>(pa + col) : 0u;
+                qf[j][ks][1] = qb < a.L ? *reinterpret_cast<const uint32_t*>(pb + col) : 0u;
+                qf[j][ks][2] = qa < a.L ? *reinterpret_cast<const uint32_t*>(pa + col + 8) : 0u;
+                qf[j][ks][3] = qb < a.L ? *reinterpret_cast<const uint32_t*>(pb + col + 8) : 0u;
+            }
+            if (PASS == 2) {
+                row_lse[j][0] = qa < a.L ? a.t_lse2[(int64_t)qa * a.H_q + hk * G + ra % G] : 0.f;
+                row_lse[j][1] = qb < a.L ? a.t_lse2[(int64_t)qb * a.H_q + hk * G + rb % G] : 0.f;
+            }
+        }
+    }
+    if (student) {
+        // rows = the CTA's queries (QPC <= 16), the rest zero
+        const int qa = q0 + g, qb = q0 + g + 8;
+        const bool va = g < QPC && qa < a.L, vb = g + 8 < QPC && qb < a.L;
+#pragma unroll
+        for (int h = 0; h < 4; ++h) {
+            swt[h][0] = (va && h < a.H_idx) ? a.w[(int64_t)qa * a.H_idx + h] : 0.f;
+            swt[h][1] = (vb && h < a.H_idx) ? a.w[(int64_t)qb * a.H_idx + h] : 0.f;
+        }
+        // the selector queries go to shared memory once (their fragments would cost 128 registers at d_idx = 128)
+        const int chunks = srow_bytes >> 4;
+        for (int id = lane; id < 16 * chunks; id += 32) {
+            const int row = id / chunks, ch = id - row * chunks;
+            uint4 v = make_uint4(0u, 0u, 0u, 0u);
+            if (row < QPC && q0 + row < a.L)
+                v = *reinterpret_cast<const uint4*>(a.sel_q + (int64_t)(q0 + row) * (a.H_idx * a.d_idx) + ch * 8);
+            asm volatile("st.shared.v4.u32 [%0], {%1,%2,%3,%4};" :: "r"(sQ + tr_sw(row, ch, srow_bytes)), "r"(v.x), "r"(v.y),
+                         "r"(v.z), "r"(v.w) : "memory");
+        }
+        __syncwarp();
+    }
+
+    // pass 2: the KL sums of this thread's (query, key lane) elements: element e = tid + 256 i -> query e / 32, lane e % 32
+    float acc_d[2] = {0.f, 0.f}, acc_a[2] = {0.f, 0.f}, acc_b[2] = {0.f, 0.f}, acc_c[2] = {0.f, 0.f};
+    float my_slse[2] = {0.f, 0.f};
+    if (PASS == 2 && warp < TR_TW) {
+#pragma unroll
+        for (int i = 0; i < 2; ++i) {
+            const int q = q0 + warp + 8 * i;
+            if (warp + 8 * i < QPC && q < a.L) my_slse[i] = a.s_lse[q];
+        }
+    }
+
+    // ------------------------------------------------------------------------------------------------------------
+    // the key loop
+    // ------------------------------------------------------------------------------------------------------------
+    auto issue = [&](int kt) {
+        if (teacher) tr_issue(k_ring + (kt % TR_STAGES) * TR_KSTAGE, a.k + (int64_t)warp * a.k_sh, a.k_st, kt * TR_KT, q_end,
+                              TR_D * 2, lane);
+        if (student) tr_issue(s_ring + (kt % TR_STAGES) * (TR_KT * srow_bytes), a.sel_k, a.H_idx * a.d_idx, kt * TR_KT, q_end,
+                              srow_bytes, lane);
+        cp_async_commit();
+    };
+    issue(0);
+    for (int kt = 0; kt < n_kt; ++kt) {
+        if (kt + 1 < n_kt) issue(kt + 1); else cp_async_commit();
+        cp_async_wait<1>();
+        __syncwarp();
+        const int t0 = kt * TR_KT, buf = kt & 1;
+        const int mi = lane >> 3, r8 = lane & 7;
+
+        if (teacher) {
+            const uint32_t kb = k_ring + (kt % TR_STAGES) * TR_KSTAGE;
+            float s[2][4][4];
+#pragma unroll
+            for (int j = 0; j < 2; ++j)
+#pragma unroll
+                for (int nt = 0; nt < 4; ++nt) s[j][nt][0] = s[j][nt][1] = s[j][nt][2] = s[j][nt][3] = 0.f;
+#pragma unroll
+            for (int ks = 0; ks < 8; ++ks)
+#pragma unroll
+                for (int half = 0; half < 2; ++half) {
+                    uint32_t b0, b1, b2, b3;
+                    ldmatrix_x4(b0, b1, b2, b3, kb + tr_sw(half * 16 + (mi >> 1) * 8 + r8, 2 * ks + (mi & 1), TR_D * 2));
+#pragma unroll
+                    for (int j = 0; j < 2; ++j) {
+                        mma_bf16_16816(s[j][half * 2], qf[j][ks][0], qf[j][ks][1], qf[j][ks][2], qf[j][ks][3], b0, b1);
+                        mma_bf16_16816(s[j][half * 2 + 1], qf[j][ks][0], qf[j][ks][1], qf[j][ks][2], qf[j][ks][3], b2, b3);
+                    }
+                }
+            // log2 domain, causal mask (key <= query) and rows past the sequence
+#pragma unroll
+            for (int j = 0; j < 2; ++j)
+#pragma unroll
+                for (int hf = 0; hf < 2; ++hf) {
+                    const int q = row_query(j, g + 8 * hf);
+                    float v[8];
+#pragma unroll
+                    for (int nt = 0; nt < 4; ++nt)
+#pragma unroll
+                        for (int e = 0; e < 2; ++e) {
+                            const int key = t0 + nt * 8 + c * 2 + e;
+                            v[nt * 2 + e] = (q < a.L && key <= q) ? s[j][nt][hf * 2 + e] * a.scale_log2 : -INFINITY;
+                        }
+                    if (PASS == 1) {
+                        float mx = v[0];
+#pragma unroll
+                        for (int i = 1; i < 8; ++i) mx = fmaxf(mx, v[i]);
+                        const float mn = fmaxf(st_m[j][hf], mx);
+                        if (mn > -INFINITY) {
+                            float sum = 0.f;
+#pragma unroll
+                            for (int i = 0; i < 8; ++i) sum += fast_exp2(v[i] - mn);
+                            st_l[j][hf] = st_l[j][hf] * fast_exp2(st_m[j][hf] - mn) + sum;
+                            st_m[j][hf] = mn;
+                        }
+                    } else {
+                        // p_h = exp2(v - lse_h); Eq. 1's sum over the heads of the group = over the G row lanes of the query
+#pragma unroll
+                        for (int i = 0; i < 8; ++i) {
+                            float p = fast_exp2(v[i] - row_lse[j][hf]);
+                            if (G >= 2) p += __shfl_xor_sync(0xffffffffu, p, 4);
+                            if (G >= 4) p += __shfl_xor_sync(0xffffffffu, p, 8);
+                            if (G >= 8) p += __shfl_xor_sync(0xffffffffu, p, 16);
+                            v[i] = p;
+                        }
+                        // (G == 16: rows g and g + 8 are the same query -- both halves add into its slot)
+                        const int r = g + 8 * hf;
+                        if (r % G == 0 || (G == 16 && g == 0)) {
+                            const int ql = j * QPT + r / G;
+#pragma unroll
+                            for (int nt = 0; nt < 4; ++nt)
+#pragma unroll
+                                for (int e = 0; e < 2; ++e)
+                                    atomicAdd(&sP[(buf * TR_QMAX + ql) * TR_KT + nt * 8 + c * 2 + e], v[nt * 2 + e]);
+                        }
+                    }
+                }
+        }
+
+        if (student) {
+            const uint32_t sb = s_ring + (kt % TR_STAGES) * (TR_KT * srow_bytes);
+            float sv[4][4];
+#pragma unroll
+            for (int nt = 0; nt < 4; ++nt) sv[nt][0] = sv[nt][1] = sv[nt][2] = sv[nt][3] = 0.f;
+#pragma unroll
+            for (int h = 0; h < 4; ++h) {
+                if (h < a.H_idx) {
+                    float acc[4][4];
+#pragma unroll
+                    for (int nt = 0; nt < 4; ++nt) acc[nt][0] = acc[nt][1] = acc[nt][2] = acc[nt][3] = 0.f;
+#pragma unroll
+                    for (int ks = 0; ks < 8; ++ks) {
+                        if (ks < ks_sel) {
+                            const int ch0 = h * (a.d_idx >> 3) + 2 * ks;
+                            uint32_t a0, a1, a2, a3;
+                            ldmatrix_x4(a0, a1, a2, a3, sQ + tr_sw((mi & 1) * 8 + r8, ch0 + (mi >> 1), srow_bytes));
+#pragma unroll
+                            for (int half = 0; half < 2; ++half) {
+                                uint32_t b0, b1, b2, b3;
+                                ldmatrix_x4(b0, b1, b2, b3, sb + tr_sw(half * 16 + (mi >> 1) * 8 + r8, ch0 + (mi & 1), srow_bytes));
+                                mma_bf16_16816(acc[half * 2], a0, a1, a2, a3, b0, b1);
+                                mma_bf16_16816(acc[half * 2 + 1], a0, a1, a2, a3, b2, b3);
+                            }
+                        }
+                    }
+#pragma unroll
+                    for (int nt = 0; nt < 4; ++nt) {
+                        sv[nt][0] = fmaf(swt[h][0], fmaxf(acc[nt][0], 0.f), sv[nt][0]);
+                        sv[nt][1] = fmaf(swt[h][0], fmaxf(acc[nt][1], 0.f), sv[nt][1]);
+                        sv[nt][2] = fmaf(swt[h][1], fmaxf(acc[nt][2], 0.f), sv[nt][2]);
+                        sv[nt][3] = fmaf(swt[h][1], fmaxf(acc[nt][3], 0.f), sv[nt][3]);
+                    }
+                }
+            }
+#pragma unroll
+            for (int hf = 0; hf < 2; ++hf) {
+                const int ql = g + 8 * hf, q = q0 + ql;
+                const bool rowok = ql < QPC && q < a.L;
+                if (PASS == 1) {
+#pragma unroll
+                    for (int nt = 0; nt < 4; ++nt) {
+                        const int key0 = t0 + nt * 8;
+                        float v0 = (rowok && key0 + c * 2 <= q) ? sv[nt][hf * 2] : -INFINITY;
+                        float v1 = (rowok && key0 + c * 2 + 1 <= q) ? sv[nt][hf * 2 + 1] : -INFINITY;
+                        // online log-sum-exp of the row (natural log; this thread's columns, merged over the quad at the end)
+                        const float mx = fmaxf(v0, v1), mn = fmaxf(st_m[0][hf], mx);
+                        if (mn > -INFINITY) {
+                            st_l[0][hf] = st_l[0][hf] * __expf(st_m[0][hf] - mn) + __expf(v0 - mn) + __expf(v1 - mn);
+                            st_m[0][hf] = mn;
+                        }
+                        // block maxima: flushed when the 8 keys end a block
+                        bm[hf] = fmaxf(bm[hf], mx);
+                        if ((key0 + 8) % a.blk == 0 || (kt == n_kt - 1 && nt == 3)) {
+                            float m = bm[hf];
+                            m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, 1));
+                            m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, 2));
+                            if (c == 0 && m > -INFINITY) a.blk_scores[(int64_t)q * a.nb_stride + key0 / a.blk] = m;
+                            bm[hf] = -INFINITY;
+                        }
+                    }
+                } else if (ql < TR_QMAX) {
+#pragma unroll
+                    for (int nt = 0; nt < 4; ++nt) {
+                        sS[(buf * TR_QMAX + ql) * TR_KT + nt * 8 + c * 2] = sv[nt][hf * 2];
+                        sS[(buf * TR_QMAX + ql) * TR_KT + nt * 8 + c * 2 + 1] = sv[nt][hf * 2 + 1];
+                    }
+                }
+            }
+        }
+
+        if (PASS == 2) {
+            __syncthreads();                    // the tile's head sums and student scores are in shared memory
+            if (warp < TR_TW) {
+#pragma unroll
+                for (int i = 0; i < 2; ++i) {
+                    const int ql = warp + 8 * i, q = q0 + ql, t = t0 + lane;
+                    if (ql < QPC) {
+                        const int at = (buf * TR_QMAX + ql) * TR_KT + lane;
+                        const float pt = sP[at] / (float)a.H_q;
+                        sP[at] = 0.f;                                   // re-armed for tile kt + 2
+                        if (q < a.L && t <= q) {
+                            const float lps = sS[at] - my_slse[i];      // log p^sigma
+                            const int b = t / a.blk;
+                            const bool in_s = (a.mask[(int64_t)q * a.mask_stride + (b >> 5)] >> (b & 31)) & 1u;
+                            if (in_s) acc_b[i] += __expf(lps);
+                            if (pt > 0.f) {
+                                const float term = pt * (__logf(pt) - lps);
+                                acc_d[i] += term;
+                                if (in_s) { acc_a[i] += pt; acc_c[i] += term; }
+                            }
+                        }
+                    }
+                }
+            }
+        }
+        __syncwarp();                           // the stage is free for the request after next
+    }
+    cp_async_wait<0>();
+
+    // ------------------------------------------------------------------------------------------------------------
+    // results
+    // ------------------------------------------------------------------------------------------------------------
+    if (PASS == 1) {
+        if (teacher) {
+#pragma unroll
+            for (int j = 0; j < 2; ++j)
+#pragma unroll
+                for (int hf = 0; hf < 2; ++hf) {
+                    float m = st_m[j][hf], l = st_l[j][hf];
+#pragma unroll
+                    for (int o = 1; o <= 2; o <<= 1) {
+                        const float m2 = __shfl_xor_sync(0xffffffffu, m, o), l2 = __shfl_xor_sync(0xffffffffu, l, o);
+                        const float M = fmaxf(m, m2);
+                        if (M > -INFINITY) { l = l * fast_exp2(m - M) + l2 * fast_exp2(m2 - M); m = M; }
+                    }
+                    const int r = g + 8 * hf, q = row_query(j, r);
+                    if (c == 0 && q < a.L) {
+                        const float lse2 = m + log2f(l);
+                        a.t_lse2[(int64_t)q * a.H_q + warp * G + r % G] = lse2;
+                        if (a.teacher_lse) a.teacher_lse[(int64_t)q * a.H_q + warp * G + r % G] = lse2 * 0.6931471805599453f;
+                    }
+                }
+        }
+        if (student) {
+#pragma unroll
+            for (int hf = 0; hf < 2; ++hf) {
+                float m = st_m[0][hf], l = st_l[0][hf];
+#pragma unroll
+                for (int o = 1; o <= 2; o <<= 1) {
+                    const float m2 = __shfl_xor_sync(0xffffffffu, m, o), l2 = __shfl_xor_sync(0xffffffffu, l, o);
+                    const float M = fmaxf(m, m2);
+                    if (M > -INFINITY) { l = l * __expf(m - M) + l2 * __expf(m2 - M); m = M; }
+                }
+                const int ql = g + 8 * hf, q = q0 + ql;
+                if (c == 0 && ql < QPC && q < a.L) a.s_lse[q] = m + __logf(l);
+            }
+        }
+    } else if (warp < TR_TW) {
+#pragma unroll
+        for (int i = 0; i < 2; ++i) {
+            float d = acc_d[i], A = acc_a[i], B = acc_b[i], C = acc_c[i];
+#pragma unroll
+            for (int o = 16; o; o >>= 1) {
+                d += __shfl_xor_sync(0xffffffffu, d, o);
+                A += __shfl_xor_sync(0xffffffffu, A, o);
+                B += __shfl_xor_sync(0xffffffffu, B, o);
+                C += __shfl_xor_sync(0xffffffffu, C, o);
+            }
+            const int ql = warp + 8 * i, q = q0 + ql;
+            if (lane == 0 && ql < QPC && q < a.L) {
+                a.dense_kl[q] = d;
+                // Eq. 4: sum_S (p/A) log((p/A) / (s/B)) = C / A - log A + log B
+                a.sparse_kl[q] = A > 0.f ? C / A - __logf(A) + __logf(B) : 0.f;
+            }
+        }
+    }
+}
+
+// row q of the selection sees q + 1 tokens
+__global__ void iota_len_kernel(int32_t* seq_len, int L) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < L) seq_len[i] = i + 1;
+}
+// block lists -> bit masks (one warp per query; the mask rows were zeroed by a memset node)
+__global__ void list_to_mask_kernel(const int32_t* indices, const int32_t* budgets, int cap, uint32_t* mask, int mask_stride,
+                                    int L) {
+    const int q = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5), lane = threadIdx.x & 31;
+    if (q >= L) return;
+    const int n = min(budgets[q], cap);
+    for (int i = lane; i < n; i += 32) {
+        const int b = indices[(int64_t)q * cap + i];
+        if (b >= 0) atomicOr(&mask[(int64_t)q * mask_stride + (b >> 5)], 1u << (b & 31));
+    }
+}
+
+struct TrainLayout {
+    size_t t_lse2, s_lse, scores, seq_len, indices, budgets, mask, total;
+    int nb_stride, mask_stride, cap, n_b;
+};
+TrainLayout train_layout(const spot_train_params* p) {
+    TrainLayout y;
+    auto up = [](size_t x) { return (x + 255) & ~(size_t)255; };
+    y.n_b = (p->L + p->blk - 1) / p->blk;
+    y.nb_stride = (y.n_b + 3) & ~3;
+    y.mask_stride = (y.n_b + 31) / 32;
+    y.cap = p->top_k < y.n_b ? p->top_k : y.n_b;
+    size_t o = 256;
+    y.t_lse2 = o; o += up((size_t)p->L * p->H_q * 4);
+    y.s_lse = o; o += up((size_t)p->L * 4);
+    y.scores = o; o += up((size_t)p->L * y.nb_stride * 4);
+    y.seq_len = o; o += up((size_t)p->L * 4);
+    y.indices = o; o += p->indices ? 0 : up((size_t)p->L * y.cap * 4);
+    y.budgets = o; o += p->budgets ? 0 : up((size_t)p->L * 4);
+    y.mask = o; o += up((size_t)p->L * y.mask_stride * 4);
+    y.total = o;
+    return y;
+}
+
+spot_status check_train(const spot_train_params* p) {
+    if (!p || !p->q || !p->k || !p->sel_q || !p->w || !p->sel_k || !p->dense_kl || !p->sparse_kl) return SPOT_ERR_INVALID_ARG;
+    if (!aligned16(p->q) || !aligned16(p->k) || !aligned16(p->sel_q) || !aligned16(p->sel_k)) return SPOT_ERR_INVALID_ARG;
+    if (p->L <= 0 || p->H_q <= 0 || p->H_kv <= 0 || p->H_q % p->H_kv != 0 || p->H_idx <= 0 || p->d_idx <= 0) return SPOT_ERR_INVALID_ARG;
+    if (p->top_k <= 0 || p->sink_blocks < 0 || p->recency_blocks < 0 || p->top_k < p->sink_blocks + p->recency_blocks)
+        return SPOT_ERR_INVALID_ARG;
+    if (p->k_stride_token < p->D || p->k_stride_token % 8 || p->k_stride_head % 8) return SPOT_ERR_INVALID_ARG;
+    if ((p->indices == nullptr) != (p->budgets == nullptr)) return SPOT_ERR_INVALID_ARG;
+    const int G = p->H_q / p->H_kv;
+    if (p->D != TR_D || p->H_kv > TR_TW || (G != 2 && G != 4 && G != 8 && G != 16)) return SPOT_ERR_UNSUPPORTED;
+    if (p->H_idx > 4 || p->d_idx % 16 != 0 || p->d_idx > 128) return SPOT_ERR_UNSUPPORTED;
+    if (p->blk != 16 && p->blk != 32 && p->blk != 64) return SPOT_ERR_UNSUPPORTED;
+    if ((p->L + p->blk - 1) / p->blk > SEL_MAX_NB) return SPOT_ERR_UNSUPPORTED;
+    if (p->indices && p->cap < ((p->L + p->blk - 1) / p->blk < p->top_k ? (p->L + p->blk - 1) / p->blk : p->top_k))
+        return SPOT_ERR_INVALID_ARG;
+    return SPOT_OK;
+}
+
+}  // namespace
+
+}  // namespace spot
+
+using namespace spot;
+
+extern "C" size_t spot_train_kl_workspace_bytes(const spot_train_params* p) {
+    if (check_train(p) != SPOT_OK) return 0;
+    return train_layout(p).total;
+}
+
+extern "C" spot_status spot_train_kl(const spot_train_params* p, void* stream) {
+    spot_status st = check_train(p);
+    if (st != SPOT_OK) return st;
+    if ((st = check_device()) != SPOT_OK) return st;
+    const TrainLayout y = train_layout(p);
+    if (!p->workspace || p->workspace_bytes < y.total) return SPOT_ERR_WORKSPACE_TOO_SMALL;
+    cudaStream_t s = (cudaStream_t)stream;
+    if (!aligned16(p->workspace)) return SPOT_ERR_INVALID_ARG;
+    char* ws = reinterpret_cast<char*>(p->workspace);
+    TrainArgs a;
+    memset(&a, 0, sizeof(a));
+    a.q = p->q; a.k = p->k; a.k_st = p->k_stride_token; a.k_sh = p->k_stride_head;
+    a.sel_q = p->sel_q; a.w = p->w; a.sel_k = p->sel_k;
+    a.L = p->L; a.H_q = p->H_q; a.H_kv = p->H_kv; a.G = p->H_q / p->H_kv; a.H_idx = p->H_idx; a.d_idx = p->d_idx; a.blk = p->blk;
+    a.scale_log2 = p->sm_scale * 1.4426950408889634f;
+    a.t_lse2 = reinterpret_cast<float*>(ws + y.t_lse2);
+    a.s_lse = reinterpret_cast<float*>(ws + y.s_lse);
+    a.blk_scores = reinterpret_cast<float*>(ws + y.scores);
+    a.nb_stride = y.nb_stride;
+    uint32_t* mask = reinterpret_cast<uint32_t*>(ws + y.mask);
+    a.mask = mask; a.mask_stride = y.mask_stride;
+    a.dense_kl = p->dense_kl; a.sparse_kl = p->sparse_kl; a.teacher_lse = p->teacher_lse;
+    int32_t* seq_len = reinterpret_cast<int32_t*>(ws + y.seq_len);
+    int32_t* indices = p->indices ? p->indices : reinterpret_cast<int32_t*>(ws + y.indices);
+    int32_t* budgets = p->budgets ? p->budgets : reinterpret_cast<int32_t*>(ws + y.budgets);
+    const int cap = p->indices ? p->cap : y.cap;
+
+    const int QPC = 32 / a.G;
+    const int grid = (p->L + QPC - 1) / QPC;
+    const int smem = TR_TW * TR_STAGES * TR_KSTAGE + TR_STAGES * TR_KT * (p->H_idx * p->d_idx * 2) + 4 * TR_QMAX * TR_KT * 4 +
+                     16 * (p->H_idx * p->d_idx * 2);
+    static unsigned long long done1 = 0, done2 = 0;
+    // (the attribute is set once per device: to the largest geometry, H_idx x d_idx = 4 x 128)
+    constexpr int smem_max = TR_TW * TR_STAGES * TR_KSTAGE + TR_STAGES * TR_KT * 1024 + 4 * TR_QMAX * TR_KT * 4 + 16 * 1024;
+    SPOT_CUDA_TRY(set_max_smem_once(train_pass_kernel<1>, smem_max, done1));
+    SPOT_CUDA_TRY(set_max_smem_once(train_pass_kernel<2>, smem_max, done2));
+    train_pass_kernel<1><<<grid, TR_THREADS, smem, s>>>(a);
+    SPOT_LAUNCH_CHECK();
+    iota_len_kernel<<<(p->L + 255) / 256, 256, 0, s>>>(seq_len, p->L);
+    SPOT_LAUNCH_CHECK();
+    // Eq. 6 per query: the selection kernel in its decode form, one row per query
+    spot_select_params sp;
+    memset(&sp, 0, sizeof(sp));
+    sp.seq_len = seq_len; sp.max_seq_len = p->L; sp.B = p->L; sp.Tq = 1; sp.H_idx = p->H_idx; sp.d_idx = p->d_idx;
+    sp.blk = p->blk; sp.q_block = 1; sp.mode = SPOT_MODE_TOPK; sp.top_k = p->top_k; sp.p = 1.0; sp.temperature = 1.0;
+    sp.sink_blocks = p->sink_blocks; sp.recency_blocks = p->recency_blocks; sp.kmin_blocks = 0;
+    sp.indices = indices; sp.cap = cap; sp.budgets = budgets; sp.nb_stride = y.nb_stride;
+    if ((st = run_select(&sp, a.blk_scores, y.nb_stride, 1, y.n_b, nullptr, s)) != SPOT_OK) return st;
+    SPOT_CUDA_TRY(cudaMemsetAsync(mask, 0, (size_t)p->L * y.mask_stride * 4, s));
+    list_to_mask_kernel<<<(p->L + 7) / 8, 256, 0, s>>>(indices, budgets, cap, mask, y.mask_stride, p->L);
+    SPOT_LAUNCH_CHECK();
+    train_pass_kernel<2><<<grid, TR_THREADS, smem, s>>>(a);
+    SPOT_LAUNCH_CHECK();
+    return SPOT_OK;
+}

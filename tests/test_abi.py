@@ -45,7 +45,8 @@ def test_struct_layout_and_strings(lib):
     assert lib.spot_struct_size(2) == C.sizeof(_lib.DecodeStepHostParams)
     assert lib.spot_struct_size(3) == C.sizeof(_lib.ProjectParams)
     assert lib.spot_struct_size(4) == C.sizeof(_lib.DecodeStepParams)
-    assert lib.spot_struct_size(5) == 0
+    assert lib.spot_struct_size(5) == C.sizeof(_lib.TrainParams)
+    assert lib.spot_struct_size(6) == 0
     assert [lib.spot_status_string(i) for i in range(5)] == [
         b"SPOT_OK", b"SPOT_ERR_INVALID_ARG", b"SPOT_ERR_UNSUPPORTED", b"SPOT_ERR_WORKSPACE_TOO_SMALL", b"SPOT_ERR_CUDA"]
     assert re.match(rb"\d+\.\d+$", lib.spot_version())
