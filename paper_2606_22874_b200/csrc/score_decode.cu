@@ -44,34 +44,33 @@ __device__ __forceinline__ void e2m1x8_to_f16x2x4(uint32_t w, uint32_t (&p)[4]) 
         : "=r"(p[0]), "=r"(p[1]), "=r"(p[2]), "=r"(p[3]) : "r"(w));
 }
 
-__device__ __forceinline__ uint32_t hfma2_u32(uint32_t a, uint32_t b, uint32_t c) {
-    uint32_t d;
-    asm("fma.rn.f16x2 %0, %1, %2, %3;" : "=r"(d) : "r"(a), "r"(b), "r"(c));
-    return d;
-}
-__device__ __forceinline__ uint32_t hsub2_u32(uint32_t a, uint32_t b) {
-    uint32_t d;
-    asm("sub.rn.f16x2 %0, %1, %2;" : "=r"(d) : "r"(a), "r"(b));
-    return d;
-}
-
 // 8 codes (one 32-bit word) -> 4 fp16 pairs; pair pp = dims (2pp, 2pp+1) of the word.
 template <int FMT>
 __device__ __forceinline__ void unpack8(uint32_t w, uint32_t (&p)[4]) {
     if (FMT == SPOT_SELK_MXFP4) {
         e2m1x8_to_f16x2x4(w, p);
     } else {
-        // u = q + 8 in each nibble.  0x6400 | u = 1024 + u (fp16); nibble at bit 4: 1024 + 16 u.
-        const uint32_t MAGIC = 0x64006400u;
-        const uint32_t C1032 = 0x64086408u;   // 1032.0 x2
-        const uint32_t SIXTEENTH = 0x2c002c00u;  // 0.0625 x2
-        const uint32_t NEG72 = 0xd480d480u;   // -72.0 x2
-        uint32_t w8 = w >> 8;
-        p[0] = hsub2_u32((w & 0x000f000fu) | MAGIC, C1032);
-        p[1] = hfma2_u32((w & 0x00f000f0u) | MAGIC, SIXTEENTH, NEG72);
-        p[2] = hsub2_u32((w8 & 0x000f000fu) | MAGIC, C1032);
-        p[3] = hfma2_u32((w8 & 0x00f000f0u) | MAGIC, SIXTEENTH, NEG72);
+        // u = q + 8 in each nibble, read as it stands: four bits in the low end of an fp16 are the SUBNORMAL u 2^-24
+        // (exact, and the tensor cores take fp16 subnormals), the nibble at bit 4 is 16 u 2^-24 -- one LOP3 per pair, no
+        // magic-number fix-up.  The factor 16 is taken out of the QUERY's copy of those dims (a power of two: exact), the
+        // factor 2^-24 goes into the power-of-two post-scale, and the offset, sum_i 8 x_i over the group, is a constant of
+        // the query, subtracted from the group's partial sum after the MMA (Q4Tile::stage_raw).  (Round 1 rebuilt q with
+        // OR 0x6400 / HSUB2 / HFMA2: 9 instructions per 8 codes against 5; the INT4 kernel was ALU-bound.)
+        const uint32_t w8 = w >> 8;
+        p[0] = w & 0x000f000fu;
+        p[1] = w & 0x00f000f0u;
+        p[2] = w8 & 0x000f000fu;
+        p[3] = w8 & 0x00f000f0u;
     }
+}
+
+// two adjacent E4M3 scale bytes -> fp32 (exact): cvt.rn.f16x2.e4m3x2, low byte -> low half
+__device__ __forceinline__ void e4m3x2_to_f32x2(uint32_t two_bytes, float& lo, float& hi) {
+    uint32_t h2;
+    asm("{ .reg .b16 t; cvt.u16.u32 t, %1; cvt.rn.f16x2.e4m3x2 %0, t; }" : "=r"(h2) : "r"(two_bytes));
+    const __half2 hh = *reinterpret_cast<const __half2*>(&h2);
+    lo = __low2float(hh);
+    hi = __high2float(hh);
 }
 
 template <int FMT>
@@ -124,19 +123,22 @@ struct ScoreCfg {
     // the running block maximum in registers.  (4 KiB slices x 4 stages per warp: no faster, 39.9 vs 38.0 us score + select.)
     // The 17 KiB 4-bit tiles of d_idx = 128 get the same treatment (12 warps instead of 6): a slice is 32 tokens' codes
     // plus their scale bytes, two bulk copies on one barrier.
+    // (round 2, measured and not kept: 32-token slices with FOUR stages per warp for the 8.5 KiB tiles of d_idx = 64 --
+    // MXFP4 scoring alone 24.4 vs 22.8 us at B = 4, 64.3 vs 57.7 us at B = 16: two copies and two barrier phases per tile
+    // cost more issue slots than the deeper ring wins back)
     static constexpr int SPLIT = FMT == SPOT_SELK_FP8_E4M3 ? TILE_BYTES / 8192 : (SELF && TILE_BYTES > 12288 ? 2 : 1);
     static constexpr int STAGE_BYTES = SELF ? TILE_BYTES / SPLIT : (TILE_BYTES + 1023) / 1024 * 1024;
     static constexpr int STAGES_RAW = SC_SMEM_BUDGET / STAGE_BYTES;
-    static constexpr int SELF_MAX = (208 * 1024 / STAGE_BYTES) / 2;           // warps that fit with 2 stages each
+    static constexpr int PER_WARP = SELF ? (STAGE_BYTES <= 4608 ? 4 : 2) : 1;
+    static constexpr int SELF_MAX = (208 * 1024 / STAGE_BYTES) / (PER_WARP ? PER_WARP : 1);   // warps that fit
     static constexpr int CONSUMERS = SELF ? (SELF_MAX > 12 ? 12 : SELF_MAX) : (STAGES_RAW > 6 ? 6 : STAGES_RAW);
-    static constexpr int PER_WARP = SELF ? 2 : 1;
     static constexpr int STAGES = CONSUMERS * PER_WARP;
     static constexpr int THREADS = (CONSUMERS + (SELF ? 0 : 1)) * 32;
     static_assert(STAGES * STAGE_BYTES <= 208 * 1024, "ring geometry");
     // query slots: one per sequence when the batch has at most Q_SLOTS of them (staged once, at kernel start), else one
     // per consumer warp (restaged whenever the warp changes sequence)
     static constexpr int Q_SLOTS = 16;
-    static constexpr int Q_SLOT_BYTES = ROW * 2 + 64;
+    static constexpr int Q_SLOT_BYTES = ROW * 2 + 128;      // + post-scales, w, and (INT4) the group offsets
     static constexpr int Q16_BYTES = Q_SLOTS * Q_SLOT_BYTES;
     static_assert(CONSUMERS <= Q_SLOTS, "a slot per consumer warp");
     static constexpr int SMEM_BYTES = 256 + 1024 + STAGES * STAGE_BYTES + 2 * STAGES * 8 + Q16_BYTES + 64;
@@ -250,6 +252,11 @@ __device__ __forceinline__ float group_update(float m, float sa, float sb, bool 
     return lane == 4 * grp ? mi : m;
 }
 
+// One query row on its way to a shared-memory slot: the global loads are issued at the very start of the kernel (two
+// DRAM round trips that would otherwise sit in front of the first tile), the conversion happens after the first tile
+// requests are out.
+struct QRaw { uint4 v[2]; float w; };
+
 // ---- BF16 tile: planes [H * D_IDX / 64][64 tokens][128 B], 128-byte swizzle --------------------------------
 template <int H, int D_IDX>
 struct Bf16Tile {
@@ -259,12 +266,22 @@ struct Bf16Tile {
     float wh[H];
 
     // slot: ROW BF16 (the query as it is) + H floats (w)
-    static __device__ __forceinline__ void stage(const ScoreArgs& a, int b, int lane, uint32_t slot) {
+    static __device__ __forceinline__ void load_raw(const ScoreArgs& a, int b, int lane, QRaw& r) {
+        constexpr int ROW = H * D_IDX;
+        static_assert(ROW / 8 <= 64, "two 16-byte chunks per lane");
+        const uint4* src = reinterpret_cast<const uint4*>(a.sel_q + (int64_t)b * ROW);
+#pragma unroll
+        for (int i = 0; i < 2; ++i)
+            if (i * 32 + lane < ROW / 8) r.v[i] = src[i * 32 + lane];
+        r.w = lane < H ? a.w[(int64_t)b * H + lane] : 0.f;
+    }
+    static __device__ __forceinline__ void stage_raw(const QRaw& r, int lane, uint32_t slot) {
         constexpr int ROW = H * D_IDX;
         uint16_t* dst = reinterpret_cast<uint16_t*>(__cvta_shared_to_generic((size_t)slot));
-        const uint4* src = reinterpret_cast<const uint4*>(a.sel_q + (int64_t)b * ROW);
-        for (int i = lane; i < ROW / 8; i += 32) reinterpret_cast<uint4*>(dst)[i] = src[i];
-        if (lane < H) reinterpret_cast<float*>(dst + ROW)[lane] = a.w[(int64_t)b * H + lane];
+#pragma unroll
+        for (int i = 0; i < 2; ++i)
+            if (i * 32 + lane < ROW / 8) reinterpret_cast<uint4*>(dst)[i * 32 + lane] = r.v[i];
+        if (lane < H) reinterpret_cast<float*>(dst + ROW)[lane] = r.w;
         __syncwarp();
     }
     __device__ __forceinline__ void fetch(int lane, uint32_t slot) {
@@ -328,9 +345,18 @@ struct Q4Tile {
     static_assert(NG % 4 == 0, "H_idx * d_idx must be a multiple of 128");
     uint32_t qf[NQL][16];
     float wq[NQL], ps[NQL];
+    float cq[NQL][2];                              // INT4: the offsets 8 sum x 2^-24 of this lane's two groups per quad load
 
     // slot: ROW halfs (the pre-scaled fp16 query) + H floats (power-of-two post-scales) + H floats (w)
-    static __device__ __forceinline__ void stage(const ScoreArgs& a, int b, int lane, uint32_t q16_addr) {
+    static __device__ __forceinline__ void load_raw(const ScoreArgs& a, int b, int lane, QRaw& r) {
+        constexpr int EPL = ROW / 32;
+        static_assert(EPL / 8 <= 2, "two 16-byte chunks per lane");
+#pragma unroll
+        for (int i = 0; i < EPL / 8; ++i)
+            r.v[i] = *reinterpret_cast<const uint4*>(a.sel_q + (int64_t)b * ROW + lane * EPL + i * 8);
+        r.w = lane < H ? a.w[(int64_t)b * H + lane] : 0.f;
+    }
+    static __device__ __forceinline__ void stage_raw(const QRaw& r, int lane, uint32_t q16_addr) {
         __half* q16 = reinterpret_cast<__half*>(__cvta_shared_to_generic((size_t)q16_addr));
         float* post = reinterpret_cast<float*>(q16 + ROW);
         // fp16 copy of q, pre-scaled per head by 2^sh so that the head's largest element lands in [2^14, 2^15).
@@ -338,14 +364,10 @@ struct Q4Tile {
         constexpr int EPL = ROW / 32, LPH = 32 / H;
         static_assert(EPL % 8 == 0 && LPH * EPL == D_IDX && (LPH & (LPH - 1)) == 0, "query staging geometry");
         __syncwarp();
-        uint4 raw[EPL / 8];
-#pragma unroll
-        for (int i = 0; i < EPL / 8; ++i)
-            raw[i] = *reinterpret_cast<const uint4*>(a.sel_q + (int64_t)b * ROW + lane * EPL + i * 8);
         float v[EPL], mx = 0.f;
 #pragma unroll
         for (int i = 0; i < EPL / 8; ++i) {
-            const uint32_t wds[4] = {raw[i].x, raw[i].y, raw[i].z, raw[i].w};
+            const uint32_t wds[4] = {r.v[i].x, r.v[i].y, r.v[i].z, r.v[i].w};
 #pragma unroll
             for (int j = 0; j < 4; ++j) { v[i * 8 + 2 * j] = bf16lo(wds[j]); v[i * 8 + 2 * j + 1] = bf16hi(wds[j]); }
         }
@@ -357,10 +379,27 @@ struct Q4Tile {
         if (mx > 0.f) sh = 14 - ilogbf(mx);
         sh = max(-100, min(100, sh));
         const float up = __uint_as_float((uint32_t)(127 + sh) << 23);
+        if (FMT == SPOT_SELK_INT4_E4M3) {
+            // (see unpack8) dims 2, 3, 6, 7 of every 8 go in divided by 16; the group offset 8 sum x, times 2^-24
+            float xs = 0.f;
 #pragma unroll
-        for (int i = 0; i < EPL; ++i) q16[lane * EPL + i] = __float2half_rn(v[i] * up);
-        if (lane % LPH == 0) post[lane / LPH] = __uint_as_float((uint32_t)(127 - sh) << 23);
-        if (lane < H) post[H + lane] = a.w[(int64_t)b * H + lane];
+            for (int i = 0; i < EPL; ++i) {
+                const bool hi_nibble = (i & 2) != 0;              // EPL % 8 == 0: i % 8 is the dim inside its 8-code word
+                const __half hq = __float2half_rn(v[i] * up * (hi_nibble ? 0.0625f : 1.0f));
+                q16[lane * EPL + i] = hq;
+                xs += __half2float(hq) * (hi_nibble ? 16.0f : 1.0f);
+            }
+            constexpr int LPG = 32 / EPL;                         // lanes per 32-element group
+#pragma unroll
+            for (int o = LPG / 2; o; o >>= 1) xs += __shfl_xor_sync(0xffffffffu, xs, o);
+            if (lane % LPG == 0) post[2 * H + lane / LPG] = xs * (8.0f * 5.9604644775390625e-08f);
+            if (lane % LPH == 0) post[lane / LPH] = __uint_as_float((uint32_t)(127 - sh + 24) << 23);
+        } else {
+#pragma unroll
+            for (int i = 0; i < EPL; ++i) q16[lane * EPL + i] = __float2half_rn(v[i] * up);
+            if (lane % LPH == 0) post[lane / LPH] = __uint_as_float((uint32_t)(127 - sh) << 23);
+        }
+        if (lane < H) post[H + lane] = r.w;
         __syncwarp();
     }
     __device__ __forceinline__ void fetch(int lane, uint32_t q16_addr) {
@@ -384,6 +423,10 @@ struct Q4Tile {
             const int head = (4 * ql + 2 * (c & 1)) / GPH;
             wq[ql] = post[H + head];
             ps[ql] = post[head];
+            if (FMT == SPOT_SELK_INT4_E4M3) {
+                cq[ql][0] = post[2 * H + 4 * ql + 2 * (c & 1)];
+                cq[ql][1] = post[2 * H + 4 * ql + 2 * (c & 1) + 1];
+            }
         }
     }
 
@@ -425,9 +468,15 @@ struct Q4Tile {
                 for (int hf = 0; hf < 2; ++hf) {
                     const int gi = 2 * (c & 1);                        // first of this lane's two groups in the quad load
                     const uint32_t sw = scw[hf][ql];                   // scale bytes of groups 4ql .. 4ql+3
-                    const float s0 = scale_to_f32<FMT>((sw >> (8 * gi)) & 0xffu);
-                    const float s1 = scale_to_f32<FMT>((sw >> (8 * (gi + 1))) & 0xffu);
-                    float d = fmaf(acc[2 * hf], s0, acc[2 * hf + 1] * s1);
+                    float s0, s1, d;
+                    if (FMT == SPOT_SELK_INT4_E4M3) {
+                        e4m3x2_to_f32x2((sw >> (8 * gi)) & 0xffffu, s0, s1);
+                        d = fmaf(acc[2 * hf] - cq[ql][0], s0, (acc[2 * hf + 1] - cq[ql][1]) * s1);
+                    } else {
+                        s0 = scale_to_f32<FMT>((sw >> (8 * gi)) & 0xffu);
+                        s1 = scale_to_f32<FMT>((sw >> (8 * (gi + 1))) & 0xffu);
+                        d = fmaf(acc[2 * hf], s0, acc[2 * hf + 1] * s1);
+                    }
                     if (GPH == 4) d += __shfl_xor_sync(0xffffffffu, d, 1);   // the head's other two groups
                     d *= ps[ql];
                     float contrib = wq[ql] * fmaxf(d, 0.f);
@@ -458,20 +507,24 @@ struct Fp8Tile {
     uint32_t qf[NQL][8];
     float wq[H], ps[H];
 
-    static __device__ __forceinline__ void stage(const ScoreArgs& a, int b, int lane, uint32_t q16_addr) {
+    static __device__ __forceinline__ void load_raw(const ScoreArgs& a, int b, int lane, QRaw& r) {
+        constexpr int EPL = ROW / 32;
+        static_assert(EPL / 8 <= 2, "two 16-byte chunks per lane");
+#pragma unroll
+        for (int i = 0; i < EPL / 8; ++i)
+            r.v[i] = *reinterpret_cast<const uint4*>(a.sel_q + (int64_t)b * ROW + lane * EPL + i * 8);
+        r.w = lane < H ? a.w[(int64_t)b * H + lane] : 0.f;
+    }
+    static __device__ __forceinline__ void stage_raw(const QRaw& r, int lane, uint32_t q16_addr) {
         __half* q16 = reinterpret_cast<__half*>(__cvta_shared_to_generic((size_t)q16_addr));
         float* post = reinterpret_cast<float*>(q16 + ROW);
         constexpr int EPL = ROW / 32, LPH = 32 / H;
         static_assert(EPL % 8 == 0 && LPH * EPL == D_IDX && (LPH & (LPH - 1)) == 0, "query staging geometry");
         __syncwarp();
-        uint4 raw[EPL / 8];
-#pragma unroll
-        for (int i = 0; i < EPL / 8; ++i)
-            raw[i] = *reinterpret_cast<const uint4*>(a.sel_q + (int64_t)b * ROW + lane * EPL + i * 8);
         float v[EPL], mx = 0.f;
 #pragma unroll
         for (int i = 0; i < EPL / 8; ++i) {
-            const uint32_t wds[4] = {raw[i].x, raw[i].y, raw[i].z, raw[i].w};
+            const uint32_t wds[4] = {r.v[i].x, r.v[i].y, r.v[i].z, r.v[i].w};
 #pragma unroll
             for (int j = 0; j < 4; ++j) { v[i * 8 + 2 * j] = bf16lo(wds[j]); v[i * 8 + 2 * j + 1] = bf16hi(wds[j]); }
         }
@@ -487,7 +540,7 @@ struct Fp8Tile {
 #pragma unroll
         for (int i = 0; i < EPL; ++i) q16[lane * EPL + i] = __float2half_rn(v[i] * up);
         if (lane % LPH == 0) post[lane / LPH] = __uint_as_float((uint32_t)(127 - sh) << 23);
-        if (lane < H) post[H + lane] = a.w[(int64_t)b * H + lane];
+        if (lane < H) post[H + lane] = r.w;
         __syncwarp();
     }
     __device__ __forceinline__ void fetch(int lane, uint32_t q16_addr) {
@@ -596,6 +649,14 @@ __global__ void __launch_bounds__((ScoreCfg<H, D_IDX, FMT>::THREADS), 1) score_d
 
     // this CTA's work list: its range of every group, in group order
     __shared__ CtaRange s_rng[SC_MAX_GROUPS];
+    using TileT = typename std::conditional<FMT == SPOT_SELK_BF16, Bf16Tile<H, D_IDX>,
+                  typename std::conditional<FMT == SPOT_SELK_FP8_E4M3, Fp8Tile<H, D_IDX>, Q4Tile<H, D_IDX, FMT>>::type>::type;
+    // the two cold global reads in front of everything -- the sequence lengths and this warp's first query row -- go
+    // out together
+    const bool q_staged = a.B <= Cfg::Q_SLOTS;
+    QRaw raw0;
+    const bool have_raw0 = q_staged && warp < SC_CONSUMERS && warp < a.B;
+    if (have_raw0) TileT::load_raw(a, warp, lane, raw0);
     if (threadIdx.x < SC_NB_CACHE && (int)threadIdx.x < a.B)
         reinterpret_cast<int*>(smem_raw)[threadIdx.x] = (seq_len_of(a, threadIdx.x) + 63) >> 6;
     __syncthreads();
@@ -608,18 +669,20 @@ __global__ void __launch_bounds__((ScoreCfg<H, D_IDX, FMT>::THREADS), 1) score_d
     cur.first(a, s_rng);
     // queries: staged once per CTA when every sequence has a slot (ScoreCfg), else per warp on every change of sequence.
     // The staging runs AFTER the first tile requests are out (below) and ends on a barrier of the consumer warps only.
-    using TileT = typename std::conditional<FMT == SPOT_SELK_BF16, Bf16Tile<H, D_IDX>,
-                  typename std::conditional<FMT == SPOT_SELK_FP8_E4M3, Fp8Tile<H, D_IDX>, Q4Tile<H, D_IDX, FMT>>::type>::type;
-    const bool q_staged = a.B <= Cfg::Q_SLOTS;
     auto stage_queries = [&]() {
         if (!q_staged) return;
-        for (int bb = warp; bb < a.B; bb += SC_CONSUMERS) TileT::stage(a, bb, lane, q16_base + bb * Cfg::Q_SLOT_BYTES);
+        for (int bb = warp; bb < a.B; bb += SC_CONSUMERS) {
+            if (bb != warp) TileT::load_raw(a, bb, lane, raw0);
+            TileT::stage_raw(raw0, lane, q16_base + bb * Cfg::Q_SLOT_BYTES);
+        }
         asm volatile("bar.sync 1, %0;" :: "n"(SC_CONSUMERS * 32) : "memory");
     };
     auto take_query = [&](TileT& tile, int bb) {
         if (q_staged) { tile.fetch(lane, q16_base + bb * Cfg::Q_SLOT_BYTES); return; }
         __syncwarp();
-        TileT::stage(a, bb, lane, q16_base + warp * Cfg::Q_SLOT_BYTES);
+        QRaw r;
+        TileT::load_raw(a, bb, lane, r);
+        TileT::stage_raw(r, lane, q16_base + warp * Cfg::Q_SLOT_BYTES);
         tile.fetch(lane, q16_base + warp * Cfg::Q_SLOT_BYTES);
         __syncwarp();
     };
@@ -657,9 +720,15 @@ __global__ void __launch_bounds__((ScoreCfg<H, D_IDX, FMT>::THREADS), 1) score_d
             if (rq % SP == SP - 1) nxt.advance(a, s_rng, SC_CONSUMERS);
             ++rq;
         };
+#ifdef SPOT_TRACE
+        if (warp == 0) SPOT_STAMP(a.sync, 6, 0);
+#endif
 #pragma unroll
         for (int j = 0; j < K; ++j) request_next();
         stage_queries();
+#ifdef SPOT_TRACE
+        if (warp == 0) SPOT_STAMP(a.sync, 6, 1);
+#endif
         int cur_b = -1, L = 0;
         for (int j = 0; j < n_w; ++j) {
             if (cur.b != cur_b) {
@@ -673,6 +742,10 @@ __global__ void __launch_bounds__((ScoreCfg<H, D_IDX, FMT>::THREADS), 1) score_d
                 const int q = j * SP + part;
                 const uint32_t s = warp * K + q % K;
                 mbar_wait(bar_full + 8 * s, (q / K) & 1);
+#ifdef SPOT_TRACE
+                if (warp == 0 && q == 0) SPOT_STAMP(a.sync, 6, 2);
+                if (warp == 0 && q == 2) SPOT_STAMP(a.sync, 6, 3);
+#endif
                 m = fmaxf(m, tile.template part_max<4 / SP>(ring + s * Cfg::STAGE_BYTES, cur.t * 64 + part * (64 / SP),
                                                             L, lane, fine, part * (4 / SP)));
                 __syncwarp();
