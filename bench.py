@@ -638,14 +638,23 @@ def run_prefill(args):
         # f2: the selector cache in a quantised format; spot_select dequantises the visible prefix into its workspace
         sel_k = torch.zeros(api.spot_selector_k_bytes(args.fmt, 1, L, wl.H_idx, wl.d_idx), dtype=torch.uint8, device=dev)
         api.spot_quantize_selector_k(sel_k_bf16, sel_k, args.fmt, 1, L, 0, L, wl.H_idx, wl.d_idx)
+    sel_q_in, q_fmt = sel_q, "bf16"
+    if args.qfmt != "bf16":
+        # f2: the queries quantised too -- FP8 x FP8 tile scores on the tensor cores, no dequantise pass (spot.h, q_fmt)
+        assert args.fmt == args.qfmt == "fp8_e4m3", "--qfmt fp8_e4m3 needs --fmt fp8_e4m3"
+        sel_q_in = torch.zeros(api.spot_selector_k_bytes(args.qfmt, 1, L, wl.H_idx, wl.d_idx), dtype=torch.uint8, device=dev)
+        api.spot_quantize_selector_k(sel_q, sel_q_in, args.qfmt, 1, L, 0, L, wl.H_idx, wl.d_idx)
+        q_fmt = args.qfmt
+    f8 = q_fmt != "bf16"
+    tc_ratio = 2.0 if f8 else 1.0          # a contraction takes the peak of its own dtype
     cap = n_kb
     nb_stride = (n_kb + 3) & ~3
     indices = torch.empty((n_qb, cap), dtype=torch.int32, device=dev)
     budgets = torch.empty((n_qb,), dtype=torch.int32, device=dev)
     scores = torch.empty((n_qb, nb_stride), dtype=torch.float32, device=dev)
     out = torch.empty((1, L, Hq, D), dtype=torch.int16, device=dev)
-    sp = api.make_select_params(sel_q, w, sel_k, args.fmt, L, None, 0, 1, L, wl.H_idx, wl.d_idx, q_start=0, blk=blk,
-                                q_block=64, mode=wl.mode, top_k=wl.top_k, p=args.p, sink_blocks=wl.sink_blocks,
+    sp = api.make_select_params(sel_q_in, w, sel_k, args.fmt, L, None, 0, 1, L, wl.H_idx, wl.d_idx, q_start=0, blk=blk,
+                                q_fmt=q_fmt, q_block=64, mode=wl.mode, top_k=wl.top_k, p=args.p, sink_blocks=wl.sink_blocks,
                                 recency_blocks=wl.recency_blocks, kmin_blocks=wl.kmin_blocks,
                                 temperature=wl.temperature, indices=indices, cap=cap, budgets=budgets,
                                 block_scores=scores, nb_stride=nb_stride)
@@ -734,6 +743,8 @@ def run_prefill(args):
         sel_k_bf16.copy_(h_selk, non_blocking=True)
         if args.fmt != "bf16":             # the cache is produced from the fresh keys inside the step
             api.spot_quantize_selector_k(sel_k_bf16, sel_k, args.fmt, 1, L, 0, L, wl.H_idx, wl.d_idx, stream)
+        if q_fmt != "bf16":
+            api.spot_quantize_selector_k(sel_q, sel_q_in, q_fmt, 1, L, 0, L, wl.H_idx, wl.d_idx, stream)
         api.spot_select(sp, stream)
         api.spot_sparse_attn_prefill(ap, stream)
         h_bud.copy_(budgets, non_blocking=True)
@@ -752,7 +763,7 @@ def run_prefill(args):
     att_flop = 4.0 * 64 * blk * D * Hq * float(bud_host.sum())
     score_s = float(np.mean(sc)) * 1e-3
     achieved = gemm_flop / score_s / 1e12
-    traffic = traffic_entry("cfg5/%s/score_prefill_kernel" % args.fmt)
+    traffic = traffic_entry("cfg5/%s/score_prefill_kernel" % (args.fmt if q_fmt == "bf16" else args.fmt + "+q"))
     # oracle on the host cores: three query blocks below position 4096
     n_tok = min(L, 4096)
     Kh = K[0, :, :n_tok].contiguous().view(torch.int16).cpu().numpy().view(np.uint16)
@@ -763,9 +774,9 @@ def run_prefill(args):
     line = {
         "metric": PF_METRIC, "value": step_mean, "unit": "ms/layer", "n_gpus": world, "steps": args.steps,
         "warmup": W, "ms_per_step": step_mean, "higher_is_better": False, "scaling": "weak", "vs_baseline": None,
-        "dtype": "bf16", "data": "synthetic",
+        "dtype": "bf16" if not f8 else "bf16 (attention), fp8_e4m3 x fp8_e4m3 -> fp32 (tile scores)", "data": "synthetic",
         "config": {"workload": "cfg5", "B": 1, "L": L, "H_q": Hq, "H_kv": Hkv, "D": D,
-                   "selector": "%dx%d %s" % (wl.H_idx, wl.d_idx, args.fmt), "blk": blk, "q_block": 64,
+                   "selector": "%dx%d %s" % (wl.H_idx, wl.d_idx, args.fmt), "selector_queries": q_fmt, "blk": blk, "q_block": 64,
                    "kv_layout": ("paged, %d tokens per page, random table" % max(args.paged, 64)) if args.paged else "[B][H_kv][L][D]", "mode": wl.mode, "p": args.p,
                    "sink/recency/kmin": [wl.sink_blocks, wl.recency_blocks, wl.kmin_blocks],
                    "mean_budget": float(bud_host.mean()), "density": float(bud_host.sum()) * blk / 64.0 / tiles,
@@ -776,9 +787,12 @@ def run_prefill(args):
                          "sparse causal attention": float(att_ms.mean()),
                          "dense causal attention (same kernel, every block)": float(np.mean(den))},
         "attention_tflops": att_flop / (float(att_ms.mean()) * 1e-3) / 1e12,
-        "roofline": {"bound": "tensor", "kernel": "score_prefill_kernel", "achieved": achieved, "peak": burst,
-                     "unit": "TFLOP/s", "frac": achieved / burst, "frac_of_sustained": achieved / sustained,
-                     "traffic": traffic, "peak_source": peak_src, "algorithmic_flops": gemm_flop},
+        "roofline": {"bound": "tensor", "kernel": "score_prefill_kernel" + ("<.., fp8 x fp8>" if f8 else ""),
+                     "achieved": achieved, "peak": burst * tc_ratio, "unit": "TFLOP/s", "frac": achieved / (burst * tc_ratio),
+                     "frac_of_sustained": achieved / (sustained * tc_ratio), "traffic": traffic,
+                     "peak_source": peak_src + (" x 2: the guide's nominal fp8 : bf16 ratio (4.5 : 2.25 PFLOP/s); no fp8 "
+                                                "peak is measured on this pool" if f8 else ""),
+                     "algorithmic_flops": gemm_flop},
         "cpu_baseline": {"value": cpu_t / cpu_tiles * tiles * 1e3, "unit": "ms/layer",
                          "cores": len(os.sched_getaffinity(0)), "kind": "oracle",
                          "sample": "query blocks %s of %d (score + select + attend; %d tiles, %d attended block pairs), "
@@ -920,6 +934,8 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="cfg3")
     ap.add_argument("--fmt", default="bf16", choices=["bf16", "mxfp4", "int4_e4m3", "fp8_e4m3"])
+    ap.add_argument("--qfmt", default="bf16", choices=["bf16", "fp8_e4m3"],
+                    help="cfg5 only: format of the selector QUERIES (fp8_e4m3 with --fmt fp8_e4m3: FP8 x FP8 tensor-core scoring)")
     ap.add_argument("--p", type=float, default=0.90)
     ap.add_argument("--L", type=int, default=0, help="cfg5 only: prompt length (default 65536)")
     ap.add_argument("--d-idx", type=int, default=0, choices=[0, 64, 128],

@@ -162,7 +162,7 @@ spot_status spot_selector_project_append(const spot_project_params* p, void* str
  *
  * Supported selector geometries: H_idx == 4 with d_idx == 64 or 128 (anything else: SPOT_ERR_UNSUPPORTED), every cache
  * format in both row forms.  Prefill rows over a quantised cache dequantise the visible prefix into the workspace
- * first (spot_select_workspace_bytes accounts for it).
+ * first (spot_select_workspace_bytes accounts for it) -- unless the queries are quantised too (q_fmt below).
  * --------------------------------------------------------------------------------------------------- */
 typedef struct {
     /* inputs */
@@ -193,6 +193,13 @@ typedef struct {
     /* scratch */
     void* workspace;
     size_t workspace_bytes;      /* >= spot_select_workspace_bytes(&params)                               */
+    /* f2 -- quantised selector QUERIES on the tensor cores ("queries and key cache").  0 (SPOT_SELK_BF16,
+     * the default): sel_q is BF16.  SPOT_SELK_FP8_E4M3: sel_q is FP8-E4M3 bytes [B][Tq][H_idx][d_idx] (what
+     * spot_quantize_selector_k writes for a cache of Tq tokens), accepted with fmt == SPOT_SELK_FP8_E4M3 and q_block == 64
+     * only (SPOT_ERR_UNSUPPORTED otherwise): the tile scores are then FP8 x FP8 products accumulated in fp32 by
+     * tcgen05.mma kind::f8f6f4 straight from the cache -- no dequantise pass, no BF16 scratch.  The result is the score of
+     * the two dequantised images (R33). */
+    int32_t q_fmt;
 } spot_select_params;
 
 size_t spot_select_workspace_bytes(const spot_select_params* p);

@@ -29,6 +29,7 @@ class SelectParams(C.Structure):
         ("indices", C.c_void_p), ("cap", C.c_int32), ("budgets", C.c_void_p),
         ("block_scores", C.c_void_p), ("block_probs", C.c_void_p), ("nb_stride", C.c_int32),
         ("workspace", C.c_void_p), ("workspace_bytes", C.c_size_t),
+        ("q_fmt", C.c_int32),
     ]
 
 

@@ -65,8 +65,9 @@ def spot_dequantize_selector_k(k_cache, k_bf16_out, fmt, B, n_tokens, token_offs
 def make_select_params(sel_q, w, sel_k, fmt, cache_stride_tokens, seq_len, max_seq_len, B, Tq, H_idx, d_idx, *,
                        q_start=0, blk=64, q_block=1, mode="dual_topp", top_k=0, p=0.9, sink_blocks=1,
                        recency_blocks=2, kmin_blocks=8, temperature=1.0, indices=None, cap=0, budgets=None,
-                       block_scores=None, block_probs=None, nb_stride=0, workspace=None):
+                       block_scores=None, block_probs=None, nb_stride=0, workspace=None, q_fmt="bf16"):
     sp = SelectParams()
+    sp.q_fmt = _fmt(q_fmt)
     sp.sel_q, sp.w, sp.sel_k = sel_q.data_ptr(), w.data_ptr(), sel_k.data_ptr()
     sp.fmt = _fmt(fmt)
     sp.cache_stride_tokens = cache_stride_tokens

@@ -35,21 +35,35 @@ constexpr int PF_THREADS = (PF_EPI_WARPS + 2) * 32;
 constexpr uint32_t PF_PLANE_BYTES = 128 * 64 * 2;          // [128 rows][64 d] BF16: one 128-byte swizzle row per token
 constexpr uint32_t PF_SMEM_MISC = 2048;        // barriers, TMEM slot, tile maxima [CHUNK][4 quarters][2 query blocks]
 
-// d_idx = 64: a head is one plane; the query tile is 64 KiB and a K stage holds all four heads of a key-block pair
-// (64 KiB, 2 stages).  d_idx = 128 (the paper's selector width): a head is two planes (the cache row
-// [H][128] read as [2H][64]); the query tile is 128 KiB, so a K stage holds ONE head of a pair (32 KiB, 3 stages) and
-// the issuer accumulates both planes (8 k-steps) into the head's accumulator.
-template <int D>
+// Geometry in BYTES per head row (HB), because that is all the tensor pipe and the TMA see: a token's selector row is
+// PF_H heads x HB bytes, cut into 128-byte planes (one 128-byte swizzle row per token per plane).
+//   HB = 128 : BF16 d_idx = 64, or FP8-E4M3 d_idx = 128 -- a head is one plane; the query tile is 64 KiB and a K stage holds
+//              all four heads of a key-block pair (64 KiB, 2 stages); four 32-byte k-steps per head.
+//   HB = 256 : BF16 d_idx = 128 (the paper's selector width) -- a head is two planes; the query tile is 128 KiB,
+//              so a K stage holds ONE head of a pair (32 KiB, 3 stages) and the issuer accumulates 8 k-steps.
+//   HB = 64  : FP8-E4M3 d_idx = 64 -- two heads share a plane (32 KiB query tile, 32 KiB K stages, 4 stages); a head is the
+//              two k-steps at byte (h & 1) * 64 of its plane.
+// F8 (f2, round 2): both operands are FP8-E4M3 bytes straight from the cache layout (`tcgen05.mma kind::f8f6f4`, K = 32
+// elements = 32 bytes per instruction, fp32 accumulate in TMEM); the BF16 forms use kind::f16 (K = 16 elements = 32 bytes).
+// The TMA maps describe bytes as BF16 pairs either way.
+template <int HB, bool F8>
 struct PfCfg {
-    static_assert(D == 64 || D == 128, "d_idx must be 64 or 128");
-    static constexpr int NSUB = D / 64;                                   // planes per head
-    static constexpr bool PER_HEAD = D == 128;                            // K ring granularity
-    static constexpr int KSTAGES = PER_HEAD ? 3 : 2;
-    static constexpr uint32_t Q_TILE_BYTES = PF_H * NSUB * PF_PLANE_BYTES;
-    static constexpr uint32_t K_STAGE_BYTES = (PER_HEAD ? NSUB : PF_H * NSUB) * PF_PLANE_BYTES;
+    static_assert(HB == 64 || HB == 128 || HB == 256, "head row of 64, 128 or 256 bytes");
+    static_assert(!(F8 && HB == 256) && !(!F8 && HB == 64), "BF16: d_idx 64 / 128; FP8: d_idx 64 / 128");
+    static constexpr int PLANES = PF_H * HB / 128;                        // planes per token row
+    static constexpr int KSTEPS = HB / 32;                                // 32-byte k-steps per head
+    static constexpr bool PER_HEAD = HB == 256;                           // K ring granularity
+    static constexpr int HEAD_PLANES = HB / 128;                          // planes per head (PER_HEAD only)
+    static constexpr int KSTAGES = PER_HEAD ? 3 : (HB == 64 ? 4 : 2);
+    static constexpr uint32_t Q_TILE_BYTES = PLANES * PF_PLANE_BYTES;
+    static constexpr uint32_t K_STAGE_BYTES = (PER_HEAD ? HEAD_PLANES : PLANES) * PF_PLANE_BYTES;
     static constexpr uint32_t SMEM_TILES = Q_TILE_BYTES + KSTAGES * K_STAGE_BYTES;
     static constexpr uint32_t SMEM_BYTES = 1024 + SMEM_TILES + PF_SMEM_MISC;   // 1024: manual alignment slack
     static_assert(SMEM_BYTES <= 227 * 1024, "shared memory");
+    // shared-memory byte offset of k-step ks of head h inside a tile of planes [plane][128 rows][128 B]
+    static constexpr uint32_t koff(int h, int ks) {
+        return (uint32_t)((h * HB + ks * 32) / 128) * PF_PLANE_BYTES + (uint32_t)((h * HB + ks * 32) % 128);
+    }
 };
 
 struct PrefillScoreArgs {
@@ -84,12 +98,12 @@ __device__ __forceinline__ bool decode_item(const PrefillScoreArgs& a, int id, i
     return nk > 0;
 }
 
-template <int D>
+template <int HB, bool F8>
 __global__ void __launch_bounds__(PF_THREADS, 1) score_prefill_kernel(const __grid_constant__ CUtensorMap tm_q,
                                                                       const __grid_constant__ CUtensorMap tm_k,
                                                                       const PrefillScoreArgs a) {
-    using Cfg = PfCfg<D>;
-    constexpr int PF_KSTAGES = Cfg::KSTAGES, NSUB = Cfg::NSUB;
+    using Cfg = PfCfg<HB, F8>;
+    constexpr int PF_KSTAGES = Cfg::KSTAGES;
     constexpr uint32_t Q_TILE_BYTES = Cfg::Q_TILE_BYTES, K_TILE_BYTES = Cfg::K_STAGE_BYTES;
     extern __shared__ unsigned char smem_raw[];
     const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
@@ -155,7 +169,7 @@ __global__ void __launch_bounds__(PF_THREADS, 1) score_prefill_kernel(const __gr
                         mbar_arrive_expect_tx(bar_k_full + 8 * s, K_TILE_BYTES);
                         // a pair that overhangs the cache is zero-filled by TMA; its second block is never used
                         tma_load_4d(k_smem + s * K_TILE_BYTES, &tm_k, bar_k_full + 8 * s, 0, (c * PF_CHUNK + 2 * pr) * 64,
-                                    hh * NSUB, b);
+                                    hh * Cfg::HEAD_PLANES, b);
                     }
                 ++n_item;
             }
@@ -191,14 +205,12 @@ __global__ void __launch_bounds__(PF_THREADS, 1) score_prefill_kernel(const __gr
                         mbar_wait(bar_t_empty + 8 * ts, ((acc / PF_TSTAGES) & 1) ^ 1);
                         tc_fence_after();
 #pragma unroll
-                        for (int sub = 0; sub < NSUB; ++sub)
-#pragma unroll
-                            for (int kk = 0; kk < 4; ++kk) {
-                                const uint64_t ad = umma_desc_sw128(q_smem + (h * NSUB + sub) * PF_PLANE_BYTES + kk * 32);
-                                const uint64_t bd = umma_desc_sw128(ka + ((Cfg::PER_HEAD ? 0 : h * NSUB) + sub) * PF_PLANE_BYTES
-                                                                    + kk * 32);
-                                umma_bf16_ss(tbase + ts * PF_N, ad, bd, idesc, (sub | kk) > 0);
-                            }
+                        for (int ks = 0; ks < Cfg::KSTEPS; ++ks) {
+                            const uint64_t ad = umma_desc_sw128(q_smem + Cfg::koff(h, ks));
+                            const uint64_t bd = umma_desc_sw128(ka + Cfg::koff(Cfg::PER_HEAD ? 0 : h, ks));
+                            if constexpr (F8) umma_f8_ss(tbase + ts * PF_N, ad, bd, umma_idesc_e4m3(PF_M, PF_N), ks > 0);
+                            else umma_bf16_ss(tbase + ts * PF_N, ad, bd, idesc, ks > 0);
+                        }
                         umma_commit(bar_t_full + 8 * ts);      // this head's accumulator is ready for the epilogue
                         if constexpr (Cfg::PER_HEAD) umma_commit(bar_k_empty + 8 * s);
                     }
@@ -340,11 +352,11 @@ bool encode_tmap_bf16_sw128(CUtensorMap* out, const void* base, int rank, const 
 }
 
 // scores: fp32 [B * Tq/64][nb_stride]; entry (row, j) is written for every key block j the row's query block can see
-template <int D>
+template <int HB, bool F8>
 static spot_status score_prefill_d(const spot_select_params* p, float* scores, int nb_stride, cudaStream_t s) {
-    using Cfg = PfCfg<D>;
-    constexpr int PF_D = 64;                                        // plane width
-    constexpr int PLANES = PF_H * Cfg::NSUB;
+    using Cfg = PfCfg<HB, F8>;
+    constexpr int PF_D = 64;                                        // plane width in BF16 pairs-of-bytes (128 bytes)
+    constexpr int PLANES = Cfg::PLANES;
     PrefillScoreArgs a;
     a.w = p->w; a.scores = scores; a.nb_stride = nb_stride;
     a.B = p->B; a.Tq = p->Tq; a.n_qb = p->Tq / 64; a.n_qt = (a.n_qb + 1) / 2;
@@ -357,7 +369,7 @@ static spot_status score_prefill_d(const spot_select_params* p, float* scores, i
     a.total_ids = (int)total;
 
     CUtensorMap tm_q, tm_k;
-    const uint64_t row_bytes = (uint64_t)PLANES * PF_D * 2;          // one token: [H][d_idx] = [PLANES][64]
+    const uint64_t row_bytes = (uint64_t)PLANES * 128;              // one token: PF_H heads x HB bytes = PLANES x 128 bytes
     {
         const uint64_t dims[4] = {(uint64_t)PF_D, (uint64_t)p->Tq, (uint64_t)PLANES, (uint64_t)p->B};
         const uint64_t strides[3] = {row_bytes, (uint64_t)PF_D * 2, (uint64_t)p->Tq * row_bytes};
@@ -367,23 +379,29 @@ static spot_status score_prefill_d(const spot_select_params* p, float* scores, i
     {
         const uint64_t dims[4] = {(uint64_t)PF_D, (uint64_t)p->cache_stride_tokens, (uint64_t)PLANES, (uint64_t)p->B};
         const uint64_t strides[3] = {row_bytes, (uint64_t)PF_D * 2, (uint64_t)p->cache_stride_tokens * row_bytes};
-        // a pair of key blocks: every head's planes (d_idx 64) or one head's two planes (d_idx 128)
-        const uint32_t box[4] = {(uint32_t)PF_D, (uint32_t)PF_N, (uint32_t)(Cfg::PER_HEAD ? Cfg::NSUB : PLANES), 1u};
+        // a pair of key blocks: every head's planes, or (HB = 256) one head's two planes
+        const uint32_t box[4] = {(uint32_t)PF_D, (uint32_t)PF_N, (uint32_t)(Cfg::PER_HEAD ? Cfg::HEAD_PLANES : PLANES), 1u};
         if (!encode_tmap_bf16_sw128(&tm_k, p->sel_k, 4, dims, strides, box)) return SPOT_ERR_CUDA;
     }
     static unsigned long long smem_attr_done = 0;
-    SPOT_CUDA_TRY(set_max_smem_once(score_prefill_kernel<D>, (int)Cfg::SMEM_BYTES, smem_attr_done));
+    SPOT_CUDA_TRY(set_max_smem_once(score_prefill_kernel<HB, F8>, (int)Cfg::SMEM_BYTES, smem_attr_done));
     const int grid = (int)(total < sm_count() ? total : sm_count());
-    SPOT_CUDA_TRY(launch_pdl(score_prefill_kernel<D>, dim3((unsigned)grid), dim3(PF_THREADS), (size_t)Cfg::SMEM_BYTES, s,
+    SPOT_CUDA_TRY(launch_pdl(score_prefill_kernel<HB, F8>, dim3((unsigned)grid), dim3(PF_THREADS), (size_t)Cfg::SMEM_BYTES, s,
                              tm_q, tm_k, a));
     return SPOT_OK;
 }
 
-spot_status score_prefill(const spot_select_params* p, float* scores, int nb_stride, cudaStream_t s) {
-    if (p->fmt != SPOT_SELK_BF16) return SPOT_ERR_UNSUPPORTED;      // quantised caches: dequantised by the caller (api.cu)
+// fp8: queries AND keys are FP8-E4M3 bytes ([..][H][d], the FP8 cache layout); else both are BF16
+spot_status score_prefill(const spot_select_params* p, float* scores, int nb_stride, bool fp8, cudaStream_t s) {
     if (p->H_idx != PF_H) return SPOT_ERR_UNSUPPORTED;
-    if (p->d_idx == 64) return score_prefill_d<64>(p, scores, nb_stride, s);
-    if (p->d_idx == 128) return score_prefill_d<128>(p, scores, nb_stride, s);
+    if (fp8) {
+        if (p->d_idx == 64) return score_prefill_d<64, true>(p, scores, nb_stride, s);
+        if (p->d_idx == 128) return score_prefill_d<128, true>(p, scores, nb_stride, s);
+        return SPOT_ERR_UNSUPPORTED;
+    }
+    if (p->fmt != SPOT_SELK_BF16) return SPOT_ERR_UNSUPPORTED;      // other quantised caches: dequantised by the caller (api.cu)
+    if (p->d_idx == 64) return score_prefill_d<128, false>(p, scores, nb_stride, s);
+    if (p->d_idx == 128) return score_prefill_d<256, false>(p, scores, nb_stride, s);
     return SPOT_ERR_UNSUPPORTED;
 }
 

@@ -232,7 +232,7 @@ class DevicePrefill:
                                     self.B, self.Tq,
                                     wl.H_idx, wl.d_idx, q_start=self.q_start, blk=wl.blk, q_block=wl.q_block,
                                     indices=indices, cap=cap, budgets=budgets, block_scores=scores,
-                                    block_probs=probs, nb_stride=nb_stride, **kw)
+                                    block_probs=probs, nb_stride=nb_stride, q_fmt=getattr(self, "q_fmt", "bf16"), **kw)
         ws = torch.empty(max(api.spot_select_workspace_bytes(sp), 16), dtype=torch.uint8, device="cuda")
         sp.workspace, sp.workspace_bytes = ws.data_ptr(), ws.numel()
         api.spot_select(sp)
@@ -253,6 +253,21 @@ class DevicePrefill:
         self.fmt = fmt
         for x in self.wls:
             x.sel_k = f32_to_bf16_bits(OQ.quantize_dequantize(fmt, x.sel_k).astype(np.float32))
+
+    def quantise_queries(self, fmt="fp8_e4m3"):
+        """f2: the chunk's selector queries through the cache quantiser (a cache of Tq tokens), kept in the quantised
+        layout for the tensor-core path (q_fmt); the workloads' BF16 queries are replaced by the ORACLE quantiser's image of
+        them, so the oracle scores (quantised q) x (quantised k)."""
+        import torch
+        from workloads import f32_to_bf16_bits
+        wl, api = self.wl, self.api
+        q8 = torch.zeros(api.spot_selector_k_bytes(fmt, self.B, self.Tq, wl.H_idx, wl.d_idx), dtype=torch.uint8, device="cuda")
+        api.spot_quantize_selector_k(self.sel_q, q8, fmt, self.B, self.Tq, 0, self.Tq, wl.H_idx, wl.d_idx)
+        self.sel_q, self.q_fmt = q8, fmt
+        for x in self.wls:
+            img = OQ.quantize_dequantize(fmt, x.sel_q[self.q_start:self.q_start + self.Tq])
+            x.sel_q = x.sel_q.copy()
+            x.sel_q[self.q_start:self.q_start + self.Tq] = f32_to_bf16_bits(img.astype(np.float32))
 
     def attend(self, indices_np, budgets_np, want_lse=False):
         import torch

@@ -427,3 +427,25 @@ def test_prefill_block16_attention_over_paged_kv(torch_cuda):
     dp.kv_strides = (Hkv * pt * D, D, pt * D)
     dp.page_table, dp.page_tokens = torch.from_numpy(table).cuda(), pt
     _check_attn_prefill(dp, lists)
+
+
+# ---------------------------------------------------------------- f2: FP8 x FP8 tile scores on the tensor cores
+@pytest.mark.parametrize("d_idx,L,q_start,Tq,B,blk", [(64, 1024, 0, 1024, 1, 64), (128, 1024, 512, 320, 2, 64),
+                                                      (128, 4608, 0, 4608, 1, 64), (64, 1024, 256, 256, 1, 16)])
+def test_prefill_fp8_queries_and_keys_on_the_tensor_cores(torch_cuda, d_idx, L, q_start, Tq, B, blk):
+    """PAPER.md:115 / :186 quantise the selector's queries as well as its key cache.  With both in FP8-E4M3 the tile
+    scores are FP8 x FP8 products accumulated in fp32 by tcgen05.mma kind::f8f6f4 straight from the cache layout (q_fmt):
+    no dequantise pass.  The oracle scores the two dequantised images (R33).  Every product of two E4M3 values has at most
+    8 significant bits, so the products are exact and the only error is the fp32 accumulation over d_idx -- the same
+    2e-5 tolerance as the BF16 GEMM, and exact index lists."""
+    geo = dict(blk=16, sink_blocks=8, recency_blocks=16, kmin_blocks=32) if blk == 16 else {}
+    wls = [_neg_weights(make_prefill_workload(seed=6606 + 7 * b, L=L, d_idx=d_idx, with_kv=False, **geo), 60 + b)
+           for b in range(B)]
+    dp = H.DevicePrefill(wls, q_start, Tq, with_kv=False)
+    dp.set_cache_format("fp8_e4m3")
+    dp.quantise_queries("fp8_e4m3")
+    report = []
+    _check_select_prefill(dp, report)
+    _check_select_prefill(dp, report, mode="topk", top_k=40 if blk == 16 else 6)
+    print("fp8 x fp8 prefill select d_idx=%d L=%d: near-tie rows %s" % (d_idx, L, report[:4]))
+    assert len(report) <= 1

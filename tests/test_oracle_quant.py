@@ -268,3 +268,39 @@ def test_fp8_cache_is_nearest_e4m3_value_per_element():
     vals = quant.dequantize_fp8_e4m3(all_codes)
     assert np.array_equal(quant.quantize_fp8_e4m3(f32_to_bf16_bits(vals.astype(np.float32))) & 0x7F, all_codes & 0x7F)
     assert quant.selector_k_bytes("fp8_e4m3", 131072 * 36 * 512) * 2 == quant.selector_k_bytes("bf16", 131072 * 36 * 512)
+
+
+def test_quantised_query_times_quantised_key_scores_are_scores_of_the_two_images():
+    """f2 / R33: "quantised queries x quantised keys" is, by definition, the score of the two dequantised images.  Pins of
+    that composition: (a) inputs that already sit on the E4M3 grid pass through the quantiser unchanged, so the quantised
+    score equals the plain one; (b) scalar loops over the E4M3 value table on a tiny case; (c) every product of two E4M3
+    values has <= 8 significant bits (what makes the FP8 x FP8 tensor-core products exact)."""
+    from fractions import Fraction
+    from oracle import quant as OQ
+    from oracle import selection as OS
+    from oracle.bf16 import f64_to_bf16_bits_exact
+    rng = np.random.default_rng(9)
+    grid = OQ.e4m3_value(np.arange(0x7F))
+    q = rng.choice(grid, size=(2, 32)) * rng.choice([-1.0, 1.0], size=(2, 32))
+    k = rng.choice(grid, size=(5, 2, 32)) * rng.choice([-1.0, 1.0], size=(5, 2, 32))
+    w = np.array([0.7, -0.3])
+    qd = OQ.quantize_dequantize("fp8_e4m3", f64_to_bf16_bits_exact(q))
+    kd = OQ.quantize_dequantize("fp8_e4m3", f64_to_bf16_bits_exact(k))
+    assert np.array_equal(qd, q) and np.array_equal(kd, k)                                 # (a)
+    got = OS.token_scores(qd, w, kd)
+    for t in range(5):                                                                     # (b)
+        want = sum(w[h] * max(0.0, sum(float(q[h, i]) * float(k[t, h, i]) for i in range(32))) for h in range(2))
+        assert abs(got[t] - want) < 1e-12
+    for a_ in grid[::7]:                                                                   # (c)
+        for b_ in grid[::5]:
+            pr = Fraction(float(a_)) * Fraction(float(b_))
+            if pr:
+                num = pr.numerator
+                while num % 2 == 0:
+                    num //= 2
+                assert num < 256
+    # off-grid inputs: the quantised score is NOT the plain one (the quantiser does something)
+    q2 = rng.standard_normal((2, 32))
+    from workloads import f32_to_bf16_bits
+    qb = f32_to_bf16_bits(q2.astype(np.float32))
+    assert not np.array_equal(OQ.quantize_dequantize("fp8_e4m3", qb), OQ.quantize_dequantize("bf16", qb))
