@@ -449,3 +449,37 @@ def test_prefill_fp8_queries_and_keys_on_the_tensor_cores(torch_cuda, d_idx, L, 
     _check_select_prefill(dp, report, mode="topk", top_k=40 if blk == 16 else 6)
     print("fp8 x fp8 prefill select d_idx=%d L=%d: near-tie rows %s" % (d_idx, L, report[:4]))
     assert len(report) <= 1
+
+
+def test_q_fmt_argument_errors(torch_cuda):
+    """spot.h, q_fmt: FP8 queries need an FP8 cache and the prefill form; any other value is an invalid argument.  Nothing
+    is written to the outputs by a refused call."""
+    from paper_2606_22874_b200 import api
+    wl = make_prefill_workload(seed=6707, L=256, with_kv=False)
+    dp = H.DevicePrefill([wl], 0, 128, with_kv=False)
+    dp.q_fmt = "fp8_e4m3"                                         # BF16 cache, FP8 query flag
+    with pytest.raises(api.SpotError) as e:
+        dp.select()
+    assert "UNSUPPORTED" in str(e.value)
+    dp.set_cache_format("mxfp4")
+    with pytest.raises(api.SpotError) as e:
+        dp.select()
+    assert "UNSUPPORTED" in str(e.value)
+    dp.set_cache_format("fp8_e4m3")
+    dp.q_fmt = "mxfp4"
+    with pytest.raises(api.SpotError) as e:
+        dp.select()
+    assert "UNSUPPORTED" in str(e.value) or "INVALID_ARG" in str(e.value)
+    sp = api.make_select_params(dp.sel_q, dp.w, dp.sel_k, "fp8_e4m3", 256, None, 0, 1, 128, wl.H_idx, wl.d_idx,
+                                q_start=0, blk=wl.blk, q_block=64, mode=wl.mode, p=wl.p)
+    sp.q_fmt = 77
+    with pytest.raises(api.SpotError) as e:
+        api.spot_select_workspace_bytes(sp)
+    assert "INVALID_ARG" in str(e.value)
+    # the decode form takes BF16 queries only
+    wd = make_prefill_workload(seed=6708, L=256, with_kv=False)
+    sp = api.make_select_params(dp.sel_q, dp.w, dp.sel_k, "fp8_e4m3", 256, None, 0, 1, 1, wd.H_idx, wd.d_idx,
+                                blk=wd.blk, q_block=1, q_fmt="fp8_e4m3", mode=wd.mode, p=wd.p)
+    with pytest.raises(api.SpotError) as e:
+        api.spot_select_workspace_bytes(sp)
+    assert "UNSUPPORTED" in str(e.value)
