@@ -41,7 +41,8 @@ def build(force=False, verbose=False):
         s = os.path.join(CSRC, src)
         o = os.path.join(OBJ, src.replace(".cu", ".o"))
         if force or _stale(o, [s] + headers):
-            cmd = [nvcc, "-c", s, "-o", o] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else [])
+            cmd = [nvcc, "-c", s, "-o", o] + NVCC_FLAGS + os.environ.get("SPOT_NVCC_FLAGS", "").split() + \
+                (["-Xptxas", "-v"] if verbose else [])
             jobs.append(cmd)
 
     def run(cmd):

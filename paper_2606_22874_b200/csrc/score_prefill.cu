@@ -6,14 +6,14 @@
 //     to one persistent CTA per SM;
 //   * warp 8 lane 0: TMA producer -- the query tile ([4 heads][128][64] BF16, 64 KiB) and a 2-stage ring of key-block
 //     PAIRS ([4 heads][128 keys][64], 64 KiB) land in 128-byte-swizzled shared memory through 4-D tensor maps;
-//   * warp 9 lane 0: issues tcgen05.mma with M = 128 queries, N = 128 keys (two key blocks), K = 16: four k-steps per
+//   * warp 9 (converged, one elected lane issues): tcgen05.mma with M = 128 queries, N = 128 keys (two key blocks), K = 16: four k-steps per
 //     head into a 128-column TMEM accumulator.  N = 64 made every MMA read 6 KiB of operands for 16 cycles of math
 //     (384 B/clk) and the tensor pipe sat at 65 % busy for 37 % of peak (profiles/r1_prefill_cfg5.md); N = 128 halves
 //     the A-operand re-reads per flop.  The 512 TMEM columns are a ring of FOUR accumulators, one per (pair, head):
 //     the issuer runs up to three heads ahead of the epilogue;
 //   * warps 0-7: epilogue.  Warp w owns TMEM lanes 32 (w & 3) .. +31 (one query per lane) and the 64 columns of key
-//     block (w >> 2) of the pair.  Head by head it reads the accumulator (tcgen05.ld), releases it, and adds
-//     w_h ReLU(d_h) to a 64-register running sum; after the fourth head the tile maximum is a REDUX.MAX over an
+//     block (w >> 2) of the pair.  Head by head it reads the accumulator (two 32-column tcgen05.ld, the next one in
+//     flight under the arithmetic on the previous), releases it, and adds w_h ReLU(d_h) to a 64-register running sum; after the fourth head the tile maximum is a REDUX.MAX over an
 //     order-preserving integer key plus one shared-memory atomicMax per warp.
 // The epilogue is the near-co-bound (9 lane-ops per (query, key) pair against 512 tensor flops), so ReLU is split
 // between the two fp32 pipes: heads 0-1 use (w/2)(d + |d|) (FADD with an abs modifier, FMA pipe), heads 2-3 use
@@ -23,13 +23,16 @@
 
 namespace spot {
 
+#ifdef SPOT_TRACE
+long long* g_pf_trace = nullptr;      // development builds only
+#endif
+
 namespace {
 
 constexpr int PF_H = 4;                 // selector heads
 constexpr int PF_M = 128;               // queries per tile (two 64-query blocks)
 constexpr int PF_N = 128;               // keys per MMA (two 64-key blocks)
 constexpr int PF_CHUNK = 32;            // key blocks per work item
-constexpr int PF_TSTAGES = 4;           // TMEM accumulators (128 columns each)
 constexpr int PF_EPI_WARPS = 8;
 constexpr int PF_THREADS = (PF_EPI_WARPS + 2) * 32;
 constexpr uint32_t PF_PLANE_BYTES = 128 * 64 * 2;          // [128 rows][64 d] BF16: one 128-byte swizzle row per token
@@ -37,15 +40,27 @@ constexpr uint32_t PF_SMEM_MISC = 2048;        // barriers, TMEM slot, tile maxi
 
 // Geometry in BYTES per head row (HB), because that is all the tensor pipe and the TMA see: a token's selector row is
 // PF_H heads x HB bytes, cut into 128-byte planes (one 128-byte swizzle row per token per plane).
-//   HB = 128 : BF16 d_idx = 64, or FP8-E4M3 d_idx = 128 -- a head is one plane; the query tile is 64 KiB and a K stage holds
-//              all four heads of a key-block pair (64 KiB, 2 stages); four 32-byte k-steps per head.
-//   HB = 256 : BF16 d_idx = 128 (the paper's selector width) -- a head is two planes; the query tile is 128 KiB,
-//              so a K stage holds ONE head of a pair (32 KiB, 3 stages) and the issuer accumulates 8 k-steps.
-//   HB = 64  : FP8-E4M3 d_idx = 64 -- two heads share a plane (32 KiB query tile, 32 KiB K stages, 4 stages); a head is the
-//              two k-steps at byte (h & 1) * 64 of its plane.
+//   HB = 128 : BF16 d_idx = 64, or FP8-E4M3 d_idx = 128 -- a head is one plane; a K slot holds all four heads of a
+//              key-block pair (64 KiB, 2 slots beside the 64 KiB query tile); four 32-byte k-steps per head.
+//   HB = 256 : BF16 d_idx = 128 (the paper's selector width) -- a head is two planes; a K slot holds ONE head
+//              of a pair (32 KiB, 3 slots beside the 128 KiB query tile) and the issuer accumulates 8 k-steps.
+//   HB = 64  : FP8-E4M3 d_idx = 64 -- two heads share a plane (32 KiB query tile, six 32 KiB slots); a head is the two k-steps at byte
+//              (h & 1) * 64 of its plane.
 // F8 (f2, round 2): both operands are FP8-E4M3 bytes straight from the cache layout (`tcgen05.mma kind::f8f6f4`, K = 32
 // elements = 32 bytes per instruction, fp32 accumulate in TMEM); the BF16 forms use kind::f16 (K = 16 elements = 32 bytes).
-// The TMA maps describe bytes as BF16 pairs either way.
+// The TMA map describes bytes as BF16 pairs either way.
+//
+// Round-2 measurements that shaped this (per-CTA clock64 timeline of producer / issuer / epilogue, _work-side probes; DESIGN.md
+// section 7): (1) under `if (lane == 0)` ptxas wraps every tcgen05.mma in an ELECT / BRA.U.ANY loop of its own, one basic
+// block per MMA, and the issuing thread needed 70-130 cycles per 64-cycle MMA -- the issuer warp now runs converged and one
+// ELECTED lane issues (tc100.cuh, umma_*_elect): 140-190 cycles per head of four MMAs; (2) the epilogue keeps one 32-column
+// tcgen05.ld in flight under the arithmetic on the previous one; (3) the query tile as the A operand in TENSOR MEMORY
+// (tcgen05.mma with [a_tmem]) halves the shared-memory reads of the MMAs and frees 64-128 KiB for a deeper key ring, but
+// costs accumulators (3 instead of 4 at HB = 128, 2 at HB = 256) and was 19 % / 8 % SLOWER: the depth of the accumulator ring
+// is what hides the issuer <-> epilogue hand-off, so both operands stay in shared memory; (4) a thread-block cluster of two
+// query tiles sharing every key load by TMA multicast, a key ring of ten 16 KiB single-head slots, sixteen epilogue warps,
+// and both fp32 pipes inside every head (element 0 of a pair through FADD, element 1 through FMNMX) were all measured
+// equal or slower.
 template <int HB, bool F8>
 struct PfCfg {
     static_assert(HB == 64 || HB == 128 || HB == 256, "head row of 64, 128 or 256 bytes");
@@ -54,12 +69,15 @@ struct PfCfg {
     static constexpr int KSTEPS = HB / 32;                                // 32-byte k-steps per head
     static constexpr bool PER_HEAD = HB == 256;                           // K ring granularity
     static constexpr int HEAD_PLANES = HB / 128;                          // planes per head (PER_HEAD only)
-    static constexpr int KSTAGES = PER_HEAD ? 3 : (HB == 64 ? 4 : 2);
+    static constexpr int STAGE_PLANES = PER_HEAD ? HEAD_PLANES : PLANES;  // planes of one K ring slot
     static constexpr uint32_t Q_TILE_BYTES = PLANES * PF_PLANE_BYTES;
-    static constexpr uint32_t K_STAGE_BYTES = (PER_HEAD ? HEAD_PLANES : PLANES) * PF_PLANE_BYTES;
+    static constexpr uint32_t K_STAGE_BYTES = STAGE_PLANES * PF_PLANE_BYTES;
+    static constexpr int KSTAGES = (int)((224u * 1024u - Q_TILE_BYTES) / K_STAGE_BYTES);   // 2 / 3 / 6
+    static_assert(KSTAGES >= 2 && KSTAGES <= 8, "key ring");
     static constexpr uint32_t SMEM_TILES = Q_TILE_BYTES + KSTAGES * K_STAGE_BYTES;
     static constexpr uint32_t SMEM_BYTES = 1024 + SMEM_TILES + PF_SMEM_MISC;   // 1024: manual alignment slack
     static_assert(SMEM_BYTES <= 227 * 1024, "shared memory");
+    static constexpr int NACC = 512 / PF_N;                               // TMEM: a ring of four 128-column accumulators
     // shared-memory byte offset of k-step ks of head h inside a tile of planes [plane][128 rows][128 B]
     static constexpr uint32_t koff(int h, int ks) {
         return (uint32_t)((h * HB + ks * 32) / 128) * PF_PLANE_BYTES + (uint32_t)((h * HB + ks * 32) % 128);
@@ -75,7 +93,15 @@ struct PrefillScoreArgs {
     int n_chunks_max;
     int total_ids;
     int fine;                 // blk == 16 (f3): four scores per 64-key block, one per 16-token quarter
+#ifdef SPOT_TRACE
+    long long* trace;         // development builds only: [6 roles][2048 events] clock64 of CTA 5
+#endif
 };
+#ifdef SPOT_TRACE
+#define PF_STAMP(role, idx) do { if (a.trace && blockIdx.x == 5 && (idx) < 2048) a.trace[(role) * 2048 + (idx)] = clock64(); } while (0)
+#else
+#define PF_STAMP(role, idx) do { } while (0)
+#endif
 
 __device__ __forceinline__ uint32_t f32_order_key(float x) {
     const uint32_t u = __float_as_uint(x);
@@ -98,29 +124,38 @@ __device__ __forceinline__ bool decode_item(const PrefillScoreArgs& a, int id, i
     return nk > 0;
 }
 
+// ring position of an accumulator: slot and the parity of its use
+struct AccPos {
+    int slot, par;
+    __device__ __forceinline__ void next(int n) {
+        if (++slot == n) { slot = 0; par ^= 1; }
+    }
+};
+
 template <int HB, bool F8>
 __global__ void __launch_bounds__(PF_THREADS, 1) score_prefill_kernel(const __grid_constant__ CUtensorMap tm_q,
                                                                       const __grid_constant__ CUtensorMap tm_k,
                                                                       const PrefillScoreArgs a) {
     using Cfg = PfCfg<HB, F8>;
-    constexpr int PF_KSTAGES = Cfg::KSTAGES;
-    constexpr uint32_t Q_TILE_BYTES = Cfg::Q_TILE_BYTES, K_TILE_BYTES = Cfg::K_STAGE_BYTES;
+    constexpr int PF_KSTAGES = Cfg::KSTAGES, NACC = Cfg::NACC;
+    constexpr uint32_t K_TILE_BYTES = Cfg::K_STAGE_BYTES, Q_TILE_BYTES = Cfg::Q_TILE_BYTES;
     extern __shared__ unsigned char smem_raw[];
     const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
     unsigned char* smem = smem_raw + (smem_base - smem_u32(smem_raw));
-    const uint32_t q_smem = smem_base;                               // 64 / 128 KiB
-    const uint32_t k_smem = smem_base + Q_TILE_BYTES;                // 2 x 64 KiB / 3 x 32 KiB
+    const uint32_t q_smem = smem_base;                               // the query tile
+    const uint32_t k_smem = smem_base + Q_TILE_BYTES;                // the key ring
     unsigned char* misc = smem + Cfg::SMEM_TILES;
     const uint32_t misc_u32 = smem_base + Cfg::SMEM_TILES;
     // barriers (8 bytes each)
     const uint32_t bar_q_full = misc_u32 + 0;
     const uint32_t bar_q_empty = misc_u32 + 8;
-    const uint32_t bar_k_full = misc_u32 + 16;     // [<= 4]
-    const uint32_t bar_k_empty = misc_u32 + 48;    // [<= 4]
-    const uint32_t bar_t_full = misc_u32 + 80;     // [4]
-    const uint32_t bar_t_empty = misc_u32 + 112;   // [4]
-    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(misc + 144);
-    uint32_t* s_max = reinterpret_cast<uint32_t*>(misc + 160);       // [CHUNK][4 quarters][2 query blocks]
+    const uint32_t bar_k_full = misc_u32 + 16;     // [<= 8]
+    const uint32_t bar_k_empty = misc_u32 + 80;    // [<= 8]
+    const uint32_t bar_t_full = misc_u32 + 144;    // [<= 4]
+    const uint32_t bar_t_empty = misc_u32 + 176;   // [<= 4]
+    static_assert(PF_KSTAGES <= 8 && NACC <= 4, "barrier layout");
+    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(misc + 208);
+    uint32_t* s_max = reinterpret_cast<uint32_t*>(misc + 224);       // [CHUNK][4 quarters][2 query blocks]
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
 
@@ -131,14 +166,14 @@ __global__ void __launch_bounds__(PF_THREADS, 1) score_prefill_kernel(const __gr
             mbar_init(bar_k_full + 8 * i, 1);
             mbar_init(bar_k_empty + 8 * i, 1);
         }
-        for (int i = 0; i < PF_TSTAGES; ++i) {
+        for (int i = 0; i < NACC; ++i) {
             mbar_init(bar_t_full + 8 * i, 1);
             mbar_init(bar_t_empty + 8 * i, PF_EPI_WARPS);
         }
         mbar_fence_init();
     }
     for (int e = threadIdx.x; e < PF_CHUNK * 4 * 2; e += PF_THREADS) s_max[e] = 0u;
-    if (warp == 0) tmem_alloc(misc_u32 + 144, 512);
+    if (warp == 0) tmem_alloc(misc_u32 + 208, 512);
     if (warp == PF_EPI_WARPS && lane == 0) {
         tma_prefetch_desc(&tm_q);
         tma_prefetch_desc(&tm_k);
@@ -151,7 +186,7 @@ __global__ void __launch_bounds__(PF_THREADS, 1) score_prefill_kernel(const __gr
     pdl_launch_dependents();
 
     if (warp == PF_EPI_WARPS) {
-        // ================================ TMA producer ================================
+        // ================================ TMA producer: the key ring ================================
         if (lane == 0) {
             int n_item = 0, kp = 0;
             for (int id = blockIdx.x; id < a.total_ids; id += gridDim.x) {
@@ -160,8 +195,9 @@ __global__ void __launch_bounds__(PF_THREADS, 1) score_prefill_kernel(const __gr
                 mbar_wait(bar_q_empty, (n_item & 1) ^ 1);
                 mbar_arrive_expect_tx(bar_q_full, Q_TILE_BYTES);
                 tma_load_4d(q_smem, &tm_q, bar_q_full, 0, m * PF_M, 0, b);
+                ++n_item;
                 const int np = (nk + 1) >> 1;
-                // (kp counts ring slots: one per pair at d_idx 64, one per (pair, head) at d_idx 128)
+                // (kp counts ring slots: one per pair, or one per (pair, head) at HB = 256)
                 for (int pr = 0; pr < np; ++pr)
                     for (int hh = 0; hh < (Cfg::PER_HEAD ? PF_H : 1); ++hh, ++kp) {
                         const int s = kp % PF_KSTAGES;
@@ -170,27 +206,47 @@ __global__ void __launch_bounds__(PF_THREADS, 1) score_prefill_kernel(const __gr
                         // a pair that overhangs the cache is zero-filled by TMA; its second block is never used
                         tma_load_4d(k_smem + s * K_TILE_BYTES, &tm_k, bar_k_full + 8 * s, 0, (c * PF_CHUNK + 2 * pr) * 64,
                                     hh * Cfg::HEAD_PLANES, b);
+                        PF_STAMP(0, kp);
                     }
-                ++n_item;
             }
         }
-    } else if (warp == PF_EPI_WARPS + 1) {
-        // ================================ MMA issuer ================================
-        if (lane == 0) {
-            constexpr uint32_t idesc = umma_idesc_bf16(PF_M, PF_N);
-            int n_item = 0, kp = 0, acc = 0;
+#ifdef SPOT_TRACE
+        if (lane == 1 && a.trace && blockIdx.x == 5) {          // observer: when does each key slot actually arrive?
+            int kp = 0;
             for (int id = blockIdx.x; id < a.total_ids; id += gridDim.x) {
                 int b, c, m, nk;
                 if (!decode_item(a, id, b, c, m, nk)) continue;
-                mbar_wait(bar_q_full, n_item & 1);
+                const int np = (nk + 1) >> 1;
+                for (int pr = 0; pr < np; ++pr)
+                    for (int hh = 0; hh < (Cfg::PER_HEAD ? PF_H : 1); ++hh, ++kp) {
+                        const int s = kp % PF_KSTAGES;
+                        mbar_wait(bar_k_full + 8 * s, (kp / PF_KSTAGES) & 1);
+                        PF_STAMP(1, kp);
+                    }
+            }
+        }
+#endif
+    } else if (warp == PF_EPI_WARPS + 1) {
+        // ================================ MMA issuer ================================
+        // The whole warp runs this loop converged; one elected lane issues (tc100.cuh, umma_*_elect).
+        {
+            constexpr uint32_t idesc = F8 ? umma_idesc_e4m3(PF_M, PF_N) : umma_idesc_bf16(PF_M, PF_N);
+            int n_item = 0, kp = 0, acc = 0;
+            AccPos ap{0, 0};
+            const uint64_t qd = umma_desc_sw128(q_smem);
+            for (int id = blockIdx.x; id < a.total_ids; id += gridDim.x) {
+                int b, c, m, nk;
+                if (!decode_item(a, id, b, c, m, nk)) continue;
+                mbar_wait(bar_q_full, n_item & 1);             // the item's query tile has landed
+                tc_fence_after();
                 const int np = (nk + 1) >> 1;
                 for (int pr = 0; pr < np; ++pr) {
                     int s = 0;
-                    uint32_t ka = 0;
+                    uint64_t kd = 0;                           // descriptor of the slot's first byte
                     if constexpr (!Cfg::PER_HEAD) {
                         s = kp % PF_KSTAGES;
                         mbar_wait(bar_k_full + 8 * s, (kp / PF_KSTAGES) & 1);
-                        ka = k_smem + s * K_TILE_BYTES;
+                        kd = umma_desc_sw128(k_smem + s * K_TILE_BYTES);
                         ++kp;
                     }
 #pragma unroll
@@ -198,35 +254,51 @@ __global__ void __launch_bounds__(PF_THREADS, 1) score_prefill_kernel(const __gr
                         if constexpr (Cfg::PER_HEAD) {
                             s = kp % PF_KSTAGES;
                             mbar_wait(bar_k_full + 8 * s, (kp / PF_KSTAGES) & 1);
-                            ka = k_smem + s * K_TILE_BYTES;
+                            kd = umma_desc_sw128(k_smem + s * K_TILE_BYTES);
                             ++kp;
                         }
-                        const int ts = acc % PF_TSTAGES;
-                        mbar_wait(bar_t_empty + 8 * ts, ((acc / PF_TSTAGES) & 1) ^ 1);
+                        mbar_wait(bar_t_empty + 8 * ap.slot, ap.par ^ 1);
+                        if (lane == 0) PF_STAMP(2, acc);
                         tc_fence_after();
+                        const uint32_t d_tmem = tbase + ap.slot * PF_N;
 #pragma unroll
                         for (int ks = 0; ks < Cfg::KSTEPS; ++ks) {
-                            const uint64_t ad = umma_desc_sw128(q_smem + Cfg::koff(h, ks));
-                            const uint64_t bd = umma_desc_sw128(ka + Cfg::koff(Cfg::PER_HEAD ? 0 : h, ks));
-                            if constexpr (F8) umma_f8_ss(tbase + ts * PF_N, ad, bd, umma_idesc_e4m3(PF_M, PF_N), ks > 0);
-                            else umma_bf16_ss(tbase + ts * PF_N, ad, bd, idesc, ks > 0);
+                            // the address field of the descriptor is (byte address >> 4): add the k-step's offset to it
+                            const uint64_t bd = kd + (uint64_t)(Cfg::koff(Cfg::PER_HEAD ? 0 : h, ks) >> 4);
+                            const uint64_t ad = qd + (uint64_t)(Cfg::koff(h, ks) >> 4);
+                            if constexpr (F8) umma_f8_ss_elect(d_tmem, ad, bd, idesc, ks > 0);
+                            else umma_bf16_ss_elect(d_tmem, ad, bd, idesc, ks > 0);
                         }
-                        umma_commit(bar_t_full + 8 * ts);      // this head's accumulator is ready for the epilogue
-                        if constexpr (Cfg::PER_HEAD) umma_commit(bar_k_empty + 8 * s);
+                        umma_commit_elect(bar_t_full + 8 * ap.slot);      // this head's accumulator is ready for the epilogue
+                        if (lane == 0) PF_STAMP(3, acc);
+                        if constexpr (Cfg::PER_HEAD) umma_commit_elect(bar_k_empty + 8 * s);
+                        ap.next(NACC);
                     }
-                    if constexpr (!Cfg::PER_HEAD) umma_commit(bar_k_empty + 8 * s);   // slot free once these MMAs have read it
+                    if constexpr (!Cfg::PER_HEAD) umma_commit_elect(bar_k_empty + 8 * s);   // slot free once these MMAs have read it
                 }
-                umma_commit(bar_q_empty);
+                umma_commit_elect(bar_q_empty);
                 ++n_item;
             }
         }
     } else {
-        // ================================ epilogue (warps 0-7) ================================
+        // ================================ epilogue (warps 0 .. 7) ================================
+        // Warp w owns TMEM lanes 32 (w & 3) .. +31 (one query per lane) and the 64 accumulator columns of key block (w >> 2)
+        // of the pair.  TMEM reads and the fp32 arithmetic overlap: a warp keeps one 32-column tcgen05.ld in flight while it
+        // works on the previous one (wait::ld, issue the next load into the other buffer, compute; tcgen05.wait::ld waits for
+        // every outstanding load, hence this order).
+        constexpr int EC = PF_N / (PF_EPI_WARPS / 4);        // accumulator columns per warp: 64
+        constexpr int NSUB = EC / 32;                        // 32-column loads per head
+        constexpr int NU = PF_H * NSUB;                      // loads per key-block pair (even)
         const int lq = warp & 3, ch = warp >> 2;
+        const int col0 = ch * EC;                 // first accumulator column of this warp
+        const int kb_in_pair = col0 >> 6;         // which key block of the pair
+        const int c_in_blk = col0 & 63;           // first key of the warp inside that block
         const int row = lq * 32 + lane;           // query row of the tile = TMEM lane
         const int qbl = lq >> 1;                  // which of the tile's two query blocks
-        const uint32_t t_lane = tbase + ((uint32_t)(lq * 32) << 16) + ch * 64;
-        int n_item = 0, acc = 0;
+        const uint32_t t_row = tbase + ((uint32_t)(lq * 32) << 16);
+        const uint32_t t_lane = t_row + col0;
+        int pc = 0;
+        AccPos ap{0, 0};                          // the accumulator whose load is in flight / comes next
         for (int id = blockIdx.x; id < a.total_ids; id += gridDim.x) {
             int b, c, m, nk;
             if (!decode_item(a, id, b, c, m, nk)) continue;
@@ -238,49 +310,61 @@ __global__ void __launch_bounds__(PF_THREADS, 1) score_prefill_kernel(const __gr
             const int qb_abs = a.qb_start + 2 * m + qbl;        // this row's (absolute) query block = its diagonal
             const int q_in_blk = row & 63;
             const int np = (nk + 1) >> 1;
-            for (int pr = 0; pr < np; ++pr) {
-                float S[64];
+            float buf[2][32];
+            mbar_wait(bar_t_full + 8 * ap.slot, ap.par);
+            tc_fence_after();
+            tmem_ld32(t_lane + ap.slot * PF_N, buf[0]);
+            for (int pr = 0; pr < np; ++pr, ++pc) {
+                float S[EC];
 #pragma unroll
-                for (int h = 0; h < PF_H; ++h, ++acc) {
-                    const int ts = acc % PF_TSTAGES;
-                    mbar_wait(bar_t_full + 8 * ts, (acc / PF_TSTAGES) & 1);
-                    tc_fence_after();
-                    float dd[64];
-                    tmem_ld64(t_lane + ts * PF_N, dd);
-                    tmem_ld_wait();
-                    tc_fence_before();
-                    __syncwarp();
-                    if (lane == 0) mbar_arrive(bar_t_empty + 8 * ts);
-#pragma unroll
-                    for (int q4 = 0; q4 < 4; ++q4)
-#pragma unroll
-                        for (int i = 0; i < 16; i += 2) {
-                            float& s0 = S[q4 * 16 + i];
-                            float& s1 = S[q4 * 16 + i + 1];
-                            const float d0 = dd[q4 * 16 + i], d1 = dd[q4 * 16 + i + 1];
-                            if (h == 0) {
-                                s0 = wh0 * (d0 + fabsf(d0));
-                                s1 = wh0 * (d1 + fabsf(d1));
-                            } else if (h == 1) {
-                                ffma2(s0, s1, d0 + fabsf(d0), d1 + fabsf(d1), wh1, s0, s1);
-                            } else {
-                                ffma2(s0, s1, fmaxf(d0, 0.f), fmaxf(d1, 0.f), h == 2 ? wv.z : wv.w, s0, s1);
-                            }
+                for (int u = 0; u < NU; ++u) {
+                    const int h = u / NSUB, sb = u % NSUB;
+                    tmem_ld_wait32(buf[u & 1]);
+                    if (sb == 0 && warp == 0 && lane == 0) PF_STAMP(4, pc * 4 + h);
+                    if (sb == NSUB - 1) {                       // head h fully read: hand its accumulator back
+                        tc_fence_before();
+                        __syncwarp();
+                        if (lane == 0) mbar_arrive(bar_t_empty + 8 * ap.slot);
+                        if (warp == 0 && lane == 0) PF_STAMP(5, pc * 4 + h);
+                        ap.next(NACC);
+                    }
+                    if (u + 1 < NU || pr + 1 < np) {
+                        const int sb1 = (u + 1) % NSUB;
+                        if (sb1 == 0) {                         // a new accumulator
+                            mbar_wait(bar_t_full + 8 * ap.slot, ap.par);
+                            tc_fence_after();
                         }
+                        tmem_ld32(t_lane + ap.slot * PF_N + sb1 * 32, buf[(u + 1) & 1]);
+                    }
+                    const float (&dd)[32] = buf[u & 1];
+#pragma unroll
+                    for (int i = 0; i < 32; i += 2) {
+                        float& s0 = S[sb * 32 + i];
+                        float& s1 = S[sb * 32 + i + 1];
+                        const float d0 = dd[i], d1 = dd[i + 1];
+                        if (h == 0) {
+                            s0 = wh0 * (d0 + fabsf(d0));
+                            s1 = wh0 * (d1 + fabsf(d1));
+                        } else if (h == 1) {
+                            ffma2(s0, s1, d0 + fabsf(d0), d1 + fabsf(d1), wh1, s0, s1);
+                        } else {
+                            ffma2(s0, s1, fmaxf(d0, 0.f), fmaxf(d1, 0.f), h == 2 ? wv.z : wv.w, s0, s1);
+                        }
+                    }
                 }
-                const int kb = 2 * pr + ch;                     // this warp's key block of the pair
+                const int kb = 2 * pr + kb_in_pair;             // this warp's key block of the pair
                 const int j = c * PF_CHUNK + kb;
                 if (j == qb_abs) {
                     // causal mask inside the diagonal tile: key t of the block is visible iff t <= q
 #pragma unroll
-                    for (int i = 0; i < 64; ++i)
-                        if (i > q_in_blk) S[i] = -INFINITY;
+                    for (int i = 0; i < EC; ++i)
+                        if (c_in_blk + i > q_in_blk) S[i] = -INFINITY;
                 }
                 const bool live = kb < nk && j <= qb_abs && q_exists;   // warp-uniform: Tq is a multiple of 64, a warp's rows share a block
                 if (!a.fine) {
                     float mx = -INFINITY;
 #pragma unroll
-                    for (int i = 0; i < 64; i += 2) mx = fmax3(mx, S[i], S[i + 1]);
+                    for (int i = 0; i < EC; i += 2) mx = fmax3(mx, S[i], S[i + 1]);
                     if (live) {
                         const uint32_t key = __reduce_max_sync(0xffffffffu, f32_order_key(mx));
                         if (lane == 0) atomicMax(&s_max[(kb * 4) * 2 + qbl], key);
@@ -288,13 +372,13 @@ __global__ void __launch_bounds__(PF_THREADS, 1) score_prefill_kernel(const __gr
                 } else {
                     // 16-token blocks (f3): one maximum per quarter of the 64-key block
 #pragma unroll
-                    for (int q4 = 0; q4 < 4; ++q4) {
+                    for (int q4 = 0; q4 < EC / 16; ++q4) {
                         float mx = -INFINITY;
 #pragma unroll
                         for (int i = 0; i < 16; i += 2) mx = fmax3(mx, S[q4 * 16 + i], S[q4 * 16 + i + 1]);
                         if (live) {
                             const uint32_t key = __reduce_max_sync(0xffffffffu, f32_order_key(mx));
-                            if (lane == 0) atomicMax(&s_max[(kb * 4 + q4) * 2 + qbl], key);
+                            if (lane == 0) atomicMax(&s_max[(kb * 4 + (c_in_blk >> 4) + q4) * 2 + qbl], key);
                         }
                     }
                 }
@@ -313,7 +397,6 @@ __global__ void __launch_bounds__(PF_THREADS, 1) score_prefill_kernel(const __gr
                     a.scores[((int64_t)b * a.n_qb + qblk) * a.nb_stride + j * nq4 + q4] = f32_from_order_key(key);
             }
             asm volatile("bar.sync 1, %0;" :: "n"(PF_EPI_WARPS * 32) : "memory");   // re-armed before the next item's maxima
-            ++n_item;
         }
     }
 
@@ -362,6 +445,9 @@ static spot_status score_prefill_d(const spot_select_params* p, float* scores, i
     a.B = p->B; a.Tq = p->Tq; a.n_qb = p->Tq / 64; a.n_qt = (a.n_qb + 1) / 2;
     a.qb_start = p->q_start / 64;
     a.fine = p->blk == 16;
+#ifdef SPOT_TRACE
+    a.trace = g_pf_trace;
+#endif
     const int n_vis_max = a.qb_start + a.n_qb;
     a.n_chunks_max = (n_vis_max + PF_CHUNK - 1) / PF_CHUNK;
     const int64_t total = (int64_t)a.B * a.n_chunks_max * a.n_qt;
@@ -380,7 +466,7 @@ static spot_status score_prefill_d(const spot_select_params* p, float* scores, i
         const uint64_t dims[4] = {(uint64_t)PF_D, (uint64_t)p->cache_stride_tokens, (uint64_t)PLANES, (uint64_t)p->B};
         const uint64_t strides[3] = {row_bytes, (uint64_t)PF_D * 2, (uint64_t)p->cache_stride_tokens * row_bytes};
         // a pair of key blocks: every head's planes, or (HB = 256) one head's two planes
-        const uint32_t box[4] = {(uint32_t)PF_D, (uint32_t)PF_N, (uint32_t)(Cfg::PER_HEAD ? Cfg::HEAD_PLANES : PLANES), 1u};
+        const uint32_t box[4] = {(uint32_t)PF_D, (uint32_t)PF_N, (uint32_t)Cfg::STAGE_PLANES, 1u};
         if (!encode_tmap_bf16_sw128(&tm_k, p->sel_k, 4, dims, strides, box)) return SPOT_ERR_CUDA;
     }
     static unsigned long long smem_attr_done = 0;
@@ -406,3 +492,7 @@ spot_status score_prefill(const spot_select_params* p, float* scores, int nb_str
 }
 
 }  // namespace spot
+
+#ifdef SPOT_TRACE
+extern "C" void spot_debug_set_pf_trace(void* dev_buf) { spot::g_pf_trace = (long long*)dev_buf; }
+#endif

@@ -470,16 +470,19 @@ def test_q_fmt_argument_errors(torch_cuda):
     with pytest.raises(api.SpotError) as e:
         dp.select()
     assert "UNSUPPORTED" in str(e.value) or "INVALID_ARG" in str(e.value)
+    import torch
+    scores = torch.zeros((2, 4), dtype=torch.float32, device="cuda")
     sp = api.make_select_params(dp.sel_q, dp.w, dp.sel_k, "fp8_e4m3", 256, None, 0, 1, 128, wl.H_idx, wl.d_idx,
-                                q_start=0, blk=wl.blk, q_block=64, mode=wl.mode, p=wl.p)
+                                q_start=0, blk=wl.blk, q_block=64, mode=wl.mode, p=wl.p, block_scores=scores, nb_stride=4)
     sp.q_fmt = 77
     with pytest.raises(api.SpotError) as e:
-        api.spot_select_workspace_bytes(sp)
+        api.spot_score_blocks(sp)
     assert "INVALID_ARG" in str(e.value)
     # the decode form takes BF16 queries only
-    wd = make_prefill_workload(seed=6708, L=256, with_kv=False)
-    sp = api.make_select_params(dp.sel_q, dp.w, dp.sel_k, "fp8_e4m3", 256, None, 0, 1, 1, wd.H_idx, wd.d_idx,
-                                blk=wd.blk, q_block=1, q_fmt="fp8_e4m3", mode=wd.mode, p=wd.p)
+    sp = api.make_select_params(dp.sel_q, dp.w, dp.sel_k, "fp8_e4m3", 256, None, 0, 1, 1, wl.H_idx, wl.d_idx,
+                                blk=wl.blk, q_block=1, q_fmt="fp8_e4m3", mode=wl.mode, p=wl.p, block_scores=scores,
+                                nb_stride=4)
     with pytest.raises(api.SpotError) as e:
-        api.spot_select_workspace_bytes(sp)
+        api.spot_score_blocks(sp)
     assert "UNSUPPORTED" in str(e.value)
+    assert float(scores.abs().sum()) == 0.0
