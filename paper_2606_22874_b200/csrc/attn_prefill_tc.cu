@@ -180,13 +180,15 @@ __global__ void __launch_bounds__(TA_THREADS, 1) attn_prefill_tc_kernel(const __
         }
     } else if (warp == 1) {
         // ================================ MMA issuer ================================
-        if (lane == 0) {
+        // The whole warp runs this converged; one ELECTED lane issues (tc100.cuh, umma_*_elect): under `if (lane == 0)`
+        // every tcgen05.mma sat in an ELECT / BRA.U.ANY loop of its own and cost the lone thread 70-130 cycles.
+        {
             constexpr uint32_t idesc_pv = umma_idesc_bf16(128, 128) | UMMA_B_MN_MAJOR;
             int nv = 0;
             for (int it = 0; it < budget; ++it) nv += visible(block_of(it)) ? 1 : 0;
             const int np = (nv + GROUP - 1) / GROUP;     // iterations: tiles of up to 128 keys (the last may be short)
             auto keys_of = [&](int n) -> int { return min(GROUP, nv - n * GROUP) * blk; };   // keys of tile n: a multiple of 16
-            // One lone thread issues every MMA, with nobody to hide its instruction latencies: descriptors are built
+            // Descriptors are built
             // once and advanced by compile-time constants (the start-address field is the low 14 bits, in 16-byte
             // units), so each tcgen05.mma costs two integer adds, not a dozen dependent ones.
             const uint64_t qd[2] = {umma_desc_sw128(q_smem), umma_desc_sw128(q_smem + TA_Q_TILE)};
@@ -194,17 +196,17 @@ __global__ void __launch_bounds__(TA_THREADS, 1) attn_prefill_tc_kernel(const __
                 const uint32_t idesc = umma_idesc_bf16(128, nkeys);
 #pragma unroll
                 for (int kk = 0; kk < 8; ++kk)
-                    umma_bf16_ss(tbase + t * 128, qd[t] + (uint64_t)(((kk >> 2) * (128 * 128) + (kk & 3) * 32) >> 4),
+                    umma_bf16_ss_elect(tbase + t * 128, qd[t] + (uint64_t)(((kk >> 2) * (128 * 128) + (kk & 3) * 32) >> 4),
                                  kd + (uint64_t)(((kk >> 2) * (128 * 128) + (kk & 3) * 32) >> 4), idesc, kk > 0);
-                umma_commit(bar_s_full + 8 * t);
+                umma_commit_elect(bar_s_full + 8 * t);
             };
             auto pv = [&](int t, uint64_t vd, bool acc, int nkeys) {   // O_t += P_t V over nkeys keys: one k-step per 16 keys
 #pragma unroll
                 for (int kk = 0; kk < 8; ++kk)
                     if (kk * 16 < nkeys)
-                        umma_bf16_ts(tbase + 256 + t * 128, tbase + t * 128 + kk * 8, vd + (uint64_t)((kk * 2048) >> 4),
+                        umma_bf16_ts_elect(tbase + 256 + t * 128, tbase + t * 128 + kk * 8, vd + (uint64_t)((kk * 2048) >> 4),
                                      idesc_pv, acc || kk > 0);
-                umma_commit(bar_o_done + 8 * t);
+                umma_commit_elect(bar_o_done + 8 * t);
             };
             if (np > 0) {
                 mbar_wait(bar_q_full, 0);
@@ -233,7 +235,7 @@ __global__ void __launch_bounds__(TA_THREADS, 1) attn_prefill_tc_kernel(const __
                         pv(1, vd, n > 0, nk0);
                         if (more) qk(1, kd1, nk1);
                     }
-                    umma_commit(bar_kv_empty + 8 * s);                  // K(n), V(n) no longer read
+                    umma_commit_elect(bar_kv_empty + 8 * s);                  // K(n), V(n) no longer read
                 }
             }
         }
