@@ -25,7 +25,10 @@
 // TMEM: S_0 | S_1 | O_0 | O_1 = 128 + 128 + 128 + 128 columns (all 512).  Grid: (tile pair, query block heaviest-first,
 // KV head) with the KV head slowest, so the CTAs in flight share one head's K/V in L2 (DRAM reads 25 GB -> 0.8 GB).
 // History (cfg5, TFLOP/s): mma.sync 328 -> tcgen05 SS 789 -> fused FFMA 805 -> P in TMEM 826 -> hoisted descriptors
-// 887 -> head-slowest grid 982 -> 128 keys per iteration 1016 -> optimistic single-pass softmax 1069 -> no ordering barriers 1096.
+// 887 -> head-slowest grid 982 -> 128 keys per iteration 1016 -> optimistic single-pass softmax 1069 -> no ordering barriers 1096
+// -> converged issuer warp with an elected lane 1105.  (Round 2, measured and dropped: 2 / 3 / 4 of every 8 exponentials through a
+// Cody-Waite + cubic polynomial on the FMA / ALU pipes instead of MUFU.EX2: 1065 / 1039 / 993 -- the softmax warps are
+// bound by issue slots, not by the 16 MUFU lanes.)
 #include "common.cuh"
 #include "tc100.cuh"
 
@@ -55,7 +58,16 @@ struct TcAttnArgs {
     float scale_log2;
     uint16_t* out;               // [B][Tq][H_q][128]
     float* lse;                  // optional [B][Tq][H_q]
+#ifdef SPOT_TRACE
+    long long* trace;            // development builds only: [12 roles][512 iterations] clock64 of one CTA
+#endif
 };
+#ifdef SPOT_TRACE
+long long* g_ta_trace = nullptr;
+#define TA_STAMP(role, it) do { if (a.trace && blockIdx.x == 0 && blockIdx.z == 0 && (it) < 512) a.trace[(role) * 512 + (it)] = clock64(); } while (0)
+#else
+#define TA_STAMP(role, it) do { } while (0)
+#endif
 
 template <int BLK>       // key block size of the index lists: 64, or 16 (f3) -- a compile-time constant: the softmax warps are a
                          // co-bound of this kernel and the 64-token form must not pay for the per-16-key causal limits
@@ -226,14 +238,18 @@ __global__ void __launch_bounds__(TA_THREADS, 1) attn_prefill_tc_kernel(const __
                     mbar_wait(bar_v_full + 8 * s, (n / TA_STAGES) & 1);
                     if (more) mbar_wait(bar_k_full + 8 * s1, ((n + 1) / TA_STAGES) & 1);
                     mbar_wait(bar_p_full, n & 1);                       // P_0(n) written, S_0 consumed, O_0 rescaled
+                    if (lane == 0) TA_STAMP(0, n);
                     tc_fence_after();
                     pv(0, vd, n > 0, nk0);
                     if (more) qk(0, kd1, nk1);
+                    if (lane == 0) TA_STAMP(1, n);
                     if (two) {
                         mbar_wait(bar_p_full + 8, n & 1);
+                        if (lane == 0) TA_STAMP(2, n);
                         tc_fence_after();
                         pv(1, vd, n > 0, nk0);
                         if (more) qk(1, kd1, nk1);
+                        if (lane == 0) TA_STAMP(3, n);
                     }
                     umma_commit_elect(bar_kv_empty + 8 * s);                  // K(n), V(n) no longer read
                 }
@@ -283,6 +299,7 @@ __global__ void __launch_bounds__(TA_THREADS, 1) attn_prefill_tc_kernel(const __
                 }
                 auto lim_of = [&](int u) -> int { return (int)((lim_pk >> (8 * u)) & 0xffull) - 1; };
                 mbar_wait(bar_s_full + 8 * t, n & 1);
+                if (lq == 0 && lane == 0) TA_STAMP(4 + 4 * t, n);
                 tc_fence_after();
                 // Optimistic single pass: exp2 against the STALE max while the row max of this tile is being found (sm_scale
                 // > 0: max on the raw logits; scale and max-subtraction are one FFMA).  P = exp2(scale x - m) rounded to
@@ -335,6 +352,7 @@ __global__ void __launch_bounds__(TA_THREADS, 1) attn_prefill_tc_kernel(const __
                         }
                     }
                 }
+                if (lq == 0 && lane == 0) TA_STAMP(5 + 4 * t, n);
                 mx *= a.scale_log2;
                 const bool need = mx > m_used + TA_RESCALE_THRESHOLD;       // (true for a row's first visible key: m_used = -inf)
                 if (__any_sync(0xffffffffu, need)) {                         // warp-uniform: tcgen05.ld/st are collective
@@ -389,6 +407,7 @@ __global__ void __launch_bounds__(TA_THREADS, 1) attn_prefill_tc_kernel(const __
                 // P goes back to tensor memory over the start of S_t: columns 32 hf .. +31 hold the 64 keys of block hf
                 // (QK_t(n+1), which rewrites S_t, is issued after PV_t(n) and the tensor pipe runs them in order)
                 // (16 columns = 32 keys per store; a short tile stores only what PV will read)
+                if (lq == 0 && lane == 0) TA_STAMP(6 + 4 * t, n);
                 tmem_st16u(t_s, pk);
                 if (nkeys > 32) tmem_st16u(t_s + 16, pk + 16);
                 if (nkeys > 64) tmem_st16u(t_s + 32, pk + 32);
@@ -397,6 +416,7 @@ __global__ void __launch_bounds__(TA_THREADS, 1) attn_prefill_tc_kernel(const __
                 tmem_st_wait();
                 tc_fence_before();
                 mbar_arrive(bar_p_full + 8 * t);
+                if (lq == 0 && lane == 0) TA_STAMP(7 + 4 * t, n);
                 ++n;
             }
             // epilogue: O / l -> BF16
@@ -460,6 +480,9 @@ spot_status attn_prefill_tc(const spot_attn_params* p, cudaStream_t stream) {
     a.blk = p->blk;
     a.scale_log2 = p->sm_scale * 1.4426950408889634f;
     a.out = p->out; a.lse = p->lse;
+#ifdef SPOT_TRACE
+    a.trace = g_ta_trace;
+#endif
     CUtensorMap tm_q, tm_k, tm_v;
     // Q as (64 d, query, head, d-half, batch): a box of 64 queries x 2 heads x 2 halves lands as
     // [half][head][query][128 B] = [half][128 rows][128 B], row = head * 64 + query.
@@ -493,3 +516,7 @@ spot_status attn_prefill_tc(const spot_attn_params* p, cudaStream_t stream) {
 }
 
 }  // namespace spot
+
+#ifdef SPOT_TRACE
+extern "C" void spot_debug_set_ta_trace(void* dev_buf) { spot::g_ta_trace = (long long*)dev_buf; }
+#endif
