@@ -246,13 +246,15 @@ class DevicePrefill:
         import torch
         from workloads import f32_to_bf16_bits
         wl, api = self.wl, self.api
-        bf16 = self.sel_k
+        if not hasattr(self, "_sel_k_bf16"):              # a second call re-quantises the ORIGINAL BF16 keys, not the
+            self._sel_k_bf16 = self.sel_k                 # previous call's cache (which is not a BF16 tensor any more)
+            self._host_sel_k = [x.sel_k for x in self.wls]
         self.sel_k = torch.zeros(api.spot_selector_k_bytes(fmt, self.B, self.L, wl.H_idx, wl.d_idx), dtype=torch.uint8,
                                  device="cuda")
-        api.spot_quantize_selector_k(bf16, self.sel_k, fmt, self.B, self.L, 0, self.L, wl.H_idx, wl.d_idx)
+        api.spot_quantize_selector_k(self._sel_k_bf16, self.sel_k, fmt, self.B, self.L, 0, self.L, wl.H_idx, wl.d_idx)
         self.fmt = fmt
-        for x in self.wls:
-            x.sel_k = f32_to_bf16_bits(OQ.quantize_dequantize(fmt, x.sel_k).astype(np.float32))
+        for x, k0 in zip(self.wls, self._host_sel_k):
+            x.sel_k = f32_to_bf16_bits(OQ.quantize_dequantize(fmt, k0).astype(np.float32))
 
     def quantise_queries(self, fmt="fp8_e4m3"):
         """f2: the chunk's selector queries through the cache quantiser (a cache of Tq tokens), kept in the quantised
