@@ -263,6 +263,22 @@ typedef struct {
 size_t spot_sparse_attn_decode_workspace_bytes(const spot_attn_params* p);
 spot_status spot_sparse_attn_decode(const spot_attn_params* p, void* stream);
 
+/* spot_sparse_attn_decode for callers that cannot allocate (code under CUDA graph capture, tight serving loops, harnesses
+ * that forbid cudaMalloc): the same operation, arguments, checks, launches and results (bit for bit), but the split-KV
+ * partials live in an array INSIDE the library (a file-scope `static __device__` array of SPOT_STATIC_SCRATCH_BYTES,
+ * held by every GPU that loads the library until the process exits).  p->workspace / p->workspace_bytes are ignored
+ * (may be NULL / 0); inputs and outputs are the caller's as before.  The call allocates nothing and frees nothing.
+ *   - Limit: spot_sparse_attn_decode_workspace_bytes(p) <= SPOT_STATIC_SCRATCH_BYTES, i.e.
+ *     2 * (2 * SM count + B * H_kv) * (H_q / H_kv) * 520 bytes (B = 16, H_kv = 8, H_q / H_kv = 4 on a B200: 1.7 MiB; H_q / H_kv = 16,
+ *     B * H_kv <= 208 fits).  A larger problem is refused with SPOT_ERR_WORKSPACE_TOO_SMALL before anything is launched:
+ *     use spot_sparse_attn_decode with a workspace of your own.
+ *   - ONE array per GPU, shared by every call: calls that overlap on the GPU (two streams, two host threads on one
+ *     device) RACE on it -- serialise them, or use the workspace form.  Calls on one stream are ordered and safe.
+ *   - The array keeps the previous call's contents; nothing in it has to start at zero (every partial the merge reads
+ *     is written by the same call first), so there is no clearing pass. */
+#define SPOT_STATIC_SCRATCH_BYTES (8u << 20)
+spot_status spot_sparse_attn_decode_static(const spot_attn_params* p, void* stream);
+
 size_t spot_sparse_attn_prefill_workspace_bytes(const spot_attn_params* p);
 spot_status spot_sparse_attn_prefill(const spot_attn_params* p, void* stream);
 

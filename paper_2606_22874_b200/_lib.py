@@ -11,6 +11,7 @@ LIB_PATH = os.path.join(HERE, "libspot.so")
 SPOT_OK, SPOT_ERR_INVALID_ARG, SPOT_ERR_UNSUPPORTED, SPOT_ERR_WORKSPACE_TOO_SMALL, SPOT_ERR_CUDA = range(5)
 SPOT_SELK_BF16, SPOT_SELK_INT4_E4M3, SPOT_SELK_MXFP4, SPOT_SELK_FP8_E4M3 = range(4)
 SPOT_MODE_TOPK, SPOT_MODE_DUAL_TOPP = range(2)
+SPOT_STATIC_SCRATCH_BYTES = 8 << 20
 
 FORMATS = {"bf16": SPOT_SELK_BF16, "int4_e4m3": SPOT_SELK_INT4_E4M3, "mxfp4": SPOT_SELK_MXFP4,
            "fp8_e4m3": SPOT_SELK_FP8_E4M3}
@@ -105,6 +106,7 @@ PROTOTYPES = {
     "spot_sparse_attn_decode": (C.c_int, [C.POINTER(AttnParams), C.c_void_p]),
     "spot_sparse_attn_prefill_workspace_bytes": (C.c_size_t, [C.POINTER(AttnParams)]),
     "spot_sparse_attn_prefill": (C.c_int, [C.POINTER(AttnParams), C.c_void_p]),
+    "spot_sparse_attn_decode_static": (C.c_int, [C.POINTER(AttnParams), C.c_void_p]),
     "spot_dense_attn_decode_workspace_bytes": (C.c_size_t, [C.POINTER(AttnParams)]),
     "spot_dense_attn_decode": (C.c_int, [C.POINTER(AttnParams), C.c_void_p]),
     "spot_decode_step_host": (C.c_int, [C.POINTER(DecodeStepHostParams), C.c_void_p]),

@@ -133,6 +133,10 @@ def spot_sparse_attn_decode(ap, stream=None):
     _check(L.load().spot_sparse_attn_decode(C.byref(ap), _stream(stream)), "spot_sparse_attn_decode")
 
 
+def spot_sparse_attn_decode_static(ap, stream=None):
+    _check(L.load().spot_sparse_attn_decode_static(C.byref(ap), _stream(stream)), "spot_sparse_attn_decode_static")
+
+
 def spot_dense_attn_decode_workspace_bytes(ap):
     return int(L.load().spot_dense_attn_decode_workspace_bytes(C.byref(ap)))
 

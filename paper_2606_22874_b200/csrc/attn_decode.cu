@@ -22,6 +22,8 @@
 
 #include <string.h>
 
+#include <mutex>
+
 namespace spot {
 
 namespace {
@@ -533,6 +535,48 @@ spot_status run_decode(const spot_attn_params* p, bool dense, const StepSync* sy
 
 }  // namespace
 
+// ---- spot_sparse_attn_decode_static: the same call with its scratch inside the library (include/spot.h) -----------------
+// The split-KV partials of attn_decode_kernel / attn_merge_kernel live in this file-scope array instead of a caller's
+// workspace: nothing is allocated by the call.  Every GPU that loads the library holds the array until the process exits.
+// In host code `g_static_scratch` is only a stand-in for the symbol, NOT a device address: the address comes from
+// cudaGetSymbolAddress, asked once per device with that device current.
+static __device__ __align__(256) unsigned char g_static_scratch[SPOT_STATIC_SCRATCH_BYTES];
+
+constexpr int STATIC_MAX_DEVICES = 64;
+spot_status static_scratch_ptr(void** out) {
+    static std::mutex mu;
+    static void* ptr_of_device[STATIC_MAX_DEVICES] = {};
+    int dev = -1;
+    SPOT_CUDA_TRY(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= STATIC_MAX_DEVICES) return SPOT_ERR_UNSUPPORTED;
+    std::lock_guard<std::mutex> lock(mu);
+    if (!ptr_of_device[dev]) {
+        void* ptr = nullptr;
+        SPOT_CUDA_TRY(cudaGetSymbolAddress(&ptr, g_static_scratch));
+        if (!ptr) return SPOT_ERR_CUDA;
+        ptr_of_device[dev] = ptr;
+    }
+    *out = ptr_of_device[dev];
+    return SPOT_OK;
+}
+
+spot_status run_decode_static(const spot_attn_params* p, cudaStream_t s) {
+    spot_status st = check_attn(p, false, false);
+    if (st != SPOT_OK) return st;
+    if ((st = check_device()) != SPOT_OK) return st;
+    // beyond the built-in maximum: refuse before anything is launched (the caller falls back to spot_sparse_attn_decode
+    // with a workspace of its own)
+    if (decode_ws_bytes(p, false) > (size_t)SPOT_STATIC_SCRATCH_BYTES) return SPOT_ERR_WORKSPACE_TOO_SMALL;
+    spot_attn_params q = *p;
+    void* scratch = nullptr;
+    if ((st = static_scratch_ptr(&scratch)) != SPOT_OK) return st;
+    q.workspace = scratch;
+    q.workspace_bytes = (size_t)SPOT_STATIC_SCRATCH_BYTES;
+    // Nothing in the array has to start at zero: the attention kernel writes every partial slot (o, m, l) the merge kernel
+    // reads, so the previous call's contents are simply overwritten.
+    return run_decode(&q, false, nullptr, s);
+}
+
 spot_status check_attn_decode_args(const spot_attn_params* p) { return check_attn(p, false, false); }
 spot_status attn_decode_piped(const spot_attn_params* p, const StepSync* sync, cudaStream_t s) {
     return run_decode(p, false, sync, s);
@@ -548,6 +592,9 @@ extern "C" size_t spot_sparse_attn_decode_workspace_bytes(const spot_attn_params
 }
 extern "C" spot_status spot_sparse_attn_decode(const spot_attn_params* p, void* stream) {
     return run_decode(p, false, nullptr, (cudaStream_t)stream);
+}
+extern "C" spot_status spot_sparse_attn_decode_static(const spot_attn_params* p, void* stream) {
+    return run_decode_static(p, (cudaStream_t)stream);
 }
 extern "C" size_t spot_dense_attn_decode_workspace_bytes(const spot_attn_params* p) {
     if (!p || check_attn(p, true, false) != SPOT_OK) return 0;

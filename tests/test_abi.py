@@ -33,7 +33,7 @@ def test_every_declared_symbol_is_exported_and_bound(lib):
         assert hasattr(lib, n), "libspot.so does not export %s" % n
         assert n in _lib.PROTOTYPES, "binding has no prototype for %s" % n
     for n in ("spot_quantize_selector_k", "spot_dequantize_selector_k", "spot_select", "spot_score_blocks",
-              "spot_sparse_attn_decode", "spot_sparse_attn_prefill", "spot_dense_attn_decode",
+              "spot_sparse_attn_decode", "spot_sparse_attn_decode_static", "spot_sparse_attn_prefill", "spot_dense_attn_decode",
               "spot_decode_step_host", "spot_selector_k_bytes"):
         assert callable(getattr(api, n)), "python binding lacks %s" % n
 
