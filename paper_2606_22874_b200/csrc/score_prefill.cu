@@ -2,8 +2,8 @@
 //   s_bar[i,j] = max_{q in i} max_{t in j, t <= q}  sum_h w_h[q] ReLU(q^I_h[q] . k^I_{h,t}).
 //
 // This IS a dense contraction (4 heads x [Tq x 64] x [64 x L_visible]), so it runs on the 5th-gen tensor cores:
-//   * work item = (128-query tile = two query blocks, chunk of up to CHUNK key blocks); items are dealt round-robin
-//     to one persistent CTA per SM;
+//   * one persistent CTA per SM; the unit of work is a STEP = (128-query tile = two query blocks, PAIR of key blocks), and
+//     every CTA gets a contiguous range of the same number of steps (ItemWalk below);
 //   * warp 8 lane 0: TMA producer -- the query tile ([4 heads][128][64] BF16, 64 KiB) and a 2-stage ring of key-block
 //     PAIRS ([4 heads][128 keys][64], 64 KiB) land in 128-byte-swizzled shared memory through 4-D tensor maps;
 //   * warp 9 (converged, one elected lane issues): tcgen05.mma with M = 128 queries, N = 128 keys (two key blocks), K = 16: four k-steps per
@@ -90,8 +90,8 @@ struct PrefillScoreArgs {
     int nb_stride;
     int B, Tq, n_qb, n_qt;    // query blocks / query tiles per sequence
     int qb_start;             // q_start / 64
-    int n_chunks_max;
-    int total_ids;
+    int64_t total_steps;      // B * steps_per_seq (ItemWalk)
+    int64_t steps_per_seq;
     int fine;                 // blk == 16 (f3): four scores per 64-key block, one per 16-token quarter
 #ifdef SPOT_TRACE
     long long* trace;         // development builds only: [6 roles][2048 events] clock64 of CTA 5
@@ -111,18 +111,64 @@ __device__ __forceinline__ float f32_from_order_key(uint32_t k) {
     return __uint_as_float((k & 0x80000000u) ? (k & 0x7fffffffu) : ~k);
 }
 
-// id -> (b, chunk c, tile m); false when the chunk lies beyond the tile's causal range
-__device__ __forceinline__ bool decode_item(const PrefillScoreArgs& a, int id, int& b, int& c, int& m, int& nk) {
-    const int per_b = a.n_chunks_max * a.n_qt;
-    b = id / per_b;
-    const int rem = id - b * per_b;
-    c = rem / a.n_qt;
-    m = rem - c * a.n_qt;
-    const int last_qb = min(2 * m + 1, a.n_qb - 1);        // last existing query block of the tile
-    const int n_vis = a.qb_start + last_qb + 1;            // key blocks the tile can see
-    nk = min(PF_CHUNK, n_vis - c * PF_CHUNK);
-    return nk > 0;
-}
+// ---- work distribution -------------------------------------------------------------------------------------------
+// A STEP is one key-block pair of one 128-query tile (16 MMAs, one pass of the epilogue); tile m of a sequence has
+// steps(m) = ceil(visible key blocks / 2) of them.  All steps, in (sequence, tile, pair) order, are cut into gridDim.x
+// contiguous ranges of equal length (+-1): every CTA does the same amount of work whatever the causal triangle looks like
+// (items of a whole 32-block chunk dealt round-robin left the SMs idle 5 % of the launch, ncu sm active vs elapsed), and
+// a CTA reloads the query tile only when its range crosses into the next tile.  A pair-step produces the complete maxima of
+// its (2 query blocks x 2 key blocks), so cutting a tile's key range between CTAs needs no reduction.
+// An ITEM is what the three roles hand to each other: up to 16 consecutive steps of one tile inside one 32-block chunk.
+struct Item {
+    int b, m, c;          // sequence, 128-query tile, 32-key-block chunk
+    int pr0, pr1;         // pairs [pr0, pr1) of the chunk
+    int nk;               // key blocks of the chunk the tile can see (1 .. PF_CHUNK)
+    bool new_tile;        // first item of this (b, m) in this CTA: the query tile has to be loaded
+};
+struct ItemWalk {
+    int b, m, p, left, steps_m;
+    bool fresh;
+    // steps of tile m: ceil(n_vis / 2), n_vis = qb_start + (last query block of the tile) + 1
+    static __device__ __forceinline__ int steps_of(const PrefillScoreArgs& a, int m) {
+        return (a.qb_start + min(2 * m + 1, a.n_qb - 1) + 2) >> 1;
+    }
+    // steps of tiles 0 .. m-1 (m <= n_qt - 1: all of them have both query blocks): sum of (m' + h), h = (qb_start + 3) / 2
+    static __device__ __forceinline__ int64_t steps_before(const PrefillScoreArgs& a, int m) {
+        return (int64_t)m * (m - 1) / 2 + (int64_t)m * ((a.qb_start + 3) >> 1);
+    }
+    __device__ __forceinline__ void init(const PrefillScoreArgs& a) {
+        const int64_t lo = a.total_steps * blockIdx.x / gridDim.x, hi = a.total_steps * (blockIdx.x + 1) / gridDim.x;
+        left = (int)(hi - lo);
+        b = (int)(lo / a.steps_per_seq);
+        const int64_t r = lo - (int64_t)b * a.steps_per_seq;
+        int m_lo = 0, m_hi = a.n_qt - 1;                     // largest m with steps_before(m) <= r
+        while (m_lo < m_hi) {
+            const int mid = (m_lo + m_hi + 1) >> 1;
+            if (steps_before(a, mid) <= r) m_lo = mid; else m_hi = mid - 1;
+        }
+        m = m_lo;
+        p = (int)(r - steps_before(a, m));
+        steps_m = steps_of(a, m);
+        fresh = true;
+    }
+    __device__ __forceinline__ bool next(const PrefillScoreArgs& a, Item& it) {
+        if (left <= 0) return false;
+        constexpr int PPC = PF_CHUNK / 2;                     // pairs per chunk
+        it.b = b; it.m = m; it.c = p / PPC; it.pr0 = p - it.c * PPC;
+        const int n = min(min(PPC - it.pr0, steps_m - p), left);
+        it.pr1 = it.pr0 + n;
+        it.nk = min(PF_CHUNK, a.qb_start + min(2 * m + 1, a.n_qb - 1) + 1 - it.c * PF_CHUNK);
+        it.new_tile = fresh;
+        fresh = false;
+        p += n; left -= n;
+        if (p == steps_m) {
+            p = 0; fresh = true;
+            if (++m == a.n_qt) { m = 0; ++b; }
+            steps_m = steps_of(a, m);
+        }
+        return true;
+    }
+};
 
 // ring position of an accumulator: slot and the parity of its use
 struct AccPos {
@@ -188,17 +234,20 @@ __global__ void __launch_bounds__(PF_THREADS, 1) score_prefill_kernel(const __gr
     if (warp == PF_EPI_WARPS) {
         // ================================ TMA producer: the key ring ================================
         if (lane == 0) {
-            int n_item = 0, kp = 0;
-            for (int id = blockIdx.x; id < a.total_ids; id += gridDim.x) {
-                int b, c, m, nk;
-                if (!decode_item(a, id, b, c, m, nk)) continue;
-                mbar_wait(bar_q_empty, (n_item & 1) ^ 1);
-                mbar_arrive_expect_tx(bar_q_full, Q_TILE_BYTES);
-                tma_load_4d(q_smem, &tm_q, bar_q_full, 0, m * PF_M, 0, b);
-                ++n_item;
-                const int np = (nk + 1) >> 1;
+            int n_tile = 0, kp = 0;
+            ItemWalk walk;
+            walk.init(a);
+            Item it;
+            while (walk.next(a, it)) {
+                const int b = it.b, c = it.c;
+                if (it.new_tile) {                             // (n_tile counts the query tiles this CTA has loaded)
+                    mbar_wait(bar_q_empty, (n_tile & 1) ^ 1);  // the previous tile's MMAs have completed
+                    mbar_arrive_expect_tx(bar_q_full, Q_TILE_BYTES);
+                    tma_load_4d(q_smem, &tm_q, bar_q_full, 0, it.m * PF_M, 0, b);
+                    ++n_tile;
+                }
                 // (kp counts ring slots: one per pair, or one per (pair, head) at HB = 256)
-                for (int pr = 0; pr < np; ++pr)
+                for (int pr = it.pr0; pr < it.pr1; ++pr)
                     for (int hh = 0; hh < (Cfg::PER_HEAD ? PF_H : 1); ++hh, ++kp) {
                         const int s = kp % PF_KSTAGES;
                         mbar_wait(bar_k_empty + 8 * s, ((kp / PF_KSTAGES) & 1) ^ 1);
@@ -213,11 +262,11 @@ __global__ void __launch_bounds__(PF_THREADS, 1) score_prefill_kernel(const __gr
 #ifdef SPOT_TRACE
         if (lane == 1 && a.trace && blockIdx.x == 5) {          // observer: when does each key slot actually arrive?
             int kp = 0;
-            for (int id = blockIdx.x; id < a.total_ids; id += gridDim.x) {
-                int b, c, m, nk;
-                if (!decode_item(a, id, b, c, m, nk)) continue;
-                const int np = (nk + 1) >> 1;
-                for (int pr = 0; pr < np; ++pr)
+            ItemWalk walk;
+            walk.init(a);
+            Item it;
+            while (walk.next(a, it)) {
+                for (int pr = it.pr0; pr < it.pr1; ++pr)
                     for (int hh = 0; hh < (Cfg::PER_HEAD ? PF_H : 1); ++hh, ++kp) {
                         const int s = kp % PF_KSTAGES;
                         mbar_wait(bar_k_full + 8 * s, (kp / PF_KSTAGES) & 1);
@@ -231,16 +280,21 @@ __global__ void __launch_bounds__(PF_THREADS, 1) score_prefill_kernel(const __gr
         // The whole warp runs this loop converged; one elected lane issues (tc100.cuh, umma_*_elect).
         {
             constexpr uint32_t idesc = F8 ? umma_idesc_e4m3(PF_M, PF_N) : umma_idesc_bf16(PF_M, PF_N);
-            int n_item = 0, kp = 0, acc = 0;
+            int n_tile = 0, kp = 0, acc = 0;
             AccPos ap{0, 0};
             const uint64_t qd = umma_desc_sw128(q_smem);
-            for (int id = blockIdx.x; id < a.total_ids; id += gridDim.x) {
-                int b, c, m, nk;
-                if (!decode_item(a, id, b, c, m, nk)) continue;
-                mbar_wait(bar_q_full, n_item & 1);             // the item's query tile has landed
-                tc_fence_after();
-                const int np = (nk + 1) >> 1;
-                for (int pr = 0; pr < np; ++pr) {
+            ItemWalk walk;
+            walk.init(a);
+            Item it;
+            while (walk.next(a, it)) {
+                if (it.new_tile) {
+                    // every MMA issued so far read the previous query tile: when they have completed, its buffer is free
+                    if (n_tile > 0) umma_commit_elect(bar_q_empty);
+                    mbar_wait(bar_q_full, n_tile & 1);         // this tile's queries have landed
+                    tc_fence_after();
+                    ++n_tile;
+                }
+                for (int pr = it.pr0; pr < it.pr1; ++pr) {
                     int s = 0;
                     uint64_t kd = 0;                           // descriptor of the slot's first byte
                     if constexpr (!Cfg::PER_HEAD) {
@@ -276,8 +330,6 @@ __global__ void __launch_bounds__(PF_THREADS, 1) score_prefill_kernel(const __gr
                     }
                     if constexpr (!Cfg::PER_HEAD) umma_commit_elect(bar_k_empty + 8 * s);   // slot free once these MMAs have read it
                 }
-                umma_commit_elect(bar_q_empty);
-                ++n_item;
             }
         }
     } else {
@@ -299,9 +351,11 @@ __global__ void __launch_bounds__(PF_THREADS, 1) score_prefill_kernel(const __gr
         const uint32_t t_lane = t_row + col0;
         int pc = 0;
         AccPos ap{0, 0};                          // the accumulator whose load is in flight / comes next
-        for (int id = blockIdx.x; id < a.total_ids; id += gridDim.x) {
-            int b, c, m, nk;
-            if (!decode_item(a, id, b, c, m, nk)) continue;
+        ItemWalk walk;
+        walk.init(a);
+        Item it;
+        while (walk.next(a, it)) {
+            const int b = it.b, c = it.c, m = it.m, nk = it.nk;
             const int q_local = m * PF_M + row;                 // query index inside the chunk of Tq queries
             const bool q_exists = q_local < a.Tq;
             float4 wv = make_float4(0.f, 0.f, 0.f, 0.f);
@@ -309,12 +363,11 @@ __global__ void __launch_bounds__(PF_THREADS, 1) score_prefill_kernel(const __gr
             const float wh0 = 0.5f * wv.x, wh1 = 0.5f * wv.y;   // heads 0-1: (w/2)(d + |d|)
             const int qb_abs = a.qb_start + 2 * m + qbl;        // this row's (absolute) query block = its diagonal
             const int q_in_blk = row & 63;
-            const int np = (nk + 1) >> 1;
             float buf[2][32];
             mbar_wait(bar_t_full + 8 * ap.slot, ap.par);
             tc_fence_after();
             tmem_ld32(t_lane + ap.slot * PF_N, buf[0]);
-            for (int pr = 0; pr < np; ++pr, ++pc) {
+            for (int pr = it.pr0; pr < it.pr1; ++pr, ++pc) {
                 float S[EC];
 #pragma unroll
                 for (int u = 0; u < NU; ++u) {
@@ -328,7 +381,7 @@ __global__ void __launch_bounds__(PF_THREADS, 1) score_prefill_kernel(const __gr
                         if (warp == 0 && lane == 0) PF_STAMP(5, pc * 4 + h);
                         ap.next(NACC);
                     }
-                    if (u + 1 < NU || pr + 1 < np) {
+                    if (u + 1 < NU || pr + 1 < it.pr1) {
                         const int sb1 = (u + 1) % NSUB;
                         if (sb1 == 0) {                         // a new accumulator
                             mbar_wait(bar_t_full + 8 * ap.slot, ap.par);
@@ -386,8 +439,9 @@ __global__ void __launch_bounds__(PF_THREADS, 1) score_prefill_kernel(const __gr
             // item done: all epilogue warps meet, then the tile maxima go out and the buffer is re-armed
             asm volatile("bar.sync 1, %0;" :: "n"(PF_EPI_WARPS * 32) : "memory");
             const int nq4 = a.fine ? 4 : 1;
-            for (int e = threadIdx.x; e < nk * nq4 * 2; e += PF_EPI_WARPS * 32) {
-                const int qq = e & 1, q4 = (e >> 1) % nq4, kb = (e >> 1) / nq4;
+            const int kb_lo = 2 * it.pr0, kb_n = min(2 * it.pr1, nk) - kb_lo;      // the key blocks this item has scored
+            for (int e = threadIdx.x; e < kb_n * nq4 * 2; e += PF_EPI_WARPS * 32) {
+                const int qq = e & 1, q4 = (e >> 1) % nq4, kb = kb_lo + (e >> 1) / nq4;
                 const int qblk = 2 * m + qq;
                 const int j = c * PF_CHUNK + kb;
                 const int slot = (kb * 4 + q4) * 2 + qq;
@@ -448,11 +502,15 @@ static spot_status score_prefill_d(const spot_select_params* p, float* scores, i
 #ifdef SPOT_TRACE
     a.trace = g_pf_trace;
 #endif
-    const int n_vis_max = a.qb_start + a.n_qb;
-    a.n_chunks_max = (n_vis_max + PF_CHUNK - 1) / PF_CHUNK;
-    const int64_t total = (int64_t)a.B * a.n_chunks_max * a.n_qt;
-    if (total > 0x7fffffff) return SPOT_ERR_UNSUPPORTED;
-    a.total_ids = (int)total;
+    // steps (ItemWalk): tiles 0 .. n_qt-2 have m + h of them, h = (qb_start + 3) / 2; the last tile may hold one query block
+    {
+        const int64_t last = a.n_qt - 1, h = (a.qb_start + 3) >> 1;
+        const int64_t last_qb = (2 * last + 1 < a.n_qb - 1) ? 2 * last + 1 : a.n_qb - 1;
+        a.steps_per_seq = last * (last - 1) / 2 + last * h + ((a.qb_start + last_qb + 2) >> 1);
+        a.total_steps = a.steps_per_seq * a.B;
+    }
+    const int64_t total = a.total_steps;
+    if (total <= 0) return SPOT_ERR_INVALID_ARG;
 
     CUtensorMap tm_q, tm_k;
     const uint64_t row_bytes = (uint64_t)PLANES * 128;              // one token: PF_H heads x HB bytes = PLANES x 128 bytes
