@@ -915,7 +915,7 @@ def run_train(args):
                    "l2": "flushed by a 512 MiB read sweep before every timed step"},
         "losses": {"dense_kl_mean": float(dkl.mean()), "sparse_kl_mean": float(skl.mean())},
         "tokens_per_s": world * L / (ms * 1e-3),
-        "roofline": {"bound": "tensor", "kernel": "train_pass_kernel (mma.sync; both passes)", "achieved": achieved,
+        "roofline": {"bound": "tensor", "kernel": "the whole call: attn_prefill_tc_kernel<64, STATS> + student_pass1_kernel (pass 1), select, train_pass_kernel<2> (pass 2, mma.sync)", "achieved": achieved,
                      "peak": sustained, "unit": "TFLOP/s", "frac": achieved / sustained, "traffic": None,
                      "peak_source": peak_src + "; sustained figure: the two passes run for milliseconds",
                      "algorithmic_flops": flop},

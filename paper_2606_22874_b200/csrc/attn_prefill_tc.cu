@@ -32,6 +32,8 @@
 #include "common.cuh"
 #include "tc100.cuh"
 
+#include <string.h>
+
 namespace spot {
 
 namespace {
@@ -58,6 +60,7 @@ struct TcAttnArgs {
     float scale_log2;
     uint16_t* out;               // [B][Tq][H_q][128]
     float* lse;                  // optional [B][Tq][H_q]
+    float* lse2;                 // STATS form: [B][Tq][H_q] log2-domain log-sum-exp of the scaled logits
 #ifdef SPOT_TRACE
     long long* trace;            // development builds only: [12 roles][512 iterations] clock64 of one CTA
 #endif
@@ -69,8 +72,11 @@ long long* g_ta_trace = nullptr;
 #define TA_STAMP(role, it) do { } while (0)
 #endif
 
-template <int BLK>       // key block size of the index lists: 64, or 16 (f3) -- a compile-time constant: the softmax warps are a
-                         // co-bound of this kernel and the 64-token form must not pay for the per-16-key causal limits
+template <int BLK, bool STATS = false>
+                         // BLK: key block size of the index lists: 64, or 16 (f3) -- a compile-time constant: the softmax warps
+                         // are a co-bound of this kernel and the 64-token form must not pay for the per-16-key causal limits.
+                         // STATS (f4, train_kl.cu): only the softmax statistics -- the log-sum-exp of every (query, head) row,
+                         // log2 domain, to a.lse2 -- no V, no P, no PV product, no output: the teacher pass 1 of Eq. 1
 __global__ void __launch_bounds__(TA_THREADS, 1) attn_prefill_tc_kernel(const __grid_constant__ CUtensorMap tm_q,
                                                                         const __grid_constant__ CUtensorMap tm_k,
                                                                         const __grid_constant__ CUtensorMap tm_v,
@@ -180,13 +186,15 @@ __global__ void __launch_bounds__(TA_THREADS, 1) attn_prefill_tc_kernel(const __
                         for (int hf = 0; hf < 2; ++hf)
                             tma_load_5d(ks + hf * (128 * 128) + u * ent_bytes, &tm_k, bar_k_full + 8 * s, 0, tok[u], hf, hk,
                                         outer[u]);
-                mbar_arrive_expect_tx(bar_v_full + 8 * s, bytes);
+                if constexpr (!STATS) {
+                    mbar_arrive_expect_tx(bar_v_full + 8 * s, bytes);
 #pragma unroll
-                for (int u = 0; u < 8; ++u)
-                    if (u < ne)
-                        for (int hf = 0; hf < 2; ++hf)
-                            tma_load_5d(ks + TA_KV_TILE + hf * (128 * 128) + u * ent_bytes, &tm_v, bar_v_full + 8 * s, 0,
-                                        tok[u], hf, hk, outer[u]);
+                    for (int u = 0; u < 8; ++u)
+                        if (u < ne)
+                            for (int hf = 0; hf < 2; ++hf)
+                                tma_load_5d(ks + TA_KV_TILE + hf * (128 * 128) + u * ent_bytes, &tm_v, bar_v_full + 8 * s, 0,
+                                            tok[u], hf, hk, outer[u]);
+                }
                 ++n;
             }
         }
@@ -235,19 +243,19 @@ __global__ void __launch_bounds__(TA_THREADS, 1) attn_prefill_tc_kernel(const __
                     const uint64_t kd1 = umma_desc_sw128(kv_smem + s1 * 2 * TA_KV_TILE);
                     const bool more = n + 1 < np;
                     const int nk0 = keys_of(n), nk1 = more ? keys_of(n + 1) : 0;
-                    mbar_wait(bar_v_full + 8 * s, (n / TA_STAGES) & 1);
+                    if constexpr (!STATS) mbar_wait(bar_v_full + 8 * s, (n / TA_STAGES) & 1);
                     if (more) mbar_wait(bar_k_full + 8 * s1, ((n + 1) / TA_STAGES) & 1);
                     mbar_wait(bar_p_full, n & 1);                       // P_0(n) written, S_0 consumed, O_0 rescaled
                     if (lane == 0) TA_STAMP(0, n);
                     tc_fence_after();
-                    pv(0, vd, n > 0, nk0);
+                    if constexpr (!STATS) pv(0, vd, n > 0, nk0);
                     if (more) qk(0, kd1, nk1);
                     if (lane == 0) TA_STAMP(1, n);
                     if (two) {
                         mbar_wait(bar_p_full + 8, n & 1);
                         if (lane == 0) TA_STAMP(2, n);
                         tc_fence_after();
-                        pv(1, vd, n > 0, nk0);
+                        if constexpr (!STATS) pv(1, vd, n > 0, nk0);
                         if (more) qk(1, kd1, nk1);
                         if (lane == 0) TA_STAMP(3, n);
                     }
@@ -360,7 +368,7 @@ __global__ void __launch_bounds__(TA_THREADS, 1) attn_prefill_tc_kernel(const __
                     const float alpha = (m_used == -INFINITY) ? 0.f : fast_exp2(m_used - m_new);   // 1 when !need
                     l *= alpha;
                     m_used = m_new;
-                    if (n > 0) {
+                    if (!STATS && n > 0) {
                         mbar_wait(bar_o_done + 8 * t, (n - 1) & 1);          // PV(n-1) has landed in O_t
                         tc_fence_after();
 #pragma unroll
@@ -408,20 +416,26 @@ __global__ void __launch_bounds__(TA_THREADS, 1) attn_prefill_tc_kernel(const __
                 // (QK_t(n+1), which rewrites S_t, is issued after PV_t(n) and the tensor pipe runs them in order)
                 // (16 columns = 32 keys per store; a short tile stores only what PV will read)
                 if (lq == 0 && lane == 0) TA_STAMP(6 + 4 * t, n);
-                tmem_st16u(t_s, pk);
-                if (nkeys > 32) tmem_st16u(t_s + 16, pk + 16);
-                if (nkeys > 64) tmem_st16u(t_s + 32, pk + 32);
-                if (nkeys > 96) tmem_st16u(t_s + 48, pk + 48);
+                if constexpr (!STATS) {
+                    tmem_st16u(t_s, pk);
+                    if (nkeys > 32) tmem_st16u(t_s + 16, pk + 16);
+                    if (nkeys > 64) tmem_st16u(t_s + 32, pk + 32);
+                    if (nkeys > 96) tmem_st16u(t_s + 48, pk + 48);
+                    tmem_st_wait();
+                }
                 l += ps0 + ps1;
-                tmem_st_wait();
-                tc_fence_before();
+                tc_fence_before();                                   // (STATS: S_t has been read, the next QK^T may overwrite it)
                 mbar_arrive(bar_p_full + 8 * t);
                 if (lq == 0 && lane == 0) TA_STAMP(7 + 4 * t, n);
                 ++n;
             }
-            // epilogue: O / l -> BF16
             const int q_row = i * 64 + ql;
             const int h = hk * G + hg;
+            if constexpr (STATS) {
+                // log2-domain log-sum-exp of the row (every query sees at least its own key: l > 0)
+                if (live) a.lse2[((int64_t)b * a.Tq + q_row) * a.H_q + h] = l > 0.f ? m_used + log2f(l) : -INFINITY;
+            } else {
+            // epilogue: O / l -> BF16
             uint16_t* orow = a.out + (((int64_t)b * a.Tq + q_row) * a.H_q + h) * 128;
             if (n > 0) {
                 mbar_wait(bar_o_done + 8 * t, (n - 1) & 1);
@@ -451,6 +465,7 @@ __global__ void __launch_bounds__(TA_THREADS, 1) attn_prefill_tc_kernel(const __
             if (a.lse && live)
                 a.lse[((int64_t)b * a.Tq + q_row) * a.H_q + h] =
                     l > 0.f ? (m_used + log2f(l)) * 0.6931471805599453f : -INFINITY;
+            }
         }
     }
 
@@ -472,17 +487,20 @@ bool make_map(CUtensorMap* m, const void* base, uint64_t rows, uint64_t row_stri
 }  // namespace
 
 // Q [B][Tq][H_q][128]; K/V with element strides; see attn_prefill.cu for the argument checks (already done).
-spot_status attn_prefill_tc(const spot_attn_params* p, cudaStream_t stream) {
+// lse2 != nullptr: the STATS form (blk 64, no page table; p->v, p->out, p->lse are not used).
+static spot_status attn_prefill_tc_launch(const spot_attn_params* p, float* lse2, cudaStream_t stream) {
     TcAttnArgs a;
     a.indices = p->indices; a.budgets = p->budgets; a.cap = p->cap;
     a.Tq = p->Tq; a.n_qb = p->Tq / 64; a.H_q = p->H_q; a.H_kv = p->H_kv; a.G = p->H_q / p->H_kv;
     a.qb_start = p->q_start / 64;
     a.blk = p->blk;
     a.scale_log2 = p->sm_scale * 1.4426950408889634f;
-    a.out = p->out; a.lse = p->lse;
+    a.out = p->out; a.lse = p->lse; a.lse2 = lse2;
 #ifdef SPOT_TRACE
     a.trace = g_ta_trace;
 #endif
+    const bool stats = lse2 != nullptr;
+    if (stats && (p->blk != 64 || p->page_table)) return SPOT_ERR_UNSUPPORTED;
     CUtensorMap tm_q, tm_k, tm_v;
     // Q as (64 d, query, head, d-half, batch): a box of 64 queries x 2 heads x 2 halves lands as
     // [half][head][query][128 B] = [half][128 rows][128 B], row = head * 64 + query.
@@ -500,12 +518,13 @@ spot_status attn_prefill_tc(const spot_attn_params* p, cudaStream_t stream) {
     if (!make_map(&tm_k, p->k, n_tok, (uint64_t)p->kv_stride_token, (uint64_t)p->H_kv, (uint64_t)p->kv_stride_head,
                   n_outer, (uint64_t)p->kv_stride_batch, (uint32_t)p->blk, 1))
         return SPOT_ERR_CUDA;
-    if (!make_map(&tm_v, p->v, n_tok, (uint64_t)p->kv_stride_token, (uint64_t)p->H_kv, (uint64_t)p->kv_stride_head,
+    if (!make_map(&tm_v, stats ? p->k : p->v, n_tok, (uint64_t)p->kv_stride_token, (uint64_t)p->H_kv, (uint64_t)p->kv_stride_head,
                   n_outer, (uint64_t)p->kv_stride_batch, (uint32_t)p->blk, 1))
         return SPOT_ERR_CUDA;
-    static unsigned long long smem_attr_done[2] = {0, 0};
-    auto kernel = p->blk == 16 ? attn_prefill_tc_kernel<16> : attn_prefill_tc_kernel<64>;
-    SPOT_CUDA_TRY(set_max_smem_once(kernel, (int)TA_SMEM_BYTES, smem_attr_done[p->blk == 16]));
+    static unsigned long long smem_attr_done[3] = {0, 0, 0};
+    auto kernel = stats ? attn_prefill_tc_kernel<64, true>
+                        : (p->blk == 16 ? attn_prefill_tc_kernel<16, false> : attn_prefill_tc_kernel<64, false>);
+    SPOT_CUDA_TRY(set_max_smem_once(kernel, (int)TA_SMEM_BYTES, smem_attr_done[stats ? 2 : (p->blk == 16)]));
     const int n_mt = (a.G * 64 + 127) / 128;
     a.n_pairs = (n_mt + 1) / 2;
     a.n_rows = p->B * a.n_qb;
@@ -513,6 +532,21 @@ spot_status attn_prefill_tc(const spot_attn_params* p, cudaStream_t stream) {
     dim3 grid((unsigned)(a.n_pairs * a.n_rows), 1u, (unsigned)p->H_kv);
     SPOT_CUDA_TRY(launch_pdl(kernel, grid, dim3(TA_THREADS), (size_t)TA_SMEM_BYTES, stream, tm_q, tm_k, tm_v, a));
     return SPOT_OK;
+}
+
+spot_status attn_prefill_tc(const spot_attn_params* p, cudaStream_t stream) { return attn_prefill_tc_launch(p, nullptr, stream); }
+
+// f4 (train_kl.cu): lse2[q][h] = log2 sum_{t <= q} 2^(scale_log2 q_h . k_{g(h), t}) of ONE sequence of L tokens (L % 64 == 0),
+// dense causal -- pass 1 of the teacher distribution (Eq. 1) on the tensor cores.
+spot_status attn_prefill_stats(const uint16_t* q, const uint16_t* k, int64_t k_stride_token, int64_t k_stride_head, int L,
+                               int H_q, int H_kv, float sm_scale, float* lse2, cudaStream_t stream) {
+    if (L <= 0 || L % 64 != 0 || !lse2) return SPOT_ERR_INVALID_ARG;
+    spot_attn_params p;
+    memset(&p, 0, sizeof(p));
+    p.q = q; p.k = k; p.v = k;
+    p.kv_stride_batch = (int64_t)L * H_kv * 128; p.kv_stride_token = k_stride_token; p.kv_stride_head = k_stride_head;
+    p.B = 1; p.Tq = L; p.q_start = 0; p.H_q = H_q; p.H_kv = H_kv; p.D = 128; p.blk = 64; p.sm_scale = sm_scale;
+    return attn_prefill_tc_launch(&p, lse2, stream);
 }
 
 }  // namespace spot

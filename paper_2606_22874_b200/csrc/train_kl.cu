@@ -15,8 +15,11 @@
 // A CTA owns 32 / G queries (G = H_q / H_kv) and walks its visible keys in tiles of 32.  Warps 0-7: one KV head each,
 // rows of the MMA = (query, head of the group), query-major, so that the head sum of Eq. 1 is a shuffle over row lanes;
 // warp 8: the selector scores of the same tile.  Every warp streams its own operand through a private cp.async ring (as
-// in attn_decode.cu); mma.sync m16n8k16, fp32 accumulate.  (A dense contraction: a tcgen05 form -- S in TMEM, rows =
-// (head, query) as in attn_prefill_tc.cu -- is the next step; this first form is correctness and a measured baseline.)
+// in attn_decode.cu); mma.sync m16n8k16, fp32 accumulate.
+// Pass 1 on the tensor cores (round 2): when L is whole 64-query blocks the teacher's log-sum-exps come from the prefill
+// attention kernel in its statistics-only form (attn_prefill_tc.cu, tcgen05 / TMEM / TMA) and the student's part from
+// student_pass1_kernel below (21.6 -> 3.5 ms at L = 16K); train_pass_kernel<1> then serves ragged L only.  Pass 2 is still this
+// mma.sync form.
 #include "select_common.cuh"
 
 #include <string.h>
@@ -25,6 +28,8 @@ namespace spot {
 
 spot_status run_select(const spot_select_params* p, const float* scores, int nb_stride, int rows_per_seq, int max_nb,
                        const StepSync* sync, cudaStream_t s);                                   // select.cu
+spot_status attn_prefill_stats(const uint16_t* q, const uint16_t* k, int64_t k_stride_token, int64_t k_stride_head, int L,
+                               int H_q, int H_kv, float sm_scale, float* lse2, cudaStream_t stream);   // attn_prefill_tc.cu
 
 namespace {
 
@@ -413,6 +418,160 @@ __global__ void __launch_bounds__(TR_THREADS, 1) train_pass_kernel(TrainArgs a) 
     }
 }
 
+// ---- pass 1, the student's part alone (used when the teacher's statistics come from the tcgen05 kernel) -------------------
+// s_lse[q] = log sum_{t <= q} exp(s_s[q, t]) and the block maxima s_bar[q, b] of every query.  A CTA owns 64 consecutive queries,
+// one m16 tile per warp, and walks the visible keys in tiles of 64 that all four warps share: the selector key rows are loaded
+// once per CTA (cooperative cp.async ring) and used by 64 queries -- in train_pass_kernel<1> a single warp per CTA served 8
+// queries through a ring of its own and the pass took as long as the teacher's (19.5 ms of 21.6 at L = 16K).
+constexpr int SP_WARPS = 4;
+constexpr int SP_THREADS = SP_WARPS * 32;
+constexpr int SP_QPC = SP_WARPS * 16;
+constexpr int SP_KT = 64;
+
+__global__ void __launch_bounds__(SP_THREADS) student_pass1_kernel(TrainArgs a, int stages) {
+    extern __shared__ __align__(128) unsigned char smem[];
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int g = lane >> 2, c = lane & 3, mi = lane >> 3, r8 = lane & 7;
+    const int n_tiles_q = (a.L + SP_QPC - 1) / SP_QPC;
+    const int q0 = (n_tiles_q - 1 - (int)blockIdx.x) * SP_QPC;         // heaviest (latest) queries first
+    const int q_end = min(q0 + SP_QPC, a.L);
+    const int n_kt = (q_end + SP_KT - 1) / SP_KT;
+    const int srow_bytes = a.H_idx * a.d_idx * 2;
+    const int chunks = srow_bytes >> 4;
+    const int stage_bytes = SP_KT * srow_bytes;
+    const uint32_t ring = smem_u32(smem);
+    const uint32_t sQ = ring + stages * stage_bytes + warp * 16 * srow_bytes;   // this warp's 16 query rows
+    const int ks_sel = a.d_idx >> 4;
+    const int qw0 = q0 + warp * 16;                                     // the warp's first query
+    const int qa = qw0 + g, qb = qw0 + g + 8;
+    const bool va = qa < a.L, vb = qb < a.L;
+    float swt[4][2];
+#pragma unroll
+    for (int h = 0; h < 4; ++h) {
+        swt[h][0] = (va && h < a.H_idx) ? a.w[(int64_t)qa * a.H_idx + h] : 0.f;
+        swt[h][1] = (vb && h < a.H_idx) ? a.w[(int64_t)qb * a.H_idx + h] : 0.f;
+    }
+    for (int id = lane; id < 16 * chunks; id += 32) {
+        const int row = id / chunks, ch = id - row * chunks;
+        uint4 v = make_uint4(0u, 0u, 0u, 0u);
+        if (qw0 + row < a.L) v = *reinterpret_cast<const uint4*>(a.sel_q + (int64_t)(qw0 + row) * (a.H_idx * a.d_idx) + ch * 8);
+        asm volatile("st.shared.v4.u32 [%0], {%1,%2,%3,%4};" :: "r"(sQ + tr_sw(row, ch, srow_bytes)), "r"(v.x), "r"(v.y),
+                     "r"(v.z), "r"(v.w) : "memory");
+    }
+    __syncwarp();
+    float st_m[2] = {-INFINITY, -INFINITY}, st_l[2] = {0.f, 0.f}, bm[2] = {-INFINITY, -INFINITY};
+
+    auto issue = [&](int kt) {
+        if (kt < n_kt) {
+            const uint32_t stage = ring + (kt % stages) * stage_bytes;
+            for (int id = tid; id < SP_KT * chunks; id += SP_THREADS) {
+                const int row = id / chunks, ch = id - row * chunks;
+                const bool ok = kt * SP_KT + row < q_end;
+                cp_async16(stage + tr_sw(row, ch, srow_bytes),
+                           a.sel_k + (int64_t)(ok ? kt * SP_KT + row : 0) * (a.H_idx * a.d_idx) + ch * 8, ok);
+            }
+        }
+        cp_async_commit();
+    };
+    for (int i = 0; i < stages - 1; ++i) issue(i);
+    for (int kt = 0; kt < n_kt; ++kt) {
+        issue(kt + stages - 1);                 // (into the stage every warp left at the end of iteration kt - 1)
+        if (stages == 3) cp_async_wait<2>(); else cp_async_wait<1>();
+        __syncthreads();                        // tile kt has landed for every thread
+        const uint32_t stage = ring + (kt % stages) * stage_bytes;
+        // the warp's last query is qw0 + 15: tiles past it hold no visible key for this warp
+        if (kt * SP_KT <= min(qw0 + 15, a.L - 1)) {
+#pragma unroll 1
+            for (int sub = 0; sub < 2; ++sub) {
+                const int t0 = kt * SP_KT + sub * 32;
+                if (t0 > min(qw0 + 15, a.L - 1)) break;
+                const uint32_t sb = stage + sub * 32 * srow_bytes;
+                float sv[4][4];
+#pragma unroll
+                for (int nt = 0; nt < 4; ++nt) sv[nt][0] = sv[nt][1] = sv[nt][2] = sv[nt][3] = 0.f;
+#pragma unroll
+                for (int h = 0; h < 4; ++h) {
+                    if (h < a.H_idx) {
+                        float acc[4][4];
+#pragma unroll
+                        for (int nt = 0; nt < 4; ++nt) acc[nt][0] = acc[nt][1] = acc[nt][2] = acc[nt][3] = 0.f;
+#pragma unroll
+                        for (int ks = 0; ks < 8; ++ks) {
+                            if (ks < ks_sel) {
+                                const int ch0 = h * (a.d_idx >> 3) + 2 * ks;
+                                uint32_t a0, a1, a2, a3;
+                                ldmatrix_x4(a0, a1, a2, a3, sQ + tr_sw((mi & 1) * 8 + r8, ch0 + (mi >> 1), srow_bytes));
+#pragma unroll
+                                for (int half = 0; half < 2; ++half) {
+                                    uint32_t b0, b1, b2, b3;
+                                    ldmatrix_x4(b0, b1, b2, b3,
+                                                sb + tr_sw(half * 16 + (mi >> 1) * 8 + r8, ch0 + (mi & 1), srow_bytes));
+                                    mma_bf16_16816(acc[half * 2], a0, a1, a2, a3, b0, b1);
+                                    mma_bf16_16816(acc[half * 2 + 1], a0, a1, a2, a3, b2, b3);
+                                }
+                            }
+                        }
+#pragma unroll
+                        for (int nt = 0; nt < 4; ++nt) {
+                            sv[nt][0] = fmaf(swt[h][0], fmaxf(acc[nt][0], 0.f), sv[nt][0]);
+                            sv[nt][1] = fmaf(swt[h][0], fmaxf(acc[nt][1], 0.f), sv[nt][1]);
+                            sv[nt][2] = fmaf(swt[h][1], fmaxf(acc[nt][2], 0.f), sv[nt][2]);
+                            sv[nt][3] = fmaf(swt[h][1], fmaxf(acc[nt][3], 0.f), sv[nt][3]);
+                        }
+                    }
+                }
+#pragma unroll
+                for (int hf = 0; hf < 2; ++hf) {
+                    const int q = qw0 + g + 8 * hf;
+                    const bool rowok = q < a.L;
+                    // the row's last key tile: its open block is flushed there (keys past q are masked)
+                    const bool last_sub = t0 + 32 > q;
+#pragma unroll
+                    for (int nt = 0; nt < 4; ++nt) {
+                        const int key0 = t0 + nt * 8;
+                        float v0 = (rowok && key0 + c * 2 <= q) ? sv[nt][hf * 2] : -INFINITY;
+                        float v1 = (rowok && key0 + c * 2 + 1 <= q) ? sv[nt][hf * 2 + 1] : -INFINITY;
+                        const float mx = fmaxf(v0, v1), mn = fmaxf(st_m[hf], mx);
+                        if (mn > -INFINITY) {
+                            st_l[hf] = st_l[hf] * __expf(st_m[hf] - mn) + __expf(v0 - mn) + __expf(v1 - mn);
+                            st_m[hf] = mn;
+                        }
+                        bm[hf] = fmaxf(bm[hf], mx);
+                        if ((key0 + 8) % a.blk == 0 || (last_sub && nt == 3)) {
+                            float m = bm[hf];
+                            m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, 1));
+                            m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, 2));
+                            if (c == 0 && m > -INFINITY) a.blk_scores[(int64_t)q * a.nb_stride + key0 / a.blk] = m;
+                            bm[hf] = -INFINITY;
+                        }
+                    }
+                }
+            }
+        }
+        __syncthreads();                        // every warp has left the stage before the request after next refills it
+    }
+    cp_async_wait<0>();
+#pragma unroll
+    for (int hf = 0; hf < 2; ++hf) {
+        float m = st_m[hf], l = st_l[hf];
+#pragma unroll
+        for (int o = 1; o <= 2; o <<= 1) {
+            const float m2 = __shfl_xor_sync(0xffffffffu, m, o), l2 = __shfl_xor_sync(0xffffffffu, l, o);
+            const float M = fmaxf(m, m2);
+            if (M > -INFINITY) { l = l * __expf(m - M) + l2 * __expf(m2 - M); m = M; }
+        }
+        const int q = qw0 + g + 8 * hf;
+        if (c == 0 && q < a.L) a.s_lse[q] = m + __logf(l);
+    }
+}
+
+// dst = src * f (the teacher's log-sum-exp from the log2 domain to natural log)
+__global__ void scale_copy_kernel(const float* __restrict__ src, float* __restrict__ dst, float f, int64_t n) {
+    pdl_wait();
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) dst[i] = src[i] * f;
+}
+
 // row q of the selection sees q + 1 tokens
 __global__ void iota_len_kernel(int32_t* seq_len, int L) {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
@@ -518,8 +677,28 @@ extern "C" spot_status spot_train_kl(const spot_train_params* p, void* stream) {
     constexpr int smem_max = TR_TW * TR_STAGES * TR_KSTAGE + TR_STAGES * TR_KT * 1024 + 4 * TR_QMAX * TR_KT * 4 + 16 * 1024;
     SPOT_CUDA_TRY(set_max_smem_once(train_pass_kernel<1>, smem_max, done1));
     SPOT_CUDA_TRY(set_max_smem_once(train_pass_kernel<2>, smem_max, done2));
-    train_pass_kernel<1><<<grid, TR_THREADS, smem, s>>>(a);
-    SPOT_LAUNCH_CHECK();
+    // Pass 1.  The teacher's part (the log-sum-exp of every (query, head) row) is flash attention's softmax statistics: when
+    // the sequence is whole 64-query blocks it runs on the tcgen05 kernel of the prefill path in its statistics-only form
+    // (attn_prefill_tc.cu), and the student's part in a kernel of its own; otherwise both in train_pass_kernel<1>.
+    if (p->L % 64 == 0) {
+        if ((st = attn_prefill_stats(p->q, p->k, p->k_stride_token, p->k_stride_head, p->L, p->H_q, p->H_kv, p->sm_scale,
+                                     a.t_lse2, s)) != SPOT_OK)
+            return st;
+        if (p->teacher_lse) {
+            scale_copy_kernel<<<(unsigned)(((int64_t)p->L * p->H_q + 255) / 256), 256, 0, s>>>(
+                a.t_lse2, p->teacher_lse, 0.6931471805599453f, (int64_t)p->L * p->H_q);
+            SPOT_LAUNCH_CHECK();
+        }
+        const int srow = p->H_idx * p->d_idx * 2, stages = 2;
+        const int sp_smem = (stages * SP_KT + SP_QPC) * srow;
+        static unsigned long long done3 = 0;
+        SPOT_CUDA_TRY(set_max_smem_once(student_pass1_kernel, (2 * SP_KT + SP_QPC) * 1024, done3));
+        student_pass1_kernel<<<(p->L + SP_QPC - 1) / SP_QPC, SP_THREADS, sp_smem, s>>>(a, stages);
+        SPOT_LAUNCH_CHECK();
+    } else {
+        train_pass_kernel<1><<<grid, TR_THREADS, smem, s>>>(a);
+        SPOT_LAUNCH_CHECK();
+    }
     iota_len_kernel<<<(p->L + 255) / 256, 256, 0, s>>>(seq_len, p->L);
     SPOT_LAUNCH_CHECK();
     // Eq. 6 per query: the selection kernel in its decode form, one row per query

@@ -58,6 +58,11 @@ def run_train(torch, wl, top_k, sink=0, rec=0, want_lists=True):
     (96, 16, 8, 64, 16, 3, 0, 0),           # G = 2: sixteen queries per CTA
     (130, 32, 2, 64, 64, 2, 0, 0),          # G = 16, two KV heads (six teacher warps idle), 64-token blocks
     (257, 32, 8, 64, 32, 100, 0, 0),        # K >= every block: SparseKL = DenseKL
+    # whole 64-query blocks: the teacher's pass 1 runs on the tcgen05 statistics kernel (attn_prefill_tc.cu, STATS form)
+    (256, 32, 8, 64, 16, 4, 0, 0),          # G = 4
+    (192, 64, 8, 128, 16, 6, 1, 2),         # G = 8: two pairs of 128-row tiles per KV head
+    (128, 16, 8, 64, 16, 3, 0, 0),          # G = 2: one tile, its upper half idle
+    (320, 32, 2, 64, 64, 2, 0, 0),          # G = 16, two KV heads
 ])
 def test_train_reductions_match_oracle(torch_cuda, L, H_q, H_kv, d_idx, blk, top_k, sink, rec):
     wl = make_prefill_workload(seed=4200 + L, L=L, H_q=H_q, H_kv=H_kv, d_idx=d_idx, blk=blk, topic_span=32)
