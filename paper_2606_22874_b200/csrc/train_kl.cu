@@ -21,6 +21,7 @@
 // student_pass1_kernel below (21.6 -> 3.5 ms at L = 16K); train_pass_kernel<1> then serves ragged L only.  Pass 2 is still this
 // mma.sync form.
 #include "select_common.cuh"
+#include "tc100.cuh"
 
 #include <string.h>
 
@@ -565,6 +566,286 @@ __global__ void __launch_bounds__(SP_THREADS) student_pass1_kernel(TrainArgs a, 
     }
 }
 
+// sum over the 32 lanes of v[j] for every j, delivered to lane j (31 shuffles instead of 32 x 5): at each level a lane keeps
+// the half of its elements that its own bit selects and adds the partner's copy of that half
+__device__ __forceinline__ float warp_transpose_sum(float (&v)[32], int lane) {
+#pragma unroll
+    for (int off = 16; off >= 1; off >>= 1) {
+        const bool up = (lane & off) != 0;
+#pragma unroll
+        for (int k = 0; k < off; ++k) {
+            const float send = up ? v[k] : v[k + off];
+            const float keep = up ? v[k + off] : v[k];
+            v[k] = keep + __shfl_xor_sync(0xffffffffu, send, off);
+        }
+    }
+    return v[0];
+}
+
+// ---- pass 2 on the tensor cores (tcgen05 / TMEM / TMA) ----------------------------------------------------------------------
+// The element-level head sum of Eq. 1 decides the layout.  The products are computed TRANSPOSED: S^T = K Q^T, the 128 keys of a
+// tile are the M rows (TMEM lanes, one key per epilogue thread) and the (head of the group, query) pairs of a 64-query block the
+// N columns.  A thread then sees, for ITS key, the logits of every head and every query in its own registers: the sum over the
+// 32 heads is plain register arithmetic, head step after head step, and only the four KL sums of a query (over keys) cross
+// lanes -- 4 values per (query, 32 keys) through a transposing shuffle tree instead of 32 per (query, key).
+//   step      = one accumulator: a KV head's (up to 4 query heads x 64 queries) columns, or the student's 4 selector heads
+//   stage     = the two operands of a step in shared memory (96 KiB: [columns][128 d] + [128 keys][128 d]), TMA ring of 2
+//   TMEM      = two accumulators of 256 columns
+//   warp 0 TMA producer, warp 1 MMA issuer (converged, one elected lane), warp 2 TMEM allocation, warps 4-11 epilogue:
+//   lane quarter = warp & 3, query half = (warp - 4) >> 2 (32 queries each, so the running head sum is 32 registers).
+// One CTA per 64-query block; it walks the visible keys in tiles of 128.
+constexpr int P2_THREADS = 12 * 32;
+constexpr int P2_QB = 64;                        // queries per CTA
+constexpr int P2_KT = 128;                       // keys per tile
+constexpr uint32_t P2_A_BYTES = 128 * 256;       // K tile: [2 d-halves][128 keys][128 B]  (student: [4 planes][128 keys][128 B] = 64 KiB)
+constexpr uint32_t P2_STAGE = 96 * 1024;         // the larger operand (64 KiB) first, the smaller (32 KiB) behind it:
+constexpr uint32_t P2_BIG = 0, P2_SMALL = 64 * 1024;   // teacher: B = queries (big), A = keys; student: A = keys (big), B = queries
+constexpr uint32_t P2_SMEM_MISC = 16 * 1024;     // lse2 [32 heads][64] (8 KiB), w [4][64], s_lse [64], tile bits [2][64], sums, barriers
+constexpr uint32_t P2_OFF_W = 8192, P2_OFF_SLSE = 9216, P2_OFF_BITS = 9472, P2_OFF_SUM = 9984, P2_OFF_BARS = 14080,
+                   P2_OFF_TMEM = 14144;
+constexpr uint32_t P2_SMEM = 1024 + 2 * P2_STAGE + P2_SMEM_MISC;
+
+struct Pass2Args {
+    const float* t_lse2;         // [L][H_q] log2 domain
+    const float* s_lse;          // [L]
+    const float* w;              // [L][4]
+    const uint32_t* mask;        // [L][mask_stride]
+    int mask_stride;
+    int L, H_q, G, d_idx, blk;
+    int hps;                     // query heads per teacher step: min(G, 4)
+    int t_steps, s_steps;        // teacher steps (H_q / hps), student steps (d_idx / 64)
+    float scale_log2;
+    float* dense_kl;
+    float* sparse_kl;
+};
+
+__global__ void __launch_bounds__(P2_THREADS, 1) train_pass2_tc_kernel(const __grid_constant__ CUtensorMap tm_q,
+                                                                       const __grid_constant__ CUtensorMap tm_k,
+                                                                       const __grid_constant__ CUtensorMap tm_sq,
+                                                                       const __grid_constant__ CUtensorMap tm_sk,
+                                                                       const Pass2Args a) {
+    extern __shared__ unsigned char smem_raw[];
+    const uint32_t base = (smem_u32(smem_raw) + 1023u) & ~1023u;
+    unsigned char* smem = smem_raw + (base - smem_u32(smem_raw));
+    unsigned char* misc = smem + 2 * P2_STAGE;
+    const uint32_t misc_u32 = base + 2 * P2_STAGE;
+    float* s_lse2 = reinterpret_cast<float*>(misc);                    // [H_q <= 32][64]
+    float* s_w = reinterpret_cast<float*>(misc + P2_OFF_W);            // [4][64]
+    float* s_slse = reinterpret_cast<float*>(misc + P2_OFF_SLSE);      // [64]
+    uint32_t* s_bits = reinterpret_cast<uint32_t*>(misc + P2_OFF_BITS);   // [2][64] mask bits of the tile's blocks
+    float* s_sum = reinterpret_cast<float*>(misc + P2_OFF_SUM);        // [4 lane quarters][64 q][4 sums]
+    const uint32_t bars = misc_u32 + P2_OFF_BARS;
+    const uint32_t bar_full = bars;            // [2] stage landed
+    const uint32_t bar_empty = bars + 16;      // [2] stage read by its MMAs
+    const uint32_t bar_t_full = bars + 32;     // [2] accumulator complete
+    const uint32_t bar_t_empty = bars + 48;    // [2] accumulator read by the 8 epilogue warps
+    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(misc + P2_OFF_TMEM);
+
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int n_qb = a.L / P2_QB;
+    const int i = n_qb - 1 - (int)blockIdx.x;                          // heaviest (latest) query block first
+    const int q0 = i * P2_QB;
+    const int n_kt = (q0 + P2_QB + P2_KT - 1) / P2_KT;                 // key tiles: keys 0 .. q0 + 63
+    const int n_steps = a.t_steps + a.s_steps;
+
+    if (threadIdx.x == 0) {
+        for (int s = 0; s < 2; ++s) {
+            mbar_init(bar_full + 8 * s, 1);
+            mbar_init(bar_empty + 8 * s, 1);
+            mbar_init(bar_t_full + 8 * s, 1);
+            mbar_init(bar_t_empty + 8 * s, 8);
+        }
+        mbar_fence_init();
+        tma_prefetch_desc(&tm_q); tma_prefetch_desc(&tm_k); tma_prefetch_desc(&tm_sq); tma_prefetch_desc(&tm_sk);
+    }
+    if (warp == 2) tmem_alloc(misc_u32 + P2_OFF_TMEM, 512);
+    // the block's per-query constants: lse2 as [head][query] (a step reads 32 consecutive queries of one head), w as [h][q]
+    for (int e = threadIdx.x; e < a.H_q * P2_QB; e += P2_THREADS) {
+        const int q = e / a.H_q, h = e - q * a.H_q;
+        s_lse2[h * P2_QB + q] = a.t_lse2[(int64_t)(q0 + q) * a.H_q + h];
+    }
+    for (int e = threadIdx.x; e < 4 * P2_QB; e += P2_THREADS) {
+        const int q = e >> 2, h = e & 3;
+        s_w[h * P2_QB + q] = a.w[(int64_t)(q0 + q) * 4 + h];
+    }
+    for (int e = threadIdx.x; e < P2_QB; e += P2_THREADS) s_slse[e] = a.s_lse[q0 + e];
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+    const uint32_t tbase = *tmem_slot;
+
+    if (warp == 0) {
+        // ================================ TMA producer ================================
+        if (lane == 0) {
+            int n = 0;
+            for (int kt = 0; kt < n_kt; ++kt)
+                for (int st = 0; st < n_steps; ++st, ++n) {
+                    const int s = n & 1;
+                    mbar_wait(bar_empty + 8 * s, ((n >> 1) & 1) ^ 1);
+                    const uint32_t sb = base + s * P2_STAGE;
+                    if (st < a.t_steps) {
+                        const int head0 = st * a.hps, hk = head0 / a.G;
+                        mbar_arrive_expect_tx(bar_full + 8 * s, (uint32_t)a.hps * 64u * 256u + P2_A_BYTES);
+                        // B: [d-half][hps heads][64 queries][128 B]
+                        tma_load_5d(sb + P2_BIG, &tm_q, bar_full + 8 * s, 0, q0, head0, 0, 0);
+                        // A: [d-half][128 keys][128 B]
+                        tma_load_5d(sb + P2_SMALL, &tm_k, bar_full + 8 * s, 0, kt * P2_KT, 0, hk, 0);
+                    } else {
+                        // the student's planes (128 B = 64 selector dims of one token): step u holds planes 4u .. 4u + 3
+                        const int pl0 = (st - a.t_steps) * 4;
+                        mbar_arrive_expect_tx(bar_full + 8 * s, 4u * 64u * 128u + 4u * 128u * 128u);
+                        tma_load_4d(sb + P2_SMALL, &tm_sq, bar_full + 8 * s, 0, q0, pl0, 0);          // [4 planes][64 q][128 B]
+                        tma_load_4d(sb + P2_BIG, &tm_sk, bar_full + 8 * s, 0, kt * P2_KT, pl0, 0);  // [4 planes][128 keys][128 B]
+                    }
+                }
+        }
+    } else if (warp == 1) {
+        // ================================ MMA issuer (converged; one elected lane issues) ================================
+        int n = 0;
+        for (int kt = 0; kt < n_kt; ++kt)
+            for (int st = 0; st < n_steps; ++st, ++n) {
+                const int s = n & 1;
+                mbar_wait(bar_full + 8 * s, (n >> 1) & 1);
+                mbar_wait(bar_t_empty + 8 * s, ((n >> 1) & 1) ^ 1);    // (accumulator slot == stage slot)
+                tc_fence_after();
+                const uint32_t sb = base + s * P2_STAGE;
+                const uint32_t d_tmem = tbase + s * 256;
+                if (st < a.t_steps) {
+                    const int N = a.hps * 64;
+                    const uint32_t idesc = umma_idesc_bf16(128, N);
+                    const uint64_t ad = umma_desc_sw128(sb + P2_SMALL), bd = umma_desc_sw128(sb + P2_BIG);
+#pragma unroll
+                    for (int ks = 0; ks < 8; ++ks) {
+                        // k-step ks: d-half ks >> 2 (a plane of [rows][128 B]), 32 bytes (ks & 3) inside the 128-byte row
+                        const uint64_t ao = (uint64_t)(((ks >> 2) * (128 * 128) + (ks & 3) * 32) >> 4);
+                        const uint64_t bo = (uint64_t)(((ks >> 2) * (N * 128) + (ks & 3) * 32) >> 4);
+                        umma_bf16_ss_elect(d_tmem, ad + ao, bd + bo, idesc, ks > 0);
+                    }
+                } else {
+                    // student: selector head h of this step = planes ppl h .. ppl h + ppl - 1 (ppl = d_idx / 64), columns 64 h'
+                    const int ppl = a.d_idx >> 6, heads = 4 / ppl;
+                    const uint32_t idesc = umma_idesc_bf16(128, 64);
+                    for (int hh = 0; hh < heads; ++hh)
+                        for (int ks = 0; ks < 4 * ppl; ++ks) {
+                            const int plane = hh * ppl + (ks >> 2);
+                            const uint64_t ad = umma_desc_sw128(sb + P2_BIG + plane * (128 * 128) + (ks & 3) * 32);
+                            const uint64_t bd = umma_desc_sw128(sb + P2_SMALL + plane * (64 * 128) + (ks & 3) * 32);
+                            umma_bf16_ss_elect(d_tmem + hh * 64, ad, bd, idesc, ks > 0);
+                        }
+                }
+                umma_commit_elect(bar_t_full + 8 * s);
+                umma_commit_elect(bar_empty + 8 * s);
+            }
+    } else if (warp >= 4) {
+        // ================================ epilogue (warps 4 .. 11) ================================
+        const int lq = warp & 3, qh = (warp - 4) >> 2;
+        const int key_l = lq * 32 + lane;                              // this thread's key inside the tile = TMEM lane
+        const uint32_t t_lane = tbase + ((uint32_t)(lq * 32) << 16) + qh * 32;
+        const int et = threadIdx.x - 128;                              // 0 .. 255 among the epilogue threads
+        const float inv_h = 1.f / (float)a.H_q;
+        const int bpt = P2_KT / a.blk;                                 // blocks per key tile (8, 4 or 2)
+        float acc_d = 0.f, acc_a = 0.f, acc_b = 0.f, acc_c = 0.f;      // lane j: the sums of query qh * 32 + j over this warp's keys
+        int n = 0;
+        for (int kt = 0; kt < n_kt; ++kt) {
+            // the tile's mask bits of every query of the block: bit u = block kt * bpt + u is in S_q
+            if (et < P2_QB) {
+                const int b0 = kt * bpt;
+                const uint32_t wd = a.mask[(int64_t)(q0 + et) * a.mask_stride + (b0 >> 5)];
+                s_bits[(kt & 1) * P2_QB + et] = (wd >> (b0 & 31)) & ((1u << bpt) - 1u);
+            }
+            float pacc[32], ss[32];
+#pragma unroll
+            for (int j = 0; j < 32; ++j) { pacc[j] = 0.f; ss[j] = 0.f; }
+            for (int st = 0; st < n_steps; ++st, ++n) {
+                const int s = n & 1;
+                mbar_wait(bar_t_full + 8 * s, (n >> 1) & 1);
+                tc_fence_after();
+                const uint32_t ta = t_lane + s * 256;
+                if (st < a.t_steps) {
+                    for (int hh = 0; hh < a.hps; ++hh) {
+                        float x[32];
+                        tmem_ld32(ta + hh * 64, x);
+                        const float4* l4 = reinterpret_cast<const float4*>(s_lse2 + (st * a.hps + hh) * P2_QB + qh * 32);
+                        tmem_ld_wait32(x);
+#pragma unroll
+                        for (int j4 = 0; j4 < 8; ++j4) {
+                            const float4 l = l4[j4];                   // (every lane reads the same words: a broadcast)
+                            pacc[4 * j4 + 0] += fast_exp2(fmaf(x[4 * j4 + 0], a.scale_log2, -l.x));
+                            pacc[4 * j4 + 1] += fast_exp2(fmaf(x[4 * j4 + 1], a.scale_log2, -l.y));
+                            pacc[4 * j4 + 2] += fast_exp2(fmaf(x[4 * j4 + 2], a.scale_log2, -l.z));
+                            pacc[4 * j4 + 3] += fast_exp2(fmaf(x[4 * j4 + 3], a.scale_log2, -l.w));
+                        }
+                    }
+                } else {
+                    const int ppl = a.d_idx >> 6, heads = 4 / ppl, h0 = (st - a.t_steps) * heads;
+                    for (int hh = 0; hh < heads; ++hh) {
+                        float x[32];
+                        tmem_ld32(ta + hh * 64, x);
+                        const float4* w4 = reinterpret_cast<const float4*>(s_w + (h0 + hh) * P2_QB + qh * 32);
+                        tmem_ld_wait32(x);
+#pragma unroll
+                        for (int j4 = 0; j4 < 8; ++j4) {
+                            const float4 wv = w4[j4];
+                            ss[4 * j4 + 0] = fmaf(wv.x, fmaxf(x[4 * j4 + 0], 0.f), ss[4 * j4 + 0]);
+                            ss[4 * j4 + 1] = fmaf(wv.y, fmaxf(x[4 * j4 + 1], 0.f), ss[4 * j4 + 1]);
+                            ss[4 * j4 + 2] = fmaf(wv.z, fmaxf(x[4 * j4 + 2], 0.f), ss[4 * j4 + 2]);
+                            ss[4 * j4 + 3] = fmaf(wv.w, fmaxf(x[4 * j4 + 3], 0.f), ss[4 * j4 + 3]);
+                        }
+                    }
+                }
+                tc_fence_before();
+                __syncwarp();
+                if (lane == 0) mbar_arrive(bar_t_empty + 8 * s);
+            }
+            // ---- the tile's contributions to the four sums of each query (Eq. 3, Eq. 4; R36: 0 log 0 = 0)
+            asm volatile("bar.sync 1, 256;" ::: "memory");              // the tile's mask bits are in shared memory
+            const int t = kt * P2_KT + key_l;
+            const int blk_in_tile = key_l / a.blk;
+            float vd[32], va[32], vb[32], vc[32];
+#pragma unroll
+            for (int j = 0; j < 32; ++j) {
+                const int ql = qh * 32 + j, q = q0 + ql;
+                float d = 0.f, A = 0.f, B = 0.f, C = 0.f;
+                if (t <= q) {
+                    const float pt = pacc[j] * inv_h;
+                    const float lps = ss[j] - s_slse[ql];
+                    const bool in_s = (s_bits[(kt & 1) * P2_QB + ql] >> blk_in_tile) & 1u;
+                    if (in_s) B = __expf(lps);
+                    if (pt > 0.f) {
+                        const float term = pt * (__logf(pt) - lps);
+                        d = term;
+                        if (in_s) { A = pt; C = term; }
+                    }
+                }
+                vd[j] = d; va[j] = A; vb[j] = B; vc[j] = C;
+            }
+            acc_d += warp_transpose_sum(vd, lane);
+            acc_a += warp_transpose_sum(va, lane);
+            acc_b += warp_transpose_sum(vb, lane);
+            acc_c += warp_transpose_sum(vc, lane);
+        }
+        // ---- the four lane quarters (32 keys each of every tile) of a query half meet in shared memory
+        float* mine = s_sum + ((lq * P2_QB) + qh * 32 + lane) * 4;
+        mine[0] = acc_d; mine[1] = acc_a; mine[2] = acc_b; mine[3] = acc_c;
+        asm volatile("bar.sync 1, 256;" ::: "memory");
+        if (et < P2_QB) {
+            float d = 0.f, A = 0.f, B = 0.f, C = 0.f;
+#pragma unroll
+            for (int k = 0; k < 4; ++k) {
+                const float* v = s_sum + (k * P2_QB + et) * 4;
+                d += v[0]; A += v[1]; B += v[2]; C += v[3];
+            }
+            a.dense_kl[q0 + et] = d;
+            // Eq. 4: sum_S (p/A) log((p/A) / (s/B)) = C / A - log A + log B
+            a.sparse_kl[q0 + et] = A > 0.f ? C / A - __logf(A) + __logf(B) : 0.f;
+        }
+    }
+
+    tc_fence_before();
+    __syncthreads();
+    if (warp == 2) tmem_dealloc(tbase, 512);
+}
+
 // dst = src * f (the teacher's log-sum-exp from the log2 domain to natural log)
 __global__ void scale_copy_kernel(const float* __restrict__ src, float* __restrict__ dst, float f, int64_t n) {
     pdl_wait();
@@ -627,6 +908,53 @@ spot_status check_train(const spot_train_params* p) {
     if ((p->L + p->blk - 1) / p->blk > SEL_MAX_NB) return SPOT_ERR_UNSUPPORTED;
     if (p->indices && p->cap < ((p->L + p->blk - 1) / p->blk < p->top_k ? (p->L + p->blk - 1) / p->blk : p->top_k))
         return SPOT_ERR_INVALID_ARG;
+    return SPOT_OK;
+}
+
+
+// pass 2 on the tensor cores: L whole 64-query blocks, H_q <= 32, selector 4 x 64 or 4 x 128
+bool pass2_tc_supported(const spot_train_params* p) {
+    const int G = p->H_q / p->H_kv;
+    return p->L % 64 == 0 && p->H_q <= 32 && p->H_idx == 4 && (p->d_idx == 64 || p->d_idx == 128) &&
+           (G == 2 || G == 4 || G == 8 || G == 16) && (p->blk == 16 || p->blk == 32 || p->blk == 64);
+}
+
+spot_status launch_pass2_tc(const spot_train_params* p, const TrainArgs& t, cudaStream_t s) {
+    Pass2Args a;
+    memset(&a, 0, sizeof(a));
+    a.t_lse2 = t.t_lse2; a.s_lse = t.s_lse; a.w = p->w; a.mask = t.mask; a.mask_stride = t.mask_stride;
+    a.L = p->L; a.H_q = p->H_q; a.G = p->H_q / p->H_kv; a.d_idx = p->d_idx; a.blk = p->blk;
+    a.hps = a.G < 4 ? a.G : 4;
+    a.t_steps = p->H_q / a.hps; a.s_steps = p->d_idx / 64;
+    a.scale_log2 = t.scale_log2;
+    a.dense_kl = p->dense_kl; a.sparse_kl = p->sparse_kl;
+    CUtensorMap tm_q, tm_k, tm_sq, tm_sk;
+    {   // Q [L][H_q][128] as (64 d, query, head, d-half, 1): a box of 64 queries x hps heads x 2 halves lands as
+        // [half][head][query][128 B] = [half][hps * 64 columns][128 B]
+        const uint64_t dims[5] = {64, (uint64_t)p->L, (uint64_t)p->H_q, 2, 1};
+        const uint64_t strides[4] = {(uint64_t)p->H_q * 256, 256, 128, (uint64_t)p->L * p->H_q * 256};
+        const uint32_t box[5] = {64, 64, (uint32_t)a.hps, 2, 1};
+        if (!encode_tmap_bf16_sw128(&tm_q, p->q, 5, dims, strides, box)) return SPOT_ERR_CUDA;
+    }
+    {   // K as (64 d, token, d-half, KV head, 1): a box of 128 keys x 2 halves lands as [half][128 keys][128 B]
+        const uint64_t dims[5] = {64, (uint64_t)p->L, 2, (uint64_t)p->H_kv, 1};
+        const uint64_t strides[4] = {(uint64_t)p->k_stride_token * 2, 128, (uint64_t)p->k_stride_head * 2,
+                                     (uint64_t)p->L * p->H_kv * 256};
+        const uint32_t box[5] = {64, 128, 2, 1, 1};
+        if (!encode_tmap_bf16_sw128(&tm_k, p->k, 5, dims, strides, box)) return SPOT_ERR_CUDA;
+    }
+    const uint64_t planes = (uint64_t)4 * p->d_idx / 64, row_bytes = planes * 128;
+    {   // selector rows [L][4 x d_idx] as (64 elements = one 128-byte plane, token, plane, 1): four planes per box
+        const uint64_t dims[4] = {64, (uint64_t)p->L, planes, 1};
+        const uint64_t strides[3] = {row_bytes, 128, (uint64_t)p->L * row_bytes};
+        const uint32_t boxq[4] = {64, 64, 4, 1}, boxk[4] = {64, 128, 4, 1};
+        if (!encode_tmap_bf16_sw128(&tm_sq, p->sel_q, 4, dims, strides, boxq)) return SPOT_ERR_CUDA;
+        if (!encode_tmap_bf16_sw128(&tm_sk, p->sel_k, 4, dims, strides, boxk)) return SPOT_ERR_CUDA;
+    }
+    static unsigned long long done = 0;
+    SPOT_CUDA_TRY(set_max_smem_once(train_pass2_tc_kernel, (int)P2_SMEM, done));
+    train_pass2_tc_kernel<<<p->L / P2_QB, P2_THREADS, P2_SMEM, s>>>(tm_q, tm_k, tm_sq, tm_sk, a);
+    SPOT_LAUNCH_CHECK();
     return SPOT_OK;
 }
 
@@ -712,6 +1040,7 @@ extern "C" spot_status spot_train_kl(const spot_train_params* p, void* stream) {
     SPOT_CUDA_TRY(cudaMemsetAsync(mask, 0, (size_t)p->L * y.mask_stride * 4, s));
     list_to_mask_kernel<<<(p->L + 7) / 8, 256, 0, s>>>(indices, budgets, cap, mask, y.mask_stride, p->L);
     SPOT_LAUNCH_CHECK();
+    if (pass2_tc_supported(p)) return launch_pass2_tc(p, a, s);
     train_pass_kernel<2><<<grid, TR_THREADS, smem, s>>>(a);
     SPOT_LAUNCH_CHECK();
     return SPOT_OK;

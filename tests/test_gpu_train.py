@@ -63,6 +63,8 @@ def run_train(torch, wl, top_k, sink=0, rec=0, want_lists=True):
     (192, 64, 8, 128, 16, 6, 1, 2),         # G = 8: two pairs of 128-row tiles per KV head
     (128, 16, 8, 64, 16, 3, 0, 0),          # G = 2: one tile, its upper half idle
     (320, 32, 2, 64, 64, 2, 0, 0),          # G = 16, two KV heads
+    (192, 32, 8, 128, 16, 6, 1, 2),         # the paper's selector width on the tcgen05 pass 2 (two student steps)
+    (448, 32, 4, 64, 32, 5, 1, 1),          # G = 8 (two teacher steps per KV head), 32-token blocks, four key tiles
 ])
 def test_train_reductions_match_oracle(torch_cuda, L, H_q, H_kv, d_idx, blk, top_k, sink, rec):
     wl = make_prefill_workload(seed=4200 + L, L=L, H_q=H_q, H_kv=H_kv, d_idx=d_idx, blk=blk, topic_span=32)
