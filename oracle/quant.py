@@ -40,8 +40,10 @@ def selector_k_bytes(fmt, n_elements):
         return n_elements // 2 + n_elements // GROUP
     if fmt == "fp8_e4m3":                # f2: one E4M3 byte per element, no scale (the paper's "0.5x" variants)
         return n_elements
-    if fmt == "int4_scale16":            # the paper's 4.5 bit/elt accounting
+    if fmt in ("int4_scale16", "int4_bf16s"):   # the paper's 4.5 bit/elt accounting: 4-bit codes + a 16-bit group scale
         return n_elements // 2 + 2 * (n_elements // GROUP)
+    if fmt == "mxint8":                  # f2: INT8 codes + one E8M0 byte per group (8.25 bit/elt; R38)
+        return n_elements + n_elements // GROUP
     raise ValueError(fmt)
 
 
@@ -198,6 +200,84 @@ def dequantize_fp8_e4m3(codes):
     return np.where(codes >> np.uint8(7), -mag, mag)
 
 
+# --------------------------------------------------------------------------
+# MXINT8 (R38): PAPER.md:184 lists INT8 among the "group-32 microscale" precisions and fixes
+# nothing else.  Reading: the OCP MX v1.0 INT8 element -- a two's-complement byte read as code * 2^-6, so that the
+# group's largest element lands in [1, 2) -- under one E8M0 shared scale per group of 32.
+# --------------------------------------------------------------------------
+
+def quantize_mxint8(k_bits):
+    """BF16 bits [..., d] -> (codes int8 [..., d] in -127..127, scale bytes uint8 [..., d/32]).
+
+    amax = max|v| over the group.  amax == 0: scale byte 127, codes 0.  Else e = floor(log2 amax) (0 = emax of the
+    element format), clamped to [-127, 127]; scale byte = e + 127; X = 2^e; code = clamp(RNE(v / X * 64), -127, 127)
+    (symmetric clamp: -128 is never produced).
+    """
+    g = _groups(k_bits)
+    amax = np.max(np.abs(g), axis=-1).astype(np.float64)
+    _, ex = np.frexp(amax)                    # amax = m * 2^ex, m in [0.5, 1)
+    e = np.where(amax > 0, ex.astype(np.int64) - 1, 0)
+    e = np.clip(e, -127, 127)
+    X = np.ldexp(1.0, e)                      # exact in float64
+    r = g.astype(np.float64) / X[..., None] * 64.0        # exact (power-of-two scalings)
+    codes = np.clip(np.rint(r), -127, 127).astype(np.int8)   # rint: half-to-even
+    scale = (e + 127).astype(np.uint8)
+    return codes.reshape(g.shape[:-2] + (-1,)), scale
+
+
+def dequantize_mxint8(codes, scale):
+    """-> float64 [..., d]; value = code * 2^(scale - 127 - 6): <= 7 significant bits, exact in BF16; code 0 -> +0.0."""
+    codes = np.asarray(codes, dtype=np.int8)
+    scale = np.asarray(scale, dtype=np.uint8)
+    c = codes.reshape(codes.shape[:-1] + (codes.shape[-1] // GROUP, GROUP)).astype(np.float64)
+    X = np.ldexp(1.0, scale.astype(np.int64) - 127 - 6)
+    out = c * X[..., None] + 0.0
+    return out.reshape(codes.shape)
+
+
+# --------------------------------------------------------------------------
+# INT4 with a 16-bit group scale (SURVEY 8f f2; DESIGN.md R39): the paper's own INT4 accounting, "4.5 bits per element",
+# 1.27 GiB against MXFP4's 1.20 GiB at Qwen3-8B / 128K (PAPER.md:188).  The paper does not say which 16-bit number the
+# scale is.  Reading: a BF16 scale (the cache's own number format); everything else as in int4_e4m3.
+# --------------------------------------------------------------------------
+
+def _f32_to_bf16_bits_rne(x):
+    """finite binary32 -> BF16 bits, round-to-nearest-even on the 16 dropped bits (integer arithmetic on the pattern)."""
+    u = np.asarray(x, dtype=np.float32).view(np.uint32).astype(np.uint64)
+    lsb = (u >> np.uint64(16)) & np.uint64(1)
+    return ((u + np.uint64(0x7FFF) + lsb) >> np.uint64(16)).astype(np.uint16)
+
+
+def quantize_int4_bf16s(k_bits):
+    """BF16 bits [..., d] -> (q int8 [..., d] in -7..7, scale BF16 bits uint16 [..., d/32]).
+
+    sf = amax / 7 (binary32); scale = RNE-to-BF16(sf); a zero scale with amax > 0 is bumped to the smallest BF16
+    subnormal (bits 0x0001); amax == 0 -> scale bits 0, all q = 0.  s = value(scale);
+    q = clamp(rint(v / s), -7, 7) with the division in binary32 and rint half-to-even.
+    """
+    g = _groups(k_bits)
+    amax = np.max(np.abs(g), axis=-1)                         # float32
+    sf = amax / np.float32(7.0)                               # binary32 RNE
+    sb = _f32_to_bf16_bits_rne(sf)
+    sb = np.where((sb == 0) & (amax > 0), np.uint16(1), sb).astype(np.uint16)
+    s = bf16_bits_to_f32(sb)                                  # exact
+    with np.errstate(divide="ignore", invalid="ignore"):
+        t = g / s[..., None]                                  # binary32 RNE
+    t = np.where(s[..., None] > 0, t, np.float32(0))
+    q = np.clip(np.rint(t), -7, 7).astype(np.int8)
+    return q.reshape(g.shape[:-2] + (-1,)), sb
+
+
+def dequantize_int4_bf16s(q, scale_bits):
+    """-> float64 [..., d]; value = q * BF16(scale), exact here.  Up to 11 significant bits: NOT a BF16 number in general
+    (the scoring kernels use the exact product; a BF16 view of it is a rounding)."""
+    q = np.asarray(q, dtype=np.int8)
+    qq = q.reshape(q.shape[:-1] + (q.shape[-1] // GROUP, GROUP)).astype(np.float64)
+    s = bf16_bits_to_f32(np.asarray(scale_bits, dtype=np.uint16)).astype(np.float64)
+    out = qq * s[..., None] + 0.0
+    return out.reshape(q.shape)
+
+
 def quantize_dequantize(fmt, k_bits):
     """Convenience: BF16 bits -> float64 dequantised keys for a format name."""
     if fmt == "bf16":
@@ -209,4 +289,8 @@ def quantize_dequantize(fmt, k_bits):
         return dequantize_int4_e4m3(*quantize_int4_e4m3(k_bits))
     if fmt == "fp8_e4m3":
         return dequantize_fp8_e4m3(quantize_fp8_e4m3(k_bits))
+    if fmt == "mxint8":
+        return dequantize_mxint8(*quantize_mxint8(k_bits))
+    if fmt == "int4_bf16s":
+        return dequantize_int4_bf16s(*quantize_int4_bf16s(k_bits))
     raise ValueError(fmt)

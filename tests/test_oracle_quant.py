@@ -304,3 +304,144 @@ def test_quantised_query_times_quantised_key_scores_are_scores_of_the_two_images
     from workloads import f32_to_bf16_bits
     qb = f32_to_bf16_bits(q2.astype(np.float32))
     assert not np.array_equal(OQ.quantize_dequantize("fp8_e4m3", qb), OQ.quantize_dequantize("bf16", qb))
+
+
+# ---- f2: MXINT8 and INT4 with a BF16 group scale (R38 / R39) ----------------------------------------------
+
+def _floor_log2(x):
+    """floor(log2 x) of a positive Fraction by exact comparisons."""
+    e = 0
+    while Fraction(2) ** (e + 1) <= x:
+        e += 1
+    while Fraction(2) ** e > x:
+        e -= 1
+    return e
+
+
+def test_mxint8_codes_match_bruteforce_rne():
+    """Every element goes to the nearest of the 255 values code * 2^(e-6), code in [-127, 127] (ties to the even code,
+    saturating), with e = floor(log2 amax) found by exact comparisons -- an independent statement of the format."""
+    rng = np.random.default_rng(21)
+    vals = rng.standard_normal((120, 32)).astype(np.float32) * np.exp(rng.uniform(-6, 6, (120, 1))).astype(np.float32)
+    # ties: with amax = 1.5 (e = 0) the grid step is 1/64; odd multiples of 1/128 are exact ties
+    vals[0] = np.array([1.5] + [(2 * i + 1) / 128.0 * (-1) ** i for i in range(31)], dtype=np.float32)
+    # clamp: amax = 1.9921875 = 255/128 -> 127.5 -> 128 by RNE -> clamped to 127; -amax likewise to -127
+    vals[1] = np.array([255 / 128.0, -255 / 128.0, 1.984375, -1.984375] + [0.0] * 28, dtype=np.float32)
+    bits = _bits(vals)
+    v = bf16_bits_to_f64(bits)
+    codes, scale = quant.quantize_mxint8(bits)
+    assert codes.dtype == np.int8 and codes.min() >= -127
+    for r in range(v.shape[0]):
+        amax = max(abs(Fraction(x)) for x in v[r])
+        e = max(-127, min(127, _floor_log2(amax))) if amax > 0 else 0
+        assert int(scale[r, 0]) == e + 127
+        step = Fraction(2) ** (e - 6)
+        for i in range(32):
+            x = Fraction(float(v[r, i])) / step
+            lo = x.numerator // x.denominator            # floor
+            frac = x - lo
+            want = lo + (1 if frac > Fraction(1, 2) or (frac == Fraction(1, 2) and lo % 2 == 1) else 0)
+            want = max(-127, min(127, want))
+            assert int(codes[r, i]) == want, (r, i, float(x))
+    assert codes[1, :4].tolist() == [127, -127, 127, -127]
+    assert codes[0, 1:5].tolist() == [0, -2, 2, -4]       # 1/128 -> 0.5 -> 0; -3/128 -> -1.5 -> -2; 5/128 -> 2; -7/128 -> -4
+
+
+def test_mxint8_roundtrip_zero_group_error_bound_and_bf16_exactness():
+    rng = np.random.default_rng(22)
+    for k in (-30, -3, 0, 7, 60):
+        c = rng.integers(-127, 128, 32)
+        c[0] = 64 + int(rng.integers(0, 64))                 # largest-magnitude class [1, 2) X: pins the scale
+        c = np.clip(c, -c[0], c[0])
+        g = c * 2.0 ** (k - 6)
+        bits = _bits(g)                                      # <= 7 significant bits: BF16-exact inputs
+        cc, ss = quant.quantize_mxint8(bits)
+        assert ss.tolist() == [k + 127] and cc.tolist() == c.tolist()
+        assert np.array_equal(quant.dequantize_mxint8(cc, ss), bf16_bits_to_f64(bits))
+    cc, ss = quant.quantize_mxint8(_bits(np.zeros(32)))
+    assert ss.tolist() == [127] and not cc.any()
+    bits = _bits(rng.standard_normal((64, 4, 64)).astype(np.float32) * 3)
+    v = bf16_bits_to_f64(bits)
+    cc, ss = quant.quantize_mxint8(bits)
+    dq = quant.dequantize_mxint8(cc, ss)
+    f64_to_bf16_bits_exact(dq)                               # raises if a dequantised key is not a BF16 number
+    X = np.ldexp(1.0, ss.astype(int) - 127)                  # [64, 4, 2]
+    err = np.abs(dq - v).reshape(64, 4, 2, 32)
+    assert np.all(err <= X[..., None] / 64)                  # half a step (X / 128), or the clamp's X / 128 .. X / 64
+    assert np.all(err[np.abs(cc).reshape(64, 4, 2, 32) < 127] <= np.broadcast_to(X[..., None] / 128, err.shape)[
+        np.abs(cc).reshape(64, 4, 2, 32) < 127])
+    assert not np.any(np.signbit(dq[dq == 0]))
+    # against the (pinned) MXFP4 quantiser: same floor(log2 amax), so the E8M0 bytes differ by E2M1's emax = 2
+    _, s4 = quant.quantize_mxfp4(bits)
+    assert np.array_equal(ss.astype(int), s4.astype(int) + 2)
+    assert quant.selector_k_bytes("mxint8", 256) == 256 + 8
+
+
+def _bf16_value(bits):
+    return Fraction(float(bf16_bits_to_f64(np.array([bits], dtype=np.uint16))[0]))
+
+
+def test_int4_bf16s_scale_is_the_nearest_bf16_to_amax_over_7_and_q_the_nearest_integer():
+    rng = np.random.default_rng(23)
+    vals = rng.standard_normal((300, 64)).astype(np.float32) * np.exp(rng.uniform(-5, 5, (300, 1))).astype(np.float32)
+    bits = _bits(vals)
+    v = bf16_bits_to_f64(bits)
+    q, sb = quant.quantize_int4_bf16s(bits)
+    assert sb.dtype == np.uint16 and q.min() >= -7 and q.max() <= 7
+    vg = v.reshape(300, 2, 32)
+    qg = q.reshape(300, 2, 32)
+    for r in range(0, 300, 3):
+        for gi in range(2):
+            amax = max(abs(Fraction(float(x))) for x in vg[r, gi])
+            want = amax / 7
+            b = int(sb[r, gi])
+            s, below, above = _bf16_value(b), _bf16_value(b - 1), _bf16_value(b + 1)
+            assert abs(s - want) <= abs(below - want) and abs(s - want) <= abs(above - want), (r, gi)
+    s = bf16_bits_to_f64(sb)
+    t = vg / s[..., None]
+    assert np.all(np.abs(qg - np.clip(t, -7, 7)) <= 0.5 + 1e-6)
+    dq = quant.dequantize_int4_bf16s(q, sb).reshape(300, 2, 32)
+    bound = s[..., None] * (0.5 + 1e-6) + np.maximum(0, np.abs(vg) - 7 * s[..., None])
+    assert np.all(np.abs(dq - vg) <= bound)
+    # the 16-bit scale is what the format buys: it sits within 2^-9 relative of amax / 7 (E4M3: 2^-4)
+    assert np.all(np.abs(s - np.abs(vg).max(-1) / 7) <= np.abs(vg).max(-1) / 7 * 2.0 ** -8)
+    # dequantised values carry up to 11 significant bits: not BF16 numbers in general
+    with pytest.raises(ValueError):
+        f64_to_bf16_bits_exact(dq)
+
+
+def test_int4_bf16s_roundtrip_special_groups_and_agreement_with_int4_e4m3_on_e4m3_scales(golden):
+    rng = np.random.default_rng(24)
+    # scales with <= 5 significant bits keep q * s inside BF16, so the inputs are exact and must round-trip
+    for sbits in (0x3F80, 0x3FC0, 0x3E10, 0x4288, 0x0080, 0x7000):
+        s = float(bf16_bits_to_f64(np.array([sbits], dtype=np.uint16))[0])
+        q = rng.integers(-7, 8, 32)
+        q[0] = 7                                             # amax = 7 s -> amax / 7 = s exactly
+        bits = _bits(q * s)
+        qq, ss = quant.quantize_int4_bf16s(bits)
+        assert ss.tolist() == [sbits] and qq.tolist() == q.tolist()
+        assert np.array_equal(quant.dequantize_int4_bf16s(qq, ss), bf16_bits_to_f64(bits))
+    qq, ss = quant.quantize_int4_bf16s(_bits(np.zeros(32)))
+    assert ss.tolist() == [0] and not qq.any()
+    tiny = np.zeros(32, dtype=np.float32)
+    tiny[5] = 2.0 ** -133                                    # smallest BF16 subnormal: amax / 7 rounds to zero -> bumped
+    qq, ss = quant.quantize_int4_bf16s(_bits(tiny))
+    assert ss.tolist() == [1] and qq[5] == 1
+    # where amax / 7 is itself an E4M3 value, both INT4 formats hold the same scale value, hence the same codes and keys
+    # (int4_e4m3 is pinned above by the survey's golden group and the E4M3 brute force)
+    for code in (0x08, 0x21, 0x38, 0x45, 0x6B):
+        s = float(quant.e4m3_value(code))
+        g = rng.standard_normal(32) * 3 * s
+        g[0] = 7 * s
+        g = np.clip(g, -7 * s, 7 * s)
+        bits = _bits(g.astype(np.float32))
+        q1, c1 = quant.quantize_int4_e4m3(bits)
+        q2, s2 = quant.quantize_int4_bf16s(bits)
+        assert c1.tolist() == [code] and float(bf16_bits_to_f64(s2)[0]) == s
+        assert np.array_equal(q1, q2)
+        assert np.array_equal(quant.dequantize_int4_e4m3(q1, c1), quant.dequantize_int4_bf16s(q2, s2))
+    # the paper's own INT4 accounting (PAPER.md:188): 4.5 bit/elt, 1.27 GiB at Qwen3-8B / 128K
+    g = golden("footprint.txt")
+    n = int(g["tokens"][0][0]) * int(g["layers"][0][0]) * int(g["h_idx"][0][0]) * int(g["d_idx"][0][0])
+    assert quant.selector_k_bytes("int4_bf16s", n) / 2.0 ** 30 == pytest.approx(float(g["int4_gib"][0][0]), abs=0.005)
+    assert quant.selector_k_bytes("int4_bf16s", n) * 32 == n * 18
