@@ -2,7 +2,7 @@
 """bench.py -- one decode layer-step of the SpotAttention hot path (selector scoring -> dual top-p -> block-sparse
 GQA attention) on synthetic Qwen3-shaped inputs, through the C ABI of include/spot.h.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg3] [--fmt bf16|mxfp4|int4_e4m3] [--p 0.9]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg3] [--fmt bf16|mxfp4|int4_e4m3|fp8_e4m3|mxint8|int4_bf16s] [--p 0.9]
     python bench.py --impl reference ...       # the fp64 CPU oracle on a bounded sample (rank 0 only)
 
 Prints ONE JSON line (rank 0).  A "step" = spot_decode_step (= spot_select + spot_sparse_attn_decode in one call) over
@@ -419,8 +419,9 @@ def run_ours(args):
     peak, peak_src = measured_peaks()
 
     def bytes_per_token(fmt):
-        return {"bf16": wl.H_idx * wl.d_idx * 2, "fp8_e4m3": wl.H_idx * wl.d_idx}.get(
-            fmt, wl.H_idx * wl.d_idx // 2 + wl.H_idx * wl.d_idx // 32)
+        n = wl.H_idx * wl.d_idx
+        return {"bf16": n * 2, "fp8_e4m3": n, "mxint8": n + n // 32, "int4_bf16s": n // 2 + n // 16}.get(
+            fmt, n // 2 + n // 32)
 
     # config 3's own subject, in the default run: the same step with the selector K-cache quantised (INT4 + E4M3 scale,
     # MXFP4), beside the BF16 control above; and BASELINE.json's second target, the prefill selector GEMM, timed alone
@@ -933,7 +934,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="cfg3")
-    ap.add_argument("--fmt", default="bf16", choices=["bf16", "mxfp4", "int4_e4m3", "fp8_e4m3"])
+    ap.add_argument("--fmt", default="bf16", choices=["bf16", "mxfp4", "int4_e4m3", "fp8_e4m3", "mxint8", "int4_bf16s"])
     ap.add_argument("--qfmt", default="bf16", choices=["bf16", "fp8_e4m3"],
                     help="cfg5 only: format of the selector QUERIES (fp8_e4m3 with --fmt fp8_e4m3: FP8 x FP8 tensor-core scoring)")
     ap.add_argument("--p", type=float, default=0.90)

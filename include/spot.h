@@ -52,7 +52,10 @@ typedef enum {
     SPOT_SELK_BF16 = 0,      /* [B][cache_stride_tokens][H_idx][d_idx] BF16                              */
     SPOT_SELK_INT4_E4M3 = 1, /* signed 4-bit codes, group 32 along d_idx, one FP8-E4M3 scale per group   */
     SPOT_SELK_MXFP4 = 2,     /* E2M1 codes, group 32 along d_idx, one E8M0 scale per group (OCP MX)      */
-    SPOT_SELK_FP8_E4M3 = 3   /* f2: one FP8-E4M3 byte per element, no scale, [B][tokens][H_idx][d_idx]   */
+    SPOT_SELK_FP8_E4M3 = 3,  /* f2: one FP8-E4M3 byte per element, no scale, [B][tokens][H_idx][d_idx]   */
+    SPOT_SELK_MXINT8 = 4,    /* f2: OCP MX INT8 codes (code * 2^-6), group 32, one E8M0 scale per group   */
+    SPOT_SELK_INT4_BF16S = 5 /* f2: signed 4-bit codes, group 32, one BF16 scale per group: the paper's   */
+                             /*     own INT4 accounting, 4.5 bit / element                 */
 } spot_selk_format;
 
 typedef enum {
@@ -80,7 +83,8 @@ size_t spot_struct_size(int which);
  * Bytes of a cache holding B sequences of cache_stride_tokens tokens each (a multiple of 64 for the 4-bit
  * formats): BF16 2*n, 4-bit formats n/2 + n/32 with n = B*tokens*H_idx*d_idx (16 -> 4.25
  * bit/element), FP8-E4M3 n (the paper's "FP8" precision; R30: RNE-satfinite cast of every
- * element, no scale).  Returns 0 on invalid arguments.
+ * element, no scale), MXINT8 n + n/32 (8.25 bit/element; R38), INT4 with a BF16 group scale n/2 + n/16
+ * (PAPER.md:188's "4.5 bits per element", 1.27 GiB at Qwen3-8B / 128K; R39).  Returns 0 on invalid arguments.
  * --------------------------------------------------------------------------------------------------- */
 size_t spot_selector_k_bytes(spot_selk_format fmt, int64_t B, int64_t cache_stride_tokens, int H_idx, int d_idx);
 
@@ -90,13 +94,17 @@ size_t spot_selector_k_bytes(spot_selk_format fmt, int64_t B, int64_t cache_stri
  * Prefill: the whole prompt; decode: n_tokens = 1 appended.  Requires d_idx % 32 == 0,
  * token_offset + n_tokens <= cache_stride_tokens.  Quantiser definitions: DESIGN.md R16 (MXFP4: scale
  * 2^(floor(log2 amax) - 2), RNE onto the E2M1 grid, saturating; INT4: scale = E4M3_rne_satfinite(amax/7),
- * q = clamp(rint(v/scale), -7, 7)).  Results are bit-exact with that definition. */
+ * q = clamp(rint(v/scale), -7, 7)); R38 (MXINT8: scale 2^floor(log2 amax), code = clamp(RNE(64 v / scale), -127, 127));
+ * R39 (INT4_BF16S: scale = RNE_bf16(amax/7), q as INT4).  Results are bit-exact with that definition. */
 spot_status spot_quantize_selector_k(const uint16_t* k_bf16, void* k_cache, spot_selk_format fmt,
                                      int64_t B, int64_t n_tokens, int64_t token_offset,
                                      int64_t cache_stride_tokens, int H_idx, int d_idx, void* stream);
 
 /* Inverse: write the dequantised keys of tokens [token_offset, token_offset + n_tokens) as BF16
- * [B][n_tokens][H_idx][d_idx] (exact: every dequantised value is representable in BF16). */
+ * [B][n_tokens][H_idx][d_idx] (exact: every dequantised value is representable in BF16 -- except SPOT_SELK_INT4_BF16S,
+ * whose values q * scale carry up to 11 significant bits: for that format this call writes their round-to-nearest-even
+ * BF16 view, a diagnostic; the scoring kernels use the exact products, and prefill selection (q_block = 64), which would
+ * go through this view, returns SPOT_ERR_UNSUPPORTED). */
 spot_status spot_dequantize_selector_k(const void* k_cache, uint16_t* k_bf16_out, spot_selk_format fmt,
                                        int64_t B, int64_t n_tokens, int64_t token_offset,
                                        int64_t cache_stride_tokens, int H_idx, int d_idx, void* stream);

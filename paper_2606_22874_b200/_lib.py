@@ -9,12 +9,12 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(HERE, "libspot.so")
 
 SPOT_OK, SPOT_ERR_INVALID_ARG, SPOT_ERR_UNSUPPORTED, SPOT_ERR_WORKSPACE_TOO_SMALL, SPOT_ERR_CUDA = range(5)
-SPOT_SELK_BF16, SPOT_SELK_INT4_E4M3, SPOT_SELK_MXFP4, SPOT_SELK_FP8_E4M3 = range(4)
+SPOT_SELK_BF16, SPOT_SELK_INT4_E4M3, SPOT_SELK_MXFP4, SPOT_SELK_FP8_E4M3, SPOT_SELK_MXINT8, SPOT_SELK_INT4_BF16S = range(6)
 SPOT_MODE_TOPK, SPOT_MODE_DUAL_TOPP = range(2)
 SPOT_STATIC_SCRATCH_BYTES = 8 << 20
 
 FORMATS = {"bf16": SPOT_SELK_BF16, "int4_e4m3": SPOT_SELK_INT4_E4M3, "mxfp4": SPOT_SELK_MXFP4,
-           "fp8_e4m3": SPOT_SELK_FP8_E4M3}
+           "fp8_e4m3": SPOT_SELK_FP8_E4M3, "mxint8": SPOT_SELK_MXINT8, "int4_bf16s": SPOT_SELK_INT4_BF16S}
 MODES = {"topk": SPOT_MODE_TOPK, "dual_topp": SPOT_MODE_DUAL_TOPP}
 
 

@@ -58,8 +58,7 @@ spot_status select_geometry(const spot_select_params* p, SelectGeom* g, bool sco
     if (!p->sel_q || !p->w || !p->sel_k) return SPOT_ERR_INVALID_ARG;
     if (score_only ? !p->block_scores : (!p->indices || !p->budgets)) return SPOT_ERR_INVALID_ARG;
     if (!aligned16(p->sel_q) || !aligned16(p->sel_k) || !aligned16(p->w)) return SPOT_ERR_INVALID_ARG;
-    if (p->fmt != SPOT_SELK_BF16 && p->fmt != SPOT_SELK_INT4_E4M3 && p->fmt != SPOT_SELK_MXFP4 &&
-        p->fmt != SPOT_SELK_FP8_E4M3) return SPOT_ERR_INVALID_ARG;
+    if (!selk_is_format(p->fmt)) return SPOT_ERR_INVALID_ARG;
     if (p->mode != SPOT_MODE_TOPK && p->mode != SPOT_MODE_DUAL_TOPP) return SPOT_ERR_INVALID_ARG;
     if (p->B <= 0 || p->Tq <= 0 || p->H_idx <= 0 || p->d_idx <= 0 || p->d_idx % 32 != 0) return SPOT_ERR_INVALID_ARG;
     if (p->blk <= 0 || (!score_only && p->cap <= 0) || p->cache_stride_tokens <= 0) return SPOT_ERR_INVALID_ARG;
@@ -72,6 +71,9 @@ spot_status select_geometry(const spot_select_params* p, SelectGeom* g, bool sco
     // quantised selector queries on the tensor cores (f2): FP8-E4M3 queries against the FP8-E4M3 cache, prefill rows only
     if (p->q_fmt != SPOT_SELK_BF16 && p->q_fmt != SPOT_SELK_FP8_E4M3) return SPOT_ERR_INVALID_ARG;
     if (p->q_fmt == SPOT_SELK_FP8_E4M3 && (p->fmt != SPOT_SELK_FP8_E4M3 || p->q_block != 64)) return SPOT_ERR_UNSUPPORTED;
+    // INT4 with BF16 group scales: its keys q * s are not BF16 numbers (R39), and the prefill form would score their
+    // dequantised BF16 view -- decode rows only
+    if (p->fmt == SPOT_SELK_INT4_BF16S && p->q_block != 1) return SPOT_ERR_UNSUPPORTED;
     // 64-token blocks, or the paper's own 16-token blocks (f3), in both row forms
     if (p->blk != 64 && p->blk != 16) return SPOT_ERR_UNSUPPORTED;
     int64_t max_tokens;

@@ -46,7 +46,14 @@ static inline int64_t ceil_div64(int64_t a, int64_t b) { return (a + b - 1) / b;
 
 // ---- quantised selector K-cache tile geometry (opaque layout, see include/spot.h) ------------------
 // A tile holds SELK_TILE tokens: [SELK_TILE][H*d/2] code bytes, then [SELK_TILE][H*d/32] scale bytes.
+// (f2: MXINT8 has H*d code bytes per token, INT4_BF16S two scale bytes per group -- selk_*_per_group below)
 constexpr int SELK_TILE = 64;
+__host__ __device__ constexpr bool selk_is_grouped(int fmt) {
+    return fmt == SPOT_SELK_INT4_E4M3 || fmt == SPOT_SELK_MXFP4 || fmt == SPOT_SELK_MXINT8 || fmt == SPOT_SELK_INT4_BF16S;
+}
+__host__ __device__ constexpr bool selk_is_format(int fmt) { return fmt == SPOT_SELK_BF16 || fmt == SPOT_SELK_FP8_E4M3 || selk_is_grouped(fmt); }
+__host__ __device__ constexpr int selk_code_bytes_per_group(int fmt) { return fmt == SPOT_SELK_MXINT8 ? 32 : 16; }
+__host__ __device__ constexpr int selk_scale_bytes_per_group(int fmt) { return fmt == SPOT_SELK_INT4_BF16S ? 2 : 1; }
 __host__ __device__ inline int64_t selk_codes_per_token(int H, int d) { return (int64_t)H * d / 2; }
 __host__ __device__ inline int64_t selk_scales_per_token(int H, int d) { return (int64_t)H * d / 32; }
 __host__ __device__ inline int64_t selk_tile_bytes(int H, int d) {

@@ -155,8 +155,7 @@ spot_status check_project(const spot_project_params* p) {
     if (p->rope_dims < 0 || p->rope_dims % 2 != 0 || p->rope_dims > p->d_idx || !(p->rope_base > 0.f))
         return SPOT_ERR_INVALID_ARG;
     if (p->rope_dims > PJ_MAX_ROPE) return SPOT_ERR_UNSUPPORTED;
-    if (p->fmt != SPOT_SELK_BF16 && p->fmt != SPOT_SELK_INT4_E4M3 && p->fmt != SPOT_SELK_MXFP4 &&
-        p->fmt != SPOT_SELK_FP8_E4M3) return SPOT_ERR_INVALID_ARG;
+    if (!selk_is_format(p->fmt)) return SPOT_ERR_INVALID_ARG;
     if (p->cache_stride_tokens <= 0) return SPOT_ERR_INVALID_ARG;
     if (p->fmt != SPOT_SELK_BF16 && p->cache_stride_tokens % SELK_TILE != 0)
         return SPOT_ERR_INVALID_ARG;

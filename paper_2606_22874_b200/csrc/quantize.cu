@@ -8,6 +8,13 @@
 //   INT4  : offset-binary u = q + 8; 32-bit word wd of a group holds dims 8wd..8wd+7 with
 //           dim 8wd + 2pp + e at nibble pp + 4e, so that (w >> 4pp) & 0x000F000F is the pair (2pp, 2pp+1)
 //           (what the fp16 magic-number unpack in score_decode.cu wants).
+//   INT4_BF16S (f2, R39): INT4's codes; the scale rows hold two bytes per group (the BF16 bits of the scale).
+//   MXINT8 (f2, R38): [64][H*d] code bytes | [64][H*d/32] E8M0 bytes.  A code byte is offset-binary u = code + 128
+//           (read as an fp16 subnormal by the scoring kernel, the offset taken on the query side).  Every 128 bytes of a
+//           token's codes are four groups as two 64-byte halves -- half hh holds bytes [16 hh, 16 hh + 16) of each of the
+//           four groups -- and ODD tokens store the two halves swapped, so that the 16-byte shared-memory loads of two
+//           adjacent token rows fall into different banks.
+#include <cuda_bf16.h>
 #include <cuda_fp8.h>
 
 #include "common.cuh"
@@ -63,8 +70,9 @@ __global__ void __launch_bounds__(256) quantize_kernel(const uint16_t* __restric
         amax = fmaxf(amax, fmaxf(fabsf(v[2 * i]), fabsf(v[2 * i + 1])));
     }
 
-    uint32_t out[4];
-    uint32_t scale_byte;
+    constexpr int CB = selk_code_bytes_per_group(FMT), SB = selk_scale_bytes_per_group(FMT);
+    uint32_t out[CB / 4];
+    uint32_t scale_bits;
     if (FMT == SPOT_SELK_MXFP4) {
         // e = floor(log2 amax) - 2 clamped to [-127, 127]; X = 2^e; code = RNE_E2M1(v / X), saturating.
         int e = 0;
@@ -72,7 +80,7 @@ __global__ void __launch_bounds__(256) quantize_kernel(const uint16_t* __restric
             e = ilogbf(amax) - 2;
             e = max(-127, min(127, e));
         }
-        scale_byte = (uint32_t)(e + 127);
+        scale_bits = (uint32_t)(e + 127);
         // 1/X = 2^-e, -e in [-125(+2), 127]: always a normal binary32 except e = 127 (unreachable: e <= 125).
         float inv = __uint_as_float((uint32_t)(127 - e) << 23);
         if (e == 127) inv = __uint_as_float(0x00400000u);   // 2^-127 (kept for completeness)
@@ -86,14 +94,38 @@ __global__ void __launch_bounds__(256) quantize_kernel(const uint16_t* __restric
             }
             out[wd] = acc;
         }
+    } else if (FMT == SPOT_SELK_MXINT8) {
+        // e = floor(log2 amax) clamped to [-127, 127]; code = clamp(RNE(v 2^(6 - e)), -127, 127); stored as u = code + 128.
+        int e = 0;
+        if (amax > 0.f) e = max(-127, min(127, ilogbf(amax)));
+        scale_bits = (uint32_t)(e + 127);
+#pragma unroll
+        for (int wd = 0; wd < 8; ++wd) {
+            uint32_t acc = 0;
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+                const float r = fminf(fmaxf(rintf(scalbnf(v[4 * wd + j], 6 - e)), -127.f), 127.f);   // scalbnf: exact
+                acc |= (uint32_t)((int)r + 128) << (8 * j);
+            }
+            out[wd] = acc;
+        }
     } else {
-        // sf = amax / 7 (binary32 RNE); code = E4M3_rne_satfinite(sf), bumped to 0x01 if it rounds to 0 with
-        // amax > 0; q = clamp(rint(v / s), -7, 7) with s = value(code); stored as u = q + 8.
+        // sf = amax / 7 (binary32 RNE); INT4_E4M3: code = E4M3_rne_satfinite(sf); INT4_BF16S: the BF16 nearest sf; either
+        // bumped to its smallest subnormal if it rounds to 0 with amax > 0; q = clamp(rint(v / s), -7, 7) with
+        // s = value(scale); stored as u = q + 8.
         float sf = __fdiv_rn(amax, 7.0f);
-        uint32_t code = (uint32_t)__nv_cvt_float_to_fp8(sf, __NV_SATFINITE, __NV_E4M3) & 0xffu;
-        if (code == 0 && amax > 0.f) code = 1;
-        scale_byte = code;
-        float s = e4m3_to_f32(code);
+        float s;
+        if (FMT == SPOT_SELK_INT4_BF16S) {
+            uint32_t sb = (uint32_t)__bfloat16_as_ushort(__float2bfloat16_rn(sf));
+            if (sb == 0 && amax > 0.f) sb = 1;
+            scale_bits = sb;
+            s = __uint_as_float(sb << 16);
+        } else {
+            uint32_t code = (uint32_t)__nv_cvt_float_to_fp8(sf, __NV_SATFINITE, __NV_E4M3) & 0xffu;
+            if (code == 0 && amax > 0.f) code = 1;
+            scale_bits = code;
+            s = e4m3_to_f32(code);
+        }
 #pragma unroll
         for (int wd = 0; wd < 4; ++wd) {
             uint32_t acc = 0;
@@ -112,12 +144,18 @@ __global__ void __launch_bounds__(256) quantize_kernel(const uint16_t* __restric
 
     int64_t tile = t / SELK_TILE;
     int r = (int)(t % SELK_TILE);
-    int64_t cpt = (int64_t)groups_per_token * 16;
-    int64_t spt = groups_per_token;
+    int64_t cpt = (int64_t)groups_per_token * CB;
+    int64_t spt = (int64_t)groups_per_token * SB;
     uint8_t* tile_base = cache + (b * tiles_per_seq + tile) * (SELK_TILE * (cpt + spt));
-    uint4 o = make_uint4(out[0], out[1], out[2], out[3]);
-    *reinterpret_cast<uint4*>(tile_base + r * cpt + gi * 16) = o;
-    tile_base[SELK_TILE * cpt + r * spt + gi] = (uint8_t)scale_byte;
+    if (FMT == SPOT_SELK_MXINT8) {
+        uint8_t* unit = tile_base + r * cpt + (gi >> 2) * 128 + (gi & 3) * 16;
+        *reinterpret_cast<uint4*>(unit + ((r & 1) ? 64 : 0)) = make_uint4(out[0], out[1], out[2], out[3]);
+        *reinterpret_cast<uint4*>(unit + ((r & 1) ? 0 : 64)) = make_uint4(out[CB / 4 - 4], out[CB / 4 - 3], out[CB / 4 - 2], out[CB / 4 - 1]);
+    } else {
+        *reinterpret_cast<uint4*>(tile_base + r * cpt + gi * 16) = make_uint4(out[0], out[1], out[2], out[3]);
+    }
+    if (SB == 2) *reinterpret_cast<uint16_t*>(tile_base + SELK_TILE * cpt + r * spt + gi * 2) = (uint16_t)scale_bits;
+    else tile_base[SELK_TILE * cpt + r * spt + gi] = (uint8_t)scale_bits;
 }
 
 template <int FMT>
@@ -132,12 +170,23 @@ __global__ void __launch_bounds__(256) dequantize_kernel(const uint8_t* __restri
     int64_t t = token_offset + (tok_lin - b * n_tokens);
     int64_t tile = t / SELK_TILE;
     int r = (int)(t % SELK_TILE);
-    int64_t cpt = (int64_t)groups_per_token * 16;
-    int64_t spt = groups_per_token;
+    constexpr int CB = selk_code_bytes_per_group(FMT), SB = selk_scale_bytes_per_group(FMT);
+    int64_t cpt = (int64_t)groups_per_token * CB;
+    int64_t spt = (int64_t)groups_per_token * SB;
     const uint8_t* tile_base = cache + (b * tiles_per_seq + tile) * (SELK_TILE * (cpt + spt));
-    uint4 c = *reinterpret_cast<const uint4*>(tile_base + r * cpt + gi * 16);
-    uint32_t sb = tile_base[SELK_TILE * cpt + r * spt + gi];
-    uint32_t w[4] = {c.x, c.y, c.z, c.w};
+    uint32_t w[CB / 4];
+    if (FMT == SPOT_SELK_MXINT8) {
+        const uint8_t* unit = tile_base + r * cpt + (gi >> 2) * 128 + (gi & 3) * 16;
+        const uint4 lo = *reinterpret_cast<const uint4*>(unit + ((r & 1) ? 64 : 0));
+        const uint4 hi = *reinterpret_cast<const uint4*>(unit + ((r & 1) ? 0 : 64));
+        w[0] = lo.x; w[1] = lo.y; w[2] = lo.z; w[3] = lo.w;
+        w[CB / 4 - 4] = hi.x; w[CB / 4 - 3] = hi.y; w[CB / 4 - 2] = hi.z; w[CB / 4 - 1] = hi.w;
+    } else {
+        const uint4 c = *reinterpret_cast<const uint4*>(tile_base + r * cpt + gi * 16);
+        w[0] = c.x; w[1] = c.y; w[2] = c.z; w[3] = c.w;
+    }
+    const uint32_t sb = SB == 2 ? (uint32_t)*reinterpret_cast<const uint16_t*>(tile_base + SELK_TILE * cpt + r * spt + gi * 2)
+                                : (uint32_t)tile_base[SELK_TILE * cpt + r * spt + gi];
     float v[32];
     if (FMT == SPOT_SELK_MXFP4) {
         float X = sb ? __uint_as_float(sb << 23) : __uint_as_float(0x00400000u);
@@ -151,20 +200,31 @@ __global__ void __launch_bounds__(256) dequantize_kernel(const uint8_t* __restri
             float val = mag * X;
             v[i] = (code & 8) ? -val : val;
         }
+    } else if (FMT == SPOT_SELK_MXINT8) {
+#pragma unroll
+        for (int i = 0; i < 32; ++i) {
+            const int code = (int)((w[i >> 2] >> (8 * (i & 3))) & 0xffu) - 128;
+            v[i] = scalbnf((float)code, (int)sb - 127 - 6) + 0.0f;          // exact: <= 7 significant bits
+        }
     } else {
-        float s = e4m3_to_f32(sb);
+        float s = FMT == SPOT_SELK_INT4_BF16S ? __uint_as_float(sb << 16) : e4m3_to_f32(sb);
 #pragma unroll
         for (int i = 0; i < 32; ++i) {
             int wd = i >> 3, j = i & 7, pp = j >> 1, e = j & 1;
             int q = (int)((w[wd] >> (4 * (pp + 4 * e))) & 0xf) - 8;
-            v[i] = (float)q * s + 0.0f;
+            v[i] = (float)q * s + 0.0f;                                    // exact in fp32 (3 x 8 significant bits)
         }
     }
     uint32_t o[16];
 #pragma unroll
     for (int i = 0; i < 16; ++i) {
-        // exact: every dequantised value has <= 8 significant bits (R16), so truncation == the value
-        o[i] = (__float_as_uint(v[2 * i]) >> 16) | (__float_as_uint(v[2 * i + 1]) & 0xffff0000u);
+        if (FMT == SPOT_SELK_INT4_BF16S) {
+            // up to 11 significant bits: the BF16 view is a rounding (R39; a diagnostic -- the scoring kernel uses q * s)
+            o[i] = pack_bf16x2(v[2 * i], v[2 * i + 1]);
+        } else {
+            // exact: every dequantised value has <= 8 significant bits (R16), so truncation == the value
+            o[i] = (__float_as_uint(v[2 * i]) >> 16) | (__float_as_uint(v[2 * i + 1]) & 0xffff0000u);
+        }
     }
     uint4* dst = reinterpret_cast<uint4*>(k_out + gid * 32);
 #pragma unroll
@@ -245,8 +305,7 @@ __global__ void __launch_bounds__(256) copy_rows_kernel(const uint4* __restrict_
 spot_status check_quant_args(const void* a, const void* b, int fmt, int64_t B, int64_t n_tokens, int64_t token_offset,
                              int64_t stride, int H, int d) {
     if (!a || !b || !aligned16(a) || !aligned16(b)) return SPOT_ERR_INVALID_ARG;
-    if (fmt != SPOT_SELK_BF16 && fmt != SPOT_SELK_INT4_E4M3 && fmt != SPOT_SELK_MXFP4 && fmt != SPOT_SELK_FP8_E4M3)
-        return SPOT_ERR_INVALID_ARG;
+    if (!selk_is_format(fmt)) return SPOT_ERR_INVALID_ARG;
     if (B <= 0 || n_tokens <= 0 || token_offset < 0 || H <= 0 || d <= 0 || d % 32 != 0) return SPOT_ERR_INVALID_ARG;
     if (token_offset + n_tokens > stride) return SPOT_ERR_INVALID_ARG;
     if (fmt != SPOT_SELK_BF16 && stride % SELK_TILE != 0) return SPOT_ERR_INVALID_ARG;
@@ -275,12 +334,14 @@ spot_status append_selector_k(const uint16_t* k_new, void* cache, int fmt, int B
     const int gpt = H * d / 32;
     const int64_t total = (int64_t)B * gpt, tiles = stride / SELK_TILE;
     const dim3 grid((unsigned)ceil_div64(total, 256));
-    if (fmt == SPOT_SELK_MXFP4)
-        SPOT_CUDA_TRY(launch_pdl(quantize_kernel<SPOT_SELK_MXFP4>, grid, dim3(256), 0, s, k_new, (uint8_t*)cache, (int64_t)1,
-                                 (int64_t)0, tiles, gpt, total, pos));
-    else
-        SPOT_CUDA_TRY(launch_pdl(quantize_kernel<SPOT_SELK_INT4_E4M3>, grid, dim3(256), 0, s, k_new, (uint8_t*)cache,
-                                 (int64_t)1, (int64_t)0, tiles, gpt, total, pos));
+#define SPOT_APPEND_AS(F)                                                                                              \
+    SPOT_CUDA_TRY(launch_pdl(quantize_kernel<F>, grid, dim3(256), 0, s, k_new, (uint8_t*)cache, (int64_t)1, (int64_t)0, tiles, \
+                             gpt, total, pos))
+    if (fmt == SPOT_SELK_MXFP4) SPOT_APPEND_AS(SPOT_SELK_MXFP4);
+    else if (fmt == SPOT_SELK_MXINT8) SPOT_APPEND_AS(SPOT_SELK_MXINT8);
+    else if (fmt == SPOT_SELK_INT4_BF16S) SPOT_APPEND_AS(SPOT_SELK_INT4_BF16S);
+    else SPOT_APPEND_AS(SPOT_SELK_INT4_E4M3);
+#undef SPOT_APPEND_AS
     return SPOT_OK;
 }
 
@@ -292,9 +353,9 @@ extern "C" size_t spot_selector_k_bytes(spot_selk_format fmt, int64_t B, int64_t
     if (B <= 0 || tokens <= 0 || H_idx <= 0 || d_idx <= 0 || d_idx % 32 != 0) return 0;
     int64_t n = B * tokens * H_idx * d_idx;
     if (fmt == SPOT_SELK_BF16) return (size_t)(2 * n);
-    if (fmt == SPOT_SELK_INT4_E4M3 || fmt == SPOT_SELK_MXFP4) {
+    if (selk_is_grouped(fmt)) {
         if (tokens % SELK_TILE != 0) return 0;
-        return (size_t)(n / 2 + n / 32);
+        return (size_t)(n / 32 * (selk_code_bytes_per_group(fmt) + selk_scale_bytes_per_group(fmt)));
     }
     if (fmt == SPOT_SELK_FP8_E4M3) return tokens % SELK_TILE != 0 ? 0 : (size_t)n;
     return 0;
@@ -325,10 +386,12 @@ extern "C" spot_status spot_quantize_selector_k(const uint16_t* k_bf16, void* k_
     int64_t total = B * n_tokens * gpt;
     int64_t tiles = cache_stride_tokens / SELK_TILE;
     unsigned grid = (unsigned)ceil_div64(total, 256);
-    if (fmt == SPOT_SELK_MXFP4)
-        quantize_kernel<SPOT_SELK_MXFP4><<<grid, 256, 0, s>>>(k_bf16, (uint8_t*)k_cache, n_tokens, token_offset, tiles, gpt, total, nullptr);
-    else
-        quantize_kernel<SPOT_SELK_INT4_E4M3><<<grid, 256, 0, s>>>(k_bf16, (uint8_t*)k_cache, n_tokens, token_offset, tiles, gpt, total, nullptr);
+#define SPOT_QUANT_AS(F) quantize_kernel<F><<<grid, 256, 0, s>>>(k_bf16, (uint8_t*)k_cache, n_tokens, token_offset, tiles, gpt, total, nullptr)
+    if (fmt == SPOT_SELK_MXFP4) SPOT_QUANT_AS(SPOT_SELK_MXFP4);
+    else if (fmt == SPOT_SELK_MXINT8) SPOT_QUANT_AS(SPOT_SELK_MXINT8);
+    else if (fmt == SPOT_SELK_INT4_BF16S) SPOT_QUANT_AS(SPOT_SELK_INT4_BF16S);
+    else SPOT_QUANT_AS(SPOT_SELK_INT4_E4M3);
+#undef SPOT_QUANT_AS
     SPOT_LAUNCH_CHECK();
     return SPOT_OK;
 }
@@ -358,10 +421,12 @@ extern "C" spot_status spot_dequantize_selector_k(const void* k_cache, uint16_t*
     int64_t total = B * n_tokens * gpt;
     int64_t tiles = cache_stride_tokens / SELK_TILE;
     unsigned grid = (unsigned)ceil_div64(total, 256);
-    if (fmt == SPOT_SELK_MXFP4)
-        dequantize_kernel<SPOT_SELK_MXFP4><<<grid, 256, 0, s>>>((const uint8_t*)k_cache, k_bf16_out, n_tokens, token_offset, tiles, gpt, total);
-    else
-        dequantize_kernel<SPOT_SELK_INT4_E4M3><<<grid, 256, 0, s>>>((const uint8_t*)k_cache, k_bf16_out, n_tokens, token_offset, tiles, gpt, total);
+#define SPOT_DEQUANT_AS(F) dequantize_kernel<F><<<grid, 256, 0, s>>>((const uint8_t*)k_cache, k_bf16_out, n_tokens, token_offset, tiles, gpt, total)
+    if (fmt == SPOT_SELK_MXFP4) SPOT_DEQUANT_AS(SPOT_SELK_MXFP4);
+    else if (fmt == SPOT_SELK_MXINT8) SPOT_DEQUANT_AS(SPOT_SELK_MXINT8);
+    else if (fmt == SPOT_SELK_INT4_BF16S) SPOT_DEQUANT_AS(SPOT_SELK_INT4_BF16S);
+    else SPOT_DEQUANT_AS(SPOT_SELK_INT4_E4M3);
+#undef SPOT_DEQUANT_AS
     SPOT_LAUNCH_CHECK();
     return SPOT_OK;
 }

@@ -21,6 +21,10 @@
 //                fixed permutation of the d_idx axis applied to both operands, chosen so that every lane's 16-byte
 //                shared-memory load lands directly in fragment registers.
 //   FP8 cache  : (f2) one cvt.rn.f16x2.e4m3x2 per pair, no scales, the same fp16 HMMA.
+//   INT4 with BF16 group scales (f2, R39): the INT4 path with two scale bytes per group, scale -> fp32 is a shift.
+//   MXINT8 cache (f2, R38): code bytes are offset-binary u = code + 128; one PRMT per pair drops each byte into the low
+//                end of an fp16 (the subnormal u 2^-24, exact), the offset 128 sum x is taken on the query side as for
+//                INT4, the E8M0 scale and 2^-6 go into the post-scale.
 // With 16-token blocks (f3, blk == 16) a tile yields its four 16-token maxima instead of one.
 #include "common.cuh"
 #include "tc100.cuh"
@@ -75,7 +79,7 @@ __device__ __forceinline__ void e4m3x2_to_f32x2(uint32_t two_bytes, float& lo, f
 
 template <int FMT>
 __device__ __forceinline__ float scale_to_f32(uint32_t byte) {
-    if (FMT == SPOT_SELK_MXFP4) {
+    if (FMT == SPOT_SELK_MXFP4 || FMT == SPOT_SELK_MXINT8) {
         return byte ? __uint_as_float(byte << 23) : __uint_as_float(0x00400000u);
     } else {
         // E4M3 -> fp32 (exact): normal: 2^(E-7)(1+m/8); subnormal: m 2^-9
@@ -106,8 +110,10 @@ __device__ __forceinline__ void bulk_load(uint32_t smem_dst, const void* gsrc, u
 template <int H, int D_IDX, int FMT>
 struct ScoreCfg {
     static constexpr int ROW = H * D_IDX;                      // elements per token
+    static constexpr int CODE_BYTES = ROW / 32 * selk_code_bytes_per_group(FMT);      // grouped formats: per token
+    static constexpr int SCALE_BYTES = ROW / 32 * selk_scale_bytes_per_group(FMT);
     static constexpr int TILE_BYTES = FMT == SPOT_SELK_BF16 ? 64 * ROW * 2
-                                      : FMT == SPOT_SELK_FP8_E4M3 ? 64 * ROW : 64 * (ROW / 2 + ROW / 32);
+                                      : FMT == SPOT_SELK_FP8_E4M3 ? 64 * ROW : 64 * (CODE_BYTES + SCALE_BYTES);
     static constexpr bool SELF = FMT != SPOT_SELK_BF16;
     // BF16 (producer ring): few big tiles (32 / 64 KiB, 1024-byte aligned for the 128-byte swizzle) and a light
     // ldmatrix + HMMA body.  One producer lane feeds the ring; every stage belongs to ONE consumer warp (stage s ->
@@ -126,7 +132,9 @@ struct ScoreCfg {
     // (round 2, measured and not kept: 32-token slices with FOUR stages per warp for the 8.5 KiB tiles of d_idx = 64 --
     // MXFP4 scoring alone 24.4 vs 22.8 us at B = 4, 64.3 vs 57.7 us at B = 16: two copies and two barrier phases per tile
     // cost more issue slots than the deeper ring wins back)
-    static constexpr int SPLIT = FMT == SPOT_SELK_FP8_E4M3 ? TILE_BYTES / 8192 : (SELF && TILE_BYTES > 12288 ? 2 : 1);
+    // MXINT8 (16.5 / 33 KiB tiles): slices of 8 KiB of codes + their scale bytes, as FP8.
+    static constexpr int SPLIT = FMT == SPOT_SELK_FP8_E4M3 ? TILE_BYTES / 8192
+                                 : FMT == SPOT_SELK_MXINT8 ? 64 * CODE_BYTES / 8192 : (SELF && TILE_BYTES > 12288 ? 2 : 1);
     static constexpr int STAGE_BYTES = SELF ? TILE_BYTES / SPLIT : (TILE_BYTES + 1023) / 1024 * 1024;
     static constexpr int STAGES_RAW = SC_SMEM_BUDGET / STAGE_BYTES;
     static constexpr int PER_WARP = SELF ? (STAGE_BYTES <= 4608 ? 4 : 2) : 1;
@@ -341,6 +349,8 @@ struct Q4Tile {
     static constexpr int NG = ROW / 32;            // groups (= scale bytes) per token
     static constexpr int NQL = NG / 4;             // 64-byte "quad loads" per token: 4 groups, one per lane of a quad
     static constexpr int GPH = D_IDX / 32;         // groups per head (2 or 4)
+    static constexpr bool IS_INT4 = FMT == SPOT_SELK_INT4_E4M3 || FMT == SPOT_SELK_INT4_BF16S;
+    static constexpr int SB = selk_scale_bytes_per_group(FMT);   // scale bytes per group (2: BF16 scales, R39)
     static_assert(GPH == 2 || GPH == 4, "d_idx must be 64 or 128 for the 4-bit scoring kernels");
     static_assert(NG % 4 == 0, "H_idx * d_idx must be a multiple of 128");
     uint32_t qf[NQL][16];
@@ -379,7 +389,7 @@ struct Q4Tile {
         if (mx > 0.f) sh = 14 - ilogbf(mx);
         sh = max(-100, min(100, sh));
         const float up = __uint_as_float((uint32_t)(127 + sh) << 23);
-        if (FMT == SPOT_SELK_INT4_E4M3) {
+        if (IS_INT4) {
             // (see unpack8) dims 2, 3, 6, 7 of every 8 go in divided by 16; the group offset 8 sum x, times 2^-24
             float xs = 0.f;
 #pragma unroll
@@ -423,7 +433,7 @@ struct Q4Tile {
             const int head = (4 * ql + 2 * (c & 1)) / GPH;
             wq[ql] = post[H + head];
             ps[ql] = post[head];
-            if (FMT == SPOT_SELK_INT4_E4M3) {
+            if (IS_INT4) {
                 cq[ql][0] = post[2 * H + 4 * ql + 2 * (c & 1)];
                 cq[ql][1] = post[2 * H + 4 * ql + 2 * (c & 1) + 1];
             }
@@ -446,7 +456,8 @@ struct Q4Tile {
 #pragma unroll
                 for (int ql = 0; ql < NQL; ++ql) {
                     cd[ql][hf] = lds128(st + tok * CPT + ql * 64 + c * 16);
-                    scw[hf][ql] = lds32(st + NIT * 16 * CPT + tok * NG + ql * 4);
+                    scw[hf][ql] = SB == 2 ? lds32(st + NIT * 16 * CPT + tok * NG * 2 + ql * 8 + 4 * (c & 1))   // this lane's two
+                                          : lds32(st + NIT * 16 * CPT + tok * NG + ql * 4);
                 }
             }
             float srow[2] = {0.f, 0.f};
@@ -469,8 +480,9 @@ struct Q4Tile {
                     const int gi = 2 * (c & 1);                        // first of this lane's two groups in the quad load
                     const uint32_t sw = scw[hf][ql];                   // scale bytes of groups 4ql .. 4ql+3
                     float s0, s1, d;
-                    if (FMT == SPOT_SELK_INT4_E4M3) {
-                        e4m3x2_to_f32x2((sw >> (8 * gi)) & 0xffffu, s0, s1);
+                    if (IS_INT4) {
+                        if (SB == 2) { s0 = __uint_as_float(sw << 16); s1 = __uint_as_float(sw & 0xffff0000u); }   // BF16 bits
+                        else e4m3x2_to_f32x2((sw >> (8 * gi)) & 0xffffu, s0, s1);
                         d = fmaf(acc[2 * hf] - cq[ql][0], s0, (acc[2 * hf + 1] - cq[ql][1]) * s1);
                     } else {
                         s0 = scale_to_f32<FMT>((sw >> (8 * gi)) & 0xffu);
@@ -485,6 +497,152 @@ struct Q4Tile {
                 }
             }
             // heads are split over quad lanes 0 and 1
+            const float sa = srow[0] + __shfl_xor_sync(0xffffffffu, srow[0], 1);
+            const float sb = srow[1] + __shfl_xor_sync(0xffffffffu, srow[1], 1);
+            const int ta = t0 + it * 16 + g, tbk = ta + 8;
+            m = group_update(m, sa, sb, ta < L, tbk < L, it0 + it, lane, fine);
+        }
+        return fine ? m : rows_max(m, lane);
+    }
+};
+
+// ---- MXINT8 tile (f2, R38): [tokens][ROW] offset-binary code bytes, then [tokens][ROW/32] E8M0 bytes ------------------
+// The Q4 scheme with 32 code bytes per group: a quad load is 128 bytes of a token (four groups), stored as two 64-byte
+// halves (quantize.cu: odd tokens keep them swapped), so that a lane's two 16-byte loads are bytes [0, 16) and [16, 32)
+// of its group and the loads of two adjacent token rows fall into different banks.
+template <int H, int D_IDX>
+struct Q8Tile {
+    static constexpr int ROW = H * D_IDX;
+    static constexpr int CPT = ROW;                // code bytes per token
+    static constexpr int NG = ROW / 32;            // groups (= scale bytes) per token
+    static constexpr int NQL = NG / 4;             // 128-byte quad loads per token
+    static constexpr int GPH = D_IDX / 32;
+    static_assert(GPH == 2 || GPH == 4, "d_idx must be 64 or 128 for the MXINT8 scoring kernel");
+    static_assert(NG % 4 == 0, "H_idx * d_idx must be a multiple of 128");
+    uint32_t qf[NQL][16];
+    float wq[NQL], ps[NQL];
+    float cq[NQL][2];                              // the offsets 128 sum x 2^-24 of this lane's two groups per quad load
+
+    static __device__ __forceinline__ void load_raw(const ScoreArgs& a, int b, int lane, QRaw& r) {
+        constexpr int EPL = ROW / 32;
+        static_assert(EPL / 8 <= 2, "two 16-byte chunks per lane");
+#pragma unroll
+        for (int i = 0; i < EPL / 8; ++i)
+            r.v[i] = *reinterpret_cast<const uint4*>(a.sel_q + (int64_t)b * ROW + lane * EPL + i * 8);
+        r.w = lane < H ? a.w[(int64_t)b * H + lane] : 0.f;
+    }
+    // slot: ROW halfs (the pre-scaled fp16 query) + H floats (power-of-two post-scales) + H floats (w) + NG floats (offsets)
+    static __device__ __forceinline__ void stage_raw(const QRaw& r, int lane, uint32_t q16_addr) {
+        __half* q16 = reinterpret_cast<__half*>(__cvta_shared_to_generic((size_t)q16_addr));
+        float* post = reinterpret_cast<float*>(q16 + ROW);
+        constexpr int EPL = ROW / 32, LPH = 32 / H;
+        static_assert(EPL % 8 == 0 && LPH * EPL == D_IDX && (LPH & (LPH - 1)) == 0, "query staging geometry");
+        __syncwarp();
+        float v[EPL], mx = 0.f;
+#pragma unroll
+        for (int i = 0; i < EPL / 8; ++i) {
+            const uint32_t wds[4] = {r.v[i].x, r.v[i].y, r.v[i].z, r.v[i].w};
+#pragma unroll
+            for (int j = 0; j < 4; ++j) { v[i * 8 + 2 * j] = bf16lo(wds[j]); v[i * 8 + 2 * j + 1] = bf16hi(wds[j]); }
+        }
+#pragma unroll
+        for (int i = 0; i < EPL; ++i) mx = fmaxf(mx, fabsf(v[i]));
+#pragma unroll
+        for (int o = LPH / 2; o; o >>= 1) mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, o));
+        int sh = 0;
+        if (mx > 0.f) sh = 14 - ilogbf(mx);
+        sh = max(-100, min(100, sh));
+        const float up = __uint_as_float((uint32_t)(127 + sh) << 23);
+        float xs = 0.f;
+#pragma unroll
+        for (int i = 0; i < EPL; ++i) {
+            const __half hq = __float2half_rn(v[i] * up);
+            q16[lane * EPL + i] = hq;
+            xs += __half2float(hq);
+        }
+        constexpr int LPG = 32 / EPL;                         // lanes per 32-element group
+#pragma unroll
+        for (int o = LPG / 2; o; o >>= 1) xs += __shfl_xor_sync(0xffffffffu, xs, o);
+        if (lane % LPG == 0) post[2 * H + lane / LPG] = xs * (128.0f * 5.9604644775390625e-08f);
+        // codes come in as u 2^-24 and mean code 2^-6: post-scale 2^(-sh + 24 - 6)
+        if (lane % LPH == 0) post[lane / LPH] = __uint_as_float((uint32_t)(127 - sh + 18) << 23);
+        if (lane < H) post[H + lane] = r.w;
+        __syncwarp();
+    }
+    __device__ __forceinline__ void fetch(int lane, uint32_t q16_addr) {
+        const int g = lane >> 2, c = lane & 3;
+        const __half* q16 = reinterpret_cast<const __half*>(__cvta_shared_to_generic((size_t)q16_addr));
+        const float* post = reinterpret_cast<const float*>(q16 + ROW);
+        // B fragments: column n of the MMA is the group held by quad-lane c == n; only lane (g == n, c == n) is non-zero
+#pragma unroll
+        for (int ql = 0; ql < NQL; ++ql) {
+            const uint4* src = reinterpret_cast<const uint4*>(q16 + (ql * 4 + c) * 32);
+#pragma unroll
+            for (int i = 0; i < 4; ++i) {
+                uint4 v = make_uint4(0, 0, 0, 0);
+                if (g == c) v = src[i];
+                qf[ql][4 * i + 0] = v.x; qf[ql][4 * i + 1] = v.y; qf[ql][4 * i + 2] = v.z; qf[ql][4 * i + 3] = v.w;
+            }
+        }
+#pragma unroll
+        for (int ql = 0; ql < NQL; ++ql) {
+            const int head = (4 * ql + 2 * (c & 1)) / GPH;
+            wq[ql] = post[H + head];
+            ps[ql] = post[head];
+            cq[ql][0] = post[2 * H + 4 * ql + 2 * (c & 1)];
+            cq[ql][1] = post[2 * H + 4 * ql + 2 * (c & 1) + 1];
+        }
+    }
+
+    template <int NIT>
+    __device__ __forceinline__ float part_max(uint32_t st, int t0, int L, int lane, bool fine, int it0) const {
+        const int g = lane >> 2, c = lane & 3;
+        const uint32_t first = (g & 1) ? 64u : 0u;            // where this token row keeps bytes [0, 16) of its groups
+        float m = -INFINITY;
+#pragma unroll 2
+        for (int it = 0; it < NIT; ++it) {
+            uint4 cd[NQL][2][2];
+            uint32_t scw[2][NQL];
+#pragma unroll
+            for (int hf = 0; hf < 2; ++hf) {
+                const int tok = it * 16 + hf * 8 + g;        // parity of tok == parity of g
+#pragma unroll
+                for (int ql = 0; ql < NQL; ++ql) {
+                    cd[ql][hf][0] = lds128(st + tok * CPT + ql * 128 + first + c * 16);
+                    cd[ql][hf][1] = lds128(st + tok * CPT + ql * 128 + (first ^ 64u) + c * 16);
+                    scw[hf][ql] = lds32(st + NIT * 16 * CPT + tok * NG + ql * 4);
+                }
+            }
+            float srow[2] = {0.f, 0.f};
+#pragma unroll
+            for (int ql = 0; ql < NQL; ++ql) {
+                float acc[4] = {0.f, 0.f, 0.f, 0.f};
+#pragma unroll
+                for (int hh = 0; hh < 2; ++hh) {
+                    const uint32_t wa[4] = {cd[ql][0][hh].x, cd[ql][0][hh].y, cd[ql][0][hh].z, cd[ql][0][hh].w};
+                    const uint32_t wb[4] = {cd[ql][1][hh].x, cd[ql][1][hh].y, cd[ql][1][hh].z, cd[ql][1][hh].w};
+#pragma unroll
+                    for (int wd = 0; wd < 4; ++wd) {
+                        // bytes (b0, b1) and (b2, b3) of the word as fp16 pairs 0x00b0, 0x00b1 | 0x00b2, 0x00b3
+                        const uint32_t a0 = __byte_perm(wa[wd], 0u, 0x4140), a2 = __byte_perm(wa[wd], 0u, 0x4342);
+                        const uint32_t a1 = __byte_perm(wb[wd], 0u, 0x4140), a3 = __byte_perm(wb[wd], 0u, 0x4342);
+                        mma_f16_16816(acc, a0, a1, a2, a3, qf[ql][8 * hh + 2 * wd], qf[ql][8 * hh + 2 * wd + 1]);
+                    }
+                }
+#pragma unroll
+                for (int hf = 0; hf < 2; ++hf) {
+                    const int gi = 2 * (c & 1);
+                    const uint32_t sw = scw[hf][ql];
+                    const float s0 = scale_to_f32<SPOT_SELK_MXINT8>((sw >> (8 * gi)) & 0xffu);
+                    const float s1 = scale_to_f32<SPOT_SELK_MXINT8>((sw >> (8 * (gi + 1))) & 0xffu);
+                    float d = fmaf(acc[2 * hf] - cq[ql][0], s0, (acc[2 * hf + 1] - cq[ql][1]) * s1);
+                    if (GPH == 4) d += __shfl_xor_sync(0xffffffffu, d, 1);
+                    d *= ps[ql];
+                    float contrib = wq[ql] * fmaxf(d, 0.f);
+                    if (GPH == 4 && (c & 1)) contrib = 0.f;
+                    srow[hf] += contrib;
+                }
+            }
             const float sa = srow[0] + __shfl_xor_sync(0xffffffffu, srow[0], 1);
             const float sb = srow[1] + __shfl_xor_sync(0xffffffffu, srow[1], 1);
             const int ta = t0 + it * 16 + g, tbk = ta + 8;
@@ -650,7 +808,8 @@ __global__ void __launch_bounds__((ScoreCfg<H, D_IDX, FMT>::THREADS), 1) score_d
     // this CTA's work list: its range of every group, in group order
     __shared__ CtaRange s_rng[SC_MAX_GROUPS];
     using TileT = typename std::conditional<FMT == SPOT_SELK_BF16, Bf16Tile<H, D_IDX>,
-                  typename std::conditional<FMT == SPOT_SELK_FP8_E4M3, Fp8Tile<H, D_IDX>, Q4Tile<H, D_IDX, FMT>>::type>::type;
+                  typename std::conditional<FMT == SPOT_SELK_FP8_E4M3, Fp8Tile<H, D_IDX>,
+                  typename std::conditional<FMT == SPOT_SELK_MXINT8, Q8Tile<H, D_IDX>, Q4Tile<H, D_IDX, FMT>>::type>::type>::type;
     // the two cold global reads in front of everything -- the sequence lengths and this warp's first query row -- go
     // out together
     const bool q_staged = a.B <= Cfg::Q_SLOTS;
@@ -710,7 +869,7 @@ __global__ void __launch_bounds__((ScoreCfg<H, D_IDX, FMT>::THREADS), 1) score_d
                               bar_full + 8 * s);
                 } else {
                     // 4-bit slice: the slice's code rows, then its scale rows (they sit behind all 64 code rows)
-                    constexpr int NTOK = 64 / SP, CODES = NTOK * (Cfg::ROW / 2), SCALES = NTOK * (Cfg::ROW / 32);
+                    constexpr int NTOK = 64 / SP, CODES = NTOK * Cfg::CODE_BYTES, SCALES = NTOK * Cfg::SCALE_BYTES;
                     static_assert(CODES + SCALES == Cfg::STAGE_BYTES && SCALES % 16 == 0, "4-bit slice geometry");
                     bulk_load(ring + s * Cfg::STAGE_BYTES, tile_src + (rq % SP) * CODES, CODES, bar_full + 8 * s);
                     bulk_load(ring + s * Cfg::STAGE_BYTES + CODES, tile_src + SP * CODES + (rq % SP) * SCALES, SCALES,
@@ -845,6 +1004,9 @@ spot_status launch_score(const spot_select_params* p, float* scores, int nb_stri
     if (p->fmt == SPOT_SELK_MXFP4) return launch_score_fmt<H, D_IDX, SPOT_SELK_MXFP4>(p, scores, nb_stride, sync, reserve_sms, s);
     if (p->fmt == SPOT_SELK_FP8_E4M3)
         return launch_score_fmt<H, D_IDX, SPOT_SELK_FP8_E4M3>(p, scores, nb_stride, sync, reserve_sms, s);
+    if (p->fmt == SPOT_SELK_MXINT8) return launch_score_fmt<H, D_IDX, SPOT_SELK_MXINT8>(p, scores, nb_stride, sync, reserve_sms, s);
+    if (p->fmt == SPOT_SELK_INT4_BF16S)
+        return launch_score_fmt<H, D_IDX, SPOT_SELK_INT4_BF16S>(p, scores, nb_stride, sync, reserve_sms, s);
     return launch_score_fmt<H, D_IDX, SPOT_SELK_INT4_E4M3>(p, scores, nb_stride, sync, reserve_sms, s);
 }
 

@@ -140,6 +140,19 @@ class DeviceDecode:
 # oracle side
 # ------------------------------------------------------------------------------------------------------
 
+def oracle_dequantised_view(fmt, k_bits):
+    """What spot_dequantize_selector_k must return for BF16 keys k_bits stored in format fmt, as float64: the oracle's
+    dequantised keys -- exactly BF16 numbers for every format but int4_bf16s, whose exact values q * s the call returns
+    rounded to nearest-even BF16 (R39; the rounding is the workloads' converter, no method arithmetic)."""
+    from workloads import f32_to_bf16_bits
+    want = OQ.quantize_dequantize(fmt, k_bits)
+    if fmt == "int4_bf16s":
+        w32 = want.astype(np.float32)
+        assert np.array_equal(w32.astype(np.float64), want)
+        want = bf16_bits_to_f64(f32_to_bf16_bits(w32))
+    return want
+
+
 def oracle_keys(wl, fmt, b):
     """fp64 selector keys of sequence b as the given cache format stores them."""
     return OQ.quantize_dequantize(fmt, wl.sel_k[b])

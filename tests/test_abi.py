@@ -65,6 +65,8 @@ def test_selector_k_bytes_matches_the_papers_footprint(lib):
     # the measured geometry: 4 x 64, 136 B per token
     assert api.spot_selector_k_bytes("mxfp4", 4, 131072, 4, 64) == 4 * 131072 * 136
     assert api.spot_selector_k_bytes("fp8_e4m3", 1, n_tok, 4, 128) * 2 == bf16           # f2: the paper's 0.5x
+    assert api.spot_selector_k_bytes("mxint8", 1, n_tok, 4, 128) * 32 == bf16 // 2 * 33   # 8.25 bit/elt (R38)
+    assert api.spot_selector_k_bytes("int4_bf16s", 1, n_tok, 4, 128) * 32 == bf16 * 9     # 4.5 bit/elt: PAPER.md:188 (R39)
     # invalid: unknown format, d_idx not a multiple of 32, capacity not a multiple of the 64-token tile
     assert lib.spot_selector_k_bytes(7, 1, 64, 4, 64) == 0
     assert api.spot_selector_k_bytes("mxfp4", 1, 64, 4, 48) == 0
@@ -104,6 +106,9 @@ def test_select_argument_errors_are_caught_on_the_host(lib):
     assert lib.spot_select_workspace_bytes(C.byref(_select_params(blk=16, cap=256, nb_stride=256))) >= 2 * 256 * 4
     assert lib.spot_select_workspace_bytes(C.byref(_select_params(blk=16, cap=256, nb_stride=256, q_block=64, Tq=64,
                                                                   seq_len=None))) > 0            # f3: prefill rows too
+    # INT4 with BF16 group scales (f2, R39) is a decode-row format: its keys are not BF16 numbers, prefill rows are refused
+    assert lib.spot_select_workspace_bytes(C.byref(_select_params(fmt=5))) > 0
+    assert lib.spot_select(C.byref(_select_params(fmt=5, q_block=64, Tq=128, seq_len=None)), None) == UNSUPPORTED
     assert lib.spot_select(None, None) == INVALID
     assert lib.spot_score_blocks(C.byref(_select_params()), None) == INVALID        # block_scores is required
     # a score-only block (what spot_score_blocks reads: no indices / budgets / cap) can size its own workspace -- a
@@ -159,7 +164,7 @@ def test_quantize_argument_errors(lib):
     assert f(None, 0x2000, 2, 1, 64, 0, 64, 4, 64, None) == INVALID
     assert f(0x1000, 0x2000, 2, 1, 64, 0, 64, 4, 48, None) == INVALID           # d_idx % 32
     assert f(0x1000, 0x2000, 2, 1, 64, 64, 64, 4, 64, None) == INVALID          # past the capacity
-    assert f(0x1000, 0x2000, 5, 1, 64, 0, 64, 4, 64, None) == INVALID           # unknown format
+    assert f(0x1000, 0x2000, 6, 1, 64, 0, 64, 4, 64, None) == INVALID           # unknown format
     assert lib.spot_dequantize_selector_k(0x1000, None, 2, 1, 64, 0, 64, 4, 64, None) == INVALID
 
 

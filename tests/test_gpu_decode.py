@@ -26,7 +26,7 @@ def torch_cuda():
 
 
 # ---------------------------------------------------------------- a0 quantisers
-@pytest.mark.parametrize("fmt", ["mxfp4", "int4_e4m3", "fp8_e4m3"])
+@pytest.mark.parametrize("fmt", ["mxfp4", "int4_e4m3", "fp8_e4m3", "mxint8", "int4_bf16s"])
 def test_quantise_dequantise_bit_exact(torch_cuda, fmt):
     torch = torch_cuda
     from paper_2606_22874_b200 import api
@@ -39,6 +39,9 @@ def test_quantise_dequantise_bit_exact(torch_cuda, fmt):
     x[0, 3, 0, :8] = [-0.0, 0.25, 0.75, 1.25, 1.75, 2.5, 3.5, 5.0]      # E2M1 ties (with amax 6 -> X = 1)
     x[0, 3, 0, 8] = 6.0
     x[0, 4, 0, :32] = np.arange(-16, 16) * 0.5              # INT4 ties at .5
+    x[0, 5, 0, :32] = [1.5] + [(2 * i + 1) / 128.0 * (-1) ** i for i in range(31)]     # MXINT8 ties (step 1/64 at amax 1.5)
+    x[0, 6, 0, :4] = [255 / 128.0, -255 / 128.0, 1.984375, -1.0]                       # MXINT8: 127.5 -> 128 -> clamp 127
+    x[0, 7, 0, :32] = 2.0 ** -133                           # smallest BF16 subnormal: scales clamp / bump
     from workloads import f32_to_bf16_bits
     bits = f32_to_bf16_bits(x).reshape(B, L, Hh, d)
     k = H.dev_u16(bits)
@@ -51,6 +54,17 @@ def test_quantise_dequantise_bit_exact(torch_cuda, fmt):
     torch.cuda.synchronize()
     got = bf16_bits_to_f64(H.to_np_u16(out))
     want = OQ.quantize_dequantize(fmt, bits)
+    if fmt == "int4_bf16s":
+        # R39: q * s carries up to 11 significant bits; the call returns its round-to-nearest-even BF16 view.  The oracle's
+        # exact values are rounded the same way here (workloads' converter, no method arithmetic); elements with
+        # |q| in {1, 2, 4} are the scale times a power of two and pass through unrounded, so the scale bits are compared too
+        want32 = want.astype(np.float32)
+        assert np.array_equal(want32.astype(np.float64), want)          # exact in binary32
+        want = bf16_bits_to_f64(f32_to_bf16_bits(want32))
+        q, sb = OQ.quantize_int4_bf16s(bits)
+        unrounded = np.isin(np.abs(q), (1, 2, 4))
+        assert unrounded.reshape(B, L, Hh, d // 32, 32).any(-1).mean() > 0.99
+        assert np.array_equal(got[unrounded], OQ.dequantize_int4_bf16s(q, sb)[unrounded])
     assert np.array_equal(got, want)                        # numeric equality: +0 == -0, everything else bit-exact
     assert cache.numel() == OQ.selector_k_bytes(fmt, B * L * Hh * d)
 
@@ -74,7 +88,7 @@ def _check_select(dd, fmt, report, **over):
     return idx, bud
 
 
-@pytest.mark.parametrize("fmt", ["bf16", "mxfp4", "int4_e4m3", "fp8_e4m3"])
+@pytest.mark.parametrize("fmt", ["bf16", "mxfp4", "int4_e4m3", "fp8_e4m3", "mxint8", "int4_bf16s"])
 @pytest.mark.parametrize("cfg", ["cfg1", "mini2", "mini3", "mini4"])
 def test_select_matches_oracle(torch_cuda, cfg, fmt):
     wl = make_config(cfg, with_kv=False)
@@ -219,6 +233,8 @@ def test_end_to_end_step_matches_oracle(torch_cuda):
                                           ("cfg4_b1", "mxfp4", (0,)), ("cfg4_b16", "mxfp4", (0, 5, 10, 15)),
                                           ("cfg3/d128", "bf16", (1,)), ("cfg3/d128", "mxfp4", (2,)),
                                           ("cfg3", "fp8_e4m3", (3,)), ("cfg3/d128", "fp8_e4m3", (0,)),
+                                          ("cfg3", "mxint8", (0,)), ("cfg3/d128", "mxint8", (3,)),
+                                          ("cfg3", "int4_bf16s", (1,)), ("cfg3/d128", "int4_bf16s", (2,)),
                                           ("cfg3/blk16", "bf16", (2,)), ("cfg3/blk16/d128", "mxfp4", (0,))])
 def test_full_size_configs_in_the_bench_configuration(torch_cuda, cfg, fmt, seqs):
     """BASELINE.json configs 2, 3 and 4 (its whole batch sweep 1 / 4 / 16) at full size (config 3: B=4, L=131072, 2048
@@ -416,7 +432,7 @@ def test_decode_step_is_capturable_in_a_cuda_graph(torch_cuda):
 F3 = dict(blk=16, sink_blocks=8, recency_blocks=16, kmin_blocks=32)
 
 
-@pytest.mark.parametrize("fmt", ["bf16", "mxfp4", "int4_e4m3", "fp8_e4m3"])
+@pytest.mark.parametrize("fmt", ["bf16", "mxfp4", "int4_e4m3", "fp8_e4m3", "mxint8", "int4_bf16s"])
 @pytest.mark.parametrize("cfg", ["mini2", "mini4"])
 def test_block16_select_matches_oracle(torch_cuda, cfg, fmt):
     """Four block maxima per 64-token tile, 4x the blocks per row (512 here), the paper's reserved tiers."""
@@ -437,7 +453,7 @@ def test_block16_select_edge_cases_and_long_rows(torch_cuda):
     for seed, L, seqs, d_idx in [(11, 64, [1, 17, 64], 64), (12, 320, [65, 129, 307], 64), (13, 2048, [2048, 1999, 777], 128)]:
         wl = make_decode_workload("e16_%d" % seed, seed, B=3, L=L, kind="gauss", seq_lens=seqs, d_idx=d_idx,
                                   with_kv=False, blk=16)
-        for fmt in ("bf16", "mxfp4", "fp8_e4m3"):
+        for fmt in ("bf16", "mxfp4", "fp8_e4m3", "mxint8", "int4_bf16s"):
             dd = H.DeviceDecode(wl, fmt, with_kv=False)
             report = []
             for over in (dict(), dict(sink_blocks=8, recency_blocks=16, kmin_blocks=32), dict(mode="topk", top_k=5)):
@@ -521,7 +537,7 @@ def test_paged_kv_decode_attention(torch_cuda, blk, page_tokens, layout):
 
 
 # ---------------------------------------------------------------- f2: quantised selector queries (decode)
-@pytest.mark.parametrize("fmt", ["mxfp4", "int4_e4m3", "fp8_e4m3"])
+@pytest.mark.parametrize("fmt", ["mxfp4", "int4_e4m3", "fp8_e4m3", "mxint8"])
 def test_quantised_query_through_the_cache_quantiser(torch_cuda, fmt):
     """PAPER.md:115 / :186 quantise the selector's queries as well as its key cache.  Every value these quantisers
     produce is exactly a BF16 number, so a quantised query is the BF16 query passed through spot_quantize_selector_k /

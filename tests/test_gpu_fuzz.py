@@ -33,6 +33,8 @@ def test_fuzz_selection(torch_cuda, chunk):
     for case in range(chunk * 30, chunk * 30 + 30):
         wl = _random_workload(rng, case, with_kv=False)
         fmt = str(rng.choice(["bf16", "mxfp4", "int4_e4m3", "fp8_e4m3"]))
+        if case % 5 == 4:                    # f2 formats of round 2 (drawn apart: the older cases keep their formats)
+            fmt = ("mxint8", "int4_bf16s")[(case // 5) % 2]
         dd = H.DeviceDecode(wl, fmt, with_kv=False)
         _check_select(dd, fmt, report)
         n_b = dd.n_b_max

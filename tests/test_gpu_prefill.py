@@ -69,7 +69,22 @@ def test_prefill_scores_and_selection(torch_cuda, L, q_start, Tq, B, over):
     print("prefill select L=%d q_start=%d Tq=%d: %d near-tie rows %s" % (L, q_start, Tq, len(report), report[:4]))
 
 
-@pytest.mark.parametrize("fmt", ["mxfp4", "int4_e4m3", "fp8_e4m3"])
+def test_prefill_over_int4_with_bf16_scales_is_refused(torch_cuda):
+    """R39: the keys of SPOT_SELK_INT4_BF16S are not BF16 numbers, and the prefill form would score their BF16 view --
+    spot_select / spot_score_blocks say UNSUPPORTED for q_block = 64 instead of rounding silently."""
+    torch = torch_cuda
+    from paper_2606_22874_b200 import api
+    wls = [make_prefill_workload(seed=6100, L=256, with_kv=False)]
+    dp = H.DevicePrefill(wls, 0, 256, with_kv=False)
+    dp.set_cache_format("mxint8")            # a cache of the right size class; the call must refuse before reading it
+    dp.sel_k = torch.zeros(api.spot_selector_k_bytes("int4_bf16s", 1, 256, dp.wl.H_idx, dp.wl.d_idx), dtype=torch.uint8,
+                           device="cuda")
+    dp.fmt = "int4_bf16s"
+    with pytest.raises(RuntimeError, match="UNSUPPORTED"):
+        dp.select()
+
+
+@pytest.mark.parametrize("fmt", ["mxfp4", "int4_e4m3", "fp8_e4m3", "mxint8"])
 def test_prefill_selection_over_a_quantised_cache(torch_cuda, fmt):
     """f2: a later chunk (batch of 2, odd number of query blocks) scored against a quantised selector cache -- the
     library dequantises the visible prefix into its workspace and runs the BF16 tile-score GEMM; the oracle scores the

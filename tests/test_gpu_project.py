@@ -16,6 +16,8 @@ from workloads import f32_to_bf16_bits, make_project_workload
 
 pytestmark = pytest.mark.gpu
 
+FMTS = ("bf16", "mxfp4", "int4_e4m3", "fp8_e4m3", "mxint8", "int4_bf16s")
+
 
 @pytest.fixture(scope="module")
 def torch_cuda():
@@ -63,7 +65,7 @@ def test_project_rope_append(torch_cuda, B, d_model, d_idx, rope_dims):
     cache_init = f32_to_bf16_bits(rng.standard_normal((B, stride, Hh, d_idx), dtype=np.float32))
     # the kernel takes ONE position per sequence (rotation angle and cache slot); run it per role
     res = {}
-    for fmt in ("bf16", "mxfp4", "int4_e4m3", "fp8_e4m3"):
+    for fmt in FMTS:
         wl_f = dict(wl)
         wl_f["pos"] = slot.astype(np.int32)
         res[fmt] = _run(torch, wl_f, fmt, stride, rope_dims, base, cache_init)
@@ -79,14 +81,14 @@ def test_project_rope_append(torch_cuda, B, d_model, d_idx, rope_dims):
             exact += int(np.sum(got == bf16_bits_to_f64(f32_to_bf16_bits(ref.astype(np.float32)))))
             total += ref.size
         assert np.allclose(w_gpu[b], w_ref, rtol=1e-5, atol=1e-6)
-        for fmt in ("bf16", "mxfp4", "int4_e4m3", "fp8_e4m3"):
+        for fmt in FMTS:
             q_f, w_f, back = res[fmt]
             assert np.array_equal(q_f, q_gpu) and np.array_equal(w_f, w_gpu)          # format-independent outputs
-            want_slot = OQ.quantize_dequantize(fmt, k_gpu_bits)
+            want_slot = H.oracle_dequantised_view(fmt, k_gpu_bits)
             assert np.array_equal(bf16_bits_to_f64(back[b, slot[b]]), want_slot), (fmt, b)
             others = np.ones(stride, dtype=bool)
             others[slot[b]] = False
-            assert np.array_equal(bf16_bits_to_f64(back[b, others]), OQ.quantize_dequantize(fmt, cache_init[b, others]))
+            assert np.array_equal(bf16_bits_to_f64(back[b, others]), H.oracle_dequantised_view(fmt, cache_init[b, others]))
     assert exact >= 0.99 * total, (exact, total)
 
 

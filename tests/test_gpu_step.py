@@ -40,7 +40,8 @@ def _check_step(dd, fmt, idx, bud, out, lse, every=1, **over):
 
 @pytest.mark.parametrize("cfg,fmt,over", [("cfg1", "bf16", {}), ("mini2", "bf16", {}), ("mini2", "mxfp4", {}),
                                           ("mini4", "int4_e4m3", {}), ("mini4", "fp8_e4m3", {}), ("mini3", "bf16", {}),
-                                          ("mini2", "bf16", F3), ("mini4", "mxfp4", F3)])
+                                          ("mini2", "bf16", F3), ("mini4", "mxfp4", F3),
+                                          ("mini2", "mxint8", {}), ("mini4", "int4_bf16s", F3)])
 def test_step_matches_oracle(torch_cuda, cfg, fmt, over):
     from paper_2606_22874_b200 import api
     wl = make_config(cfg, **over)
