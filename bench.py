@@ -642,12 +642,12 @@ def run_prefill(args):
     sel_q_in, q_fmt = sel_q, "bf16"
     if args.qfmt != "bf16":
         # f2: the queries quantised too -- FP8 x FP8 tile scores on the tensor cores, no dequantise pass (spot.h, q_fmt)
-        assert args.fmt == args.qfmt == "fp8_e4m3", "--qfmt fp8_e4m3 needs --fmt fp8_e4m3"
+        assert args.fmt == args.qfmt and args.qfmt in ("fp8_e4m3", "mxfp4"), "--qfmt X needs --fmt X (fp8_e4m3 or mxfp4)"
         sel_q_in = torch.zeros(api.spot_selector_k_bytes(args.qfmt, 1, L, wl.H_idx, wl.d_idx), dtype=torch.uint8, device=dev)
         api.spot_quantize_selector_k(sel_q, sel_q_in, args.qfmt, 1, L, 0, L, wl.H_idx, wl.d_idx)
         q_fmt = args.qfmt
     f8 = q_fmt != "bf16"
-    tc_ratio = 2.0 if f8 else 1.0          # a contraction takes the peak of its own dtype
+    tc_ratio = {"bf16": 1.0, "fp8_e4m3": 2.0, "mxfp4": 4.0}[q_fmt]         # a contraction takes the peak of its own dtype
     cap = n_kb
     nb_stride = (n_kb + 3) & ~3
     indices = torch.empty((n_qb, cap), dtype=torch.int32, device=dev)
@@ -775,7 +775,7 @@ def run_prefill(args):
     line = {
         "metric": PF_METRIC, "value": step_mean, "unit": "ms/layer", "n_gpus": world, "steps": args.steps,
         "warmup": W, "ms_per_step": step_mean, "higher_is_better": False, "scaling": "weak", "vs_baseline": None,
-        "dtype": "bf16" if not f8 else "bf16 (attention), fp8_e4m3 x fp8_e4m3 -> fp32 (tile scores)", "data": "synthetic",
+        "dtype": "bf16" if not f8 else "bf16 (attention), %s x %s -> fp32 (tile scores)" % (q_fmt, q_fmt), "data": "synthetic",
         "config": {"workload": "cfg5", "B": 1, "L": L, "H_q": Hq, "H_kv": Hkv, "D": D,
                    "selector": "%dx%d %s" % (wl.H_idx, wl.d_idx, args.fmt), "selector_queries": q_fmt, "blk": blk, "q_block": 64,
                    "kv_layout": ("paged, %d tokens per page, random table" % max(args.paged, 64)) if args.paged else "[B][H_kv][L][D]", "mode": wl.mode, "p": args.p,
@@ -788,11 +788,11 @@ def run_prefill(args):
                          "sparse causal attention": float(att_ms.mean()),
                          "dense causal attention (same kernel, every block)": float(np.mean(den))},
         "attention_tflops": att_flop / (float(att_ms.mean()) * 1e-3) / 1e12,
-        "roofline": {"bound": "tensor", "kernel": "score_prefill_kernel" + ("<.., fp8 x fp8>" if f8 else ""),
+        "roofline": {"bound": "tensor", "kernel": "score_prefill_kernel" + ("<.., %s x %s>" % (q_fmt, q_fmt) if f8 else ""),
                      "achieved": achieved, "peak": burst * tc_ratio, "unit": "TFLOP/s", "frac": achieved / (burst * tc_ratio),
                      "frac_of_sustained": achieved / (sustained * tc_ratio), "traffic": traffic,
-                     "peak_source": peak_src + (" x 2: the guide's nominal fp8 : bf16 ratio (4.5 : 2.25 PFLOP/s); no fp8 "
-                                                "peak is measured on this pool" if f8 else ""),
+                     "peak_source": peak_src + ((" x %g: the guide's nominal %s : bf16 ratio (%g : 2.25 PFLOP/s); no such "
+                                                 "peak is measured on this pool") % (tc_ratio, q_fmt, 2.25 * tc_ratio) if f8 else ""),
                      "algorithmic_flops": gemm_flop},
         "cpu_baseline": {"value": cpu_t / cpu_tiles * tiles * 1e3, "unit": "ms/layer",
                          "cores": len(os.sched_getaffinity(0)), "kind": "oracle",
@@ -935,7 +935,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="cfg3")
     ap.add_argument("--fmt", default="bf16", choices=["bf16", "mxfp4", "int4_e4m3", "fp8_e4m3", "mxint8", "int4_bf16s"])
-    ap.add_argument("--qfmt", default="bf16", choices=["bf16", "fp8_e4m3"],
+    ap.add_argument("--qfmt", default="bf16", choices=["bf16", "fp8_e4m3", "mxfp4"],
                     help="cfg5 only: format of the selector QUERIES (fp8_e4m3 with --fmt fp8_e4m3: FP8 x FP8 tensor-core scoring)")
     ap.add_argument("--p", type=float, default=0.90)
     ap.add_argument("--L", type=int, default=0, help="cfg5 only: prompt length (default 65536)")

@@ -206,7 +206,11 @@ typedef struct {
      * spot_quantize_selector_k writes for a cache of Tq tokens), accepted with fmt == SPOT_SELK_FP8_E4M3 and q_block == 64
      * only (SPOT_ERR_UNSUPPORTED otherwise): the tile scores are then FP8 x FP8 products accumulated in fp32 by
      * tcgen05.mma kind::f8f6f4 straight from the cache -- no dequantise pass, no BF16 scratch.  The result is the score of
-     * the two dequantised images (R33). */
+     * the two dequantised images (R33).  SPOT_SELK_MXFP4: sel_q is an MXFP4 cache of Tq tokens per sequence
+     * (spot_quantize_selector_k with cache_stride_tokens = Tq; spot_selector_k_bytes(MXFP4, B, Tq, ..) bytes), accepted
+     * with fmt == SPOT_SELK_MXFP4 and q_block == 64 only: E2M1 x E2M1 products times the two groups' UE8M0 scales,
+     * accumulated in fp32 by tcgen05.mma kind::mxf4.block_scale (group scales through tensor memory), again straight from
+     * the opaque cache layout and with the score of the two dequantised images as the result. */
     int32_t q_fmt;
 } spot_select_params;
 

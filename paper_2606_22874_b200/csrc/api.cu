@@ -38,7 +38,7 @@ int sm_count() {
 // kernels implemented in the other translation units
 spot_status score_decode(const spot_select_params* p, float* scores, int nb_stride, const StepSync* sync, int reserve_sms,
                          cudaStream_t s);
-spot_status score_prefill(const spot_select_params* p, float* scores, int nb_stride, bool fp8, cudaStream_t s);
+spot_status score_prefill(const spot_select_params* p, float* scores, int nb_stride, int q_fmt, cudaStream_t s);
 spot_status run_select(const spot_select_params* p, const float* scores, int nb_stride, int rows_per_seq, int max_nb,
                        const StepSync* sync, cudaStream_t s);
 spot_status attn_decode_piped(const spot_attn_params* p, const StepSync* sync, cudaStream_t s);     // attn_decode.cu
@@ -69,8 +69,9 @@ spot_status select_geometry(const spot_select_params* p, SelectGeom* g, bool sco
     if (p->fmt != SPOT_SELK_BF16 && p->cache_stride_tokens % SELK_TILE != 0)
         return SPOT_ERR_INVALID_ARG;
     // quantised selector queries on the tensor cores (f2): FP8-E4M3 queries against the FP8-E4M3 cache, prefill rows only
-    if (p->q_fmt != SPOT_SELK_BF16 && p->q_fmt != SPOT_SELK_FP8_E4M3) return SPOT_ERR_INVALID_ARG;
-    if (p->q_fmt == SPOT_SELK_FP8_E4M3 && (p->fmt != SPOT_SELK_FP8_E4M3 || p->q_block != 64)) return SPOT_ERR_UNSUPPORTED;
+    // (and, round 2, MXFP4 queries -- a cache of Tq tokens per sequence -- against the MXFP4 cache, block-scaled)
+    if (p->q_fmt != SPOT_SELK_BF16 && p->q_fmt != SPOT_SELK_FP8_E4M3 && p->q_fmt != SPOT_SELK_MXFP4) return SPOT_ERR_INVALID_ARG;
+    if (p->q_fmt != SPOT_SELK_BF16 && (p->fmt != p->q_fmt || p->q_block != 64)) return SPOT_ERR_UNSUPPORTED;
     // INT4 with BF16 group scales: its keys q * s are not BF16 numbers (R39), and the prefill form would score their
     // dequantised BF16 view -- decode rows only
     if (p->fmt == SPOT_SELK_INT4_BF16S && p->q_block != 1) return SPOT_ERR_UNSUPPORTED;
@@ -105,7 +106,7 @@ spot_status select_geometry(const spot_select_params* p, SelectGeom* g, bool sco
 // the BF16 tile-score GEMM runs on that (every dequantised value is exactly a BF16 number).  What the paper's own
 // kernels do ("dequantisation overhead"); a fused unpack inside the GEMM's operand path is the next form.
 size_t prefill_scratch_bytes(const spot_select_params* p) {
-    if (p->q_block == 1 || p->fmt == SPOT_SELK_BF16 || p->q_fmt == SPOT_SELK_FP8_E4M3) return 0;
+    if (p->q_block == 1 || p->fmt == SPOT_SELK_BF16 || p->q_fmt != SPOT_SELK_BF16) return 0;
     return 256 + (size_t)p->B * ((size_t)p->q_start + p->Tq) * p->H_idx * p->d_idx * 2;
 }
 
@@ -145,8 +146,9 @@ int reserve_for_select(int B) { return B < 8 ? B : 8; }
 spot_status score_any(const spot_select_params* p, float* scores, int nb_stride, void* scratch_area, const StepSync* sync,
                       cudaStream_t s) {
     if (p->q_block == 1) return score_decode(p, scores, nb_stride, sync, sync ? reserve_for_select(p->B) : 0, s);
-    if (p->q_fmt == SPOT_SELK_FP8_E4M3) return score_prefill(p, scores, nb_stride, true, s);   // FP8 x FP8, no dequantise pass
-    if (p->fmt == SPOT_SELK_BF16) return score_prefill(p, scores, nb_stride, false, s);
+    // FP8 x FP8 / MXFP4 x MXFP4: straight from the cache layouts, no dequantise pass
+    if (p->q_fmt == SPOT_SELK_FP8_E4M3 || p->q_fmt == SPOT_SELK_MXFP4) return score_prefill(p, scores, nb_stride, p->q_fmt, s);
+    if (p->fmt == SPOT_SELK_BF16) return score_prefill(p, scores, nb_stride, SPOT_SELK_BF16, s);
     uint16_t* deq = reinterpret_cast<uint16_t*>((reinterpret_cast<uintptr_t>(scratch_area) + 255) & ~(uintptr_t)255);
     const int tok = p->q_start + p->Tq;
     spot_status st = spot_dequantize_selector_k(p->sel_k, deq, (spot_selk_format)p->fmt, p->B, tok, 0, p->cache_stride_tokens, p->H_idx,
@@ -154,7 +156,7 @@ spot_status score_any(const spot_select_params* p, float* scores, int nb_stride,
     if (st != SPOT_OK) return st;
     spot_select_params q = *p;
     q.sel_k = deq; q.fmt = SPOT_SELK_BF16; q.cache_stride_tokens = tok;
-    return score_prefill(&q, scores, nb_stride, false, s);
+    return score_prefill(&q, scores, nb_stride, SPOT_SELK_BF16, s);
 }
 
 }  // namespace

@@ -34,7 +34,6 @@ constexpr int PF_M = 128;               // queries per tile (two 64-query blocks
 constexpr int PF_N = 128;               // keys per MMA (two 64-key blocks)
 constexpr int PF_CHUNK = 32;            // key blocks per work item
 constexpr int PF_EPI_WARPS = 8;
-constexpr int PF_THREADS = (PF_EPI_WARPS + 2) * 32;
 constexpr uint32_t PF_PLANE_BYTES = 128 * 64 * 2;          // [128 rows][64 d] BF16: one 128-byte swizzle row per token
 constexpr uint32_t PF_SMEM_MISC = 2048;        // barriers, TMEM slot, tile maxima [CHUNK][4 quarters][2 query blocks]
 
@@ -61,23 +60,46 @@ constexpr uint32_t PF_SMEM_MISC = 2048;        // barriers, TMEM slot, tile maxi
 // query tiles sharing every key load by TMA multicast, a key ring of ten 16 KiB single-head slots, sixteen epilogue warps,
 // and both fp32 pipes inside every head (element 0 of a pair through FADD, element 1 through FMNMX) were all measured
 // equal or slower.
-template <int HB, bool F8>
+// MX4 (f2, round 2): both operands are MXFP4 straight from the opaque cache layout (quantize.cu) -- a token row of packed
+// E2M1 codes is PF_H * HB bytes with HB = 32 (d_idx 64) or 64 (d_idx 128), one 128-byte swizzle row per 128 bytes, and
+// `tcgen05.mma kind::mxf4.block_scale.block32` multiplies in the UE8M0 group scales itself (K = 64 elements = 32 bytes per
+// instruction, two scales per row and instruction).  The scales travel beside the codes (plain bulk copies of the tiles'
+// scale rows into the tail of the slot) and four extra warps (one per TMEM lane quarter) move them into tensor memory in
+// the layout the MMA reads (tc100.cuh) -- 16 columns for the query tile, 16 per key slot, which leaves room for a ring of
+// THREE accumulators.
+constexpr int PF_BF16 = 0, PF_F8 = 1, PF_MX4 = 2;
+template <int HB, int KIND>
 struct PfCfg {
-    static_assert(HB == 64 || HB == 128 || HB == 256, "head row of 64, 128 or 256 bytes");
-    static_assert(!(F8 && HB == 256) && !(!F8 && HB == 64), "BF16: d_idx 64 / 128; FP8: d_idx 64 / 128");
+    static constexpr bool F8 = KIND == PF_F8, MX4 = KIND == PF_MX4;
+    static_assert(HB == 32 || HB == 64 || HB == 128 || HB == 256, "head row of 32, 64, 128 or 256 bytes");
+    static_assert(MX4 ? (HB == 32 || HB == 64) : F8 ? (HB == 64 || HB == 128) : (HB == 128 || HB == 256),
+                  "BF16: d_idx 64 / 128; FP8: d_idx 64 / 128; MXFP4: d_idx 64 / 128");
     static constexpr int PLANES = PF_H * HB / 128;                        // planes per token row
     static constexpr int KSTEPS = HB / 32;                                // 32-byte k-steps per head
     static constexpr bool PER_HEAD = HB == 256;                           // K ring granularity
     static constexpr int HEAD_PLANES = HB / 128;                          // planes per head (PER_HEAD only)
     static constexpr int STAGE_PLANES = PER_HEAD ? HEAD_PLANES : PLANES;  // planes of one K ring slot
-    static constexpr uint32_t Q_TILE_BYTES = PLANES * PF_PLANE_BYTES;
-    static constexpr uint32_t K_STAGE_BYTES = STAGE_PLANES * PF_PLANE_BYTES;
-    static constexpr int KSTAGES = (int)((224u * 1024u - Q_TILE_BYTES) / K_STAGE_BYTES);   // 2 / 3 / 6
+    static constexpr int NG = MX4 ? PF_H * HB / 16 : 0;                   // MX4: scale bytes per token (8 / 16)
+    static constexpr uint32_t SF_BYTES = MX4 ? 2048u : 0u;                // room for [128 rows][NG] scale bytes behind the codes
+    static constexpr uint32_t Q_CODE_BYTES = PLANES * PF_PLANE_BYTES;
+    static constexpr uint32_t K_CODE_BYTES = STAGE_PLANES * PF_PLANE_BYTES;
+    static constexpr uint32_t Q_TILE_BYTES = Q_CODE_BYTES + SF_BYTES;
+    static constexpr uint32_t K_STAGE_BYTES = K_CODE_BYTES + SF_BYTES;
+    static constexpr int KSTAGES = MX4 ? 4 : (int)((224u * 1024u - Q_TILE_BYTES) / K_STAGE_BYTES);   // 2 / 3 / 6
     static_assert(KSTAGES >= 2 && KSTAGES <= 8, "key ring");
     static constexpr uint32_t SMEM_TILES = Q_TILE_BYTES + KSTAGES * K_STAGE_BYTES;
     static constexpr uint32_t SMEM_BYTES = 1024 + SMEM_TILES + PF_SMEM_MISC;   // 1024: manual alignment slack
     static_assert(SMEM_BYTES <= 227 * 1024, "shared memory");
-    static constexpr int NACC = 512 / PF_N;                               // TMEM: a ring of four 128-column accumulators
+    // (three accumulators instead of four cost the FP8 kernel 6 %: 1.065 against 1.004 ms at cfg5)
+    static constexpr int NACC = MX4 ? 3 : 512 / PF_N;                     // TMEM: a ring of 128-column accumulators
+    static constexpr int SF_WARPS = MX4 ? 4 : 0;
+    // MX4: 16 warps = four warpgroups, so that the register file can be re-cut between the roles (setmaxnreg works on
+    // whole warpgroups): 448 threads under one launch bound left the epilogue 128 registers and ~300 bytes of spills
+    // (tile-score GEMM 1.46 ms against FP8's 1.00 ms); warps 14-15 only take part in the barriers
+    static constexpr int THREADS = MX4 ? 512 : (PF_EPI_WARPS + 2) * 32;
+    // MX4 tensor-memory columns behind the accumulators: the query tile's scale words, then one block per key slot
+    static constexpr uint32_t SFQ_COL = NACC * PF_N, SFK_COL = SFQ_COL + 16;
+    static_assert(!MX4 || SFK_COL + 16 * KSTAGES <= 512, "tensor memory");
     // shared-memory byte offset of k-step ks of head h inside a tile of planes [plane][128 rows][128 B]
     static constexpr uint32_t koff(int h, int ks) {
         return (uint32_t)((h * HB + ks * 32) / 128) * PF_PLANE_BYTES + (uint32_t)((h * HB + ks * 32) % 128);
@@ -93,6 +115,10 @@ struct PrefillScoreArgs {
     int64_t total_steps;      // B * steps_per_seq (ItemWalk)
     int64_t steps_per_seq;
     int fine;                 // blk == 16 (f3): four scores per 64-key block, one per 16-token quarter
+    // MX4: the two caches (queries: a cache of Tq tokens per sequence) for the bulk copies of the scale rows
+    const uint8_t* q_cache;
+    const uint8_t* k_cache;
+    int q_tiles, k_tiles;     // 64-token tiles per sequence
 #ifdef SPOT_TRACE
     long long* trace;         // development builds only: [6 roles][2048 events] clock64 of CTA 5
 #endif
@@ -103,6 +129,11 @@ struct PrefillScoreArgs {
 #define PF_STAMP(role, idx) do { } while (0)
 #endif
 
+// contiguous global -> shared bulk copy (bytes a multiple of 16), completion counted on an mbarrier
+__device__ __forceinline__ void bulk_load(uint32_t smem_dst, const void* gsrc, uint32_t bytes, uint32_t bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 :: "r"(smem_dst), "l"(gsrc), "r"(bytes), "r"(bar) : "memory");
+}
 __device__ __forceinline__ uint32_t f32_order_key(float x) {
     const uint32_t u = __float_as_uint(x);
     return (u & 0x80000000u) ? ~u : (u | 0x80000000u);
@@ -178,11 +209,13 @@ struct AccPos {
     }
 };
 
-template <int HB, bool F8>
-__global__ void __launch_bounds__(PF_THREADS, 1) score_prefill_kernel(const __grid_constant__ CUtensorMap tm_q,
+template <int HB, int KIND>
+__global__ void __launch_bounds__((PfCfg<HB, KIND>::THREADS), 1) score_prefill_kernel(const __grid_constant__ CUtensorMap tm_q,
                                                                       const __grid_constant__ CUtensorMap tm_k,
                                                                       const PrefillScoreArgs a) {
-    using Cfg = PfCfg<HB, F8>;
+    using Cfg = PfCfg<HB, KIND>;
+    constexpr bool F8 = Cfg::F8, MX4 = Cfg::MX4;
+    constexpr int PF_THREADS = Cfg::THREADS;
     constexpr int PF_KSTAGES = Cfg::KSTAGES, NACC = Cfg::NACC;
     constexpr uint32_t K_TILE_BYTES = Cfg::K_STAGE_BYTES, Q_TILE_BYTES = Cfg::Q_TILE_BYTES;
     extern __shared__ unsigned char smem_raw[];
@@ -202,6 +235,8 @@ __global__ void __launch_bounds__(PF_THREADS, 1) score_prefill_kernel(const __gr
     static_assert(PF_KSTAGES <= 8 && NACC <= 4, "barrier layout");
     uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(misc + 208);
     uint32_t* s_max = reinterpret_cast<uint32_t*>(misc + 224);       // [CHUNK][4 quarters][2 query blocks]
+    const uint32_t bar_sfq_full = misc_u32 + 1280;                   // MX4: the scale words are in tensor memory
+    const uint32_t bar_sfk_full = misc_u32 + 1288;                   // [<= 8]
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
 
@@ -215,6 +250,10 @@ __global__ void __launch_bounds__(PF_THREADS, 1) score_prefill_kernel(const __gr
         for (int i = 0; i < NACC; ++i) {
             mbar_init(bar_t_full + 8 * i, 1);
             mbar_init(bar_t_empty + 8 * i, PF_EPI_WARPS);
+        }
+        if constexpr (MX4) {
+            mbar_init(bar_sfq_full, Cfg::SF_WARPS);
+            for (int i = 0; i < PF_KSTAGES; ++i) mbar_init(bar_sfk_full + 8 * i, Cfg::SF_WARPS);
         }
         mbar_fence_init();
     }
@@ -231,6 +270,8 @@ __global__ void __launch_bounds__(PF_THREADS, 1) score_prefill_kernel(const __gr
     pdl_wait();
     pdl_launch_dependents();
 
+    if (warp >= PF_EPI_WARPS) {
+    if constexpr (MX4) asm volatile("setmaxnreg.dec.sync.aligned.u32 56;");      // warpgroups 2, 3 (producer, issuer, scale movers)
     if (warp == PF_EPI_WARPS) {
         // ================================ TMA producer: the key ring ================================
         if (lane == 0) {
@@ -242,8 +283,20 @@ __global__ void __launch_bounds__(PF_THREADS, 1) score_prefill_kernel(const __gr
                 const int b = it.b, c = it.c;
                 if (it.new_tile) {                             // (n_tile counts the query tiles this CTA has loaded)
                     mbar_wait(bar_q_empty, (n_tile & 1) ^ 1);  // the previous tile's MMAs have completed
-                    mbar_arrive_expect_tx(bar_q_full, Q_TILE_BYTES);
-                    tma_load_4d(q_smem, &tm_q, bar_q_full, 0, it.m * PF_M, 0, b);
+                    if constexpr (MX4) {
+                        // codes: two 64-token tiles of the query cache (dims: 128 B, 64 rows, tiles, planes); scale rows: one
+                        // bulk copy per tile that exists (a tile past the chunk holds no queries: its rows are masked)
+                        const int t0 = 2 * it.m, nt = min(2, a.q_tiles - t0);
+                        constexpr uint32_t SC = 64 * Cfg::NG, TB = 64 * (Cfg::PLANES * 128 + Cfg::NG);
+                        mbar_arrive_expect_tx(bar_q_full, Cfg::Q_CODE_BYTES + nt * SC);
+                        tma_load_4d(q_smem, &tm_q, bar_q_full, 0, 0, b * a.q_tiles + t0, 0);
+                        for (int i = 0; i < nt; ++i)
+                            bulk_load(q_smem + Cfg::Q_CODE_BYTES + i * SC,
+                                      a.q_cache + ((int64_t)b * a.q_tiles + t0 + i) * TB + 64 * Cfg::PLANES * 128, SC, bar_q_full);
+                    } else {
+                        mbar_arrive_expect_tx(bar_q_full, Q_TILE_BYTES);
+                        tma_load_4d(q_smem, &tm_q, bar_q_full, 0, it.m * PF_M, 0, b);
+                    }
                     ++n_tile;
                 }
                 // (kp counts ring slots: one per pair, or one per (pair, head) at HB = 256)
@@ -251,10 +304,23 @@ __global__ void __launch_bounds__(PF_THREADS, 1) score_prefill_kernel(const __gr
                     for (int hh = 0; hh < (Cfg::PER_HEAD ? PF_H : 1); ++hh, ++kp) {
                         const int s = kp % PF_KSTAGES;
                         mbar_wait(bar_k_empty + 8 * s, ((kp / PF_KSTAGES) & 1) ^ 1);
+                        if constexpr (MX4) {
+                            const int t0 = c * PF_CHUNK + 2 * pr, nt = min(2, a.k_tiles - t0);
+                            constexpr uint32_t SC = 64 * Cfg::NG, TB = 64 * (Cfg::PLANES * 128 + Cfg::NG);
+                            mbar_arrive_expect_tx(bar_k_full + 8 * s, Cfg::K_CODE_BYTES + nt * SC);
+                            // (a pair that overhangs the sequence reads the next sequence's first tile, or zeros past the
+                            // cache: its second block is never used)
+                            tma_load_4d(k_smem + s * K_TILE_BYTES, &tm_k, bar_k_full + 8 * s, 0, 0, b * a.k_tiles + t0, 0);
+                            for (int i = 0; i < nt; ++i)
+                                bulk_load(k_smem + s * K_TILE_BYTES + Cfg::K_CODE_BYTES + i * SC,
+                                          a.k_cache + ((int64_t)b * a.k_tiles + t0 + i) * TB + 64 * Cfg::PLANES * 128, SC,
+                                          bar_k_full + 8 * s);
+                        } else {
                         mbar_arrive_expect_tx(bar_k_full + 8 * s, K_TILE_BYTES);
                         // a pair that overhangs the cache is zero-filled by TMA; its second block is never used
                         tma_load_4d(k_smem + s * K_TILE_BYTES, &tm_k, bar_k_full + 8 * s, 0, (c * PF_CHUNK + 2 * pr) * 64,
                                     hh * Cfg::HEAD_PLANES, b);
+                        }
                         PF_STAMP(0, kp);
                     }
             }
@@ -279,7 +345,7 @@ __global__ void __launch_bounds__(PF_THREADS, 1) score_prefill_kernel(const __gr
         // ================================ MMA issuer ================================
         // The whole warp runs this loop converged; one elected lane issues (tc100.cuh, umma_*_elect).
         {
-            constexpr uint32_t idesc = F8 ? umma_idesc_e4m3(PF_M, PF_N) : umma_idesc_bf16(PF_M, PF_N);
+            constexpr uint32_t idesc = MX4 ? umma_idesc_mxf4(PF_M, PF_N) : F8 ? umma_idesc_e4m3(PF_M, PF_N) : umma_idesc_bf16(PF_M, PF_N);
             int n_tile = 0, kp = 0, acc = 0;
             AccPos ap{0, 0};
             const uint64_t qd = umma_desc_sw128(q_smem);
@@ -291,6 +357,7 @@ __global__ void __launch_bounds__(PF_THREADS, 1) score_prefill_kernel(const __gr
                     // every MMA issued so far read the previous query tile: when they have completed, its buffer is free
                     if (n_tile > 0) umma_commit_elect(bar_q_empty);
                     mbar_wait(bar_q_full, n_tile & 1);         // this tile's queries have landed
+                    if constexpr (MX4) mbar_wait(bar_sfq_full, n_tile & 1);   // ... and their scale words sit in tensor memory
                     tc_fence_after();
                     ++n_tile;
                 }
@@ -300,6 +367,7 @@ __global__ void __launch_bounds__(PF_THREADS, 1) score_prefill_kernel(const __gr
                     if constexpr (!Cfg::PER_HEAD) {
                         s = kp % PF_KSTAGES;
                         mbar_wait(bar_k_full + 8 * s, (kp / PF_KSTAGES) & 1);
+                        if constexpr (MX4) mbar_wait(bar_sfk_full + 8 * s, (kp / PF_KSTAGES) & 1);
                         kd = umma_desc_sw128(k_smem + s * K_TILE_BYTES);
                         ++kp;
                     }
@@ -320,7 +388,13 @@ __global__ void __launch_bounds__(PF_THREADS, 1) score_prefill_kernel(const __gr
                             // the address field of the descriptor is (byte address >> 4): add the k-step's offset to it
                             const uint64_t bd = kd + (uint64_t)(Cfg::koff(Cfg::PER_HEAD ? 0 : h, ks) >> 4);
                             const uint64_t ad = qd + (uint64_t)(Cfg::koff(h, ks) >> 4);
-                            if constexpr (F8) umma_f8_ss_elect(d_tmem, ad, bd, idesc, ks > 0);
+                            if constexpr (MX4) {
+                                // the k-step's two scales: groups g0, g0 + 1 of the token row = bytes g0 % 4, + 1 of scale word g0 / 4
+                                const int g0 = (h * HB + ks * 32) / 16;
+                                umma_mxf4_ss_elect(d_tmem, ad, bd, idesc | umma_idesc_sf_ids(g0 & 3, g0 & 3),
+                                                   tbase + Cfg::SFQ_COL + 4 * (g0 >> 2),
+                                                   tbase + Cfg::SFK_COL + 16 * s + 4 * (g0 >> 2), ks > 0);
+                            } else if constexpr (F8) umma_f8_ss_elect(d_tmem, ad, bd, idesc, ks > 0);
                             else umma_bf16_ss_elect(d_tmem, ad, bd, idesc, ks > 0);
                         }
                         umma_commit_elect(bar_t_full + 8 * ap.slot);      // this head's accumulator is ready for the epilogue
@@ -332,7 +406,48 @@ __global__ void __launch_bounds__(PF_THREADS, 1) score_prefill_kernel(const __gr
                 }
             }
         }
+    } else if (warp < PF_EPI_WARPS + 2 + Cfg::SF_WARPS) {
+        // ================================ MX4: scale words into tensor memory (warps 10 .. 13) ================================
+        // Warp w serves TMEM lane quarter w % 4 (the MMA wants the same words in all four).  A slot's scale bytes lie behind
+        // its codes as [128 rows][NG]; word wd of row r goes to column 4 wd + r / 32 of the slot's block, lane r % 32.
+        if constexpr (MX4) {
+            constexpr int NW = Cfg::NG / 4;                  // 32-bit scale words per row: 2 (d_idx 64) / 4 (d_idx 128)
+            const uint32_t lane_base = tbase + ((uint32_t)((warp & 3) * 32) << 16);
+            auto move = [&](uint32_t sf_smem, uint32_t col, uint32_t bar) {
+                uint32_t r[4 * NW];
+#pragma unroll
+                for (int wd = 0; wd < NW; ++wd)
+#pragma unroll
+                    for (int j = 0; j < 4; ++j)
+                        asm volatile("ld.shared.u32 %0, [%1];" : "=r"(r[4 * wd + j])
+                                     : "r"(sf_smem + (uint32_t)((lane + 32 * j) * Cfg::NG + 4 * wd)));
+#pragma unroll
+                for (int wd = 0; wd < NW; ++wd) tmem_st4u(lane_base + col + 4 * wd, r + 4 * wd);
+                tmem_st_wait();
+                tc_fence_before();
+                __syncwarp();
+                if (lane == 0) mbar_arrive(bar);
+            };
+            int n_tile = 0, kp = 0;
+            ItemWalk walk;
+            walk.init(a);
+            Item it;
+            while (walk.next(a, it)) {
+                if (it.new_tile) {
+                    mbar_wait(bar_q_full, n_tile & 1);
+                    move(q_smem + Cfg::Q_CODE_BYTES, Cfg::SFQ_COL, bar_sfq_full);
+                    ++n_tile;
+                }
+                for (int pr = it.pr0; pr < it.pr1; ++pr, ++kp) {
+                    const int s = kp % PF_KSTAGES;
+                    mbar_wait(bar_k_full + 8 * s, (kp / PF_KSTAGES) & 1);
+                    move(k_smem + s * K_TILE_BYTES + Cfg::K_CODE_BYTES, Cfg::SFK_COL + 16 * s, bar_sfk_full + 8 * s);
+                }
+            }
+        }
+    }
     } else {
+        if constexpr (MX4) asm volatile("setmaxnreg.inc.sync.aligned.u32 192;");  // warpgroups 0, 1
         // ================================ epilogue (warps 0 .. 7) ================================
         // Warp w owns TMEM lanes 32 (w & 3) .. +31 (one query per lane) and the 64 accumulator columns of key block (w >> 2)
         // of the pair.  TMEM reads and the fp32 arithmetic overlap: a warp keeps one 32-column tcgen05.ld in flight while it
@@ -489,9 +604,9 @@ bool encode_tmap_bf16_sw128(CUtensorMap* out, const void* base, int rank, const 
 }
 
 // scores: fp32 [B * Tq/64][nb_stride]; entry (row, j) is written for every key block j the row's query block can see
-template <int HB, bool F8>
+template <int HB, int KIND>
 static spot_status score_prefill_d(const spot_select_params* p, float* scores, int nb_stride, cudaStream_t s) {
-    using Cfg = PfCfg<HB, F8>;
+    using Cfg = PfCfg<HB, KIND>;
     constexpr int PF_D = 64;                                        // plane width in BF16 pairs-of-bytes (128 bytes)
     constexpr int PLANES = Cfg::PLANES;
     PrefillScoreArgs a;
@@ -514,6 +629,25 @@ static spot_status score_prefill_d(const spot_select_params* p, float* scores, i
 
     CUtensorMap tm_q, tm_k;
     const uint64_t row_bytes = (uint64_t)PLANES * 128;              // one token: PF_H heads x HB bytes = PLANES x 128 bytes
+    a.q_cache = nullptr; a.k_cache = nullptr; a.q_tiles = a.k_tiles = 0;
+    if constexpr (Cfg::MX4) {
+        // both operands in the opaque MXFP4 layout: 64-token tiles of [64][row_bytes] code bytes + [64][NG] scale bytes.
+        // The map walks the code rows: (128 bytes, 64 rows of a tile, tiles of the whole cache, planes); a box is two tiles
+        // of every plane, which lands as [plane][128 rows][128 B] in shared memory
+        if (p->Tq % 64 != 0 || p->cache_stride_tokens % 64 != 0) return SPOT_ERR_INVALID_ARG;
+        const uint64_t tile_bytes = 64 * (row_bytes + Cfg::NG);
+        a.q_cache = (const uint8_t*)p->sel_q; a.k_cache = (const uint8_t*)p->sel_k;
+        a.q_tiles = p->Tq / 64; a.k_tiles = (int)(p->cache_stride_tokens / 64);
+        const void* base[2] = {p->sel_q, p->sel_k};
+        const int tiles[2] = {a.q_tiles, a.k_tiles};
+        CUtensorMap* tm[2] = {&tm_q, &tm_k};
+        for (int i = 0; i < 2; ++i) {
+            const uint64_t dims[4] = {(uint64_t)PF_D, 64, (uint64_t)p->B * tiles[i], (uint64_t)PLANES};
+            const uint64_t strides[3] = {row_bytes, tile_bytes, 128};
+            const uint32_t box[4] = {(uint32_t)PF_D, 64u, 2u, (uint32_t)PLANES};
+            if (!encode_tmap_bf16_sw128(tm[i], base[i], 4, dims, strides, box)) return SPOT_ERR_CUDA;
+        }
+    } else {
     {
         const uint64_t dims[4] = {(uint64_t)PF_D, (uint64_t)p->Tq, (uint64_t)PLANES, (uint64_t)p->B};
         const uint64_t strides[3] = {row_bytes, (uint64_t)PF_D * 2, (uint64_t)p->Tq * row_bytes};
@@ -527,25 +661,32 @@ static spot_status score_prefill_d(const spot_select_params* p, float* scores, i
         const uint32_t box[4] = {(uint32_t)PF_D, (uint32_t)PF_N, (uint32_t)Cfg::STAGE_PLANES, 1u};
         if (!encode_tmap_bf16_sw128(&tm_k, p->sel_k, 4, dims, strides, box)) return SPOT_ERR_CUDA;
     }
+    }
     static unsigned long long smem_attr_done = 0;
-    SPOT_CUDA_TRY(set_max_smem_once(score_prefill_kernel<HB, F8>, (int)Cfg::SMEM_BYTES, smem_attr_done));
+    SPOT_CUDA_TRY(set_max_smem_once(score_prefill_kernel<HB, KIND>, (int)Cfg::SMEM_BYTES, smem_attr_done));
     const int grid = (int)(total < sm_count() ? total : sm_count());
-    SPOT_CUDA_TRY(launch_pdl(score_prefill_kernel<HB, F8>, dim3((unsigned)grid), dim3(PF_THREADS), (size_t)Cfg::SMEM_BYTES, s,
+    SPOT_CUDA_TRY(launch_pdl(score_prefill_kernel<HB, KIND>, dim3((unsigned)grid), dim3(Cfg::THREADS), (size_t)Cfg::SMEM_BYTES, s,
                              tm_q, tm_k, a));
     return SPOT_OK;
 }
 
-// fp8: queries AND keys are FP8-E4M3 bytes ([..][H][d], the FP8 cache layout); else both are BF16
-spot_status score_prefill(const spot_select_params* p, float* scores, int nb_stride, bool fp8, cudaStream_t s) {
+// q_fmt: SPOT_SELK_FP8_E4M3 -- queries AND keys are FP8-E4M3 bytes ([..][H][d], the FP8 cache layout); SPOT_SELK_MXFP4 --
+// both are MXFP4 caches (the queries: a cache of Tq tokens per sequence); SPOT_SELK_BF16 -- both are BF16
+spot_status score_prefill(const spot_select_params* p, float* scores, int nb_stride, int q_fmt, cudaStream_t s) {
     if (p->H_idx != PF_H) return SPOT_ERR_UNSUPPORTED;
-    if (fp8) {
-        if (p->d_idx == 64) return score_prefill_d<64, true>(p, scores, nb_stride, s);
-        if (p->d_idx == 128) return score_prefill_d<128, true>(p, scores, nb_stride, s);
+    if (q_fmt == SPOT_SELK_FP8_E4M3) {
+        if (p->d_idx == 64) return score_prefill_d<64, PF_F8>(p, scores, nb_stride, s);
+        if (p->d_idx == 128) return score_prefill_d<128, PF_F8>(p, scores, nb_stride, s);
+        return SPOT_ERR_UNSUPPORTED;
+    }
+    if (q_fmt == SPOT_SELK_MXFP4) {
+        if (p->d_idx == 64) return score_prefill_d<32, PF_MX4>(p, scores, nb_stride, s);
+        if (p->d_idx == 128) return score_prefill_d<64, PF_MX4>(p, scores, nb_stride, s);
         return SPOT_ERR_UNSUPPORTED;
     }
     if (p->fmt != SPOT_SELK_BF16) return SPOT_ERR_UNSUPPORTED;      // other quantised caches: dequantised by the caller (api.cu)
-    if (p->d_idx == 64) return score_prefill_d<128, false>(p, scores, nb_stride, s);
-    if (p->d_idx == 128) return score_prefill_d<256, false>(p, scores, nb_stride, s);
+    if (p->d_idx == 64) return score_prefill_d<128, PF_BF16>(p, scores, nb_stride, s);
+    if (p->d_idx == 128) return score_prefill_d<256, PF_BF16>(p, scores, nb_stride, s);
     return SPOT_ERR_UNSUPPORTED;
 }
 

@@ -160,6 +160,32 @@ __device__ __forceinline__ void umma_f8_ss_elect(uint32_t d_tmem, uint64_t a_des
         "@q tcgen05.mma.cta_group::1.kind::f8f6f4 [%0], %1, %2, %3, p;\n\t}"
         :: "r"(d_tmem), "l"(a_desc), "l"(b_desc), "r"(idesc), "r"((uint32_t)accumulate) : "memory");
 }
+// kind::mxf4 block-scaled instruction descriptor: E2M1 x E2M1 (packed two per byte) -> FP32, both K-major, K = 64 per
+// instruction, one UE8M0 scale per 32 elements of K for every row of A and of B (`.block32`).  a_format = b_format = 1
+// (E2M1), bit 23 = scale format UE8M0, bits [29, 31) / [4, 6) = byte offset of the instruction's first scale inside the
+// row's 32-bit scale word in tensor memory (0 or 2: a word holds the scales of two instructions).
+__host__ __device__ constexpr uint32_t umma_idesc_mxf4(int M, int N) {
+    return (1u << 7) | (1u << 10) | ((uint32_t)(N >> 3) << 17) | (1u << 23) | ((uint32_t)(M >> 4) << 24);
+}
+__host__ __device__ constexpr uint32_t umma_idesc_sf_ids(uint32_t a_sf_byte, uint32_t b_sf_byte) {
+    return (a_sf_byte << 29) | (b_sf_byte << 4);
+}
+// Scale words in tensor memory (the layout tcgen05.mma expects for M = N = 128): the word of row r sits in column
+// (r / 32) of a 4-column block, on lane r % 32 of EVERY 32-lane quarter (the four copies are the same).
+__device__ __forceinline__ void umma_mxf4_ss_elect(uint32_t d_tmem, uint64_t a_desc, uint64_t b_desc, uint32_t idesc,
+                                                   uint32_t sfa_tmem, uint32_t sfb_tmem, bool accumulate) {
+    asm volatile(
+        "{\n\t.reg .pred p, q;\n\t"
+        "setp.ne.b32 p, %4, 0;\n\t"
+        "elect.sync _|q, 0xffffffff;\n\t"
+        "@q tcgen05.mma.cta_group::1.kind::mxf4.block_scale.block32 [%0], %1, %2, %3, [%5], [%6], p;\n\t}"
+        :: "r"(d_tmem), "l"(a_desc), "l"(b_desc), "r"(idesc), "r"((uint32_t)accumulate), "r"(sfa_tmem), "r"(sfb_tmem)
+        : "memory");
+}
+__device__ __forceinline__ void tmem_st4u(uint32_t taddr, const uint32_t* r) {
+    asm volatile("tcgen05.st.sync.aligned.32x32b.x4.b32 [%0], {%1,%2,%3,%4};"
+                 :: "r"(taddr), "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3]) : "memory");
+}
 __device__ __forceinline__ void umma_commit_elect(uint32_t bar) {
     asm volatile(
         "{\n\t.reg .pred q;\n\t"

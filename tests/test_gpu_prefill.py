@@ -466,6 +466,30 @@ def test_prefill_fp8_queries_and_keys_on_the_tensor_cores(torch_cuda, d_idx, L, 
     assert len(report) <= 1
 
 
+# ---------------------------------------------------------------- f2: MXFP4 x MXFP4 block-scaled tile scores
+@pytest.mark.parametrize("d_idx,L,q_start,Tq,B,blk", [(64, 1024, 0, 1024, 1, 64), (128, 1024, 512, 320, 2, 64),
+                                                      (128, 4608, 0, 4608, 1, 64), (64, 1024, 256, 256, 1, 16),
+                                                      (64, 2112, 1024, 1088, 2, 64), (128, 448, 0, 448, 3, 16)])
+def test_prefill_mxfp4_queries_and_keys_block_scaled_on_the_tensor_cores(torch_cuda, d_idx, L, q_start, Tq, B, blk):
+    """PAPER.md:115 / :184-188: queries and key cache in FP4 "group-32 microscale".  With both in MXFP4 the tile scores are
+    E2M1 x E2M1 products times the two groups' UE8M0 scales, accumulated in fp32 by tcgen05.mma kind::mxf4.block_scale
+    straight from the opaque cache layout (q_fmt = mxfp4): no dequantise pass, the scales go through tensor memory.  The
+    oracle scores the two dequantised images (R33).  Products and power-of-two scales are exact; the error is the fp32
+    accumulation over d_idx terms -- the BF16 GEMM's 2e-5 tolerance, exact index lists.  Odd numbers of query blocks and of
+    visible key blocks exercise the half-filled tiles (scale rows that are never loaded must stay out of every result)."""
+    geo = dict(blk=16, sink_blocks=8, recency_blocks=16, kmin_blocks=32) if blk == 16 else {}
+    wls = [_neg_weights(make_prefill_workload(seed=6806 + 7 * b, L=L, d_idx=d_idx, with_kv=False, **geo), 50 + b)
+           for b in range(B)]
+    dp = H.DevicePrefill(wls, q_start, Tq, with_kv=False)
+    dp.set_cache_format("mxfp4")
+    dp.quantise_queries("mxfp4")
+    report = []
+    _check_select_prefill(dp, report)
+    _check_select_prefill(dp, report, mode="topk", top_k=40 if blk == 16 else 6)
+    print("mxfp4 x mxfp4 prefill select d_idx=%d L=%d: near-tie rows %s" % (d_idx, L, report[:4]))
+    assert len(report) <= 1
+
+
 def test_q_fmt_argument_errors(torch_cuda):
     """spot.h, q_fmt: FP8 queries need an FP8 cache and the prefill form; any other value is an invalid argument.  Nothing
     is written to the outputs by a refused call."""
