@@ -18,8 +18,8 @@
 // in attn_decode.cu); mma.sync m16n8k16, fp32 accumulate.
 // Pass 1 on the tensor cores (round 2): when L is whole 64-query blocks the teacher's log-sum-exps come from the prefill
 // attention kernel in its statistics-only form (attn_prefill_tc.cu, tcgen05 / TMEM / TMA) and the student's part from
-// student_pass1_kernel below (21.6 -> 3.5 ms at L = 16K); train_pass_kernel<1> then serves ragged L only.  Pass 2 is still this
-// mma.sync form.
+// student_pass1_kernel below (21.6 -> 3.5 ms at L = 16K); train_pass_kernel<1> then serves ragged L only.  Pass 2 runs on
+// train_pass2_tc_kernel (tcgen05) for the same whole-block sequences, on train_pass_kernel<2> otherwise.
 #include "select_common.cuh"
 #include "tc100.cuh"
 
@@ -53,6 +53,8 @@ struct TrainArgs {
     float scale_log2;
     float* t_lse2;               // [L][H_q] log2-domain log-sum-exp of the scaled teacher logits
     float* s_lse;                // [L] natural-log log-sum-exp of the student scores
+    float* sp_part;              // [L][sp_nch][2]: (max, sum) of a query's student scores over one chunk of keys (student_pass1_kernel)
+    int sp_nch;                  // chunks of SP_CHUNK key tiles per row
     float* blk_scores;           // [L][nb_stride]
     int nb_stride;
     const uint32_t* mask;        // [L][mask_stride] bit b: block b is in S_q
@@ -424,19 +426,27 @@ __global__ void __launch_bounds__(TR_THREADS, 1) train_pass_kernel(TrainArgs a) 
 // one m16 tile per warp, and walks the visible keys in tiles of 64 that all four warps share: the selector key rows are loaded
 // once per CTA (cooperative cp.async ring) and used by 64 queries -- in train_pass_kernel<1> a single warp per CTA served 8
 // queries through a ring of its own and the pass took as long as the teacher's (19.5 ms of 21.6 at L = 16K).
+// (round 2, later) The causal triangle is cut along the keys too: CTA (chunk c, query tile) walks 32 key tiles of 32 keys only
+// and leaves one (max, sum) pair per query, which student_combine_kernel folds into s_lse.  One CTA per 64 queries over the whole
+// row had 256 CTAs of four warps for 148 SMs, the heaviest one alone on the critical path (1.9 ms at L = 16K, tensor pipe 6 %,
+// 26 % issue utilisation with one or two warps per scheduler); 1024-key chunks of 32-key tiles (64 KiB of shared memory: three
+// CTAs per SM) bring spot_train_kl at L = 16K from 5.80 to 4.72 ms.
 constexpr int SP_WARPS = 4;
 constexpr int SP_THREADS = SP_WARPS * 32;
 constexpr int SP_QPC = SP_WARPS * 16;
-constexpr int SP_KT = 64;
+constexpr int SP_KT = 32;
+constexpr int SP_CHUNK = 32;                   // key tiles per CTA (1024 keys)
 
 __global__ void __launch_bounds__(SP_THREADS) student_pass1_kernel(TrainArgs a, int stages) {
     extern __shared__ __align__(128) unsigned char smem[];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int g = lane >> 2, c = lane & 3, mi = lane >> 3, r8 = lane & 7;
     const int n_tiles_q = (a.L + SP_QPC - 1) / SP_QPC;
-    const int q0 = (n_tiles_q - 1 - (int)blockIdx.x) * SP_QPC;         // heaviest (latest) queries first
+    const int q0 = (n_tiles_q - 1 - (int)blockIdx.y) * SP_QPC;         // heaviest (latest) queries first
     const int q_end = min(q0 + SP_QPC, a.L);
-    const int n_kt = (q_end + SP_KT - 1) / SP_KT;
+    const int kt_lo = (int)blockIdx.x * SP_CHUNK;
+    const int n_kt = min((q_end + SP_KT - 1) / SP_KT, kt_lo + SP_CHUNK);   // this CTA's key tiles: [kt_lo, n_kt)
+    if (kt_lo >= n_kt) return;                                          // the chunk lies past the tile's diagonal
     const int srow_bytes = a.H_idx * a.d_idx * 2;
     const int chunks = srow_bytes >> 4;
     const int stage_bytes = SP_KT * srow_bytes;
@@ -462,11 +472,12 @@ __global__ void __launch_bounds__(SP_THREADS) student_pass1_kernel(TrainArgs a, 
     __syncwarp();
     float st_m[2] = {-INFINITY, -INFINITY}, st_l[2] = {0.f, 0.f}, bm[2] = {-INFINITY, -INFINITY};
 
+    const int csh = (chunks & (chunks - 1)) == 0 ? 31 - __clz(chunks) : -1;    // 16-byte chunks per row: a power of two as a rule
     auto issue = [&](int kt) {
         if (kt < n_kt) {
             const uint32_t stage = ring + (kt % stages) * stage_bytes;
             for (int id = tid; id < SP_KT * chunks; id += SP_THREADS) {
-                const int row = id / chunks, ch = id - row * chunks;
+                const int row = csh >= 0 ? id >> csh : id / chunks, ch = id - row * chunks;
                 const bool ok = kt * SP_KT + row < q_end;
                 cp_async16(stage + tr_sw(row, ch, srow_bytes),
                            a.sel_k + (int64_t)(ok ? kt * SP_KT + row : 0) * (a.H_idx * a.d_idx) + ch * 8, ok);
@@ -474,8 +485,8 @@ __global__ void __launch_bounds__(SP_THREADS) student_pass1_kernel(TrainArgs a, 
         }
         cp_async_commit();
     };
-    for (int i = 0; i < stages - 1; ++i) issue(i);
-    for (int kt = 0; kt < n_kt; ++kt) {
+    for (int i = 0; i < stages - 1; ++i) issue(kt_lo + i);
+    for (int kt = kt_lo; kt < n_kt; ++kt) {
         issue(kt + stages - 1);                 // (into the stage every warp left at the end of iteration kt - 1)
         if (stages == 3) cp_async_wait<2>(); else cp_async_wait<1>();
         __syncthreads();                        // tile kt has landed for every thread
@@ -483,7 +494,7 @@ __global__ void __launch_bounds__(SP_THREADS) student_pass1_kernel(TrainArgs a, 
         // the warp's last query is qw0 + 15: tiles past it hold no visible key for this warp
         if (kt * SP_KT <= min(qw0 + 15, a.L - 1)) {
 #pragma unroll 1
-            for (int sub = 0; sub < 2; ++sub) {
+            for (int sub = 0; sub < SP_KT / 32; ++sub) {
                 const int t0 = kt * SP_KT + sub * 32;
                 if (t0 > min(qw0 + 15, a.L - 1)) break;
                 const uint32_t sb = stage + sub * 32 * srow_bytes;
@@ -562,8 +573,24 @@ __global__ void __launch_bounds__(SP_THREADS) student_pass1_kernel(TrainArgs a, 
             if (M > -INFINITY) { l = l * __expf(m - M) + l2 * __expf(m2 - M); m = M; }
         }
         const int q = qw0 + g + 8 * hf;
-        if (c == 0 && q < a.L) a.s_lse[q] = m + __logf(l);
+        if (c == 0 && q < a.L)
+            *reinterpret_cast<float2*>(a.sp_part + ((int64_t)q * a.sp_nch + blockIdx.x) * 2) = make_float2(m, l);
     }
+}
+
+// s_lse[q] = log sum exp over the chunks of keys row q can see (chunk c covers SP_CHUNK * SP_KT = 1024 keys from 1024 c)
+__global__ void __launch_bounds__(256) student_combine_kernel(const float* __restrict__ part, int nch, float* __restrict__ s_lse,
+                                                              int L) {
+    const int q = blockIdx.x * blockDim.x + threadIdx.x;
+    if (q >= L) return;
+    const int n = q / (SP_CHUNK * SP_KT) + 1;                 // chunks that hold a key t <= q
+    float m = -INFINITY, l = 0.f;
+    for (int i = 0; i < n && i < nch; ++i) {
+        const float2 p = *reinterpret_cast<const float2*>(part + ((int64_t)q * nch + i) * 2);
+        const float M = fmaxf(m, p.x);
+        if (M > -INFINITY) { l = l * __expf(m - M) + p.y * __expf(p.x - M); m = M; }
+    }
+    s_lse[q] = m + __logf(l);
 }
 
 // sum over the 32 lanes of v[j] for every j, delivered to lane j (31 shuffles instead of 32 x 5): at each level a lane keeps
@@ -871,8 +898,8 @@ __global__ void list_to_mask_kernel(const int32_t* indices, const int32_t* budge
 }
 
 struct TrainLayout {
-    size_t t_lse2, s_lse, scores, seq_len, indices, budgets, mask, total;
-    int nb_stride, mask_stride, cap, n_b;
+    size_t t_lse2, s_lse, sp_part, scores, seq_len, indices, budgets, mask, total;
+    int nb_stride, mask_stride, cap, n_b, sp_nch;
 };
 TrainLayout train_layout(const spot_train_params* p) {
     TrainLayout y;
@@ -884,6 +911,8 @@ TrainLayout train_layout(const spot_train_params* p) {
     size_t o = 256;
     y.t_lse2 = o; o += up((size_t)p->L * p->H_q * 4);
     y.s_lse = o; o += up((size_t)p->L * 4);
+    y.sp_nch = ((p->L + SP_KT - 1) / SP_KT + SP_CHUNK - 1) / SP_CHUNK;
+    y.sp_part = o; o += up((size_t)p->L * y.sp_nch * 8);
     y.scores = o; o += up((size_t)p->L * y.nb_stride * 4);
     y.seq_len = o; o += up((size_t)p->L * 4);
     y.indices = o; o += p->indices ? 0 : up((size_t)p->L * y.cap * 4);
@@ -986,6 +1015,7 @@ extern "C" spot_status spot_train_kl(const spot_train_params* p, void* stream) {
     a.scale_log2 = p->sm_scale * 1.4426950408889634f;
     a.t_lse2 = reinterpret_cast<float*>(ws + y.t_lse2);
     a.s_lse = reinterpret_cast<float*>(ws + y.s_lse);
+    a.sp_part = reinterpret_cast<float*>(ws + y.sp_part); a.sp_nch = y.sp_nch;
     a.blk_scores = reinterpret_cast<float*>(ws + y.scores);
     a.nb_stride = y.nb_stride;
     uint32_t* mask = reinterpret_cast<uint32_t*>(ws + y.mask);
@@ -1021,7 +1051,9 @@ extern "C" spot_status spot_train_kl(const spot_train_params* p, void* stream) {
         const int sp_smem = (stages * SP_KT + SP_QPC) * srow;
         static unsigned long long done3 = 0;
         SPOT_CUDA_TRY(set_max_smem_once(student_pass1_kernel, (2 * SP_KT + SP_QPC) * 1024, done3));
-        student_pass1_kernel<<<(p->L + SP_QPC - 1) / SP_QPC, SP_THREADS, sp_smem, s>>>(a, stages);
+        student_pass1_kernel<<<dim3((unsigned)a.sp_nch, (unsigned)((p->L + SP_QPC - 1) / SP_QPC)), SP_THREADS, sp_smem, s>>>(a, stages);
+        SPOT_LAUNCH_CHECK();
+        student_combine_kernel<<<(p->L + 255) / 256, 256, 0, s>>>(a.sp_part, a.sp_nch, a.s_lse, p->L);
         SPOT_LAUNCH_CHECK();
     } else {
         train_pass_kernel<1><<<grid, TR_THREADS, smem, s>>>(a);

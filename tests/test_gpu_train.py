@@ -65,6 +65,7 @@ def run_train(torch, wl, top_k, sink=0, rec=0, want_lists=True):
     (320, 32, 2, 64, 64, 2, 0, 0),          # G = 16, two KV heads
     (192, 32, 8, 128, 16, 6, 1, 2),         # the paper's selector width on the tcgen05 pass 2 (two student steps)
     (448, 32, 4, 64, 32, 5, 1, 1),          # G = 8 (two teacher steps per KV head), 32-token blocks, four key tiles
+    (2176, 16, 8, 64, 16, 24, 1, 2),        # three 1024-key chunks per row in the student's pass 1 (partials + combine kernel)
 ])
 def test_train_reductions_match_oracle(torch_cuda, L, H_q, H_kv, d_idx, blk, top_k, sink, rec):
     wl = make_prefill_workload(seed=4200 + L, L=L, H_q=H_q, H_kv=H_kv, d_idx=d_idx, blk=blk, topic_span=32)
