@@ -428,7 +428,8 @@ def run_ours(args):
     formats, prefill_roofline = None, None
     if args.extras and args.fmt == "bf16" and args.workload == "cfg3" and not args.paged and wl.blk == 64:
         formats = {"bf16": {"us": step_mean * 1e3, "selector_cache_bytes": int(sel_bytes), "bytes_per_token": bytes_per_token("bf16")}}
-        for fmt in ("mxfp4", "int4_e4m3"):
+        # (round 2: all five quantised precisions the paper lists -- FP4, INT4 with an E4M3 or a 16-bit scale, FP8, INT8)
+        for fmt in ("mxfp4", "int4_e4m3", "int4_bf16s", "fp8_e4m3", "mxint8"):
             n_f = max(3, min(args.steps, 10))
             sel_k_f = torch.zeros(api.spot_selector_k_bytes(fmt, Bn, L, wl.H_idx, wl.d_idx), dtype=torch.uint8, device=dev)
             api.spot_quantize_selector_k(sel_k, sel_k_f, fmt, Bn, L, 0, L, wl.H_idx, wl.d_idx)

@@ -22,6 +22,8 @@
 #include "common.cuh"
 #include "tc100.cuh"
 
+#include <string.h>
+
 namespace spot {
 
 #ifdef SPOT_TRACE
@@ -116,6 +118,12 @@ struct PrefillScoreArgs {
     int64_t total_steps;      // B * steps_per_seq (ItemWalk)
     int64_t steps_per_seq;
     int fine;                 // blk == 16 (f3): four scores per 64-key block, one per 16-token quarter
+    // rows form (f4, the student's pass 1 of spot_train_kl; B = 1, q_start = 0): instead of one score per (query block, key
+    // block) every QUERY gets, per 64-key block j it can see, the maxima of its blk-token blocks (row_blk[q][j * 64 / blk ..])
+    // and the pair (max, sum exp(s - max)) over the block's visible keys (row_part[j][q]: a log-sum-exp in pieces)
+    float* row_blk;           // nullptr: the tile-score form
+    float2* row_part;         // [Tq / 64][Tq]
+    int row_stride, row_blk_tokens;
     // MX4: the two caches (queries: a cache of Tq tokens per sequence) for the bulk copies of the scale rows
     const uint8_t* q_cache;
     const uint8_t* k_cache;
@@ -529,7 +537,36 @@ __global__ void __launch_bounds__((PfCfg<HB, KIND>::THREADS), 1) score_prefill_k
                         if (c_in_blk + i > q_in_blk) S[i] = -INFINITY;
                 }
                 const bool live = kb < nk && j <= qb_abs && q_exists;   // warp-uniform: Tq is a multiple of 64, a warp's rows share a block
-                if (!a.fine) {
+                if (a.row_blk) {
+                    // rows form: this lane's query against the 64 keys of block j (masked keys are -inf: the diagonal block
+                    // keeps at least key t = q0 for every row)
+                    if (live) {
+                        float q4m[4];
+#pragma unroll
+                        for (int q4 = 0; q4 < 4; ++q4) {
+                            float mx = -INFINITY;
+#pragma unroll
+                            for (int i = 0; i < 16; i += 2) mx = fmax3(mx, S[q4 * 16 + i], S[q4 * 16 + i + 1]);
+                            q4m[q4] = mx;
+                        }
+                        const float mrow = fmaxf(fmaxf(q4m[0], q4m[1]), fmaxf(q4m[2], q4m[3]));
+                        float l0 = 0.f, l1 = 0.f;
+#pragma unroll
+                        for (int i = 0; i < EC; i += 2) {
+                            l0 += fast_exp2((S[i] - mrow) * 1.4426950408889634f);
+                            l1 += fast_exp2((S[i + 1] - mrow) * 1.4426950408889634f);
+                        }
+                        a.row_part[(int64_t)j * a.Tq + q_local] = make_float2(mrow, l0 + l1);
+                        float* dst = a.row_blk + (int64_t)q_local * a.row_stride;
+                        if (a.row_blk_tokens == 16) {
+                            *reinterpret_cast<float4*>(dst + j * 4) = make_float4(q4m[0], q4m[1], q4m[2], q4m[3]);
+                        } else if (a.row_blk_tokens == 32) {
+                            *reinterpret_cast<float2*>(dst + j * 2) = make_float2(fmaxf(q4m[0], q4m[1]), fmaxf(q4m[2], q4m[3]));
+                        } else {
+                            dst[j] = mrow;
+                        }
+                    }
+                } else if (!a.fine) {
                     float mx = -INFINITY;
 #pragma unroll
                     for (int i = 0; i < EC; i += 2) mx = fmax3(mx, S[i], S[i + 1]);
@@ -551,6 +588,7 @@ __global__ void __launch_bounds__((PfCfg<HB, KIND>::THREADS), 1) score_prefill_k
                     }
                 }
             }
+            if (a.row_blk) continue;                             // rows form: everything went out per step
             // item done: all epilogue warps meet, then the tile maxima go out and the buffer is re-armed
             asm volatile("bar.sync 1, %0;" :: "n"(PF_EPI_WARPS * 32) : "memory");
             const int nq4 = a.fine ? 4 : 1;
@@ -604,8 +642,11 @@ bool encode_tmap_bf16_sw128(CUtensorMap* out, const void* base, int rank, const 
 }
 
 // scores: fp32 [B * Tq/64][nb_stride]; entry (row, j) is written for every key block j the row's query block can see
+struct PrefillRowsOut { float* blk_scores; int stride; float2* part; };
+
 template <int HB, int KIND>
-static spot_status score_prefill_d(const spot_select_params* p, float* scores, int nb_stride, cudaStream_t s) {
+static spot_status score_prefill_d(const spot_select_params* p, float* scores, int nb_stride, cudaStream_t s,
+                                   const PrefillRowsOut* rows = nullptr) {
     using Cfg = PfCfg<HB, KIND>;
     constexpr int PF_D = 64;                                        // plane width in BF16 pairs-of-bytes (128 bytes)
     constexpr int PLANES = Cfg::PLANES;
@@ -614,6 +655,10 @@ static spot_status score_prefill_d(const spot_select_params* p, float* scores, i
     a.B = p->B; a.Tq = p->Tq; a.n_qb = p->Tq / 64; a.n_qt = (a.n_qb + 1) / 2;
     a.qb_start = p->q_start / 64;
     a.fine = p->blk == 16;
+    a.row_blk = rows ? rows->blk_scores : nullptr;
+    a.row_part = rows ? rows->part : nullptr;
+    a.row_stride = rows ? rows->stride : 0;
+    a.row_blk_tokens = p->blk;
 #ifdef SPOT_TRACE
     a.trace = g_pf_trace;
 #endif
@@ -687,6 +732,22 @@ spot_status score_prefill(const spot_select_params* p, float* scores, int nb_str
     if (p->fmt != SPOT_SELK_BF16) return SPOT_ERR_UNSUPPORTED;      // other quantised caches: dequantised by the caller (api.cu)
     if (p->d_idx == 64) return score_prefill_d<128, PF_BF16>(p, scores, nb_stride, s);
     if (p->d_idx == 128) return score_prefill_d<256, PF_BF16>(p, scores, nb_stride, s);
+    return SPOT_ERR_UNSUPPORTED;
+}
+
+// f4 (train_kl.cu): the student's pass 1 on the same kernel in its rows form -- one sequence of L = whole 64-query blocks,
+// BF16 selector queries / keys [L][4][d_idx]; blk_scores [L][stride] gets every query's block maxima, part [L / 64][L] the
+// per-64-key (max, sum exp) pairs of its scores.  blk in {16, 32, 64}.
+spot_status score_prefill_rows(const uint16_t* sel_q, const float* w, const uint16_t* sel_k, int L, int H_idx, int d_idx,
+                               int blk, float* blk_scores, int stride, float2* part, cudaStream_t s) {
+    if (H_idx != PF_H || L % 64 != 0 || (blk != 16 && blk != 32 && blk != 64)) return SPOT_ERR_UNSUPPORTED;
+    spot_select_params p;
+    memset(&p, 0, sizeof(p));
+    p.sel_q = sel_q; p.w = w; p.sel_k = sel_k; p.fmt = SPOT_SELK_BF16; p.cache_stride_tokens = L;
+    p.B = 1; p.Tq = L; p.H_idx = H_idx; p.d_idx = d_idx; p.q_start = 0; p.blk = blk; p.q_block = 64;
+    const PrefillRowsOut rows{blk_scores, stride, part};
+    if (d_idx == 64) return score_prefill_d<128, PF_BF16>(&p, nullptr, 0, s, &rows);
+    if (d_idx == 128) return score_prefill_d<256, PF_BF16>(&p, nullptr, 0, s, &rows);
     return SPOT_ERR_UNSUPPORTED;
 }
 

@@ -18,7 +18,9 @@
 // in attn_decode.cu); mma.sync m16n8k16, fp32 accumulate.
 // Pass 1 on the tensor cores (round 2): when L is whole 64-query blocks the teacher's log-sum-exps come from the prefill
 // attention kernel in its statistics-only form (attn_prefill_tc.cu, tcgen05 / TMEM / TMA) and the student's part from
-// student_pass1_kernel below (21.6 -> 3.5 ms at L = 16K); train_pass_kernel<1> then serves ragged L only.  Pass 2 runs on
+// score_prefill_kernel in its rows form (score_prefill.cu: per query the block maxima and a log-sum-exp in 64-key pieces, folded
+// by student_combine_rows_kernel) -- or, for selectors of fewer than four heads, from student_pass1_kernel below (mma.sync);
+// train_pass_kernel<1> then serves ragged L only.  Pass 2 runs on
 // train_pass2_tc_kernel (tcgen05) for the same whole-block sequences, on train_pass_kernel<2> otherwise.
 #include "select_common.cuh"
 #include "tc100.cuh"
@@ -31,6 +33,9 @@ spot_status run_select(const spot_select_params* p, const float* scores, int nb_
                        const StepSync* sync, cudaStream_t s);                                   // select.cu
 spot_status attn_prefill_stats(const uint16_t* q, const uint16_t* k, int64_t k_stride_token, int64_t k_stride_head, int L,
                                int H_q, int H_kv, float sm_scale, float* lse2, cudaStream_t stream);   // attn_prefill_tc.cu
+
+spot_status score_prefill_rows(const uint16_t* sel_q, const float* w, const uint16_t* sel_k, int L, int H_idx, int d_idx,
+                               int blk, float* blk_scores, int stride, float2* part, cudaStream_t s);   // score_prefill.cu
 
 namespace {
 
@@ -593,6 +598,20 @@ __global__ void __launch_bounds__(256) student_combine_kernel(const float* __res
     s_lse[q] = m + __logf(l);
 }
 
+// the same for the rows form of score_prefill_kernel: part[j][q] = (max, sum exp) of row q over the 64 keys of block j
+__global__ void __launch_bounds__(256) student_combine_rows_kernel(const float2* __restrict__ part, float* __restrict__ s_lse, int L) {
+    const int q = blockIdx.x * blockDim.x + threadIdx.x;
+    if (q >= L) return;
+    float m = -INFINITY, l = 0.f;
+    for (int j = 0; j <= q / 64; ++j) {
+        const float2 p = part[(int64_t)j * L + q];
+        const float M = fmaxf(m, p.x);
+        l = l * __expf(m - M) + p.y * __expf(p.x - M);       // (block 0 always holds key 0: M is finite from the first step)
+        m = M;
+    }
+    s_lse[q] = m + __logf(l);
+}
+
 // sum over the 32 lanes of v[j] for every j, delivered to lane j (31 shuffles instead of 32 x 5): at each level a lane keeps
 // the half of its elements that its own bit selects and adds the partner's copy of that half
 __device__ __forceinline__ float warp_transpose_sum(float (&v)[32], int lane) {
@@ -912,7 +931,10 @@ TrainLayout train_layout(const spot_train_params* p) {
     y.t_lse2 = o; o += up((size_t)p->L * p->H_q * 4);
     y.s_lse = o; o += up((size_t)p->L * 4);
     y.sp_nch = ((p->L + SP_KT - 1) / SP_KT + SP_CHUNK - 1) / SP_CHUNK;
-    y.sp_part = o; o += up((size_t)p->L * y.sp_nch * 8);
+    // (or, on the tensor-core path of the student's pass 1, [L / 64][L] pairs: score_prefill_rows)
+    const size_t rows_part = p->L % 64 == 0 ? (size_t)(p->L / 64) * p->L * 8 : 0;
+    const size_t chunk_part = (size_t)p->L * y.sp_nch * 8;
+    y.sp_part = o; o += up(rows_part > chunk_part ? rows_part : chunk_part);
     y.scores = o; o += up((size_t)p->L * y.nb_stride * 4);
     y.seq_len = o; o += up((size_t)p->L * 4);
     y.indices = o; o += p->indices ? 0 : up((size_t)p->L * y.cap * 4);
@@ -1047,6 +1069,16 @@ extern "C" spot_status spot_train_kl(const spot_train_params* p, void* stream) {
                 a.t_lse2, p->teacher_lse, 0.6931471805599453f, (int64_t)p->L * p->H_q);
             SPOT_LAUNCH_CHECK();
         }
+        // the student's part: the tile-score GEMM of the prefill path in its rows form (tcgen05) where its geometry fits,
+        // else student_pass1_kernel (mma.sync)
+        const bool rows_tc = p->H_idx == 4 && (p->d_idx == 64 || p->d_idx == 128) && (p->blk == 16 || p->blk == 32 || p->blk == 64);
+        if (rows_tc) {
+            if ((st = score_prefill_rows(p->sel_q, p->w, p->sel_k, p->L, p->H_idx, p->d_idx, p->blk, a.blk_scores, a.nb_stride,
+                                         reinterpret_cast<float2*>(a.sp_part), s)) != SPOT_OK)
+                return st;
+            student_combine_rows_kernel<<<(p->L + 255) / 256, 256, 0, s>>>(reinterpret_cast<const float2*>(a.sp_part), a.s_lse, p->L);
+            SPOT_LAUNCH_CHECK();
+        } else {
         const int srow = p->H_idx * p->d_idx * 2, stages = 2;
         const int sp_smem = (stages * SP_KT + SP_QPC) * srow;
         static unsigned long long done3 = 0;
@@ -1055,6 +1087,7 @@ extern "C" spot_status spot_train_kl(const spot_train_params* p, void* stream) {
         SPOT_LAUNCH_CHECK();
         student_combine_kernel<<<(p->L + 255) / 256, 256, 0, s>>>(a.sp_part, a.sp_nch, a.s_lse, p->L);
         SPOT_LAUNCH_CHECK();
+        }
     } else {
         train_pass_kernel<1><<<grid, TR_THREADS, smem, s>>>(a);
         SPOT_LAUNCH_CHECK();

@@ -68,7 +68,18 @@ def run_train(torch, wl, top_k, sink=0, rec=0, want_lists=True):
     (2176, 16, 8, 64, 16, 24, 1, 2),        # three 1024-key chunks per row in the student's pass 1 (partials + combine kernel)
 ])
 def test_train_reductions_match_oracle(torch_cuda, L, H_q, H_kv, d_idx, blk, top_k, sink, rec):
-    wl = make_prefill_workload(seed=4200 + L, L=L, H_q=H_q, H_kv=H_kv, d_idx=d_idx, blk=blk, topic_span=32)
+    _train_case(torch_cuda, L, H_q, H_kv, d_idx, blk, top_k, sink, rec, 4)
+
+
+def test_train_reductions_two_selector_heads(torch_cuda):
+    """H_idx = 2 with whole 64-query blocks: the teacher's pass 1 on the tcgen05 statistics kernel, the student's on
+    student_pass1_kernel + student_combine_kernel (mma.sync; two 1024-key chunks per late row), pass 2 on train_pass_kernel<2>
+    -- the forms the 4-head geometries no longer reach now that their student pass runs on score_prefill_kernel's rows form."""
+    _train_case(torch_cuda, 1088, 16, 8, 64, 16, 12, 1, 1, 2)
+
+
+def _train_case(torch_cuda, L, H_q, H_kv, d_idx, blk, top_k, sink, rec, H_idx):
+    wl = make_prefill_workload(seed=4200 + L, L=L, H_q=H_q, H_kv=H_kv, H_idx=H_idx, d_idx=d_idx, blk=blk, topic_span=32)
     rng = np.random.Generator(np.random.Philox(77 + L))
     wl.w = np.where(rng.random(wl.w.shape) < 0.2, -wl.w, wl.w).astype(np.float32)       # some negative weights (R13)
     dkl, skl, lse, idx, bud = run_train(torch_cuda, wl, top_k, sink, rec)
