@@ -28,7 +28,9 @@
 // 887 -> head-slowest grid 982 -> 128 keys per iteration 1016 -> optimistic single-pass softmax 1069 -> no ordering barriers 1096
 // -> converged issuer warp with an elected lane 1105.  (Round 2, measured and dropped: 2 / 3 / 4 of every 8 exponentials through a
 // Cody-Waite + cubic polynomial on the FMA / ALU pipes instead of MUFU.EX2: 1065 / 1039 / 993 -- the softmax warps are
-// bound by issue slots, not by the 16 MUFU lanes.)
+// bound by issue slots, not by the 16 MUFU lanes.  Also measured and dropped: P handed to the issuer in HALVES of 64 keys, each
+// a softmax step of its own with its own barrier, so that PV of the first half runs under the exponentials of the second:
+// 954 against 1100 TFLOP/s at cfg5 -- twice the hand-offs per tile cost more than the overlap returns.)
 #include "common.cuh"
 #include "tc100.cuh"
 
