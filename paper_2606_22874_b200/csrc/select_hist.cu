@@ -352,21 +352,52 @@ __global__ void __launch_bounds__(SH_N / SH_E) select_hist_kernel(SelectArgs a) 
                         s_tau = lo;
                     }
                 } else {
-                    // two counting passes: (mass query only) how many keys stay in front of the cut, then the key
-                    // of the wanted rank
+                    // Sort the bin's (key, mass) pairs by key, in place: a bitonic network in its all-ascending form (first
+                    // sub-step of every block size compares i with i ^ (k - 1), the others i with i ^ j), so that positions
+                    // past cB act as +inf padding and a comparator that reaches one is a no-op.  Equal keys carry equal masses
+                    // and ties are broken by BLOCK INDEX at emission, from the threshold key alone -- the order of equal keys
+                    // inside the bin decides nothing, and nothing after this reads the bin in its scattered order.  Then the
+                    // cut is a prefix sum over the sorted masses and the threshold the key at that rank.  (Until the end of
+                    // round 2 this was two O(cB^2 / threads) counting passes: one block of score exactly 0 beside 8191 scores
+                    // within 1e-3 of each other put every residual key into one bin and the row took 5.9 ms.)
+                    for (int k = 2; (k >> 1) < cB; k <<= 1) {
+                        bool first = true;
+                        for (int jj = k >> 1; jj > 0; jj >>= 1, first = false) {
+                            const int mask = first ? k - 1 : jj;
+                            for (int x = tid; x < cB; x += SH_T) {
+                                const int y = x ^ mask;
+                                if (y > x && y < cB) {
+                                    const uint32_t kx = s_k[sB + x], ky = s_k[sB + y];
+                                    if (kx > ky) {
+                                        s_k[sB + x] = ky; s_k[sB + y] = kx;
+                                        const double ex = s_e[sB + x];
+                                        s_e[sB + x] = s_e[sB + y]; s_e[sB + y] = ex;
+                                    }
+                                }
+                            }
+                            __syncthreads();
+                        }
+                    }
                     int n_in = want;
                     if (by_mass) {
-                        int cnt = 0;
-#pragma unroll 1
-                        for (int x = tid; x < cB; x += SH_T) {
-                            const uint32_t kx = s_k[sB + x];
-                            double cum = base;
-                            for (int j = 0; j < cB; ++j) {
-                                const uint32_t kj = s_k[sB + j];
-                                if (kj < kx || (kj == kx && j <= x)) cum += s_e[sB + j];
-                            }
-                            if (cum < target) ++cnt;
+                        // keys in front of the cut: running mass (inclusive, fp64) still below the target
+                        const int per = (cB + SH_T - 1) / SH_T;
+                        const int x0 = min(tid * per, cB), x1 = min(x0 + per, cB);
+                        double loc = 0.0;
+                        for (int x = x0; x < x1; ++x) loc += s_e[sB + x];
+                        double inc = loc;
+#pragma unroll
+                        for (int o = 1; o < 32; o <<= 1) {
+                            const double up = __shfl_up_sync(0xffffffffu, inc, o);
+                            if (lane >= o) inc += up;
                         }
+                        if (lane == 31) s_wd[warp] = inc;
+                        __syncthreads();
+                        double cum = base;
+                        for (int w = 0; w < warp; ++w) cum += s_wd[w];
+                        cum += inc - loc;
+                        int cnt = 0;
+                        for (int x = x0; x < x1; ++x) { cum += s_e[sB + x]; cnt += cum < target ? 1 : 0; }
                         cnt = __reduce_add_sync(0xffffffffu, cnt);
                         if (lane == 0 && cnt) atomicAdd(&s_nin, cnt);
                         __syncthreads();
@@ -374,16 +405,7 @@ __global__ void __launch_bounds__(SH_N / SH_E) select_hist_kernel(SelectArgs a) 
                         __syncthreads();
                     }
                     n_in = max(0, min(n_in, cB - 1));
-#pragma unroll 1
-                    for (int x = tid; x < cB; x += SH_T) {
-                        const uint32_t kx = s_k[sB + x];
-                        int rank = 0;
-                        for (int j = 0; j < cB; ++j) {
-                            const uint32_t kj = s_k[sB + j];
-                            rank += (kj < kx || (kj == kx && j < x)) ? 1 : 0;
-                        }
-                        if (rank == n_in) { s_tau = kx; s_nin = n_in; }
-                    }
+                    if (tid == 0) { s_tau = s_k[sB + n_in]; s_nin = n_in; }
                 }
             }
             __syncthreads();

@@ -564,3 +564,41 @@ def test_quantised_query_through_the_cache_quantiser(torch_cuda, fmt):
     report = []
     _check_select(dd, fmt, report)
     _check_select(dd, fmt, report, mode="topk", top_k=16)
+
+
+# ---------------------------------------------------------------- selection latency on a degenerate score distribution
+@pytest.mark.parametrize("blk", [64, 16])
+def test_one_outlier_beside_near_equal_scores_is_exact_and_not_slow(torch_cuda, blk):
+    """One block whose score is exactly 0 beside 2047 / 8191 block scores within 1e-3 of each other: the histogram's linear bins
+    span [0, max], so every other residual key lands in ONE bin and the cut falls inside it.  The selection must still be the
+    oracle's, and the row must not take milliseconds (the bin is sorted in place: tens of microseconds; the counting passes
+    it replaced took 0.3 ms at 2048 blocks and 5.9 ms at 8192)."""
+    torch = torch_cuda
+    from workloads import f32_to_bf16_bits
+    from workloads.bf16 import bf16_bits_to_f32
+    L = 131072
+    wl = make_decode_workload("one_outlier", 7, B=1, L=L, kind="zipf", with_kv=False, blk=blk)
+    rng = np.random.default_rng(3)
+    q = bf16_bits_to_f32(wl.sel_q[0])
+    qhat = q / np.linalg.norm(q, axis=-1, keepdims=True)
+    k = (4.0 * qhat[None] * (1.0 + 1e-3 * rng.standard_normal((L, 1, 1)))).astype(np.float32)
+    k[5 * blk:6 * blk] = 0.0
+    wl.sel_k[0] = f32_to_bf16_bits(k)
+    dd = H.DeviceDecode(wl, "bf16", with_kv=False)
+    report = []
+    _check_select(dd, "bf16", report)
+    _check_select(dd, "bf16", report, p=0.5)
+    _check_select(dd, "bf16", report, mode="topk", top_k=1000)
+    assert all(r[3] == "exact" for r in report), report
+    for _ in range(3):
+        dd.select(want_scores=False, want_probs=False)
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
+    torch.cuda.synchronize()
+    ev[0].record()
+    for _ in range(5):
+        dd.select(want_scores=False, want_probs=False)
+    ev[1].record()
+    torch.cuda.synchronize()
+    per_call_ms = ev[0].elapsed_time(ev[1]) / 5
+    print("one-outlier row, blk %d: %.3f ms per select call (harness allocations included)" % (blk, per_call_ms))
+    assert per_call_ms < 1.0
