@@ -490,6 +490,33 @@ def test_prefill_mxfp4_queries_and_keys_block_scaled_on_the_tensor_cores(torch_c
     assert len(report) <= 1
 
 
+@pytest.mark.parametrize("fmt,d_idx", [("mxfp4", 64), ("mxfp4", 128), ("fp8_e4m3", 128)])
+def test_full_size_cfg5_low_precision_tile_scores(torch_cuda, fmt, d_idx):
+    """The low-precision tensor-core forms of the tile-score GEMM at config 5's full size (L = 65536, one chunk), launched as
+    `bench.py --workload cfg5 --fmt X --qfmt X` launches them: a seeded sample of query blocks (the first two, the last, an odd
+    one and nine others), each checked on its whole selection row -- tile scores at 2e-5 and the index list / budget against
+    the oracle run on the two dequantised images (R33)."""
+    L = 65536
+    n_qb = L // 64
+    wl = make_prefill_workload(seed=5005, L=L, d_idx=d_idx, with_kv=False)
+    dp = H.DevicePrefill([wl], 0, L, with_kv=False)
+    dp.set_cache_format(fmt)
+    dp.quantise_queries(fmt)
+    idx, bud, scores, probs = dp.select(want_probs=False)
+    rng = np.random.Generator(np.random.Philox(65005 + d_idx))
+    sample = sorted(set([0, 1, 513, n_qb - 1]) | set(rng.choice(np.arange(2, n_qb - 1), size=9, replace=False).tolist()))
+    near = []
+    for i in sample:
+        (s_bar, sel), = H.oracle_select_prefill(wl, i * 64, 64)
+        np.testing.assert_allclose(scores[i, :len(s_bar)], s_bar, rtol=2e-5, atol=2e-5)
+        cls = H.classify_selection(s_bar, sel, idx[i], int(bud[i]), wl.p)
+        assert not cls.startswith("FAIL"), "query block %d: %s" % (i, cls)
+        if cls != "exact":
+            near.append((i, cls))
+    print("cfg5 %s x %s d_idx %d: %d sampled query blocks, near-tie rows %s" % (fmt, fmt, d_idx, len(sample), near))
+    assert len(near) <= 1
+
+
 def test_q_fmt_argument_errors(torch_cuda):
     """spot.h, q_fmt: FP8 queries need an FP8 cache and the prefill form; any other value is an invalid argument.  Nothing
     is written to the outputs by a refused call."""
