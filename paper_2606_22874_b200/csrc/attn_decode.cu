@@ -355,7 +355,7 @@ __global__ void __launch_bounds__(ATT_WARPS * 32, 2) attn_decode_kernel(AttnArgs
 
 // merge the partials of one (sequence, query head): one warp each.  The contributors of segment s = (b, hk) are the
 // CTAs whose ranges overlap the segment's units; their slots are CTA + s.
-constexpr int MERGE_WARPS = 4;
+constexpr int MERGE_WARPS = 8;
 __global__ void __launch_bounds__(MERGE_WARPS * 32) attn_merge_kernel(AttnArgs a) {
     // one CTA per (sequence, query head); its warps split the row's partials between them
     __shared__ float s_acc[MERGE_WARPS][ATT_D + 4];
@@ -408,32 +408,57 @@ __global__ void __launch_bounds__(MERGE_WARPS * 32) attn_merge_kernel(AttnArgs a
             }
             return;
         }
-        // the row maximum over every contributor (each warp reads all of them: <= a few hundred floats)
-        float M = -INFINITY;
-        for (int t = lane; t < n_contrib; t += 32) M = fmaxf(M, a.part_ml[(slot_of(t) * G + r) * 2]);
-#pragma unroll
-        for (int o = 16; o; o >>= 1) M = fmaxf(M, __shfl_xor_sync(0xffffffffu, M, o));
-        const float Mu = (M == -INFINITY) ? 0.f : M;
+        // Every warp folds its share of the contributors with a running maximum of its own (online log-sum-exp: no pass over
+        // all the maxima in front of the loads -- one L2 round trip less on the tail of the step), four partials in flight
+        // at a time; warp 0 then combines the warps' (m, l, acc).
+        float m_w = -INFINITY, lsum = 0.f;
         float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
-        float lsum = 0.f;
-#pragma unroll 4
-        for (int t = warp; t < n_contrib; t += MERGE_WARPS) {
-            const int64_t pr = slot_of(t) * G + r;
-            const float2 ml = *reinterpret_cast<const float2*>(a.part_ml + pr * 2);
-            const float4 o = *reinterpret_cast<const float4*>(a.part_o + pr * ATT_D + lane * 4);
-            const float f = fast_exp2(ml.x - Mu);
-            acc.x += f * o.x; acc.y += f * o.y; acc.z += f * o.z; acc.w += f * o.w;
-            lsum += f * ml.y;
+        for (int t0 = warp; t0 < n_contrib; t0 += 4 * MERGE_WARPS) {
+            float2 ml[4];
+            float4 o[4];
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+                const int t = t0 + u * MERGE_WARPS;
+                ml[u] = make_float2(-INFINITY, 0.f);
+                o[u] = make_float4(0.f, 0.f, 0.f, 0.f);
+                if (t < n_contrib) {
+                    const int64_t pr = slot_of(t) * G + r;
+                    ml[u] = *reinterpret_cast<const float2*>(a.part_ml + pr * 2);
+                    o[u] = *reinterpret_cast<const float4*>(a.part_o + pr * ATT_D + lane * 4);
+                }
+            }
+            float m_new = m_w;
+#pragma unroll
+            for (int u = 0; u < 4; ++u) m_new = fmaxf(m_new, ml[u].x);
+            if (m_new > -INFINITY) {
+                const float f_old = fast_exp2(m_w - m_new);        // exp2(-inf) = 0 on the first contributors
+                acc.x *= f_old; acc.y *= f_old; acc.z *= f_old; acc.w *= f_old;
+                lsum *= f_old;
+#pragma unroll
+                for (int u = 0; u < 4; ++u) {
+                    const float f = fast_exp2(ml[u].x - m_new);    // (a padding entry has m = -inf: f = 0)
+                    acc.x += f * o[u].x; acc.y += f * o[u].y; acc.z += f * o[u].z; acc.w += f * o[u].w;
+                    lsum += f * ml[u].y;
+                }
+                m_w = m_new;
+            }
         }
         *reinterpret_cast<float4*>(&s_acc[warp][lane * 4]) = acc;
-        if (lane == 0) s_acc[warp][ATT_D] = lsum;
+        if (lane == 0) { s_acc[warp][ATT_D] = lsum; s_acc[warp][ATT_D + 1] = m_w; }
         __syncthreads();
         if (warp == 0) {
+            float M = -INFINITY;
 #pragma unroll
-            for (int w = 1; w < MERGE_WARPS; ++w) {
+            for (int w = 0; w < MERGE_WARPS; ++w) M = fmaxf(M, s_acc[w][ATT_D + 1]);
+            const float Mu = (M == -INFINITY) ? 0.f : M;
+            acc = make_float4(0.f, 0.f, 0.f, 0.f);
+            lsum = 0.f;
+#pragma unroll
+            for (int w = 0; w < MERGE_WARPS; ++w) {
+                const float f = fast_exp2(s_acc[w][ATT_D + 1] - Mu);
                 const float4 o = *reinterpret_cast<const float4*>(&s_acc[w][lane * 4]);
-                acc.x += o.x; acc.y += o.y; acc.z += o.z; acc.w += o.w;
-                lsum += s_acc[w][ATT_D];
+                acc.x += f * o.x; acc.y += f * o.y; acc.z += f * o.z; acc.w += f * o.w;
+                lsum += f * s_acc[w][ATT_D];
             }
             const float inv = lsum > 0.f ? 1.f / lsum : 0.f;
             if (!dry) {
