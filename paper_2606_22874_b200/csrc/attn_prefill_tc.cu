@@ -30,7 +30,9 @@
 // Cody-Waite + cubic polynomial on the FMA / ALU pipes instead of MUFU.EX2: 1065 / 1039 / 993 -- the softmax warps are
 // bound by issue slots, not by the 16 MUFU lanes.  Also measured and dropped: P handed to the issuer in HALVES of 64 keys, each
 // a softmax step of its own with its own barrier, so that PV of the first half runs under the exponentials of the second:
-// 954 against 1100 TFLOP/s at cfg5 -- twice the hand-offs per tile cost more than the overlap returns (and its parity was not green yet: a few rows off).)
+// 954 against 1100 TFLOP/s at cfg5 -- twice the hand-offs per tile cost more than the overlap returns (and its parity was not green yet: a few rows off); one issuer warp PER TILE (each tile's chain on a warp of its own instead of one
+// warp alternating between the tiles; parity green): 916 TFLOP/s -- the fixed PV0 QK0 | PV1 QK1 order of the single issuer is
+// what keeps the two tiles half an iteration apart.)
 #include "common.cuh"
 #include "tc100.cuh"
 
