@@ -579,6 +579,8 @@ def run_prefill(args):
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
     L = args.L or 65536
+    assert args.fmt != "int4_bf16s", ("--fmt int4_bf16s is a decode-row format: its keys q * s are not BF16 numbers and prefill "
+                                      "selection over it returns SPOT_ERR_UNSUPPORTED (DESIGN.md R39)")
     geo = dict(D_IDX_OVERRIDE)
     if args.blk == 16:                # the paper's 16-token key blocks with its 8 / 16 / 32 reserved blocks (f3)
         geo.update(blk=16, sink_blocks=8, recency_blocks=16, kmin_blocks=32)
