@@ -112,7 +112,7 @@ def test_select_edge_cases(torch_cuda):
                                   with_kv=False)
         if seed == 2:
             wl.sel_k[2, 64:128] = wl.sel_k[2, 128:192]      # blocks 1 and 2 tie exactly -> index tie-break (R7)
-        for fmt in ("bf16", "mxfp4", "int4_e4m3", "fp8_e4m3"):
+        for fmt in ("bf16", "mxfp4", "int4_e4m3", "fp8_e4m3", "mxint8", "int4_bf16s"):
             dd = H.DeviceDecode(wl, fmt, with_kv=False)
             report = []
             for over in (dict(), dict(p=0.5, kmin_blocks=0), dict(sink_blocks=0, recency_blocks=0, kmin_blocks=0),
