@@ -27,7 +27,7 @@ def decode_cases():
     from tests import _harness as H
     from workloads import make_decode_workload
     F3 = dict(blk=16, sink_blocks=8, recency_blocks=16, kmin_blocks=32)
-    for fmt in ("bf16", "mxfp4", "int4_e4m3", "fp8_e4m3"):
+    for fmt in ("bf16", "mxfp4", "int4_e4m3", "fp8_e4m3", "mxint8", "int4_bf16s"):
         for over in ({}, F3):
             wl = make_decode_workload("san", 7, B=3, L=1280, kind="zipf", seq_lens=[1280, 1000, 333], **over)
             dd = H.DeviceDecode(wl, fmt)
@@ -156,7 +156,7 @@ def guarded_cases():
     from tests import _harness as H
     from workloads import make_decode_workload, make_prefill_workload
     for fmt, over in (("bf16", {}), ("mxfp4", {}), ("int4_e4m3", dict(blk=16, sink_blocks=8, recency_blocks=16, kmin_blocks=32)),
-                      ("fp8_e4m3", {})):
+                      ("fp8_e4m3", {}), ("mxint8", {}), ("int4_bf16s", dict(blk=16, sink_blocks=8, recency_blocks=16, kmin_blocks=32))):
         wl = make_decode_workload("guard", 13, B=5, L=2048 + 64, kind="zipf", seq_lens=[2112, 2048, 1999, 65, 1], **over)
         dd = H.DeviceDecode(wl, fmt)
         dp = dd.step_params()
@@ -182,17 +182,20 @@ def guarded_cases():
         for r in runs[1:]:
             assert all(torch.equal(x, y) for x, y in zip(r, runs[0])), "decode step %s: runs differ" % fmt
         print("guarded decode step", fmt, "blk", wl.blk, "ok, budgets", dd.budgets.tolist())
-    for d_idx in (64, 128):
+    for d_idx, qfmt in ((64, None), (128, None), (64, "mxfp4"), (128, "mxfp4"), (128, "fp8_e4m3")):
         wl = make_prefill_workload(seed=90 + d_idx, L=1024, d_idx=d_idx)
         dpf = H.DevicePrefill([wl], 256, 448)
+        if qfmt:                              # low-precision tensor-core tile scores: quantised cache AND queries (q_fmt)
+            dpf.set_cache_format(qfmt)
+            dpf.quantise_queries(qfmt)
         outs = []
         for _ in range(3):
             idx, bud, scores, _ = dpf.select()
             out, lse = dpf.attend(idx, bud, want_lse=True)
             outs.append((idx.copy(), bud.copy(), scores[:, :4].copy(), out.copy()))
         for r in outs[1:]:
-            assert all(np.array_equal(x, y) for x, y in zip(r, outs[0])), "prefill d_idx %d: runs differ" % d_idx
-        print("deterministic prefill d_idx", d_idx, "ok")
+            assert all(np.array_equal(x, y) for x, y in zip(r, outs[0])), "prefill d_idx %d %s: runs differ" % (d_idx, qfmt)
+        print("deterministic prefill d_idx", d_idx, qfmt or "bf16", "ok")
 
 
 if __name__ == "__main__":
