@@ -111,8 +111,12 @@ def test_fuzz_prefill(torch_cuda, chunk):
                for b in range(B)]
         dp = H.DevicePrefill(wls, qb0 * 64, nqb * 64)
         fmt = str(rng.choice(["bf16", "bf16", "mxfp4", "fp8_e4m3"]))
+        if case % 3 == 2:                    # round 2: the MXINT8 cache (dequantise pass) and the low-precision tensor-core forms
+            fmt = ("mxint8", "mxfp4", "fp8_e4m3")[(case // 3) % 3]
         if fmt != "bf16":
             dp.set_cache_format(fmt)
+            if case % 3 == 2 and fmt != "mxint8":
+                dp.quantise_queries(fmt)     # q_fmt: MXFP4 x MXFP4 / FP8 x FP8 tile scores straight from the caches
         report = []
         _check_select_prefill(dp, report, **over)
         lists = [[sel.indices.tolist() for _, sel in H.oracle_select_prefill(w, dp.q_start, dp.Tq, **over)] for w in wls]
@@ -161,8 +165,12 @@ def test_fuzz_prefill_block16(torch_cuda):
                for b in range(B)]
         dp = H.DevicePrefill(wls, qb0 * 64, nqb * 64)
         fmt = str(rng.choice(["bf16", "bf16", "mxfp4", "fp8_e4m3"]))
+        if case % 3 == 2:                    # round 2: the MXINT8 cache (dequantise pass) and the low-precision tensor-core forms
+            fmt = ("mxint8", "mxfp4", "fp8_e4m3")[(case // 3) % 3]
         if fmt != "bf16":
             dp.set_cache_format(fmt)
+            if case % 3 == 2 and fmt != "mxint8":
+                dp.quantise_queries(fmt)     # q_fmt: MXFP4 x MXFP4 / FP8 x FP8 tile scores straight from the caches
         report = []
         _check_select_prefill(dp, report, **over)
         lists = [[sel.indices.tolist() for _, sel in H.oracle_select_prefill(w, dp.q_start, dp.Tq, **over)] for w in wls]
