@@ -74,6 +74,9 @@ __device__ __forceinline__ int seq_blocks(const AttnArgs& a, int b) {
 // A pipelined step cuts the unit list twice: sequences [0, split) first, then [split, B), split = ceil(B / 2).  The first
 // half's index lists are ready when the scoring stream ends (their selection ran beside the scoring of the second half);
 // the second half's are long there when a CTA finishes its first range.
+// (Measured and not kept, end of round 2: phase 0 = the scoring grid's FIRST group, B / 4 sequences, whose lists are the ones
+// ready when the scoring stream ends -- at B = 8, L = 32K attention then starts 5 us earlier, and the step got 5 us LONGER
+// (113.9 -> 119.1 us; B = 4 and 16 unchanged): a phase of ~11 units per CTA is all ramp.)
 __device__ __forceinline__ int phase_split(const AttnArgs& a) { return (a.B + 1) >> 1; }
 __device__ __forceinline__ int phase_lo(const AttnArgs& a, int phase) { return (a.n_phases == 2 && phase == 1) ? phase_split(a) : 0; }
 __device__ __forceinline__ int phase_hi(const AttnArgs& a, int phase) { return (a.n_phases == 2 && phase == 0) ? phase_split(a) : a.B; }
