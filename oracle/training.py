@@ -115,3 +115,27 @@ def training_reductions(Q, K, sm_scale, sel_q, w, sel_k, blk, k_blocks, sink_blo
     return dict(dense_kl=dense_kl(p_tau, p_sigma),
                 sparse_kl=sparse_kl(p_tau, p_sigma, s_s, blk, k_blocks, sink_blocks, recency_blocks),
                 teacher_lse=lse, p_tau=p_tau, p_sigma=p_sigma, s_s=s_s)
+
+
+def training_row(q, Q_row, K_prefix, sm_scale, sel_q_row, w_row, sel_k_prefix, blk, k_blocks, sink_blocks=0, recency_blocks=0):
+    """Row q of training_reductions from the causal prefix alone (row q of every quantity above depends on the keys t <= q
+    only) -- the same definitions through the same sub-functions, for sampled rows of sequences too long for the L x L
+    matrices (pinned against training_reductions on a short sequence, tests/test_oracle_training.py).
+    Q_row [H_q, D], K_prefix [q + 1, H_kv, D], sel_q_row [H, d], w_row [H], sel_k_prefix [q + 1, H, d]
+    -> dict(dense_kl, sparse_kl, teacher_lse [H_q], s_s [q + 1])."""
+    Q_row = np.asarray(Q_row, dtype=np.float64)
+    K_prefix = np.asarray(K_prefix, dtype=np.float64)
+    assert K_prefix.shape[0] == q + 1
+    H_q = Q_row.shape[0]
+    G = H_q // K_prefix.shape[1]
+    s_t = np.stack([sm_scale * (K_prefix[:, h // G, :] @ Q_row[h]) for h in range(H_q)])      # [H_q, q + 1]
+    m = s_t.max(axis=-1)
+    lse = m + np.log(np.exp(s_t - m[:, None]).sum(axis=-1))
+    p_tau = _row_softmax(s_t).mean(axis=0)                                                     # Eq. 1: softmax, then mean
+    s_s = OS.token_scores(sel_q_row, w_row, np.asarray(sel_k_prefix))
+    p_sigma = _row_softmax(np.asarray(s_s, dtype=np.float64)[None])[0]                         # Eq. 2
+    dkl = kl_rows(p_tau[None], p_sigma[None])[0]                                               # Eq. 3
+    msk = selected_tokens(s_s, q, blk, k_blocks, sink_blocks, recency_blocks)                  # R35
+    pt, ps = p_tau[msk], p_sigma[msk]
+    skl = kl_rows((pt / pt.sum())[None], (ps / ps.sum())[None])[0] if pt.sum() > 0 else 0.0    # Eq. 4, R36
+    return dict(dense_kl=dkl, sparse_kl=skl, teacher_lse=lse, s_s=np.asarray(s_s, dtype=np.float64))

@@ -119,3 +119,17 @@ def test_sparse_kl_is_nonnegative_and_differs_from_dense():
     assert np.all(out["sparse_kl"] >= -1e-15)
     assert np.abs(out["sparse_kl"][32:] - out["dense_kl"][32:]).max() > 1e-3
     assert np.allclose(out["sparse_kl"][:16], out["dense_kl"][:16], atol=1e-14)      # <= 4 blocks visible: all selected
+
+
+def test_training_row_equals_the_rows_of_the_full_reductions():
+    """training_row (the prefix form used for sampled rows of long sequences) against training_reductions, which the tests
+    above pin: every row of a short sequence, reserved blocks and ragged last blocks included."""
+    Q, K, sq, w, sk = _rand(11, L=53)
+    for blk, kb, sink, rec in ((4, 3, 0, 0), (8, 4, 1, 1), (16, 2, 0, 1)):
+        full = OT.training_reductions(Q, K, 0.3, sq, w, sk, blk, kb, sink, rec)
+        for q in range(53):
+            row = OT.training_row(q, Q[q], K[:q + 1], 0.3, sq[q], w[q], sk[:q + 1], blk, kb, sink, rec)
+            assert abs(row["dense_kl"] - full["dense_kl"][q]) <= 1e-12
+            assert abs(row["sparse_kl"] - full["sparse_kl"][q]) <= 1e-12
+            assert np.allclose(row["teacher_lse"], full["teacher_lse"][q], atol=1e-12)
+            assert np.allclose(row["s_s"], full["s_s"][q, :q + 1], atol=0, rtol=0)
