@@ -177,7 +177,7 @@ extern "C" const char* spot_status_string(spot_status s) {
 }
 
 extern "C" int spot_last_cuda_error(void) { return g_last_cuda_error; }
-extern "C" const char* spot_version(void) { return "0.2"; }
+extern "C" const char* spot_version(void) { return "0.3"; }   // 0.3: SPOT_SELK_MXINT8 / _INT4_BF16S, q_fmt = MXFP4
 extern "C" size_t spot_struct_size(int which) {
     switch (which) {
         case 0: return sizeof(spot_select_params);
