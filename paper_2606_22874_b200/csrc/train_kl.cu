@@ -60,6 +60,7 @@ struct TrainArgs {
     float* s_lse;                // [L] natural-log log-sum-exp of the student scores
     float* sp_part;              // [L][sp_nch][2]: (max, sum) of a query's student scores over one chunk of keys (student_pass1_kernel)
     int sp_nch;                  // chunks of SP_CHUNK key tiles per row
+    float* p2_part;              // [chunks][L][4]: per-chunk sums of train_pass2_tc_kernel (P2_KT_CHUNK key tiles per chunk)
     float* blk_scores;           // [L][nb_stride]
     int nb_stride;
     const uint32_t* mask;        // [L][mask_stride] bit b: block b is in S_q
@@ -663,6 +664,11 @@ struct Pass2Args {
     float scale_log2;
     float* dense_kl;
     float* sparse_kl;
+    // the causal triangle is cut along the keys too: CTA (query block, chunk c) walks key tiles [c kt_chunk, (c + 1) kt_chunk)
+    // and leaves its four sums per query in part[c][q][4]; pass2_finalize_kernel adds the chunks and forms the two KLs.  (One
+    // CTA per query block over all its keys: 256 CTAs of 1 .. 128 tiles on 148 SMs, the heaviest alone at the end.)
+    float* part;
+    int kt_chunk;
 };
 
 __global__ void __launch_bounds__(P2_THREADS, 1) train_pass2_tc_kernel(const __grid_constant__ CUtensorMap tm_q,
@@ -692,6 +698,8 @@ __global__ void __launch_bounds__(P2_THREADS, 1) train_pass2_tc_kernel(const __g
     const int i = n_qb - 1 - (int)blockIdx.x;                          // heaviest (latest) query block first
     const int q0 = i * P2_QB;
     const int n_kt = (q0 + P2_QB + P2_KT - 1) / P2_KT;                 // key tiles: keys 0 .. q0 + 63
+    const int kt_lo = (int)blockIdx.y * a.kt_chunk, kt_hi = min(n_kt, kt_lo + a.kt_chunk);   // this CTA's chunk of them
+    if (kt_lo >= n_kt) return;                                         // (the whole CTA: the chunk lies past the diagonal)
     const int n_steps = a.t_steps + a.s_steps;
 
     if (threadIdx.x == 0) {
@@ -724,7 +732,7 @@ __global__ void __launch_bounds__(P2_THREADS, 1) train_pass2_tc_kernel(const __g
         // ================================ TMA producer ================================
         if (lane == 0) {
             int n = 0;
-            for (int kt = 0; kt < n_kt; ++kt)
+            for (int kt = kt_lo; kt < kt_hi; ++kt)
                 for (int st = 0; st < n_steps; ++st, ++n) {
                     const int s = n & 1;
                     mbar_wait(bar_empty + 8 * s, ((n >> 1) & 1) ^ 1);
@@ -748,7 +756,7 @@ __global__ void __launch_bounds__(P2_THREADS, 1) train_pass2_tc_kernel(const __g
     } else if (warp == 1) {
         // ================================ MMA issuer (converged; one elected lane issues) ================================
         int n = 0;
-        for (int kt = 0; kt < n_kt; ++kt)
+        for (int kt = kt_lo; kt < kt_hi; ++kt)
             for (int st = 0; st < n_steps; ++st, ++n) {
                 const int s = n & 1;
                 mbar_wait(bar_full + 8 * s, (n >> 1) & 1);
@@ -792,7 +800,7 @@ __global__ void __launch_bounds__(P2_THREADS, 1) train_pass2_tc_kernel(const __g
         const int bpt = P2_KT / a.blk;                                 // blocks per key tile (8, 4 or 2)
         float acc_d = 0.f, acc_a = 0.f, acc_b = 0.f, acc_c = 0.f;      // lane j: the sums of query qh * 32 + j over this warp's keys
         int n = 0;
-        for (int kt = 0; kt < n_kt; ++kt) {
+        for (int kt = kt_lo; kt < kt_hi; ++kt) {
             // the tile's mask bits of every query of the block: bit u = block kt * bpt + u is in S_q
             if (et < P2_QB) {
                 const int b0 = kt * bpt;
@@ -881,15 +889,30 @@ __global__ void __launch_bounds__(P2_THREADS, 1) train_pass2_tc_kernel(const __g
                 const float* v = s_sum + (k * P2_QB + et) * 4;
                 d += v[0]; A += v[1]; B += v[2]; C += v[3];
             }
-            a.dense_kl[q0 + et] = d;
-            // Eq. 4: sum_S (p/A) log((p/A) / (s/B)) = C / A - log A + log B
-            a.sparse_kl[q0 + et] = A > 0.f ? C / A - __logf(A) + __logf(B) : 0.f;
+            *reinterpret_cast<float4*>(a.part + ((int64_t)blockIdx.y * a.L + q0 + et) * 4) = make_float4(d, A, B, C);
         }
     }
 
     tc_fence_before();
     __syncthreads();
     if (warp == 2) tmem_dealloc(tbase, 512);
+}
+
+// pass 2, last step: the per-chunk sums of every query -> DenseKL (Eq. 3) and SparseKL (Eq. 4)
+__global__ void __launch_bounds__(256) pass2_finalize_kernel(const float* __restrict__ part, int kt_chunk, int L,
+                                                             float* __restrict__ dense_kl, float* __restrict__ sparse_kl) {
+    const int q = blockIdx.x * blockDim.x + threadIdx.x;
+    if (q >= L) return;
+    const int n_kt = ((q / P2_QB) * P2_QB + P2_QB + P2_KT - 1) / P2_KT;      // key tiles of the query's block
+    const int nch = (n_kt + kt_chunk - 1) / kt_chunk;
+    float d = 0.f, A = 0.f, B = 0.f, C = 0.f;
+    for (int c = 0; c < nch; ++c) {
+        const float4 v = *reinterpret_cast<const float4*>(part + ((int64_t)c * L + q) * 4);
+        d += v.x; A += v.y; B += v.z; C += v.w;
+    }
+    dense_kl[q] = d;
+    // Eq. 4: sum_S (p/A) log((p/A) / (s/B)) = C / A - log A + log B
+    sparse_kl[q] = A > 0.f ? C / A - __logf(A) + __logf(B) : 0.f;
 }
 
 // dst = src * f (the teacher's log-sum-exp from the log2 domain to natural log)
@@ -916,8 +939,9 @@ __global__ void list_to_mask_kernel(const int32_t* indices, const int32_t* budge
     }
 }
 
+constexpr int P2_KT_CHUNK = 16;                 // key tiles (of 128 keys) per CTA of train_pass2_tc_kernel
 struct TrainLayout {
-    size_t t_lse2, s_lse, sp_part, scores, seq_len, indices, budgets, mask, total;
+    size_t t_lse2, s_lse, sp_part, p2_part, scores, seq_len, indices, budgets, mask, total;
     int nb_stride, mask_stride, cap, n_b, sp_nch;
 };
 TrainLayout train_layout(const spot_train_params* p) {
@@ -935,6 +959,7 @@ TrainLayout train_layout(const spot_train_params* p) {
     const size_t rows_part = p->L % 64 == 0 ? (size_t)(p->L / 64) * p->L * 8 : 0;
     const size_t chunk_part = (size_t)p->L * y.sp_nch * 8;
     y.sp_part = o; o += up(rows_part > chunk_part ? rows_part : chunk_part);
+    y.p2_part = o; o += up((size_t)((p->L + 128 * P2_KT_CHUNK - 1) / (128 * P2_KT_CHUNK)) * p->L * 16);
     y.scores = o; o += up((size_t)p->L * y.nb_stride * 4);
     y.seq_len = o; o += up((size_t)p->L * 4);
     y.indices = o; o += p->indices ? 0 : up((size_t)p->L * y.cap * 4);
@@ -979,6 +1004,7 @@ spot_status launch_pass2_tc(const spot_train_params* p, const TrainArgs& t, cuda
     a.t_steps = p->H_q / a.hps; a.s_steps = p->d_idx / 64;
     a.scale_log2 = t.scale_log2;
     a.dense_kl = p->dense_kl; a.sparse_kl = p->sparse_kl;
+    a.part = t.p2_part; a.kt_chunk = P2_KT_CHUNK;
     CUtensorMap tm_q, tm_k, tm_sq, tm_sk;
     {   // Q [L][H_q][128] as (64 d, query, head, d-half, 1): a box of 64 queries x hps heads x 2 halves lands as
         // [half][head][query][128 B] = [half][hps * 64 columns][128 B]
@@ -1004,7 +1030,10 @@ spot_status launch_pass2_tc(const spot_train_params* p, const TrainArgs& t, cuda
     }
     static unsigned long long done = 0;
     SPOT_CUDA_TRY(set_max_smem_once(train_pass2_tc_kernel, (int)P2_SMEM, done));
-    train_pass2_tc_kernel<<<p->L / P2_QB, P2_THREADS, P2_SMEM, s>>>(tm_q, tm_k, tm_sq, tm_sk, a);
+    const int nch = ((p->L + P2_KT - 1) / P2_KT + P2_KT_CHUNK - 1) / P2_KT_CHUNK;
+    train_pass2_tc_kernel<<<dim3((unsigned)(p->L / P2_QB), (unsigned)nch), P2_THREADS, P2_SMEM, s>>>(tm_q, tm_k, tm_sq, tm_sk, a);
+    SPOT_LAUNCH_CHECK();
+    pass2_finalize_kernel<<<(p->L + 255) / 256, 256, 0, s>>>(a.part, a.kt_chunk, p->L, p->dense_kl, p->sparse_kl);
     SPOT_LAUNCH_CHECK();
     return SPOT_OK;
 }
@@ -1038,6 +1067,7 @@ extern "C" spot_status spot_train_kl(const spot_train_params* p, void* stream) {
     a.t_lse2 = reinterpret_cast<float*>(ws + y.t_lse2);
     a.s_lse = reinterpret_cast<float*>(ws + y.s_lse);
     a.sp_part = reinterpret_cast<float*>(ws + y.sp_part); a.sp_nch = y.sp_nch;
+    a.p2_part = reinterpret_cast<float*>(ws + y.p2_part);
     a.blk_scores = reinterpret_cast<float*>(ws + y.scores);
     a.nb_stride = y.nb_stride;
     uint32_t* mask = reinterpret_cast<uint32_t*>(ws + y.mask);
