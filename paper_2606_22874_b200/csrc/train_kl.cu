@@ -599,18 +599,26 @@ __global__ void __launch_bounds__(256) student_combine_kernel(const float* __res
     s_lse[q] = m + __logf(l);
 }
 
-// the same for the rows form of score_prefill_kernel: part[j][q] = (max, sum exp) of row q over the 64 keys of block j
+// the same for the rows form of score_prefill_kernel: part[j][q] = (max, sum exp) of row q over the 64 keys of block j.
+// Thread (q, u) folds blocks u, u + 8, ..; the eight threads of a row (consecutive lanes) then fold their pairs.
 __global__ void __launch_bounds__(256) student_combine_rows_kernel(const float2* __restrict__ part, float* __restrict__ s_lse, int L) {
-    const int q = blockIdx.x * blockDim.x + threadIdx.x;
-    if (q >= L) return;
+    const int t = blockIdx.x * blockDim.x + threadIdx.x;
+    const int q = t >> 3, u = t & 7;
     float m = -INFINITY, l = 0.f;
-    for (int j = 0; j <= q / 64; ++j) {
-        const float2 p = part[(int64_t)j * L + q];
-        const float M = fmaxf(m, p.x);
-        l = l * __expf(m - M) + p.y * __expf(p.x - M);       // (block 0 always holds key 0: M is finite from the first step)
-        m = M;
+    if (q < L)
+        for (int j = u; j <= q / 64; j += 8) {
+            const float2 p = part[(int64_t)j * L + q];
+            const float M = fmaxf(m, p.x);
+            l = l * __expf(m - M) + p.y * __expf(p.x - M);   // (p.x is finite: every visible block holds a visible key)
+            m = M;
+        }
+#pragma unroll
+    for (int o = 1; o < 8; o <<= 1) {
+        const float m2 = __shfl_xor_sync(0xffffffffu, m, o), l2 = __shfl_xor_sync(0xffffffffu, l, o);
+        const float M = fmaxf(m, m2);
+        if (M > -INFINITY) { l = l * __expf(m - M) + l2 * __expf(m2 - M); m = M; }
     }
-    s_lse[q] = m + __logf(l);
+    if (q < L && u == 0) s_lse[q] = m + __logf(l);
 }
 
 // sum over the 32 lanes of v[j] for every j, delivered to lane j (31 shuffles instead of 32 x 5): at each level a lane keeps
@@ -1106,7 +1114,7 @@ extern "C" spot_status spot_train_kl(const spot_train_params* p, void* stream) {
             if ((st = score_prefill_rows(p->sel_q, p->w, p->sel_k, p->L, p->H_idx, p->d_idx, p->blk, a.blk_scores, a.nb_stride,
                                          reinterpret_cast<float2*>(a.sp_part), s)) != SPOT_OK)
                 return st;
-            student_combine_rows_kernel<<<(p->L + 255) / 256, 256, 0, s>>>(reinterpret_cast<const float2*>(a.sp_part), a.s_lse, p->L);
+            student_combine_rows_kernel<<<(8 * p->L + 255) / 256, 256, 0, s>>>(reinterpret_cast<const float2*>(a.sp_part), a.s_lse, p->L);
             SPOT_LAUNCH_CHECK();
         } else {
         const int srow = p->H_idx * p->d_idx * 2, stages = 2;
