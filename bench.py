@@ -205,7 +205,32 @@ def prefill_gemm_roofline(dev, steps, warmup, clocks_index):
     tiles = n_qb * (n_qb + 1) // 2
     flop = 2.0 * 64 * 64 * wl.d_idx * wl.H_idx * tiles
     achieved = flop / (float(np.mean(ts)) * 1e-3) / 1e12
+    # f2 (round 2): the same GEMM with queries AND keys in a quantised cache format, straight from the caches on the
+    # low-precision tensor-core paths (q_fmt: FP8 x FP8 kind::f8f6f4, MXFP4 x MXFP4 kind::mxf4.block_scale), timed the same way
+    low = {}
+    for fmt in ("fp8_e4m3", "mxfp4"):
+        k_f = torch.zeros(api.spot_selector_k_bytes(fmt, 1, L, wl.H_idx, wl.d_idx), dtype=torch.uint8, device=dev)
+        q_f = torch.zeros_like(k_f)
+        api.spot_quantize_selector_k(sel_k, k_f, fmt, 1, L, 0, L, wl.H_idx, wl.d_idx)
+        api.spot_quantize_selector_k(sel_q, q_f, fmt, 1, L, 0, L, wl.H_idx, wl.d_idx)
+        sp_f = api.make_select_params(q_f, w, k_f, fmt, L, None, 0, 1, L, wl.H_idx, wl.d_idx, q_start=0, blk=64,
+                                      q_block=64, q_fmt=fmt, block_scores=scores, nb_stride=nb_stride)
+        tf = []
+        for i in range(max(3, steps // 2) + 2):
+            flush.view(torch.int64).sum()
+            a_, b_ = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a_.record(stream)
+            api.spot_score_blocks(sp_f, stream)
+            b_.record(stream)
+            torch.cuda.synchronize()
+            if i >= 2:
+                tf.append(a_.elapsed_time(b_))
+        low[fmt] = {"ms": float(np.mean(tf)), "tflops_equivalent": flop / (float(np.mean(tf)) * 1e-3) / 1e12,
+                    "operand_bytes": int(k_f.numel() + q_f.numel()),
+                    "traffic": traffic_entry("cfg5/%s+q/score_prefill_kernel" % fmt)}
+        del k_f, q_f
     return {"bound": "tensor", "kernel": "score_prefill_kernel", "workload": "cfg5 (L=65536, one chunk, selector 4x64 bf16)",
+            "low_precision_q_and_k": low,
             "ms": float(np.mean(ts)), "achieved": achieved, "peak": burst, "unit": "TFLOP/s", "frac": achieved / burst,
             "frac_of_sustained": achieved / sustained, "algorithmic_flops": flop,
             "traffic": traffic_entry("cfg5/bf16/score_prefill_kernel"), "peak_source": peak_src,
